@@ -1,0 +1,271 @@
+"""ctypes face of oracle/fe_oracle.c plus the two harness-level algorithms that sit on top of the oracle's
+apply: 20-step Lanczos bounds (reading R10) and Rayleigh-Ritz (Eq. 23-24, l.210-219; readings R8, R9).
+
+TEST INFRASTRUCTURE: imported only by tests/, __graft_entry__.smoke() and bench.py's cpu_baseline legs.
+"""
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libfe_oracle.so")
+_lib = None
+
+
+def build_oracle(force=False):
+    """gcc -O2 (no fast-math) build of the plain-C oracle into oracle/libfe_oracle.so."""
+    src = os.path.join(_HERE, "fe_oracle.c")
+    hdr = os.path.join(_HERE, "fe_oracle.h")
+    if (not force and os.path.exists(_SO)
+            and os.path.getmtime(_SO) >= max(os.path.getmtime(src), os.path.getmtime(hdr))):
+        return _SO
+    cmd = ["gcc", "-O2", "-std=c99", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared", "-o", _SO, src, "-lm"]
+    subprocess.check_call(cmd)
+    return _SO
+
+
+def _load():
+    global _lib
+    if _lib is not None:
+        return _lib
+    build_oracle()
+    L = C.CDLL(_SO)
+    dp, ip, i64p, u8p = (C.POINTER(C.c_double), C.POINTER(C.c_int32), C.POINTER(C.c_int64), C.POINTER(C.c_uint8))
+    vp = C.c_void_p
+    sig = {
+        "orc_gll": (C.c_int, [C.c_int, dp, dp]),
+        "orc_gauss": (C.c_int, [C.c_int, dp, dp]),
+        "orc_lagrange": (C.c_double, [C.c_int, dp, C.c_int, C.c_double]),
+        "orc_lagrange_deriv": (C.c_double, [C.c_int, dp, C.c_int, C.c_double]),
+        "orc_mesh_create": (vp, [dp, C.c_int, dp, C.c_int, dp, C.c_int, C.c_int]),
+        "orc_mesh_destroy": (None, [vp]),
+        "orc_num_nodes": (C.c_int64, [vp]),
+        "orc_num_free": (C.c_int64, [vp]),
+        "orc_num_cells": (C.c_int64, [vp]),
+        "orc_nodes_per_cell": (C.c_int, [vp]),
+        "orc_quad_per_cell": (C.c_int, [vp]),
+        "orc_get_l2g": (None, [vp, ip]),
+        "orc_get_node_coords": (None, [vp, dp]),
+        "orc_get_quad_coords": (None, [vp, dp]),
+        "orc_get_mass": (None, [vp, dp]),
+        "orc_get_mask": (None, [vp, u8p]),
+        "orc_cell_matrix": (None, [vp, C.c_int64, dp, C.c_double, C.c_double, dp]),
+        "orc_build_cell_matrices": (None, [vp, dp, dp]),
+        "orc_assemble": (vp, [vp, dp, C.c_int]),
+        "orc_csr_destroy": (None, [vp]),
+        "orc_csr_nnz": (C.c_int64, [vp]),
+        "orc_csr_copy": (None, [vp, i64p, ip, dp]),
+        "orc_csr_apply": (None, [vp, vp, dp, C.c_int, dp, dp, C.c_int]),
+        "orc_cellwise_apply": (None, [vp, dp, dp, C.c_int, dp, dp]),
+        "orc_apply_rows": (None, [vp, dp, dp, C.c_int, dp, i64p, C.c_int64, dp]),
+        "orc_filter": (C.c_int, [vp, vp, dp, dp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_int]),
+    }
+    for name, (res, args) in sig.items():
+        f = getattr(L, name)
+        f.restype, f.argtypes = res, args
+    _lib = L
+    return L
+
+
+def _d(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double)) if a is not None else None
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def gll(p):
+    x, w = np.empty(p + 1), np.empty(p + 1)
+    _load().orc_gll(p, _d(x), _d(w))
+    return x, w
+
+
+def gauss(nq):
+    x, w = np.empty(nq), np.empty(nq)
+    _load().orc_gauss(nq, _d(x), _d(w))
+    return x, w
+
+
+def lagrange(nodes, a, x):
+    nodes = _f64(nodes)
+    return _load().orc_lagrange(len(nodes), _d(nodes), a, float(x))
+
+
+def lagrange_deriv(nodes, a, x):
+    nodes = _f64(nodes)
+    return _load().orc_lagrange_deriv(len(nodes), _d(nodes), a, float(x))
+
+
+class OracleMesh:
+    """Mesh + operator of the oracle.  set_potential() builds every cell matrix by explicit quadrature;
+    assemble() builds the CSR of H~ (configs 1, 2, 5); without it, apply() uses the cell-wise form."""
+
+    def __init__(self, xe, ye, ze, p):
+        L = _load()
+        self.xe, self.ye, self.ze = _f64(xe), _f64(ye), _f64(ze)
+        self.p = int(p)
+        self._h = L.orc_mesh_create(_d(self.xe), len(self.xe) - 1, _d(self.ye), len(self.ye) - 1,
+                                    _d(self.ze), len(self.ze) - 1, self.p)
+        if not self._h:
+            raise ValueError("orc_mesh_create failed")
+        self.N = L.orc_num_nodes(self._h)
+        self.N_free = L.orc_num_free(self._h)
+        self.ncells = L.orc_num_cells(self._h)
+        self.nc = L.orc_nodes_per_cell(self._h)
+        self.nq3 = L.orc_quad_per_cell(self._h)
+        self.He = None
+        self.Vq = None
+        self._csr = None
+        self._csr_raw = None
+
+    def __del__(self):
+        try:
+            L = _load()
+            for h in (self._csr, self._csr_raw):
+                if h:
+                    L.orc_csr_destroy(h)
+            if self._h:
+                L.orc_mesh_destroy(self._h)
+        except Exception:
+            pass
+
+    # ---- tables -------------------------------------------------------------------------------------------
+    def l2g(self):
+        a = np.empty((self.ncells, self.nc), dtype=np.int32)
+        _load().orc_get_l2g(self._h, a.ctypes.data_as(C.POINTER(C.c_int32)))
+        return a
+
+    def node_coords(self):
+        a = np.empty((self.N, 3))
+        _load().orc_get_node_coords(self._h, _d(a))
+        return a
+
+    def quad_coords(self):
+        a = np.empty((self.ncells * self.nq3, 3))
+        _load().orc_get_quad_coords(self._h, _d(a))
+        return a
+
+    def mass(self):
+        a = np.empty(self.N)
+        _load().orc_get_mass(self._h, _d(a))
+        return a
+
+    def mask(self):
+        a = np.empty(self.N, dtype=np.uint8)
+        _load().orc_get_mask(self._h, a.ctypes.data_as(C.POINTER(C.c_uint8)))
+        return a
+
+    # ---- operator -----------------------------------------------------------------------------------------
+    def cell_matrix(self, e, Vq_cell=None, kin=0.5, pot=1.0):
+        He = np.empty((self.nc, self.nc))
+        v = _f64(Vq_cell) if Vq_cell is not None else None
+        _load().orc_cell_matrix(self._h, int(e), _d(v), float(kin), float(pot), _d(He))
+        return He
+
+    def set_potential(self, Vq, build=True):
+        self.Vq = _f64(Vq).reshape(-1)
+        assert self.Vq.size == self.ncells * self.nq3
+        L = _load()
+        for name in ("_csr", "_csr_raw"):
+            if getattr(self, name):
+                L.orc_csr_destroy(getattr(self, name))
+                setattr(self, name, None)
+        self.He = None
+        if build:
+            self.He = np.empty((self.ncells, self.nc, self.nc))
+            L.orc_build_cell_matrices(self._h, _d(self.Vq), _d(self.He))
+
+    def assemble(self):
+        if self._csr is None:
+            self._csr = _load().orc_assemble(self._h, _d(self.He), 1)
+        return self
+
+    def csr(self, scaled=True):
+        """(row_ptr, col, val) of H~ (scaled) or of the raw assembled H."""
+        L = _load()
+        if scaled:
+            self.assemble()
+            h = self._csr
+        else:
+            if self._csr_raw is None:
+                self._csr_raw = L.orc_assemble(self._h, _d(self.He), 0)
+            h = self._csr_raw
+        nnz = L.orc_csr_nnz(h)
+        rp, col, val = np.empty(self.N + 1, dtype=np.int64), np.empty(nnz, dtype=np.int32), np.empty(nnz)
+        L.orc_csr_copy(h, rp.ctypes.data_as(C.POINTER(C.c_int64)), col.ctypes.data_as(C.POINTER(C.c_int32)), _d(val))
+        return rp, col, val
+
+    def apply(self, X, eps=None, nthreads=1, cellwise=False):
+        X = _f64(X)
+        B = X.shape[1]
+        e = _f64(eps) if eps is not None else None
+        Y = np.empty_like(X)
+        L = _load()
+        if self._csr is not None and not cellwise:
+            L.orc_csr_apply(self._h, self._csr, _d(X), B, _d(e), _d(Y), int(nthreads))
+        else:
+            L.orc_cellwise_apply(self._h, _d(self.He), _d(X), B, _d(e), _d(Y))
+        return Y
+
+    def apply_rows(self, X, rows, eps=None):
+        X = _f64(X)
+        B = X.shape[1]
+        rows = np.ascontiguousarray(rows, dtype=np.int64)
+        e = _f64(eps) if eps is not None else None
+        Y = np.empty((len(rows), B))
+        _load().orc_apply_rows(self._h, _d(self.Vq), _d(X), B, _d(e), rows.ctypes.data_as(C.POINTER(C.c_int64)),
+                               len(rows), _d(Y))
+        return Y
+
+    def filter(self, X, m, a, b, a0, nthreads=1, cellwise=False):
+        Y = _f64(X).copy()
+        B = Y.shape[1]
+        use_csr = self._csr is not None and not cellwise
+        rc = _load().orc_filter(self._h, self._csr if use_csr else None, _d(self.He), _d(Y), B, int(m),
+                                float(a), float(b), float(a0), int(nthreads))
+        if rc != 0:
+            raise ValueError("orc_filter: need a0 < a < b and m >= 1")
+        return Y
+
+
+def lanczos_bounds(mesh, v0, k=20, nthreads=1):
+    """Reading R10 (survey 8(c) step 8): k Lanczos steps on H~ (free rows) from the given start vector, no
+    re-orthogonalisation; returns (theta_min, theta_max, beta_k).  b = theta_max + beta_k, a0 = theta_min."""
+    mask = mesh.mask().astype(np.float64)
+    v = _f64(v0).reshape(-1) * mask
+    v = v / np.linalg.norm(v)
+    v_prev = np.zeros_like(v)
+    beta = 0.0
+    alphas, betas = [], []
+    for _ in range(k):
+        w = mesh.apply(v.reshape(-1, 1), nthreads=nthreads).reshape(-1)
+        alpha = float(w @ v)
+        w = w - alpha * v - beta * v_prev
+        beta = float(np.linalg.norm(w))
+        alphas.append(alpha)
+        betas.append(beta)
+        if beta == 0.0:
+            break
+        v_prev, v = v, w / beta
+    T = np.diag(alphas) + np.diag(betas[:-1], 1) + np.diag(betas[:-1], -1)
+    theta = np.linalg.eigvalsh(T)
+    return float(theta[0]), float(theta[-1]), float(betas[-1])
+
+
+def rayleigh_ritz(mesh, Y, nthreads=1):
+    """PAPER.md Eq. 23-24 (l.210-219) with readings R8 (H~_Y = Y^T H~ Y) and R9 (CholQR2):
+    S = Y^T Y = L L^T, Q = Y L^{-T} (twice), G = Q^T H~ Q, G v = theta v, X = Q V.  Returns (theta, X, Q)."""
+    mask = mesh.mask().astype(np.float64)[:, None]
+    Q = _f64(Y) * mask
+    for _ in range(2):
+        S = Q.T @ Q
+        Lc = np.linalg.cholesky(S)
+        Q = np.linalg.solve(Lc, Q.T).T  # Q L^{-T}
+    HQ = mesh.apply(Q, nthreads=nthreads)
+    G = Q.T @ HQ
+    G = 0.5 * (G + G.T)
+    theta, V = np.linalg.eigh(G)
+    return theta, Q @ V, Q

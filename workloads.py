@@ -1,0 +1,196 @@
+"""Seeded synthetic inputs for the five BASELINE.json workloads (readings R11-R13, R18, R19 in DESIGN.md).
+
+This module serves BOTH the CUDA product's harness (bench.py, tests) and the CPU oracle's harness and holds
+none of the method's arithmetic: it only defines mesh edges, atoms, potentials evaluated at coordinates the
+caller supplies, random blocks and shifts.  Random numbers are counter based (splitmix64 -> uniform (0,1] ->
+Box-Muller), so any element can be regenerated on its own; blocks are generated ONCE and the same array is
+handed to both paths.
+
+The workloads are stand-ins shaped like the paper's GPU benchmarks (p=6 meshes with 2.6 M
+and 7.2 M basis functions, 40 / 100 electrons); no item of any external data set is reproduced.
+"""
+import math
+
+import numpy as np
+
+_GAMMA = np.uint64(0x9E3779B97F4A7C15)
+_M1 = np.uint64(0xBF58476D1CE4E5B9)
+_M2 = np.uint64(0x94D049BB133111EB)
+
+
+def splitmix64(seed, start, count):
+    """Outputs start .. start+count-1 of the splitmix64 stream of `seed` (counter based, uint64)."""
+    with np.errstate(over="ignore"):
+        i = np.arange(start + 1, start + count + 1, dtype=np.uint64)
+        z = np.uint64(seed) + i * _GAMMA
+        z = (z ^ (z >> np.uint64(30))) * _M1
+        z = (z ^ (z >> np.uint64(27))) * _M2
+        return z ^ (z >> np.uint64(31))
+
+
+def uniform01(seed, start, count):
+    """Uniform on (0, 1]: ((z >> 11) + 1) * 2^-53."""
+    z = splitmix64(seed, start, count)
+    return ((z >> np.uint64(11)).astype(np.float64) + 1.0) * (1.0 / 9007199254740992.0)
+
+
+def normal(seed, count, start=0):
+    """N(0,1) numbers start..start+count-1: number 2k / 2k+1 = r cos(t) / r sin(t), r = sqrt(-2 ln u_{2k}),
+    t = 2 pi u_{2k+1}."""
+    k0, k1 = start // 2, (start + count + 1) // 2
+    out = np.empty(2 * (k1 - k0))
+    chunk = 1 << 22
+    for k in range(k0, k1, chunk):
+        kk = min(k1, k + chunk)
+        u = uniform01(seed, 2 * k, 2 * (kk - k))
+        r = np.sqrt(-2.0 * np.log(u[0::2]))
+        t = (2.0 * math.pi) * u[1::2]
+        out[2 * (k - k0):2 * (kk - k0):2] = r * np.cos(t)
+        out[2 * (k - k0) + 1:2 * (kk - k0):2] = r * np.sin(t)
+    return out[start - 2 * k0:start - 2 * k0 + count]
+
+
+def random_block(seed, N, B, mask=None):
+    """X (N x B, node-major, vector fastest), all rows N(0,1), then boundary rows zeroed (R13)."""
+    X = normal(seed, N * B).reshape(N, B)
+    if mask is not None:
+        X[np.asarray(mask) == 0] = 0.0
+    return X
+
+
+def uniform_edges(lo, hi, cells):
+    return lo + (hi - lo) * np.arange(cells + 1, dtype=np.float64) / cells
+
+
+def graded_edges(half_width=15.0, cells_per_side=20, h0=0.2, ratio=1.15, hmax=1.5):
+    """Reading R11: symmetric about 0, h_k = s*min(hmax, h0*ratio^k) outward, s scales the sum to half_width."""
+    h = np.minimum(hmax, h0 * ratio ** np.arange(cells_per_side, dtype=np.float64))
+    h *= half_width / h.sum()
+    pos = np.concatenate([[0.0], np.cumsum(h)])
+    pos[-1] = half_width
+    return np.concatenate([-pos[:0:-1], pos])
+
+
+def atoms(seed, count, zmax):
+    """Reading R12: positions uniform in [-5,5]^3, Z uniform integer in {1..zmax}."""
+    u = uniform01(seed, 0, 4 * count).reshape(count, 4)
+    R = -5.0 + 10.0 * u[:, :3]
+    Z = np.minimum(zmax, 1 + np.floor(u[:, 3] * zmax)).astype(np.float64)
+    return R, Z
+
+
+def harmonic(xyz):
+    """V = 1/2 |r|^2 (config 1)."""
+    return 0.5 * np.einsum("ij,ij->i", xyz, xyz)
+
+
+def soft_coulomb(xyz, R, Z, soft2=0.25):
+    """V(r) = -sum_a Z_a / sqrt(|r-R_a|^2 + 0.25) (configs 2-5)."""
+    V = np.zeros(len(xyz))
+    for Ra, Za in zip(np.atleast_2d(R), np.atleast_1d(Z)):
+        d = xyz - Ra
+        V -= Za / np.sqrt(np.einsum("ij,ij->i", d, d) + soft2)
+    return V
+
+
+def shifts(seed, B, lo=-2.0, hi=0.0):
+    """eps sorted ascending, uniform in [lo, hi] (R18)."""
+    return np.sort(lo + (hi - lo) * uniform01(seed, 0, B))
+
+
+class Workload:
+    """One BASELINE.json config: mesh edges, order, block width, filter degree, potential recipe, seeds."""
+
+    def __init__(self, index, name, edges, p, B, m, potential, x_seed, atom_seed=None, n_atoms=0, zmax=0,
+                 eps_seed=None, n_applies=1):
+        self.index, self.name = index, name
+        self.xe, self.ye, self.ze = edges
+        self.p, self.B, self.m = p, B, m
+        self.potential, self.x_seed = potential, x_seed
+        self.atom_seed, self.n_atoms, self.zmax = atom_seed, n_atoms, zmax
+        self.eps_seed, self.n_applies = eps_seed, n_applies
+
+    @property
+    def cells(self):
+        return (len(self.xe) - 1, len(self.ye) - 1, len(self.ze) - 1)
+
+    @property
+    def nodes_per_axis(self):
+        return tuple(c * self.p + 1 for c in self.cells)
+
+    @property
+    def N(self):
+        nx, ny, nz = self.nodes_per_axis
+        return nx * ny * nz
+
+    @property
+    def N_free(self):
+        nx, ny, nz = self.nodes_per_axis
+        return (nx - 2) * (ny - 2) * (nz - 2)
+
+    @property
+    def ncells(self):
+        cx, cy, cz = self.cells
+        return cx * cy * cz
+
+    def atom_list(self):
+        if self.potential == "single":
+            return np.zeros((1, 3)), np.array([4.0])
+        return atoms(self.atom_seed, self.n_atoms, self.zmax)
+
+    def V(self, quad_xyz):
+        """Potential at the quadrature points the caller supplies (cells*n_q^3 x 3)."""
+        if self.potential == "harmonic":
+            return harmonic(quad_xyz)
+        R, Z = self.atom_list()
+        return soft_coulomb(quad_xyz, R, Z)
+
+    def X(self, mask=None, seed=None, B=None):
+        return random_block(self.x_seed if seed is None else seed, self.N, self.B if B is None else B, mask)
+
+    def eps(self):
+        return shifts(self.eps_seed, self.B) if self.eps_seed is not None else None
+
+    def describe(self):
+        cx, cy, cz = self.cells
+        return "cfg%d %s: %dx%dx%d cells p=%d N=%d B=%d m=%d" % (self.index, self.name, cx, cy, cz, self.p,
+                                                                   self.N, self.B, self.m)
+
+
+def config(i):
+    """BASELINE.json configs 1..5."""
+    if i == 1:
+        e = uniform_edges(-6.0, 6.0, 4)
+        return Workload(1, "tiny-harmonic", (e, e, e), 2, 8, 10, "harmonic", x_seed=0)
+    if i == 2:
+        e = uniform_edges(-10.0, 10.0, 16)
+        return Workload(2, "single-atom-well", (e, e, e), 4, 64, 20, "single", x_seed=1)
+    if i == 3:
+        e = uniform_edges(-12.0, 12.0, 24)
+        return Workload(3, "small-molecule", (e, e, e), 6, 64, 30, "atoms", x_seed=2, atom_seed=1003, n_atoms=10,
+                        zmax=8)
+    if i == 4:
+        e = graded_edges()
+        return Workload(4, "graded-100e-molecule", (e, e, e), 6, 128, 40, "atoms", x_seed=3, atom_seed=1004,
+                        n_atoms=20, zmax=9)
+    if i == 5:
+        e = uniform_edges(-10.0, 10.0, 16)
+        return Workload(5, "adjoint-shifted-apply", (e, e, e), 4, 64, 0, "single", x_seed=4, eps_seed=2005,
+                        n_applies=200)
+    raise ValueError("config index 1..5")
+
+
+def reduced(i, cells):
+    """Same recipe as config i (order, cell size, potential) on a centred sub-box of cells^3 cells: the bounded
+    sample the CPU baseline times, and the small parity meshes of the tests."""
+    w = config(i)
+
+    def centre(e):
+        c = len(e) - 1
+        k = min(cells, c)
+        lo = (c - k) // 2
+        return np.array(e[lo:lo + k + 1])
+
+    w.xe, w.ye, w.ze = centre(w.xe), centre(w.ye), centre(w.ze)
+    w.name += "-sub%d" % cells
+    return w
