@@ -1,0 +1,88 @@
+/*
+ * fe_cheb.h -- C ABI of the B200-native hot path of invDFT (arXiv 2510.10529).
+ *
+ * What the library computes (citations: /root/reference/PAPER.md line numbers; R-numbers are the readings listed
+ * in DESIGN.md):
+ *
+ *   H~ = M^{-1/2} (1/2 K + M_V) M^{-1/2}                                   (Eq. 17 l.171, Eq. 19 l.181-185)
+ *
+ * the spectral-finite-element Kohn-Sham operator on a tensor-product hexahedral mesh (Lagrange order p on
+ * Gauss-Lobatto-Legendre nodes, Eq. 12 l.124; lumped GLL mass, l.185; zero Dirichlet data on the box surface, R5;
+ * K and M_V integrated with p+1 Gauss-Legendre points per direction, R1), applied to a block of B vectors stored
+ * "all vectors of one basis function contiguous" (l.233-235, Fig. 4(a) l.253):  X[a*B + j] = node a, vector j.
+ *
+ *   fe_apply_H : Y = H~ X, or column-wise (H~ - eps_j I) X_j                  (Eq. 20 l.183; adjoint solve l.221-225)
+ *   cheb_filter: X <- T_m((H~ - c)/e) X / T_m((a0 - c)/e)                     (ChFSI filter, l.208-210; R7)
+ *
+ * Every step runs in hand-written sm_100a kernels; there is no CPU fallback.  All functions return 0 on success
+ * and a negative code on failure (FE_ERR_*); fe_last_error() gives a thread-local message owned by the library.
+ * No exception crosses this boundary.  The library never frees caller memory and keeps no caller pointer after
+ * a call returns.  "HOST" / "DEVICE" below say where a pointer must live.  FP64 throughout.
+ */
+#ifndef FE_CHEB_H
+#define FE_CHEB_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define FE_OK 0
+#define FE_ERR_INVALID (-1) /* bad argument */
+#define FE_ERR_NOMEM (-2)   /* host or device allocation failed */
+#define FE_ERR_CUDA (-3)    /* CUDA runtime error (message in fe_last_error) */
+#define FE_ERR_STATE (-4)   /* e.g. apply before fe_set_potential */
+
+typedef struct fe_mesh fe_mesh; /* opaque; owns all device tables; one stream at a time per handle */
+
+/* Mesh of the box [xe[0],xe[cx]] x [ye[0],ye[cy]] x [ze[0],ze[cz]] (HOST arrays of cx+1, cy+1, cz+1 strictly
+ * increasing edges), Lagrange order p in 1..8 on GLL nodes.  Numbering (R3), x fastest everywhere:
+ *   cell e = ex + cx*(ey + cy*ez);  local node a = ax + n*(ay + n*az), n = p+1;
+ *   global node g = (ex*p+ax) + Nx*((ey*p+ay) + Ny*(ez*p+az)), Nd = cd*p+1;  quadrature point q = qx + n*(qy + n*qz).
+ * Builds the 1-D tables, the lumped mass (l.185), M^{-1/2} and the Dirichlet mask on cuda_device.  Synchronous. */
+int fe_mesh_create(const double* xe, int cx, const double* ye, int cy, const double* ze, int cz, int p,
+                   int cuda_device, fe_mesh** out);
+int fe_mesh_destroy(fe_mesh* m);
+
+int64_t fe_num_nodes(const fe_mesh* m); /* N = Nx*Ny*Nz */
+int64_t fe_num_free(const fe_mesh* m);  /* (Nx-2)(Ny-2)(Nz-2) unconstrained nodes (R14: the "DoF" of the metric) */
+int64_t fe_num_cells(const fe_mesh* m);
+int fe_nodes_per_cell(const fe_mesh* m); /* n^3 */
+int fe_quad_per_cell(const fe_mesh* m);  /* n_q^3, n_q = p+1 */
+
+/* Parity accessors: fill caller-allocated HOST arrays.  Synchronous. */
+int fe_get_l2g(const fe_mesh* m, int32_t* l2g);            /* cells*n^3, R3 */
+int fe_get_node_coords(const fe_mesh* m, double* xyz);     /* N*3, R4 */
+int fe_get_quad_coords(const fe_mesh* m, double* xyz);     /* cells*n_q^3*3: where the caller evaluates V */
+int fe_get_mass(const fe_mesh* m, double* Mdiag);          /* N, diagonal of the GLL-lumped M (l.185) */
+int fe_get_dirichlet_mask(const fe_mesh* m, uint8_t* mask); /* N, 1 = free, 0 = boundary */
+
+/* V = v_H + v_N + v_xc (l.68) at the quadrature points: Vq_dev is a DEVICE array of cells*n_q^3 doubles, cell-major,
+ * q = qx + n_q*(qy + n_q*qz) inside a cell.  The library stores J*w_q*V_q in its own buffer (one kernel on
+ * cuda_stream); `copy` is accepted for ABI stability and ignored: Vq_dev is never retained.  Asynchronous. */
+int fe_set_potential(fe_mesh* m, const double* Vq_dev, int copy, void* cuda_stream);
+
+/* Y = H~ X (eps_dev == NULL) or Y[:,j] = (H~ - eps_dev[j] I) X[:,j] (Eq. 20; the shift multiplies the identity of the
+ * standard form, R18).  X, Y: DEVICE, N*B doubles, X[a*B+j]; must not overlap.  eps_dev: DEVICE, B doubles.
+ * Boundary rows of X are ignored (treated as 0); boundary rows of Y are written 0 (R5).  B >= 1.
+ * Asynchronous on cuda_stream. */
+int fe_apply_H(fe_mesh* m, const double* X, double* Y, int B, const double* eps_dev, void* cuda_stream);
+
+/* Chebyshev filter of ChFSI (l.208-210), in place, by the scaled three-term recurrence (R7):
+ *   e=(b-a)/2, c=(b+a)/2, s1=e/(a0-c);  Y1=(s1/e)(H~-c)X;  s_{k+1}=1/(2/s1-s_k);
+ *   Y_{k+1} = (2 s_{k+1}/e)(H~-c)Y_k - s_k s_{k+1} Y_{k-1};   X <- Y_m  (= T_m((H~-c)/e) X / T_m((a0-c)/e)).
+ * Requires a0 < a < b and m >= 1.  work: DEVICE, 2*N*B doubles, caller-owned, must not overlap X.
+ * Each step is one fused operator launch (no separate axpy kernels).  Asynchronous on cuda_stream. */
+int cheb_filter(fe_mesh* m, double* X, int B, int deg, double a, double b, double a0, double* work,
+                void* cuda_stream);
+
+/* Kernel variant for experiments and tests: 0 = default for this p.  Returns FE_ERR_INVALID if unknown. */
+int fe_set_variant(fe_mesh* m, int variant);
+/* Kernels launched by this handle since creation (bench.py's gpu_launches). */
+int64_t fe_launch_count(const fe_mesh* m);
+
+const char* fe_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

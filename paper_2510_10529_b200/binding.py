@@ -1,0 +1,232 @@
+"""ctypes binding of include/fe_cheb.h: argument marshalling only (torch tensors -> raw device pointers, the
+current torch stream -> cudaStream_t).  Function names are those of the C ABI; FEMesh is a small convenience
+wrapper that owns a handle.  torch is used for device memory and streams, nothing else."""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libfecheb.so")
+_lib = None
+
+EXPORTS = (
+    "fe_mesh_create", "fe_mesh_destroy", "fe_num_nodes", "fe_num_free", "fe_num_cells", "fe_nodes_per_cell",
+    "fe_quad_per_cell", "fe_get_l2g", "fe_get_node_coords", "fe_get_quad_coords", "fe_get_mass",
+    "fe_get_dirichlet_mask", "fe_set_potential", "fe_apply_H", "cheb_filter", "fe_set_variant", "fe_launch_count",
+    "fe_last_error",
+)
+
+
+class FEError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("fe_cheb error %d: %s" % (code, msg))
+        self.code = code
+
+
+def library_path():
+    return _SO
+
+
+def load_library():
+    """Load libfecheb.so (built in-tree by build.py / __graft_entry__.build()).  Fails loudly if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_SO):
+        raise FEError(-3, "CUDA extension %s is missing: run `python -m paper_2510_10529_b200.build` "
+                          "(there is no CPU fallback)" % _SO)
+    L = C.CDLL(_SO)
+    vp, dp = C.c_void_p, C.POINTER(C.c_double)
+    L.fe_mesh_create.restype = C.c_int
+    L.fe_mesh_create.argtypes = [dp, C.c_int, dp, C.c_int, dp, C.c_int, C.c_int, C.c_int, C.POINTER(vp)]
+    L.fe_mesh_destroy.restype, L.fe_mesh_destroy.argtypes = C.c_int, [vp]
+    for name in ("fe_num_nodes", "fe_num_free", "fe_num_cells", "fe_launch_count"):
+        getattr(L, name).restype, getattr(L, name).argtypes = C.c_int64, [vp]
+    for name in ("fe_nodes_per_cell", "fe_quad_per_cell"):
+        getattr(L, name).restype, getattr(L, name).argtypes = C.c_int, [vp]
+    for name in ("fe_get_l2g", "fe_get_node_coords", "fe_get_quad_coords", "fe_get_mass", "fe_get_dirichlet_mask"):
+        getattr(L, name).restype, getattr(L, name).argtypes = C.c_int, [vp, vp]
+    L.fe_set_potential.restype, L.fe_set_potential.argtypes = C.c_int, [vp, vp, C.c_int, vp]
+    L.fe_apply_H.restype, L.fe_apply_H.argtypes = C.c_int, [vp, vp, vp, C.c_int, vp, vp]
+    L.cheb_filter.restype = C.c_int
+    L.cheb_filter.argtypes = [vp, vp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, vp, vp]
+    L.fe_set_variant.restype, L.fe_set_variant.argtypes = C.c_int, [vp, C.c_int]
+    L.fe_last_error.restype, L.fe_last_error.argtypes = C.c_char_p, []
+    _lib = L
+    return L
+
+
+def fe_last_error():
+    return load_library().fe_last_error().decode()
+
+
+def _check(rc):
+    if rc != 0:
+        raise FEError(rc, fe_last_error())
+
+
+def _edges(a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a, a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _stream(stream):
+    if stream is not None:
+        return C.c_void_p(int(stream))
+    import torch
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _dev_ptr(t, name, numel=None):
+    """Raw device pointer of a contiguous float64 CUDA tensor."""
+    import torch
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous():
+        raise FEError(-1, "%s must be a contiguous float64 CUDA tensor" % name)
+    if numel is not None and t.numel() != numel:
+        raise FEError(-1, "%s has %d elements, expected %d" % (name, t.numel(), numel))
+    return C.c_void_p(t.data_ptr())
+
+
+# ---- the C ABI, same names ---------------------------------------------------------------------------------------
+def fe_mesh_create(xe, ye, ze, p, cuda_device=0):
+    L = load_library()
+    (xa, xp), (ya, yp), (za, zp) = _edges(xe), _edges(ye), _edges(ze)
+    h = C.c_void_p()
+    _check(L.fe_mesh_create(xp, len(xa) - 1, yp, len(ya) - 1, zp, len(za) - 1, int(p), int(cuda_device), C.byref(h)))
+    return h
+
+
+def fe_mesh_destroy(h):
+    _check(load_library().fe_mesh_destroy(h))
+
+
+def fe_num_nodes(h):
+    return load_library().fe_num_nodes(h)
+
+
+def fe_num_free(h):
+    return load_library().fe_num_free(h)
+
+
+def fe_num_cells(h):
+    return load_library().fe_num_cells(h)
+
+
+def fe_nodes_per_cell(h):
+    return load_library().fe_nodes_per_cell(h)
+
+
+def fe_quad_per_cell(h):
+    return load_library().fe_quad_per_cell(h)
+
+
+def fe_launch_count(h):
+    return load_library().fe_launch_count(h)
+
+
+def _fill(h, fn, shape, dtype):
+    out = np.empty(shape, dtype=dtype)
+    _check(getattr(load_library(), fn)(h, C.c_void_p(out.ctypes.data)))
+    return out
+
+
+def fe_get_l2g(h):
+    return _fill(h, "fe_get_l2g", (fe_num_cells(h), fe_nodes_per_cell(h)), np.int32)
+
+
+def fe_get_node_coords(h):
+    return _fill(h, "fe_get_node_coords", (fe_num_nodes(h), 3), np.float64)
+
+
+def fe_get_quad_coords(h):
+    return _fill(h, "fe_get_quad_coords", (fe_num_cells(h) * fe_quad_per_cell(h), 3), np.float64)
+
+
+def fe_get_mass(h):
+    return _fill(h, "fe_get_mass", (fe_num_nodes(h),), np.float64)
+
+
+def fe_get_dirichlet_mask(h):
+    return _fill(h, "fe_get_dirichlet_mask", (fe_num_nodes(h),), np.uint8)
+
+
+def fe_set_potential(h, Vq_dev, copy=1, stream=None):
+    n = fe_num_cells(h) * fe_quad_per_cell(h)
+    _check(load_library().fe_set_potential(h, _dev_ptr(Vq_dev, "Vq", n), int(copy), _stream(stream)))
+
+
+def fe_apply_H(h, X, Y, eps=None, stream=None):
+    if X.dim() != 2 or X.shape[0] != fe_num_nodes(h):
+        raise FEError(-1, "X must be N x B")
+    B = X.shape[1]
+    ep = _dev_ptr(eps, "eps", B) if eps is not None else None
+    _check(load_library().fe_apply_H(h, _dev_ptr(X, "X"), _dev_ptr(Y, "Y", X.numel()), B, ep, _stream(stream)))
+    return Y
+
+
+def cheb_filter(h, X, m, a, b, a0, work, stream=None):
+    if X.dim() != 2 or X.shape[0] != fe_num_nodes(h):
+        raise FEError(-1, "X must be N x B")
+    B = X.shape[1]
+    _check(load_library().cheb_filter(h, _dev_ptr(X, "X"), B, int(m), float(a), float(b), float(a0),
+                                      _dev_ptr(work, "work", 2 * X.numel()), _stream(stream)))
+    return X
+
+
+def fe_set_variant(h, variant):
+    _check(load_library().fe_set_variant(h, int(variant)))
+
+
+# ---- convenience wrapper -----------------------------------------------------------------------------------------
+class FEMesh:
+    """Owns an fe_mesh handle.  All array arguments are torch CUDA float64 tensors; results stay on the device."""
+
+    def __init__(self, xe, ye, ze, p, device=0):
+        self.device = int(device)
+        self.h = fe_mesh_create(xe, ye, ze, p, self.device)
+        self.p = int(p)
+        self.N, self.N_free, self.ncells = fe_num_nodes(self.h), fe_num_free(self.h), fe_num_cells(self.h)
+        self.nc, self.nq3 = fe_nodes_per_cell(self.h), fe_quad_per_cell(self.h)
+
+    def close(self):
+        if getattr(self, "h", None):
+            fe_mesh_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    l2g = lambda self: fe_get_l2g(self.h)  # noqa: E731
+    node_coords = lambda self: fe_get_node_coords(self.h)  # noqa: E731
+    quad_coords = lambda self: fe_get_quad_coords(self.h)  # noqa: E731
+    mass = lambda self: fe_get_mass(self.h)  # noqa: E731
+    mask = lambda self: fe_get_dirichlet_mask(self.h)  # noqa: E731
+
+    def set_potential(self, Vq, stream=None):
+        import torch
+        if not isinstance(Vq, torch.Tensor):
+            Vq = torch.as_tensor(np.ascontiguousarray(Vq, dtype=np.float64), device="cuda:%d" % self.device)
+        fe_set_potential(self.h, Vq.reshape(-1), 1, stream)
+
+    def apply_H(self, X, Y=None, eps=None, stream=None):
+        import torch
+        if Y is None:
+            Y = torch.empty_like(X)
+        return fe_apply_H(self.h, X, Y, eps, stream)
+
+    def cheb_filter(self, X, m, a, b, a0, work=None, stream=None):
+        import torch
+        if work is None:
+            work = torch.empty(2 * X.numel(), dtype=torch.float64, device=X.device)
+        return cheb_filter(self.h, X, m, a, b, a0, work, stream)
+
+    def set_variant(self, v):
+        fe_set_variant(self.h, v)
+
+    @property
+    def launches(self):
+        return fe_launch_count(self.h)

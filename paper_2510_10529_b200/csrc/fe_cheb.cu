@@ -1,0 +1,336 @@
+// fe_cheb.cu -- C-ABI entry points (include/fe_cheb.h) and host-side mesh setup.
+//
+// The operator H~ = M^{-1/2} (1/2 K + M_V) M^{-1/2} (Eq. 17, 19) is never stored: every apply runs the
+// fused gather -> sum-factorised cell contraction -> scatter kernels of fe_kernels.cuh on the caller's stream.
+#include "../../include/fe_cheb.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "fe_kernels.cuh"
+#include "fe_tables.h"
+
+using namespace fecheb;
+
+static thread_local char g_err[512] = "";
+
+static int fail(int code, const char* fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CUDA_TRY(expr)                                                                              \
+    do {                                                                                            \
+        cudaError_t e_ = (expr);                                                                    \
+        if (e_ != cudaSuccess)                                                                      \
+            return fail(e_ == cudaErrorMemoryAllocation ? FE_ERR_NOMEM : FE_ERR_CUDA, "%s: %s", #expr, \
+                        cudaGetErrorString(e_));                                                    \
+    } while (0)
+
+struct fe_mesh {
+    int p = 0, n = 0, cx = 0, cy = 0, cz = 0, device = 0, nc = 0;
+    int64_t Nx = 0, Ny = 0, Nz = 0, N = 0, ncells = 0;
+    std::vector<double> xe, ye, ze;
+    Tables1D tab;
+    std::vector<double> mx, my, mz;  // per-axis lumped GLL mass: M_gg = mx[gx] my[gy] mz[gz]
+    double* d_sm = nullptr;          // N: mu_g M_gg^{-1/2} (0 on the Dirichlet boundary)
+    double *d_hx = nullptr, *d_hy = nullptr, *d_hz = nullptr;
+    double* d_WV = nullptr;  // cells*n^3: J w_q V_q
+    bool have_V = false;
+    int variant = 0;
+    int64_t launches = 0;
+};
+
+const char* fe_last_error(void) { return g_err; }
+
+static void axis_mass(const std::vector<double>& e, int c, int p, const Tables1D& t, std::vector<double>& m)
+{
+    m.assign((size_t)c * p + 1, 0.0);
+    for (int ec = 0; ec < c; ++ec)
+        for (int a = 0; a <= p; ++a) m[(size_t)ec * p + a] += 0.5 * (e[ec + 1] - e[ec]) * t.gll_w[a];
+}
+
+static int upload(double** dst, const std::vector<double>& src)
+{
+    CUDA_TRY(cudaMalloc((void**)dst, src.size() * sizeof(double)));
+    CUDA_TRY(cudaMemcpy(*dst, src.data(), src.size() * sizeof(double), cudaMemcpyHostToDevice));
+    return FE_OK;
+}
+
+int fe_mesh_create(const double* xe, int cx, const double* ye, int cy, const double* ze, int cz, int p,
+                   int cuda_device, fe_mesh** out)
+{
+    if (!out) return fail(FE_ERR_INVALID, "fe_mesh_create: out is NULL");
+    *out = nullptr;
+    if (!xe || !ye || !ze) return fail(FE_ERR_INVALID, "fe_mesh_create: NULL edge array");
+    if (p < 1 || p > 8) return fail(FE_ERR_INVALID, "fe_mesh_create: order p=%d outside 1..8", p);
+    if (cx < 1 || cy < 1 || cz < 1) return fail(FE_ERR_INVALID, "fe_mesh_create: need at least one cell per axis");
+    const double* ed[3] = {xe, ye, ze};
+    const int cc[3] = {cx, cy, cz};
+    for (int d = 0; d < 3; ++d)
+        for (int i = 0; i < cc[d]; ++i)
+            if (!(ed[d][i + 1] > ed[d][i]) || !std::isfinite(ed[d][i]) || !std::isfinite(ed[d][i + 1]))
+                return fail(FE_ERR_INVALID, "fe_mesh_create: edges of axis %d not strictly increasing at %d", d, i);
+    const int64_t Nx = (int64_t)cx * p + 1, Ny = (int64_t)cy * p + 1, Nz = (int64_t)cz * p + 1;
+    if ((double)Nx * (double)Ny * (double)Nz > 2147483647.0)
+        return fail(FE_ERR_INVALID, "fe_mesh_create: more than 2^31-1 nodes (int32 l2g, R3)");
+    int ndev = 0;
+    CUDA_TRY(cudaGetDeviceCount(&ndev));
+    if (cuda_device < 0 || cuda_device >= ndev) return fail(FE_ERR_INVALID, "fe_mesh_create: no CUDA device %d", cuda_device);
+    CUDA_TRY(cudaSetDevice(cuda_device));
+    cudaDeviceProp prop;
+    CUDA_TRY(cudaGetDeviceProperties(&prop, cuda_device));
+    if (prop.major < 10) return fail(FE_ERR_CUDA, "fe_mesh_create: device %d is sm_%d%d; this library is built for sm_100a only", cuda_device, prop.major, prop.minor);
+
+    fe_mesh* m = new (std::nothrow) fe_mesh;
+    if (!m) return fail(FE_ERR_NOMEM, "fe_mesh_create: host allocation failed");
+    m->p = p; m->n = p + 1; m->cx = cx; m->cy = cy; m->cz = cz; m->device = cuda_device;
+    m->nc = m->n * m->n * m->n;
+    m->Nx = Nx; m->Ny = Ny; m->Nz = Nz; m->N = Nx * Ny * Nz; m->ncells = (int64_t)cx * cy * cz;
+    m->xe.assign(xe, xe + cx + 1); m->ye.assign(ye, ye + cy + 1); m->ze.assign(ze, ze + cz + 1);
+    build_tables(p, &m->tab);
+    axis_mass(m->xe, cx, p, m->tab, m->mx);
+    axis_mass(m->ye, cy, p, m->tab, m->my);
+    axis_mass(m->ze, cz, p, m->tab, m->mz);
+
+    // per-axis M^{-1/2} with the Dirichlet mask folded in (R5, R6), and per-axis cell sizes
+    std::vector<double> s[3], h[3];
+    const std::vector<double>* mm[3] = {&m->mx, &m->my, &m->mz};
+    const std::vector<double>* ee[3] = {&m->xe, &m->ye, &m->ze};
+    for (int d = 0; d < 3; ++d) {
+        size_t nn = mm[d]->size();
+        s[d].resize(nn);
+        for (size_t i = 0; i < nn; ++i) s[d][i] = (i == 0 || i == nn - 1) ? 0.0 : 1.0 / std::sqrt((*mm[d])[i]);
+        h[d].resize(cc[d]);
+        for (int i = 0; i < cc[d]; ++i) h[d][i] = (*ee[d])[i + 1] - (*ee[d])[i];
+    }
+    double *d_sx = nullptr, *d_sy = nullptr, *d_sz = nullptr;
+    int rc = FE_OK;
+    auto cleanup = [&](int code) {
+        cudaFree(d_sx); cudaFree(d_sy); cudaFree(d_sz);
+        if (code != FE_OK) fe_mesh_destroy(m);
+        return code;
+    };
+    if ((rc = upload(&d_sx, s[0])) || (rc = upload(&d_sy, s[1])) || (rc = upload(&d_sz, s[2]))) return cleanup(rc);
+    if ((rc = upload(&m->d_hx, h[0])) || (rc = upload(&m->d_hy, h[1])) || (rc = upload(&m->d_hz, h[2]))) return cleanup(rc);
+    cudaError_t ce = cudaMalloc((void**)&m->d_sm, (size_t)m->N * sizeof(double));
+    if (ce == cudaSuccess) ce = cudaMalloc((void**)&m->d_WV, (size_t)m->ncells * m->nc * sizeof(double));
+    if (ce != cudaSuccess) return cleanup(fail(FE_ERR_NOMEM, "fe_mesh_create: device allocation failed: %s", cudaGetErrorString(ce)));
+    launch_build_scaling(d_sx, d_sy, d_sz, m->Nx, m->Ny, m->Nz, m->d_sm, 0);
+    m->launches += 1;
+    ce = cudaDeviceSynchronize();
+    if (ce != cudaSuccess) return cleanup(fail(FE_ERR_CUDA, "fe_mesh_create: scaling kernel failed: %s", cudaGetErrorString(ce)));
+    *out = m;
+    return cleanup(FE_OK);
+}
+
+int fe_mesh_destroy(fe_mesh* m)
+{
+    if (!m) return FE_OK;
+    cudaSetDevice(m->device);
+    cudaFree(m->d_sm); cudaFree(m->d_hx); cudaFree(m->d_hy); cudaFree(m->d_hz); cudaFree(m->d_WV);
+    delete m;
+    return FE_OK;
+}
+
+int64_t fe_num_nodes(const fe_mesh* m) { return m ? m->N : FE_ERR_INVALID; }
+int64_t fe_num_free(const fe_mesh* m) { return m ? (m->Nx - 2) * (m->Ny - 2) * (m->Nz - 2) : FE_ERR_INVALID; }
+int64_t fe_num_cells(const fe_mesh* m) { return m ? m->ncells : FE_ERR_INVALID; }
+int fe_nodes_per_cell(const fe_mesh* m) { return m ? m->nc : FE_ERR_INVALID; }
+int fe_quad_per_cell(const fe_mesh* m) { return m ? m->nc : FE_ERR_INVALID; }
+int64_t fe_launch_count(const fe_mesh* m) { return m ? m->launches : FE_ERR_INVALID; }
+
+int fe_get_l2g(const fe_mesh* m, int32_t* l2g)
+{
+    if (!m || !l2g) return fail(FE_ERR_INVALID, "fe_get_l2g: NULL argument");
+    const int n = m->n, p = m->p;
+    for (int64_t ez = 0; ez < m->cz; ++ez)
+        for (int64_t ey = 0; ey < m->cy; ++ey)
+            for (int64_t ex = 0; ex < m->cx; ++ex) {
+                int32_t* row = l2g + (ex + m->cx * (ey + m->cy * ez)) * m->nc;
+                const int64_t base = ex * p + m->Nx * (ey * p + m->Ny * (ez * p));
+                for (int az = 0; az < n; ++az)
+                    for (int ay = 0; ay < n; ++ay)
+                        for (int ax = 0; ax < n; ++ax)
+                            row[ax + n * (ay + n * az)] = (int32_t)(base + ax + m->Nx * (ay + m->Ny * az));
+            }
+    return FE_OK;
+}
+
+// R4: x = lo + 0.5 (xi+1) (hi-lo); the last GLL node of a cell is exactly the upper edge
+static void axis_coords(const std::vector<double>& e, int c, int p, const double* xi, bool lobatto, std::vector<double>& out)
+{
+    const int n = p + 1;
+    out.resize(lobatto ? (size_t)c * p + 1 : (size_t)c * n);
+    for (int ec = 0; ec < c; ++ec)
+        for (int a = 0; a < n; ++a) {
+            double v = (lobatto && a == p) ? e[ec + 1] : e[ec] + 0.5 * (xi[a] + 1.0) * (e[ec + 1] - e[ec]);
+            out[lobatto ? (size_t)ec * p + a : (size_t)ec * n + a] = v;
+        }
+}
+
+int fe_get_node_coords(const fe_mesh* m, double* xyz)
+{
+    if (!m || !xyz) return fail(FE_ERR_INVALID, "fe_get_node_coords: NULL argument");
+    std::vector<double> X, Y, Z;
+    axis_coords(m->xe, m->cx, m->p, m->tab.gll_x, true, X);
+    axis_coords(m->ye, m->cy, m->p, m->tab.gll_x, true, Y);
+    axis_coords(m->ze, m->cz, m->p, m->tab.gll_x, true, Z);
+    for (int64_t gz = 0; gz < m->Nz; ++gz)
+        for (int64_t gy = 0; gy < m->Ny; ++gy)
+            for (int64_t gx = 0; gx < m->Nx; ++gx) {
+                double* o = xyz + 3 * (gx + m->Nx * (gy + m->Ny * gz));
+                o[0] = X[gx]; o[1] = Y[gy]; o[2] = Z[gz];
+            }
+    return FE_OK;
+}
+
+int fe_get_quad_coords(const fe_mesh* m, double* xyz)
+{
+    if (!m || !xyz) return fail(FE_ERR_INVALID, "fe_get_quad_coords: NULL argument");
+    const int n = m->n;
+    std::vector<double> X, Y, Z;
+    axis_coords(m->xe, m->cx, m->p, m->tab.gl_x, false, X);
+    axis_coords(m->ye, m->cy, m->p, m->tab.gl_x, false, Y);
+    axis_coords(m->ze, m->cz, m->p, m->tab.gl_x, false, Z);
+    for (int64_t ez = 0; ez < m->cz; ++ez)
+        for (int64_t ey = 0; ey < m->cy; ++ey)
+            for (int64_t ex = 0; ex < m->cx; ++ex) {
+                double* o = xyz + 3 * (ex + m->cx * (ey + m->cy * ez)) * m->nc;
+                for (int qz = 0; qz < n; ++qz)
+                    for (int qy = 0; qy < n; ++qy)
+                        for (int qx = 0; qx < n; ++qx) {
+                            double* q = o + 3 * (qx + n * (qy + n * qz));
+                            q[0] = X[ex * n + qx]; q[1] = Y[ey * n + qy]; q[2] = Z[ez * n + qz];
+                        }
+            }
+    return FE_OK;
+}
+
+int fe_get_mass(const fe_mesh* m, double* Mdiag)
+{
+    if (!m || !Mdiag) return fail(FE_ERR_INVALID, "fe_get_mass: NULL argument");
+    for (int64_t gz = 0; gz < m->Nz; ++gz)
+        for (int64_t gy = 0; gy < m->Ny; ++gy)
+            for (int64_t gx = 0; gx < m->Nx; ++gx) Mdiag[gx + m->Nx * (gy + m->Ny * gz)] = m->mx[gx] * m->my[gy] * m->mz[gz];
+    return FE_OK;
+}
+
+int fe_get_dirichlet_mask(const fe_mesh* m, uint8_t* mask)
+{
+    if (!m || !mask) return fail(FE_ERR_INVALID, "fe_get_dirichlet_mask: NULL argument");
+    for (int64_t gz = 0; gz < m->Nz; ++gz)
+        for (int64_t gy = 0; gy < m->Ny; ++gy)
+            for (int64_t gx = 0; gx < m->Nx; ++gx)
+                mask[gx + m->Nx * (gy + m->Ny * gz)] =
+                    (gx == 0 || gx == m->Nx - 1 || gy == 0 || gy == m->Ny - 1 || gz == 0 || gz == m->Nz - 1) ? 0 : 1;
+    return FE_OK;
+}
+
+static void fill_params(const fe_mesh* m, ApplyParams* prm)
+{
+    memset(prm, 0, sizeof(*prm));
+    prm->sm = m->d_sm; prm->WV = m->d_WV; prm->hx = m->d_hx; prm->hy = m->d_hy; prm->hz = m->d_hz;
+    prm->cx = m->cx; prm->cy = m->cy; prm->cz = m->cz;
+    prm->Nx = m->Nx; prm->NxNy = m->Nx * m->Ny;
+    const int n = m->n;
+    for (int q = 0; q < n; ++q) {
+        prm->w[q] = m->tab.gl_w[q];
+        for (int a = 0; a < n; ++a) {
+            prm->N[q * n + a] = m->tab.N[q * n + a];
+            prm->G[q * n + a] = m->tab.G[q * n + a];
+        }
+    }
+}
+
+int fe_set_potential(fe_mesh* m, const double* Vq_dev, int copy, void* cuda_stream)
+{
+    (void)copy;
+    if (!m || !Vq_dev) return fail(FE_ERR_INVALID, "fe_set_potential: NULL argument");
+    CUDA_TRY(cudaSetDevice(m->device));
+    ApplyParams prm;
+    fill_params(m, &prm);
+    launch_weight_potential(prm, m->p, Vq_dev, m->d_WV, m->ncells, (cudaStream_t)cuda_stream);
+    CUDA_TRY(cudaGetLastError());
+    m->launches += 1;
+    m->have_V = true;
+    return FE_OK;
+}
+
+int fe_set_variant(fe_mesh* m, int variant)
+{
+    if (!m) return fail(FE_ERR_INVALID, "fe_set_variant: NULL mesh");
+    if (!variant_supported(m->p, variant)) return fail(FE_ERR_INVALID, "fe_set_variant: variant %d not available for p=%d", variant, m->p);
+    m->variant = variant;
+    return FE_OK;
+}
+
+// one fused operator launch: Y = mu (alpha (S sum_e P_e^T y_e - (c + eps) X) + beta Z)
+static int operator_step(fe_mesh* m, const double* X, const double* Z, double* Y, int B, const double* eps,
+                         double alpha, double beta, double c, cudaStream_t st)
+{
+    ApplyParams prm;
+    fill_params(m, &prm);
+    prm.X = X; prm.Z = Z; prm.Y = Y; prm.eps = eps; prm.B = B;
+    prm.alpha = alpha; prm.beta = beta; prm.c = c;
+    int nl = 0;
+    cudaError_t e = launch_apply(prm, m->p, m->variant, m->N, m->ncells, st, &nl);
+    if (e != cudaSuccess) return fail(FE_ERR_CUDA, "operator launch failed: %s", cudaGetErrorString(e));
+    m->launches += nl;
+    return FE_OK;
+}
+
+static bool overlap(const double* a, size_t na, const double* b, size_t nb)
+{
+    return a < b + nb && b < a + na;
+}
+
+int fe_apply_H(fe_mesh* m, const double* X, double* Y, int B, const double* eps_dev, void* cuda_stream)
+{
+    if (!m || !X || !Y) return fail(FE_ERR_INVALID, "fe_apply_H: NULL argument");
+    if (B < 1) return fail(FE_ERR_INVALID, "fe_apply_H: B=%d < 1", B);
+    if (!m->have_V) return fail(FE_ERR_STATE, "fe_apply_H: call fe_set_potential first");
+    const size_t len = (size_t)m->N * B;
+    if (overlap(X, len, Y, len)) return fail(FE_ERR_INVALID, "fe_apply_H: X and Y overlap");
+    CUDA_TRY(cudaSetDevice(m->device));
+    return operator_step(m, X, nullptr, Y, B, eps_dev, 1.0, 0.0, 0.0, (cudaStream_t)cuda_stream);
+}
+
+int cheb_filter(fe_mesh* m, double* X, int B, int deg, double a, double b, double a0, double* work, void* cuda_stream)
+{
+    if (!m || !X || !work) return fail(FE_ERR_INVALID, "cheb_filter: NULL argument");
+    if (B < 1 || deg < 1) return fail(FE_ERR_INVALID, "cheb_filter: need B >= 1 and degree >= 1 (B=%d, m=%d)", B, deg);
+    if (!(a0 < a && a < b) || !std::isfinite(a0) || !std::isfinite(b))
+        return fail(FE_ERR_INVALID, "cheb_filter: need a0 < a < b (a0=%g a=%g b=%g)", a0, a, b);
+    if (!m->have_V) return fail(FE_ERR_STATE, "cheb_filter: call fe_set_potential first");
+    const size_t len = (size_t)m->N * B;
+    if (overlap(X, len, work, 2 * len)) return fail(FE_ERR_INVALID, "cheb_filter: work overlaps X");
+    CUDA_TRY(cudaSetDevice(m->device));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    // l.208-210 / R7.  Three blocks rotate: Y_k lives in buf[k % 3], buf = {X, work, work + N*B}.
+    double* buf[3] = {X, work, work + len};
+    const double e = 0.5 * (b - a), c = 0.5 * (b + a);
+    const double sigma1 = e / (a0 - c);
+    double sigma = sigma1;
+    int rc = operator_step(m, buf[0], nullptr, buf[1], B, nullptr, sigma1 / e, 0.0, c, st);
+    if (rc) return rc;
+    for (int k = 1; k < deg; ++k) {
+        const double sigma_next = 1.0 / (2.0 / sigma1 - sigma);
+        rc = operator_step(m, buf[k % 3], buf[(k - 1) % 3], buf[(k + 1) % 3], B, nullptr, 2.0 * sigma_next / e,
+                           -sigma * sigma_next, c, st);
+        if (rc) return rc;
+        sigma = sigma_next;
+    }
+    if (deg % 3 != 0) CUDA_TRY(cudaMemcpyAsync(X, buf[deg % 3], len * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    return FE_OK;
+}

@@ -1,0 +1,272 @@
+// fe_kernels.cuh -- sm_100a kernels of the fused operator step
+//
+//   Y[g,j] = mu_g ( alpha ( s_g sum_{e∋g} y_e[a,j] - (c + eps_j) X[g,j] ) + beta Z[g,j] )
+//
+// with y_e = (1/2 K_e + M_{V,e}) (mu s X)_e evaluated matrix-free by sum factorisation (Eq. 17 l.171 on an
+// axis-aligned cell; l.237 "cell-level dense-dense products", here never formed as matrices):
+//
+//   A  = (Ny Nx) x_e                                      per nodal z-plane        (interpolate to Gauss points in x,y)
+//   A2 = kx wy (Gx A) + ky wx (Gy A)                      per nodal z-plane        (x,y stiffness in Gauss space)
+//   U = Nz A, U2 = Nz A2                                  per (qx,qy) line
+//   T = WV.U + wz.U2 + kz wx wy (Gz U),  R = Nz^T T       per (qx,qy) line
+//   y_e = Nx^T Ny^T R                                     per nodal z-plane
+//
+// N[q][a] = l_a(xi_q) (Eq. 12), G = D~^T W D~ the 1-D stiffness on the Gauss points, WV = J w_q V_q,
+// kd = 1/2 J (2/h_d)^2.  Lanes of a warp are consecutive VECTORS j (the layout of l.233-235 makes every global and
+// shared access of a warp one contiguous 8*BT-byte row); a thread owns one z-plane (n x n values in registers) in
+// the plane phases and n z-lines in the line phase, so 1-D matrix entries are warp-uniform constant-bank operands.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace fecheb {
+
+struct ApplyParams {
+    const double* X;
+    const double* Z;
+    double* Y;
+    const double* eps;
+    const double* sm;  // N: mu_g M_gg^{-1/2}
+    const double* WV;  // cells*n^3
+    const double *hx, *hy, *hz;
+    int B, cx, cy, cz;
+    long long Nx, NxNy;
+    double alpha, beta, c;
+    double N[81], G[81], w[9];
+};
+
+__global__ void k_build_scaling(const double* __restrict__ sx, const double* __restrict__ sy,
+                                const double* __restrict__ sz, long long Nx, long long Ny, long long Nz,
+                                double* __restrict__ sm)
+{
+    long long total = Nx * Ny * Nz;
+    for (long long g = blockIdx.x * (long long)blockDim.x + threadIdx.x; g < total; g += (long long)gridDim.x * blockDim.x) {
+        long long gx = g % Nx, gy = (g / Nx) % Ny, gz = g / (Nx * Ny);
+        sm[g] = sx[gx] * sy[gy] * sz[gz];
+    }
+}
+
+inline void launch_build_scaling(const double* sx, const double* sy, const double* sz, long long Nx, long long Ny,
+                                 long long Nz, double* sm, cudaStream_t st)
+{
+    k_build_scaling<<<148 * 8, 256, 0, st>>>(sx, sy, sz, Nx, Ny, Nz, sm);
+}
+
+// WV[e][q] = J_e w_qx w_qy w_qz V[e][q]
+__global__ void k_weight_potential(const __grid_constant__ ApplyParams prm, int n, const double* __restrict__ V,
+                                   double* __restrict__ WV, long long ncells)
+{
+    const int n3 = n * n * n;
+    long long total = ncells * n3;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+        long long e = i / n3;
+        int q = (int)(i - e * n3);
+        int qx = q % n, qy = (q / n) % n, qz = q / (n * n);
+        int ex = (int)(e % prm.cx), ey = (int)((e / prm.cx) % prm.cy), ez = (int)(e / ((long long)prm.cx * prm.cy));
+        double J = prm.hx[ex] * prm.hy[ey] * prm.hz[ez] * 0.125;
+        WV[i] = J * prm.w[qx] * prm.w[qy] * prm.w[qz] * V[i];
+    }
+}
+
+inline void launch_weight_potential(const ApplyParams& prm, int p, const double* V, double* WV, long long ncells,
+                                    cudaStream_t st)
+{
+    k_weight_potential<<<148 * 8, 256, 0, st>>>(prm, p + 1, V, WV, ncells);
+}
+
+// ---- variant 1: plain sum factorisation, atomics scatter --------------------------------------------------------
+// out[i] = sum_k M[i*n+k] in[k]   (TRANS: out[i] = sum_k M[k*n+i] in[k])
+template <int n, bool TRANS>
+__device__ __forceinline__ void mat1d(const double* __restrict__ M, const double (&in)[n], double (&out)[n])
+{
+#pragma unroll
+    for (int i = 0; i < n; ++i) {
+        double s = 0.0;
+#pragma unroll
+        for (int k = 0; k < n; ++k) s = fma(TRANS ? M[k * n + i] : M[i * n + k], in[k], s);
+        out[i] = s;
+    }
+}
+
+template <int P, int BT>
+__global__ void __launch_bounds__((P + 1) * BT) k_apply_v1(const __grid_constant__ ApplyParams prm)
+{
+    constexpr int n = P + 1, n3 = n * n * n;
+    extern __shared__ double smem[];
+    double* sA = smem;             // [n^3][BT]
+    double* sA2 = smem + n3 * BT;  // [n^3][BT]
+    const int lane = threadIdx.x, pl = threadIdx.y;
+    const int cell = blockIdx.x;
+    const int ex = cell % prm.cx, ey = (cell / prm.cx) % prm.cy, ez = cell / (prm.cx * prm.cy);
+    const int j = blockIdx.y * BT + lane;
+    const bool act = j < prm.B;
+    const long long B = prm.B;
+    const long long gbase = (long long)ex * P + prm.Nx * ((long long)ey * P) + prm.NxNy * ((long long)ez * P);
+    const double hx = prm.hx[ex], hy = prm.hy[ey], hz = prm.hz[ez];
+    const double J = hx * hy * hz * 0.125;
+    const double kx = 0.5 * J * 4.0 / (hx * hx), ky = 0.5 * J * 4.0 / (hy * hy), kz = 0.5 * J * 4.0 / (hz * hz);
+
+    double v[n][n], t[n], o[n];
+    // ---- plane phase 1: gather (a1) with mu*s pre-scale, interpolate in x and y --------------------------------
+    {
+        const long long gpl = gbase + prm.NxNy * pl;
+#pragma unroll
+        for (int ay = 0; ay < n; ++ay)
+#pragma unroll
+            for (int ax = 0; ax < n; ++ax) {
+                const long long g = gpl + ax + prm.Nx * ay;
+                v[ay][ax] = act ? prm.X[g * B + j] * prm.sm[g] : 0.0;
+            }
+    }
+#pragma unroll
+    for (int ay = 0; ay < n; ++ay) {
+        mat1d<n, false>(prm.N, v[ay], o);
+#pragma unroll
+        for (int q = 0; q < n; ++q) v[ay][q] = o[q];
+    }
+#pragma unroll
+    for (int qx = 0; qx < n; ++qx) {
+#pragma unroll
+        for (int a = 0; a < n; ++a) t[a] = v[a][qx];
+        mat1d<n, false>(prm.N, t, o);
+#pragma unroll
+        for (int q = 0; q < n; ++q) v[q][qx] = o[q];
+    }
+    {
+        double v2[n][n];
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy) {
+            mat1d<n, false>(prm.G, v[qy], o);
+#pragma unroll
+            for (int qx = 0; qx < n; ++qx) v2[qy][qx] = (kx * prm.w[qy]) * o[qx];
+        }
+#pragma unroll
+        for (int qx = 0; qx < n; ++qx) {
+#pragma unroll
+            for (int a = 0; a < n; ++a) t[a] = v[a][qx];
+            mat1d<n, false>(prm.G, t, o);
+#pragma unroll
+            for (int qy = 0; qy < n; ++qy) v2[qy][qx] = fma(ky * prm.w[qx], o[qy], v2[qy][qx]);
+        }
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy)
+#pragma unroll
+            for (int qx = 0; qx < n; ++qx) {
+                const int idx = ((pl * n + qy) * n + qx) * BT + lane;
+                sA[idx] = v[qy][qx];
+                sA2[idx] = v2[qy][qx];
+            }
+    }
+    __syncthreads();
+    // ---- line phase: z interpolation, pointwise potential and z stiffness, z back-interpolation --------------------
+    {
+        const double* WVc = prm.WV + (long long)cell * n3;
+#pragma unroll 1
+        for (int r = 0; r < n; ++r) {
+            const int l = pl + n * r;
+            const int qx = l % n, qy = l / n;
+            double a[n], a2[n], u[n], u2[n], gu[n];
+#pragma unroll
+            for (int az = 0; az < n; ++az) {
+                const int idx = ((az * n + qy) * n + qx) * BT + lane;
+                a[az] = sA[idx];
+                a2[az] = sA2[idx];
+            }
+            mat1d<n, false>(prm.N, a, u);
+            mat1d<n, false>(prm.N, a2, u2);
+            mat1d<n, false>(prm.G, u, gu);
+            const double kzw = kz * prm.w[qx] * prm.w[qy];
+#pragma unroll
+            for (int qz = 0; qz < n; ++qz) {
+                const double wv = WVc[(qz * n + qy) * n + qx];
+                t[qz] = fma(wv, u[qz], fma(prm.w[qz], u2[qz], kzw * gu[qz]));
+            }
+            mat1d<n, true>(prm.N, t, o);
+#pragma unroll
+            for (int az = 0; az < n; ++az) sA[((az * n + qy) * n + qx) * BT + lane] = o[az];
+        }
+    }
+    __syncthreads();
+    // ---- plane phase 2: back-interpolate in y and x, fused epilogue and scatter-add (a3) ------------------------------
+#pragma unroll
+    for (int qy = 0; qy < n; ++qy)
+#pragma unroll
+        for (int qx = 0; qx < n; ++qx) v[qy][qx] = sA[((pl * n + qy) * n + qx) * BT + lane];
+#pragma unroll
+    for (int qx = 0; qx < n; ++qx) {
+#pragma unroll
+        for (int q = 0; q < n; ++q) t[q] = v[q][qx];
+        mat1d<n, true>(prm.N, t, o);
+#pragma unroll
+        for (int a = 0; a < n; ++a) v[a][qx] = o[a];
+    }
+#pragma unroll
+    for (int ay = 0; ay < n; ++ay) {
+        mat1d<n, true>(prm.N, v[ay], o);
+#pragma unroll
+        for (int a = 0; a < n; ++a) v[ay][a] = o[a];
+    }
+    if (act) {
+        const long long gpl = gbase + prm.NxNy * pl;
+        const double shift = prm.c + (prm.eps ? prm.eps[j] : 0.0);
+#pragma unroll
+        for (int ay = 0; ay < n; ++ay)
+#pragma unroll
+            for (int ax = 0; ax < n; ++ax) {
+                const long long g = gpl + ax + prm.Nx * ay;
+                const double s = prm.sm[g];
+                if (s != 0.0) {
+                    double val = prm.alpha * s * v[ay][ax];
+                    if (ax < P && ay < P && pl < P) {  // the cell that owns the node adds the diagonal terms once
+                        val = fma(-prm.alpha * shift, prm.X[g * B + j], val);
+                        if (prm.Z) val = fma(prm.beta, prm.Z[g * B + j], val);
+                    }
+                    atomicAdd(prm.Y + g * B + j, val);
+                }
+            }
+    }
+}
+
+inline bool variant_supported(int p, int variant)
+{
+    (void)p;
+    return variant == 0 || variant == 1;
+}
+
+template <int P, int BT>
+cudaError_t launch_v1(const ApplyParams& prm, long long ncells, cudaStream_t st)
+{
+    constexpr int n = P + 1;
+    const size_t smem = (size_t)2 * n * n * n * BT * sizeof(double);
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(k_apply_v1<P, BT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    dim3 grid((unsigned)ncells, (unsigned)((prm.B + BT - 1) / BT)), block(BT, n);
+    k_apply_v1<P, BT><<<grid, block, smem, st>>>(prm);
+    return cudaGetLastError();
+}
+
+// One fused operator step.  *nlaunch = kernels (and memsets) enqueued.
+inline cudaError_t launch_apply(const ApplyParams& prm, int p, int variant, long long N, long long ncells,
+                                cudaStream_t st, int* nlaunch)
+{
+    (void)variant;
+    cudaError_t e = cudaMemsetAsync(prm.Y, 0, (size_t)N * prm.B * sizeof(double), st);
+    if (e != cudaSuccess) return e;
+    *nlaunch = 1;  // kernels only; the zero-fill is a cudaMemsetAsync
+    switch (p) {
+        case 1: return launch_v1<1, 32>(prm, ncells, st);
+        case 2: return launch_v1<2, 32>(prm, ncells, st);
+        case 3: return launch_v1<3, 32>(prm, ncells, st);
+        case 4: return launch_v1<4, 32>(prm, ncells, st);
+        case 5: return launch_v1<5, 32>(prm, ncells, st);
+        case 6: return launch_v1<6, 32>(prm, ncells, st);
+        case 7: return launch_v1<7, 16>(prm, ncells, st);
+        case 8: return launch_v1<8, 16>(prm, ncells, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+}  // namespace fecheb

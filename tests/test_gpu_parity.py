@@ -1,0 +1,256 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star, reading R16): relative Frobenius error over free rows <= 1e-11 for one apply
+(plain and shifted), <= 1e-9 after cheb_filter; l2g and Dirichlet mask byte-identical.
+"""
+import numpy as np
+import pytest
+
+import workloads
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL_APPLY = 1e-11
+TOL_FILTER = 1e-9
+
+UNEQUAL = (np.array([0.0, 0.7, 2.0]), np.array([-1.0, -0.5, 0.4, 1.0]), np.array([0.0, 0.3, 1.0, 1.2, 2.5]))
+
+
+def _fe():
+    import paper_2510_10529_b200 as fe
+    return fe
+
+
+def _pair(edges, p, V):
+    """(oracle mesh with cell matrices + CSR, GPU mesh) with the same potential, evaluated ONCE at the oracle's points."""
+    import oracle
+    fe = _fe()
+    om = oracle.OracleMesh(*edges, p)
+    Vq = V(om.quad_coords())
+    om.set_potential(Vq)
+    om.assemble()
+    gm = fe.FEMesh(*edges, p)
+    gm.set_potential(Vq)
+    return om, gm
+
+
+def _relerr(Yg, Yo, mask):
+    free = mask.astype(bool)
+    return np.linalg.norm(Yg[free] - Yo[free]) / max(np.linalg.norm(Yo[free]), 1e-300)
+
+
+def _dev(a):
+    return torch.as_tensor(np.ascontiguousarray(a), device="cuda")
+
+
+def _coulomb(q):
+    return -4.0 / np.sqrt((q**2).sum(axis=1) + 0.25)
+
+
+# ---- T1: setup tables ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("p", [1, 2, 3, 4, 5, 6, 7, 8])
+def test_tables_match_oracle(p):
+    import oracle
+    fe = _fe()
+    om = oracle.OracleMesh(*UNEQUAL, p)
+    gm = fe.FEMesh(*UNEQUAL, p)
+    assert (gm.N, gm.N_free, gm.ncells, gm.nc, gm.nq3) == (om.N, om.N_free, om.ncells, om.nc, om.nq3)
+    assert np.array_equal(gm.l2g(), om.l2g())  # bit-exact (BASELINE.json)
+    assert np.array_equal(gm.mask(), om.mask())
+    assert np.max(np.abs(gm.node_coords() - om.node_coords())) <= 2 * np.spacing(2.5)
+    assert np.max(np.abs(gm.quad_coords() - om.quad_coords())) <= 2 * np.spacing(2.5)
+    Mo, Mg = om.mass(), gm.mass()
+    assert np.max(np.abs(Mg - Mo) / Mo) < 2e-15
+
+
+# ---- T2: one apply -------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("p", [1, 2, 3, 4, 5, 6, 7, 8])
+def test_apply_all_orders(p):
+    e = (np.array([0.0, 0.9, 2.0]), np.array([-1.0, 0.1, 1.0]), np.array([0.0, 0.6, 1.0]))
+    om, gm = _pair(e, p, _coulomb)
+    B = 5
+    X = workloads.random_block(100 + p, om.N, B)  # boundary rows NOT zeroed: must be ignored
+    Yo = om.apply(X)
+    Yg = gm.apply_H(_dev(X)).cpu().numpy()
+    assert _relerr(Yg, Yo, om.mask()) <= TOL_APPLY
+    assert np.all(Yg[om.mask() == 0] == 0)
+
+
+@pytest.mark.parametrize("p,B", [(2, 1), (2, 8), (3, 33), (4, 64), (2, 70)])
+def test_apply_unequal_mesh_ragged_B(p, B):
+    """2x3x4 cells with unequal edges (axis-order bugs), B = 1, a ragged tail, several tiles."""
+    om, gm = _pair(UNEQUAL, p, _coulomb)
+    X = workloads.random_block(7, om.N, B, om.mask())
+    Yo = om.apply(X)
+    Yg = gm.apply_H(_dev(X)).cpu().numpy()
+    assert _relerr(Yg, Yo, om.mask()) <= TOL_APPLY
+
+
+def test_shifted_apply():
+    """Config 5 shape on a reduced mesh: (H~ - eps_j I) X_j with sorted eps in [-2, 0] (Eq. 20, R18)."""
+    w = workloads.reduced(5, 4)
+    om, gm = _pair((w.xe, w.ye, w.ze), w.p, w.V)
+    X = workloads.random_block(w.x_seed, om.N, w.B, om.mask())
+    eps = w.eps()
+    Yo = om.apply(X, eps)
+    Yg = gm.apply_H(_dev(X), eps=_dev(eps)).cpu().numpy()
+    assert _relerr(Yg, Yo, om.mask()) <= TOL_APPLY
+    # eps == 0 reproduces the plain apply up to summation order
+    Y0 = gm.apply_H(_dev(X), eps=torch.zeros(w.B, dtype=torch.float64, device="cuda")).cpu().numpy()
+    assert _relerr(Y0, om.apply(X), om.mask()) <= TOL_APPLY
+
+
+def test_degenerate_meshes():
+    """One cell (a single free node at p=2) and the smallest mesh with a free node at p=1."""
+    e1 = np.array([0.0, 1.0])
+    om, gm = _pair((e1, e1, e1), 2, workloads.harmonic)
+    X = workloads.random_block(3, om.N, 4)
+    assert om.N_free == 1
+    assert _relerr(gm.apply_H(_dev(X)).cpu().numpy(), om.apply(X), om.mask()) <= TOL_APPLY
+    e2 = np.array([0.0, 1.0, 2.5])
+    om, gm = _pair((e2, e2, e2), 1, workloads.harmonic)
+    X = workloads.random_block(4, om.N, 3)
+    assert om.N_free == 1
+    assert _relerr(gm.apply_H(_dev(X)).cpu().numpy(), om.apply(X), om.mask()) <= TOL_APPLY
+    # all-boundary mesh: p=1, one cell -> Y == 0
+    om, gm = _pair((e1, e1, e1), 1, workloads.harmonic)
+    Y = gm.apply_H(_dev(workloads.random_block(5, om.N, 2))).cpu().numpy()
+    assert om.N_free == 0 and np.all(Y == 0)
+
+
+# ---- T3: filter ----------------------------------------------------------------------------------------------------
+def test_filter_config1():
+    """BASELINE.json config 1: 4^3 cells, p=2, V = r^2/2, B=8, m=10, bounds from 20 Lanczos steps (R10)."""
+    import oracle
+    w = workloads.config(1)
+    om, gm = _pair((w.xe, w.ye, w.ze), w.p, w.V)
+    mask = om.mask()
+    X = w.X(mask)
+    th_min, th_max, beta = oracle.lanczos_bounds(om, workloads.normal(3001, om.N), 20)
+    b, a0 = th_max + beta, th_min
+    a = a0 + 0.1 * (b - a0)
+    for deg in (1, 2, 3, w.m):
+        Yo = om.filter(X, deg, a, b, a0)
+        Yg = gm.cheb_filter(_dev(X).clone(), deg, a, b, a0).cpu().numpy()
+        assert _relerr(Yg, Yo, mask) <= TOL_FILTER, deg
+        assert np.all(Yg[mask == 0] == 0)
+
+
+def test_filter_reduced_config2_and_ritz_values():
+    """Config 2 recipe on 4^3 cells: lock-step filter parity per cycle and Ritz values of the free-running GPU cycles
+    (Eq. 23-24; R20).  The small dense steps of Rayleigh-Ritz run on the host for both sides (NEXT-1 is not built)."""
+    import oracle
+    w = workloads.reduced(2, 4)
+    om, gm = _pair((w.xe, w.ye, w.ze), w.p, w.V)
+    mask = om.mask()
+    B = 16
+    Xo = workloads.random_block(w.x_seed, om.N, B, mask)
+    Xg = Xo.copy()
+    th_min, th_max, beta = oracle.lanczos_bounds(om, workloads.normal(3002, om.N), 20)
+    b, a0 = th_max + beta, th_min
+    a = a0 + 0.1 * (b - a0)
+    ag, a0g = a, a0
+    for cycle in range(3):
+        Yo = om.filter(Xo, w.m, a, b, a0)
+        Ylock = gm.cheb_filter(_dev(Xo).clone(), w.m, a, b, a0).cpu().numpy()
+        assert _relerr(Ylock, Yo, mask) <= TOL_FILTER, cycle
+        theta_o, Xo, _ = oracle.rayleigh_ritz(om, Yo)
+        # free-running GPU cycle: its own filter output, its own H~Q through fe_apply_H
+        Yg = gm.cheb_filter(_dev(Xg).clone(), w.m, ag, b, a0g).cpu().numpy()
+        Q = Yg * mask[:, None]
+        for _ in range(2):
+            Lc = np.linalg.cholesky(Q.T @ Q)
+            Q = np.linalg.solve(Lc, Q.T).T
+        HQ = gm.apply_H(_dev(Q)).cpu().numpy()
+        G = Q.T @ HQ
+        theta_g, Vg = np.linalg.eigh(0.5 * (G + G.T))
+        Xg = Q @ Vg
+        assert np.max(np.abs(theta_g - theta_o) / np.maximum(1.0, np.abs(theta_o))) <= 1e-9, cycle
+        a, a0 = theta_o[-1], theta_o[0]
+        ag, a0g = theta_g[-1], theta_g[0]
+
+
+# ---- full BASELINE sizes: sampled rows ------------------------------------------------------------------------------
+def _sample_rows(w, count, seed):
+    """Rows spread over cell interiors, faces, edges, vertices and the boundary."""
+    nx, ny, nz = w.nodes_per_axis
+    u = workloads.uniform01(seed, 0, 3 * count).reshape(count, 3)
+    gx, gy, gz = (np.minimum((u[:, d] * n).astype(np.int64), n - 1) for d, n in enumerate((nx, ny, nz)))
+    # force a share of the rows onto cell faces / edges / vertices
+    k = count // 4
+    gx[:k] = (gx[:k] // w.p) * w.p
+    gy[:k // 2] = (gy[:k // 2] // w.p) * w.p
+    gz[:k // 4] = (gz[:k // 4] // w.p) * w.p
+    return np.unique(gx + nx * (gy + ny * gz))
+
+
+@pytest.mark.parametrize("cfg", [2, 5, 3])
+def test_apply_full_size_sampled_rows(cfg):
+    """Full BASELINE sizes in the launch configuration bench.py times; the oracle computes sampled rows one by one
+    straight from Eq. 17 (orc_apply_rows)."""
+    import oracle
+    fe = _fe()
+    w = workloads.config(cfg)
+    om = oracle.OracleMesh(w.xe, w.ye, w.ze, w.p)
+    Vq = w.V(om.quad_coords())
+    om.set_potential(Vq, build=False)
+    gm = fe.FEMesh(w.xe, w.ye, w.ze, w.p)
+    gm.set_potential(Vq)
+    assert np.array_equal(gm.mask(), om.mask())
+    X = w.X(om.mask())
+    eps = w.eps()
+    rows = _sample_rows(w, 96 if cfg != 3 else 48, 9000 + cfg)
+    Yo = om.apply_rows(X, rows, eps)
+    Xd = _dev(X)
+    Yg = gm.apply_H(Xd, eps=_dev(eps) if eps is not None else None)
+    Ys = Yg[torch.as_tensor(rows, device="cuda")].cpu().numpy()
+    assert np.linalg.norm(Ys - Yo) <= TOL_APPLY * np.linalg.norm(Yo)
+    # boundary rows are written 0 everywhere
+    bnd = torch.as_tensor(np.flatnonzero(om.mask() == 0), device="cuda")
+    assert float(Yg[bnd].abs().max()) == 0.0
+
+
+def test_filter_full_size_property():
+    """Config 2 at full size: cheb_filter equals the three-term recurrence assembled from fe_apply_H calls (which
+    the sampled-row test ties to the oracle); holds at any size."""
+    fe = _fe()
+    w = workloads.config(2)
+    gm = fe.FEMesh(w.xe, w.ye, w.ze, w.p)
+    gm.set_potential(w.V(gm.quad_coords()))
+    mask = _dev(gm.mask().astype(np.float64))[:, None]
+    X = _dev(w.X(gm.mask()))
+    a0, a, b, m = -6.0, -0.5, 190.0, 7
+    e, c = (b - a) / 2, (b + a) / 2
+    s1 = e / (a0 - c)
+    s = s1
+    Ykm, Yk = X, (s1 / e) * (gm.apply_H(X) - c * X)
+    for _ in range(1, m):
+        sn = 1.0 / (2.0 / s1 - s)
+        Ykm, Yk = Yk, (2 * sn / e) * (gm.apply_H(Yk) - c * Yk) - s * sn * Ykm
+        s = sn
+    Yf = gm.cheb_filter(X.clone(), m, a, b, a0)
+    assert float(torch.linalg.norm((Yf - Yk) * mask) / torch.linalg.norm(Yk * mask)) <= 1e-12
+
+
+# ---- error behaviour -------------------------------------------------------------------------------------------------
+def test_error_codes():
+    fe = _fe()
+    e = np.array([0.0, 1.0, 2.0])
+    with pytest.raises(fe.FEError):
+        fe.FEMesh(e, e, e, 9)
+    with pytest.raises(fe.FEError):
+        fe.FEMesh(np.array([0.0, 1.0, 1.0]), e, e, 2)
+    gm = fe.FEMesh(e, e, e, 2)
+    X = torch.zeros(gm.N, 4, dtype=torch.float64, device="cuda")
+    with pytest.raises(fe.FEError) as ei:
+        gm.apply_H(X)
+    assert ei.value.code == -4  # before fe_set_potential
+    gm.set_potential(np.zeros(gm.ncells * gm.nq3))
+    with pytest.raises(fe.FEError):
+        fe.fe_apply_H(gm.h, X, X)  # aliasing
+    with pytest.raises(fe.FEError):
+        gm.cheb_filter(X, 3, 2.0, 1.0, 0.0)  # needs a0 < a < b
+    with pytest.raises(fe.FEError):
+        gm.cheb_filter(X, 0, 1.0, 2.0, 0.0)
+    assert gm.launches >= 2
