@@ -53,7 +53,7 @@ class ClockSampler:
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.FIELDS,
-                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                       "--format=csv,noheader,nounits", "-lms", "50"], stdout=self.f,
                                       stderr=subprocess.DEVNULL)
         except OSError:
             self.p = None
@@ -149,9 +149,12 @@ def run_reference(args):
     print(json.dumps(line))
 
 
-def time_workload(fe, torch, w, steps, warmup, dev, seed_offset=0, with_e2e=False, dist=None, sample_clocks=False):
+def time_workload(fe, torch, w, steps, warmup, dev, seed_offset=0, with_e2e=False, dist=None, sample_clocks=False,
+                  variant=0):
     """Device-resident timing of `steps` cheb_filter calls (config 5: blocks of 200 shifted applies)."""
     gm = fe.FEMesh(w.xe, w.ye, w.ze, w.p, device=dev)
+    if variant:
+        gm.set_variant(variant)
     Vq = w.V(gm.quad_coords())
     gm.set_potential(Vq)
     mask = torch.as_tensor(gm.mask().astype(np.float64), device="cuda")[:, None]
@@ -242,7 +245,7 @@ def summarize(w, r, total_ms_per_step, n_ranks=1):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", type=int, default=2, choices=[2, 3, 4, 5])
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
@@ -269,9 +272,7 @@ def main():
     torch.cuda.set_device(local)
     w = workloads.config(args.workload)
     r = time_workload(fe, torch, w, args.steps, args.warmup, local, seed_offset=rank, with_e2e=True, dist=dist,
-                      sample_clocks=(rank == 0))
-    if args.variant:
-        pass
+                      sample_clocks=(rank == 0), variant=args.variant)
     ms = torch.tensor([r["ms_per_step"], r["e2e_s_per_step"] * 1e3], dtype=torch.float64, device="cuda")
     if dist is not None:
         dist.all_reduce(ms, op=dist.ReduceOp.MAX)  # max over ranks; columns are sharded with no exchange (weak)
@@ -309,7 +310,7 @@ def main():
                 continue
             wi = workloads.config(idx)
             try:
-                ri = time_workload(fe, torch, wi, 2 if idx == 4 else 3, 1 if idx == 4 else 2, local)
+                ri = time_workload(fe, torch, wi, 2 if idx == 4 else 3, 1 if idx == 4 else 2, local, variant=args.variant)
                 vi, rfi = summarize(wi, ri, ri["ms_per_step"])
                 extra["cfg%d" % idx] = {"workload": wi.describe(), "value": vi, "unit": UNIT, "ms_per_step": ri["ms_per_step"],
                                         "roofline_frac": rfi["frac"], "achieved_tflops": rfi["achieved"]}

@@ -237,6 +237,21 @@ int fe_get_dirichlet_mask(const fe_mesh* m, uint8_t* mask)
     return FE_OK;
 }
 
+// even-odd split of a centro-symmetric n x n matrix (row-major M[i*n+k]); transpose selects M^T
+static void make_eo(const double* M, int n, bool transpose, EOTab* T)
+{
+    const int h = n / 2, c = (n + 1) / 2;
+    memset(T, 0, sizeof(*T));
+    auto at = [&](int i, int k) { return transpose ? M[k * n + i] : M[i * n + k]; };
+    for (int i = 0; i < c; ++i) {
+        for (int k = 0; k < h; ++k) {
+            T->S[i * h + k] = 0.5 * (at(i, k) + at(i, n - 1 - k));
+            if (i < h) T->A[i * h + k] = 0.5 * (at(i, k) - at(i, n - 1 - k));
+        }
+        if (n % 2 == 1) T->Mid[i] = at(i, h);
+    }
+}
+
 static void fill_params(const fe_mesh* m, ApplyParams* prm)
 {
     memset(prm, 0, sizeof(*prm));
@@ -251,6 +266,9 @@ static void fill_params(const fe_mesh* m, ApplyParams* prm)
             prm->G[q * n + a] = m->tab.G[q * n + a];
         }
     }
+    make_eo(m->tab.N, n, false, &prm->eoN);
+    make_eo(m->tab.N, n, true, &prm->eoNT);
+    make_eo(m->tab.G, n, false, &prm->eoG);
 }
 
 int fe_set_potential(fe_mesh* m, const double* Vq_dev, int copy, void* cuda_stream)

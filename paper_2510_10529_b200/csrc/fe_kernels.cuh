@@ -20,6 +20,14 @@
 
 namespace fecheb {
 
+// Even-odd form of a centro-symmetric n x n matrix M (M[i][k] = M[n-1-i][n-1-k]), h = n/2, c = (n+1)/2:
+//   S[i*h+k] = (M[i][k] + M[i][n-1-k])/2 (i<c), A[i*h+k] = (M[i][k] - M[i][n-1-k])/2 (i<h), Mid[i] = M[i][h] (n odd).
+// out[i] = E_i + O_i, out[n-1-i] = E_i - O_i with E = S (in + flip in) + Mid in[h], O = A (in - flip in): about half
+// the multiplications of the plain product.
+struct EOTab {
+    double S[20], A[16], Mid[5];
+};
+
 struct ApplyParams {
     const double* X;
     const double* Z;
@@ -32,6 +40,7 @@ struct ApplyParams {
     long long Nx, NxNy;
     double alpha, beta, c;
     double N[81], G[81], w[9];
+    EOTab eoN, eoNT, eoG;  // even-odd split of N, N^T and G (all centro-symmetric: GLL and Gauss points are symmetric)
 };
 
 __global__ void k_build_scaling(const double* __restrict__ sx, const double* __restrict__ sy,
@@ -226,10 +235,211 @@ __global__ void __launch_bounds__((P + 1) * BT) k_apply_v1(const __grid_constant
     }
 }
 
+
+// ---- variant 2: even-odd sum factorisation, potential staged in shared memory --------------------------------------
+template <int n>
+__device__ __forceinline__ void mat1d_eo(const EOTab& T, const double (&in)[n], double (&out)[n])
+{
+    constexpr int h = n / 2, c = (n + 1) / 2;
+    double e[h], o[h];
+#pragma unroll
+    for (int k = 0; k < h; ++k) {
+        e[k] = in[k] + in[n - 1 - k];
+        o[k] = in[k] - in[n - 1 - k];
+    }
+#pragma unroll
+    for (int i = 0; i < c; ++i) {
+        double se;
+        if (n % 2 == 1) {
+            se = T.Mid[i] * in[h];
+#pragma unroll
+            for (int k = 0; k < h; ++k) se = fma(T.S[i * h + k], e[k], se);
+        } else {
+            se = T.S[i * h] * e[0];
+#pragma unroll
+            for (int k = 1; k < h; ++k) se = fma(T.S[i * h + k], e[k], se);
+        }
+        if (i < h) {
+            double so = T.A[i * h] * o[0];
+#pragma unroll
+            for (int k = 1; k < h; ++k) so = fma(T.A[i * h + k], o[k], so);
+            out[i] = se + so;
+            out[n - 1 - i] = se - so;
+        } else {
+            out[i] = se;
+        }
+    }
+}
+
+template <int P, int BT, int MINB>
+__global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_v2(const __grid_constant__ ApplyParams prm)
+{
+    constexpr int n = P + 1, n3 = n * n * n;
+    extern __shared__ double smem[];
+    double* sA = smem;             // [n^3][BT]
+    double* sA2 = smem + n3 * BT;  // [n^3][BT]
+    double* sWV = sA2 + n3 * BT;   // [n^3]
+    const int lane = threadIdx.x, pl = threadIdx.y;
+    const int cell = blockIdx.x;
+    const int ex = cell % prm.cx, ey = (cell / prm.cx) % prm.cy, ez = cell / (prm.cx * prm.cy);
+    const int j = blockIdx.y * BT + lane;
+    const bool act = j < prm.B;
+    const long long B = prm.B;
+    const long long gpl = (long long)ex * P + prm.Nx * ((long long)ey * P) + prm.NxNy * ((long long)ez * P + pl);
+    const double hx = prm.hx[ex], hy = prm.hy[ey], hz = prm.hz[ez];
+    const double J = hx * hy * hz * 0.125;
+    const double kx = 2.0 * J / (hx * hx), ky = 2.0 * J / (hy * hy), kz = 2.0 * J / (hz * hz);
+
+    double v[n][n], t[n], o[n];
+    // ---- plane phase 1: gather (a1) with mu*s pre-scale; interpolate in x and y; x,y stiffness ------------------------
+#pragma unroll
+    for (int ay = 0; ay < n; ++ay)
+#pragma unroll
+        for (int ax = 0; ax < n; ++ax) {
+            const long long g = gpl + ax + prm.Nx * ay;
+            v[ay][ax] = act ? prm.X[g * B + j] * prm.sm[g] : 0.0;
+        }
+    {
+        const double* WVc = prm.WV + (long long)cell * n3;
+        for (int i = pl * BT + lane; i < n3; i += n * BT) sWV[i] = WVc[i];
+    }
+#pragma unroll
+    for (int ay = 0; ay < n; ++ay) {
+        mat1d_eo<n>(prm.eoN, v[ay], o);
+#pragma unroll
+        for (int q = 0; q < n; ++q) v[ay][q] = o[q];
+    }
+#pragma unroll
+    for (int qx = 0; qx < n; ++qx) {
+#pragma unroll
+        for (int a = 0; a < n; ++a) t[a] = v[a][qx];
+        mat1d_eo<n>(prm.eoN, t, o);
+#pragma unroll
+        for (int q = 0; q < n; ++q) v[q][qx] = o[q];
+    }
+    {
+        double v2[n][n];
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy) {
+            mat1d_eo<n>(prm.eoG, v[qy], o);
+            const double f = kx * prm.w[qy];
+#pragma unroll
+            for (int qx = 0; qx < n; ++qx) v2[qy][qx] = f * o[qx];
+        }
+#pragma unroll
+        for (int qx = 0; qx < n; ++qx) {
+#pragma unroll
+            for (int a = 0; a < n; ++a) t[a] = v[a][qx];
+            mat1d_eo<n>(prm.eoG, t, o);
+            const double f = ky * prm.w[qx];
+#pragma unroll
+            for (int qy = 0; qy < n; ++qy) v2[qy][qx] = fma(f, o[qy], v2[qy][qx]);
+        }
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy)
+#pragma unroll
+            for (int qx = 0; qx < n; ++qx) {
+                const int idx = ((pl * n + qy) * n + qx) * BT + lane;
+                sA[idx] = v[qy][qx];
+                sA2[idx] = v2[qy][qx];
+            }
+    }
+    __syncthreads();
+    // ---- line phase: thread owns the n z-lines (qx = pl, qy = 0..n-1) -------------------------------------------------
+    {
+        const int qx = pl;
+        const double kzwx = kz * prm.w[qx];
+#pragma unroll 1
+        for (int qy = 0; qy < n; ++qy) {
+            double a[n], a2[n], u[n], u2[n], gu[n];
+#pragma unroll
+            for (int az = 0; az < n; ++az) {
+                const int idx = ((az * n + qy) * n + qx) * BT + lane;
+                a[az] = sA[idx];
+                a2[az] = sA2[idx];
+            }
+            mat1d_eo<n>(prm.eoN, a, u);
+            mat1d_eo<n>(prm.eoN, a2, u2);
+            mat1d_eo<n>(prm.eoG, u, gu);
+            const double kzw = kzwx * prm.w[qy];
+#pragma unroll
+            for (int qz = 0; qz < n; ++qz) {
+                const double wv = sWV[(qz * n + qy) * n + qx];
+                t[qz] = fma(wv, u[qz], fma(prm.w[qz], u2[qz], kzw * gu[qz]));
+            }
+            mat1d_eo<n>(prm.eoNT, t, o);
+#pragma unroll
+            for (int az = 0; az < n; ++az) sA[((az * n + qy) * n + qx) * BT + lane] = o[az];
+        }
+    }
+    __syncthreads();
+    // ---- plane phase 2: back-interpolate in y and x; fused epilogue and scatter-add (a3) ------------------------------
+#pragma unroll
+    for (int qy = 0; qy < n; ++qy)
+#pragma unroll
+        for (int qx = 0; qx < n; ++qx) v[qy][qx] = sA[((pl * n + qy) * n + qx) * BT + lane];
+#pragma unroll
+    for (int qx = 0; qx < n; ++qx) {
+#pragma unroll
+        for (int q = 0; q < n; ++q) t[q] = v[q][qx];
+        mat1d_eo<n>(prm.eoNT, t, o);
+#pragma unroll
+        for (int a = 0; a < n; ++a) v[a][qx] = o[a];
+    }
+#pragma unroll
+    for (int ay = 0; ay < n; ++ay) {
+        mat1d_eo<n>(prm.eoNT, v[ay], o);
+#pragma unroll
+        for (int a = 0; a < n; ++a) v[ay][a] = o[a];
+    }
+    if (act) {
+        const double ashift = -prm.alpha * (prm.c + (prm.eps ? prm.eps[j] : 0.0));
+        const bool zterm = prm.Z != nullptr;
+#pragma unroll
+        for (int ay = 0; ay < n; ++ay) {
+            double s[n], xo[n], zo[n];
+            const bool own_row = (ay < P) && (pl < P);
+#pragma unroll
+            for (int ax = 0; ax < n; ++ax) {
+                const long long g = gpl + ax + prm.Nx * ay;
+                s[ax] = prm.sm[g];
+                const bool own = own_row && ax < P && s[ax] != 0.0;
+                xo[ax] = own ? prm.X[g * B + j] : 0.0;
+                zo[ax] = (own && zterm) ? prm.Z[g * B + j] : 0.0;
+            }
+#pragma unroll
+            for (int ax = 0; ax < n; ++ax) {
+                if (s[ax] != 0.0) {
+                    const long long g = gpl + ax + prm.Nx * ay;
+                    double val = (prm.alpha * s[ax]) * v[ay][ax];
+                    if (own_row && ax < P) val = fma(ashift, xo[ax], fma(prm.beta, zo[ax], val));
+                    atomicAdd(prm.Y + g * B + j, val);
+                }
+            }
+        }
+    }
+}
+
+template <int P, int BT, int MINB>
+cudaError_t launch_v2(const ApplyParams& prm, long long ncells, cudaStream_t st)
+{
+    constexpr int n = P + 1;
+    const size_t smem = ((size_t)2 * n * n * n * BT + n * n * n) * sizeof(double);
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(k_apply_v2<P, BT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    dim3 grid((unsigned)ncells, (unsigned)((prm.B + BT - 1) / BT)), block(BT, n);
+    k_apply_v2<P, BT, MINB><<<grid, block, smem, st>>>(prm);
+    return cudaGetLastError();
+}
+
 inline bool variant_supported(int p, int variant)
 {
     (void)p;
-    return variant == 0 || variant == 1;
+    return variant >= 0 && variant <= 2;
 }
 
 template <int P, int BT>
@@ -252,10 +462,21 @@ cudaError_t launch_v1(const ApplyParams& prm, long long ncells, cudaStream_t st)
 inline cudaError_t launch_apply(const ApplyParams& prm, int p, int variant, long long N, long long ncells,
                                 cudaStream_t st, int* nlaunch)
 {
-    (void)variant;
     cudaError_t e = cudaMemsetAsync(prm.Y, 0, (size_t)N * prm.B * sizeof(double), st);
     if (e != cudaSuccess) return e;
     *nlaunch = 1;  // kernels only; the zero-fill is a cudaMemsetAsync
+    if (variant != 1) {
+        switch (p) {
+            case 1: return launch_v2<1, 32, 8>(prm, ncells, st);
+            case 2: return launch_v2<2, 32, 6>(prm, ncells, st);
+            case 3: return launch_v2<3, 32, 4>(prm, ncells, st);
+            case 4: return launch_v2<4, 32, 3>(prm, ncells, st);
+            case 5: return launch_v2<5, 32, 1>(prm, ncells, st);
+            case 6: return launch_v2<6, 16, 2>(prm, ncells, st);
+            case 7: return launch_v2<7, 16, 1>(prm, ncells, st);
+            case 8: return launch_v2<8, 16, 1>(prm, ncells, st);
+        }
+    }
     switch (p) {
         case 1: return launch_v1<1, 32>(prm, ncells, st);
         case 2: return launch_v1<2, 32>(prm, ncells, st);
