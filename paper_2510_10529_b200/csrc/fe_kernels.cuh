@@ -436,10 +436,210 @@ cudaError_t launch_v2(const ApplyParams& prm, long long ncells, cudaStream_t st)
     return cudaGetLastError();
 }
 
+// ---- variant 3: v2 + scaling tile in shared memory + cp.async prefetch of the owner rows of X and Z ------------------
+__device__ __forceinline__ void cp_async8(void* smem_dst, const void* gsrc, bool valid)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    const int sz = valid ? 8 : 0;  // src-size 0 zero-fills the 8 destination bytes
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(d), "l"(gsrc), "r"(sz) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+template <int P, int BT, int MINB>
+__global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_v3(const __grid_constant__ ApplyParams prm)
+{
+    constexpr int n = P + 1, n3 = n * n * n;
+    extern __shared__ double smem[];
+    double* sA = smem;             // [n^3][BT]
+    double* sA2 = smem + n3 * BT;  // [n^3][BT]
+    double* sWV = sA2 + n3 * BT;   // [n^3]  J w V of this cell
+    double* sS = sWV + n3;         // [n^3]  mu * M^{-1/2} at the cell's nodes
+    const int lane = threadIdx.x, pl = threadIdx.y;
+    const int cell = blockIdx.x;
+    const int ex = cell % prm.cx, ey = (cell / prm.cx) % prm.cy, ez = cell / (prm.cx * prm.cy);
+    const int j = blockIdx.y * BT + lane;
+    const bool act = j < prm.B;
+    const long long B = prm.B;
+    const long long g0 = (long long)ex * P + prm.Nx * ((long long)ey * P) + prm.NxNy * ((long long)ez * P);
+    const long long gpl = g0 + prm.NxNy * pl;
+    const double* Xp = prm.X + gpl * B + j;
+    const double hx = prm.hx[ex], hy = prm.hy[ey], hz = prm.hz[ez];
+    const double J = hx * hy * hz * 0.125;
+    const double kx = 2.0 * J / (hx * hx), ky = 2.0 * J / (hy * hy), kz = 2.0 * J / (hz * hz);
+
+    double v[n][n], t[n], o[n];
+    // ---- plane phase 1 ---------------------------------------------------------------------------------------------
+#pragma unroll
+    for (int ay = 0; ay < n; ++ay)
+#pragma unroll
+        for (int ax = 0; ax < n; ++ax) v[ay][ax] = act ? Xp[(ax + prm.Nx * ay) * B] : 0.0;
+    {
+        const double* WVc = prm.WV + (long long)cell * n3;
+        for (int i = pl * BT + lane; i < n3; i += n * BT) {
+            sWV[i] = WVc[i];
+            const int ax = i % n, ay = (i / n) % n, az = i / (n * n);
+            sS[i] = prm.sm[g0 + ax + prm.Nx * ay + prm.NxNy * az];
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int ay = 0; ay < n; ++ay)
+#pragma unroll
+        for (int ax = 0; ax < n; ++ax) v[ay][ax] *= sS[(pl * n + ay) * n + ax];
+#pragma unroll
+    for (int ay = 0; ay < n; ++ay) {
+        mat1d_eo<n>(prm.eoN, v[ay], o);
+#pragma unroll
+        for (int q = 0; q < n; ++q) v[ay][q] = o[q];
+    }
+#pragma unroll
+    for (int qx = 0; qx < n; ++qx) {
+#pragma unroll
+        for (int a = 0; a < n; ++a) t[a] = v[a][qx];
+        mat1d_eo<n>(prm.eoN, t, o);
+#pragma unroll
+        for (int q = 0; q < n; ++q) v[q][qx] = o[q];
+    }
+    {
+        double v2[n][n];
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy) {
+            mat1d_eo<n>(prm.eoG, v[qy], o);
+            const double f = kx * prm.w[qy];
+#pragma unroll
+            for (int qx = 0; qx < n; ++qx) v2[qy][qx] = f * o[qx];
+        }
+#pragma unroll
+        for (int qx = 0; qx < n; ++qx) {
+#pragma unroll
+            for (int a = 0; a < n; ++a) t[a] = v[a][qx];
+            mat1d_eo<n>(prm.eoG, t, o);
+            const double f = ky * prm.w[qx];
+#pragma unroll
+            for (int qy = 0; qy < n; ++qy) v2[qy][qx] = fma(f, o[qy], v2[qy][qx]);
+        }
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy)
+#pragma unroll
+            for (int qx = 0; qx < n; ++qx) {
+                const int idx = ((pl * n + qy) * n + qx) * BT + lane;
+                sA[idx] = v[qy][qx];
+                sA2[idx] = v2[qy][qx];
+            }
+    }
+    __syncthreads();
+    // ---- line phase ------------------------------------------------------------------------------------------------
+    {
+        const int qx = pl;
+        const double kzwx = kz * prm.w[qx];
+#pragma unroll 1
+        for (int qy = 0; qy < n; ++qy) {
+            double a[n], a2[n], u[n], u2[n], gu[n];
+#pragma unroll
+            for (int az = 0; az < n; ++az) {
+                const int idx = ((az * n + qy) * n + qx) * BT + lane;
+                a[az] = sA[idx];
+                a2[az] = sA2[idx];
+            }
+            mat1d_eo<n>(prm.eoN, a, u);
+            mat1d_eo<n>(prm.eoN, a2, u2);
+            mat1d_eo<n>(prm.eoG, u, gu);
+            const double kzw = kzwx * prm.w[qy];
+#pragma unroll
+            for (int qz = 0; qz < n; ++qz) {
+                const double wv = sWV[(qz * n + qy) * n + qx];
+                t[qz] = fma(wv, u[qz], fma(prm.w[qz], u2[qz], kzw * gu[qz]));
+            }
+            mat1d_eo<n>(prm.eoNT, t, o);
+#pragma unroll
+            for (int az = 0; az < n; ++az) sA[((az * n + qy) * n + qx) * BT + lane] = o[az];
+        }
+    }
+    __syncthreads();
+    // ---- plane phase 2 ---------------------------------------------------------------------------------------------
+    // The A2 rows of this thread's plane are dead now: prefetch the owner rows of Z (and of X, for the diagonal
+    // term) into them with cp.async while the back-interpolation runs.  Row (ay,ax) of Z -> sA2 plane row (ay,ax);
+    // row (ay,ax) of X -> the unused last row/column slots and, for the rest, sA after R has been consumed.
+    const bool zterm = prm.Z != nullptr;
+    const bool own_pl = pl < P;
+    double* zbuf = sA2 + (size_t)pl * n * n * BT + lane;
+    double* xbuf = sA + (size_t)pl * n * n * BT + lane;
+    if (own_pl && zterm) {
+        const double* Zp = prm.Z + gpl * B + j;
+#pragma unroll
+        for (int ay = 0; ay < P; ++ay)
+#pragma unroll
+            for (int ax = 0; ax < P; ++ax) cp_async8(zbuf + (ay * n + ax) * BT, Zp + (ax + prm.Nx * ay) * B, act);
+    }
+    cp_async_commit();
+#pragma unroll
+    for (int qy = 0; qy < n; ++qy)
+#pragma unroll
+        for (int qx = 0; qx < n; ++qx) v[qy][qx] = sA[((pl * n + qy) * n + qx) * BT + lane];
+#pragma unroll
+    for (int qx = 0; qx < n; ++qx) {
+#pragma unroll
+        for (int q = 0; q < n; ++q) t[q] = v[q][qx];
+        mat1d_eo<n>(prm.eoNT, t, o);
+#pragma unroll
+        for (int a = 0; a < n; ++a) v[a][qx] = o[a];
+    }
+    // every R value of this plane has been consumed by the arithmetic above: its sA rows can take the X rows
+    if (own_pl) {
+#pragma unroll
+        for (int ay = 0; ay < P; ++ay)
+#pragma unroll
+            for (int ax = 0; ax < P; ++ax) cp_async8(xbuf + (ay * n + ax) * BT, Xp + (ax + prm.Nx * ay) * B, act);
+    }
+    cp_async_commit();
+#pragma unroll
+    for (int ay = 0; ay < n; ++ay) {
+        mat1d_eo<n>(prm.eoNT, v[ay], o);
+#pragma unroll
+        for (int a = 0; a < n; ++a) v[ay][a] = o[a];
+    }
+    cp_async_wait_all();
+    if (act) {
+        const double ashift = -prm.alpha * (prm.c + (prm.eps ? prm.eps[j] : 0.0));
+        double* Yp = prm.Y + gpl * B + j;
+#pragma unroll
+        for (int ay = 0; ay < n; ++ay)
+#pragma unroll
+            for (int ax = 0; ax < n; ++ax) {
+                const double sc = sS[(pl * n + ay) * n + ax];
+                double val = (prm.alpha * sc) * v[ay][ax];
+                if (ax < P && ay < P) {
+                    if (own_pl && __double2hiint(sc) != 0) {  // owner of a free node adds the diagonal terms once
+                        val = fma(ashift, xbuf[(ay * n + ax) * BT], val);
+                        if (zterm) val = fma(prm.beta, zbuf[(ay * n + ax) * BT], val);
+                    }
+                }
+                atomicAdd(Yp + (ax + prm.Nx * ay) * B, val);
+            }
+    }
+}
+
+template <int P, int BT, int MINB>
+cudaError_t launch_v3(const ApplyParams& prm, long long ncells, cudaStream_t st)
+{
+    constexpr int n = P + 1;
+    const size_t smem = ((size_t)2 * n * n * n * BT + 2 * n * n * n) * sizeof(double);
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(k_apply_v3<P, BT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    dim3 grid((unsigned)ncells, (unsigned)((prm.B + BT - 1) / BT)), block(BT, n);
+    k_apply_v3<P, BT, MINB><<<grid, block, smem, st>>>(prm);
+    return cudaGetLastError();
+}
+
 inline bool variant_supported(int p, int variant)
 {
     (void)p;
-    return variant >= 0 && variant <= 2;
+    return variant >= 0 && variant <= 3;
 }
 
 template <int P, int BT>
@@ -465,7 +665,19 @@ inline cudaError_t launch_apply(const ApplyParams& prm, int p, int variant, long
     cudaError_t e = cudaMemsetAsync(prm.Y, 0, (size_t)N * prm.B * sizeof(double), st);
     if (e != cudaSuccess) return e;
     *nlaunch = 1;  // kernels only; the zero-fill is a cudaMemsetAsync
-    if (variant != 1) {
+    if (variant == 0 || variant == 3) {
+        switch (p) {
+            case 1: return launch_v3<1, 32, 8>(prm, ncells, st);
+            case 2: return launch_v3<2, 32, 6>(prm, ncells, st);
+            case 3: return launch_v3<3, 32, 4>(prm, ncells, st);
+            case 4: return launch_v3<4, 32, 3>(prm, ncells, st);
+            case 5: return launch_v3<5, 32, 1>(prm, ncells, st);
+            case 6: return launch_v3<6, 16, 2>(prm, ncells, st);
+            case 7: return launch_v3<7, 16, 1>(prm, ncells, st);
+            case 8: return launch_v3<8, 16, 1>(prm, ncells, st);
+        }
+    }
+    if (variant == 2) {
         switch (p) {
             case 1: return launch_v2<1, 32, 8>(prm, ncells, st);
             case 2: return launch_v2<2, 32, 6>(prm, ncells, st);
