@@ -28,6 +28,11 @@ UNIT = "GDoF-vectors/s"
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE k_apply launch from the committed `ncu --set full` captures
+# (profiles/r1_c2_k_apply_full.md, profiles/r1_c3_k_apply_full.md); the zero-fill memset adds N*B*8 bytes on top.
+NCU_TRAFFIC_BYTES = {2: 428.05e6 + 111.56e6, 3: 4.9201e9 + 1.5490e9}
+
+
 def algorithmic_flops_per_cell_vector(p):
     """matrix-free sum factorisation, 24 n^4 + 9 n^3 flops per cell-vector."""
     n = p + 1
@@ -273,10 +278,9 @@ def main():
     w = workloads.config(args.workload)
     r = time_workload(fe, torch, w, args.steps, args.warmup, local, seed_offset=rank, with_e2e=True, dist=dist,
                       sample_clocks=(rank == 0), variant=args.variant)
-    ms = torch.tensor([r["ms_per_step"], r["e2e_s_per_step"] * 1e3], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(ms, op=dist.ReduceOp.MAX)  # max over ranks; columns are sharded with no exchange (weak)
-    ms_step, e2e_ms = float(ms[0]), float(ms[1])
+    from paper_2510_10529_b200.colsplit import max_over_ranks
+    # max over ranks; columns are sharded with no exchange (weak scaling)
+    ms_step, e2e_ms = max_over_ranks([r["ms_per_step"], r["e2e_s_per_step"] * 1e3], dist, device="cuda")
     value, roof = summarize(w, r, ms_step, world)
     hbm_peak = None
     try:
@@ -285,6 +289,8 @@ def main():
     except Exception:
         pass
     alg_bytes = (24 if w.m > 0 else 16) * r["N"] * r["B"]
+    roof["traffic"] = NCU_TRAFFIC_BYTES.get(args.workload)
+    roof["algorithmic_bytes"] = alg_bytes
     roof["hbm_frac_of_measured"] = (alg_bytes / (roof["launch_ms"] * 1e-3) / 1e9 / hbm_peak) if hbm_peak else None
     if rank != 0:
         if dist is not None:

@@ -301,6 +301,7 @@ static int operator_step(fe_mesh* m, const double* X, const double* Z, double* Y
     fill_params(m, &prm);
     prm.X = X; prm.Z = Z; prm.Y = Y; prm.eps = eps; prm.B = B;
     prm.alpha = alpha; prm.beta = beta; prm.c = c;
+    for (int q = 0; q < m->n; ++q) prm.aw[q] = alpha * prm.w[q];
     int nl = 0;
     cudaError_t e = launch_apply(prm, m->p, m->variant, m->N, m->ncells, st, &nl);
     if (e != cudaSuccess) return fail(FE_ERR_CUDA, "operator launch failed: %s", cudaGetErrorString(e));

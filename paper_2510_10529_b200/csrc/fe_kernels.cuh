@@ -40,6 +40,7 @@ struct ApplyParams {
     long long Nx, NxNy;
     double alpha, beta, c;
     double N[81], G[81], w[9];
+    double aw[9];  // alpha * w (variant 4)
     EOTab eoN, eoNT, eoG;  // even-odd split of N, N^T and G (all centro-symmetric: GLL and Gauss points are symmetric)
 };
 
@@ -636,10 +637,218 @@ cudaError_t launch_v3(const ApplyParams& prm, long long ncells, cudaStream_t st)
     return cudaGetLastError();
 }
 
+// ---- variant 4: v3 + 32-bit offsets from a CTA-uniform base, alpha folded into the staged potential and weights,
+//                 line phase run as plane passes (one 1-D table per pass, so table entries stay in uniform registers)
+template <int P, int BT, int MINB>
+__global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_v4(const __grid_constant__ ApplyParams prm)
+{
+    constexpr int n = P + 1, n3 = n * n * n;
+    extern __shared__ double smem[];
+    double* sA = smem;             // [n^3][BT]
+    double* sA2 = smem + n3 * BT;  // [n^3][BT]
+    double* sWV = sA2 + n3 * BT;   // [n^3]  alpha J w V of this cell
+    double* sS = sWV + n3;         // [n^3]  mu * M^{-1/2} at the cell's nodes
+    const int lane = threadIdx.x, pl = threadIdx.y;
+    const int cell = blockIdx.x;
+    const int ex = cell % prm.cx, ey = (cell / prm.cx) % prm.cy, ez = cell / (prm.cx * prm.cy);
+    const int j = blockIdx.y * BT + lane;
+    const bool act = j < prm.B;
+    // CTA-uniform 64-bit bases; everything a thread touches lies within 2^32 bytes of them (checked at launch)
+    const long long g0 = (long long)ex * P + prm.Nx * ((long long)ey * P) + prm.NxNy * ((long long)ez * P);
+    const double* __restrict__ Xc = prm.X + g0 * prm.B;
+    const double* __restrict__ Zc = prm.Z + g0 * prm.B;
+    double* __restrict__ Yc = prm.Y + g0 * prm.B;
+    const unsigned uB = (unsigned)prm.B, rs = (unsigned)prm.Nx * uB;
+    const unsigned tb = (unsigned)pl * (unsigned)prm.NxNy * uB + (unsigned)j;
+    unsigned ro[n], co[n];
+#pragma unroll
+    for (int i = 0; i < n; ++i) {
+        ro[i] = tb + i * rs;
+        co[i] = i * uB;
+    }
+    const double hx = prm.hx[ex], hy = prm.hy[ey], hz = prm.hz[ez];
+    const double J = hx * hy * hz * 0.125;
+    const double kx = 2.0 * J / (hx * hx), ky = 2.0 * J / (hy * hy), kz = prm.alpha * 2.0 * J / (hz * hz);
+
+    double v[n][n], t[n], o[n];
+    // ---- plane phase 1 ---------------------------------------------------------------------------------------------
+#pragma unroll
+    for (int ay = 0; ay < n; ++ay)
+#pragma unroll
+        for (int ax = 0; ax < n; ++ax) v[ay][ax] = act ? Xc[ro[ay] + co[ax]] : 0.0;
+    {
+        const double* WVc = prm.WV + (long long)cell * n3;
+        for (int i = pl * BT + lane; i < n3; i += n * BT) {
+            sWV[i] = prm.alpha * WVc[i];
+            const int ax = i % n, ay = (i / n) % n, az = i / (n * n);
+            sS[i] = prm.sm[g0 + ax + prm.Nx * ay + prm.NxNy * az];
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int ay = 0; ay < n; ++ay)
+#pragma unroll
+        for (int ax = 0; ax < n; ++ax) v[ay][ax] *= sS[(pl * n + ay) * n + ax];
+#pragma unroll
+    for (int ay = 0; ay < n; ++ay) {
+        mat1d_eo<n>(prm.eoN, v[ay], o);
+#pragma unroll
+        for (int q = 0; q < n; ++q) v[ay][q] = o[q];
+    }
+#pragma unroll
+    for (int qx = 0; qx < n; ++qx) {
+#pragma unroll
+        for (int a = 0; a < n; ++a) t[a] = v[a][qx];
+        mat1d_eo<n>(prm.eoN, t, o);
+#pragma unroll
+        for (int q = 0; q < n; ++q) v[q][qx] = o[q];
+    }
+    {
+        double v2[n][n];
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy) {
+            mat1d_eo<n>(prm.eoG, v[qy], o);
+            const double f = kx * prm.w[qy];
+#pragma unroll
+            for (int qx = 0; qx < n; ++qx) v2[qy][qx] = f * o[qx];
+        }
+#pragma unroll
+        for (int qx = 0; qx < n; ++qx) {
+#pragma unroll
+            for (int a = 0; a < n; ++a) t[a] = v[a][qx];
+            mat1d_eo<n>(prm.eoG, t, o);
+            const double f = ky * prm.w[qx];
+#pragma unroll
+            for (int qy = 0; qy < n; ++qy) v2[qy][qx] = fma(f, o[qy], v2[qy][qx]);
+        }
+        double* pa = sA + (size_t)pl * n * n * BT + lane;
+        double* pa2 = sA2 + (size_t)pl * n * n * BT + lane;
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy)
+#pragma unroll
+            for (int qx = 0; qx < n; ++qx) {
+                pa[(qy * n + qx) * BT] = v[qy][qx];
+                pa2[(qy * n + qx) * BT] = v2[qy][qx];
+            }
+    }
+    __syncthreads();
+    // ---- line phase as plane passes: the thread owns the yz-plane qx = pl --------------------------------------------
+    {
+        double* la = sA + (size_t)pl * BT + lane;    // + ((az*n + qy)*n)*BT
+        double* la2 = sA2 + (size_t)pl * BT + lane;
+        const double* lw = sWV + pl;                 // + (qz*n + qy)*n
+        // pass 1: U = Nz A
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy) {
+#pragma unroll
+            for (int az = 0; az < n; ++az) t[az] = la[((az * n + qy) * n) * BT];
+            mat1d_eo<n>(prm.eoN, t, v[qy]);
+        }
+        // pass 2: T = (alpha WV) . U + (alpha kz wx wy) (Gz U), in place
+        const double kzwx = kz * prm.w[pl];
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy) {
+            mat1d_eo<n>(prm.eoG, v[qy], o);
+            const double kzw = kzwx * prm.w[qy];
+#pragma unroll
+            for (int qz = 0; qz < n; ++qz) v[qy][qz] = fma(lw[(qz * n + qy) * n], v[qy][qz], kzw * o[qz]);
+        }
+        // pass 3: T += (alpha wz) . (Nz A2)
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy) {
+#pragma unroll
+            for (int az = 0; az < n; ++az) t[az] = la2[((az * n + qy) * n) * BT];
+            mat1d_eo<n>(prm.eoN, t, o);
+#pragma unroll
+            for (int qz = 0; qz < n; ++qz) v[qy][qz] = fma(prm.aw[qz], o[qz], v[qy][qz]);
+        }
+        // pass 4: R = Nz^T T, back into the A field
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy) {
+            mat1d_eo<n>(prm.eoNT, v[qy], o);
+#pragma unroll
+            for (int az = 0; az < n; ++az) la[((az * n + qy) * n) * BT] = o[az];
+        }
+    }
+    __syncthreads();
+    // ---- plane phase 2 ---------------------------------------------------------------------------------------------
+    const bool zterm = prm.Z != nullptr;
+    const bool own_pl = pl < P;
+    double* zbuf = sA2 + (size_t)pl * n * n * BT + lane;
+    double* xbuf = sA + (size_t)pl * n * n * BT + lane;
+    if (own_pl && zterm) {
+#pragma unroll
+        for (int ay = 0; ay < P; ++ay)
+#pragma unroll
+            for (int ax = 0; ax < P; ++ax) cp_async8(zbuf + (ay * n + ax) * BT, Zc + (ro[ay] + co[ax]), act);
+    }
+    cp_async_commit();
+#pragma unroll
+    for (int qy = 0; qy < n; ++qy)
+#pragma unroll
+        for (int qx = 0; qx < n; ++qx) v[qy][qx] = xbuf[(qy * n + qx) * BT];
+#pragma unroll
+    for (int qx = 0; qx < n; ++qx) {
+#pragma unroll
+        for (int q = 0; q < n; ++q) t[q] = v[q][qx];
+        mat1d_eo<n>(prm.eoNT, t, o);
+#pragma unroll
+        for (int a = 0; a < n; ++a) v[a][qx] = o[a];
+    }
+    if (own_pl) {
+#pragma unroll
+        for (int ay = 0; ay < P; ++ay)
+#pragma unroll
+            for (int ax = 0; ax < P; ++ax) cp_async8(xbuf + (ay * n + ax) * BT, Xc + (ro[ay] + co[ax]), act);
+    }
+    cp_async_commit();
+#pragma unroll
+    for (int ay = 0; ay < n; ++ay) {
+        mat1d_eo<n>(prm.eoNT, v[ay], o);
+#pragma unroll
+        for (int a = 0; a < n; ++a) v[ay][a] = o[a];
+    }
+    cp_async_wait_all();
+    if (act) {
+        const double ashift = -prm.alpha * (prm.c + (prm.eps ? prm.eps[j] : 0.0));
+        const double* ss = sS + pl * n * n;
+#pragma unroll
+        for (int ay = 0; ay < n; ++ay)
+#pragma unroll
+            for (int ax = 0; ax < n; ++ax) {
+                const double sc = ss[ay * n + ax];
+                double val = sc * v[ay][ax];
+                if (ax < P && ay < P) {
+                    if (own_pl && __double2hiint(sc) != 0) {  // owner of a free node adds the diagonal terms once
+                        val = fma(ashift, xbuf[(ay * n + ax) * BT], val);
+                        if (zterm) val = fma(prm.beta, zbuf[(ay * n + ax) * BT], val);
+                    }
+                }
+                atomicAdd(Yc + (ro[ay] + co[ax]), val);
+            }
+    }
+}
+
+template <int P, int BT, int MINB>
+cudaError_t launch_v4(const ApplyParams& prm, long long ncells, cudaStream_t st)
+{
+    constexpr int n = P + 1;
+    const size_t smem = ((size_t)2 * n * n * n * BT + 2 * n * n * n) * sizeof(double);
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(k_apply_v4<P, BT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    dim3 grid((unsigned)ncells, (unsigned)((prm.B + BT - 1) / BT)), block(BT, n);
+    k_apply_v4<P, BT, MINB><<<grid, block, smem, st>>>(prm);
+    return cudaGetLastError();
+}
+
 inline bool variant_supported(int p, int variant)
 {
     (void)p;
-    return variant >= 0 && variant <= 3;
+    return variant >= 0 && variant <= 4;
 }
 
 template <int P, int BT>
@@ -665,7 +874,21 @@ inline cudaError_t launch_apply(const ApplyParams& prm, int p, int variant, long
     cudaError_t e = cudaMemsetAsync(prm.Y, 0, (size_t)N * prm.B * sizeof(double), st);
     if (e != cudaSuccess) return e;
     *nlaunch = 1;  // kernels only; the zero-fill is a cudaMemsetAsync
-    if (variant == 0 || variant == 3) {
+    // variant 4 addresses with 32-bit byte offsets from a per-cell base: one cell's node box times B must fit
+    const bool fits32 = (double)(p + 1) * (double)prm.NxNy * (double)prm.B * 8.0 < 4.0e9;
+    if (variant == 4 && fits32) {
+        switch (p) {
+            case 1: return launch_v4<1, 32, 8>(prm, ncells, st);
+            case 2: return launch_v4<2, 32, 6>(prm, ncells, st);
+            case 3: return launch_v4<3, 32, 4>(prm, ncells, st);
+            case 4: return launch_v4<4, 32, 3>(prm, ncells, st);
+            case 5: return launch_v4<5, 32, 1>(prm, ncells, st);
+            case 6: return launch_v4<6, 16, 2>(prm, ncells, st);
+            case 7: return launch_v4<7, 16, 1>(prm, ncells, st);
+            case 8: return launch_v4<8, 16, 1>(prm, ncells, st);
+        }
+    }
+    if (variant == 0 || variant == 3 || variant == 4) {
         switch (p) {
             case 1: return launch_v3<1, 32, 8>(prm, ncells, st);
             case 2: return launch_v3<2, 32, 6>(prm, ncells, st);
