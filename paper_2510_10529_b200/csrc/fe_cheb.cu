@@ -4,15 +4,18 @@
 // fused gather -> sum-factorised cell contraction -> scatter kernels of fe_kernels.cuh on the caller's stream.
 #include "../../include/fe_cheb.h"
 
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include <cmath>
+#include <cstdint>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
 #include <new>
 #include <vector>
 
+#include "fe_apply_tma.cuh"
 #include "fe_kernels.cuh"
 #include "fe_tables.h"
 
@@ -46,12 +49,47 @@ struct fe_mesh {
     double* d_sm = nullptr;          // N: mu_g M_gg^{-1/2} (0 on the Dirichlet boundary)
     double *d_hx = nullptr, *d_hy = nullptr, *d_hz = nullptr;
     double* d_WV = nullptr;  // cells*n^3: J w_q V_q
+    double* d_VZ = nullptr;  // cells*n*n*NP: V_q hz^2/2, [qx][qy][qz] rows padded to NP (TMA kernel)
+    double *d_sx = nullptr, *d_sy = nullptr, *d_sz = nullptr;  // per-axis mu M^{-1/2}
+    EOTab eoN, eoNT, eoG;    // even-odd halves of N' = diag(sqrt w) N, N'^T, G' = diag(w^-1/2) G diag(w^-1/2)
     bool have_V = false;
     int variant = 0;
     int64_t launches = 0;
 };
 
 const char* fe_last_error(void) { return g_err; }
+
+// even-odd split of a centro-symmetric n x n matrix (row-major M[i*n+k]); transpose selects M^T
+static void make_eo(const double* M, int n, bool transpose, EOTab* T)
+{
+    const int h = n / 2, c = (n + 1) / 2;
+    memset(T, 0, sizeof(*T));
+    auto at = [&](int i, int k) { return transpose ? M[k * n + i] : M[i * n + k]; };
+    for (int i = 0; i < c; ++i) {
+        for (int k = 0; k < h; ++k) {
+            T->S[i * h + k] = 0.5 * (at(i, k) + at(i, n - 1 - k));
+            if (i < h) T->A[i * h + k] = 0.5 * (at(i, k) - at(i, n - 1 - k));
+        }
+        if (n % 2 == 1) T->Mid[i] = at(i, h);
+    }
+}
+
+static int small_tile(int n) { return n * n * (n + (n & 1)); }
+
+// Gauss weights folded into the 1-D tables (fe_apply_tma.cuh): N' = diag(sqrt w) N, G' = diag(w^-1/2) G diag(w^-1/2)
+static void build_folded_tables(fe_mesh* m)
+{
+    const int n = m->n;
+    double Np[kMaxN * kMaxN], Gp[kMaxN * kMaxN];
+    for (int q = 0; q < n; ++q)
+        for (int a = 0; a < n; ++a) {
+            Np[q * n + a] = std::sqrt(m->tab.gl_w[q]) * m->tab.N[q * n + a];
+            Gp[q * n + a] = m->tab.G[q * n + a] / std::sqrt(m->tab.gl_w[q] * m->tab.gl_w[a]);
+        }
+    make_eo(Np, n, false, &m->eoN);
+    make_eo(Np, n, true, &m->eoNT);
+    make_eo(Gp, n, false, &m->eoG);
+}
 
 static void axis_mass(const std::vector<double>& e, int c, int p, const Tables1D& t, std::vector<double>& m)
 {
@@ -114,22 +152,24 @@ int fe_mesh_create(const double* xe, int cx, const double* ye, int cy, const dou
         h[d].resize(cc[d]);
         for (int i = 0; i < cc[d]; ++i) h[d][i] = (*ee[d])[i + 1] - (*ee[d])[i];
     }
-    double *d_sx = nullptr, *d_sy = nullptr, *d_sz = nullptr;
     int rc = FE_OK;
     auto cleanup = [&](int code) {
-        cudaFree(d_sx); cudaFree(d_sy); cudaFree(d_sz);
         if (code != FE_OK) fe_mesh_destroy(m);
         return code;
     };
-    if ((rc = upload(&d_sx, s[0])) || (rc = upload(&d_sy, s[1])) || (rc = upload(&d_sz, s[2]))) return cleanup(rc);
+    if ((rc = upload(&m->d_sx, s[0])) || (rc = upload(&m->d_sy, s[1])) || (rc = upload(&m->d_sz, s[2]))) return cleanup(rc);
     if ((rc = upload(&m->d_hx, h[0])) || (rc = upload(&m->d_hy, h[1])) || (rc = upload(&m->d_hz, h[2]))) return cleanup(rc);
     cudaError_t ce = cudaMalloc((void**)&m->d_sm, (size_t)m->N * sizeof(double));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&m->d_WV, (size_t)m->ncells * m->nc * sizeof(double));
+    if (ce == cudaSuccess) ce = cudaMalloc((void**)&m->d_VZ, (size_t)m->ncells * small_tile(m->n) * sizeof(double));
     if (ce != cudaSuccess) return cleanup(fail(FE_ERR_NOMEM, "fe_mesh_create: device allocation failed: %s", cudaGetErrorString(ce)));
-    launch_build_scaling(d_sx, d_sy, d_sz, m->Nx, m->Ny, m->Nz, m->d_sm, 0);
+    ce = cudaMemset(m->d_VZ, 0, (size_t)m->ncells * small_tile(m->n) * sizeof(double));
+    if (ce != cudaSuccess) return cleanup(fail(FE_ERR_CUDA, "fe_mesh_create: memset failed: %s", cudaGetErrorString(ce)));
+    launch_build_scaling(m->d_sx, m->d_sy, m->d_sz, m->Nx, m->Ny, m->Nz, m->d_sm, 0);
     m->launches += 1;
     ce = cudaDeviceSynchronize();
     if (ce != cudaSuccess) return cleanup(fail(FE_ERR_CUDA, "fe_mesh_create: scaling kernel failed: %s", cudaGetErrorString(ce)));
+    build_folded_tables(m);
     *out = m;
     return cleanup(FE_OK);
 }
@@ -139,6 +179,7 @@ int fe_mesh_destroy(fe_mesh* m)
     if (!m) return FE_OK;
     cudaSetDevice(m->device);
     cudaFree(m->d_sm); cudaFree(m->d_hx); cudaFree(m->d_hy); cudaFree(m->d_hz); cudaFree(m->d_WV);
+    cudaFree(m->d_VZ); cudaFree(m->d_sx); cudaFree(m->d_sy); cudaFree(m->d_sz);
     delete m;
     return FE_OK;
 }
@@ -237,21 +278,6 @@ int fe_get_dirichlet_mask(const fe_mesh* m, uint8_t* mask)
     return FE_OK;
 }
 
-// even-odd split of a centro-symmetric n x n matrix (row-major M[i*n+k]); transpose selects M^T
-static void make_eo(const double* M, int n, bool transpose, EOTab* T)
-{
-    const int h = n / 2, c = (n + 1) / 2;
-    memset(T, 0, sizeof(*T));
-    auto at = [&](int i, int k) { return transpose ? M[k * n + i] : M[i * n + k]; };
-    for (int i = 0; i < c; ++i) {
-        for (int k = 0; k < h; ++k) {
-            T->S[i * h + k] = 0.5 * (at(i, k) + at(i, n - 1 - k));
-            if (i < h) T->A[i * h + k] = 0.5 * (at(i, k) - at(i, n - 1 - k));
-        }
-        if (n % 2 == 1) T->Mid[i] = at(i, h);
-    }
-}
-
 static void fill_params(const fe_mesh* m, ApplyParams* prm)
 {
     memset(prm, 0, sizeof(*prm));
@@ -278,7 +304,7 @@ int fe_set_potential(fe_mesh* m, const double* Vq_dev, int copy, void* cuda_stre
     CUDA_TRY(cudaSetDevice(m->device));
     ApplyParams prm;
     fill_params(m, &prm);
-    launch_weight_potential(prm, m->p, Vq_dev, m->d_WV, m->ncells, (cudaStream_t)cuda_stream);
+    launch_weight_potential(prm, m->p, Vq_dev, m->d_WV, m->d_VZ, m->ncells, (cudaStream_t)cuda_stream);
     CUDA_TRY(cudaGetLastError());
     m->launches += 1;
     m->have_V = true;
@@ -309,6 +335,95 @@ static int operator_step(fe_mesh* m, const double* X, const double* Z, double* Y
     return FE_OK;
 }
 
+// ---- TMA path (fe_apply_tma.cuh) -----------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn encode_fn()
+{
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        cudaDriverEntryPointQueryResult qr;
+        void* p = nullptr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr) == cudaSuccess &&
+            qr == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+// the block as a 4-D tensor (j, gx, gy, gz) of doubles with a box of (bt, bx, by, bz) elements
+static int make_map(CUtensorMap* out, const fe_mesh* m, const double* base, int B, int bt, int bx, int by, int bz)
+{
+    EncodeTiledFn enc = encode_fn();
+    if (!enc) return fail(FE_ERR_CUDA, "cuTensorMapEncodeTiled not available from this driver");
+    cuuint64_t dims[4] = {(cuuint64_t)B, (cuuint64_t)m->Nx, (cuuint64_t)m->Ny, (cuuint64_t)m->Nz};
+    cuuint64_t strides[3] = {(cuuint64_t)B * 8, (cuuint64_t)B * 8 * m->Nx, (cuuint64_t)B * 8 * m->Nx * m->Ny};
+    cuuint32_t box[4] = {(cuuint32_t)bt, (cuuint32_t)bx, (cuuint32_t)by, (cuuint32_t)bz}, es[4] = {1, 1, 1, 1};
+    CUresult r = enc(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, (void*)base, dims, strides, box, es,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(FE_ERR_CUDA, "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r);
+    return FE_OK;
+}
+
+// the three views of one block the TMA kernel uses
+struct BlockMaps {
+    CUtensorMap n3, n1, p1;
+};
+
+static int make_block_maps(BlockMaps* bm, const fe_mesh* m, const double* base, int B)
+{
+    const int bt = tma_bt(m->p), n = m->n, p = m->p;
+    int rc;
+    if ((rc = make_map(&bm->n3, m, base, B, bt, n, n, n))) return rc;
+    if ((rc = make_map(&bm->n1, m, base, B, bt, n, n, 1))) return rc;
+    return make_map(&bm->p1, m, base, B, bt, p, p, 1);
+}
+
+// bulk tensor copies need 16-byte aligned bases and row pitches (B even)
+static bool tma_eligible(const fe_mesh* m, int B, const void* a, const void* b, const void* c)
+{
+    if (m->variant != 0 && m->variant != 5) return false;
+    if (B % 2 != 0 || !encode_fn()) return false;
+    return (((uintptr_t)a | (uintptr_t)b | (uintptr_t)c) & 15) == 0;
+}
+
+static void fill_tma_params(const fe_mesh* m, TmaParams* prm, int B)
+{
+    memset(prm, 0, sizeof(*prm));
+    prm->VZ = m->d_VZ; prm->sx = m->d_sx; prm->sy = m->d_sy; prm->sz = m->d_sz;
+    prm->hx = m->d_hx; prm->hy = m->d_hy; prm->hz = m->d_hz;
+    prm->B = B; prm->cx = m->cx; prm->cy = m->cy; prm->cz = m->cz;
+    prm->eoN = m->eoN; prm->eoNT = m->eoNT; prm->eoG = m->eoG;
+}
+
+// Y += alpha s sum_e yhat_e(X) + kappa X (owner),  W = beta_next X (pre-initialisation of the next target), one launch
+static int tma_step(fe_mesh* m, const BlockMaps& X, const BlockMaps& Y, const BlockMaps* W, int B, const double* eps,
+                    double alpha, double c, bool owner, double beta_next, bool first, cudaStream_t st)
+{
+    TmaParams prm;
+    fill_tma_params(m, &prm, B);
+    prm.mXn = X.n3; prm.mYn1 = Y.n1; prm.mYp1 = Y.p1; prm.mWp1 = W ? W->p1 : Y.p1;
+    prm.eps = eps; prm.alpha = alpha; prm.c = c; prm.owner = owner ? 1 : 0;
+    prm.preinit = W ? 1 : 0; prm.beta_next = beta_next;
+    cudaError_t e = launch_apply_tma(prm, m->p, m->ncells, first, st);
+    if (e != cudaSuccess) return fail(FE_ERR_CUDA, "operator launch failed: %s", cudaGetErrorString(e));
+    m->launches += 1;
+    return FE_OK;
+}
+
+static int zero_faces(fe_mesh* m, double* Y, int B, cudaStream_t st)
+{
+    k_zero_faces<<<148 * 4, 256, 0, st>>>(Y, m->Nx, m->Ny, m->Nz, B);
+    CUDA_TRY(cudaGetLastError());
+    m->launches += 1;
+    return FE_OK;
+}
+
 static bool overlap(const double* a, size_t na, const double* b, size_t nb)
 {
     return a < b + nb && b < a + na;
@@ -322,7 +437,15 @@ int fe_apply_H(fe_mesh* m, const double* X, double* Y, int B, const double* eps_
     const size_t len = (size_t)m->N * B;
     if (overlap(X, len, Y, len)) return fail(FE_ERR_INVALID, "fe_apply_H: X and Y overlap");
     CUDA_TRY(cudaSetDevice(m->device));
-    return operator_step(m, X, nullptr, Y, B, eps_dev, 1.0, 0.0, 0.0, (cudaStream_t)cuda_stream);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (tma_eligible(m, B, X, Y, eps_dev)) {
+        BlockMaps mx, my;
+        int rc;
+        if ((rc = make_block_maps(&mx, m, X, B)) || (rc = make_block_maps(&my, m, Y, B))) return rc;
+        CUDA_TRY(cudaMemsetAsync(Y, 0, len * sizeof(double), st));
+        return tma_step(m, mx, my, nullptr, B, eps_dev, 1.0, 0.0, eps_dev != nullptr, 0.0, true, st);
+    }
+    return operator_step(m, X, nullptr, Y, B, eps_dev, 1.0, 0.0, 0.0, st);
 }
 
 int cheb_filter(fe_mesh* m, double* X, int B, int deg, double a, double b, double a0, double* work, void* cuda_stream)
@@ -341,6 +464,28 @@ int cheb_filter(fe_mesh* m, double* X, int B, int deg, double a, double b, doubl
     const double e = 0.5 * (b - a), c = 0.5 * (b + a);
     const double sigma1 = e / (a0 - c);
     double sigma = sigma1;
+    if (tma_eligible(m, B, X, work, work + len)) {
+        // Pre-initialised recurrence: step k adds alpha_k (H~ - c) Y_k into buf[(k+1)%3], which step k-1 filled with
+        // beta_k Y_{k-1}; it stores beta_{k+1} Y_k into buf[(k+2)%3].  No zero-fill or read of Y_{k-1} per step.
+        BlockMaps bm[3];
+        int rc;
+        for (int i = 0; i < 3; ++i)
+            if ((rc = make_block_maps(&bm[i], m, buf[i], B))) return rc;
+        CUDA_TRY(cudaMemsetAsync(buf[1], 0, len * sizeof(double), st));
+        if ((rc = zero_faces(m, buf[0], B, st)) || (rc = zero_faces(m, buf[2], B, st))) return rc;
+        double s_cur = sigma1;  // sigma_{k+1} at iteration k
+        for (int k = 0; k < deg; ++k) {
+            const double s_next = 1.0 / (2.0 / sigma1 - s_cur);  // sigma_{k+2}
+            const double alpha = (k == 0) ? s_cur / e : 2.0 * s_cur / e;
+            const bool pre = k + 1 < deg;  // beta_{k+1} = -sigma_{k+1} sigma_{k+2}
+            rc = tma_step(m, bm[k % 3], bm[(k + 1) % 3], pre ? &bm[(k + 2) % 3] : nullptr, B, nullptr, alpha, c, true,
+                          -s_cur * s_next, k == 0, st);
+            if (rc) return rc;
+            s_cur = s_next;
+        }
+        if (deg % 3 != 0) CUDA_TRY(cudaMemcpyAsync(X, buf[deg % 3], len * sizeof(double), cudaMemcpyDeviceToDevice, st));
+        return FE_OK;
+    }
     int rc = operator_step(m, buf[0], nullptr, buf[1], B, nullptr, sigma1 / e, 0.0, c, st);
     if (rc) return rc;
     for (int k = 1; k < deg; ++k) {

@@ -61,10 +61,11 @@ inline void launch_build_scaling(const double* sx, const double* sy, const doubl
     k_build_scaling<<<148 * 8, 256, 0, st>>>(sx, sy, sz, Nx, Ny, Nz, sm);
 }
 
-// WV[e][q] = J_e w_qx w_qy w_qz V[e][q]
+// WV[e][q] = J_e w_qx w_qy w_qz V[e][q];  VZ[e][(qx*n+qy)*NP+qz] = V[e][q] hz^2/2 (TMA kernel; NP = n rounded up to even)
 __global__ void k_weight_potential(const __grid_constant__ ApplyParams prm, int n, const double* __restrict__ V,
-                                   double* __restrict__ WV, long long ncells)
+                                   double* __restrict__ WV, double* __restrict__ VZ, long long ncells)
 {
+    const int NP = n + (n & 1);
     const int n3 = n * n * n;
     long long total = ncells * n3;
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
@@ -74,13 +75,14 @@ __global__ void k_weight_potential(const __grid_constant__ ApplyParams prm, int 
         int ex = (int)(e % prm.cx), ey = (int)((e / prm.cx) % prm.cy), ez = (int)(e / ((long long)prm.cx * prm.cy));
         double J = prm.hx[ex] * prm.hy[ey] * prm.hz[ez] * 0.125;
         WV[i] = J * prm.w[qx] * prm.w[qy] * prm.w[qz] * V[i];
+        VZ[e * (n * n * NP) + (qx * n + qy) * NP + qz] = 0.5 * prm.hz[ez] * prm.hz[ez] * V[i];
     }
 }
 
-inline void launch_weight_potential(const ApplyParams& prm, int p, const double* V, double* WV, long long ncells,
-                                    cudaStream_t st)
+inline void launch_weight_potential(const ApplyParams& prm, int p, const double* V, double* WV, double* VZ,
+                                    long long ncells, cudaStream_t st)
 {
-    k_weight_potential<<<148 * 8, 256, 0, st>>>(prm, p + 1, V, WV, ncells);
+    k_weight_potential<<<148 * 8, 256, 0, st>>>(prm, p + 1, V, WV, VZ, ncells);
 }
 
 // ---- variant 1: plain sum factorisation, atomics scatter --------------------------------------------------------
