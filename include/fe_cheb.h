@@ -75,7 +75,8 @@ int fe_apply_H(fe_mesh* m, const double* X, double* Y, int B, const double* eps_
 int cheb_filter(fe_mesh* m, double* X, int B, int deg, double a, double b, double a0, double* work,
                 void* cuda_stream);
 
-/* Kernel variant for experiments and tests: 0 = default for this p.  Returns FE_ERR_INVALID if unknown. */
+/* Kernel variant for experiments and tests: 0 = default (TMA generation when B is even and the blocks are 16-byte
+ * aligned, else the legacy atomics kernel), 5 = same, 1..4 = legacy generations.  FE_ERR_INVALID if unknown. */
 int fe_set_variant(fe_mesh* m, int variant);
 /* Kernels launched by this handle since creation (bench.py's gpu_launches). */
 int64_t fe_launch_count(const fe_mesh* m);

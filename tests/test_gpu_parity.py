@@ -77,6 +77,44 @@ def test_apply_all_orders(p):
     assert np.all(Yg[om.mask() == 0] == 0)
 
 
+@pytest.mark.parametrize("variant", [3, 5])
+@pytest.mark.parametrize("p", [1, 2, 3, 4, 5, 6, 7, 8])
+def test_apply_all_orders_both_kernel_generations(p, variant):
+    """Even B takes the TMA kernel (variant 5 = default), variant 3 forces the legacy atomics kernel; B = 6 is a
+    ragged tail of the 16/32-wide vector box (out-of-bounds columns of the tensor tile)."""
+    e = (np.array([0.0, 0.9, 2.0]), np.array([-1.0, 0.1, 1.0]), np.array([0.0, 0.6, 1.0]))
+    om, gm = _pair(e, p, _coulomb)
+    gm.set_variant(variant)
+    B = 6
+    X = workloads.random_block(200 + p, om.N, B)  # boundary rows NOT zeroed: must be ignored
+    eps = workloads.shifts(2100 + p, B)
+    Yo = om.apply(X, eps)
+    Yg = gm.apply_H(_dev(X), eps=_dev(eps)).cpu().numpy()
+    assert _relerr(Yg, Yo, om.mask()) <= TOL_APPLY
+    assert np.all(Yg[om.mask() == 0] == 0)
+
+
+@pytest.mark.parametrize("p,B,deg,variant", [(1, 4, 5, 5), (3, 10, 4, 5), (4, 34, 6, 5), (5, 6, 3, 5), (6, 18, 5, 5),
+                                             (7, 4, 2, 5), (8, 2, 4, 5), (6, 18, 5, 3), (4, 7, 4, 0), (6, 3, 3, 0)])
+def test_filter_unequal_mesh_all_paths(p, B, deg, variant):
+    """cheb_filter on the 2x3x4 unequal mesh: pre-initialised TMA recurrence (even B) and the legacy path (odd B or
+    variant 3); caller data in the Dirichlet rows of X must be ignored (R5) and come back as 0."""
+    om, gm = _pair(UNEQUAL, p, _coulomb)
+    gm.set_variant(variant)
+    mask = om.mask()
+    X = workloads.random_block(300 + p, om.N, B)  # garbage in boundary rows
+    X0 = X * mask[:, None]
+    import oracle
+    th_min, th_max, beta = oracle.lanczos_bounds(om, workloads.normal(3100 + p, om.N), 20)
+    b, a0 = th_max + beta, th_min
+    a = a0 + 0.1 * (b - a0)
+    Yo = om.filter(X0, deg, a, b, a0)
+    work = torch.full((2 * om.N * B,), 7.5, dtype=torch.float64, device="cuda")  # dirty work space
+    Yg = gm.cheb_filter(_dev(X).clone(), deg, a, b, a0, work).cpu().numpy()
+    assert _relerr(Yg, Yo, mask) <= TOL_FILTER
+    assert np.all(Yg[mask == 0] == 0)
+
+
 @pytest.mark.parametrize("p,B", [(2, 1), (2, 8), (3, 33), (4, 64), (2, 70)])
 def test_apply_unequal_mesh_ragged_B(p, B):
     """2x3x4 cells with unequal edges (axis-order bugs), B = 1, a ragged tail, several tiles."""
