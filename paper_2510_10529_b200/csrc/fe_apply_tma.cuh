@@ -101,32 +101,45 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
 {
     constexpr int n = P + 1, n2 = n * n, n3 = n * n * n, NP = TmaShape<n>::NP, SMALL = TmaShape<n>::SMALL;
     extern __shared__ __align__(128) double smem[];
-    double* bufA = smem;                // [n^3][BT]  X -> A -> R -> scaled output
-    double* bufB = smem + n3 * BT;      // [n^3][BT]  owner term -> A2
-    double* sVZ = bufB + n3 * BT;       // [qx][qy][NP]
+    double* buf0 = smem;                // [n^3][BT]  the two tile buffers swap roles every unit:
+    double* buf1 = smem + n3 * BT;      // [n^3][BT]    bufX: X -> A -> R -> scaled output;  bufO: owner term -> A2 -> next X
+    double* sVZ = buf1 + n3 * BT;       // [qx][qy][NP]
     double* sIn = sVZ + SMALL;          // [az][ay][NP]  s_g
     double* sOut = sIn + SMALL;         // [az][ay][NP]  alpha kz s_g
     unsigned long long* bar = (unsigned long long*)(sOut + SMALL);
     const int lane = threadIdx.x, pl = threadIdx.y, tid = pl * BT + lane;
-    const int cell = blockIdx.x;
-    const int ex = cell % prm.cx, ey = (cell / prm.cx) % prm.cy, ez = cell / (prm.cx * prm.cy);
-    const int j0 = blockIdx.y * BT;
-    const int gx0 = ex * P, gy0 = ey * P, gz0 = ez * P;
+    const int nbt = (prm.B + BT - 1) / BT;
+    const long long nunits = (long long)prm.cx * prm.cy * prm.cz * nbt;  // unit = (cell, tile of BT vectors), tile fastest
+    const bool issuer = (lane == 0) && (pl < P);
+    const bool early = prm.owner || prm.preinit;
 
     if (tid == 0) {
         mbar_init(bar, 1);
+        const long long u = blockIdx.x;
+        const int cell = (int)(u / nbt), ex = cell % prm.cx, ey = (cell / prm.cx) % prm.cy, ez = cell / (prm.cx * prm.cy);
         mbar_expect_tx(bar, (unsigned)((n3 * BT + SMALL) * sizeof(double)));
-        tma_load4(bufA, &prm.mXn, j0, gx0, gy0, gz0, bar);
+        tma_load4(buf0, &prm.mXn, (int)(u % nbt) * BT, ex * P, ey * P, ez * P, bar);
         bulk_load(sVZ, prm.VZ + (size_t)cell * SMALL, (unsigned)(SMALL * sizeof(double)), bar);
     }
+    __syncthreads();
+    unsigned parity = 0;
+    double* bufA = buf0;
+    double* bufB = buf1;
+    // persistent over units: the next unit's X tile lands in bufB while plane phase 2 of this unit runs out of bufA
+    for (long long u = blockIdx.x; u < nunits; u += gridDim.x) {
+    const int cell = (int)(u / nbt);
+    const int ex = cell % prm.cx, ey = (cell / prm.cx) % prm.cy, ez = cell / (prm.cx * prm.cy);
+    const int j0 = (int)(u % nbt) * BT;
+    const int gx0 = ex * P, gy0 = ey * P, gz0 = ez * P;
     const double hx = prm.hx[ex], hy = prm.hy[ey], hz = prm.hz[ez];
-    {
+    {   // scale tiles of this thread's own nodal plane (read back only by the lanes of this plane)
         const double akz = prm.alpha * 0.25 * hx * hy / hz;  // alpha * 2J/hz^2, J = hx hy hz / 8
-        for (int i = tid; i < SMALL; i += n * BT) {
-            const int ax = i % NP, ay = (i / NP) % n, az = i / (NP * n);
-            const double s = ax < n ? prm.sx[gx0 + ax] * prm.sy[gy0 + ay] * prm.sz[gz0 + az] : 0.0;
-            sIn[i] = s;
-            sOut[i] = akz * s;
+        const double szv = prm.sz[gz0 + pl];
+        for (int i = lane; i < n * NP; i += BT) {
+            const int ax = i % NP, ay = i / NP;
+            const double s = ax < n ? prm.sx[gx0 + ax] * prm.sy[gy0 + ay] * szv : 0.0;
+            sIn[pl * n * NP + i] = s;
+            sOut[pl * n * NP + i] = akz * s;
         }
     }
     const double ry = (hx * hx) / (hy * hy);   // ky/kx
@@ -136,8 +149,10 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
         const int j = j0 + lane;
         kappa = -prm.alpha * (prm.c + ((prm.eps && j < prm.B) ? prm.eps[j] : 0.0));
     }
-    __syncthreads();
-    mbar_wait(bar, 0);
+    if (lane == 0) bulk_wait_read0();  // the previous unit's reduce-add has read its source (now bufB)
+    __syncwarp();
+    mbar_wait(bar, parity);
+    parity ^= 1;
 
     double v[n][n], t[n], o[n];
     double* pA = bufA + (size_t)pl * n2 * BT + lane;
@@ -148,8 +163,6 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
     for (int ay = 0; ay < n; ++ay)
 #pragma unroll
         for (int ax = 0; ax < n; ++ax) v[ay][ax] = pA[(ay * n + ax) * BT];
-    const bool issuer = (lane == 0) && (pl < P);
-    const bool early = prm.owner || prm.preinit;
     if (early) {
         if (pl < P) {
             // compact p x p sub-planes: beta' X -> own plane of bufA (store to W), kappa X -> own plane of bufB (add to Y)
@@ -251,6 +264,13 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
         }
     }
     __syncthreads();
+    if (tid == 0 && u + gridDim.x < nunits) {  // bufB (A2) and sVZ are dead: bring in the next unit
+        const long long un = u + gridDim.x;
+        const int cn = (int)(un / nbt), nx = cn % prm.cx, ny = (cn / prm.cx) % prm.cy, nz = cn / (prm.cx * prm.cy);
+        mbar_expect_tx(bar, (unsigned)((n3 * BT + SMALL) * sizeof(double)));
+        tma_load4(bufB, &prm.mXn, (int)(un % nbt) * BT, nx * P, ny * P, nz * P, bar);
+        bulk_load(sVZ, prm.VZ + (size_t)cn * SMALL, (unsigned)(SMALL * sizeof(double)), bar);
+    }
     // ---- plane phase 2: back-interpolate in y and x, scale by alpha kz s_g, one bulk reduce-add per nodal plane ---------
 #pragma unroll
     for (int qy = 0; qy < n; ++qy)
@@ -276,12 +296,15 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
     if (lane == 0) {
         tma_reduce_add4(&prm.mYn1, pA, j0, gx0, gy0, gz0 + pl);
         bulk_commit();
-        bulk_wait_read0();  // shared memory must stay valid until the bulk engine has read it
     }
+    double* tmp = bufA; bufA = bufB; bufB = tmp;
+    }  // units
+    if (lane == 0) bulk_wait_read0();  // shared memory must stay valid until the bulk engine has read it
 }
 
+// ctas > 0: persistent launch with that many CTAs (each walks units blockIdx.x, +ctas, ...); 0: one CTA per unit
 template <int P, int BT, int MINB>
-cudaError_t launch_tma(const TmaParams& prm, long long ncells, bool first, cudaStream_t st)
+cudaError_t launch_tma(const TmaParams& prm, long long ncells, bool first, cudaStream_t st, int ctas)
 {
     constexpr int n = P + 1;
     constexpr size_t smem = tma_smem_bytes<P, BT>();
@@ -293,7 +316,10 @@ cudaError_t launch_tma(const TmaParams& prm, long long ncells, bool first, cudaS
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    dim3 grid((unsigned)ncells, (unsigned)((prm.B + BT - 1) / BT)), block(BT, n);
+    const long long nunits = ncells * ((prm.B + BT - 1) / BT);
+    long long g = nunits;
+    if (ctas > 0 && (long long)ctas * MINB < g) g = (long long)ctas * MINB;
+    dim3 grid((unsigned)g), block(BT, n);
     if (first)
         k_apply_tma<P, BT, MINB, true><<<grid, block, smem, st>>>(prm);
     else
@@ -302,19 +328,24 @@ cudaError_t launch_tma(const TmaParams& prm, long long ncells, bool first, cudaS
 }
 
 // box width (vectors per CTA) of the TMA kernel for order p
-inline int tma_bt(int p) { return p >= 6 ? 16 : 32; }
+inline int tma_bt(int p, int variant = 0) { return (p >= 6 && variant != 6) ? 16 : 32; }
 
-inline cudaError_t launch_apply_tma(const TmaParams& prm, int p, long long ncells, bool first, cudaStream_t st)
+// variant 7: persistent grid of sms x (resident CTAs per SM) CTAs, each walking units with the next X tile
+// prefetched (measured no faster than one CTA per unit, the default); 6 = 32-wide box at p = 6
+inline cudaError_t launch_apply_tma(const TmaParams& prm, int p, long long ncells, bool first, cudaStream_t st,
+                                    int variant, int sms)
 {
+    if (variant != 7) sms = 0;
+    if (variant == 6 && p == 6) return launch_tma<6, 32, 1>(prm, ncells, first, st, sms);
     switch (p) {
-        case 1: return launch_tma<1, 32, 8>(prm, ncells, first, st);
-        case 2: return launch_tma<2, 32, 6>(prm, ncells, first, st);
-        case 3: return launch_tma<3, 32, 4>(prm, ncells, first, st);
-        case 4: return launch_tma<4, 32, 3>(prm, ncells, first, st);
-        case 5: return launch_tma<5, 32, 1>(prm, ncells, first, st);
-        case 6: return launch_tma<6, 16, 2>(prm, ncells, first, st);
-        case 7: return launch_tma<7, 16, 1>(prm, ncells, first, st);
-        case 8: return launch_tma<8, 16, 1>(prm, ncells, first, st);
+        case 1: return launch_tma<1, 32, 8>(prm, ncells, first, st, sms);
+        case 2: return launch_tma<2, 32, 6>(prm, ncells, first, st, sms);
+        case 3: return launch_tma<3, 32, 4>(prm, ncells, first, st, sms);
+        case 4: return launch_tma<4, 32, 3>(prm, ncells, first, st, sms);
+        case 5: return launch_tma<5, 32, 1>(prm, ncells, first, st, sms);
+        case 6: return launch_tma<6, 16, 2>(prm, ncells, first, st, sms);
+        case 7: return launch_tma<7, 16, 1>(prm, ncells, first, st, sms);
+        case 8: return launch_tma<8, 16, 1>(prm, ncells, first, st, sms);
     }
     return cudaErrorInvalidValue;
 }

@@ -54,6 +54,7 @@ struct fe_mesh {
     EOTab eoN, eoNT, eoG;    // even-odd halves of N' = diag(sqrt w) N, N'^T, G' = diag(w^-1/2) G diag(w^-1/2)
     bool have_V = false;
     int variant = 0;
+    int sms = 0;  // multiprocessors of the device (persistent grid size)
     int64_t launches = 0;
 };
 
@@ -134,6 +135,7 @@ int fe_mesh_create(const double* xe, int cx, const double* ye, int cy, const dou
     if (!m) return fail(FE_ERR_NOMEM, "fe_mesh_create: host allocation failed");
     m->p = p; m->n = p + 1; m->cx = cx; m->cy = cy; m->cz = cz; m->device = cuda_device;
     m->nc = m->n * m->n * m->n;
+    m->sms = prop.multiProcessorCount;
     m->Nx = Nx; m->Ny = Ny; m->Nz = Nz; m->N = Nx * Ny * Nz; m->ncells = (int64_t)cx * cy * cz;
     m->xe.assign(xe, xe + cx + 1); m->ye.assign(ye, ye + cy + 1); m->ze.assign(ze, ze + cz + 1);
     build_tables(p, &m->tab);
@@ -377,7 +379,7 @@ struct BlockMaps {
 
 static int make_block_maps(BlockMaps* bm, const fe_mesh* m, const double* base, int B)
 {
-    const int bt = tma_bt(m->p), n = m->n, p = m->p;
+    const int bt = tma_bt(m->p, m->variant), n = m->n, p = m->p;
     int rc;
     if ((rc = make_map(&bm->n3, m, base, B, bt, n, n, n))) return rc;
     if ((rc = make_map(&bm->n1, m, base, B, bt, n, n, 1))) return rc;
@@ -387,7 +389,7 @@ static int make_block_maps(BlockMaps* bm, const fe_mesh* m, const double* base, 
 // bulk tensor copies need 16-byte aligned bases and row pitches (B even)
 static bool tma_eligible(const fe_mesh* m, int B, const void* a, const void* b, const void* c)
 {
-    if (m->variant != 0 && m->variant != 5) return false;
+    if (m->variant != 0 && m->variant < 5) return false;
     if (B % 2 != 0 || !encode_fn()) return false;
     return (((uintptr_t)a | (uintptr_t)b | (uintptr_t)c) & 15) == 0;
 }
@@ -410,7 +412,7 @@ static int tma_step(fe_mesh* m, const BlockMaps& X, const BlockMaps& Y, const Bl
     prm.mXn = X.n3; prm.mYn1 = Y.n1; prm.mYp1 = Y.p1; prm.mWp1 = W ? W->p1 : Y.p1;
     prm.eps = eps; prm.alpha = alpha; prm.c = c; prm.owner = owner ? 1 : 0;
     prm.preinit = W ? 1 : 0; prm.beta_next = beta_next;
-    cudaError_t e = launch_apply_tma(prm, m->p, m->ncells, first, st);
+    cudaError_t e = launch_apply_tma(prm, m->p, m->ncells, first, st, m->variant, m->sms);
     if (e != cudaSuccess) return fail(FE_ERR_CUDA, "operator launch failed: %s", cudaGetErrorString(e));
     m->launches += 1;
     return FE_OK;
