@@ -32,7 +32,7 @@ struct TmaParams {
     const double* eps;
     const double* VZ;  // cells * n*n*NP: V_q hz^2/2, [qx][qy][qz padded to NP]
     const double *sx, *sy, *sz;  // per-axis mu M^{-1/2}
-    const double *hx, *hy, *hz;
+    const double *gx, *gy, *gz;  // per-axis cell geometry, 4 doubles per cell: h, h^2, 1/h^2, 1/h
     int B, cx, cy, cz;
     int owner, preinit;
     double alpha, c, beta_next;
@@ -96,7 +96,7 @@ constexpr size_t tma_smem_bytes()
 }
 
 // FIRST: X is caller data whose Dirichlet rows may hold anything (R5) -> mask them in the owner / pre-init terms.
-template <int P, int BT, int MINB, bool FIRST>
+template <int P, int BT, int MINB, bool FIRST, bool PERSIST>
 __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_constant__ TmaParams prm)
 {
     constexpr int n = P + 1, n2 = n * n, n3 = n * n * n, NP = TmaShape<n>::NP, SMALL = TmaShape<n>::SMALL;
@@ -131,9 +131,11 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
     const int ex = cell % prm.cx, ey = (cell / prm.cx) % prm.cy, ez = cell / (prm.cx * prm.cy);
     const int j0 = (int)(u % nbt) * BT;
     const int gx0 = ex * P, gy0 = ey * P, gz0 = ez * P;
-    const double hx = prm.hx[ex], hy = prm.hy[ey], hz = prm.hz[ez];
+    const double4 qx = *reinterpret_cast<const double4*>(prm.gx + 4 * ex);
+    const double4 qy = *reinterpret_cast<const double4*>(prm.gy + 4 * ey);
+    const double4 qz = *reinterpret_cast<const double4*>(prm.gz + 4 * ez);
     {   // scale tiles of this thread's own nodal plane (read back only by the lanes of this plane)
-        const double akz = prm.alpha * 0.25 * hx * hy / hz;  // alpha * 2J/hz^2, J = hx hy hz / 8
+        const double akz = prm.alpha * 0.25 * qx.x * qy.x * qz.w;  // alpha * 2J/hz^2, J = hx hy hz / 8
         const double szv = prm.sz[gz0 + pl];
         for (int i = lane; i < n * NP; i += BT) {
             const int ax = i % NP, ay = i / NP;
@@ -142,8 +144,8 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
             sOut[pl * n * NP + i] = akz * s;
         }
     }
-    const double ry = (hx * hx) / (hy * hy);   // ky/kx
-    const double rxz = (hz * hz) / (hx * hx);  // kx/kz
+    const double ry = qx.y * qy.z;   // ky/kx = hx^2/hy^2
+    const double rxz = qz.y * qx.z;  // kx/kz = hz^2/hx^2
     double kappa = 0.0;
     if (prm.owner) {
         const int j = j0 + lane;
@@ -264,7 +266,7 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
         }
     }
     __syncthreads();
-    if (tid == 0 && u + gridDim.x < nunits) {  // bufB (A2) and sVZ are dead: bring in the next unit
+    if (PERSIST && tid == 0 && u + gridDim.x < nunits) {  // bufB (A2) and sVZ are dead: bring in the next unit
         const long long un = u + gridDim.x;
         const int cn = (int)(un / nbt), nx = cn % prm.cx, ny = (cn / prm.cx) % prm.cy, nz = cn / (prm.cx * prm.cy);
         mbar_expect_tx(bar, (unsigned)((n3 * BT + SMALL) * sizeof(double)));
@@ -297,6 +299,7 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
         tma_reduce_add4(&prm.mYn1, pA, j0, gx0, gy0, gz0 + pl);
         bulk_commit();
     }
+    if (!PERSIST) break;
     double* tmp = bufA; bufA = bufB; bufB = tmp;
     }  // units
     if (lane == 0) bulk_wait_read0();  // shared memory must stay valid until the bulk engine has read it
@@ -310,20 +313,30 @@ cudaError_t launch_tma(const TmaParams& prm, long long ncells, bool first, cudaS
     constexpr size_t smem = tma_smem_bytes<P, BT>();
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_apply_tma<P, BT, MINB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(k_apply_tma<P, BT, MINB, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(k_apply_tma<P, BT, MINB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            e = cudaFuncSetAttribute(k_apply_tma<P, BT, MINB, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(k_apply_tma<P, BT, MINB, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(k_apply_tma<P, BT, MINB, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         configured = true;
     }
     const long long nunits = ncells * ((prm.B + BT - 1) / BT);
-    long long g = nunits;
-    if (ctas > 0 && (long long)ctas * MINB < g) g = (long long)ctas * MINB;
-    dim3 grid((unsigned)g), block(BT, n);
-    if (first)
-        k_apply_tma<P, BT, MINB, true><<<grid, block, smem, st>>>(prm);
-    else
-        k_apply_tma<P, BT, MINB, false><<<grid, block, smem, st>>>(prm);
+    const bool persist = ctas > 0 && (long long)ctas * MINB < nunits;
+    dim3 grid((unsigned)(persist ? (long long)ctas * MINB : nunits)), block(BT, n);
+    if (persist) {
+        if (first)
+            k_apply_tma<P, BT, MINB, true, true><<<grid, block, smem, st>>>(prm);
+        else
+            k_apply_tma<P, BT, MINB, false, true><<<grid, block, smem, st>>>(prm);
+    } else {
+        if (first)
+            k_apply_tma<P, BT, MINB, true, false><<<grid, block, smem, st>>>(prm);
+        else
+            k_apply_tma<P, BT, MINB, false, false><<<grid, block, smem, st>>>(prm);
+    }
     return cudaGetLastError();
 }
 

@@ -51,6 +51,7 @@ struct fe_mesh {
     double* d_WV = nullptr;  // cells*n^3: J w_q V_q
     double* d_VZ = nullptr;  // cells*n*n*NP: V_q hz^2/2, [qx][qy][qz] rows padded to NP (TMA kernel)
     double *d_sx = nullptr, *d_sy = nullptr, *d_sz = nullptr;  // per-axis mu M^{-1/2}
+    double *d_gx = nullptr, *d_gy = nullptr, *d_gz = nullptr;  // per-axis cell geometry: h, h^2, 1/h^2, 1/h
     EOTab eoN, eoNT, eoG;    // even-odd halves of N' = diag(sqrt w) N, N'^T, G' = diag(w^-1/2) G diag(w^-1/2)
     bool have_V = false;
     int variant = 0;
@@ -160,6 +161,10 @@ int fe_mesh_create(const double* xe, int cx, const double* ye, int cy, const dou
         return code;
     };
     if ((rc = upload(&m->d_sx, s[0])) || (rc = upload(&m->d_sy, s[1])) || (rc = upload(&m->d_sz, s[2]))) return cleanup(rc);
+    std::vector<double> g[3];
+    for (int d = 0; d < 3; ++d)
+        for (double hv : h[d]) { g[d].push_back(hv); g[d].push_back(hv * hv); g[d].push_back(1.0 / (hv * hv)); g[d].push_back(1.0 / hv); }
+    if ((rc = upload(&m->d_gx, g[0])) || (rc = upload(&m->d_gy, g[1])) || (rc = upload(&m->d_gz, g[2]))) return cleanup(rc);
     if ((rc = upload(&m->d_hx, h[0])) || (rc = upload(&m->d_hy, h[1])) || (rc = upload(&m->d_hz, h[2]))) return cleanup(rc);
     cudaError_t ce = cudaMalloc((void**)&m->d_sm, (size_t)m->N * sizeof(double));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&m->d_WV, (size_t)m->ncells * m->nc * sizeof(double));
@@ -181,6 +186,7 @@ int fe_mesh_destroy(fe_mesh* m)
     if (!m) return FE_OK;
     cudaSetDevice(m->device);
     cudaFree(m->d_sm); cudaFree(m->d_hx); cudaFree(m->d_hy); cudaFree(m->d_hz); cudaFree(m->d_WV);
+    cudaFree(m->d_gx); cudaFree(m->d_gy); cudaFree(m->d_gz);
     cudaFree(m->d_VZ); cudaFree(m->d_sx); cudaFree(m->d_sy); cudaFree(m->d_sz);
     delete m;
     return FE_OK;
@@ -398,7 +404,7 @@ static void fill_tma_params(const fe_mesh* m, TmaParams* prm, int B)
 {
     memset(prm, 0, sizeof(*prm));
     prm->VZ = m->d_VZ; prm->sx = m->d_sx; prm->sy = m->d_sy; prm->sz = m->d_sz;
-    prm->hx = m->d_hx; prm->hy = m->d_hy; prm->hz = m->d_hz;
+    prm->gx = m->d_gx; prm->gy = m->d_gy; prm->gz = m->d_gz;
     prm->B = B; prm->cx = m->cx; prm->cy = m->cy; prm->cz = m->cz;
     prm->eoN = m->eoN; prm->eoNT = m->eoNT; prm->eoG = m->eoG;
 }
