@@ -28,9 +28,9 @@ UNIT = "GDoF-vectors/s"
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE k_apply launch from the committed `ncu --set full` captures
-# (profiles/r1_c2_k_apply_full.md, profiles/r1_c3_k_apply_full.md); the zero-fill memset adds N*B*8 bytes on top.
-NCU_TRAFFIC_BYTES = {2: 428.05e6 + 111.56e6, 3: 4.9201e9 + 1.5490e9}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE k_apply_tma launch from the committed `ncu --set full` captures
+# (profiles/r1b_c2_k_apply_tma_full.md, profiles/r1b_c3_k_apply_tma_full.md)
+NCU_TRAFFIC_BYTES = {2: 286.17e6 + 220.99e6, 3: 3.6583e9 + 3.3016e9}
 
 
 def algorithmic_flops_per_cell_vector(p):
@@ -241,7 +241,7 @@ def summarize(w, r, total_ms_per_step, n_ranks=1):
     ach = flops_launch / dur / 1e12
     return value, {"bound": "alu", "achieved": ach, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
                    "frac": ach / FP64_PEAK_TFLOPS, "traffic": None,
-                   "kernel": "k_apply<p=%d> (one fused operator step incl. its zero-fill)" % w.p,
+                   "kernel": "k_apply_tma<p=%d> (one fused operator step: filter time / m, CUDA events on the launching stream)" % w.p,
                    "launch_ms": dur * 1e3,
                    "peak_source": "derived: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md); DFMA microbenchmark 36.8",
                    "hbm_frac_of_measured": None}
