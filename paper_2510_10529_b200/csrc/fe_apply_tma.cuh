@@ -204,7 +204,32 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
 #pragma unroll
         for (int q = 0; q < n; ++q) v[q][qx] = o[q];
     }
-    {
+    if (early) {  // the bulk operations must have read their shared-memory sources before A / A2 overwrite them
+        if (issuer) bulk_wait_read0();
+        __syncwarp();
+    }
+    if constexpr (n >= 7) {
+        // large planes: park A in shared memory first and re-read its columns for the y stiffness, so that only one
+        // plane (plus a line) is live in registers instead of two
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy)
+#pragma unroll
+            for (int qx = 0; qx < n; ++qx) pA[(qy * n + qx) * BT] = v[qy][qx];
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy) {
+            mat1d_eo<n>(prm.eoG, v[qy], o);
+#pragma unroll
+            for (int qx = 0; qx < n; ++qx) v[qy][qx] = o[qx];
+        }
+#pragma unroll
+        for (int qx = 0; qx < n; ++qx) {
+#pragma unroll
+            for (int a = 0; a < n; ++a) t[a] = pA[(a * n + qx) * BT];
+            mat1d_eo<n>(prm.eoG, t, o);
+#pragma unroll
+            for (int qy = 0; qy < n; ++qy) pB[(qy * n + qx) * BT] = fma(ry, o[qy], v[qy][qx]);
+        }
+    } else {
         double v2[n][n];
 #pragma unroll
         for (int qy = 0; qy < n; ++qy) mat1d_eo<n>(prm.eoG, v[qy], v2[qy]);
@@ -215,10 +240,6 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
             mat1d_eo<n>(prm.eoG, t, o);
 #pragma unroll
             for (int qy = 0; qy < n; ++qy) v2[qy][qx] = fma(ry, o[qy], v2[qy][qx]);
-        }
-        if (early) {  // the bulk operations must have read their shared-memory sources before A / A2 overwrite them
-            if (issuer) bulk_wait_read0();
-            __syncwarp();
         }
 #pragma unroll
         for (int qy = 0; qy < n; ++qy)
@@ -340,16 +361,23 @@ cudaError_t launch_tma(const TmaParams& prm, long long ncells, bool first, cudaS
     return cudaGetLastError();
 }
 
-// box width (vectors per CTA) of the TMA kernel for order p
-inline int tma_bt(int p, int variant = 0) { return (p >= 6 && variant != 6) ? 16 : 32; }
+// Launch shape of the TMA kernel.  Variants: 0 = default, 5 = one CTA per unit everywhere, 6 = 32-wide box at p = 6 with
+// one CTA per unit, 7 = persistent everywhere, 8 = 32-wide persistent at p = 6 (= the default when B > 16).
+// p = 6 default: ONE persistent 7-warp CTA per SM walking (cell, 32 vectors) units.  Its warps run the same 74 KB of
+// straight-line code nearly in lockstep and share instruction-cache lines; two independent 16-wide CTAs per SM
+// each stream the code through the 32 KB L1.5 on their own (ncu: no_instruction stall 0.9 -> 0.08 per issue).
+inline bool tma_wide6(int p, int variant, int B)
+{
+    return p == 6 && (variant == 6 || variant == 8 || (variant == 0 && B > 16));
+}
+inline int tma_bt(int p, int variant, int B) { return (p >= 6 && !tma_wide6(p, variant, B)) ? 16 : 32; }
 
-// variant 7: persistent grid of sms x (resident CTAs per SM) CTAs, each walking units with the next X tile
-// prefetched (measured no faster than one CTA per unit, the default); 6 = 32-wide box at p = 6
 inline cudaError_t launch_apply_tma(const TmaParams& prm, int p, long long ncells, bool first, cudaStream_t st,
                                     int variant, int sms)
 {
-    if (variant != 7) sms = 0;
-    if (variant == 6 && p == 6) return launch_tma<6, 32, 1>(prm, ncells, first, st, sms);
+    const bool wide6 = tma_wide6(p, variant, prm.B);
+    if (!(variant == 7 || variant == 8 || (variant == 0 && wide6))) sms = 0;
+    if (wide6) return launch_tma<6, 32, 1>(prm, ncells, first, st, sms);
     switch (p) {
         case 1: return launch_tma<1, 32, 8>(prm, ncells, first, st, sms);
         case 2: return launch_tma<2, 32, 6>(prm, ncells, first, st, sms);

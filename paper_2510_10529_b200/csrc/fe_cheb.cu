@@ -385,7 +385,7 @@ struct BlockMaps {
 
 static int make_block_maps(BlockMaps* bm, const fe_mesh* m, const double* base, int B)
 {
-    const int bt = tma_bt(m->p, m->variant), n = m->n, p = m->p;
+    const int bt = tma_bt(m->p, m->variant, B), n = m->n, p = m->p;
     int rc;
     if ((rc = make_map(&bm->n3, m, base, B, bt, n, n, n))) return rc;
     if ((rc = make_map(&bm->n1, m, base, B, bt, n, n, 1))) return rc;

@@ -850,7 +850,7 @@ cudaError_t launch_v4(const ApplyParams& prm, long long ncells, cudaStream_t st)
 inline bool variant_supported(int p, int variant)
 {
     (void)p;
-    return variant >= 0 && variant <= 7;  // 5 = TMA generation (the default for even B), 1-4 legacy
+    return variant >= 0 && variant <= 8;  // 5 = TMA generation (the default for even B), 1-4 legacy
 }
 
 template <int P, int BT>
