@@ -30,13 +30,12 @@ struct TmaParams {
     CUtensorMap mYp1;  // Y : box (BT,p,p,1), reduce-add of the owner term kappa_j X
     CUtensorMap mWp1;  // W : box (BT,p,p,1), store of beta' X
     const double* eps;
-    const double* VZ;  // cells * n*n*NP: V_q hz^2/2, [qx][qy][qz padded to NP]
-    const double *sx, *sy, *sz;  // per-axis mu M^{-1/2}
-    const double *gx, *gy, *gz;  // per-axis cell geometry, 4 doubles per cell: h, h^2, 1/h^2, 1/h
+    const double* rec;  // cells * REC: per-cell record  VZ = V_q hz^2/2 [qx][qy][NP] | s_g [az][ay][NP] | kz s_g | ky/kx, kx/kz
     int B, cx, cy, cz;
     int owner, preinit;
     double alpha, c, beta_next;
     EOTab eoN, eoNT, eoG;  // even-odd halves of N', N'^T, G'
+    EOTab eoNTa;           // alpha N'^T (the last back-interpolation carries the step's alpha)
 };
 
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -78,6 +77,11 @@ __device__ __forceinline__ void tma_store4(const CUtensorMap* m, const void* src
     asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.tile.bulk_group [%0, {%2,%3,%4,%5}], [%1];"
                  ::"l"(m), "r"(smem_u32(src)), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
 }
+__device__ __forceinline__ void tma_prefetch_l2(const CUtensorMap* m, int c0, int c1, int c2, int c3)
+{
+    asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1,%2,%3,%4}];"
+                 ::"l"(m), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
@@ -86,27 +90,29 @@ template <int n>
 struct TmaShape {
     static constexpr int NP = n + (n & 1);  // rows of the small tiles padded to an even length (16-byte LDS.128)
     static constexpr int SMALL = n * n * NP;
+    // per-cell record in global memory, brought in by ONE bulk copy per unit: VZ | s_g | kz s_g | ry, rxz, pad
+    static constexpr int REC = 3 * SMALL + 8;
 };
 
 template <int P, int BT>
 constexpr size_t tma_smem_bytes()
 {
     constexpr int n = P + 1;
-    return ((size_t)2 * n * n * n * BT + 3 * TmaShape<n>::SMALL) * sizeof(double) + 16;
+    return ((size_t)2 * n * n * n * BT + 2 * TmaShape<n>::REC) * sizeof(double) + 16;
 }
 
 // FIRST: X is caller data whose Dirichlet rows may hold anything (R5) -> mask them in the owner / pre-init terms.
 template <int P, int BT, int MINB, bool FIRST, bool PERSIST>
 __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_constant__ TmaParams prm)
 {
-    constexpr int n = P + 1, n2 = n * n, n3 = n * n * n, NP = TmaShape<n>::NP, SMALL = TmaShape<n>::SMALL;
+    constexpr int n = P + 1, n2 = n * n, n3 = n * n * n, NP = TmaShape<n>::NP, SMALL = TmaShape<n>::SMALL,
+                  REC = TmaShape<n>::REC;
     extern __shared__ __align__(128) double smem[];
-    double* buf0 = smem;                // [n^3][BT]  the two tile buffers swap roles every unit:
-    double* buf1 = smem + n3 * BT;      // [n^3][BT]    bufX: X -> A -> R -> scaled output;  bufO: owner term -> A2 -> next X
-    double* sVZ = buf1 + n3 * BT;       // [qx][qy][NP]
-    double* sIn = sVZ + SMALL;          // [az][ay][NP]  s_g
-    double* sOut = sIn + SMALL;         // [az][ay][NP]  alpha kz s_g
-    unsigned long long* bar = (unsigned long long*)(sOut + SMALL);
+    double* buf0 = smem;                // [n^3][BT]  bufA: X -> A (dead after pass 1 of the line phase) -> next unit's X
+    double* buf1 = smem + n3 * BT;      // [n^3][BT]  bufB: owner term -> A2 -> R -> scaled output (source of the reduce-add)
+    double* rec0 = buf1 + n3 * BT;      // two cell records (double-buffered like the tiles): VZ [qx][qy][NP],
+    double* rec1 = rec0 + REC;          //   s_g [az][ay][NP], kz s_g [az][ay][NP], {ky/kx, kx/kz}
+    unsigned long long* bar = (unsigned long long*)(rec1 + REC);  // bar[0]: tile + record landed; bar[1]: A consumed
     const int lane = threadIdx.x, pl = threadIdx.y, tid = pl * BT + lane;
     const int nbt = (prm.B + BT - 1) / BT;
     const long long nunits = (long long)prm.cx * prm.cy * prm.cz * nbt;  // unit = (cell, tile of BT vectors), tile fastest
@@ -115,46 +121,43 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
 
     if (tid == 0) {
         mbar_init(bar, 1);
+        mbar_init(bar + 1, (n * BT + 31) / 32);
         const long long u = blockIdx.x;
         const int cell = (int)(u / nbt), ex = cell % prm.cx, ey = (cell / prm.cx) % prm.cy, ez = cell / (prm.cx * prm.cy);
-        mbar_expect_tx(bar, (unsigned)((n3 * BT + SMALL) * sizeof(double)));
+        mbar_expect_tx(bar, (unsigned)((n3 * BT + REC) * sizeof(double)));
         tma_load4(buf0, &prm.mXn, (int)(u % nbt) * BT, ex * P, ey * P, ez * P, bar);
-        bulk_load(sVZ, prm.VZ + (size_t)cell * SMALL, (unsigned)(SMALL * sizeof(double)), bar);
+        bulk_load(rec0, prm.rec + (size_t)cell * REC, (unsigned)(REC * sizeof(double)), bar);
     }
     __syncthreads();
     unsigned parity = 0;
-    double* bufA = buf0;
-    double* bufB = buf1;
-    // persistent over units: the next unit's X tile lands in bufB while plane phase 2 of this unit runs out of bufA
+    double* const bufA = buf0;
+    double* const bufB = buf1;
+    double* rec = rec0;
+    double* recN = rec1;
+    // persistent over units: the next unit's X tile lands in bufA as soon as every warp is past pass 1 of the line phase
     for (long long u = blockIdx.x; u < nunits; u += gridDim.x) {
     const int cell = (int)(u / nbt);
     const int ex = cell % prm.cx, ey = (cell / prm.cx) % prm.cy, ez = cell / (prm.cx * prm.cy);
     const int j0 = (int)(u % nbt) * BT;
     const int gx0 = ex * P, gy0 = ey * P, gz0 = ez * P;
-    const double4 qx = *reinterpret_cast<const double4*>(prm.gx + 4 * ex);
-    const double4 qy = *reinterpret_cast<const double4*>(prm.gy + 4 * ey);
-    const double4 qz = *reinterpret_cast<const double4*>(prm.gz + 4 * ez);
-    {   // scale tiles of this thread's own nodal plane (read back only by the lanes of this plane)
-        const double akz = prm.alpha * 0.25 * qx.x * qy.x * qz.w;  // alpha * 2J/hz^2, J = hx hy hz / 8
-        const double szv = prm.sz[gz0 + pl];
-        for (int i = lane; i < n * NP; i += BT) {
-            const int ax = i % NP, ay = i / NP;
-            const double s = ax < n ? prm.sx[gx0 + ax] * prm.sy[gy0 + ay] * szv : 0.0;
-            sIn[pl * n * NP + i] = s;
-            sOut[pl * n * NP + i] = akz * s;
-        }
-    }
-    const double ry = qx.y * qy.z;   // ky/kx = hx^2/hy^2
-    const double rxz = qz.y * qx.z;  // kx/kz = hz^2/hx^2
     double kappa = 0.0;
     if (prm.owner) {
         const int j = j0 + lane;
         kappa = -prm.alpha * (prm.c + ((prm.eps && j < prm.B) ? prm.eps[j] : 0.0));
     }
-    if (lane == 0) bulk_wait_read0();  // the previous unit's reduce-add has read its source (now bufB)
+    if (PERSIST && tid == 0 && u + gridDim.x < nunits) {  // pull the next unit's X tile into L2 a whole unit ahead
+        const long long un = u + gridDim.x;
+        const int cn = (int)(un / nbt), nx = cn % prm.cx, ny = (cn / prm.cx) % prm.cy, nz = cn / (prm.cx * prm.cy);
+        tma_prefetch_l2(&prm.mXn, (int)(un % nbt) * BT, nx * P, ny * P, nz * P);
+    }
+    if (lane == 0) bulk_wait_read0();  // the previous unit's reduce-add has read its source (bufB)
     __syncwarp();
     mbar_wait(bar, parity);
     parity ^= 1;
+    const double* sVZ = rec;
+    const double* sIn = rec + SMALL;
+    const double* sOut = rec + 2 * SMALL;
+    const double ry = rec[3 * SMALL], rxz = rec[3 * SMALL + 1];  // ky/kx = hx^2/hy^2, kx/kz = hz^2/hx^2
 
     double v[n][n], t[n], o[n];
     double* pA = bufA + (size_t)pl * n2 * BT + lane;
@@ -262,12 +265,24 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
             for (int az = 0; az < n; ++az) t[az] = la[((az * n + qy) * n) * BT];
             mat1d_eo<n>(prm.eoN, t, v[qy]);
         }
+        if (PERSIST) {  // this warp no longer needs A: when all warps say so, bufA can take the next unit's X
+            __syncwarp();
+            if ((tid & 31) == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar + 1)) : "memory");
+        }
         // pass 2: T = VZ . U + G'z U
 #pragma unroll
         for (int qy = 0; qy < n; ++qy) {
             mat1d_eo<n>(prm.eoG, v[qy], o);
 #pragma unroll
             for (int qz = 0; qz < n; ++qz) v[qy][qz] = fma(lv[qy * NP + qz], v[qy][qz], o[qz]);
+        }
+        if (PERSIST && tid == 0 && u + gridDim.x < nunits) {
+            const long long un = u + gridDim.x;
+            const int cn = (int)(un / nbt), nx = cn % prm.cx, ny = (cn / prm.cx) % prm.cy, nz = cn / (prm.cx * prm.cy);
+            mbar_wait(bar + 1, parity ^ 1);  // parity was flipped after this unit's tile wait
+            mbar_expect_tx(bar, (unsigned)((n3 * BT + REC) * sizeof(double)));
+            tma_load4(bufA, &prm.mXn, (int)(un % nbt) * BT, nx * P, ny * P, nz * P, bar);
+            bulk_load(recN, prm.rec + (size_t)cn * REC, (unsigned)(REC * sizeof(double)), bar);
         }
         // pass 3: T += (kx/kz) N'z A2
 #pragma unroll
@@ -278,27 +293,20 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
 #pragma unroll
             for (int qz = 0; qz < n; ++qz) v[qy][qz] = fma(rxz, o[qz], v[qy][qz]);
         }
-        // pass 4: R = N'z^T T, back into the A field
+        // pass 4: R = N'z^T T, into the lines of the A2 field this thread has just consumed
 #pragma unroll
         for (int qy = 0; qy < n; ++qy) {
             mat1d_eo<n>(prm.eoNT, v[qy], o);
 #pragma unroll
-            for (int az = 0; az < n; ++az) la[((az * n + qy) * n) * BT] = o[az];
+            for (int az = 0; az < n; ++az) lb[((az * n + qy) * n) * BT] = o[az];
         }
     }
     __syncthreads();
-    if (PERSIST && tid == 0 && u + gridDim.x < nunits) {  // bufB (A2) and sVZ are dead: bring in the next unit
-        const long long un = u + gridDim.x;
-        const int cn = (int)(un / nbt), nx = cn % prm.cx, ny = (cn / prm.cx) % prm.cy, nz = cn / (prm.cx * prm.cy);
-        mbar_expect_tx(bar, (unsigned)((n3 * BT + SMALL) * sizeof(double)));
-        tma_load4(bufB, &prm.mXn, (int)(un % nbt) * BT, nx * P, ny * P, nz * P, bar);
-        bulk_load(sVZ, prm.VZ + (size_t)cn * SMALL, (unsigned)(SMALL * sizeof(double)), bar);
-    }
     // ---- plane phase 2: back-interpolate in y and x, scale by alpha kz s_g, one bulk reduce-add per nodal plane ---------
 #pragma unroll
     for (int qy = 0; qy < n; ++qy)
 #pragma unroll
-        for (int qx = 0; qx < n; ++qx) v[qy][qx] = pA[(qy * n + qx) * BT];
+        for (int qx = 0; qx < n; ++qx) v[qy][qx] = pB[(qy * n + qx) * BT];
 #pragma unroll
     for (int qx = 0; qx < n; ++qx) {
 #pragma unroll
@@ -310,18 +318,18 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
     const double* sout_pl = sOut + pl * n * NP;
 #pragma unroll
     for (int ay = 0; ay < n; ++ay) {
-        mat1d_eo<n>(prm.eoNT, v[ay], o);
+        mat1d_eo<n>(prm.eoNTa, v[ay], o);
 #pragma unroll
-        for (int ax = 0; ax < n; ++ax) pA[(ay * n + ax) * BT] = sout_pl[ay * NP + ax] * o[ax];
+        for (int ax = 0; ax < n; ++ax) pB[(ay * n + ax) * BT] = sout_pl[ay * NP + ax] * o[ax];
     }
     fence_async_smem();
     __syncwarp();
     if (lane == 0) {
-        tma_reduce_add4(&prm.mYn1, pA, j0, gx0, gy0, gz0 + pl);
+        tma_reduce_add4(&prm.mYn1, pB, j0, gx0, gy0, gz0 + pl);
         bulk_commit();
     }
     if (!PERSIST) break;
-    double* tmp = bufA; bufA = bufB; bufB = tmp;
+    double* tmp = rec; rec = recN; recN = tmp;
     }  // units
     if (lane == 0) bulk_wait_read0();  // shared memory must stay valid until the bulk engine has read it
 }
@@ -389,6 +397,27 @@ inline cudaError_t launch_apply_tma(const TmaParams& prm, int p, long long ncell
         case 8: return launch_tma<8, 16, 1>(prm, ncells, first, st, sms);
     }
     return cudaErrorInvalidValue;
+}
+
+// the mesh-dependent part of the cell records: s_g and kz s_g at the cell's nodes, ky/kx and kx/kz (VZ is written by
+// k_weight_potential); sx, sy, sz = per-axis mu M^{-1/2}, hx, hy, hz = per-axis cell sizes
+__global__ void k_build_records(double* __restrict__ rec, int n, int cx, int cy, long long ncells,
+                                const double* __restrict__ sx, const double* __restrict__ sy,
+                                const double* __restrict__ sz, const double* __restrict__ hx,
+                                const double* __restrict__ hy, const double* __restrict__ hz)
+{
+    const int NP = n + (n & 1), SMALL = n * n * NP, REC = 3 * SMALL + 8, p = n - 1;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < ncells * SMALL; i += (long long)gridDim.x * blockDim.x) {
+        const long long e = i / SMALL;
+        const int k = (int)(i - e * SMALL), ax = k % NP, ay = (k / NP) % n, az = k / (NP * n);
+        const int ex = (int)(e % cx), ey = (int)((e / cx) % cy), ez = (int)(e / ((long long)cx * cy));
+        const double s = ax < n ? sx[ex * p + ax] * sy[ey * p + ay] * sz[ez * p + az] : 0.0;
+        const double kz = 0.25 * hx[ex] * hy[ey] / hz[ez];  // 2J/hz^2, J = hx hy hz / 8
+        double* r = rec + e * REC;
+        r[SMALL + k] = s;
+        r[2 * SMALL + k] = kz * s;
+        if (k < 8) r[3 * SMALL + k] = k == 0 ? (hx[ex] * hx[ex]) / (hy[ey] * hy[ey]) : k == 1 ? (hz[ez] * hz[ez]) / (hx[ex] * hx[ex]) : 0.0;
+    }
 }
 
 // zero the six boundary faces of a node-major block (rows of B doubles)

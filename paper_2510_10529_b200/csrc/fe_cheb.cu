@@ -49,9 +49,8 @@ struct fe_mesh {
     double* d_sm = nullptr;          // N: mu_g M_gg^{-1/2} (0 on the Dirichlet boundary)
     double *d_hx = nullptr, *d_hy = nullptr, *d_hz = nullptr;
     double* d_WV = nullptr;  // cells*n^3: J w_q V_q
-    double* d_VZ = nullptr;  // cells*n*n*NP: V_q hz^2/2, [qx][qy][qz] rows padded to NP (TMA kernel)
+    double* d_VZ = nullptr;  // cells*REC: per-cell records of the TMA kernel (VZ | s_g | kz s_g | ky/kx, kx/kz)
     double *d_sx = nullptr, *d_sy = nullptr, *d_sz = nullptr;  // per-axis mu M^{-1/2}
-    double *d_gx = nullptr, *d_gy = nullptr, *d_gz = nullptr;  // per-axis cell geometry: h, h^2, 1/h^2, 1/h
     EOTab eoN, eoNT, eoG;    // even-odd halves of N' = diag(sqrt w) N, N'^T, G' = diag(w^-1/2) G diag(w^-1/2)
     bool have_V = false;
     int variant = 0;
@@ -76,7 +75,7 @@ static void make_eo(const double* M, int n, bool transpose, EOTab* T)
     }
 }
 
-static int small_tile(int n) { return n * n * (n + (n & 1)); }
+static int small_tile(int n) { return 3 * n * n * (n + (n & 1)) + 8; }  // REC of fe_apply_tma.cuh
 
 // Gauss weights folded into the 1-D tables (fe_apply_tma.cuh): N' = diag(sqrt w) N, G' = diag(w^-1/2) G diag(w^-1/2)
 static void build_folded_tables(fe_mesh* m)
@@ -161,10 +160,6 @@ int fe_mesh_create(const double* xe, int cx, const double* ye, int cy, const dou
         return code;
     };
     if ((rc = upload(&m->d_sx, s[0])) || (rc = upload(&m->d_sy, s[1])) || (rc = upload(&m->d_sz, s[2]))) return cleanup(rc);
-    std::vector<double> g[3];
-    for (int d = 0; d < 3; ++d)
-        for (double hv : h[d]) { g[d].push_back(hv); g[d].push_back(hv * hv); g[d].push_back(1.0 / (hv * hv)); g[d].push_back(1.0 / hv); }
-    if ((rc = upload(&m->d_gx, g[0])) || (rc = upload(&m->d_gy, g[1])) || (rc = upload(&m->d_gz, g[2]))) return cleanup(rc);
     if ((rc = upload(&m->d_hx, h[0])) || (rc = upload(&m->d_hy, h[1])) || (rc = upload(&m->d_hz, h[2]))) return cleanup(rc);
     cudaError_t ce = cudaMalloc((void**)&m->d_sm, (size_t)m->N * sizeof(double));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&m->d_WV, (size_t)m->ncells * m->nc * sizeof(double));
@@ -172,6 +167,8 @@ int fe_mesh_create(const double* xe, int cx, const double* ye, int cy, const dou
     if (ce != cudaSuccess) return cleanup(fail(FE_ERR_NOMEM, "fe_mesh_create: device allocation failed: %s", cudaGetErrorString(ce)));
     ce = cudaMemset(m->d_VZ, 0, (size_t)m->ncells * small_tile(m->n) * sizeof(double));
     if (ce != cudaSuccess) return cleanup(fail(FE_ERR_CUDA, "fe_mesh_create: memset failed: %s", cudaGetErrorString(ce)));
+    k_build_records<<<148 * 8, 256>>>(m->d_VZ, m->n, m->cx, m->cy, m->ncells, m->d_sx, m->d_sy, m->d_sz, m->d_hx, m->d_hy, m->d_hz);
+    m->launches += 1;
     launch_build_scaling(m->d_sx, m->d_sy, m->d_sz, m->Nx, m->Ny, m->Nz, m->d_sm, 0);
     m->launches += 1;
     ce = cudaDeviceSynchronize();
@@ -186,7 +183,6 @@ int fe_mesh_destroy(fe_mesh* m)
     if (!m) return FE_OK;
     cudaSetDevice(m->device);
     cudaFree(m->d_sm); cudaFree(m->d_hx); cudaFree(m->d_hy); cudaFree(m->d_hz); cudaFree(m->d_WV);
-    cudaFree(m->d_gx); cudaFree(m->d_gy); cudaFree(m->d_gz);
     cudaFree(m->d_VZ); cudaFree(m->d_sx); cudaFree(m->d_sy); cudaFree(m->d_sz);
     delete m;
     return FE_OK;
@@ -403,8 +399,7 @@ static bool tma_eligible(const fe_mesh* m, int B, const void* a, const void* b, 
 static void fill_tma_params(const fe_mesh* m, TmaParams* prm, int B)
 {
     memset(prm, 0, sizeof(*prm));
-    prm->VZ = m->d_VZ; prm->sx = m->d_sx; prm->sy = m->d_sy; prm->sz = m->d_sz;
-    prm->gx = m->d_gx; prm->gy = m->d_gy; prm->gz = m->d_gz;
+    prm->rec = m->d_VZ;
     prm->B = B; prm->cx = m->cx; prm->cy = m->cy; prm->cz = m->cz;
     prm->eoN = m->eoN; prm->eoNT = m->eoNT; prm->eoG = m->eoG;
 }
@@ -418,6 +413,10 @@ static int tma_step(fe_mesh* m, const BlockMaps& X, const BlockMaps& Y, const Bl
     prm.mXn = X.n3; prm.mYn1 = Y.n1; prm.mYp1 = Y.p1; prm.mWp1 = W ? W->p1 : Y.p1;
     prm.eps = eps; prm.alpha = alpha; prm.c = c; prm.owner = owner ? 1 : 0;
     prm.preinit = W ? 1 : 0; prm.beta_next = beta_next;
+    prm.eoNTa = m->eoNT;
+    for (double& x : prm.eoNTa.S) x *= alpha;
+    for (double& x : prm.eoNTa.A) x *= alpha;
+    for (double& x : prm.eoNTa.Mid) x *= alpha;
     cudaError_t e = launch_apply_tma(prm, m->p, m->ncells, first, st, m->variant, m->sms);
     if (e != cudaSuccess) return fail(FE_ERR_CUDA, "operator launch failed: %s", cudaGetErrorString(e));
     m->launches += 1;

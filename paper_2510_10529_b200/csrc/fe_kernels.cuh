@@ -61,7 +61,8 @@ inline void launch_build_scaling(const double* sx, const double* sy, const doubl
     k_build_scaling<<<148 * 8, 256, 0, st>>>(sx, sy, sz, Nx, Ny, Nz, sm);
 }
 
-// WV[e][q] = J_e w_qx w_qy w_qz V[e][q];  VZ[e][(qx*n+qy)*NP+qz] = V[e][q] hz^2/2 (TMA kernel; NP = n rounded up to even)
+// WV[e][q] = J_e w_qx w_qy w_qz V[e][q];  VZ = first tile of the cell record of the TMA kernel:
+// rec[e*REC + (qx*n+qy)*NP+qz] = V[e][q] hz^2/2, NP = n rounded up to even, REC = 3 n n NP + 8
 __global__ void k_weight_potential(const __grid_constant__ ApplyParams prm, int n, const double* __restrict__ V,
                                    double* __restrict__ WV, double* __restrict__ VZ, long long ncells)
 {
@@ -75,7 +76,7 @@ __global__ void k_weight_potential(const __grid_constant__ ApplyParams prm, int 
         int ex = (int)(e % prm.cx), ey = (int)((e / prm.cx) % prm.cy), ez = (int)(e / ((long long)prm.cx * prm.cy));
         double J = prm.hx[ex] * prm.hy[ey] * prm.hz[ez] * 0.125;
         WV[i] = J * prm.w[qx] * prm.w[qy] * prm.w[qz] * V[i];
-        VZ[e * (n * n * NP) + (qx * n + qy) * NP + qz] = 0.5 * prm.hz[ez] * prm.hz[ez] * V[i];
+        VZ[e * (3 * n * n * NP + 8) + (qx * n + qy) * NP + qz] = 0.5 * prm.hz[ez] * prm.hz[ez] * V[i];
     }
 }
 
