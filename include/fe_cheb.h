@@ -75,6 +75,15 @@ int fe_apply_H(fe_mesh* m, const double* X, double* Y, int B, const double* eps_
 int cheb_filter(fe_mesh* m, double* X, int B, int deg, double a, double b, double a0, double* work,
                 void* cuda_stream);
 
+/* Rayleigh-Ritz step of ChFSI in span(Y) (Eq. 23-24 l.210-219; R8: H~_Y = Y^T H~ Y; R9: the Cholesky of Y^T Y is
+ * done twice, CholQR2):  S = Y^T Y = L L^T, Q = Y L^{-T} (twice);  G = Q^T H~ Q;  G v = theta v;  Y <- Q V.
+ * Y: DEVICE, N*B doubles, in: filtered block (Dirichlet rows ignored), out: Ritz vectors (orthonormal columns, Ritz
+ * values ascending).  theta_host: HOST, B doubles.  work: DEVICE, N*B doubles, must not overlap Y.  1 <= B <= 128.
+ * The tall-skinny products (Gram matrices, rotations) and H~ Q run on the device; the B x B Cholesky and the
+ * symmetric eigenproblem run on the host.  SYNCHRONOUS: returns after cuda_stream has drained.
+ * FE_ERR_STATE if Y^T Y is not numerically positive definite. */
+int fe_rayleigh_ritz(fe_mesh* m, double* Y, int B, double* theta_host, double* work, void* cuda_stream);
+
 /* Kernel variant for experiments and tests: 0 = default (TMA generation when B is even and the blocks are 16-byte
  * aligned, else the legacy atomics kernel), 5 = same, 1..4 = legacy generations.  FE_ERR_INVALID if unknown. */
 int fe_set_variant(fe_mesh* m, int variant);

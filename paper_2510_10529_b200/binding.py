@@ -13,8 +13,8 @@ _lib = None
 EXPORTS = (
     "fe_mesh_create", "fe_mesh_destroy", "fe_num_nodes", "fe_num_free", "fe_num_cells", "fe_nodes_per_cell",
     "fe_quad_per_cell", "fe_get_l2g", "fe_get_node_coords", "fe_get_quad_coords", "fe_get_mass",
-    "fe_get_dirichlet_mask", "fe_set_potential", "fe_apply_H", "cheb_filter", "fe_set_variant", "fe_launch_count",
-    "fe_last_error",
+    "fe_get_dirichlet_mask", "fe_set_potential", "fe_apply_H", "cheb_filter", "fe_rayleigh_ritz", "fe_set_variant",
+    "fe_launch_count", "fe_last_error",
 )
 
 
@@ -51,6 +51,7 @@ def load_library():
     L.fe_apply_H.restype, L.fe_apply_H.argtypes = C.c_int, [vp, vp, vp, C.c_int, vp, vp]
     L.cheb_filter.restype = C.c_int
     L.cheb_filter.argtypes = [vp, vp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, vp, vp]
+    L.fe_rayleigh_ritz.restype, L.fe_rayleigh_ritz.argtypes = C.c_int, [vp, vp, C.c_int, vp, vp, vp]
     L.fe_set_variant.restype, L.fe_set_variant.argtypes = C.c_int, [vp, C.c_int]
     L.fe_last_error.restype, L.fe_last_error.argtypes = C.c_char_p, []
     _lib = L
@@ -174,6 +175,18 @@ def cheb_filter(h, X, m, a, b, a0, work, stream=None):
     return X
 
 
+def fe_rayleigh_ritz(h, Y, work, stream=None):
+    """Y (device, N x B) <- Ritz vectors in span(Y); returns the B Ritz values (numpy, ascending)."""
+    import numpy as np
+    if Y.dim() != 2 or Y.shape[0] != fe_num_nodes(h):
+        raise FEError(-1, "Y must be N x B")
+    B = Y.shape[1]
+    theta = np.empty(B, dtype=np.float64)
+    _check(load_library().fe_rayleigh_ritz(h, _dev_ptr(Y, "Y"), B, theta.ctypes.data_as(C.c_void_p),
+                                           _dev_ptr(work, "work", Y.numel()), _stream(stream)))
+    return theta
+
+
 def fe_set_variant(h, variant):
     _check(load_library().fe_set_variant(h, int(variant)))
 
@@ -223,6 +236,12 @@ class FEMesh:
         if work is None:
             work = torch.empty(2 * X.numel(), dtype=torch.float64, device=X.device)
         return cheb_filter(self.h, X, m, a, b, a0, work, stream)
+
+    def rayleigh_ritz(self, Y, work=None, stream=None):
+        import torch
+        if work is None:
+            work = torch.empty(Y.numel(), dtype=torch.float64, device=Y.device)
+        return fe_rayleigh_ritz(self.h, Y, work, stream)
 
     def set_variant(self, v):
         fe_set_variant(self.h, v)

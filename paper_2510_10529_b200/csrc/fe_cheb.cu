@@ -7,6 +7,7 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdint>
 #include <cstdarg>
@@ -16,6 +17,7 @@
 #include <vector>
 
 #include "fe_apply_tma.cuh"
+#include "fe_rr.cuh"
 #include "fe_kernels.cuh"
 #include "fe_tables.h"
 
@@ -54,6 +56,7 @@ struct fe_mesh {
     EOTab eoN, eoNT, eoG;    // even-odd halves of N' = diag(sqrt w) N, N'^T, G' = diag(w^-1/2) G diag(w^-1/2)
     bool have_V = false;
     int variant = 0;
+    double* d_small = nullptr;  // 2 * 128 * 128: B x B scratch of the Rayleigh-Ritz step
     int sms = 0;  // multiprocessors of the device (persistent grid size)
     int64_t launches = 0;
 };
@@ -183,6 +186,7 @@ int fe_mesh_destroy(fe_mesh* m)
     if (!m) return FE_OK;
     cudaSetDevice(m->device);
     cudaFree(m->d_sm); cudaFree(m->d_hx); cudaFree(m->d_hy); cudaFree(m->d_hz); cudaFree(m->d_WV);
+    cudaFree(m->d_small);
     cudaFree(m->d_VZ); cudaFree(m->d_sx); cudaFree(m->d_sy); cudaFree(m->d_sz);
     delete m;
     return FE_OK;
@@ -503,5 +507,137 @@ int cheb_filter(fe_mesh* m, double* X, int B, int deg, double a, double b, doubl
         sigma = sigma_next;
     }
     if (deg % 3 != 0) CUDA_TRY(cudaMemcpyAsync(X, buf[deg % 3], len * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    return FE_OK;
+}
+
+// ---- Rayleigh-Ritz (NEXT-1; Eq. 23-24 l.210-219; readings R8, R9) ------------------------------------------
+// small dense helpers on the host (B <= 128): Cholesky S = L L^T, R = L^{-T}, cyclic Jacobi for the symmetric B x B problem
+static bool chol_lower(std::vector<double>& S, int B)
+{
+    for (int j = 0; j < B; ++j) {
+        double d = S[(size_t)j * B + j];
+        for (int k = 0; k < j; ++k) d -= S[(size_t)j * B + k] * S[(size_t)j * B + k];
+        if (!(d > 0.0)) return false;
+        d = std::sqrt(d);
+        S[(size_t)j * B + j] = d;
+        for (int i = j + 1; i < B; ++i) {
+            double v = S[(size_t)i * B + j];
+            for (int k = 0; k < j; ++k) v -= S[(size_t)i * B + k] * S[(size_t)j * B + k];
+            S[(size_t)i * B + j] = v / d;
+        }
+    }
+    return true;
+}
+
+// R = L^{-T} (upper triangular, row-major R[i*B+j]) from the lower factor stored in the lower triangle of L
+static void inv_lower_transposed(const std::vector<double>& L, int B, std::vector<double>& R)
+{
+    std::vector<double> Li((size_t)B * B, 0.0);  // L^{-1}, lower
+    for (int c = 0; c < B; ++c) {
+        Li[(size_t)c * B + c] = 1.0 / L[(size_t)c * B + c];
+        for (int i = c + 1; i < B; ++i) {
+            double v = 0.0;
+            for (int k = c; k < i; ++k) v -= L[(size_t)i * B + k] * Li[(size_t)k * B + c];
+            Li[(size_t)i * B + c] = v / L[(size_t)i * B + i];
+        }
+    }
+    R.assign((size_t)B * B, 0.0);
+    for (int i = 0; i < B; ++i)
+        for (int j = i; j < B; ++j) R[(size_t)i * B + j] = Li[(size_t)j * B + i];
+}
+
+// eigenvalues ascending in w, eigenvectors in the COLUMNS of V (row-major V[i*B+k] = component i of vector k)
+static void jacobi_eigh(std::vector<double> G, int B, std::vector<double>& w, std::vector<double>& V)
+{
+    V.assign((size_t)B * B, 0.0);
+    for (int i = 0; i < B; ++i) V[(size_t)i * B + i] = 1.0;
+    for (int sweep = 0; sweep < 60; ++sweep) {
+        double off = 0.0, diag = 0.0;
+        for (int i = 0; i < B; ++i)
+            for (int j = 0; j < B; ++j) (i == j ? diag : off) += G[(size_t)i * B + j] * G[(size_t)i * B + j];
+        if (off <= 1e-32 * diag) break;
+        for (int p = 0; p < B - 1; ++p)
+            for (int q = p + 1; q < B; ++q) {
+                const double apq = G[(size_t)p * B + q];
+                if (apq == 0.0) continue;
+                const double theta = (G[(size_t)q * B + q] - G[(size_t)p * B + p]) / (2.0 * apq);
+                const double t = (theta >= 0 ? 1.0 : -1.0) / (std::fabs(theta) + std::sqrt(theta * theta + 1.0));
+                const double c = 1.0 / std::sqrt(t * t + 1.0), s = t * c;
+                for (int k = 0; k < B; ++k) {
+                    const double gkp = G[(size_t)k * B + p], gkq = G[(size_t)k * B + q];
+                    G[(size_t)k * B + p] = c * gkp - s * gkq;
+                    G[(size_t)k * B + q] = s * gkp + c * gkq;
+                }
+                for (int k = 0; k < B; ++k) {
+                    const double gpk = G[(size_t)p * B + k], gqk = G[(size_t)q * B + k];
+                    G[(size_t)p * B + k] = c * gpk - s * gqk;
+                    G[(size_t)q * B + k] = s * gpk + c * gqk;
+                }
+                for (int k = 0; k < B; ++k) {
+                    const double vkp = V[(size_t)k * B + p], vkq = V[(size_t)k * B + q];
+                    V[(size_t)k * B + p] = c * vkp - s * vkq;
+                    V[(size_t)k * B + q] = s * vkp + c * vkq;
+                }
+            }
+    }
+    std::vector<int> idx(B);
+    for (int i = 0; i < B; ++i) idx[i] = i;
+    std::sort(idx.begin(), idx.end(), [&](int a, int b) { return G[(size_t)a * B + a] < G[(size_t)b * B + b]; });
+    std::vector<double> Vs((size_t)B * B);
+    w.resize(B);
+    for (int k = 0; k < B; ++k) {
+        w[k] = G[(size_t)idx[k] * B + idx[k]];
+        for (int i = 0; i < B; ++i) Vs[(size_t)i * B + k] = V[(size_t)i * B + idx[k]];
+    }
+    V.swap(Vs);
+}
+
+// one CholQR pass: S = Y^T Y (device) -> L, R = L^{-T} (host) -> Y <- Y R (device)
+static int cholqr_pass(fe_mesh* m, double* Y, int B, cudaStream_t st)
+{
+    const size_t bb = (size_t)B * B;
+    CUDA_TRY(cudaMemsetAsync(m->d_small, 0, bb * sizeof(double), st));
+    CUDA_TRY(launch_gram(Y, Y, m->N, B, m->d_small, m->sms, st));
+    std::vector<double> S(bb), R;
+    CUDA_TRY(cudaMemcpyAsync(S.data(), m->d_small, bb * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    for (int i = 0; i < B; ++i)
+        for (int j = 0; j < i; ++j) S[(size_t)i * B + j] = S[(size_t)j * B + i] = 0.5 * (S[(size_t)i * B + j] + S[(size_t)j * B + i]);
+    if (!chol_lower(S, B)) return fail(FE_ERR_STATE, "fe_rayleigh_ritz: Y^T Y is not positive definite (rank-deficient block)");
+    inv_lower_transposed(S, B, R);
+    CUDA_TRY(cudaMemcpyAsync(m->d_small + bb, R.data(), bb * sizeof(double), cudaMemcpyHostToDevice, st));
+    CUDA_TRY(launch_rightmul(Y, m->d_small + bb, m->N, B, m->sms, st));
+    CUDA_TRY(cudaStreamSynchronize(st));  // R is a host temporary
+    m->launches += 2;
+    return FE_OK;
+}
+
+int fe_rayleigh_ritz(fe_mesh* m, double* Y, int B, double* theta_host, double* work, void* cuda_stream)
+{
+    if (!m || !Y || !theta_host || !work) return fail(FE_ERR_INVALID, "fe_rayleigh_ritz: NULL argument");
+    if (B < 1 || B > 128) return fail(FE_ERR_INVALID, "fe_rayleigh_ritz: B=%d outside 1..128", B);
+    if (!m->have_V) return fail(FE_ERR_STATE, "fe_rayleigh_ritz: call fe_set_potential first");
+    const size_t len = (size_t)m->N * B, bb = (size_t)B * B;
+    if (overlap(Y, len, work, len)) return fail(FE_ERR_INVALID, "fe_rayleigh_ritz: work overlaps Y");
+    CUDA_TRY(cudaSetDevice(m->device));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (!m->d_small) CUDA_TRY(cudaMalloc((void**)&m->d_small, 2 * 128 * 128 * sizeof(double)));
+    int rc;
+    if ((rc = zero_faces(m, Y, B, st))) return rc;                          // R5: Dirichlet rows do not take part
+    if ((rc = cholqr_pass(m, Y, B, st)) || (rc = cholqr_pass(m, Y, B, st))) return rc;  // R9: CholQR2, Y is now Q
+    if ((rc = fe_apply_H(m, Y, work, B, nullptr, cuda_stream))) return rc;  // H~ Q
+    CUDA_TRY(cudaMemsetAsync(m->d_small, 0, bb * sizeof(double), st));
+    CUDA_TRY(launch_gram(Y, work, m->N, B, m->d_small, m->sms, st));        // R8: H~_Y = Q^T H~ Q
+    std::vector<double> G(bb), w, V;
+    CUDA_TRY(cudaMemcpyAsync(G.data(), m->d_small, bb * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    for (int i = 0; i < B; ++i)
+        for (int j = 0; j < i; ++j) G[(size_t)i * B + j] = G[(size_t)j * B + i] = 0.5 * (G[(size_t)i * B + j] + G[(size_t)j * B + i]);
+    jacobi_eigh(G, B, w, V);
+    for (int k = 0; k < B; ++k) theta_host[k] = w[k];
+    CUDA_TRY(cudaMemcpyAsync(m->d_small + bb, V.data(), bb * sizeof(double), cudaMemcpyHostToDevice, st));
+    CUDA_TRY(launch_rightmul(Y, m->d_small + bb, m->N, B, m->sms, st));     // X = Q V
+    CUDA_TRY(cudaStreamSynchronize(st));
+    m->launches += 2;
     return FE_OK;
 }

@@ -209,6 +209,35 @@ def test_filter_reduced_config2_and_ritz_values():
         ag, a0g = theta_g[-1], theta_g[0]
 
 
+@pytest.mark.parametrize("p,B", [(2, 8), (4, 16), (3, 37), (2, 128)])
+def test_device_rayleigh_ritz(p, B):
+    """fe_rayleigh_ritz (NEXT-1: device Gram / rotation kernels, host B x B Cholesky and Jacobi) against the oracle's
+    Eq. 23-24: Ritz values <= 1e-9 (R16); vectors are compared through what is unique (R17): orthonormality, the
+    spanned subspace, and the Ritz residual relation Q^T H~ Q = diag(theta)."""
+    import oracle
+    w = workloads.reduced(2, 4)
+    om, gm = _pair((w.xe, w.ye, w.ze), p, w.V)
+    mask = om.mask()
+    free = mask.astype(bool)
+    Y = workloads.random_block(500 + p, om.N, B)  # garbage in the Dirichlet rows: must not take part
+    th_min, th_max, beta = oracle.lanczos_bounds(om, workloads.normal(3200 + p, om.N), 20)
+    b, a0 = th_max + beta, th_min
+    Yf = om.filter(Y * mask[:, None], 4, a0 + 0.1 * (b - a0), b, a0)  # mildly filtered block (conditioned, not orthogonal)
+    Yin = Yf.copy()
+    Yin[~free] = 3.25
+    theta_o, Xo, _ = oracle.rayleigh_ritz(om, Yf)
+    Xd = _dev(Yin)
+    theta_g = gm.rayleigh_ritz(Xd)
+    Xg = Xd.cpu().numpy()
+    assert np.max(np.abs(theta_g - theta_o) / np.maximum(1.0, np.abs(theta_o))) <= 1e-9
+    assert np.all(Xg[~free] == 0)
+    assert np.max(np.abs(Xg.T @ Xg - np.eye(B))) <= 1e-12
+    # same subspace: projecting the oracle's Ritz vectors onto span(Xg) loses nothing
+    assert np.linalg.norm(Xo - Xg @ (Xg.T @ Xo)) <= 1e-9 * np.linalg.norm(Xo)
+    G = Xg.T @ om.apply(Xg)
+    assert np.max(np.abs(G - np.diag(theta_g))) <= 1e-9 * max(1.0, np.max(np.abs(theta_g)))
+
+
 # ---- full BASELINE sizes: sampled rows ------------------------------------------------------------------------------
 def _sample_rows(w, count, seed):
     """Rows spread over cell interiors, faces, edges, vertices and the boundary."""
