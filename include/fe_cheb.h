@@ -84,6 +84,28 @@ int cheb_filter(fe_mesh* m, double* X, int B, int deg, double a, double b, doubl
  * FE_ERR_STATE if Y^T Y is not numerically positive definite. */
 int fe_rayleigh_ritz(fe_mesh* m, double* Y, int B, double* theta_host, double* work, void* cuda_stream);
 
+/* Block preconditioned MINRES for the adjoint systems (l.221-225):  (H~ - eps_j I) x_j = g_j  for j = 0..B-1 (Eq. 20,
+ * l.183), every column with its own Paige-Saunders recurrences, all columns advancing together so that a Krylov
+ * step is ONE fused fe_apply_H launch with per-column shifts.  Starts from x = 0; Dirichlet rows of G are ignored and
+ * those of X are 0.  When g_j is orthogonal to the null vectors of a singular (H~ - eps_j I), so is the Krylov space
+ * and the result is the component p_perp of l.223; the component along the null vectors (Eq. 8) is added with
+ * fe_add_subspace.  precondition != 0: inverse diagonal of the mass-scaled negative Laplacian
+ * 1/diag(M^{-1/2} (1/2 K) M^{-1/2}) (l.225, positive definite); 0: identity.
+ * A column stops when its (preconditioned) residual estimate phibar_j <= tol * beta1_j; the call stops when all have,
+ * or after maxit steps (checked every 8 steps: this call synchronises the stream).
+ * G: DEVICE N*B (read only); X: DEVICE N*B (out); eps_dev: DEVICE B doubles or NULL; work: DEVICE 6*N*B doubles;
+ * relres_host: HOST B doubles (phibar_j / beta1_j at exit) or NULL; iters_host: HOST int or NULL.  1 <= B <= 128. */
+int fe_minres_shifted(fe_mesh* m, const double* G, double* X, int B, const double* eps_dev, int maxit, double tol,
+                      int precondition, double* relres_host, int* iters_host, double* work, void* cuda_stream);
+
+/* C = A^T Bm (B x B, row-major, HOST) of two DEVICE N x B blocks: the tall-skinny Gram product of Eq. 23 (Y^T Y,
+ * Y^T H~ Y) and of the projections Psi^T P of the adjoint solve.  All N rows take part.  Synchronous. */
+int fe_gram(fe_mesh* m, const double* A, const double* Bm, int B, double* C_host, void* cuda_stream);
+
+/* P <- P + Psi D  (N x B block times a HOST B x B row-major matrix D): the completion p = p_perp + Psi~_k d_k of
+ * l.223.  Psi, P: DEVICE N*B, must not overlap.  Synchronous. */
+int fe_add_subspace(fe_mesh* m, const double* Psi, const double* D_host, double* P, int B, void* cuda_stream);
+
 /* Kernel variant for experiments and tests: 0 = default (TMA generation when B is even and the blocks are 16-byte
  * aligned, else the legacy atomics kernel), 5 = same, 1..4 = legacy generations.  FE_ERR_INVALID if unknown. */
 int fe_set_variant(fe_mesh* m, int variant);

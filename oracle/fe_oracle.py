@@ -1,5 +1,6 @@
 """ctypes face of oracle/fe_oracle.c plus the two harness-level algorithms that sit on top of the oracle's
-apply: 20-step Lanczos bounds (reading R10) and Rayleigh-Ritz (Eq. 23-24, l.210-219; readings R8, R9).
+apply: 20-step Lanczos bounds (reading R10), Rayleigh-Ritz (Eq. 23-24, l.210-219; readings R8, R9) and the
+preconditioned MINRES of the adjoint solve (l.221-225).
 
 TEST INFRASTRUCTURE: imported only by tests/, __graft_entry__.smoke() and bench.py's cpu_baseline legs.
 """
@@ -269,3 +270,74 @@ def rayleigh_ritz(mesh, Y, nthreads=1):
     G = 0.5 * (G + G.T)
     theta, V = np.linalg.eigh(G)
     return theta, Q @ V, Q
+
+
+def laplacian_precond(mesh):
+    """Inverse diagonal of the mass-scaled negative Laplacian, 1 / diag(M^{-1/2} (1/2 K) M^{-1/2}) on free rows and 0
+    on Dirichlet rows: the MINRES preconditioner of PAPER.md l.225.  Diagonal taken entry by entry from the cell
+    matrices of Eq. 17 with the potential switched off."""
+    l2g = mesh.l2g()
+    d = np.zeros(mesh.N)
+    for e in range(mesh.ncells):
+        Ke = mesh.cell_matrix(e, None, kin=0.5, pot=0.0)
+        np.add.at(d, l2g[e], np.diag(Ke))
+    mask = mesh.mask().astype(bool)
+    out = np.zeros(mesh.N)
+    out[mask] = mesh.mass()[mask] / d[mask]
+    return out
+
+
+def minres_shifted(mesh, G, eps=None, maxit=200, tol=1e-10, Minv=None, nthreads=1):
+    """Preconditioned MINRES (Paige & Saunders 1975, the method PAPER.md l.223-225 names, ref. [59]) for
+    (H~ - eps_j I) x_j = g_j, column by column, x_0 = 0, on the free rows.  Minv: diagonal preconditioner (N) or None.
+    A column stops when phibar <= tol * beta1 (estimate of the preconditioned residual norm).
+    Returns (X, phibar / beta1, iterations of the slowest column)."""
+    G = _f64(G)
+    N, B = G.shape
+    mask = mesh.mask().astype(np.float64)
+    Mi = mask if Minv is None else _f64(Minv) * mask
+    X = np.zeros((N, B))
+    rel = np.zeros(B)
+    itmax = 0
+    for j in range(B):
+        ej = None if eps is None else np.array([eps[j]])
+        b = G[:, j] * mask
+        r1 = b.copy()
+        y = Mi * r1
+        beta1 = np.sqrt(max(r1 @ y, 0.0))
+        if beta1 == 0.0:
+            continue
+        oldb, beta, dbar, epsln, phibar = 0.0, beta1, 0.0, 0.0, beta1
+        cs, sn = -1.0, 0.0
+        w = np.zeros(N)
+        w2 = np.zeros(N)
+        r2 = r1.copy()
+        x = np.zeros(N)
+        itn = 0
+        while itn < maxit and phibar > tol * beta1 and beta > 0.0:
+            itn += 1
+            v = y / beta
+            y = mesh.apply(v[:, None], ej, nthreads=nthreads)[:, 0]
+            if itn >= 2:
+                y = y - (beta / oldb) * r1
+            alfa = v @ y
+            y = y - (alfa / beta) * r2
+            r1, r2 = r2, y
+            y = Mi * r2
+            oldb, beta = beta, np.sqrt(max(r2 @ y, 0.0))
+            oldeps = epsln
+            delta = cs * dbar + sn * alfa
+            gbar = sn * dbar - cs * alfa
+            epsln = sn * beta
+            dbar = -cs * beta
+            gamma = max(np.hypot(gbar, beta), np.finfo(float).eps)
+            cs, sn = gbar / gamma, beta / gamma
+            phi = cs * phibar
+            phibar = sn * phibar
+            w1, w2 = w2, w
+            w = (v - oldeps * w1 - delta * w2) / gamma
+            x = x + phi * w
+        X[:, j] = x
+        rel[j] = phibar / beta1
+        itmax = max(itmax, itn)
+    return X, rel, itmax

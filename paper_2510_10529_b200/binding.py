@@ -13,7 +13,8 @@ _lib = None
 EXPORTS = (
     "fe_mesh_create", "fe_mesh_destroy", "fe_num_nodes", "fe_num_free", "fe_num_cells", "fe_nodes_per_cell",
     "fe_quad_per_cell", "fe_get_l2g", "fe_get_node_coords", "fe_get_quad_coords", "fe_get_mass",
-    "fe_get_dirichlet_mask", "fe_set_potential", "fe_apply_H", "cheb_filter", "fe_rayleigh_ritz", "fe_set_variant",
+    "fe_get_dirichlet_mask", "fe_set_potential", "fe_apply_H", "cheb_filter", "fe_rayleigh_ritz", "fe_minres_shifted", "fe_add_subspace", "fe_gram",
+    "fe_set_variant",
     "fe_launch_count", "fe_last_error",
 )
 
@@ -52,6 +53,10 @@ def load_library():
     L.cheb_filter.restype = C.c_int
     L.cheb_filter.argtypes = [vp, vp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, vp, vp]
     L.fe_rayleigh_ritz.restype, L.fe_rayleigh_ritz.argtypes = C.c_int, [vp, vp, C.c_int, vp, vp, vp]
+    L.fe_minres_shifted.restype = C.c_int
+    L.fe_minres_shifted.argtypes = [vp, vp, vp, C.c_int, vp, C.c_int, C.c_double, C.c_int, vp, vp, vp, vp]
+    L.fe_gram.restype, L.fe_gram.argtypes = C.c_int, [vp, vp, vp, C.c_int, vp, vp]
+    L.fe_add_subspace.restype, L.fe_add_subspace.argtypes = C.c_int, [vp, vp, vp, vp, C.c_int, vp]
     L.fe_set_variant.restype, L.fe_set_variant.argtypes = C.c_int, [vp, C.c_int]
     L.fe_last_error.restype, L.fe_last_error.argtypes = C.c_char_p, []
     _lib = L
@@ -187,6 +192,42 @@ def fe_rayleigh_ritz(h, Y, work, stream=None):
     return theta
 
 
+def fe_minres_shifted(h, G, X, eps, maxit, tol, precondition, work, stream=None):
+    """Returns (relres (numpy, B), iterations)."""
+    import numpy as np
+    if G.dim() != 2 or G.shape[0] != fe_num_nodes(h):
+        raise FEError(-1, "G must be N x B")
+    B = G.shape[1]
+    relres = np.empty(B, dtype=np.float64)
+    iters = C.c_int(0)
+    ep = _dev_ptr(eps, "eps", B) if eps is not None else None
+    _check(load_library().fe_minres_shifted(h, _dev_ptr(G, "G"), _dev_ptr(X, "X", G.numel()), B, ep, int(maxit),
+                                            float(tol), int(bool(precondition)), relres.ctypes.data_as(C.c_void_p),
+                                            C.byref(iters), _dev_ptr(work, "work", 6 * G.numel()), _stream(stream)))
+    return relres, iters.value
+
+
+def fe_gram(h, A, Bm, stream=None):
+    """A^T Bm as a numpy B x B array."""
+    import numpy as np
+    B = A.shape[1]
+    out = np.empty((B, B), dtype=np.float64)
+    _check(load_library().fe_gram(h, _dev_ptr(A, "A"), _dev_ptr(Bm, "Bm", A.numel()), B,
+                                  out.ctypes.data_as(C.c_void_p), _stream(stream)))
+    return out
+
+
+def fe_add_subspace(h, Psi, D, P, stream=None):
+    import numpy as np
+    B = Psi.shape[1]
+    Dh = np.ascontiguousarray(D, dtype=np.float64)
+    if Dh.shape != (B, B):
+        raise FEError(-1, "D must be B x B")
+    _check(load_library().fe_add_subspace(h, _dev_ptr(Psi, "Psi"), Dh.ctypes.data_as(C.c_void_p),
+                                          _dev_ptr(P, "P", Psi.numel()), B, _stream(stream)))
+    return P
+
+
 def fe_set_variant(h, variant):
     _check(load_library().fe_set_variant(h, int(variant)))
 
@@ -242,6 +283,19 @@ class FEMesh:
         if work is None:
             work = torch.empty(Y.numel(), dtype=torch.float64, device=Y.device)
         return fe_rayleigh_ritz(self.h, Y, work, stream)
+
+    def minres_shifted(self, G, eps=None, maxit=200, tol=1e-10, precondition=True, stream=None):
+        import torch
+        X = torch.empty_like(G)
+        work = torch.empty(6 * G.numel(), dtype=torch.float64, device=G.device)
+        relres, iters = fe_minres_shifted(self.h, G, X, eps, maxit, tol, precondition, work, stream)
+        return X, relres, iters
+
+    def gram(self, A, Bm, stream=None):
+        return fe_gram(self.h, A, Bm, stream)
+
+    def add_subspace(self, Psi, D, P, stream=None):
+        return fe_add_subspace(self.h, Psi, D, P, stream)
 
     def set_variant(self, v):
         fe_set_variant(self.h, v)

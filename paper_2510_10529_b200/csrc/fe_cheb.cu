@@ -17,6 +17,7 @@
 #include <vector>
 
 #include "fe_apply_tma.cuh"
+#include "fe_minres.cuh"
 #include "fe_rr.cuh"
 #include "fe_kernels.cuh"
 #include "fe_tables.h"
@@ -56,6 +57,9 @@ struct fe_mesh {
     EOTab eoN, eoNT, eoG;    // even-odd halves of N' = diag(sqrt w) N, N'^T, G' = diag(w^-1/2) G diag(w^-1/2)
     bool have_V = false;
     int variant = 0;
+    double* d_minv = nullptr;   // N: MINRES preconditioner, 1 / diag(M^{-1/2} 1/2 K M^{-1/2}) on free rows (built on first use)
+    double* d_mask = nullptr;   // N: 1 on free rows, 0 on Dirichlet rows (the unpreconditioned MINRES)
+    double* d_scal = nullptr;   // 17 * 128 doubles + 1 int: MINRES column scalars
     double* d_small = nullptr;  // 2 * 128 * 128: B x B scratch of the Rayleigh-Ritz step
     int sms = 0;  // multiprocessors of the device (persistent grid size)
     int64_t launches = 0;
@@ -186,7 +190,7 @@ int fe_mesh_destroy(fe_mesh* m)
     if (!m) return FE_OK;
     cudaSetDevice(m->device);
     cudaFree(m->d_sm); cudaFree(m->d_hx); cudaFree(m->d_hy); cudaFree(m->d_hz); cudaFree(m->d_WV);
-    cudaFree(m->d_small);
+    cudaFree(m->d_small); cudaFree(m->d_minv); cudaFree(m->d_mask); cudaFree(m->d_scal);
     cudaFree(m->d_VZ); cudaFree(m->d_sx); cudaFree(m->d_sy); cudaFree(m->d_sz);
     delete m;
     return FE_OK;
@@ -606,7 +610,7 @@ static int cholqr_pass(fe_mesh* m, double* Y, int B, cudaStream_t st)
     if (!chol_lower(S, B)) return fail(FE_ERR_STATE, "fe_rayleigh_ritz: Y^T Y is not positive definite (rank-deficient block)");
     inv_lower_transposed(S, B, R);
     CUDA_TRY(cudaMemcpyAsync(m->d_small + bb, R.data(), bb * sizeof(double), cudaMemcpyHostToDevice, st));
-    CUDA_TRY(launch_rightmul(Y, m->d_small + bb, m->N, B, m->sms, st));
+    CUDA_TRY(launch_rightmul(Y, m->d_small + bb, Y, 0, m->N, B, m->sms, st));
     CUDA_TRY(cudaStreamSynchronize(st));  // R is a host temporary
     m->launches += 2;
     return FE_OK;
@@ -636,8 +640,157 @@ int fe_rayleigh_ritz(fe_mesh* m, double* Y, int B, double* theta_host, double* w
     jacobi_eigh(G, B, w, V);
     for (int k = 0; k < B; ++k) theta_host[k] = w[k];
     CUDA_TRY(cudaMemcpyAsync(m->d_small + bb, V.data(), bb * sizeof(double), cudaMemcpyHostToDevice, st));
-    CUDA_TRY(launch_rightmul(Y, m->d_small + bb, m->N, B, m->sms, st));     // X = Q V
+    CUDA_TRY(launch_rightmul(Y, m->d_small + bb, Y, 0, m->N, B, m->sms, st));     // X = Q V
     CUDA_TRY(cudaStreamSynchronize(st));
     m->launches += 2;
+    return FE_OK;
+}
+
+// ---- block preconditioned MINRES around the shifted apply (NEXT-2; Eq. 20 l.183) ----------------
+// per-axis diagonals of the Gauss-quadrature 1-D stiffness (2/h) N^T G N and mass (h/2) N^T W N, assembled over cells
+static void axis_diagonals(const fe_mesh* m, const std::vector<double>& e, int c, std::vector<double>& kd, std::vector<double>& md)
+{
+    const int n = m->n, p = m->p;
+    std::vector<double> kh(n, 0.0), mh(n, 0.0);
+    for (int a = 0; a < n; ++a)
+        for (int q = 0; q < n; ++q) {
+            mh[a] += m->tab.gl_w[q] * m->tab.N[q * n + a] * m->tab.N[q * n + a];
+            for (int r = 0; r < n; ++r) kh[a] += m->tab.N[q * n + a] * m->tab.G[q * n + r] * m->tab.N[r * n + a];
+        }
+    kd.assign((size_t)c * p + 1, 0.0);
+    md.assign((size_t)c * p + 1, 0.0);
+    for (int ec = 0; ec < c; ++ec) {
+        const double h = e[ec + 1] - e[ec];
+        for (int a = 0; a < n; ++a) {
+            kd[(size_t)ec * p + a] += 2.0 / h * kh[a];
+            md[(size_t)ec * p + a] += 0.5 * h * mh[a];
+        }
+    }
+}
+
+__global__ void k_nonzero_to_one(double* __restrict__ a, long long n)
+{
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        a[i] = a[i] != 0.0 ? 1.0 : 0.0;
+}
+
+static int ensure_minres_tables(fe_mesh* m)
+{
+    if (m->d_minv) return FE_OK;
+    std::vector<double> k[3], md[3];
+    axis_diagonals(m, m->xe, m->cx, k[0], md[0]);
+    axis_diagonals(m, m->ye, m->cy, k[1], md[1]);
+    axis_diagonals(m, m->ze, m->cz, k[2], md[2]);
+    double* d[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    int rc = FE_OK;
+    for (int i = 0; i < 3 && !rc; ++i) {
+        rc = upload(&d[i], k[i]);
+        if (!rc) rc = upload(&d[3 + i], md[i]);
+    }
+    cudaError_t ce = cudaSuccess;
+    if (!rc) ce = cudaMalloc((void**)&m->d_minv, (size_t)m->N * sizeof(double));
+    if (!rc && ce == cudaSuccess) ce = cudaMalloc((void**)&m->d_mask, (size_t)m->N * sizeof(double));
+    if (!rc && ce == cudaSuccess) ce = cudaMalloc((void**)&m->d_scal, (17 * 128 + 2) * sizeof(double));
+    if (!rc && ce == cudaSuccess) {
+        k_build_precond<<<148 * 8, 256>>>(m->d_minv, m->Nx, m->Ny, m->Nz, d[0], d[1], d[2], d[3], d[4], d[5], m->d_sx, m->d_sy, m->d_sz);
+        k_build_scaling<<<148 * 8, 256>>>(m->d_sx, m->d_sy, m->d_sz, m->Nx, m->Ny, m->Nz, m->d_mask);
+        k_nonzero_to_one<<<148 * 4, 256>>>(m->d_mask, m->N);  // mu M^{-1/2} -> {0, 1}
+        ce = cudaDeviceSynchronize();
+        m->launches += 2;
+    }
+    for (double* q : d) cudaFree(q);
+    if (rc) return rc;
+    if (ce != cudaSuccess) return fail(FE_ERR_CUDA, "fe_minres_shifted: building the preconditioner failed: %s", cudaGetErrorString(ce));
+    return FE_OK;
+}
+
+int fe_minres_shifted(fe_mesh* m, const double* G, double* X, int B, const double* eps_dev, int maxit, double tol,
+                      int precondition, double* relres_host, int* iters_host, double* work, void* cuda_stream)
+{
+    if (!m || !G || !X || !work) return fail(FE_ERR_INVALID, "fe_minres_shifted: NULL argument");
+    if (B < 1 || B > 128) return fail(FE_ERR_INVALID, "fe_minres_shifted: B=%d outside 1..128", B);
+    if (maxit < 1 || !(tol >= 0.0)) return fail(FE_ERR_INVALID, "fe_minres_shifted: need maxit >= 1 and tol >= 0");
+    if (!m->have_V) return fail(FE_ERR_STATE, "fe_minres_shifted: call fe_set_potential first");
+    const size_t len = (size_t)m->N * B;
+    if (overlap(X, len, work, 6 * len) || overlap(G, len, work, 6 * len) || overlap(G, len, X, len))
+        return fail(FE_ERR_INVALID, "fe_minres_shifted: G, X and work must not overlap");
+    CUDA_TRY(cudaSetDevice(m->device));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int rc = ensure_minres_tables(m);
+    if (rc) return rc;
+    const double* Minv = precondition ? m->d_minv : m->d_mask;
+    double *R1 = work, *R2 = work + len, *Y = work + 2 * len, *V = work + 3 * len, *W1 = work + 4 * len, *W2 = work + 5 * len;
+    MinresScalars q;
+    double* s = m->d_scal;
+    double** f[] = {&q.beta, &q.oldb, &q.alfa, &q.betasq, &q.dbar, &q.epsln, &q.oldeps, &q.phibar, &q.cs, &q.sn,
+                    &q.gamma, &q.delta, &q.phi, &q.beta1, &q.s, &q.c1, &q.c2};
+    for (int i = 0; i < 17; ++i) *f[i] = s + (size_t)i * 128;
+    q.itn = (int*)(s + 17 * 128);
+    const int grid = m->sms * 8;
+    const dim3 blk(kMRx, kMRy);
+    CUDA_TRY(cudaMemsetAsync(q.betasq, 0, 128 * sizeof(double), st));
+    k_minres_init<<<grid, blk, 0, st>>>(G, Minv, R1, R2, Y, X, W1, W2, m->N, B, q.betasq);
+    k_minres_scalars<<<1, 128, 0, st>>>(q, B, 0, tol);
+    m->launches += 3;
+    std::vector<double> phibar(B), beta1(B);
+    int it = 0;
+    bool done = false;
+    while (it < maxit && !done) {
+        k_minres_scalars<<<1, 128, 0, st>>>(q, B, 1, tol);
+        k_minres_scale<<<grid, blk, 0, st>>>(Y, V, m->N, B, q.s);
+        if ((rc = fe_apply_H(m, V, Y, B, eps_dev, cuda_stream))) return rc;  // y = (H~ - eps_j) v
+        k_minres_alfa<<<grid, blk, 0, st>>>(Y, R1, V, m->N, B, q.c1, q.alfa);
+        k_minres_beta<<<grid, blk, 0, st>>>(Y, R1, R2, Minv, m->N, B, q.alfa, q.beta, q.betasq);
+        k_minres_scalars<<<1, 128, 0, st>>>(q, B, 2, tol);
+        k_minres_update<<<grid, blk, 0, st>>>(V, W1, W2, X, m->N, B, q.oldeps, q.delta, q.gamma, q.phi);
+        CUDA_TRY(cudaGetLastError());
+        m->launches += 6;
+        std::swap(R1, R2);
+        std::swap(W1, W2);
+        ++it;
+        if (it % 8 == 0 || it == maxit) {
+            CUDA_TRY(cudaMemcpyAsync(phibar.data(), q.phibar, B * sizeof(double), cudaMemcpyDeviceToHost, st));
+            CUDA_TRY(cudaMemcpyAsync(beta1.data(), q.beta1, B * sizeof(double), cudaMemcpyDeviceToHost, st));
+            CUDA_TRY(cudaStreamSynchronize(st));
+            done = true;
+            for (int j = 0; j < B; ++j)
+                if (beta1[j] > 0.0 && phibar[j] > tol * beta1[j]) done = false;
+        }
+    }
+    if (relres_host)
+        for (int j = 0; j < B; ++j) relres_host[j] = beta1[j] > 0.0 ? phibar[j] / beta1[j] : 0.0;
+    if (iters_host) *iters_host = it;
+    return FE_OK;
+}
+
+int fe_add_subspace(fe_mesh* m, const double* Psi, const double* D_host, double* P, int B, void* cuda_stream)
+{
+    if (!m || !Psi || !D_host || !P) return fail(FE_ERR_INVALID, "fe_add_subspace: NULL argument");
+    if (B < 1 || B > 128) return fail(FE_ERR_INVALID, "fe_add_subspace: B=%d outside 1..128", B);
+    const size_t len = (size_t)m->N * B, bb = (size_t)B * B;
+    if (overlap(Psi, len, P, len)) return fail(FE_ERR_INVALID, "fe_add_subspace: Psi and P overlap");
+    CUDA_TRY(cudaSetDevice(m->device));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (!m->d_small) CUDA_TRY(cudaMalloc((void**)&m->d_small, 2 * 128 * 128 * sizeof(double)));
+    CUDA_TRY(cudaMemcpyAsync(m->d_small + bb, D_host, bb * sizeof(double), cudaMemcpyHostToDevice, st));
+    CUDA_TRY(launch_rightmul(Psi, m->d_small + bb, P, 1, m->N, B, m->sms, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    m->launches += 1;
+    return FE_OK;
+}
+
+int fe_gram(fe_mesh* m, const double* A, const double* Bm, int B, double* C_host, void* cuda_stream)
+{
+    if (!m || !A || !Bm || !C_host) return fail(FE_ERR_INVALID, "fe_gram: NULL argument");
+    if (B < 1 || B > 128) return fail(FE_ERR_INVALID, "fe_gram: B=%d outside 1..128", B);
+    CUDA_TRY(cudaSetDevice(m->device));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t bb = (size_t)B * B;
+    if (!m->d_small) CUDA_TRY(cudaMalloc((void**)&m->d_small, 2 * 128 * 128 * sizeof(double)));
+    CUDA_TRY(cudaMemsetAsync(m->d_small, 0, bb * sizeof(double), st));
+    CUDA_TRY(launch_gram(A, Bm, m->N, B, m->d_small, m->sms, st));
+    CUDA_TRY(cudaMemcpyAsync(C_host, m->d_small, bb * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    m->launches += 1;
     return FE_OK;
 }

@@ -1,0 +1,197 @@
+// fe_minres.cuh -- block preconditioned MINRES around the shifted apply (NEXT-2; Eq. 20 l.183)
+//
+// Every column j solves its own system (H~ - eps_j I) p_j = g_j with its own Paige-Saunders recurrences; the
+// columns advance in lock-step so that each Krylov step is ONE fused fe_apply_H launch for the whole block.  The
+// vector updates of a step are three fused elementwise kernels that also produce the column-wise inner products
+// (alfa_j = v_j.y_j, beta_j^2 = r_j.M^{-1} r_j); the Givens / Lanczos scalars live in device arrays of length B
+// and are advanced by a one-warp-per-block kernel, so an iteration needs no host synchronisation.
+// Preconditioner (l.225): inverse diagonal of the mass-scaled negative Laplacian, positive on free rows.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace fecheb {
+
+struct MinresScalars {  // B doubles each, device
+    double *beta, *oldb, *alfa, *betasq, *dbar, *epsln, *oldeps, *phibar, *cs, *sn, *gamma, *delta, *phi, *beta1;
+    double *s, *c1, *c2;  // 1/beta, beta/oldb, alfa/beta of the running step
+    int* itn;
+};
+
+constexpr int kMRx = 32, kMRy = 8, kMaxColTiles = 4;  // B <= 128
+
+// column-wise partial sums of a thread block -> atomicAdd into out[j]
+__device__ __forceinline__ void block_col_reduce(double (&acc)[kMaxColTiles], int B, double* out)
+{
+    __shared__ double red[kMRy][kMRx];
+#pragma unroll
+    for (int t = 0; t < kMaxColTiles; ++t) {
+        const int j = t * kMRx + threadIdx.x;
+        if (t * kMRx >= B) break;
+        red[threadIdx.y][threadIdx.x] = acc[t];
+        __syncthreads();
+        if (threadIdx.y == 0 && j < B) {
+            double sum = 0.0;
+#pragma unroll
+            for (int y = 0; y < kMRy; ++y) sum += red[y][threadIdx.x];
+            atomicAdd(out + j, sum);
+        }
+        __syncthreads();
+    }
+}
+
+// phase 0 (start):  r1 = r2 = g (masked); y = Minv r; betasq = r.y; x = w = w2 = 0
+__global__ void k_minres_init(const double* __restrict__ G, const double* __restrict__ Minv, double* __restrict__ R1,
+                              double* __restrict__ R2, double* __restrict__ Y, double* __restrict__ X,
+                              double* __restrict__ W, double* __restrict__ W2, long long N, int B, double* betasq)
+{
+    double acc[kMaxColTiles] = {0, 0, 0, 0};
+    for (long long r = blockIdx.x * (long long)kMRy + threadIdx.y; r < N; r += (long long)gridDim.x * kMRy) {
+        const double mi = Minv[r];
+#pragma unroll
+        for (int t = 0; t < kMaxColTiles; ++t) {
+            const int j = t * kMRx + threadIdx.x;
+            if (j < B) {
+                const long long i = r * B + j;
+                const double g = mi != 0.0 ? G[i] : 0.0;  // Dirichlet rows do not take part (R5)
+                const double y = mi * g;
+                R1[i] = g; R2[i] = g; Y[i] = y; X[i] = 0.0; W[i] = 0.0; W2[i] = 0.0;
+                acc[t] = fma(g, y, acc[t]);
+            }
+        }
+    }
+    block_col_reduce(acc, B, betasq);
+}
+
+// phase A:  v = s_j y   (v overwrites y's old role through the pointer rotation done by the host)
+__global__ void k_minres_scale(const double* __restrict__ Y, double* __restrict__ V, long long N, int B,
+                               const double* __restrict__ s)
+{
+    for (long long r = blockIdx.x * (long long)kMRy + threadIdx.y; r < N; r += (long long)gridDim.x * kMRy)
+#pragma unroll
+        for (int t = 0; t < kMaxColTiles; ++t) {
+            const int j = t * kMRx + threadIdx.x;
+            if (j < B) V[r * B + j] = s[j] * Y[r * B + j];
+        }
+}
+
+// phase B:  y <- y - c1_j r1 ;  alfa_j = v_j . y_j
+__global__ void k_minres_alfa(double* __restrict__ Y, const double* __restrict__ R1, const double* __restrict__ V,
+                              long long N, int B, const double* __restrict__ c1, double* alfa)
+{
+    double acc[kMaxColTiles] = {0, 0, 0, 0};
+    for (long long r = blockIdx.x * (long long)kMRy + threadIdx.y; r < N; r += (long long)gridDim.x * kMRy)
+#pragma unroll
+        for (int t = 0; t < kMaxColTiles; ++t) {
+            const int j = t * kMRx + threadIdx.x;
+            if (j < B) {
+                const long long i = r * B + j;
+                const double y = fma(-c1[j], R1[i], Y[i]);
+                Y[i] = y;
+                acc[t] = fma(V[i], y, acc[t]);
+            }
+        }
+    block_col_reduce(acc, B, alfa);
+}
+
+// phase C:  t = y - c2_j r2 ;  r1 <- t (the host swaps r1/r2 afterwards) ;  y <- Minv t ;  betasq_j = t_j . y_j
+__global__ void k_minres_beta(double* __restrict__ Y, double* __restrict__ R1, const double* __restrict__ R2,
+                              const double* __restrict__ Minv, long long N, int B, const double* __restrict__ alfa,
+                              const double* __restrict__ beta, double* betasq)
+{
+    double acc[kMaxColTiles] = {0, 0, 0, 0};
+    for (long long r = blockIdx.x * (long long)kMRy + threadIdx.y; r < N; r += (long long)gridDim.x * kMRy) {
+        const double mi = Minv[r];
+#pragma unroll
+        for (int t = 0; t < kMaxColTiles; ++t) {
+            const int j = t * kMRx + threadIdx.x;
+            if (j < B) {
+                const long long i = r * B + j;
+                const double c2 = beta[j] > 0.0 ? alfa[j] / beta[j] : 0.0;
+                const double tt = fma(-c2, R2[i], Y[i]);
+                const double y = mi * tt;
+                R1[i] = tt;
+                Y[i] = y;
+                acc[t] = fma(tt, y, acc[t]);
+            }
+        }
+    }
+    block_col_reduce(acc, B, betasq);
+}
+
+// phase D:  w_new = (v - oldeps_j w1 - delta_j w2) / gamma_j  (into w1's storage) ;  x += phi_j w_new
+__global__ void k_minres_update(const double* __restrict__ V, double* __restrict__ W1, const double* __restrict__ W2,
+                                double* __restrict__ X, long long N, int B, const double* __restrict__ oldeps,
+                                const double* __restrict__ delta, const double* __restrict__ gamma,
+                                const double* __restrict__ phi)
+{
+    for (long long r = blockIdx.x * (long long)kMRy + threadIdx.y; r < N; r += (long long)gridDim.x * kMRy)
+#pragma unroll
+        for (int t = 0; t < kMaxColTiles; ++t) {
+            const int j = t * kMRx + threadIdx.x;
+            if (j < B) {
+                const long long i = r * B + j;
+                const double w = (V[i] - oldeps[j] * W1[i] - delta[j] * W2[i]) / gamma[j];
+                W1[i] = w;
+                X[i] = fma(phi[j], w, X[i]);
+            }
+        }
+}
+
+// scalar recurrences, one thread per column.  stage 0: after init (beta1); stage 1: before the step (s, c1);
+// stage 2: after phase C (Lanczos beta, Givens rotation, phi)
+__global__ void k_minres_scalars(MinresScalars q, int B, int stage, double tol)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= B) return;
+    if (stage == 0) {
+        const double b1 = sqrt(fmax(q.betasq[j], 0.0));
+        q.beta1[j] = b1; q.beta[j] = b1; q.oldb[j] = 0.0; q.dbar[j] = 0.0; q.epsln[j] = 0.0; q.phibar[j] = b1;
+        q.cs[j] = -1.0; q.sn[j] = 0.0; q.betasq[j] = 0.0; q.alfa[j] = 0.0;
+        q.gamma[j] = 1.0; q.delta[j] = 0.0; q.oldeps[j] = 0.0; q.phi[j] = 0.0;
+        if (j == 0) *q.itn = 0;
+    } else if (stage == 1) {
+        const double beta = q.beta[j], oldb = q.oldb[j];
+        const bool live = beta > 0.0 && q.phibar[j] > tol * q.beta1[j];  // a converged column stops moving
+        q.s[j] = live ? 1.0 / beta : 0.0;
+        q.c1[j] = (live && oldb > 0.0) ? beta / oldb : 0.0;
+        q.alfa[j] = 0.0;
+        q.betasq[j] = 0.0;
+    } else {
+        const bool live = q.s[j] != 0.0;
+        const double alfa = q.alfa[j], oldb = q.beta[j];
+        const double beta = sqrt(fmax(q.betasq[j], 0.0));
+        if (!live) { q.phi[j] = 0.0; q.gamma[j] = 1.0; q.delta[j] = 0.0; q.oldeps[j] = 0.0; return; }
+        const double cs = q.cs[j], sn = q.sn[j], dbar = q.dbar[j];
+        const double oldeps = q.epsln[j];
+        const double delta = cs * dbar + sn * alfa;
+        const double gbar = sn * dbar - cs * alfa;
+        const double epsln = sn * beta;
+        const double dbar2 = -cs * beta;
+        const double gamma = fmax(sqrt(gbar * gbar + beta * beta), 2.220446049250313e-16);
+        const double cs2 = gbar / gamma, sn2 = beta / gamma;
+        q.phi[j] = cs2 * q.phibar[j];
+        q.phibar[j] = sn2 * q.phibar[j];
+        q.oldeps[j] = oldeps; q.delta[j] = delta; q.gamma[j] = gamma; q.epsln[j] = epsln; q.dbar[j] = dbar2;
+        q.cs[j] = cs2; q.sn[j] = sn2; q.oldb[j] = oldb; q.beta[j] = beta;
+        if (j == 0) *q.itn += 1;
+    }
+}
+
+// Minv[g] = s_g^2 / diag(1/2 K)_g on free rows (0 on Dirichlet rows): inverse diagonal of the mass-scaled negative
+// Laplacian, from per-axis diagonals: diag(1/2 K) = 1/2 (kx my mz + mx ky mz + mx my kz) with the Gauss-quadrature
+// 1-D stiffness / mass diagonals k?, m?;  s? = per-axis mu M^{-1/2}
+__global__ void k_build_precond(double* __restrict__ Minv, long long Nx, long long Ny, long long Nz,
+                                const double* __restrict__ kx, const double* __restrict__ ky, const double* __restrict__ kz,
+                                const double* __restrict__ mx, const double* __restrict__ my, const double* __restrict__ mz,
+                                const double* __restrict__ sx, const double* __restrict__ sy, const double* __restrict__ sz)
+{
+    const long long total = Nx * Ny * Nz;
+    for (long long g = blockIdx.x * (long long)blockDim.x + threadIdx.x; g < total; g += (long long)gridDim.x * blockDim.x) {
+        const long long ix = g % Nx, iy = (g / Nx) % Ny, iz = g / (Nx * Ny);
+        const double s = sx[ix] * sy[iy] * sz[iz];
+        const double d = 0.5 * (kx[ix] * my[iy] * mz[iz] + mx[ix] * ky[iy] * mz[iz] + mx[ix] * my[iy] * kz[iz]);
+        Minv[g] = s != 0.0 ? 1.0 / (s * s * d) : 0.0;
+    }
+}
+
+}  // namespace fecheb

@@ -63,10 +63,10 @@ __global__ void __launch_bounds__(kRRThreads) k_gram(const double* __restrict__ 
         }
 }
 
-// Y[r*B + j] <- sum_i Y[r*B + i] * R[i*B + j], in place (each CTA stages its rows before overwriting them)
+// Out[r*B + j] (+)= sum_i Y[r*B + i] * R[i*B + j];  Out may be Y (each CTA stages its rows before overwriting them)
 template <int T>
-__global__ void __launch_bounds__(kRRThreads) k_rightmul(double* __restrict__ Y, const double* __restrict__ R,
-                                                         long long N, int B)
+__global__ void __launch_bounds__(kRRThreads) k_rightmul(const double* Y, const double* __restrict__ R, double* Out,
+                                                         int accumulate, long long N, int B)
 {
     extern __shared__ double sm[];
     double* sR = sm;              // [B][B]
@@ -102,8 +102,8 @@ __global__ void __launch_bounds__(kRRThreads) k_rightmul(double* __restrict__ Y,
         for (int k = 0; k < T; ++k) {
             const int j = tj + 16 * k;
             if (j < B) {
-                if (ti < rows) Y[(r0 + ti) * B + j] = acc[0][k];
-                if (ti + 16 < rows) Y[(r0 + ti + 16) * B + j] = acc[1][k];
+                if (ti < rows) Out[(r0 + ti) * B + j] = acc[0][k] + (accumulate ? Out[(r0 + ti) * B + j] : 0.0);
+                if (ti + 16 < rows) Out[(r0 + ti + 16) * B + j] = acc[1][k] + (accumulate ? Out[(r0 + ti + 16) * B + j] : 0.0);
             }
         }
     }
@@ -127,7 +127,8 @@ inline cudaError_t launch_gram(const double* A, const double* Bm, long long N, i
     return cudaGetLastError();
 }
 
-inline cudaError_t launch_rightmul(double* Y, const double* R, long long N, int B, int sms, cudaStream_t st)
+inline cudaError_t launch_rightmul(const double* Y, const double* R, double* Out, int accumulate, long long N, int B,
+                                   int sms, cudaStream_t st)
 {
     const size_t smem = ((size_t)B * B + (size_t)kRRRows * (B + 1)) * sizeof(double);
     const int T = (B + 15) / 16;
@@ -142,10 +143,10 @@ inline cudaError_t launch_rightmul(double* Y, const double* R, long long N, int 
         configured = true;
     }
     const int grid = sms * (B > 64 ? 1 : 2);
-    if (T <= 1) k_rightmul<1><<<grid, kRRThreads, smem, st>>>(Y, R, N, B);
-    else if (T <= 2) k_rightmul<2><<<grid, kRRThreads, smem, st>>>(Y, R, N, B);
-    else if (T <= 4) k_rightmul<4><<<grid, kRRThreads, smem, st>>>(Y, R, N, B);
-    else k_rightmul<8><<<grid, kRRThreads, smem, st>>>(Y, R, N, B);
+    if (T <= 1) k_rightmul<1><<<grid, kRRThreads, smem, st>>>(Y, R, Out, accumulate, N, B);
+    else if (T <= 2) k_rightmul<2><<<grid, kRRThreads, smem, st>>>(Y, R, Out, accumulate, N, B);
+    else if (T <= 4) k_rightmul<4><<<grid, kRRThreads, smem, st>>>(Y, R, Out, accumulate, N, B);
+    else k_rightmul<8><<<grid, kRRThreads, smem, st>>>(Y, R, Out, accumulate, N, B);
     return cudaGetLastError();
 }
 

@@ -380,6 +380,42 @@ def test_rayleigh_ritz():
     assert np.linalg.norm(R[:, 0]) < 1e-4
 
 
+# ---- MINRES of the adjoint solve (l.221-225) -------------------------------------------------------------------------
+def test_minres_against_dense_solves():
+    """The oracle's MINRES is pinned to LAPACK: a regular shifted system against numpy.linalg.solve, and the singular
+    system of l.221 ((H~ - theta_k) with g orthogonal to the null vector) against the pseudo-inverse solution, which is
+    the component p_perp the paper's Krylov argument singles out.  The preconditioner against the CSR diagonal."""
+    w = workloads.config(1)
+    m = _mesh((w.xe, w.ye, w.ze), w.p, w.V)
+    free = m.mask().astype(bool)
+    A = _csr(m).toarray()[np.ix_(free, free)]
+    lam, U = np.linalg.eigh(A)
+    # preconditioner = inverse diagonal of the mass-scaled (1/2)K: compare with the CSR of the potential-free operator
+    m0 = _mesh((w.xe, w.ye, w.ze), w.p, lambda q: np.zeros(len(q)))
+    K = _csr(m0).toarray()
+    Mi = oracle.laplacian_precond(m)
+    assert np.allclose(Mi[free], 1.0 / np.diag(K)[free], rtol=1e-13) and np.all(Mi[~free] == 0) and np.all(Mi[free] > 0)
+    B = 4
+    G = workloads.random_block(77, m.N, B, m.mask())
+    eps = np.array([-1.0, 0.3, 2.2, 5.1])  # inside the spectrum: indefinite systems
+    for Minv in (None, Mi):
+        X, rel, it = oracle.minres_shifted(m, G, eps, maxit=2000, tol=1e-13, Minv=Minv)
+        for j in range(B):
+            xref = np.linalg.solve(A - eps[j] * np.eye(A.shape[0]), G[free, j])
+            assert np.linalg.norm(X[free, j] - xref) <= 1e-8 * np.linalg.norm(xref), (j, it)
+        assert np.all(X[~free] == 0)
+    # singular case: eps = a (3-fold degenerate) eigenvalue, g orthogonal to its null vectors Psi_k
+    k = 3
+    Psi = U[:, np.abs(lam - lam[k]) < 1e-8]
+    assert Psi.shape[1] == 3
+    Gs = G[:, :1].copy()
+    Gs[free, 0] -= Psi @ (Psi.T @ Gs[free, 0])
+    Xs, rel, it = oracle.minres_shifted(m, Gs, np.array([lam[k]]), maxit=2000, tol=1e-10)
+    xp = np.linalg.pinv(A - lam[k] * np.eye(A.shape[0]), rcond=1e-10) @ Gs[free, 0]
+    assert np.linalg.norm(Xs[free, 0] - xp) <= 1e-7 * np.linalg.norm(xp)
+    assert np.max(np.abs(Psi.T @ Xs[free, 0])) <= 1e-7 * np.linalg.norm(xp)  # p_perp is orthogonal to the null vectors
+
+
 # ---- inputs module ------------------------------------------------------------------------------------------
 def test_inputs_generator():
     z = workloads.splitmix64(0, 0, 3)
