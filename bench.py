@@ -233,6 +233,47 @@ def time_workload(fe, torch, w, steps, warmup, dev, seed_offset=0, with_e2e=Fals
     return res
 
 
+def time_consumers(fe, torch, w, dev):
+    """NEXT-1 / NEXT-2 on the workload's mesh (informational, --extra): one Rayleigh-Ritz call on a filtered block and
+    a fixed number of preconditioned MINRES steps with the config-5 shifts."""
+    gm = fe.FEMesh(w.xe, w.ye, w.ze, w.p, device=dev)
+    gm.set_potential(w.V(gm.quad_coords()))
+    N, B = gm.N, w.B
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(99)
+    mask = torch.as_tensor(gm.mask().astype(np.float64), device="cuda")[:, None]
+    X = torch.randn(N, B, dtype=torch.float64, device="cuda", generator=gen) * mask
+    a0, a, b = spectrum_bounds(w)
+    gm.cheb_filter(X, 4, a, b, a0)
+    work = torch.empty(N * B, dtype=torch.float64, device="cuda")
+    Y = X.clone()
+    gm.rayleigh_ritz(Y, work)  # warm-up
+    Y.copy_(X)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    gm.rayleigh_ritz(Y, work)
+    torch.cuda.synchronize()
+    rr_ms = (time.perf_counter() - t0) * 1e3
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(10):
+        gm.gram(X, Y)
+    e1.record()
+    torch.cuda.synchronize()
+    gram_ms = e0.elapsed_time(e1) / 10
+    eps = torch.as_tensor(workloads.shifts(2005, B), device="cuda")
+    G = torch.randn(N, B, dtype=torch.float64, device="cuda", generator=gen) * mask
+    gm.minres_shifted(G, eps, maxit=8, tol=0.0)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    _, _, it = gm.minres_shifted(G, eps, maxit=48, tol=0.0)
+    torch.cuda.synchronize()
+    mr_ms = (time.perf_counter() - t0) * 1e3 / it
+    return {"mesh": w.describe(), "rayleigh_ritz_ms": rr_ms, "gram_ms": gram_ms,
+            "gram_tflops": 2.0 * N * B * B / (gram_ms * 1e-3) / 1e12, "gram_gbs": 16.0 * N * B / (gram_ms * 1e-3) / 1e9,
+            "minres_ms_per_step": mr_ms, "minres_steps_timed": it}
+
+
 def summarize(w, r, total_ms_per_step, n_ranks=1):
     dofvec = r["N_free"] * r["B"] * r["napply"] * n_ranks
     value = dofvec / (total_ms_per_step * 1e-3) / 1e9
@@ -325,6 +366,11 @@ def main():
                 extra["cfg%d" % idx] = {"error": str(ex)[:200]}
             torch.cuda.empty_cache()
         line["other_workloads"] = extra
+        try:
+            line["consumers"] = time_consumers(fe, torch, w, local)
+        except Exception as ex:
+            line["consumers"] = {"error": str(ex)[:200]}
+        torch.cuda.empty_cache()
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(args.workload, SAMPLE_CELLS[args.workload])
     print(json.dumps(line))

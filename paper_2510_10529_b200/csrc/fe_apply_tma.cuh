@@ -3,7 +3,7 @@
 //   Y[g,j] (+)= s_g sum_{e∋g} yhat_e[a,j]  +  kappa_j X[g,j]          (reduce-add into a pre-initialised Y)
 //   W[g,j]   = beta' X[g,j]                                            (pre-initialises the NEXT step's target)
 //
-// One CTA = one cell x BT vectors.  a1 (gather) is ONE cp.async.bulk.tensor load of the cell's n x n x n x BT box of
+// Unit of work = one cell x BT vectors (one CTA per unit, or a persistent CTA walking units).  a1 (gather) is ONE cp.async.bulk.tensor load of the cell's n x n x n x BT box of
 // X (the layout of PAPER.md l.233-235 makes the block a 4-D tensor (j, gx, gy, gz)); a3 (scatter) is one
 // cp.reduce.async.bulk.tensor .add per nodal plane, so no thread computes a global address or issues an atomic.
 // The recurrence terms of the Chebyshev step (l.208-210; R7) need no read of Y_{k-1} at all: step k-1 stores
@@ -15,7 +15,7 @@
 //   A  = (N'y N'x) xhat                 A2 = G'x A + (ky/kx) G'y A                     per nodal z-plane
 //   U  = N'z A ;  T = VZ.U + G'z U + (kx/kz) N'z A2 ;  R = N'z^T T                      per (qx,qy) line
 //   yhat/kz = N'x^T N'y^T R                                                            per nodal z-plane
-// VZ = V_q hz^2/2 (= J V_q / kz); the output scale tile carries alpha kz s_g.
+// VZ = V_q hz^2/2 (= J V_q / kz); the output scale tile carries kz s_g and the last back-interpolation table alpha.
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
