@@ -515,7 +515,7 @@ int cheb_filter(fe_mesh* m, double* X, int B, int deg, double a, double b, doubl
 }
 
 // ---- Rayleigh-Ritz (NEXT-1; Eq. 23-24 l.210-219; readings R8, R9) ------------------------------------------
-// small dense helpers on the host (B <= 128): Cholesky S = L L^T, R = L^{-T}, cyclic Jacobi for the symmetric B x B problem
+// small dense helpers on the host (B <= 128): Cholesky S = L L^T, R = L^{-T}, tridiagonal QR for the symmetric B x B problem
 static bool chol_lower(std::vector<double>& S, int B)
 {
     for (int j = 0; j < B; ++j) {
@@ -550,50 +550,102 @@ static void inv_lower_transposed(const std::vector<double>& L, int B, std::vecto
         for (int j = i; j < B; ++j) R[(size_t)i * B + j] = Li[(size_t)j * B + i];
 }
 
-// eigenvalues ascending in w, eigenvectors in the COLUMNS of V (row-major V[i*B+k] = component i of vector k)
-static void jacobi_eigh(std::vector<double> G, int B, std::vector<double>& w, std::vector<double>& V)
+// Symmetric B x B eigenproblem on the host: Householder reduction to tridiagonal form, then implicit-shift QR sweeps
+// (Wilkinson shift, deflation from the bottom) with the rotations accumulated.  Eigenvalues ascending in w,
+// eigenvectors in the COLUMNS of V (row-major V[i*B+k] = component i of vector k).  O(B^3), ~10x fewer flops than
+// cyclic Jacobi, which dominated fe_rayleigh_ritz at B = 64.
+static void sym_eigh(std::vector<double> A, int n, std::vector<double>& w, std::vector<double>& V)
 {
-    V.assign((size_t)B * B, 0.0);
-    for (int i = 0; i < B; ++i) V[(size_t)i * B + i] = 1.0;
-    for (int sweep = 0; sweep < 60; ++sweep) {
-        double off = 0.0, diag = 0.0;
-        for (int i = 0; i < B; ++i)
-            for (int j = 0; j < B; ++j) (i == j ? diag : off) += G[(size_t)i * B + j] * G[(size_t)i * B + j];
-        if (off <= 1e-32 * diag) break;
-        for (int p = 0; p < B - 1; ++p)
-            for (int q = p + 1; q < B; ++q) {
-                const double apq = G[(size_t)p * B + q];
-                if (apq == 0.0) continue;
-                const double theta = (G[(size_t)q * B + q] - G[(size_t)p * B + p]) / (2.0 * apq);
-                const double t = (theta >= 0 ? 1.0 : -1.0) / (std::fabs(theta) + std::sqrt(theta * theta + 1.0));
-                const double c = 1.0 / std::sqrt(t * t + 1.0), s = t * c;
-                for (int k = 0; k < B; ++k) {
-                    const double gkp = G[(size_t)k * B + p], gkq = G[(size_t)k * B + q];
-                    G[(size_t)k * B + p] = c * gkp - s * gkq;
-                    G[(size_t)k * B + q] = s * gkp + c * gkq;
-                }
-                for (int k = 0; k < B; ++k) {
-                    const double gpk = G[(size_t)p * B + k], gqk = G[(size_t)q * B + k];
-                    G[(size_t)p * B + k] = c * gpk - s * gqk;
-                    G[(size_t)q * B + k] = s * gpk + c * gqk;
-                }
-                for (int k = 0; k < B; ++k) {
-                    const double vkp = V[(size_t)k * B + p], vkq = V[(size_t)k * B + q];
-                    V[(size_t)k * B + p] = c * vkp - s * vkq;
-                    V[(size_t)k * B + q] = s * vkp + c * vkq;
-                }
+    std::vector<double> Zt((size_t)n * n, 0.0);  // Zt[k*n + i] = component i of basis vector k
+    for (int i = 0; i < n; ++i) Zt[(size_t)i * n + i] = 1.0;
+    std::vector<double> v(n), pv(n);
+    for (int k = 0; k + 2 < n; ++k) {  // reflector acting on indices k+1..n-1 zeroes A[k+2.., k]
+        double nrm = 0.0;
+        for (int i = k + 1; i < n; ++i) nrm += A[(size_t)i * n + k] * A[(size_t)i * n + k];
+        nrm = std::sqrt(nrm);
+        if (nrm == 0.0) continue;
+        const double x0 = A[(size_t)(k + 1) * n + k];
+        const double alpha = x0 > 0.0 ? -nrm : nrm;
+        double vn = 0.0;
+        for (int i = k + 1; i < n; ++i) {
+            v[i] = A[(size_t)i * n + k] - (i == k + 1 ? alpha : 0.0);
+            vn += v[i] * v[i];
+        }
+        if (vn == 0.0) continue;
+        const double inv = 1.0 / std::sqrt(vn);
+        for (int i = k + 1; i < n; ++i) v[i] *= inv;
+        // A <- H A H, H = I - 2 v v^T: p = A v, K = v.p, q = p - K v, A -= 2 (v q^T + q v^T)
+        double K = 0.0;
+        for (int i = k; i < n; ++i) {
+            double t = 0.0;
+            for (int jx = k + 1; jx < n; ++jx) t += A[(size_t)i * n + jx] * v[jx];
+            pv[i] = t;
+        }
+        for (int i = k + 1; i < n; ++i) K += v[i] * pv[i];
+        // column/row k: only the reflector's action on A[k+1.., k] matters: it becomes (alpha, 0, ..., 0)
+        for (int i = k + 1; i < n; ++i) {
+            const double val = (i == k + 1) ? alpha : 0.0;
+            A[(size_t)i * n + k] = val;
+            A[(size_t)k * n + i] = val;
+        }
+        for (int i = k + 1; i < n; ++i) pv[i] -= K * v[i];
+        for (int i = k + 1; i < n; ++i)
+            for (int jx = k + 1; jx < n; ++jx) A[(size_t)i * n + jx] -= 2.0 * (v[i] * pv[jx] + pv[i] * v[jx]);
+        // Z <- Z H on the basis:  Z[:, j] -= 2 (Z v) v_j
+        for (int i = 0; i < n; ++i) pv[i] = 0.0;
+        for (int jx = k + 1; jx < n; ++jx)
+            for (int i = 0; i < n; ++i) pv[i] += Zt[(size_t)jx * n + i] * v[jx];
+        for (int jx = k + 1; jx < n; ++jx)
+            for (int i = 0; i < n; ++i) Zt[(size_t)jx * n + i] -= 2.0 * pv[i] * v[jx];
+    }
+    std::vector<double> d(n), e(n > 1 ? n - 1 : 0);
+    for (int i = 0; i < n; ++i) d[i] = A[(size_t)i * n + i];
+    for (int i = 0; i + 1 < n; ++i) e[i] = A[(size_t)(i + 1) * n + i];
+    const double eps = 2.220446049250313e-16;
+    int hi = n - 1, guard = 0;
+    while (hi > 0 && guard < 100 * n) {
+        if (std::fabs(e[hi - 1]) <= eps * (std::fabs(d[hi - 1]) + std::fabs(d[hi]))) {
+            e[hi - 1] = 0.0;
+            --hi;
+            continue;
+        }
+        ++guard;
+        int lo = hi - 1;
+        while (lo > 0 && std::fabs(e[lo - 1]) > eps * (std::fabs(d[lo - 1]) + std::fabs(d[lo]))) --lo;
+        const double dd = 0.5 * (d[hi - 1] - d[hi]), eh = e[hi - 1];
+        const double mu = d[hi] - eh * eh / (dd + (dd >= 0.0 ? 1.0 : -1.0) * std::hypot(dd, eh));
+        double x = d[lo] - mu, z = e[lo];
+        for (int k = lo; k < hi; ++k) {
+            const double r = std::hypot(x, z);
+            const double c = r > 0.0 ? x / r : 1.0, sn = r > 0.0 ? z / r : 0.0;
+            if (k > lo) e[k - 1] = r;
+            const double a = d[k], b = e[k], dn = d[k + 1];
+            d[k] = c * c * a + 2.0 * c * sn * b + sn * sn * dn;
+            d[k + 1] = sn * sn * a - 2.0 * c * sn * b + c * c * dn;
+            e[k] = c * sn * (dn - a) + (c * c - sn * sn) * b;
+            x = e[k];
+            if (k + 1 < hi) {
+                z = sn * e[k + 1];
+                e[k + 1] = c * e[k + 1];
             }
+            double* q0 = &Zt[(size_t)k * n];
+            double* q1 = &Zt[(size_t)(k + 1) * n];
+            for (int i = 0; i < n; ++i) {
+                const double u0 = q0[i], u1 = q1[i];
+                q0[i] = c * u0 + sn * u1;
+                q1[i] = -sn * u0 + c * u1;
+            }
+        }
     }
-    std::vector<int> idx(B);
-    for (int i = 0; i < B; ++i) idx[i] = i;
-    std::sort(idx.begin(), idx.end(), [&](int a, int b) { return G[(size_t)a * B + a] < G[(size_t)b * B + b]; });
-    std::vector<double> Vs((size_t)B * B);
-    w.resize(B);
-    for (int k = 0; k < B; ++k) {
-        w[k] = G[(size_t)idx[k] * B + idx[k]];
-        for (int i = 0; i < B; ++i) Vs[(size_t)i * B + k] = V[(size_t)i * B + idx[k]];
+    std::vector<int> idx(n);
+    for (int i = 0; i < n; ++i) idx[i] = i;
+    std::sort(idx.begin(), idx.end(), [&](int a, int b) { return d[a] < d[b]; });
+    w.resize(n);
+    V.assign((size_t)n * n, 0.0);
+    for (int k = 0; k < n; ++k) {
+        w[k] = d[idx[k]];
+        for (int i = 0; i < n; ++i) V[(size_t)i * n + k] = Zt[(size_t)idx[k] * n + i];
     }
-    V.swap(Vs);
 }
 
 // one CholQR pass: S = Y^T Y (device) -> L, R = L^{-T} (host) -> Y <- Y R (device)
@@ -637,7 +689,7 @@ int fe_rayleigh_ritz(fe_mesh* m, double* Y, int B, double* theta_host, double* w
     CUDA_TRY(cudaStreamSynchronize(st));
     for (int i = 0; i < B; ++i)
         for (int j = 0; j < i; ++j) G[(size_t)i * B + j] = G[(size_t)j * B + i] = 0.5 * (G[(size_t)i * B + j] + G[(size_t)j * B + i]);
-    jacobi_eigh(G, B, w, V);
+    sym_eigh(G, B, w, V);
     for (int k = 0; k < B; ++k) theta_host[k] = w[k];
     CUDA_TRY(cudaMemcpyAsync(m->d_small + bb, V.data(), bb * sizeof(double), cudaMemcpyHostToDevice, st));
     CUDA_TRY(launch_rightmul(Y, m->d_small + bb, Y, 0, m->N, B, m->sms, st));     // X = Q V

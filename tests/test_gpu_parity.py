@@ -205,7 +205,7 @@ def test_filter_reduced_config2_and_ritz_values():
 
 @pytest.mark.parametrize("p,B", [(2, 8), (4, 16), (3, 37), (2, 128)])
 def test_device_rayleigh_ritz(p, B):
-    """fe_rayleigh_ritz (NEXT-1: device Gram / rotation kernels, host B x B Cholesky and Jacobi) against the oracle's
+    """fe_rayleigh_ritz (NEXT-1: device Gram / rotation kernels, host B x B Cholesky and eigensolver) against the oracle's
     Eq. 23-24: Ritz values <= 1e-9 (R16); vectors are compared through what is unique (R17): orthonormality, the
     spanned subspace, and the Ritz residual relation Q^T H~ Q = diag(theta)."""
     import oracle
