@@ -315,6 +315,30 @@ def _sample_rows(w, count, seed):
     return np.unique(gx + nx * (gy + ny * gz))
 
 
+def test_apply_config4_mesh_sampled_rows():
+    """Config 4's graded 40^3-cell p=6 mesh (14 M nodes) at full size, in the persistent 32-vector launch shape the
+    bench times, on a 32-column slice of the block (columns are independent, R22): sampled rows against Eq. 17."""
+    import oracle
+    fe = _fe()
+    w = workloads.config(4)
+    om = oracle.OracleMesh(w.xe, w.ye, w.ze, w.p)
+    Vq = w.V(om.quad_coords())
+    om.set_potential(Vq, build=False)
+    gm = fe.FEMesh(w.xe, w.ye, w.ze, w.p)
+    gm.set_potential(Vq)
+    B = 32
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(4004)
+    Xd = torch.randn(gm.N, B, dtype=torch.float64, device="cuda", generator=gen)  # seeded device input, copied out below
+    rows = _sample_rows(w, 40, 9004)
+    # the oracle needs the whole block on the host only where the sampled rows reach: copy it once
+    X = Xd.cpu().numpy()
+    Yo = om.apply_rows(X * om.mask()[:, None], rows, None)
+    Yg = gm.apply_H(Xd)
+    Ys = Yg[torch.as_tensor(rows, device="cuda")].cpu().numpy()
+    assert np.linalg.norm(Ys - Yo) <= TOL_APPLY * np.linalg.norm(Yo)
+
+
 @pytest.mark.parametrize("cfg", [2, 5, 3])
 def test_apply_full_size_sampled_rows(cfg):
     """Full BASELINE sizes in the launch configuration bench.py times; the oracle computes sampled rows one by one
