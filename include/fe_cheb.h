@@ -107,7 +107,8 @@ int fe_gram(fe_mesh* m, const double* A, const double* Bm, int B, double* C_host
 int fe_add_subspace(fe_mesh* m, const double* Psi, const double* D_host, double* P, int B, void* cuda_stream);
 
 /* Kernel variant for experiments and tests: 0 = default (TMA generation when B is even and the blocks are 16-byte
- * aligned, else the legacy atomics kernel), 5 = same, 1..4 = legacy generations.  FE_ERR_INVALID if unknown. */
+ * aligned, else the legacy atomics kernel), 3 = legacy kernel always, 5..8 = launch shapes of the TMA kernel
+ * (fe_apply_tma.cuh).  FE_ERR_INVALID if unknown. */
 int fe_set_variant(fe_mesh* m, int variant);
 /* Kernels launched by this handle since creation (bench.py's gpu_launches). */
 int64_t fe_launch_count(const fe_mesh* m);

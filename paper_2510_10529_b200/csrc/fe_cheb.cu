@@ -339,7 +339,6 @@ static int operator_step(fe_mesh* m, const double* X, const double* Z, double* Y
     fill_params(m, &prm);
     prm.X = X; prm.Z = Z; prm.Y = Y; prm.eps = eps; prm.B = B;
     prm.alpha = alpha; prm.beta = beta; prm.c = c;
-    for (int q = 0; q < m->n; ++q) prm.aw[q] = alpha * prm.w[q];
     int nl = 0;
     cudaError_t e = launch_apply(prm, m->p, m->variant, m->N, m->ncells, st, &nl);
     if (e != cudaSuccess) return fail(FE_ERR_CUDA, "operator launch failed: %s", cudaGetErrorString(e));
@@ -399,7 +398,7 @@ static int make_block_maps(BlockMaps* bm, const fe_mesh* m, const double* base, 
 // bulk tensor copies need 16-byte aligned bases and row pitches (B even)
 static bool tma_eligible(const fe_mesh* m, int B, const void* a, const void* b, const void* c)
 {
-    if (m->variant != 0 && m->variant < 5) return false;
+    if (m->variant == 3) return false;
     if (B % 2 != 0 || !encode_fn()) return false;
     return (((uintptr_t)a | (uintptr_t)b | (uintptr_t)c) & 15) == 0;
 }

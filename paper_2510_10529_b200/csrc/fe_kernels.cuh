@@ -40,7 +40,6 @@ struct ApplyParams {
     long long Nx, NxNy;
     double alpha, beta, c;
     double N[81], G[81], w[9];
-    double aw[9];  // alpha * w (variant 4)
     EOTab eoN, eoNT, eoG;  // even-odd split of N, N^T and G (all centro-symmetric: GLL and Gauss points are symmetric)
 };
 
@@ -86,161 +85,7 @@ inline void launch_weight_potential(const ApplyParams& prm, int p, const double*
     k_weight_potential<<<148 * 8, 256, 0, st>>>(prm, p + 1, V, WV, VZ, ncells);
 }
 
-// ---- variant 1: plain sum factorisation, atomics scatter --------------------------------------------------------
-// out[i] = sum_k M[i*n+k] in[k]   (TRANS: out[i] = sum_k M[k*n+i] in[k])
-template <int n, bool TRANS>
-__device__ __forceinline__ void mat1d(const double* __restrict__ M, const double (&in)[n], double (&out)[n])
-{
-#pragma unroll
-    for (int i = 0; i < n; ++i) {
-        double s = 0.0;
-#pragma unroll
-        for (int k = 0; k < n; ++k) s = fma(TRANS ? M[k * n + i] : M[i * n + k], in[k], s);
-        out[i] = s;
-    }
-}
-
-template <int P, int BT>
-__global__ void __launch_bounds__((P + 1) * BT) k_apply_v1(const __grid_constant__ ApplyParams prm)
-{
-    constexpr int n = P + 1, n3 = n * n * n;
-    extern __shared__ double smem[];
-    double* sA = smem;             // [n^3][BT]
-    double* sA2 = smem + n3 * BT;  // [n^3][BT]
-    const int lane = threadIdx.x, pl = threadIdx.y;
-    const int cell = blockIdx.x;
-    const int ex = cell % prm.cx, ey = (cell / prm.cx) % prm.cy, ez = cell / (prm.cx * prm.cy);
-    const int j = blockIdx.y * BT + lane;
-    const bool act = j < prm.B;
-    const long long B = prm.B;
-    const long long gbase = (long long)ex * P + prm.Nx * ((long long)ey * P) + prm.NxNy * ((long long)ez * P);
-    const double hx = prm.hx[ex], hy = prm.hy[ey], hz = prm.hz[ez];
-    const double J = hx * hy * hz * 0.125;
-    const double kx = 0.5 * J * 4.0 / (hx * hx), ky = 0.5 * J * 4.0 / (hy * hy), kz = 0.5 * J * 4.0 / (hz * hz);
-
-    double v[n][n], t[n], o[n];
-    // ---- plane phase 1: gather (a1) with mu*s pre-scale, interpolate in x and y --------------------------------
-    {
-        const long long gpl = gbase + prm.NxNy * pl;
-#pragma unroll
-        for (int ay = 0; ay < n; ++ay)
-#pragma unroll
-            for (int ax = 0; ax < n; ++ax) {
-                const long long g = gpl + ax + prm.Nx * ay;
-                v[ay][ax] = act ? prm.X[g * B + j] * prm.sm[g] : 0.0;
-            }
-    }
-#pragma unroll
-    for (int ay = 0; ay < n; ++ay) {
-        mat1d<n, false>(prm.N, v[ay], o);
-#pragma unroll
-        for (int q = 0; q < n; ++q) v[ay][q] = o[q];
-    }
-#pragma unroll
-    for (int qx = 0; qx < n; ++qx) {
-#pragma unroll
-        for (int a = 0; a < n; ++a) t[a] = v[a][qx];
-        mat1d<n, false>(prm.N, t, o);
-#pragma unroll
-        for (int q = 0; q < n; ++q) v[q][qx] = o[q];
-    }
-    {
-        double v2[n][n];
-#pragma unroll
-        for (int qy = 0; qy < n; ++qy) {
-            mat1d<n, false>(prm.G, v[qy], o);
-#pragma unroll
-            for (int qx = 0; qx < n; ++qx) v2[qy][qx] = (kx * prm.w[qy]) * o[qx];
-        }
-#pragma unroll
-        for (int qx = 0; qx < n; ++qx) {
-#pragma unroll
-            for (int a = 0; a < n; ++a) t[a] = v[a][qx];
-            mat1d<n, false>(prm.G, t, o);
-#pragma unroll
-            for (int qy = 0; qy < n; ++qy) v2[qy][qx] = fma(ky * prm.w[qx], o[qy], v2[qy][qx]);
-        }
-#pragma unroll
-        for (int qy = 0; qy < n; ++qy)
-#pragma unroll
-            for (int qx = 0; qx < n; ++qx) {
-                const int idx = ((pl * n + qy) * n + qx) * BT + lane;
-                sA[idx] = v[qy][qx];
-                sA2[idx] = v2[qy][qx];
-            }
-    }
-    __syncthreads();
-    // ---- line phase: z interpolation, pointwise potential and z stiffness, z back-interpolation --------------------
-    {
-        const double* WVc = prm.WV + (long long)cell * n3;
-#pragma unroll 1
-        for (int r = 0; r < n; ++r) {
-            const int l = pl + n * r;
-            const int qx = l % n, qy = l / n;
-            double a[n], a2[n], u[n], u2[n], gu[n];
-#pragma unroll
-            for (int az = 0; az < n; ++az) {
-                const int idx = ((az * n + qy) * n + qx) * BT + lane;
-                a[az] = sA[idx];
-                a2[az] = sA2[idx];
-            }
-            mat1d<n, false>(prm.N, a, u);
-            mat1d<n, false>(prm.N, a2, u2);
-            mat1d<n, false>(prm.G, u, gu);
-            const double kzw = kz * prm.w[qx] * prm.w[qy];
-#pragma unroll
-            for (int qz = 0; qz < n; ++qz) {
-                const double wv = WVc[(qz * n + qy) * n + qx];
-                t[qz] = fma(wv, u[qz], fma(prm.w[qz], u2[qz], kzw * gu[qz]));
-            }
-            mat1d<n, true>(prm.N, t, o);
-#pragma unroll
-            for (int az = 0; az < n; ++az) sA[((az * n + qy) * n + qx) * BT + lane] = o[az];
-        }
-    }
-    __syncthreads();
-    // ---- plane phase 2: back-interpolate in y and x, fused epilogue and scatter-add (a3) ------------------------------
-#pragma unroll
-    for (int qy = 0; qy < n; ++qy)
-#pragma unroll
-        for (int qx = 0; qx < n; ++qx) v[qy][qx] = sA[((pl * n + qy) * n + qx) * BT + lane];
-#pragma unroll
-    for (int qx = 0; qx < n; ++qx) {
-#pragma unroll
-        for (int q = 0; q < n; ++q) t[q] = v[q][qx];
-        mat1d<n, true>(prm.N, t, o);
-#pragma unroll
-        for (int a = 0; a < n; ++a) v[a][qx] = o[a];
-    }
-#pragma unroll
-    for (int ay = 0; ay < n; ++ay) {
-        mat1d<n, true>(prm.N, v[ay], o);
-#pragma unroll
-        for (int a = 0; a < n; ++a) v[ay][a] = o[a];
-    }
-    if (act) {
-        const long long gpl = gbase + prm.NxNy * pl;
-        const double shift = prm.c + (prm.eps ? prm.eps[j] : 0.0);
-#pragma unroll
-        for (int ay = 0; ay < n; ++ay)
-#pragma unroll
-            for (int ax = 0; ax < n; ++ax) {
-                const long long g = gpl + ax + prm.Nx * ay;
-                const double s = prm.sm[g];
-                if (s != 0.0) {
-                    double val = prm.alpha * s * v[ay][ax];
-                    if (ax < P && ay < P && pl < P) {  // the cell that owns the node adds the diagonal terms once
-                        val = fma(-prm.alpha * shift, prm.X[g * B + j], val);
-                        if (prm.Z) val = fma(prm.beta, prm.Z[g * B + j], val);
-                    }
-                    atomicAdd(prm.Y + g * B + j, val);
-                }
-            }
-    }
-}
-
-
-// ---- variant 2: even-odd sum factorisation, potential staged in shared memory --------------------------------------
+// ---- even-odd form of the 1-D contractions (shared by every kernel generation) ---------------------------------------
 template <int n>
 __device__ __forceinline__ void mat1d_eo(const EOTab& T, const double (&in)[n], double (&out)[n])
 {
@@ -275,172 +120,9 @@ __device__ __forceinline__ void mat1d_eo(const EOTab& T, const double (&in)[n], 
     }
 }
 
-template <int P, int BT, int MINB>
-__global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_v2(const __grid_constant__ ApplyParams prm)
-{
-    constexpr int n = P + 1, n3 = n * n * n;
-    extern __shared__ double smem[];
-    double* sA = smem;             // [n^3][BT]
-    double* sA2 = smem + n3 * BT;  // [n^3][BT]
-    double* sWV = sA2 + n3 * BT;   // [n^3]
-    const int lane = threadIdx.x, pl = threadIdx.y;
-    const int cell = blockIdx.x;
-    const int ex = cell % prm.cx, ey = (cell / prm.cx) % prm.cy, ez = cell / (prm.cx * prm.cy);
-    const int j = blockIdx.y * BT + lane;
-    const bool act = j < prm.B;
-    const long long B = prm.B;
-    const long long gpl = (long long)ex * P + prm.Nx * ((long long)ey * P) + prm.NxNy * ((long long)ez * P + pl);
-    const double hx = prm.hx[ex], hy = prm.hy[ey], hz = prm.hz[ez];
-    const double J = hx * hy * hz * 0.125;
-    const double kx = 2.0 * J / (hx * hx), ky = 2.0 * J / (hy * hy), kz = 2.0 * J / (hz * hz);
-
-    double v[n][n], t[n], o[n];
-    // ---- plane phase 1: gather (a1) with mu*s pre-scale; interpolate in x and y; x,y stiffness ------------------------
-#pragma unroll
-    for (int ay = 0; ay < n; ++ay)
-#pragma unroll
-        for (int ax = 0; ax < n; ++ax) {
-            const long long g = gpl + ax + prm.Nx * ay;
-            v[ay][ax] = act ? prm.X[g * B + j] * prm.sm[g] : 0.0;
-        }
-    {
-        const double* WVc = prm.WV + (long long)cell * n3;
-        for (int i = pl * BT + lane; i < n3; i += n * BT) sWV[i] = WVc[i];
-    }
-#pragma unroll
-    for (int ay = 0; ay < n; ++ay) {
-        mat1d_eo<n>(prm.eoN, v[ay], o);
-#pragma unroll
-        for (int q = 0; q < n; ++q) v[ay][q] = o[q];
-    }
-#pragma unroll
-    for (int qx = 0; qx < n; ++qx) {
-#pragma unroll
-        for (int a = 0; a < n; ++a) t[a] = v[a][qx];
-        mat1d_eo<n>(prm.eoN, t, o);
-#pragma unroll
-        for (int q = 0; q < n; ++q) v[q][qx] = o[q];
-    }
-    {
-        double v2[n][n];
-#pragma unroll
-        for (int qy = 0; qy < n; ++qy) {
-            mat1d_eo<n>(prm.eoG, v[qy], o);
-            const double f = kx * prm.w[qy];
-#pragma unroll
-            for (int qx = 0; qx < n; ++qx) v2[qy][qx] = f * o[qx];
-        }
-#pragma unroll
-        for (int qx = 0; qx < n; ++qx) {
-#pragma unroll
-            for (int a = 0; a < n; ++a) t[a] = v[a][qx];
-            mat1d_eo<n>(prm.eoG, t, o);
-            const double f = ky * prm.w[qx];
-#pragma unroll
-            for (int qy = 0; qy < n; ++qy) v2[qy][qx] = fma(f, o[qy], v2[qy][qx]);
-        }
-#pragma unroll
-        for (int qy = 0; qy < n; ++qy)
-#pragma unroll
-            for (int qx = 0; qx < n; ++qx) {
-                const int idx = ((pl * n + qy) * n + qx) * BT + lane;
-                sA[idx] = v[qy][qx];
-                sA2[idx] = v2[qy][qx];
-            }
-    }
-    __syncthreads();
-    // ---- line phase: thread owns the n z-lines (qx = pl, qy = 0..n-1) -------------------------------------------------
-    {
-        const int qx = pl;
-        const double kzwx = kz * prm.w[qx];
-#pragma unroll 1
-        for (int qy = 0; qy < n; ++qy) {
-            double a[n], a2[n], u[n], u2[n], gu[n];
-#pragma unroll
-            for (int az = 0; az < n; ++az) {
-                const int idx = ((az * n + qy) * n + qx) * BT + lane;
-                a[az] = sA[idx];
-                a2[az] = sA2[idx];
-            }
-            mat1d_eo<n>(prm.eoN, a, u);
-            mat1d_eo<n>(prm.eoN, a2, u2);
-            mat1d_eo<n>(prm.eoG, u, gu);
-            const double kzw = kzwx * prm.w[qy];
-#pragma unroll
-            for (int qz = 0; qz < n; ++qz) {
-                const double wv = sWV[(qz * n + qy) * n + qx];
-                t[qz] = fma(wv, u[qz], fma(prm.w[qz], u2[qz], kzw * gu[qz]));
-            }
-            mat1d_eo<n>(prm.eoNT, t, o);
-#pragma unroll
-            for (int az = 0; az < n; ++az) sA[((az * n + qy) * n + qx) * BT + lane] = o[az];
-        }
-    }
-    __syncthreads();
-    // ---- plane phase 2: back-interpolate in y and x; fused epilogue and scatter-add (a3) ------------------------------
-#pragma unroll
-    for (int qy = 0; qy < n; ++qy)
-#pragma unroll
-        for (int qx = 0; qx < n; ++qx) v[qy][qx] = sA[((pl * n + qy) * n + qx) * BT + lane];
-#pragma unroll
-    for (int qx = 0; qx < n; ++qx) {
-#pragma unroll
-        for (int q = 0; q < n; ++q) t[q] = v[q][qx];
-        mat1d_eo<n>(prm.eoNT, t, o);
-#pragma unroll
-        for (int a = 0; a < n; ++a) v[a][qx] = o[a];
-    }
-#pragma unroll
-    for (int ay = 0; ay < n; ++ay) {
-        mat1d_eo<n>(prm.eoNT, v[ay], o);
-#pragma unroll
-        for (int a = 0; a < n; ++a) v[ay][a] = o[a];
-    }
-    if (act) {
-        const double ashift = -prm.alpha * (prm.c + (prm.eps ? prm.eps[j] : 0.0));
-        const bool zterm = prm.Z != nullptr;
-#pragma unroll
-        for (int ay = 0; ay < n; ++ay) {
-            double s[n], xo[n], zo[n];
-            const bool own_row = (ay < P) && (pl < P);
-#pragma unroll
-            for (int ax = 0; ax < n; ++ax) {
-                const long long g = gpl + ax + prm.Nx * ay;
-                s[ax] = prm.sm[g];
-                const bool own = own_row && ax < P && s[ax] != 0.0;
-                xo[ax] = own ? prm.X[g * B + j] : 0.0;
-                zo[ax] = (own && zterm) ? prm.Z[g * B + j] : 0.0;
-            }
-#pragma unroll
-            for (int ax = 0; ax < n; ++ax) {
-                if (s[ax] != 0.0) {
-                    const long long g = gpl + ax + prm.Nx * ay;
-                    double val = (prm.alpha * s[ax]) * v[ay][ax];
-                    if (own_row && ax < P) val = fma(ashift, xo[ax], fma(prm.beta, zo[ax], val));
-                    atomicAdd(prm.Y + g * B + j, val);
-                }
-            }
-        }
-    }
-}
-
-template <int P, int BT, int MINB>
-cudaError_t launch_v2(const ApplyParams& prm, long long ncells, cudaStream_t st)
-{
-    constexpr int n = P + 1;
-    const size_t smem = ((size_t)2 * n * n * n * BT + n * n * n) * sizeof(double);
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_apply_v2<P, BT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
-    dim3 grid((unsigned)ncells, (unsigned)((prm.B + BT - 1) / BT)), block(BT, n);
-    k_apply_v2<P, BT, MINB><<<grid, block, smem, st>>>(prm);
-    return cudaGetLastError();
-}
-
-// ---- variant 3: v2 + scaling tile in shared memory + cp.async prefetch of the owner rows of X and Z ------------------
+// ---- legacy generation (variant 3): per-thread gather, potential and scaling tiles in shared memory, cp.async
+//      prefetch of the owner rows of X and Z, red.global.add.f64 scatter into a zero-filled Y.  Takes the blocks the
+//      TMA kernel cannot (odd B, unaligned bases) and serves as an independent cross-check in the tests.
 __device__ __forceinline__ void cp_async8(void* smem_dst, const void* gsrc, bool valid)
 {
     const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
@@ -640,234 +322,10 @@ cudaError_t launch_v3(const ApplyParams& prm, long long ncells, cudaStream_t st)
     return cudaGetLastError();
 }
 
-// ---- variant 4: v3 + 32-bit offsets from a CTA-uniform base, alpha folded into the staged potential and weights,
-//                 line phase run as plane passes (one 1-D table per pass, so table entries stay in uniform registers)
-template <int P, int BT, int MINB>
-__global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_v4(const __grid_constant__ ApplyParams prm)
-{
-    constexpr int n = P + 1, n3 = n * n * n;
-    extern __shared__ double smem[];
-    double* sA = smem;             // [n^3][BT]
-    double* sA2 = smem + n3 * BT;  // [n^3][BT]
-    double* sWV = sA2 + n3 * BT;   // [n^3]  alpha J w V of this cell
-    double* sS = sWV + n3;         // [n^3]  mu * M^{-1/2} at the cell's nodes
-    const int lane = threadIdx.x, pl = threadIdx.y;
-    const int cell = blockIdx.x;
-    const int ex = cell % prm.cx, ey = (cell / prm.cx) % prm.cy, ez = cell / (prm.cx * prm.cy);
-    const int j = blockIdx.y * BT + lane;
-    const bool act = j < prm.B;
-    // CTA-uniform 64-bit bases; everything a thread touches lies within 2^32 bytes of them (checked at launch)
-    const long long g0 = (long long)ex * P + prm.Nx * ((long long)ey * P) + prm.NxNy * ((long long)ez * P);
-    const double* __restrict__ Xc = prm.X + g0 * prm.B;
-    const double* __restrict__ Zc = prm.Z + g0 * prm.B;
-    double* __restrict__ Yc = prm.Y + g0 * prm.B;
-    const unsigned uB = (unsigned)prm.B, rs = (unsigned)prm.Nx * uB;
-    const unsigned tb = (unsigned)pl * (unsigned)prm.NxNy * uB + (unsigned)j;
-    unsigned ro[n], co[n];
-#pragma unroll
-    for (int i = 0; i < n; ++i) {
-        ro[i] = tb + i * rs;
-        co[i] = i * uB;
-    }
-    const double hx = prm.hx[ex], hy = prm.hy[ey], hz = prm.hz[ez];
-    const double J = hx * hy * hz * 0.125;
-    const double kx = 2.0 * J / (hx * hx), ky = 2.0 * J / (hy * hy), kz = prm.alpha * 2.0 * J / (hz * hz);
-
-    double v[n][n], t[n], o[n];
-    // ---- plane phase 1 ---------------------------------------------------------------------------------------------
-#pragma unroll
-    for (int ay = 0; ay < n; ++ay)
-#pragma unroll
-        for (int ax = 0; ax < n; ++ax) v[ay][ax] = act ? Xc[ro[ay] + co[ax]] : 0.0;
-    {
-        const double* WVc = prm.WV + (long long)cell * n3;
-        for (int i = pl * BT + lane; i < n3; i += n * BT) {
-            sWV[i] = prm.alpha * WVc[i];
-            const int ax = i % n, ay = (i / n) % n, az = i / (n * n);
-            sS[i] = prm.sm[g0 + ax + prm.Nx * ay + prm.NxNy * az];
-        }
-    }
-    __syncthreads();
-#pragma unroll
-    for (int ay = 0; ay < n; ++ay)
-#pragma unroll
-        for (int ax = 0; ax < n; ++ax) v[ay][ax] *= sS[(pl * n + ay) * n + ax];
-#pragma unroll
-    for (int ay = 0; ay < n; ++ay) {
-        mat1d_eo<n>(prm.eoN, v[ay], o);
-#pragma unroll
-        for (int q = 0; q < n; ++q) v[ay][q] = o[q];
-    }
-#pragma unroll
-    for (int qx = 0; qx < n; ++qx) {
-#pragma unroll
-        for (int a = 0; a < n; ++a) t[a] = v[a][qx];
-        mat1d_eo<n>(prm.eoN, t, o);
-#pragma unroll
-        for (int q = 0; q < n; ++q) v[q][qx] = o[q];
-    }
-    {
-        double v2[n][n];
-#pragma unroll
-        for (int qy = 0; qy < n; ++qy) {
-            mat1d_eo<n>(prm.eoG, v[qy], o);
-            const double f = kx * prm.w[qy];
-#pragma unroll
-            for (int qx = 0; qx < n; ++qx) v2[qy][qx] = f * o[qx];
-        }
-#pragma unroll
-        for (int qx = 0; qx < n; ++qx) {
-#pragma unroll
-            for (int a = 0; a < n; ++a) t[a] = v[a][qx];
-            mat1d_eo<n>(prm.eoG, t, o);
-            const double f = ky * prm.w[qx];
-#pragma unroll
-            for (int qy = 0; qy < n; ++qy) v2[qy][qx] = fma(f, o[qy], v2[qy][qx]);
-        }
-        double* pa = sA + (size_t)pl * n * n * BT + lane;
-        double* pa2 = sA2 + (size_t)pl * n * n * BT + lane;
-#pragma unroll
-        for (int qy = 0; qy < n; ++qy)
-#pragma unroll
-            for (int qx = 0; qx < n; ++qx) {
-                pa[(qy * n + qx) * BT] = v[qy][qx];
-                pa2[(qy * n + qx) * BT] = v2[qy][qx];
-            }
-    }
-    __syncthreads();
-    // ---- line phase as plane passes: the thread owns the yz-plane qx = pl --------------------------------------------
-    {
-        double* la = sA + (size_t)pl * BT + lane;    // + ((az*n + qy)*n)*BT
-        double* la2 = sA2 + (size_t)pl * BT + lane;
-        const double* lw = sWV + pl;                 // + (qz*n + qy)*n
-        // pass 1: U = Nz A
-#pragma unroll
-        for (int qy = 0; qy < n; ++qy) {
-#pragma unroll
-            for (int az = 0; az < n; ++az) t[az] = la[((az * n + qy) * n) * BT];
-            mat1d_eo<n>(prm.eoN, t, v[qy]);
-        }
-        // pass 2: T = (alpha WV) . U + (alpha kz wx wy) (Gz U), in place
-        const double kzwx = kz * prm.w[pl];
-#pragma unroll
-        for (int qy = 0; qy < n; ++qy) {
-            mat1d_eo<n>(prm.eoG, v[qy], o);
-            const double kzw = kzwx * prm.w[qy];
-#pragma unroll
-            for (int qz = 0; qz < n; ++qz) v[qy][qz] = fma(lw[(qz * n + qy) * n], v[qy][qz], kzw * o[qz]);
-        }
-        // pass 3: T += (alpha wz) . (Nz A2)
-#pragma unroll
-        for (int qy = 0; qy < n; ++qy) {
-#pragma unroll
-            for (int az = 0; az < n; ++az) t[az] = la2[((az * n + qy) * n) * BT];
-            mat1d_eo<n>(prm.eoN, t, o);
-#pragma unroll
-            for (int qz = 0; qz < n; ++qz) v[qy][qz] = fma(prm.aw[qz], o[qz], v[qy][qz]);
-        }
-        // pass 4: R = Nz^T T, back into the A field
-#pragma unroll
-        for (int qy = 0; qy < n; ++qy) {
-            mat1d_eo<n>(prm.eoNT, v[qy], o);
-#pragma unroll
-            for (int az = 0; az < n; ++az) la[((az * n + qy) * n) * BT] = o[az];
-        }
-    }
-    __syncthreads();
-    // ---- plane phase 2 ---------------------------------------------------------------------------------------------
-    const bool zterm = prm.Z != nullptr;
-    const bool own_pl = pl < P;
-    double* zbuf = sA2 + (size_t)pl * n * n * BT + lane;
-    double* xbuf = sA + (size_t)pl * n * n * BT + lane;
-    if (own_pl && zterm) {
-#pragma unroll
-        for (int ay = 0; ay < P; ++ay)
-#pragma unroll
-            for (int ax = 0; ax < P; ++ax) cp_async8(zbuf + (ay * n + ax) * BT, Zc + (ro[ay] + co[ax]), act);
-    }
-    cp_async_commit();
-#pragma unroll
-    for (int qy = 0; qy < n; ++qy)
-#pragma unroll
-        for (int qx = 0; qx < n; ++qx) v[qy][qx] = xbuf[(qy * n + qx) * BT];
-#pragma unroll
-    for (int qx = 0; qx < n; ++qx) {
-#pragma unroll
-        for (int q = 0; q < n; ++q) t[q] = v[q][qx];
-        mat1d_eo<n>(prm.eoNT, t, o);
-#pragma unroll
-        for (int a = 0; a < n; ++a) v[a][qx] = o[a];
-    }
-    if (own_pl) {
-#pragma unroll
-        for (int ay = 0; ay < P; ++ay)
-#pragma unroll
-            for (int ax = 0; ax < P; ++ax) cp_async8(xbuf + (ay * n + ax) * BT, Xc + (ro[ay] + co[ax]), act);
-    }
-    cp_async_commit();
-#pragma unroll
-    for (int ay = 0; ay < n; ++ay) {
-        mat1d_eo<n>(prm.eoNT, v[ay], o);
-#pragma unroll
-        for (int a = 0; a < n; ++a) v[ay][a] = o[a];
-    }
-    cp_async_wait_all();
-    if (act) {
-        const double ashift = -prm.alpha * (prm.c + (prm.eps ? prm.eps[j] : 0.0));
-        const double* ss = sS + pl * n * n;
-#pragma unroll
-        for (int ay = 0; ay < n; ++ay)
-#pragma unroll
-            for (int ax = 0; ax < n; ++ax) {
-                const double sc = ss[ay * n + ax];
-                double val = sc * v[ay][ax];
-                if (ax < P && ay < P) {
-                    if (own_pl && __double2hiint(sc) != 0) {  // owner of a free node adds the diagonal terms once
-                        val = fma(ashift, xbuf[(ay * n + ax) * BT], val);
-                        if (zterm) val = fma(prm.beta, zbuf[(ay * n + ax) * BT], val);
-                    }
-                }
-                atomicAdd(Yc + (ro[ay] + co[ax]), val);
-            }
-    }
-}
-
-template <int P, int BT, int MINB>
-cudaError_t launch_v4(const ApplyParams& prm, long long ncells, cudaStream_t st)
-{
-    constexpr int n = P + 1;
-    const size_t smem = ((size_t)2 * n * n * n * BT + 2 * n * n * n) * sizeof(double);
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_apply_v4<P, BT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
-    dim3 grid((unsigned)ncells, (unsigned)((prm.B + BT - 1) / BT)), block(BT, n);
-    k_apply_v4<P, BT, MINB><<<grid, block, smem, st>>>(prm);
-    return cudaGetLastError();
-}
-
 inline bool variant_supported(int p, int variant)
 {
     (void)p;
-    return variant >= 0 && variant <= 8;  // 5 = TMA generation (the default for even B), 1-4 legacy
-}
-
-template <int P, int BT>
-cudaError_t launch_v1(const ApplyParams& prm, long long ncells, cudaStream_t st)
-{
-    constexpr int n = P + 1;
-    const size_t smem = (size_t)2 * n * n * n * BT * sizeof(double);
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_apply_v1<P, BT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
-    dim3 grid((unsigned)ncells, (unsigned)((prm.B + BT - 1) / BT)), block(BT, n);
-    k_apply_v1<P, BT><<<grid, block, smem, st>>>(prm);
-    return cudaGetLastError();
+    return variant == 0 || variant == 3 || (variant >= 5 && variant <= 8);
 }
 
 // One fused operator step.  *nlaunch = kernels (and memsets) enqueued.
@@ -877,53 +335,16 @@ inline cudaError_t launch_apply(const ApplyParams& prm, int p, int variant, long
     cudaError_t e = cudaMemsetAsync(prm.Y, 0, (size_t)N * prm.B * sizeof(double), st);
     if (e != cudaSuccess) return e;
     *nlaunch = 1;  // kernels only; the zero-fill is a cudaMemsetAsync
-    // variant 4 addresses with 32-bit byte offsets from a per-cell base: one cell's node box times B must fit
-    const bool fits32 = (double)(p + 1) * (double)prm.NxNy * (double)prm.B * 8.0 < 4.0e9;
-    if (variant == 4 && fits32) {
-        switch (p) {
-            case 1: return launch_v4<1, 32, 8>(prm, ncells, st);
-            case 2: return launch_v4<2, 32, 6>(prm, ncells, st);
-            case 3: return launch_v4<3, 32, 4>(prm, ncells, st);
-            case 4: return launch_v4<4, 32, 3>(prm, ncells, st);
-            case 5: return launch_v4<5, 32, 1>(prm, ncells, st);
-            case 6: return launch_v4<6, 16, 2>(prm, ncells, st);
-            case 7: return launch_v4<7, 16, 1>(prm, ncells, st);
-            case 8: return launch_v4<8, 16, 1>(prm, ncells, st);
-        }
-    }
-    if (variant == 0 || variant == 3 || variant == 4) {
-        switch (p) {
-            case 1: return launch_v3<1, 32, 8>(prm, ncells, st);
-            case 2: return launch_v3<2, 32, 6>(prm, ncells, st);
-            case 3: return launch_v3<3, 32, 4>(prm, ncells, st);
-            case 4: return launch_v3<4, 32, 3>(prm, ncells, st);
-            case 5: return launch_v3<5, 32, 1>(prm, ncells, st);
-            case 6: return launch_v3<6, 16, 2>(prm, ncells, st);
-            case 7: return launch_v3<7, 16, 1>(prm, ncells, st);
-            case 8: return launch_v3<8, 16, 1>(prm, ncells, st);
-        }
-    }
-    if (variant == 2) {
-        switch (p) {
-            case 1: return launch_v2<1, 32, 8>(prm, ncells, st);
-            case 2: return launch_v2<2, 32, 6>(prm, ncells, st);
-            case 3: return launch_v2<3, 32, 4>(prm, ncells, st);
-            case 4: return launch_v2<4, 32, 3>(prm, ncells, st);
-            case 5: return launch_v2<5, 32, 1>(prm, ncells, st);
-            case 6: return launch_v2<6, 16, 2>(prm, ncells, st);
-            case 7: return launch_v2<7, 16, 1>(prm, ncells, st);
-            case 8: return launch_v2<8, 16, 1>(prm, ncells, st);
-        }
-    }
+    (void)variant;
     switch (p) {
-        case 1: return launch_v1<1, 32>(prm, ncells, st);
-        case 2: return launch_v1<2, 32>(prm, ncells, st);
-        case 3: return launch_v1<3, 32>(prm, ncells, st);
-        case 4: return launch_v1<4, 32>(prm, ncells, st);
-        case 5: return launch_v1<5, 32>(prm, ncells, st);
-        case 6: return launch_v1<6, 32>(prm, ncells, st);
-        case 7: return launch_v1<7, 16>(prm, ncells, st);
-        case 8: return launch_v1<8, 16>(prm, ncells, st);
+        case 1: return launch_v3<1, 32, 8>(prm, ncells, st);
+        case 2: return launch_v3<2, 32, 6>(prm, ncells, st);
+        case 3: return launch_v3<3, 32, 4>(prm, ncells, st);
+        case 4: return launch_v3<4, 32, 3>(prm, ncells, st);
+        case 5: return launch_v3<5, 32, 1>(prm, ncells, st);
+        case 6: return launch_v3<6, 16, 2>(prm, ncells, st);
+        case 7: return launch_v3<7, 16, 1>(prm, ncells, st);
+        case 8: return launch_v3<8, 16, 1>(prm, ncells, st);
     }
     return cudaErrorInvalidValue;
 }
