@@ -106,6 +106,12 @@ int fe_gram(fe_mesh* m, const double* A, const double* Bm, int B, double* C_host
  * l.223.  Psi, P: DEVICE N*B, must not overlap.  Synchronous. */
 int fe_add_subspace(fe_mesh* m, const double* Psi, const double* D_host, double* P, int B, void* cuda_stream);
 
+/* Electron density at the quadrature points (Eq. 4 l.73-77):  rho[e][q] = sum_j f[j] psi_j(x_q)^2 with
+ * psi_j = M^{-1/2} psi~_j (the API vectors are psi~ = M^{1/2} psi, Eq. 19; Dirichlet rows count as 0), in the layout of
+ * fe_set_potential's Vq (cells*n_q^3, cell-major, q = qx + n_q*(qy + n_q*qz)).  X: DEVICE N*B; f_dev: DEVICE B
+ * occupancies; rho_dev: DEVICE cells*n_q^3 doubles (overwritten).  Asynchronous on cuda_stream. */
+int fe_density(fe_mesh* m, const double* X, int B, const double* f_dev, double* rho_dev, void* cuda_stream);
+
 /* Kernel variant for experiments and tests: 0 = default (TMA generation when B is even and the blocks are 16-byte
  * aligned, else the legacy atomics kernel), 3 = legacy kernel always, 5..8 = launch shapes of the TMA kernel
  * (fe_apply_tma.cuh).  FE_ERR_INVALID if unknown. */

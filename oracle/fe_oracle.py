@@ -341,3 +341,26 @@ def minres_shifted(mesh, G, eps=None, maxit=200, tol=1e-10, Minv=None, nthreads=
         rel[j] = phibar / beta1
         itmax = max(itmax, itn)
     return X, rel, itmax
+
+
+def density(mesh, X, f):
+    """rho[e, q] = sum_j f_j psi_j(x_q)^2 at the Gauss points of every cell (Eq. 4, l.73-77), psi = M^{-1/2} psi~
+    with zero Dirichlet rows; psi_j(x_q) = sum_a Phi_a(x_q) psi_{j,a} written out with the Lagrange basis of Eq. 12."""
+    X = _f64(X)
+    p, n = mesh.p, mesh.p + 1
+    xg, _ = gll(p)
+    xq, _ = gauss(n)
+    L1 = np.array([[lagrange(xg, a, xq[q]) for a in range(n)] for q in range(n)])  # L1[q, a]
+    s = np.zeros(mesh.N)
+    free = mesh.mask().astype(bool)
+    s[free] = 1.0 / np.sqrt(mesh.mass()[free])
+    psi = X * s[:, None]
+    l2g = mesh.l2g()
+    rho = np.zeros((mesh.ncells, n ** 3))
+    fw = _f64(f)
+    for e in range(mesh.ncells):
+        loc = psi[l2g[e]].reshape(n, n, n, -1)  # [az, ay, ax, j]
+        val = np.einsum("ra,sb,tc,cbaj->rstj", L1, L1, L1, loc)  # [qx, qy, qz, j]: Phi_a = l_ax l_ay l_az
+        r = np.einsum("rstj,j->rst", val ** 2, fw)
+        rho[e] = r.transpose(2, 1, 0).reshape(-1)  # q = qx + n (qy + n qz)
+    return rho

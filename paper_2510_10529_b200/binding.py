@@ -13,7 +13,7 @@ _lib = None
 EXPORTS = (
     "fe_mesh_create", "fe_mesh_destroy", "fe_num_nodes", "fe_num_free", "fe_num_cells", "fe_nodes_per_cell",
     "fe_quad_per_cell", "fe_get_l2g", "fe_get_node_coords", "fe_get_quad_coords", "fe_get_mass",
-    "fe_get_dirichlet_mask", "fe_set_potential", "fe_apply_H", "cheb_filter", "fe_rayleigh_ritz", "fe_minres_shifted", "fe_add_subspace", "fe_gram",
+    "fe_get_dirichlet_mask", "fe_set_potential", "fe_apply_H", "cheb_filter", "fe_rayleigh_ritz", "fe_minres_shifted", "fe_add_subspace", "fe_gram", "fe_density",
     "fe_set_variant",
     "fe_launch_count", "fe_last_error",
 )
@@ -55,6 +55,7 @@ def load_library():
     L.fe_rayleigh_ritz.restype, L.fe_rayleigh_ritz.argtypes = C.c_int, [vp, vp, C.c_int, vp, vp, vp]
     L.fe_minres_shifted.restype = C.c_int
     L.fe_minres_shifted.argtypes = [vp, vp, vp, C.c_int, vp, C.c_int, C.c_double, C.c_int, vp, vp, vp, vp]
+    L.fe_density.restype, L.fe_density.argtypes = C.c_int, [vp, vp, C.c_int, vp, vp, vp]
     L.fe_gram.restype, L.fe_gram.argtypes = C.c_int, [vp, vp, vp, C.c_int, vp, vp]
     L.fe_add_subspace.restype, L.fe_add_subspace.argtypes = C.c_int, [vp, vp, vp, vp, C.c_int, vp]
     L.fe_set_variant.restype, L.fe_set_variant.argtypes = C.c_int, [vp, C.c_int]
@@ -207,6 +208,14 @@ def fe_minres_shifted(h, G, X, eps, maxit, tol, precondition, work, stream=None)
     return relres, iters.value
 
 
+def fe_density(h, X, f, rho, stream=None):
+    B = X.shape[1]
+    n = fe_num_cells(h) * fe_quad_per_cell(h)
+    _check(load_library().fe_density(h, _dev_ptr(X, "X"), B, _dev_ptr(f, "f", B), _dev_ptr(rho, "rho", n),
+                                     _stream(stream)))
+    return rho
+
+
 def fe_gram(h, A, Bm, stream=None):
     """A^T Bm as a numpy B x B array."""
     import numpy as np
@@ -290,6 +299,11 @@ class FEMesh:
         work = torch.empty(6 * G.numel(), dtype=torch.float64, device=G.device)
         relres, iters = fe_minres_shifted(self.h, G, X, eps, maxit, tol, precondition, work, stream)
         return X, relres, iters
+
+    def density(self, X, f, stream=None):
+        import torch
+        rho = torch.empty(self.ncells * self.nq3, dtype=torch.float64, device=X.device)
+        return fe_density(self.h, X, f, rho, stream)
 
     def gram(self, A, Bm, stream=None):
         return fe_gram(self.h, A, Bm, stream)

@@ -17,6 +17,7 @@
 #include <vector>
 
 #include "fe_apply_tma.cuh"
+#include "fe_density.cuh"
 #include "fe_minres.cuh"
 #include "fe_rr.cuh"
 #include "fe_kernels.cuh"
@@ -842,6 +843,26 @@ int fe_gram(fe_mesh* m, const double* A, const double* Bm, int B, double* C_host
     CUDA_TRY(launch_gram(A, Bm, m->N, B, m->d_small, m->sms, st));
     CUDA_TRY(cudaMemcpyAsync(C_host, m->d_small, bb * sizeof(double), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
+    m->launches += 1;
+    return FE_OK;
+}
+
+// ---- density at the quadrature points (NEXT-4; Eq. 4 l.73-77) ------------------------------------------------
+int fe_density(fe_mesh* m, const double* X, int B, const double* f_dev, double* rho_dev, void* cuda_stream)
+{
+    if (!m || !X || !f_dev || !rho_dev) return fail(FE_ERR_INVALID, "fe_density: NULL argument");
+    if (B < 1) return fail(FE_ERR_INVALID, "fe_density: B=%d < 1", B);
+    CUDA_TRY(cudaSetDevice(m->device));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    DensityParams prm;
+    memset(&prm, 0, sizeof(prm));
+    prm.X = X; prm.f = f_dev; prm.sm = m->d_sm; prm.rho = rho_dev;
+    prm.B = B; prm.cx = m->cx; prm.cy = m->cy; prm.cz = m->cz;
+    prm.Nx = m->Nx; prm.NxNy = m->Nx * m->Ny;
+    prm.eoN = m->eoN;
+    for (int q = 0; q < m->n; ++q) prm.iw[q] = 1.0 / std::sqrt(m->tab.gl_w[q]);
+    CUDA_TRY(cudaMemsetAsync(rho_dev, 0, (size_t)m->ncells * m->nc * sizeof(double), st));
+    CUDA_TRY(launch_density(prm, m->p, m->ncells, st));
     m->launches += 1;
     return FE_OK;
 }

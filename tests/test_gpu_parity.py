@@ -301,6 +301,21 @@ def test_adjoint_null_space_completion():
     assert np.linalg.norm(Pf - Pref) <= 1e-12 * np.linalg.norm(Pref)
 
 
+@pytest.mark.parametrize("p,B", [(1, 2), (2, 8), (3, 33), (4, 64), (6, 40), (8, 5)])
+def test_density_at_quadrature_points(p, B):
+    """fe_density (NEXT-4, Eq. 4) against the oracle's definition on the unequal 2x3x4 mesh: several vector tiles, a
+    ragged tail, data in the Dirichlet rows that must not contribute."""
+    import oracle
+    fe = _fe()
+    om = oracle.OracleMesh(*UNEQUAL, p)
+    gm = fe.FEMesh(*UNEQUAL, p)
+    X = workloads.random_block(700 + p, om.N, B)
+    f = 2.0 * workloads.uniform01(701 + p, 0, B)
+    rho_o = oracle.density(om, X, f).reshape(-1)
+    rho_g = gm.density(_dev(X), _dev(f)).cpu().numpy()
+    assert np.linalg.norm(rho_g - rho_o) <= 1e-12 * np.linalg.norm(rho_o)
+
+
 # ---- full BASELINE sizes: sampled rows ------------------------------------------------------------------------------
 def _sample_rows(w, count, seed):
     """Rows spread over cell interiors, faces, edges, vertices and the boundary."""

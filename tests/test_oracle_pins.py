@@ -416,6 +416,51 @@ def test_minres_against_dense_solves():
     assert np.max(np.abs(Psi.T @ Xs[free, 0])) <= 1e-7 * np.linalg.norm(xp)  # p_perp is orthogonal to the null vectors
 
 
+# ---- density at the quadrature points (Eq. 4) -----------------------------------------------------------------------
+def _bubble_fields(xyz, edges):
+    """Two polynomials of degree <= 3 per variable that vanish on the box surface (exactly representable at p >= 3)."""
+    (x0, x1), (y0, y1), (z0, z1) = [(e[0], e[-1]) for e in edges]
+    x, y, z = xyz[:, 0], xyz[:, 1], xyz[:, 2]
+    bub = (x - x0) * (x1 - x) * (y - y0) * (y1 - y) * (z - z0) * (z1 - z)
+    return np.stack([bub * (1.0 + 0.3 * x - 0.2 * y + 0.5 * z), bub * (0.7 - 0.4 * x * y + 0.1 * z)], axis=1)
+
+
+def test_density_polynomial_closed_form():
+    """Eq. 4: rho(x_q) = sum_j f_j psi_j(x_q)^2.  For psi in the FE space (polynomials of degree <= p per variable that
+    satisfy the Dirichlet condition) interpolation is exact, so the oracle must return f . psi(x_q)^2 evaluated from
+    the closed form at the quadrature coordinates; and int rho = sum_q J w_q rho_q integrates psi^2 exactly."""
+    m = oracle.OracleMesh(*UNEQUAL, 3)
+    psi_nodes = _bubble_fields(m.node_coords(), UNEQUAL)
+    X = psi_nodes * np.sqrt(m.mass())[:, None]  # psi~ = M^{1/2} psi (Eq. 19)
+    f = np.array([2.0, 0.5])
+    rho = oracle.density(m, X, f)
+    ref = (_bubble_fields(m.quad_coords(), UNEQUAL) ** 2) @ f
+    assert np.max(np.abs(rho.reshape(-1) - ref)) <= 1e-13 * np.max(np.abs(ref))
+    # the integral with p+1 Gauss points is exact for degree 2p+1 = 7 > 6: compare with the analytic integral of the
+    # first field's square computed by high-order 1-D Gauss rules on the whole box
+    xq, wq = np.polynomial.legendre.leggauss(12)
+    pts, wts = [], []
+    for e in UNEQUAL:
+        a, b = e[0], e[-1]
+        pts.append(0.5 * (b - a) * xq + 0.5 * (a + b))
+        wts.append(0.5 * (b - a) * wq)
+    Xg, Yg, Zg = np.meshgrid(*pts, indexing="ij")
+    Wg = wts[0][:, None, None] * wts[1][None, :, None] * wts[2][None, None, :]
+    grid = np.stack([Xg.ravel(), Yg.ravel(), Zg.ravel()], axis=1)
+    exact = ((_bubble_fields(grid, UNEQUAL) ** 2) @ f * Wg.ravel()).sum()
+    n = m.p + 1
+    gx, gw = oracle.gauss(n)
+    hx, hy, hz = (np.diff(e) for e in UNEQUAL)
+    cx, cy = len(hx), len(hy)
+    total = 0.0
+    for e in range(m.ncells):
+        ex, ey, ez = e % cx, (e // cx) % cy, e // (cx * cy)
+        J = hx[ex] * hy[ey] * hz[ez] / 8.0
+        w3 = (gw[None, None, :] * gw[None, :, None] * gw[:, None, None]).reshape(-1)  # q = qx + n(qy + n qz)
+        total += J * (w3 * rho[e]).sum()
+    assert abs(total - exact) <= 1e-12 * abs(exact)
+
+
 # ---- inputs module ------------------------------------------------------------------------------------------
 def test_inputs_generator():
     z = workloads.splitmix64(0, 0, 3)
