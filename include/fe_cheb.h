@@ -112,6 +112,13 @@ int fe_add_subspace(fe_mesh* m, const double* Psi, const double* D_host, double*
  * occupancies; rho_dev: DEVICE cells*n_q^3 doubles (overwritten).  Asynchronous on cuda_stream. */
 int fe_density(fe_mesh* m, const double* X, int B, const double* f_dev, double* rho_dev, void* cuda_stream);
 
+/* Spectral bounds for the filter window (reading R10; BASELINE.json config 1 "bounds from 20 Lanczos steps"): k Lanczos
+ * steps on H~ (free rows) from the start vector v0 (DEVICE, N doubles, Dirichlet rows ignored, normalised inside),
+ * no re-orthogonalisation.  out3_host (HOST, 3 doubles) = {theta_min, theta_max, beta_k} of the k x k tridiagonal
+ * matrix; the caller takes b = theta_max + beta_k, a0 = theta_min.  work: DEVICE, 3*N doubles.  1 <= k <= 128.
+ * Synchronous (two inner products per step come back to the host). */
+int fe_lanczos_bounds(fe_mesh* m, const double* v0_dev, int k, double* out3_host, double* work, void* cuda_stream);
+
 /* Kernel variant for experiments and tests: 0 = default (TMA generation when B is even and the blocks are 16-byte
  * aligned, else the legacy atomics kernel), 3 = legacy kernel always, 5..8 = launch shapes of the TMA kernel
  * (fe_apply_tma.cuh).  FE_ERR_INVALID if unknown. */

@@ -13,7 +13,7 @@ _lib = None
 EXPORTS = (
     "fe_mesh_create", "fe_mesh_destroy", "fe_num_nodes", "fe_num_free", "fe_num_cells", "fe_nodes_per_cell",
     "fe_quad_per_cell", "fe_get_l2g", "fe_get_node_coords", "fe_get_quad_coords", "fe_get_mass",
-    "fe_get_dirichlet_mask", "fe_set_potential", "fe_apply_H", "cheb_filter", "fe_rayleigh_ritz", "fe_minres_shifted", "fe_add_subspace", "fe_gram", "fe_density",
+    "fe_get_dirichlet_mask", "fe_set_potential", "fe_apply_H", "cheb_filter", "fe_rayleigh_ritz", "fe_minres_shifted", "fe_add_subspace", "fe_gram", "fe_density", "fe_lanczos_bounds",
     "fe_set_variant",
     "fe_launch_count", "fe_last_error",
 )
@@ -56,6 +56,7 @@ def load_library():
     L.fe_minres_shifted.restype = C.c_int
     L.fe_minres_shifted.argtypes = [vp, vp, vp, C.c_int, vp, C.c_int, C.c_double, C.c_int, vp, vp, vp, vp]
     L.fe_density.restype, L.fe_density.argtypes = C.c_int, [vp, vp, C.c_int, vp, vp, vp]
+    L.fe_lanczos_bounds.restype, L.fe_lanczos_bounds.argtypes = C.c_int, [vp, vp, C.c_int, vp, vp, vp]
     L.fe_gram.restype, L.fe_gram.argtypes = C.c_int, [vp, vp, vp, C.c_int, vp, vp]
     L.fe_add_subspace.restype, L.fe_add_subspace.argtypes = C.c_int, [vp, vp, vp, vp, C.c_int, vp]
     L.fe_set_variant.restype, L.fe_set_variant.argtypes = C.c_int, [vp, C.c_int]
@@ -216,6 +217,18 @@ def fe_density(h, X, f, rho, stream=None):
     return rho
 
 
+def fe_lanczos_bounds(h, v0, k=20, stream=None):
+    """(theta_min, theta_max, beta_k) after k Lanczos steps from the device vector v0 (N)."""
+    import numpy as np
+    import torch
+    N = fe_num_nodes(h)
+    out = np.empty(3, dtype=np.float64)
+    work = torch.empty(3 * N, dtype=torch.float64, device=v0.device)
+    _check(load_library().fe_lanczos_bounds(h, _dev_ptr(v0, "v0", N), int(k), out.ctypes.data_as(C.c_void_p),
+                                            _dev_ptr(work, "work"), _stream(stream)))
+    return float(out[0]), float(out[1]), float(out[2])
+
+
 def fe_gram(h, A, Bm, stream=None):
     """A^T Bm as a numpy B x B array."""
     import numpy as np
@@ -304,6 +317,9 @@ class FEMesh:
         import torch
         rho = torch.empty(self.ncells * self.nq3, dtype=torch.float64, device=X.device)
         return fe_density(self.h, X, f, rho, stream)
+
+    def lanczos_bounds(self, v0, k=20, stream=None):
+        return fe_lanczos_bounds(self.h, v0, k, stream)
 
     def gram(self, A, Bm, stream=None):
         return fe_gram(self.h, A, Bm, stream)

@@ -866,3 +866,91 @@ int fe_density(fe_mesh* m, const double* X, int B, const double* f_dev, double* 
     m->launches += 1;
     return FE_OK;
 }
+
+// ---- spectral bounds for the filter: k Lanczos steps on H~ (reading R10; BASELINE config 1 "bounds from 20 Lanczos
+//      steps").  Single vector: the applies take the legacy kernel (B = 1), the vector updates are three tiny kernels.
+__global__ void k_lz_dot(const double* __restrict__ a, const double* __restrict__ b, long long n, double* out)
+{
+    double s = 0.0;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) s = fma(a[i], b[i], s);
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    __shared__ double red[8];
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t += red[w];
+        atomicAdd(out, t);
+    }
+}
+// w <- (w - a v - b u) * scale_w ;  optional masked copy-in: v0 -> v with Dirichlet rows zeroed
+__global__ void k_lz_update(double* __restrict__ w, const double* __restrict__ v, const double* __restrict__ u, long long n,
+                            double a, double b)
+{
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        w[i] = w[i] - a * v[i] - b * u[i];
+}
+__global__ void k_lz_scale(double* __restrict__ dst, const double* __restrict__ src, const double* __restrict__ mask,
+                           long long n, double s)
+{
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        dst[i] = (mask && mask[i] == 0.0) ? 0.0 : s * src[i];
+}
+
+static int lz_dot(fe_mesh* m, const double* a, const double* b, double* out_host, cudaStream_t st)
+{
+    CUDA_TRY(cudaMemsetAsync(m->d_small, 0, sizeof(double), st));
+    k_lz_dot<<<m->sms * 4, 256, 0, st>>>(a, b, m->N, m->d_small);
+    CUDA_TRY(cudaMemcpyAsync(out_host, m->d_small, sizeof(double), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    m->launches += 1;
+    return FE_OK;
+}
+
+int fe_lanczos_bounds(fe_mesh* m, const double* v0_dev, int k, double* out3_host, double* work, void* cuda_stream)
+{
+    if (!m || !v0_dev || !out3_host || !work) return fail(FE_ERR_INVALID, "fe_lanczos_bounds: NULL argument");
+    if (k < 1 || k > 128) return fail(FE_ERR_INVALID, "fe_lanczos_bounds: k=%d outside 1..128", k);
+    if (!m->have_V) return fail(FE_ERR_STATE, "fe_lanczos_bounds: call fe_set_potential first");
+    CUDA_TRY(cudaSetDevice(m->device));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (!m->d_small) CUDA_TRY(cudaMalloc((void**)&m->d_small, 2 * 128 * 128 * sizeof(double)));
+    const long long N = m->N;
+    const int grid = m->sms * 4;
+    double *v = work, *u = work + N, *w = work + 2 * N;  // v_j, v_{j-1}, w
+    int rc;
+    double nrm2 = 0.0;
+    k_lz_scale<<<grid, 256, 0, st>>>(v, v0_dev, m->d_sm, N, 1.0);  // Dirichlet rows do not take part (R5)
+    if ((rc = lz_dot(m, v, v, &nrm2, st))) return rc;
+    if (!(nrm2 > 0.0)) return fail(FE_ERR_INVALID, "fe_lanczos_bounds: start vector is zero on the free rows");
+    k_lz_scale<<<grid, 256, 0, st>>>(v, v, nullptr, N, 1.0 / std::sqrt(nrm2));
+    CUDA_TRY(cudaMemsetAsync(u, 0, (size_t)N * sizeof(double), st));
+    std::vector<double> al, be;
+    double beta = 0.0;
+    for (int j = 0; j < k; ++j) {
+        if ((rc = fe_apply_H(m, v, w, 1, nullptr, cuda_stream))) return rc;
+        double alpha = 0.0, b2 = 0.0;
+        if ((rc = lz_dot(m, w, v, &alpha, st))) return rc;
+        k_lz_update<<<grid, 256, 0, st>>>(w, v, u, N, alpha, beta);
+        if ((rc = lz_dot(m, w, w, &b2, st))) return rc;
+        beta = std::sqrt(b2);
+        al.push_back(alpha);
+        be.push_back(beta);
+        m->launches += 2;
+        if (beta == 0.0) break;
+        k_lz_scale<<<grid, 256, 0, st>>>(w, w, nullptr, N, 1.0 / beta);
+        double* t = u; u = v; v = w; w = t;  // v_{j-1} <- v_j <- w / beta
+    }
+    CUDA_TRY(cudaGetLastError());
+    const int kk = (int)al.size();
+    std::vector<double> T((size_t)kk * kk, 0.0), th, V;
+    for (int i = 0; i < kk; ++i) {
+        T[(size_t)i * kk + i] = al[i];
+        if (i + 1 < kk) T[(size_t)i * kk + i + 1] = T[(size_t)(i + 1) * kk + i] = be[i];
+    }
+    sym_eigh(T, kk, th, V);
+    out3_host[0] = th.front();
+    out3_host[1] = th.back();
+    out3_host[2] = be.back();
+    return FE_OK;
+}

@@ -316,6 +316,35 @@ def test_density_at_quadrature_points(p, B):
     assert np.linalg.norm(rho_g - rho_o) <= 1e-12 * np.linalg.norm(rho_o)
 
 
+def test_device_lanczos_bounds_and_chfsi_cycles():
+    """fe_lanczos_bounds against the oracle's 20-step Lanczos (R10), then BASELINE config 2's recipe end to end on the
+    device — bounds, five filter + Rayleigh-Ritz cycles (R20) — against the same cycles on the oracle: Ritz values of
+    the final cycle <= 1e-9 (R16)."""
+    import oracle
+    w = workloads.reduced(2, 4)
+    om, gm = _pair((w.xe, w.ye, w.ze), w.p, w.V)
+    mask = om.mask()
+    v0 = workloads.normal(3400, om.N)
+    lo_o, hi_o, be_o = oracle.lanczos_bounds(om, v0, 20)
+    lo_g, hi_g, be_g = gm.lanczos_bounds(_dev(v0), 20)
+    scale = max(abs(hi_o), 1.0)
+    assert abs(lo_g - lo_o) <= 1e-8 * scale and abs(hi_g - hi_o) <= 1e-8 * scale and abs(be_g - be_o) <= 1e-7 * scale
+    B = 16
+    Xo = workloads.random_block(w.x_seed, om.N, B, mask)
+    Xg = _dev(Xo)
+    bo, a0o = hi_o + be_o, lo_o
+    ao = a0o + 0.1 * (bo - a0o)
+    bg, a0g = hi_g + be_g, lo_g
+    ag = a0g + 0.1 * (bg - a0g)
+    for cycle in range(5):
+        theta_o, Xo, _ = oracle.rayleigh_ritz(om, om.filter(Xo, w.m, ao, bo, a0o))
+        gm.cheb_filter(Xg, w.m, ag, bg, a0g)
+        theta_g = gm.rayleigh_ritz(Xg)
+        ao, a0o = theta_o[-1], theta_o[0]
+        ag, a0g = theta_g[-1], theta_g[0]
+    assert np.max(np.abs(theta_g - theta_o) / np.maximum(1.0, np.abs(theta_o))) <= 1e-9
+
+
 # ---- full BASELINE sizes: sampled rows ------------------------------------------------------------------------------
 def _sample_rows(w, count, seed):
     """Rows spread over cell interiors, faces, edges, vertices and the boundary."""
