@@ -5,7 +5,8 @@
 //
 // Unit of work = one cell x BT vectors (one CTA per unit, or a persistent CTA walking units).  a1 (gather) is ONE
 // cp.async.bulk.tensor load of the cell's n x n x n x BT box of X (the layout of PAPER.md l.233-235 makes the block a
-// 4-D tensor (j, gx, gy, gz)); a3 (scatter) is one cp.reduce.async.bulk.tensor .add per nodal plane, so no thread computes a global address or issues an atomic.
+// 4-D tensor (j, gx, gy, gz)); a3 (scatter) is one cp.reduce.async.bulk.tensor .add per nodal plane, so no thread
+// computes a global address or issues an atomic.
 // The recurrence terms of the Chebyshev step (l.208-210; R7) need no read of Y_{k-1} at all: step k-1 stores
 // beta_k Y_{k-1} into the buffer that becomes Y_{k+1} (the "pre-initialisation"), and step k adds
 // kappa_j Y_k = -alpha (c + eps_j) Y_k from the owner cell of each node plus alpha s_g sum_e yhat_e.
