@@ -27,7 +27,8 @@ namespace fecheb {
 
 struct TmaParams {
     CUtensorMap mXn;   // X : box (BT,n,n,n), load
-    CUtensorMap mYn1;  // Y : box (BT,n,n,1), reduce-add
+    CUtensorMap mYh1;  // Y : box (BT,n,ceil(n/2),1), reduce-add of the first rows of an output plane
+    CUtensorMap mYh2;  // Y : box (BT,n,floor(n/2),1), reduce-add of the remaining rows
     CUtensorMap mYp1;  // Y : box (BT,p,p,1), reduce-add of the owner term kappa_j X
     CUtensorMap mWp1;  // W : box (BT,p,p,1), store of beta' X
     const double* eps;
@@ -317,16 +318,28 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
         for (int a = 0; a < n; ++a) v[a][qx] = o[a];
     }
     const double* sout_pl = sOut + pl * n * NP;
+    constexpr int H1 = (n + 1) / 2;  // the plane leaves in two bulk reduce-adds: the first overlaps the remaining rows
 #pragma unroll
     for (int ay = 0; ay < n; ++ay) {
         mat1d_eo<n>(prm.eoNTa, v[ay], o);
 #pragma unroll
         for (int ax = 0; ax < n; ++ax) pB[(ay * n + ax) * BT] = sout_pl[ay * NP + ax] * o[ax];
+        if (ay == H1 - 1 && H1 < n) {
+            fence_async_smem();
+            __syncwarp();
+            if (lane == 0) {
+                tma_reduce_add4(&prm.mYh1, pB, j0, gx0, gy0, gz0 + pl);
+                bulk_commit();
+            }
+        }
     }
     fence_async_smem();
     __syncwarp();
     if (lane == 0) {
-        tma_reduce_add4(&prm.mYn1, pB, j0, gx0, gy0, gz0 + pl);
+        if (H1 < n)
+            tma_reduce_add4(&prm.mYh2, pB + (size_t)H1 * n * BT, j0, gx0, gy0 + H1, gz0 + pl);
+        else
+            tma_reduce_add4(&prm.mYh1, pB, j0, gx0, gy0, gz0 + pl);
         bulk_commit();
     }
     if (!PERSIST) break;

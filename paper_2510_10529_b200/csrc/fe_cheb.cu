@@ -384,7 +384,7 @@ static int make_map(CUtensorMap* out, const fe_mesh* m, const double* base, int 
 
 // the three views of one block the TMA kernel uses
 struct BlockMaps {
-    CUtensorMap n3, n1, p1;
+    CUtensorMap n3, h1, h2, p1;  // tile load; the two row halves of an output plane; owner sub-plane
 };
 
 static int make_block_maps(BlockMaps* bm, const fe_mesh* m, const double* base, int B)
@@ -392,7 +392,8 @@ static int make_block_maps(BlockMaps* bm, const fe_mesh* m, const double* base, 
     const int bt = tma_bt(m->p, m->variant, B), n = m->n, p = m->p;
     int rc;
     if ((rc = make_map(&bm->n3, m, base, B, bt, n, n, n))) return rc;
-    if ((rc = make_map(&bm->n1, m, base, B, bt, n, n, 1))) return rc;
+    if ((rc = make_map(&bm->h1, m, base, B, bt, n, (n + 1) / 2, 1))) return rc;
+    if ((rc = make_map(&bm->h2, m, base, B, bt, n, n / 2 > 0 ? n / 2 : 1, 1))) return rc;
     return make_map(&bm->p1, m, base, B, bt, p, p, 1);
 }
 
@@ -418,7 +419,7 @@ static int tma_step(fe_mesh* m, const BlockMaps& X, const BlockMaps& Y, const Bl
 {
     TmaParams prm;
     fill_tma_params(m, &prm, B);
-    prm.mXn = X.n3; prm.mYn1 = Y.n1; prm.mYp1 = Y.p1; prm.mWp1 = W ? W->p1 : Y.p1;
+    prm.mXn = X.n3; prm.mYh1 = Y.h1; prm.mYh2 = Y.h2; prm.mYp1 = Y.p1; prm.mWp1 = W ? W->p1 : Y.p1;
     prm.eps = eps; prm.alpha = alpha; prm.c = c; prm.owner = owner ? 1 : 0;
     prm.preinit = W ? 1 : 0; prm.beta_next = beta_next;
     prm.eoNTa = m->eoNT;
