@@ -79,11 +79,6 @@ __device__ __forceinline__ void tma_store4(const CUtensorMap* m, const void* src
     asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.tile.bulk_group [%0, {%2,%3,%4,%5}], [%1];"
                  ::"l"(m), "r"(smem_u32(src)), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
 }
-__device__ __forceinline__ void tma_prefetch_l2(const CUtensorMap* m, int c0, int c1, int c2, int c3)
-{
-    asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1,%2,%3,%4}];"
-                 ::"l"(m), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
-}
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
@@ -146,11 +141,6 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
     if (prm.owner) {
         const int j = j0 + lane;
         kappa = -prm.alpha * (prm.c + ((prm.eps && j < prm.B) ? prm.eps[j] : 0.0));
-    }
-    if (PERSIST && tid == 0 && u + gridDim.x < nunits) {  // pull the next unit's X tile into L2 a whole unit ahead
-        const long long un = u + gridDim.x;
-        const int cn = (int)(un / nbt), nx = cn % prm.cx, ny = (cn / prm.cx) % prm.cy, nz = cn / (prm.cx * prm.cy);
-        tma_prefetch_l2(&prm.mXn, (int)(un % nbt) * BT, nx * P, ny * P, nz * P);
     }
     if (lane == 0) bulk_wait_read0();  // the previous unit's reduce-add has read its source (bufB)
     __syncwarp();
