@@ -298,13 +298,7 @@ static void fill_params(const fe_mesh* m, ApplyParams* prm)
     prm->cx = m->cx; prm->cy = m->cy; prm->cz = m->cz;
     prm->Nx = m->Nx; prm->NxNy = m->Nx * m->Ny;
     const int n = m->n;
-    for (int q = 0; q < n; ++q) {
-        prm->w[q] = m->tab.gl_w[q];
-        for (int a = 0; a < n; ++a) {
-            prm->N[q * n + a] = m->tab.N[q * n + a];
-            prm->G[q * n + a] = m->tab.G[q * n + a];
-        }
-    }
+    for (int q = 0; q < n; ++q) prm->w[q] = m->tab.gl_w[q];
     make_eo(m->tab.N, n, false, &prm->eoN);
     make_eo(m->tab.N, n, true, &prm->eoNT);
     make_eo(m->tab.G, n, false, &prm->eoG);

@@ -39,7 +39,7 @@ struct ApplyParams {
     int B, cx, cy, cz;
     long long Nx, NxNy;
     double alpha, beta, c;
-    double N[81], G[81], w[9];
+    double w[9];  // Gauss weights
     EOTab eoN, eoNT, eoG;  // even-odd split of N, N^T and G (all centro-symmetric: GLL and Gauss points are symmetric)
 };
 
