@@ -9,6 +9,8 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <cstdint>
+
 namespace fecheb {
 
 constexpr int kRRThreads = 256;  // 16 x 16 threads, each owning a T x T block of the B x B matrix
@@ -109,11 +111,193 @@ __global__ void __launch_bounds__(kRRThreads) k_rightmul(const double* Y, const 
     }
 }
 
+// ---- fast paths for even B: 16-byte cp.async staging into a two-stage ring, 128-bit shared-memory reads ------------------
+__device__ __forceinline__ void rr_cp16(void* dst, const void* src, bool valid)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(dst);
+    const int sz = valid ? 16 : 0;  // src-size 0 zero-fills the 16 destination bytes
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(src), "r"(sz) : "memory");
+}
+__device__ __forceinline__ void rr_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int K>
+__device__ __forceinline__ void rr_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(K) : "memory"); }
+
+// thread t of 16 owns the index pairs {2t + 32m, 2t + 32m + 1 : m < T/2}: 16-byte reads, conflict-free across the 16
+__device__ __forceinline__ int rr_own(int t, int k) { return 2 * t + 32 * (k >> 1) + (k & 1); }
+
+// stage `rows` rows of a node-major block (pitch B) into smem rows of pitch BP; rows beyond N are zero-filled
+__device__ __forceinline__ void rr_stage(double* dst, const double* src, long long r0, int rows_tile, long long N, int B, int BP)
+{
+    const int chunks = B / 2;
+    for (int i = threadIdx.x; i < rows_tile * chunks; i += kRRThreads) {
+        const int r = i / chunks, c = i - r * chunks;
+        const bool ok = r0 + r < N;
+        rr_cp16(dst + r * BP + 2 * c, src + (ok ? (r0 + r) * B + 2 * c : 0), ok);
+    }
+}
+
+template <int T>
+__global__ void __launch_bounds__(kRRThreads) k_gram2(const double* __restrict__ A, const double* __restrict__ Bm,
+                                                      long long N, int B, double* __restrict__ C)
+{
+    constexpr int BP = 16 * T, R = kRRRows;
+    extern __shared__ __align__(16) double sm[];
+    const bool same = (A == Bm);
+    double* sA = sm;                               // [2][R][BP]
+    double* sB = same ? sm : sm + 2 * R * BP;      // [2][R][BP]
+    const int ti = threadIdx.x / 16, tj = threadIdx.x % 16;
+    for (int i = threadIdx.x; i < (same ? 2 : 4) * R * BP; i += kRRThreads) sm[i] = 0.0;  // the pad columns stay 0
+    __syncthreads();
+    double acc[T][T];
+#pragma unroll
+    for (int a = 0; a < T; ++a)
+#pragma unroll
+        for (int b = 0; b < T; ++b) acc[a][b] = 0.0;
+    const long long ntiles = (N + R - 1) / R;
+    long long tile = blockIdx.x;
+    if (tile < ntiles) {
+        rr_stage(sA, A, tile * R, R, N, B, BP);
+        if (!same) rr_stage(sB, Bm, tile * R, R, N, B, BP);
+    }
+    rr_commit();
+    int st = 0;
+    for (; tile < ntiles; tile += gridDim.x, st ^= 1) {
+        const long long nxt = tile + gridDim.x;
+        if (nxt < ntiles) {
+            rr_stage(sA + (st ^ 1) * R * BP, A, nxt * R, R, N, B, BP);
+            if (!same) rr_stage(sB + (st ^ 1) * R * BP, Bm, nxt * R, R, N, B, BP);
+        }
+        rr_commit();
+        rr_wait<1>();
+        __syncthreads();
+        const double* pa = sA + st * R * BP;
+        const double* pb = sB + st * R * BP;
+#pragma unroll 4
+        for (int r = 0; r < R; ++r) {
+            double a[T], b[T];
+#pragma unroll
+            for (int k = 0; k < T; k += 2) {
+                const double2 va = *reinterpret_cast<const double2*>(pa + r * BP + rr_own(ti, k));
+                const double2 vb = *reinterpret_cast<const double2*>(pb + r * BP + rr_own(tj, k));
+                a[k] = va.x; a[k + 1] = va.y; b[k] = vb.x; b[k + 1] = vb.y;
+            }
+#pragma unroll
+            for (int x = 0; x < T; ++x)
+#pragma unroll
+                for (int y = 0; y < T; ++y) acc[x][y] = fma(a[x], b[y], acc[x][y]);
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int x = 0; x < T; ++x)
+#pragma unroll
+        for (int y = 0; y < T; ++y) {
+            const int i = rr_own(ti, x), j = rr_own(tj, y);
+            if (i < B && j < B) atomicAdd(C + (size_t)i * B + j, acc[x][y]);
+        }
+}
+
+// RT rows per thread (tile of 16*RT rows), T columns per thread; the B x B factor stays in shared memory
+template <int T, int RT>
+__global__ void __launch_bounds__(kRRThreads) k_rightmul2(const double* Y, const double* __restrict__ Rm, double* Out,
+                                                          int accumulate, long long N, int B)
+{
+    constexpr int BP = 16 * T, R = 16 * RT;
+    extern __shared__ __align__(16) double sm[];
+    double* sR = sm;                 // [B][BP]
+    double* sY = sm + (size_t)B * BP;  // [2][R][BP]
+    const int ti = threadIdx.x / 16, tj = threadIdx.x % 16;
+    for (int i = threadIdx.x; i < B * BP + 2 * R * BP; i += kRRThreads) sm[i] = 0.0;
+    __syncthreads();
+    for (int i = threadIdx.x; i < B * B; i += kRRThreads) sR[(i / B) * BP + (i % B)] = Rm[i];
+    const long long ntiles = (N + R - 1) / R;
+    long long tile = blockIdx.x;
+    if (tile < ntiles) rr_stage(sY, Y, tile * R, R, N, B, BP);
+    rr_commit();
+    int st = 0;
+    for (; tile < ntiles; tile += gridDim.x, st ^= 1) {
+        const long long nxt = tile + gridDim.x;
+        if (nxt < ntiles) rr_stage(sY + (st ^ 1) * R * BP, Y, nxt * R, R, N, B, BP);
+        rr_commit();
+        rr_wait<1>();
+        __syncthreads();
+        const double* py = sY + st * R * BP;
+        double acc[RT][T];
+#pragma unroll
+        for (int a = 0; a < RT; ++a)
+#pragma unroll
+            for (int b = 0; b < T; ++b) acc[a][b] = 0.0;
+#pragma unroll 2
+        for (int i = 0; i < B; i += 2) {  // B is even
+            double2 y[RT];
+#pragma unroll
+            for (int m = 0; m < RT; ++m) y[m] = *reinterpret_cast<const double2*>(py + (ti + 16 * m) * BP + i);
+#pragma unroll
+            for (int k = 0; k < T; k += 2) {
+                const double2 r0 = *reinterpret_cast<const double2*>(sR + i * BP + rr_own(tj, k));
+                const double2 r1 = *reinterpret_cast<const double2*>(sR + (i + 1) * BP + rr_own(tj, k));
+#pragma unroll
+                for (int m = 0; m < RT; ++m) {
+                    acc[m][k] = fma(y[m].x, r0.x, acc[m][k]);
+                    acc[m][k + 1] = fma(y[m].x, r0.y, acc[m][k + 1]);
+                    acc[m][k] = fma(y[m].y, r1.x, acc[m][k]);
+                    acc[m][k + 1] = fma(y[m].y, r1.y, acc[m][k + 1]);
+                }
+            }
+        }
+        const long long r0g = tile * R;
+#pragma unroll
+        for (int m = 0; m < RT; ++m) {
+            const long long r = r0g + ti + 16 * m;
+            if (r < N) {
+#pragma unroll
+                for (int k = 0; k < T; k += 2) {
+                    const int j = rr_own(tj, k);
+                    if (j < B) {  // j even and B even: the pair is inside
+                        double2 o = make_double2(acc[m][k], acc[m][k + 1]);
+                        double2* dst = reinterpret_cast<double2*>(Out + r * B + j);
+                        if (accumulate) { const double2 old = *dst; o.x += old.x; o.y += old.y; }
+                        *dst = o;
+                    }
+                }
+            }
+        }
+        __syncthreads();
+    }
+}
+
+template <int T>
+cudaError_t launch_gram2(const double* A, const double* Bm, long long N, int B, double* C, int sms, cudaStream_t st)
+{
+    const size_t smem = (size_t)(A == Bm ? 2 : 4) * kRRRows * 16 * T * sizeof(double);
+    cudaError_t e = cudaFuncSetAttribute(k_gram2<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * kRRRows * 16 * T * 8);
+    if (e != cudaSuccess) return e;
+    k_gram2<T><<<sms * 2, kRRThreads, smem, st>>>(A, Bm, N, B, C);
+    return cudaGetLastError();
+}
+
+template <int T, int RT>
+cudaError_t launch_rightmul2(const double* Y, const double* R, double* Out, int accumulate, long long N, int B, int sms,
+                             cudaStream_t st)
+{
+    const size_t smem = ((size_t)B * 16 * T + (size_t)2 * 16 * RT * 16 * T) * sizeof(double);
+    cudaError_t e = cudaFuncSetAttribute(k_rightmul2<T, RT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_rightmul2<T, RT><<<sms * (smem > 100 * 1024 ? 1 : 2), kRRThreads, smem, st>>>(Y, R, Out, accumulate, N, B);
+    return cudaGetLastError();
+}
+
 inline cudaError_t launch_gram(const double* A, const double* Bm, long long N, int B, double* C, int sms, cudaStream_t st)
 {
     const size_t smem = (size_t)2 * kRRRows * B * sizeof(double);
     const int T = (B + 15) / 16;
     if (T > 8) return cudaErrorInvalidValue;
+    if (B % 2 == 0 && (((uintptr_t)A | (uintptr_t)Bm) & 15) == 0) {  // even B, 16-byte aligned rows: the fast path
+        if (T <= 2) return launch_gram2<2>(A, Bm, N, B, C, sms, st);
+        if (T <= 4) return launch_gram2<4>(A, Bm, N, B, C, sms, st);
+        if (T <= 6) return launch_gram2<6>(A, Bm, N, B, C, sms, st);
+        return launch_gram2<8>(A, Bm, N, B, C, sms, st);
+    }
     static bool configured = false;
     if (!configured) {
         cudaFuncSetAttribute(k_gram<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * kRRRows * 128 * 8);
@@ -133,6 +317,12 @@ inline cudaError_t launch_rightmul(const double* Y, const double* R, double* Out
     const size_t smem = ((size_t)B * B + (size_t)kRRRows * (B + 1)) * sizeof(double);
     const int T = (B + 15) / 16;
     if (T > 8) return cudaErrorInvalidValue;
+    if (B % 2 == 0 && (((uintptr_t)Y | (uintptr_t)Out) & 15) == 0) {
+        if (T <= 2) return launch_rightmul2<2, 4>(Y, R, Out, accumulate, N, B, sms, st);
+        if (T <= 4) return launch_rightmul2<4, 4>(Y, R, Out, accumulate, N, B, sms, st);
+        if (T <= 6) return launch_rightmul2<6, 2>(Y, R, Out, accumulate, N, B, sms, st);
+        return launch_rightmul2<8, 2>(Y, R, Out, accumulate, N, B, sms, st);
+    }
     static bool configured = false;
     if (!configured) {
         const int mx = (128 * 128 + kRRRows * 129) * 8;
