@@ -203,7 +203,7 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
         if (issuer) bulk_wait_read0();
         __syncwarp();
     }
-    if constexpr (n >= 8) {
+    if constexpr (n >= 7) {
         // large planes: park A in shared memory first and re-read its columns for the y stiffness, so that only one
         // plane (plus a line) is live in registers instead of two
 #pragma unroll
