@@ -7,7 +7,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.path.join(_HERE, "libfecheb.so")
+_SO = os.environ.get("FECHEB_LIB") or os.path.join(_HERE, "libfecheb.so")  # FECHEB_LIB: A/B builds of the library
 _lib = None
 
 EXPORTS = (
