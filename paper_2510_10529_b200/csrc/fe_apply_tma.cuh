@@ -390,7 +390,10 @@ inline cudaError_t launch_apply_tma(const TmaParams& prm, int p, long long ncell
                                     int variant, int sms)
 {
     const bool wide6 = tma_wide6(p, variant, prm.B);
-    if (!(variant == 7 || variant == 8 || (variant == 0 && wide6))) sms = 0;
+    // default: persistent wherever only one CTA fits an SM (p = 5, 7, 8 and the 32-wide p = 6 shape): nothing else
+    // would hide the tile latency there; with several CTAs per SM one CTA per unit measured faster (p <= 4)
+    const bool one_cta = wide6 || p == 5 || p >= 7;
+    if (!(variant == 7 || variant == 8 || (variant == 0 && one_cta))) sms = 0;
     if (wide6) return launch_tma<6, 32, 1>(prm, ncells, first, st, sms);
     switch (p) {
         case 1: return launch_tma<1, 32, 8>(prm, ncells, first, st, sms);
