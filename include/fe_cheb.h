@@ -75,6 +75,13 @@ int fe_apply_H(fe_mesh* m, const double* X, double* Y, int B, const double* eps_
 int cheb_filter(fe_mesh* m, double* X, int B, int deg, double a, double b, double a0, double* work,
                 void* cuda_stream);
 
+/* The same filter end to end from a HOST block (N*B doubles, X[a*B+j], filtered in place; pinned memory makes the
+ * copies asynchronous): host->device copy, cheb_filter, device->host copy.  Columns are independent, so for B a
+ * multiple of 32 (B > 32) chunks of 32 columns are pipelined on two internal streams and the PCIe transfers of one
+ * chunk overlap the filter of the other.  The device staging (3*N*min(B,64) doubles) lives in the handle.
+ * SYNCHRONOUS: returns when X_host holds the result.  This is the call bench.py's `e2e` times. */
+int cheb_filter_host(fe_mesh* m, double* X_host, int B, int deg, double a, double b, double a0);
+
 /* Rayleigh-Ritz step of ChFSI in span(Y) (Eq. 23-24 l.210-219; R8: H~_Y = Y^T H~ Y; R9: the Cholesky of Y^T Y is
  * done twice, CholQR2):  S = Y^T Y = L L^T, Q = Y L^{-T} (twice);  G = Q^T H~ Q;  G v = theta v;  Y <- Q V.
  * Y: DEVICE, N*B doubles, in: filtered block (Dirichlet rows ignored), out: Ritz vectors (orthonormal columns, Ritz

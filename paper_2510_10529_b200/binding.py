@@ -13,7 +13,7 @@ _lib = None
 EXPORTS = (
     "fe_mesh_create", "fe_mesh_destroy", "fe_num_nodes", "fe_num_free", "fe_num_cells", "fe_nodes_per_cell",
     "fe_quad_per_cell", "fe_get_l2g", "fe_get_node_coords", "fe_get_quad_coords", "fe_get_mass",
-    "fe_get_dirichlet_mask", "fe_set_potential", "fe_apply_H", "cheb_filter", "fe_rayleigh_ritz", "fe_minres_shifted", "fe_add_subspace", "fe_gram", "fe_density", "fe_lanczos_bounds",
+    "fe_get_dirichlet_mask", "fe_set_potential", "fe_apply_H", "cheb_filter", "cheb_filter_host", "fe_rayleigh_ritz", "fe_minres_shifted", "fe_add_subspace", "fe_gram", "fe_density", "fe_lanczos_bounds",
     "fe_set_variant",
     "fe_launch_count", "fe_last_error",
 )
@@ -52,6 +52,8 @@ def load_library():
     L.fe_apply_H.restype, L.fe_apply_H.argtypes = C.c_int, [vp, vp, vp, C.c_int, vp, vp]
     L.cheb_filter.restype = C.c_int
     L.cheb_filter.argtypes = [vp, vp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, vp, vp]
+    L.cheb_filter_host.restype = C.c_int
+    L.cheb_filter_host.argtypes = [vp, vp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double]
     L.fe_rayleigh_ritz.restype, L.fe_rayleigh_ritz.argtypes = C.c_int, [vp, vp, C.c_int, vp, vp, vp]
     L.fe_minres_shifted.restype = C.c_int
     L.fe_minres_shifted.argtypes = [vp, vp, vp, C.c_int, vp, C.c_int, C.c_double, C.c_int, vp, vp, vp, vp]
@@ -182,6 +184,24 @@ def cheb_filter(h, X, m, a, b, a0, work, stream=None):
     return X
 
 
+def cheb_filter_host(h, X_host, m, a, b, a0):
+    """X_host: contiguous float64 CPU tensor or numpy array N x B (pinned memory overlaps best); filtered in place."""
+    import numpy as np
+    if isinstance(X_host, np.ndarray):
+        if X_host.dtype != np.float64 or not X_host.flags["C_CONTIGUOUS"] or X_host.ndim != 2:
+            raise FEError(-1, "X_host must be a C-contiguous float64 N x B array")
+        ptr, shape = X_host.ctypes.data_as(C.c_void_p), X_host.shape
+    else:
+        import torch
+        if X_host.is_cuda or X_host.dtype != torch.float64 or not X_host.is_contiguous() or X_host.dim() != 2:
+            raise FEError(-1, "X_host must be a contiguous float64 CPU tensor N x B")
+        ptr, shape = C.c_void_p(X_host.data_ptr()), tuple(X_host.shape)
+    if shape[0] != fe_num_nodes(h):
+        raise FEError(-1, "X_host must be N x B")
+    _check(load_library().cheb_filter_host(h, ptr, int(shape[1]), int(m), float(a), float(b), float(a0)))
+    return X_host
+
+
 def fe_rayleigh_ritz(h, Y, work, stream=None):
     """Y (device, N x B) <- Ritz vectors in span(Y); returns the B Ritz values (numpy, ascending)."""
     import numpy as np
@@ -299,6 +319,9 @@ class FEMesh:
         if work is None:
             work = torch.empty(2 * X.numel(), dtype=torch.float64, device=X.device)
         return cheb_filter(self.h, X, m, a, b, a0, work, stream)
+
+    def cheb_filter_host(self, X_host, m, a, b, a0):
+        return cheb_filter_host(self.h, X_host, m, a, b, a0)
 
     def rayleigh_ritz(self, Y, work=None, stream=None):
         import torch

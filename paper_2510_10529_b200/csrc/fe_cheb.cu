@@ -61,6 +61,9 @@ struct fe_mesh {
     double* d_minv = nullptr;   // N: MINRES preconditioner, 1 / diag(M^{-1/2} 1/2 K M^{-1/2}) on free rows (built on first use)
     double* d_mask = nullptr;   // N: 1 on free rows, 0 on Dirichlet rows (the unpreconditioned MINRES)
     double* d_scal = nullptr;   // 17 * 128 doubles + 1 int: MINRES column scalars
+    double* d_host = nullptr;   // device staging of cheb_filter_host (grown on demand)
+    size_t host_cap = 0;
+    cudaStream_t hstream[2] = {nullptr, nullptr};
     double* d_small = nullptr;  // 2 * 128 * 128: B x B scratch of the Rayleigh-Ritz step
     int sms = 0;  // multiprocessors of the device (persistent grid size)
     int64_t launches = 0;
@@ -191,6 +194,8 @@ int fe_mesh_destroy(fe_mesh* m)
     if (!m) return FE_OK;
     cudaSetDevice(m->device);
     cudaFree(m->d_sm); cudaFree(m->d_hx); cudaFree(m->d_hy); cudaFree(m->d_hz); cudaFree(m->d_WV);
+    cudaFree(m->d_host);
+    for (cudaStream_t s : m->hstream) if (s) cudaStreamDestroy(s);
     cudaFree(m->d_small); cudaFree(m->d_minv); cudaFree(m->d_mask); cudaFree(m->d_scal);
     cudaFree(m->d_VZ); cudaFree(m->d_sx); cudaFree(m->d_sy); cudaFree(m->d_sz);
     delete m;
@@ -947,5 +952,42 @@ int fe_lanczos_bounds(fe_mesh* m, const double* v0_dev, int k, double* out3_host
     out3_host[0] = th.front();
     out3_host[1] = th.back();
     out3_host[2] = be.back();
+    return FE_OK;
+}
+
+// ---- host-buffer entry: the filter end to end (H2D, filter, D2H), column chunks pipelined on two streams -----------------
+int cheb_filter_host(fe_mesh* m, double* X_host, int B, int deg, double a, double b, double a0)
+{
+    if (!m || !X_host) return fail(FE_ERR_INVALID, "cheb_filter_host: NULL argument");
+    if (B < 1 || deg < 1) return fail(FE_ERR_INVALID, "cheb_filter_host: need B >= 1 and degree >= 1 (B=%d, m=%d)", B, deg);
+    if (!(a0 < a && a < b)) return fail(FE_ERR_INVALID, "cheb_filter_host: need a0 < a < b");
+    if (!m->have_V) return fail(FE_ERR_STATE, "cheb_filter_host: call fe_set_potential first");
+    CUDA_TRY(cudaSetDevice(m->device));
+    // columns are independent in the filter: chunks of 32 columns go through copy-in, filter, copy-out
+    // on alternating streams, so the PCIe transfers of one chunk overlap the filter of the other
+    const int BC = (B % 32 == 0 && B > 32) ? 32 : B;
+    const int nchunks = B / BC;
+    const size_t clen = (size_t)m->N * BC;
+    const int nbuf = nchunks > 1 ? 2 : 1;
+    if (m->host_cap < clen * 3 * nbuf) {
+        cudaFree(m->d_host);
+        m->d_host = nullptr;
+        m->host_cap = 0;
+        CUDA_TRY(cudaMalloc((void**)&m->d_host, clen * 3 * nbuf * sizeof(double)));
+        m->host_cap = clen * 3 * nbuf;
+    }
+    for (int i = 0; i < 2; ++i)
+        if (!m->hstream[i]) CUDA_TRY(cudaStreamCreateWithFlags(&m->hstream[i], cudaStreamNonBlocking));
+    CUDA_TRY(cudaDeviceSynchronize());
+    const size_t hp = (size_t)B * sizeof(double), dp = (size_t)BC * sizeof(double);
+    for (int c = 0; c < nchunks; ++c) {
+        cudaStream_t st = m->hstream[c % nbuf];
+        double* Xd = m->d_host + (size_t)(c % nbuf) * 3 * clen;
+        CUDA_TRY(cudaMemcpy2DAsync(Xd, dp, X_host + (size_t)c * BC, hp, dp, (size_t)m->N, cudaMemcpyHostToDevice, st));
+        int rc = cheb_filter(m, Xd, BC, deg, a, b, a0, Xd + clen, (void*)st);
+        if (rc) return rc;
+        CUDA_TRY(cudaMemcpy2DAsync(X_host + (size_t)c * BC, hp, Xd, dp, dp, (size_t)m->N, cudaMemcpyDeviceToHost, st));
+    }
+    for (int i = 0; i < nbuf; ++i) CUDA_TRY(cudaStreamSynchronize(m->hstream[i]));
     return FE_OK;
 }

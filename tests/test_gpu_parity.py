@@ -345,6 +345,26 @@ def test_device_lanczos_bounds_and_chfsi_cycles():
     assert np.max(np.abs(theta_g - theta_o) / np.maximum(1.0, np.abs(theta_o))) <= 1e-9
 
 
+@pytest.mark.parametrize("B", [6, 64, 96])
+def test_filter_from_host_buffers(B):
+    """cheb_filter_host (H2D, filter, D2H through the C ABI; chunks of 32 columns on two streams when B % 32 == 0)
+    against the oracle and against the device-resident call."""
+    w = workloads.config(1)
+    om, gm = _pair((w.xe, w.ye, w.ze), w.p, w.V)
+    mask = om.mask()
+    X = workloads.random_block(800 + B, om.N, B)  # data in the Dirichlet rows: ignored, returned as 0
+    a0, a, b = 1.0, 3.0, 25.0
+    Yo = om.filter(X * mask[:, None], 7, a, b, a0)
+    Xh = torch.as_tensor(X.copy()).pin_memory()
+    gm.cheb_filter_host(Xh, 7, a, b, a0)
+    assert _relerr(Xh.numpy(), Yo, mask) <= TOL_FILTER
+    assert np.all(Xh.numpy()[mask == 0] == 0)
+    Xn = X.copy()  # pageable numpy memory works too
+    gm.cheb_filter_host(Xn, 7, a, b, a0)
+    Yd = gm.cheb_filter(_dev(X).clone(), 7, a, b, a0).cpu().numpy()
+    assert _relerr(Xn, Yd, mask) <= 1e-13
+
+
 # ---- full BASELINE sizes: sampled rows ------------------------------------------------------------------------------
 def _sample_rows(w, count, seed):
     """Rows spread over cell interiors, faces, edges, vertices and the boundary."""
