@@ -429,16 +429,20 @@ def test_apply_full_size_sampled_rows(cfg):
     assert float(Yg[bnd].abs().max()) == 0.0
 
 
-def test_filter_full_size_property():
-    """Config 2 at full size: cheb_filter equals the three-term recurrence assembled from fe_apply_H calls (which
-    the sampled-row test ties to the oracle); holds at any size."""
+@pytest.mark.parametrize("cfg", [2, 3])
+def test_filter_full_size_property(cfg):
+    """Configs 2 and 3 at full size, in the launch shapes bench.py times (one CTA per unit at p=4, the persistent
+    32-wide CTA at p=6): cheb_filter (pre-initialised recurrence) equals the three-term recurrence assembled from
+    fe_apply_H calls (which the sampled-row tests tie to the oracle); holds at any size."""
     fe = _fe()
-    w = workloads.config(2)
+    w = workloads.config(cfg)
     gm = fe.FEMesh(w.xe, w.ye, w.ze, w.p)
     gm.set_potential(w.V(gm.quad_coords()))
     mask = _dev(gm.mask().astype(np.float64))[:, None]
-    X = _dev(w.X(gm.mask()))
-    a0, a, b, m = -6.0, -0.5, 190.0, 7
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(5000 + cfg)
+    X = torch.randn(gm.N, w.B, dtype=torch.float64, device="cuda", generator=gen) * mask
+    a0, a, b, m = -6.0, -0.5, (190.0 if cfg == 2 else 1200.0), 7
     e, c = (b - a) / 2, (b + a) / 2
     s1 = e / (a0 - c)
     s = s1
