@@ -127,7 +127,9 @@ int fe_density(fe_mesh* m, const double* X, int B, const double* f_dev, double* 
 int fe_lanczos_bounds(fe_mesh* m, const double* v0_dev, int k, double* out3_host, double* work, void* cuda_stream);
 
 /* Kernel variant for experiments and tests: 0 = default (TMA generation when B is even and the blocks are 16-byte
- * aligned, else the legacy atomics kernel), 3 = legacy kernel always, 5..8 = launch shapes of the TMA kernel
+ * aligned, else the legacy atomics kernel), 3 = legacy kernel always, 4 = legacy kernel with a colour-ordered
+ * scatter (the 8 parity classes of the cell grid launched in order: cells of one class share no node, so every sum
+ * has a fixed order and results are bit-reproducible; slower), 5..8 = launch shapes of the TMA kernel
  * (fe_apply_tma.cuh).  FE_ERR_INVALID if unknown. */
 int fe_set_variant(fe_mesh* m, int variant);
 /* Kernels launched by this handle since creation (bench.py's gpu_launches). */

@@ -399,7 +399,7 @@ static int make_block_maps(BlockMaps* bm, const fe_mesh* m, const double* base, 
 // bulk tensor copies need 16-byte aligned bases and row pitches (B even)
 static bool tma_eligible(const fe_mesh* m, int B, const void* a, const void* b, const void* c)
 {
-    if (m->variant == 3) return false;
+    if (m->variant == 3 || m->variant == 4) return false;
     if (B % 2 != 0 || !encode_fn()) return false;
     return (((uintptr_t)a | (uintptr_t)b | (uintptr_t)c) & 15) == 0;
 }

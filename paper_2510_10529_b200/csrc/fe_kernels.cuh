@@ -40,6 +40,9 @@ struct ApplyParams {
     long long Nx, NxNy;
     double alpha, beta, c;
     double w[9];  // Gauss weights
+    // colour-ordered scatter (variant 4): this launch covers the cells (2i+ox, 2j+oy, 2k+oz) only; cells of one colour
+    // share no node, so launching the 8 colours in order makes every sum order fixed (bit-reproducible results)
+    int coloured, ox, oy, oz, ccx, ccy;
     EOTab eoN, eoNT, eoG;  // even-odd split of N, N^T and G (all centro-symmetric: GLL and Gauss points are symmetric)
 };
 
@@ -142,8 +145,14 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_v3(const __grid_co
     double* sWV = sA2 + n3 * BT;   // [n^3]  J w V of this cell
     double* sS = sWV + n3;         // [n^3]  mu * M^{-1/2} at the cell's nodes
     const int lane = threadIdx.x, pl = threadIdx.y;
-    const int cell = blockIdx.x;
-    const int ex = cell % prm.cx, ey = (cell / prm.cx) % prm.cy, ez = cell / (prm.cx * prm.cy);
+    int cell = blockIdx.x;
+    int ex = cell % prm.cx, ey = (cell / prm.cx) % prm.cy, ez = cell / (prm.cx * prm.cy);
+    if (prm.coloured) {
+        ex = 2 * (cell % prm.ccx) + prm.ox;
+        ey = 2 * ((cell / prm.ccx) % prm.ccy) + prm.oy;
+        ez = 2 * (cell / (prm.ccx * prm.ccy)) + prm.oz;
+        cell = ex + prm.cx * (ey + prm.cy * ez);
+    }
     const int j = blockIdx.y * BT + lane;
     const bool act = j < prm.B;
     const long long B = prm.B;
@@ -325,7 +334,7 @@ cudaError_t launch_v3(const ApplyParams& prm, long long ncells, cudaStream_t st)
 inline bool variant_supported(int p, int variant)
 {
     (void)p;
-    return variant == 0 || variant == 3 || (variant >= 5 && variant <= 8);
+    return variant == 0 || variant == 3 || variant == 4 || (variant >= 5 && variant <= 8);
 }
 
 // One fused operator step.  *nlaunch = kernels (and memsets) enqueued.
@@ -335,17 +344,34 @@ inline cudaError_t launch_apply(const ApplyParams& prm, int p, int variant, long
     cudaError_t e = cudaMemsetAsync(prm.Y, 0, (size_t)N * prm.B * sizeof(double), st);
     if (e != cudaSuccess) return e;
     *nlaunch = 1;  // kernels only; the zero-fill is a cudaMemsetAsync
-    (void)variant;
-    switch (p) {
-        case 1: return launch_v3<1, 32, 8>(prm, ncells, st);
-        case 2: return launch_v3<2, 32, 6>(prm, ncells, st);
-        case 3: return launch_v3<3, 32, 4>(prm, ncells, st);
-        case 4: return launch_v3<4, 32, 3>(prm, ncells, st);
-        case 5: return launch_v3<5, 32, 1>(prm, ncells, st);
-        case 6: return launch_v3<6, 16, 2>(prm, ncells, st);
-        case 7: return launch_v3<7, 16, 1>(prm, ncells, st);
-        case 8: return launch_v3<8, 16, 1>(prm, ncells, st);
+    auto launch = [&](const ApplyParams& q, long long nc) -> cudaError_t {
+        switch (p) {
+            case 1: return launch_v3<1, 32, 8>(q, nc, st);
+            case 2: return launch_v3<2, 32, 6>(q, nc, st);
+            case 3: return launch_v3<3, 32, 4>(q, nc, st);
+            case 4: return launch_v3<4, 32, 3>(q, nc, st);
+            case 5: return launch_v3<5, 32, 1>(q, nc, st);
+            case 6: return launch_v3<6, 16, 2>(q, nc, st);
+            case 7: return launch_v3<7, 16, 1>(q, nc, st);
+            case 8: return launch_v3<8, 16, 1>(q, nc, st);
+        }
+        return cudaErrorInvalidValue;
+    };
+    if (variant != 4) return launch(prm, ncells);
+    // colour-ordered: 8 launches over the 2x2x2 parity classes of the cell grid, in a fixed order
+    *nlaunch = 0;
+    for (int col = 0; col < 8; ++col) {
+        ApplyParams q = prm;
+        q.coloured = 1;
+        q.ox = col & 1; q.oy = (col >> 1) & 1; q.oz = (col >> 2) & 1;
+        const int ccx = (prm.cx - q.ox + 1) / 2, ccy = (prm.cy - q.oy + 1) / 2, ccz = (prm.cz - q.oz + 1) / 2;
+        if (ccx <= 0 || ccy <= 0 || ccz <= 0) continue;
+        q.ccx = ccx; q.ccy = ccy;
+        e = launch(q, (long long)ccx * ccy * ccz);
+        if (e != cudaSuccess) return e;
+        *nlaunch += 1;
     }
+    return cudaSuccess;
     return cudaErrorInvalidValue;
 }
 

@@ -365,6 +365,30 @@ def test_filter_from_host_buffers(B):
     assert _relerr(Xn, Yd, mask) <= 1e-13
 
 
+def test_colour_ordered_scatter_is_reproducible_and_agrees():
+    """Variant 4 (SURVEY a3 "atomic or colour-ordered"): two runs are bit-identical, and the atomic paths (TMA bulk
+    reduce-add, legacy red.global) agree with it to rounding — the deterministic mode doubles as a race oracle (R17)."""
+    om, gm = _pair(UNEQUAL, 4, _coulomb)
+    mask = om.mask()
+    B = 10
+    X = workloads.random_block(900, om.N, B, mask)
+    eps = workloads.shifts(2900, B)
+    Xd, ed = _dev(X), _dev(eps)
+    gm.set_variant(4)
+    Y1 = gm.apply_H(Xd, eps=ed).clone()
+    Y2 = gm.apply_H(Xd, eps=ed).clone()
+    F1 = gm.cheb_filter(Xd.clone(), 6, -2.0, 400.0, -12.0)
+    F2 = gm.cheb_filter(Xd.clone(), 6, -2.0, 400.0, -12.0)
+    assert torch.equal(Y1, Y2) and torch.equal(F1, F2)
+    assert _relerr(Y1.cpu().numpy(), om.apply(X, eps), mask) <= TOL_APPLY
+    for variant in (0, 3):
+        gm.set_variant(variant)
+        Ya = gm.apply_H(Xd, eps=ed)
+        Fa = gm.cheb_filter(Xd.clone(), 6, -2.0, 400.0, -12.0)
+        assert float(torch.linalg.norm(Ya - Y1) / torch.linalg.norm(Y1)) <= 1e-14
+        assert float(torch.linalg.norm(Fa - F1) / torch.linalg.norm(F1)) <= 1e-13
+
+
 # ---- full BASELINE sizes: sampled rows ------------------------------------------------------------------------------
 def _sample_rows(w, count, seed):
     """Rows spread over cell interiors, faces, edges, vertices and the boundary."""
