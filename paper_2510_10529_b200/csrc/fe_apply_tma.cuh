@@ -131,7 +131,7 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
     double* const bufB = buf1;
     double* rec = rec0;
     double* recN = rec1;
-    // persistent over units: the next unit's X tile lands in bufA as soon as every warp is past pass 1 of the line phase
+    // persistent over units: the next unit's X tile is requested during the line phase, once every warp is past pass 1
     for (long long u = blockIdx.x; u < nunits; u += gridDim.x) {
     const int cell = (int)(u / nbt);
     const int ex = cell % prm.cx, ey = (cell / prm.cx) % prm.cy, ez = cell / (prm.cx * prm.cy);
@@ -278,8 +278,9 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
             for (int qz = 0; qz < n; ++qz) v[qy][qz] = fma(rxz, o[qz], v[qy][qz]);
         }
         // next-tile request, between passes 3 and 4 (measured: after pass 2 -0.7 %, after pass 4 -8 %: the tile must be
-        // in flight for about a third of the unit).  The producer duty sits on warp 3: with 32-wide tiles warps map 0,4 / 1,5 / 2,6 / 3 onto the four sub-partitions,
-        // so warp 3 is the one with issue slots to spare (measured +1.2 % over thread 0)
+        // in flight for about a third of the unit).  The producer duty sits on warp 3: with 32-wide tiles warps map
+        // 0,4 / 1,5 / 2,6 / 3 onto the four sub-partitions, so warp 3 is the one with issue slots to spare (measured
+        // +1.2 % over thread 0)
         if (PERSIST && tid == (n > 3 ? 3 * BT : 0) && u + gridDim.x < nunits) {
             const long long un = u + gridDim.x;
             const int cn = (int)(un / nbt), nx = cn % prm.cx, ny = (cn / prm.cx) % prm.cy, nz = cn / (prm.cx * prm.cy);
@@ -297,7 +298,7 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
         }
     }
     __syncthreads();
-    // ---- plane phase 2: back-interpolate in y and x, scale by alpha kz s_g, one bulk reduce-add per nodal plane ---------
+    // ---- plane phase 2: back-interpolate in y and x, scale by alpha kz s_g, two bulk reduce-adds per nodal plane --------
 #pragma unroll
     for (int qy = 0; qy < n; ++qy)
 #pragma unroll
