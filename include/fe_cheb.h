@@ -126,6 +126,14 @@ int fe_density(fe_mesh* m, const double* X, int B, const double* f_dev, double* 
  * Synchronous (two inner products per step come back to the host). */
 int fe_lanczos_bounds(fe_mesh* m, const double* v0_dev, int k, double* out3_host, double* work, void* cuda_stream);
 
+/* Potential-only operator  Y = M^{-1/2} M_U M^{-1/2} X,  (M_U)_ab = int N_a U N_b  with the field U given at the
+ * quadrature points like V (DEVICE, cells*n_q^3), without touching the potential set by fe_set_potential.  It is the
+ * integral of the adjoint right-hand side (Eq. 18, l.174-177) with U = 4 w (rho_data - rho):
+ *   g~ = [M^{-1/2} M_U M^{-1/2} Psi~] diag(f) - Psi~ (D + D^T)
+ * (the second term is fe_add_subspace; the lumped GLL mass makes M^{-1/2} M M^{-1/2} the identity).  X, Y: DEVICE N*B,
+ * no overlap; Dirichlet rows ignored / written 0.  Runs the legacy kernel with the stiffness switched off.  Asynchronous. */
+int fe_apply_potential(fe_mesh* m, const double* Uq_dev, const double* X, double* Y, int B, void* cuda_stream);
+
 /* Kernel variant for experiments and tests: 0 = default (TMA generation when B is even and the blocks are 16-byte
  * aligned, else the legacy atomics kernel), 3 = legacy kernel always, 4 = legacy kernel with a colour-ordered
  * scatter (the 8 parity classes of the cell grid launched in order: cells of one class share no node, so every sum

@@ -364,3 +364,28 @@ def density(mesh, X, f):
         r = np.einsum("rstj,j->rst", val ** 2, fw)
         rho[e] = r.transpose(2, 1, 0).reshape(-1)  # q = qx + n (qy + n qz)
     return rho
+
+
+def adjoint_rhs(mesh, Psi, f, Uq, D):
+    """g~ of PAPER.md Eq. 18 (l.174-177) in the scaled space of Eq. 19-20, for one block of orbitals Psi~ (N x B):
+    g_a^{(i)} = int [ f_i U psi^{(i)} - sum_j (D + D^T)_{ij} psi^{(j)} ] N_a dr with U = 4 w (rho_data - rho) given at the
+    quadrature points;  g~ = M^{-1/2} g, psi = M^{-1/2} psi~.  The first integral is M_U psi with (M_U)_ab = int N_a U N_b
+    taken entry by entry from the cell matrices of Eq. 17 with the kinetic part switched off; the second is M psi with
+    the lumped GLL mass (l.185), i.e. the identity in the scaled space.  Dirichlet rows are 0."""
+    Psi = _f64(Psi)
+    N, B = Psi.shape
+    free = mesh.mask().astype(bool)
+    s = np.zeros(N)
+    s[free] = 1.0 / np.sqrt(mesh.mass()[free])
+    psi = Psi * s[:, None]
+    l2g = mesh.l2g()
+    Uq = _f64(Uq).reshape(mesh.ncells, -1)
+    g = np.zeros((N, B))
+    for e in range(mesh.ncells):
+        MU = mesh.cell_matrix(e, Uq[e], kin=0.0, pot=1.0)
+        g[l2g[e]] += MU @ psi[l2g[e]]
+    g = g * _f64(f)[None, :]
+    DD = _f64(D) + _f64(D).T
+    gt = g * s[:, None] - (Psi * free[:, None]) @ DD.T  # column i: sum_j (D + D^T)_{ij} psi~^{(j)}
+    gt[~free] = 0.0
+    return gt

@@ -13,7 +13,7 @@ _lib = None
 EXPORTS = (
     "fe_mesh_create", "fe_mesh_destroy", "fe_num_nodes", "fe_num_free", "fe_num_cells", "fe_nodes_per_cell",
     "fe_quad_per_cell", "fe_get_l2g", "fe_get_node_coords", "fe_get_quad_coords", "fe_get_mass",
-    "fe_get_dirichlet_mask", "fe_set_potential", "fe_apply_H", "cheb_filter", "cheb_filter_host", "fe_rayleigh_ritz", "fe_minres_shifted", "fe_add_subspace", "fe_gram", "fe_density", "fe_lanczos_bounds",
+    "fe_get_dirichlet_mask", "fe_set_potential", "fe_apply_H", "cheb_filter", "cheb_filter_host", "fe_rayleigh_ritz", "fe_minres_shifted", "fe_add_subspace", "fe_gram", "fe_density", "fe_lanczos_bounds", "fe_apply_potential",
     "fe_set_variant",
     "fe_launch_count", "fe_last_error",
 )
@@ -59,6 +59,7 @@ def load_library():
     L.fe_minres_shifted.argtypes = [vp, vp, vp, C.c_int, vp, C.c_int, C.c_double, C.c_int, vp, vp, vp, vp]
     L.fe_density.restype, L.fe_density.argtypes = C.c_int, [vp, vp, C.c_int, vp, vp, vp]
     L.fe_lanczos_bounds.restype, L.fe_lanczos_bounds.argtypes = C.c_int, [vp, vp, C.c_int, vp, vp, vp]
+    L.fe_apply_potential.restype, L.fe_apply_potential.argtypes = C.c_int, [vp, vp, vp, vp, C.c_int, vp]
     L.fe_gram.restype, L.fe_gram.argtypes = C.c_int, [vp, vp, vp, C.c_int, vp, vp]
     L.fe_add_subspace.restype, L.fe_add_subspace.argtypes = C.c_int, [vp, vp, vp, vp, C.c_int, vp]
     L.fe_set_variant.restype, L.fe_set_variant.argtypes = C.c_int, [vp, C.c_int]
@@ -249,6 +250,13 @@ def fe_lanczos_bounds(h, v0, k=20, stream=None):
     return float(out[0]), float(out[1]), float(out[2])
 
 
+def fe_apply_potential(h, Uq, X, Y, stream=None):
+    n = fe_num_cells(h) * fe_quad_per_cell(h)
+    _check(load_library().fe_apply_potential(h, _dev_ptr(Uq, "Uq", n), _dev_ptr(X, "X"), _dev_ptr(Y, "Y", X.numel()),
+                                             X.shape[1], _stream(stream)))
+    return Y
+
+
 def fe_gram(h, A, Bm, stream=None):
     """A^T Bm as a numpy B x B array."""
     import numpy as np
@@ -343,6 +351,12 @@ class FEMesh:
 
     def lanczos_bounds(self, v0, k=20, stream=None):
         return fe_lanczos_bounds(self.h, v0, k, stream)
+
+    def apply_potential(self, Uq, X, Y=None, stream=None):
+        import torch
+        if Y is None:
+            Y = torch.empty_like(X)
+        return fe_apply_potential(self.h, Uq, X, Y, stream)
 
     def gram(self, A, Bm, stream=None):
         return fe_gram(self.h, A, Bm, stream)

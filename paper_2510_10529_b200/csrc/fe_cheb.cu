@@ -61,6 +61,7 @@ struct fe_mesh {
     double* d_minv = nullptr;   // N: MINRES preconditioner, 1 / diag(M^{-1/2} 1/2 K M^{-1/2}) on free rows (built on first use)
     double* d_mask = nullptr;   // N: 1 on free rows, 0 on Dirichlet rows (the unpreconditioned MINRES)
     double* d_scal = nullptr;   // 17 * 128 doubles + 1 int: MINRES column scalars
+    double *d_WU = nullptr, *d_VZU = nullptr;  // fe_apply_potential: J w U of the caller's field (+ unused record output)
     double* d_host = nullptr;   // device staging of cheb_filter_host (grown on demand)
     size_t host_cap = 0;
     cudaStream_t hstream[2] = {nullptr, nullptr};
@@ -194,7 +195,7 @@ int fe_mesh_destroy(fe_mesh* m)
     if (!m) return FE_OK;
     cudaSetDevice(m->device);
     cudaFree(m->d_sm); cudaFree(m->d_hx); cudaFree(m->d_hy); cudaFree(m->d_hz); cudaFree(m->d_WV);
-    cudaFree(m->d_host);
+    cudaFree(m->d_host); cudaFree(m->d_WU); cudaFree(m->d_VZU);
     for (cudaStream_t s : m->hstream) if (s) cudaStreamDestroy(s);
     cudaFree(m->d_small); cudaFree(m->d_minv); cudaFree(m->d_mask); cudaFree(m->d_scal);
     cudaFree(m->d_VZ); cudaFree(m->d_sx); cudaFree(m->d_sy); cudaFree(m->d_sz);
@@ -970,7 +971,7 @@ int cheb_filter_host(fe_mesh* m, double* X_host, int B, int deg, double a, doubl
     const size_t clen = (size_t)m->N * BC;
     const int nbuf = nchunks > 1 ? 2 : 1;
     if (m->host_cap < clen * 3 * nbuf) {
-        cudaFree(m->d_host);
+        cudaFree(m->d_host); cudaFree(m->d_WU); cudaFree(m->d_VZU);
         m->d_host = nullptr;
         m->host_cap = 0;
         CUDA_TRY(cudaMalloc((void**)&m->d_host, clen * 3 * nbuf * sizeof(double)));
@@ -989,5 +990,34 @@ int cheb_filter_host(fe_mesh* m, double* X_host, int B, int deg, double a, doubl
         CUDA_TRY(cudaMemcpy2DAsync(X_host + (size_t)c * BC, hp, Xd, dp, dp, (size_t)m->N, cudaMemcpyDeviceToHost, st));
     }
     for (int i = 0; i < nbuf; ++i) CUDA_TRY(cudaStreamSynchronize(m->hstream[i]));
+    return FE_OK;
+}
+
+// ---- potential-only operator (first term of the adjoint right-hand side, Eq. 18 l.174-177) ----------------------------
+int fe_apply_potential(fe_mesh* m, const double* Uq_dev, const double* X, double* Y, int B, void* cuda_stream)
+{
+    if (!m || !Uq_dev || !X || !Y) return fail(FE_ERR_INVALID, "fe_apply_potential: NULL argument");
+    if (B < 1) return fail(FE_ERR_INVALID, "fe_apply_potential: B=%d < 1", B);
+    const size_t len = (size_t)m->N * B;
+    if (overlap(X, len, Y, len)) return fail(FE_ERR_INVALID, "fe_apply_potential: X and Y overlap");
+    CUDA_TRY(cudaSetDevice(m->device));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t nq = (size_t)m->ncells * m->nc;
+    if (!m->d_WU) {  // J w U of the field handed in, and a scratch record array for the kernel's other output
+        CUDA_TRY(cudaMalloc((void**)&m->d_WU, nq * sizeof(double)));
+        CUDA_TRY(cudaMalloc((void**)&m->d_VZU, (size_t)m->ncells * small_tile(m->n) * sizeof(double)));
+    }
+    ApplyParams prm;
+    fill_params(m, &prm);
+    launch_weight_potential(prm, m->p, Uq_dev, m->d_WU, m->d_VZU, m->ncells, st);
+    CUDA_TRY(cudaGetLastError());
+    prm.X = X; prm.Z = nullptr; prm.Y = Y; prm.eps = nullptr; prm.B = B;
+    prm.alpha = 1.0; prm.beta = 0.0; prm.c = 0.0;
+    prm.WV = m->d_WU;
+    prm.nokin = 1;
+    int nl = 0;
+    cudaError_t e = launch_apply(prm, m->p, 3, m->N, m->ncells, st, &nl);
+    if (e != cudaSuccess) return fail(FE_ERR_CUDA, "fe_apply_potential: launch failed: %s", cudaGetErrorString(e));
+    m->launches += 1 + nl;
     return FE_OK;
 }

@@ -43,6 +43,7 @@ struct ApplyParams {
     // colour-ordered scatter (variant 4): this launch covers the cells (2i+ox, 2j+oy, 2k+oz) only; cells of one colour
     // share no node, so launching the 8 colours in order makes every sum order fixed (bit-reproducible results)
     int coloured, ox, oy, oz, ccx, ccy;
+    int nokin;  // potential-only operator M^{-1/2} M_U M^{-1/2} (fe_apply_potential): the stiffness factors are 0
     EOTab eoN, eoNT, eoG;  // even-odd split of N, N^T and G (all centro-symmetric: GLL and Gauss points are symmetric)
 };
 
@@ -161,7 +162,8 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_v3(const __grid_co
     const double* Xp = prm.X + gpl * B + j;
     const double hx = prm.hx[ex], hy = prm.hy[ey], hz = prm.hz[ez];
     const double J = hx * hy * hz * 0.125;
-    const double kx = 2.0 * J / (hx * hx), ky = 2.0 * J / (hy * hy), kz = 2.0 * J / (hz * hz);
+    const double kin = prm.nokin ? 0.0 : 2.0 * J;
+    const double kx = kin / (hx * hx), ky = kin / (hy * hy), kz = kin / (hz * hz);
 
     double v[n][n], t[n], o[n];
     // ---- plane phase 1 ---------------------------------------------------------------------------------------------

@@ -389,6 +389,34 @@ def test_colour_ordered_scatter_is_reproducible_and_agrees():
         assert float(torch.linalg.norm(Fa - F1) / torch.linalg.norm(F1)) <= 1e-13
 
 
+@pytest.mark.parametrize("p,B", [(2, 4), (4, 10), (6, 7)])
+def test_adjoint_right_hand_side(p, B):
+    """Eq. 18 assembled from the device pieces — fe_apply_potential (int N_a U psi), the occupancy scaling, and
+    fe_add_subspace for the (D + D^T) term — against the oracle's explicit-quadrature g~ (NEXT-4)."""
+    import oracle
+    fe = _fe()
+    om = oracle.OracleMesh(*UNEQUAL, p)
+    gm = fe.FEMesh(*UNEQUAL, p)
+    gm.set_potential(_coulomb(gm.quad_coords()))  # the stored potential must not leak into the result
+    mask = om.mask()
+    Psi = workloads.random_block(950 + p, om.N, B, mask)
+    f = 2.0 * workloads.uniform01(951 + p, 0, B)
+    D = workloads.normal(952 + p, B * B).reshape(B, B)
+    Uq = np.cos(om.quad_coords()).prod(axis=1) - 0.3  # any smooth field at the quadrature points (4 w (rho_data - rho))
+    Go = oracle.adjoint_rhs(om, Psi, f, Uq, D)
+    Pd = _dev(Psi)
+    G = gm.apply_potential(_dev(Uq), Pd)
+    G *= _dev(f)[None, :]
+    gm.add_subspace(Pd, -(D + D.T), G)
+    assert _relerr(G.cpu().numpy(), Go, mask) <= TOL_APPLY
+    assert np.all(G.cpu().numpy()[mask == 0] == 0)
+    # the operator set by fe_set_potential is untouched
+    X = workloads.random_block(953, om.N, 4, mask)
+    om.set_potential(_coulomb(om.quad_coords()))
+    om.assemble()
+    assert _relerr(gm.apply_H(_dev(X)).cpu().numpy(), om.apply(X), mask) <= TOL_APPLY
+
+
 # ---- full BASELINE sizes: sampled rows ------------------------------------------------------------------------------
 def _sample_rows(w, count, seed):
     """Rows spread over cell interiors, faces, edges, vertices and the boundary."""

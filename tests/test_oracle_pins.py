@@ -461,6 +461,36 @@ def test_density_polynomial_closed_form():
     assert abs(total - exact) <= 1e-12 * abs(exact)
 
 
+def test_adjoint_rhs_weak_form():
+    """Eq. 18: sum_a c_a g_a^{(i)} = int f_i U psi_i phi - sum_j (D+D^T)_ij int psi_j phi for phi = sum_a c_a N_a.  With
+    polynomial psi, phi (degree <= 3 per variable, zero on the boundary) and linear U the first integrand has degree 7 =
+    2p+1 at p = 3: the p+1 Gauss points integrate it exactly, so it must equal a 12-point reference integral of the
+    closed forms; the second term is the lumped GLL mass inner product (l.185)."""
+    m = oracle.OracleMesh(*UNEQUAL, 3)
+    xyz = m.node_coords()
+    fields = _bubble_fields(xyz, UNEQUAL)
+    psi_nodes, phi_nodes = fields[:, :1], fields[:, 1]
+    sqrtM = np.sqrt(m.mass())
+    U = lambda q: 1.0 + 0.5 * q[:, 0] - 0.25 * q[:, 1] + 0.125 * q[:, 2]
+    f = np.array([1.7])
+    D = np.array([[0.3]])
+    gt = oracle.adjoint_rhs(m, psi_nodes * sqrtM[:, None], f, U(m.quad_coords()), D)
+    lhs = float((gt[:, 0] * sqrtM) @ phi_nodes)  # g = M^{1/2} g~ ; sum_a c_a g_a
+    xq, wq = np.polynomial.legendre.leggauss(12)
+    pts, wts = [], []
+    for e in UNEQUAL:
+        a, b = e[0], e[-1]
+        pts.append(0.5 * (b - a) * xq + 0.5 * (a + b))
+        wts.append(0.5 * (b - a) * wq)
+    Xg, Yg, Zg = np.meshgrid(*pts, indexing="ij")
+    Wg = (wts[0][:, None, None] * wts[1][None, :, None] * wts[2][None, None, :]).ravel()
+    grid = np.stack([Xg.ravel(), Yg.ravel(), Zg.ravel()], axis=1)
+    F = _bubble_fields(grid, UNEQUAL)
+    first = f[0] * float((U(grid) * F[:, 0] * F[:, 1] * Wg).sum())
+    second = (D + D.T)[0, 0] * float((m.mass() * psi_nodes[:, 0]) @ phi_nodes)  # lumped mass: int psi phi ~ psi^T M phi
+    assert abs(lhs - (first - second)) <= 1e-11 * max(abs(first), abs(second))
+
+
 # ---- inputs module ------------------------------------------------------------------------------------------
 def test_inputs_generator():
     z = workloads.splitmix64(0, 0, 3)
