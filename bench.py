@@ -337,6 +337,10 @@ def main():
     roof["traffic"] = NCU_TRAFFIC_BYTES.get(args.workload)
     roof["algorithmic_bytes"] = alg_bytes
     roof["hbm_frac_of_measured"] = (alg_bytes / (roof["launch_ms"] * 1e-3) / 1e9 / hbm_peak) if hbm_peak else None
+    ck = r.get("clocks") or {}
+    if ck.get("sm_mhz") and ck.get("sm_max_mhz"):
+        # the FP64 peak above assumes the maximum SM clock; long runs sit in sw_power_cap below it
+        roof["frac_at_sampled_clock"] = roof["frac"] * ck["sm_max_mhz"] / ck["sm_mhz"]
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
