@@ -183,12 +183,11 @@ def time_workload(fe, torch, w, steps, warmup, dev, seed_offset=0, with_e2e=Fals
             for t in range(w.n_applies):
                 gm.apply_H(X if t % 2 == 0 else pristine, Y0 if t % 2 == 0 else Y1, eps)
 
-    def restore():
-        for X in Xs:
-            X.copy_(pristine)
+    def restore(i):  # only the block the coming step filters
+        Xs[i % nrot].copy_(pristine)
 
     for i in range(warmup):
-        restore()
+        restore(i)
         one_step(i)
     torch.cuda.synchronize()
     sampler = ClockSampler(dev) if sample_clocks else None
@@ -198,7 +197,7 @@ def time_workload(fe, torch, w, steps, warmup, dev, seed_offset=0, with_e2e=Fals
         dist.barrier()
     torch.cuda.synchronize()
     for i in range(steps):
-        restore()  # outside the timed events
+        restore(i)  # outside the timed events
         ev[i][0].record()
         one_step(i)
         ev[i][1].record()
