@@ -12,6 +12,7 @@
 #include <cstdint>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -410,6 +411,9 @@ static void fill_tma_params(const fe_mesh* m, TmaParams* prm, int B)
     memset(prm, 0, sizeof(*prm));
     prm->rec = m->d_VZ;
     prm->B = B; prm->cx = m->cx; prm->cy = m->cy; prm->cz = m->cz;
+    // blocked walk (fe_apply_tma.cuh: walk_cell) once one x-y slab of cell tiles no longer sits comfortably in the 126 MB L2
+    const double slab_bytes = (double)m->cx * m->cy * m->nc * B * 8.0;
+    prm->blk4 = (m->cy % 4 == 0 && m->cz % 4 == 0 && slab_bytes > 32.0e6) ? 1 : 0;
     prm->eoN = m->eoN; prm->eoNT = m->eoNT; prm->eoG = m->eoG;
 }
 
