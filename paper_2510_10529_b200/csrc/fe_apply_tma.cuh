@@ -35,7 +35,7 @@ struct TmaParams {
     const double* rec;  // cells * REC: per-cell record  VZ = V_q hz^2/2 [qx][qy][NP] | s_g [az][ay][NP] | kz s_g | ky/kx, kx/kz
     int B, cx, cy, cz;
     int owner, preinit;
-    int blk4;  // cy and cz are multiples of 4: blocked walk order (walk_cell)
+    int blk;   // block edge T of the walk order (walk_cell), a divisor of cy and cz
     double alpha, c, beta_next;
     EOTab eoN, eoNT, eoG;  // even-odd halves of N', N'^T, G'
     EOTab eoNTa;           // alpha N'^T (the last back-interpolation carries the step's alpha)
@@ -84,22 +84,17 @@ __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.comm
 __device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
-// Walk order of the cells: x fastest inside 4 x 4 blocks of (y, z) columns when cy and cz are multiples of 4 (blk4 = 1),
-// so that the z-neighbours of a cell are at most 4 cx cells away in the walk and their shared face is still in L2;
-// plain x-y-z order otherwise.  `k` is the position in the walk; the record of cell (ex,ey,ez) is at ex + cx (ey + cy ez).
-__device__ __forceinline__ void walk_cell(int k, int cx, int cy, int blk4, int& ex, int& ey, int& ez)
+// Walk order of the cells: x fastest inside T x T blocks of (y, z) columns (T divides cy and cz; T = 1 is the plain
+// x-y-z order), so that the z-neighbour of a cell is at most T cx cells away in the walk and the shared face is still in
+// L2 when it is gathered / reduced into.  `k` is the position in the walk; the record of cell (ex,ey,ez) is at
+// ex + cx (ey + cy ez).
+__device__ __forceinline__ void walk_cell(int k, int cx, int cy, int T, int& ex, int& ey, int& ez)
 {
-    if (blk4) {
-        const int per = cx * 16, b = k / per, r = k - b * per, nby = cy >> 2;
-        ex = r % cx;
-        const int ly = (r / cx) & 3, lz = r / (4 * cx);
-        ey = 4 * (b % nby) + ly;
-        ez = 4 * (b / nby) + lz;
-    } else {
-        ex = k % cx;
-        ey = (k / cx) % cy;
-        ez = k / (cx * cy);
-    }
+    const int per = cx * T * T, b = k / per, r = k - b * per, nby = cy / T;
+    ex = r % cx;
+    const int q = r / cx, ly = q % T, lz = q / T;
+    ey = T * (b % nby) + ly;
+    ez = T * (b / nby) + lz;
 }
 
 template <int n>
@@ -140,7 +135,7 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
         mbar_init(bar + 1, (n * BT + 31) / 32);
         const long long u = blockIdx.x;
         int ex, ey, ez;
-        walk_cell((int)(u / nbt), prm.cx, prm.cy, prm.blk4, ex, ey, ez);
+        walk_cell((int)(u / nbt), prm.cx, prm.cy, prm.blk, ex, ey, ez);
         const int cell = ex + prm.cx * (ey + prm.cy * ez);
         mbar_expect_tx(bar, (unsigned)((n3 * BT + REC) * sizeof(double)));
         tma_load4(buf0, &prm.mXn, (int)(u % nbt) * BT, ex * P, ey * P, ez * P, bar);
@@ -155,7 +150,7 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
     // persistent over units: the next unit's X tile is requested during the line phase, once every warp is past pass 1
     for (long long u = blockIdx.x; u < nunits; u += gridDim.x) {
     int ex, ey, ez;
-    walk_cell((int)(u / nbt), prm.cx, prm.cy, prm.blk4, ex, ey, ez);
+    walk_cell((int)(u / nbt), prm.cx, prm.cy, prm.blk, ex, ey, ez);
     const int j0 = (int)(u % nbt) * BT;
     const int gx0 = ex * P, gy0 = ey * P, gz0 = ez * P;
     double kappa = 0.0;
@@ -305,7 +300,7 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
         if (PERSIST && tid == (n > 3 ? 3 * BT : 0) && u + gridDim.x < nunits) {
             const long long un = u + gridDim.x;
             int nx, ny, nz;
-            walk_cell((int)(un / nbt), prm.cx, prm.cy, prm.blk4, nx, ny, nz);
+            walk_cell((int)(un / nbt), prm.cx, prm.cy, prm.blk, nx, ny, nz);
             const int cn = nx + prm.cx * (ny + prm.cy * nz);
             mbar_wait(bar + 1, parity ^ 1);  // parity was flipped after this unit's tile wait
             mbar_expect_tx(bar, (unsigned)((n3 * BT + REC) * sizeof(double)));

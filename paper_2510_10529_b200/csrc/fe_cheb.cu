@@ -411,9 +411,13 @@ static void fill_tma_params(const fe_mesh* m, TmaParams* prm, int B)
     memset(prm, 0, sizeof(*prm));
     prm->rec = m->d_VZ;
     prm->B = B; prm->cx = m->cx; prm->cy = m->cy; prm->cz = m->cz;
-    // blocked walk (fe_apply_tma.cuh: walk_cell) once one x-y slab of cell tiles no longer sits comfortably in the 126 MB L2
-    const double slab_bytes = (double)m->cx * m->cy * m->nc * B * 8.0;
-    prm->blk4 = (m->cy % 4 == 0 && m->cz % 4 == 0 && slab_bytes > 32.0e6) ? 1 : 0;
+    // blocked walk (fe_apply_tma.cuh: walk_cell): the largest block edge T in {8, 4, 2} that divides cy and cz and keeps
+    // T rows of cells (their X and Y tiles) within about half of the 126 MB L2; T = 1 when a whole x-y slab fits anyway
+    const double cell_bytes = (double)m->nc * B * 16.0;
+    prm->blk = 1;
+    if ((double)m->cx * m->cy * cell_bytes > 64.0e6)
+        for (int T = 8; T >= 2; T /= 2)
+            if (m->cy % T == 0 && m->cz % T == 0 && (double)T * m->cx * cell_bytes <= 64.0e6) { prm->blk = T; break; }
     prm->eoN = m->eoN; prm->eoNT = m->eoNT; prm->eoG = m->eoG;
 }
 
