@@ -30,7 +30,7 @@ FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE k_apply_tma launch from the committed `ncu --set full` captures
 # (profiles/r1b_c2_k_apply_tma_full.md, profiles/r1b_c3_k_apply_tma_full.md)
-NCU_TRAFFIC_BYTES = {2: 296.26e6 + 220.24e6, 3: 3.4568e9 + 3.1578e9}
+NCU_TRAFFIC_BYTES = {2: 296.28e6 + 221.12e6, 3: 3.4418e9 + 3.1540e9}
 
 
 def algorithmic_flops_per_cell_vector(p):
