@@ -780,7 +780,7 @@ int fe_minres_shifted(fe_mesh* m, const double* G, double* X, int B, const doubl
     int rc = ensure_minres_tables(m);
     if (rc) return rc;
     const double* Minv = precondition ? m->d_minv : m->d_mask;
-    double *R1 = work, *R2 = work + len, *Y = work + 2 * len, *V = work + 3 * len, *W1 = work + 4 * len, *W2 = work + 5 * len;
+    double *R1 = work, *R2 = work + len, *Y = work + 2 * len, *HY = work + 3 * len, *W1 = work + 4 * len, *W2 = work + 5 * len;
     MinresScalars q;
     double* s = m->d_scal;
     double** f[] = {&q.beta, &q.oldb, &q.alfa, &q.betasq, &q.dbar, &q.epsln, &q.oldeps, &q.phibar, &q.cs, &q.sn,
@@ -798,14 +798,14 @@ int fe_minres_shifted(fe_mesh* m, const double* G, double* X, int B, const doubl
     bool done = false;
     while (it < maxit && !done) {
         k_minres_scalars<<<1, 128, 0, st>>>(q, B, 1, tol);
-        k_minres_scale<<<grid, blk, 0, st>>>(Y, V, m->N, B, q.s);
-        if ((rc = fe_apply_H(m, V, Y, B, eps_dev, cuda_stream))) return rc;  // y = (H~ - eps_j) v
-        k_minres_alfa<<<grid, blk, 0, st>>>(Y, R1, V, m->N, B, q.c1, q.alfa);
-        k_minres_beta<<<grid, blk, 0, st>>>(Y, R1, R2, Minv, m->N, B, q.alfa, q.beta, q.betasq);
+        if ((rc = fe_apply_H(m, Y, HY, B, eps_dev, cuda_stream))) return rc;  // hy = (H~ - eps_j) y,  y = beta v
+        k_minres_alfa<<<grid, blk, 0, st>>>(Y, HY, R1, m->N, B, q.s, q.c1, q.alfa);
+        k_minres_beta<<<grid, blk, 0, st>>>(HY, R1, R2, Minv, m->N, B, q.alfa, q.beta, q.betasq);
         k_minres_scalars<<<1, 128, 0, st>>>(q, B, 2, tol);
-        k_minres_update<<<grid, blk, 0, st>>>(V, W1, W2, X, m->N, B, q.oldeps, q.delta, q.gamma, q.phi);
+        k_minres_update<<<grid, blk, 0, st>>>(Y, W1, W2, X, m->N, B, q.s, q.oldeps, q.delta, q.gamma, q.phi);
         CUDA_TRY(cudaGetLastError());
-        m->launches += 6;
+        m->launches += 5;
+        std::swap(Y, HY);  // the preconditioned residual of this step is the next step's y
         std::swap(R1, R2);
         std::swap(W1, W2);
         ++it;

@@ -2,8 +2,9 @@
 //
 // Every column j solves its own system (H~ - eps_j I) p_j = g_j with its own Paige-Saunders recurrences; the
 // columns advance in lock-step so that each Krylov step is ONE fused fe_apply_H launch for the whole block.  The
-// vector updates of a step are three fused elementwise kernels that also produce the column-wise inner products
-// (alfa_j = v_j.y_j, beta_j^2 = r_j.M^{-1} r_j); the Givens / Lanczos scalars live in device arrays of length B
+// vector updates of a step are three fused elementwise kernels (the normalised Lanczos vector v = y / beta is never
+// stored: the apply runs on y and the scale is folded into what follows) that also produce the column-wise inner
+// products (alfa_j = v_j.y_j, beta_j^2 = r_j.M^{-1} r_j); the Givens / Lanczos scalars live in device arrays of length B
 // and are advanced by a one-warp-per-block kernel, so an iteration needs no host synchronisation.
 // Preconditioner (l.225): inverse diagonal of the mass-scaled negative Laplacian, positive on free rows.
 #pragma once
@@ -62,21 +63,10 @@ __global__ void k_minres_init(const double* __restrict__ G, const double* __rest
     block_col_reduce(acc, B, betasq);
 }
 
-// phase A:  v = s_j y   (v overwrites y's old role through the pointer rotation done by the host)
-__global__ void k_minres_scale(const double* __restrict__ Y, double* __restrict__ V, long long N, int B,
-                               const double* __restrict__ s)
-{
-    for (long long r = blockIdx.x * (long long)kMRy + threadIdx.y; r < N; r += (long long)gridDim.x * kMRy)
-#pragma unroll
-        for (int t = 0; t < kMaxColTiles; ++t) {
-            const int j = t * kMRx + threadIdx.x;
-            if (j < B) V[r * B + j] = s[j] * Y[r * B + j];
-        }
-}
-
-// phase B:  y <- y - c1_j r1 ;  alfa_j = v_j . y_j
-__global__ void k_minres_alfa(double* __restrict__ Y, const double* __restrict__ R1, const double* __restrict__ V,
-                              long long N, int B, const double* __restrict__ c1, double* alfa)
+// phase B:  the apply ran on the un-normalised y (= beta v):  hy = (H~ - eps) y.  Here  y' = s_j hy - c1_j r1  and
+// alfa_j = v_j . y'_j  with  v = s_j y  formed on the fly (v is never stored); y' overwrites hy.
+__global__ void k_minres_alfa(const double* __restrict__ Yold, double* __restrict__ HY, const double* __restrict__ R1,
+                              long long N, int B, const double* __restrict__ s, const double* __restrict__ c1, double* alfa)
 {
     double acc[kMaxColTiles] = {0, 0, 0, 0};
     for (long long r = blockIdx.x * (long long)kMRy + threadIdx.y; r < N; r += (long long)gridDim.x * kMRy)
@@ -85,9 +75,10 @@ __global__ void k_minres_alfa(double* __restrict__ Y, const double* __restrict__
             const int j = t * kMRx + threadIdx.x;
             if (j < B) {
                 const long long i = r * B + j;
-                const double y = fma(-c1[j], R1[i], Y[i]);
-                Y[i] = y;
-                acc[t] = fma(V[i], y, acc[t]);
+                const double sj = s[j];
+                const double y = fma(sj, HY[i], -c1[j] * R1[i]);
+                HY[i] = y;
+                acc[t] = fma(sj * Yold[i], y, acc[t]);
             }
         }
     block_col_reduce(acc, B, alfa);
@@ -118,11 +109,11 @@ __global__ void k_minres_beta(double* __restrict__ Y, double* __restrict__ R1, c
     block_col_reduce(acc, B, betasq);
 }
 
-// phase D:  w_new = (v - oldeps_j w1 - delta_j w2) / gamma_j  (into w1's storage) ;  x += phi_j w_new
-__global__ void k_minres_update(const double* __restrict__ V, double* __restrict__ W1, const double* __restrict__ W2,
-                                double* __restrict__ X, long long N, int B, const double* __restrict__ oldeps,
-                                const double* __restrict__ delta, const double* __restrict__ gamma,
-                                const double* __restrict__ phi)
+// phase D:  w_new = (v - oldeps_j w1 - delta_j w2) / gamma_j  (into w1's storage), v = s_j y_old ;  x += phi_j w_new
+__global__ void k_minres_update(const double* __restrict__ Yold, double* __restrict__ W1, const double* __restrict__ W2,
+                                double* __restrict__ X, long long N, int B, const double* __restrict__ s,
+                                const double* __restrict__ oldeps, const double* __restrict__ delta,
+                                const double* __restrict__ gamma, const double* __restrict__ phi)
 {
     for (long long r = blockIdx.x * (long long)kMRy + threadIdx.y; r < N; r += (long long)gridDim.x * kMRy)
 #pragma unroll
@@ -130,7 +121,7 @@ __global__ void k_minres_update(const double* __restrict__ V, double* __restrict
             const int j = t * kMRx + threadIdx.x;
             if (j < B) {
                 const long long i = r * B + j;
-                const double w = (V[i] - oldeps[j] * W1[i] - delta[j] * W2[i]) / gamma[j];
+                const double w = (s[j] * Yold[i] - oldeps[j] * W1[i] - delta[j] * W2[i]) / gamma[j];
                 W1[i] = w;
                 X[i] = fma(phi[j], w, X[i]);
             }
