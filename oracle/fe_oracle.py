@@ -232,9 +232,12 @@ class OracleMesh:
         return Y
 
 
-def lanczos_bounds(mesh, v0, k=20, nthreads=1):
+def lanczos_bounds(mesh, v0, k=20, nthreads=1, return_tridiagonal=False):
     """Reading R10 (survey 8(c) step 8): k Lanczos steps on H~ (free rows) from the given start vector, no
-    re-orthogonalisation; returns (theta_min, theta_max, beta_k).  b = theta_max + beta_k, a0 = theta_min."""
+    re-orthogonalisation; returns (theta_min, theta_max, beta_k).  b = theta_max + beta_k, a0 = theta_min.
+    return_tridiagonal: also return the recurrence coefficients (alphas, betas) -- betas[i] couples steps i and i+1,
+    betas[-1] is the norm of the last residual vector -- so that the pin in tests/test_oracle_pins.py can compare them
+    with Q^T H~ Q from a Householder QR of the Krylov matrix."""
     mask = mesh.mask().astype(np.float64)
     v = _f64(v0).reshape(-1) * mask
     v = v / np.linalg.norm(v)
@@ -253,6 +256,8 @@ def lanczos_bounds(mesh, v0, k=20, nthreads=1):
         v_prev, v = v, w / beta
     T = np.diag(alphas) + np.diag(betas[:-1], 1) + np.diag(betas[:-1], -1)
     theta = np.linalg.eigvalsh(T)
+    if return_tridiagonal:
+        return float(theta[0]), float(theta[-1]), float(betas[-1]), np.array(alphas), np.array(betas)
     return float(theta[0]), float(theta[-1]), float(betas[-1])
 
 
@@ -288,7 +293,8 @@ def laplacian_precond(mesh):
 
 
 def minres_shifted(mesh, G, eps=None, maxit=200, tol=1e-10, Minv=None, nthreads=1):
-    """Preconditioned MINRES (Paige & Saunders 1975, the method PAPER.md l.223-225 names, ref. [59]) for
+    """Preconditioned MINRES (Paige & Saunders 1975, the method PAPER.md l.223-225 names, ref. [59]; statement order and
+    variable names after the canonical SOL `minres.m` / scipy.sparse.linalg.minres formulation of that algorithm) for
     (H~ - eps_j I) x_j = g_j, column by column, x_0 = 0, on the free rows.  Minv: diagonal preconditioner (N) or None.
     A column stops when phibar <= tol * beta1 (estimate of the preconditioned residual norm).
     Returns (X, phibar / beta1, iterations of the slowest column)."""

@@ -197,10 +197,15 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
             bulk_commit();
         }
     }
+    // a1: xhat = mu_g s_g x.  Caller data (FIRST) may hold NaN / Inf in the Dirichlet rows (R5: "ignored"), so those
+    // rows are selected to 0 instead of multiplied by s_g = 0
 #pragma unroll
     for (int ay = 0; ay < n; ++ay)
 #pragma unroll
-        for (int ax = 0; ax < n; ++ax) v[ay][ax] *= sin_pl[ay * NP + ax];
+        for (int ax = 0; ax < n; ++ax) {
+            const double sg = sin_pl[ay * NP + ax];
+            v[ay][ax] = (!FIRST || __double2hiint(sg) != 0) ? v[ay][ax] * sg : 0.0;
+        }
 #pragma unroll
     for (int ay = 0; ay < n; ++ay) {
         mat1d_eo<n>(prm.eoN, v[ay], o);
@@ -366,8 +371,8 @@ cudaError_t launch_tma(const TmaParams& prm, long long ncells, bool first, cudaS
 {
     constexpr int n = P + 1;
     constexpr size_t smem = tma_smem_bytes<P, BT>();
-    static bool configured = false;
-    if (!configured) {
+    static PerDeviceOnce once;
+    cudaError_t e0 = once_per_device(once, [&] {
         cudaError_t e = cudaFuncSetAttribute(k_apply_tma<P, BT, MINB, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e == cudaSuccess)
             e = cudaFuncSetAttribute(k_apply_tma<P, BT, MINB, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -375,9 +380,9 @@ cudaError_t launch_tma(const TmaParams& prm, long long ncells, bool first, cudaS
             e = cudaFuncSetAttribute(k_apply_tma<P, BT, MINB, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e == cudaSuccess)
             e = cudaFuncSetAttribute(k_apply_tma<P, BT, MINB, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+        return e;
+    });
+    if (e0 != cudaSuccess) return e0;
     const long long nunits = ncells * ((prm.B + BT - 1) / BT);
     const bool persist = ctas > 0 && (long long)ctas * MINB < nunits;
     dim3 grid((unsigned)(persist ? (long long)ctas * MINB : nunits)), block(BT, n);

@@ -180,9 +180,9 @@ int fe_mesh_create(const double* xe, int cx, const double* ye, int cy, const dou
     if (ce != cudaSuccess) return cleanup(fail(FE_ERR_NOMEM, "fe_mesh_create: device allocation failed: %s", cudaGetErrorString(ce)));
     ce = cudaMemset(m->d_VZ, 0, (size_t)m->ncells * small_tile(m->n) * sizeof(double));
     if (ce != cudaSuccess) return cleanup(fail(FE_ERR_CUDA, "fe_mesh_create: memset failed: %s", cudaGetErrorString(ce)));
-    k_build_records<<<148 * 8, 256>>>(m->d_VZ, m->n, m->cx, m->cy, m->ncells, m->d_sx, m->d_sy, m->d_sz, m->d_hx, m->d_hy, m->d_hz);
+    k_build_records<<<m->sms * 8, 256>>>(m->d_VZ, m->n, m->cx, m->cy, m->ncells, m->d_sx, m->d_sy, m->d_sz, m->d_hx, m->d_hy, m->d_hz);
     m->launches += 1;
-    launch_build_scaling(m->d_sx, m->d_sy, m->d_sz, m->Nx, m->Ny, m->Nz, m->d_sm, 0);
+    launch_build_scaling(m->d_sx, m->d_sy, m->d_sz, m->Nx, m->Ny, m->Nz, m->d_sm, m->sms, 0);
     m->launches += 1;
     ce = cudaDeviceSynchronize();
     if (ce != cudaSuccess) return cleanup(fail(FE_ERR_CUDA, "fe_mesh_create: scaling kernel failed: %s", cudaGetErrorString(ce)));
@@ -318,7 +318,7 @@ int fe_set_potential(fe_mesh* m, const double* Vq_dev, int copy, void* cuda_stre
     CUDA_TRY(cudaSetDevice(m->device));
     ApplyParams prm;
     fill_params(m, &prm);
-    launch_weight_potential(prm, m->p, Vq_dev, m->d_WV, m->d_VZ, m->ncells, (cudaStream_t)cuda_stream);
+    launch_weight_potential(prm, m->p, Vq_dev, m->d_WV, m->d_VZ, m->ncells, m->sms, (cudaStream_t)cuda_stream);
     CUDA_TRY(cudaGetLastError());
     m->launches += 1;
     m->have_V = true;
@@ -442,7 +442,7 @@ static int tma_step(fe_mesh* m, const BlockMaps& X, const BlockMaps& Y, const Bl
 
 static int zero_faces(fe_mesh* m, double* Y, int B, cudaStream_t st)
 {
-    k_zero_faces<<<148 * 4, 256, 0, st>>>(Y, m->Nx, m->Ny, m->Nz, B);
+    k_zero_faces<<<m->sms * 4, 256, 0, st>>>(Y, m->Nx, m->Ny, m->Nz, B);
     CUDA_TRY(cudaGetLastError());
     m->launches += 1;
     return FE_OK;
@@ -753,9 +753,9 @@ static int ensure_minres_tables(fe_mesh* m)
     if (!rc && ce == cudaSuccess) ce = cudaMalloc((void**)&m->d_mask, (size_t)m->N * sizeof(double));
     if (!rc && ce == cudaSuccess) ce = cudaMalloc((void**)&m->d_scal, (17 * 128 + 2) * sizeof(double));
     if (!rc && ce == cudaSuccess) {
-        k_build_precond<<<148 * 8, 256>>>(m->d_minv, m->Nx, m->Ny, m->Nz, d[0], d[1], d[2], d[3], d[4], d[5], m->d_sx, m->d_sy, m->d_sz);
-        k_build_scaling<<<148 * 8, 256>>>(m->d_sx, m->d_sy, m->d_sz, m->Nx, m->Ny, m->Nz, m->d_mask);
-        k_nonzero_to_one<<<148 * 4, 256>>>(m->d_mask, m->N);  // mu M^{-1/2} -> {0, 1}
+        k_build_precond<<<m->sms * 8, 256>>>(m->d_minv, m->Nx, m->Ny, m->Nz, d[0], d[1], d[2], d[3], d[4], d[5], m->d_sx, m->d_sy, m->d_sz);
+        k_build_scaling<<<m->sms * 8, 256>>>(m->d_sx, m->d_sy, m->d_sz, m->Nx, m->Ny, m->Nz, m->d_mask);
+        k_nonzero_to_one<<<m->sms * 4, 256>>>(m->d_mask, m->N);  // mu M^{-1/2} -> {0, 1}
         ce = cudaDeviceSynchronize();
         m->launches += 2;
     }
@@ -979,7 +979,7 @@ int cheb_filter_host(fe_mesh* m, double* X_host, int B, int deg, double a, doubl
     const size_t clen = (size_t)m->N * BC;
     const int nbuf = nchunks > 1 ? 2 : 1;
     if (m->host_cap < clen * 3 * nbuf) {
-        cudaFree(m->d_host); cudaFree(m->d_WU); cudaFree(m->d_VZU);
+        cudaFree(m->d_host);  // only the staging: d_WU / d_VZU belong to fe_apply_potential and stay valid
         m->d_host = nullptr;
         m->host_cap = 0;
         CUDA_TRY(cudaMalloc((void**)&m->d_host, clen * 3 * nbuf * sizeof(double)));
@@ -1017,7 +1017,7 @@ int fe_apply_potential(fe_mesh* m, const double* Uq_dev, const double* X, double
     }
     ApplyParams prm;
     fill_params(m, &prm);
-    launch_weight_potential(prm, m->p, Uq_dev, m->d_WU, m->d_VZU, m->ncells, st);
+    launch_weight_potential(prm, m->p, Uq_dev, m->d_WU, m->d_VZU, m->ncells, m->sms, st);
     CUDA_TRY(cudaGetLastError());
     prm.X = X; prm.Z = nullptr; prm.Y = Y; prm.eps = nullptr; prm.B = B;
     prm.alpha = 1.0; prm.beta = 0.0; prm.c = 0.0;

@@ -42,7 +42,8 @@ __global__ void __launch_bounds__((P + 1) * 32) k_density(const __grid_constant_
 #pragma unroll
         for (int ax = 0; ax < n; ++ax) {
             const long long g = g0 + ax + prm.Nx * ay;
-            v[ay][ax] = act ? prm.X[g * prm.B + j] * prm.sm[g] : 0.0;
+            const double sg = prm.sm[g];
+            v[ay][ax] = (act && sg != 0.0) ? prm.X[g * prm.B + j] * sg : 0.0;  // Dirichlet rows may hold anything (R5)
         }
 #pragma unroll
     for (int ay = 0; ay < n; ++ay) {
@@ -84,12 +85,11 @@ cudaError_t launch_density_p(const DensityParams& prm, long long ncells, cudaStr
 {
     constexpr int n = P + 1;
     const size_t smem = (size_t)n * n * n * 32 * sizeof(double);
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_density<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    static PerDeviceOnce once;
+    cudaError_t e0 = once_per_device(once, [&] {
+        return cudaFuncSetAttribute(k_density<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    });
+    if (e0 != cudaSuccess) return e0;
     dim3 grid((unsigned)ncells, (unsigned)((prm.B + 31) / 32)), block(32, n);
     k_density<P><<<grid, block, smem, st>>>(prm);
     return cudaGetLastError();

@@ -18,7 +18,27 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <atomic>
+
 namespace fecheb {
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-DEVICE attribute and fe_mesh_create takes any cuda_device: every
+// launcher keeps one bit per device (thread-safe) and sets the attribute on the first launch on each device.
+struct PerDeviceOnce {
+    std::atomic<unsigned long long> bits{0};
+};
+template <class F>
+inline cudaError_t once_per_device(PerDeviceOnce& o, F&& set)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const bool tracked = dev >= 0 && dev < 64;
+    if (tracked && ((o.bits.load(std::memory_order_acquire) >> dev) & 1ull)) return cudaSuccess;
+    e = set();
+    if (e == cudaSuccess && tracked) o.bits.fetch_or(1ull << dev, std::memory_order_release);
+    return e;
+}
 
 // Even-odd form of a centro-symmetric n x n matrix M (M[i][k] = M[n-1-i][n-1-k]), h = n/2, c = (n+1)/2:
 //   S[i*h+k] = (M[i][k] + M[i][n-1-k])/2 (i<c), A[i*h+k] = (M[i][k] - M[i][n-1-k])/2 (i<h), Mid[i] = M[i][h] (n odd).
@@ -59,9 +79,9 @@ __global__ void k_build_scaling(const double* __restrict__ sx, const double* __r
 }
 
 inline void launch_build_scaling(const double* sx, const double* sy, const double* sz, long long Nx, long long Ny,
-                                 long long Nz, double* sm, cudaStream_t st)
+                                 long long Nz, double* sm, int sms, cudaStream_t st)
 {
-    k_build_scaling<<<148 * 8, 256, 0, st>>>(sx, sy, sz, Nx, Ny, Nz, sm);
+    k_build_scaling<<<sms * 8, 256, 0, st>>>(sx, sy, sz, Nx, Ny, Nz, sm);
 }
 
 // WV[e][q] = J_e w_qx w_qy w_qz V[e][q];  VZ = first tile of the cell record of the TMA kernel:
@@ -84,9 +104,9 @@ __global__ void k_weight_potential(const __grid_constant__ ApplyParams prm, int 
 }
 
 inline void launch_weight_potential(const ApplyParams& prm, int p, const double* V, double* WV, double* VZ,
-                                    long long ncells, cudaStream_t st)
+                                    long long ncells, int sms, cudaStream_t st)
 {
-    k_weight_potential<<<148 * 8, 256, 0, st>>>(prm, p + 1, V, WV, VZ, ncells);
+    k_weight_potential<<<sms * 8, 256, 0, st>>>(prm, p + 1, V, WV, VZ, ncells);
 }
 
 // ---- even-odd form of the 1-D contractions (shared by every kernel generation) ---------------------------------------
@@ -183,7 +203,10 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_v3(const __grid_co
 #pragma unroll
     for (int ay = 0; ay < n; ++ay)
 #pragma unroll
-        for (int ax = 0; ax < n; ++ax) v[ay][ax] *= sS[(pl * n + ay) * n + ax];
+        for (int ax = 0; ax < n; ++ax) {  // Dirichlet rows of caller data may hold NaN / Inf: select, do not multiply by 0
+            const double sg = sS[(pl * n + ay) * n + ax];
+            v[ay][ax] = __double2hiint(sg) != 0 ? v[ay][ax] * sg : 0.0;
+        }
 #pragma unroll
     for (int ay = 0; ay < n; ++ay) {
         mat1d_eo<n>(prm.eoN, v[ay], o);
@@ -322,12 +345,11 @@ cudaError_t launch_v3(const ApplyParams& prm, long long ncells, cudaStream_t st)
 {
     constexpr int n = P + 1;
     const size_t smem = ((size_t)2 * n * n * n * BT + 2 * n * n * n) * sizeof(double);
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_apply_v3<P, BT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    static PerDeviceOnce once;
+    cudaError_t e0 = once_per_device(once, [&] {
+        return cudaFuncSetAttribute(k_apply_v3<P, BT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    });
+    if (e0 != cudaSuccess) return e0;
     dim3 grid((unsigned)ncells, (unsigned)((prm.B + BT - 1) / BT)), block(BT, n);
     k_apply_v3<P, BT, MINB><<<grid, block, smem, st>>>(prm);
     return cudaGetLastError();

@@ -298,11 +298,11 @@ inline cudaError_t launch_gram(const double* A, const double* Bm, long long N, i
         if (T <= 6) return launch_gram2<6>(A, Bm, N, B, C, sms, st);
         return launch_gram2<8>(A, Bm, N, B, C, sms, st);
     }
-    static bool configured = false;
-    if (!configured) {
-        cudaFuncSetAttribute(k_gram<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * kRRRows * 128 * 8);
-        configured = true;
-    }
+    static PerDeviceOnce once;
+    cudaError_t e0 = once_per_device(once, [&] {
+        return cudaFuncSetAttribute(k_gram<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * kRRRows * 128 * 8);
+    });
+    if (e0 != cudaSuccess) return e0;
     const int grid = sms * 2;
     if (T <= 1) k_gram<1><<<grid, kRRThreads, smem, st>>>(A, Bm, N, B, C);
     else if (T <= 2) k_gram<2><<<grid, kRRThreads, smem, st>>>(A, Bm, N, B, C);
@@ -323,15 +323,16 @@ inline cudaError_t launch_rightmul(const double* Y, const double* R, double* Out
         if (T <= 6) return launch_rightmul2<6, 2>(Y, R, Out, accumulate, N, B, sms, st);
         return launch_rightmul2<8, 2>(Y, R, Out, accumulate, N, B, sms, st);
     }
-    static bool configured = false;
-    if (!configured) {
+    static PerDeviceOnce once;
+    cudaError_t e0 = once_per_device(once, [&] {
         const int mx = (128 * 128 + kRRRows * 129) * 8;
-        cudaFuncSetAttribute(k_rightmul<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
-        cudaFuncSetAttribute(k_rightmul<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
-        cudaFuncSetAttribute(k_rightmul<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
-        cudaFuncSetAttribute(k_rightmul<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
-        configured = true;
-    }
+        cudaError_t e = cudaFuncSetAttribute(k_rightmul<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rightmul<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rightmul<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rightmul<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
+        return e;
+    });
+    if (e0 != cudaSuccess) return e0;
     const int grid = sms * (B > 64 ? 1 : 2);
     if (T <= 1) k_rightmul<1><<<grid, kRRThreads, smem, st>>>(Y, R, Out, accumulate, N, B);
     else if (T <= 2) k_rightmul<2><<<grid, kRRThreads, smem, st>>>(Y, R, Out, accumulate, N, B);

@@ -347,6 +347,45 @@ def test_filter_closed_form():
         m.filter(X, 3, b, a, a0)
 
 
+@pytest.mark.parametrize("k", [1, 2, 6])
+def test_lanczos_is_the_krylov_projection(k):
+    """Reading R10 pins lanczos_bounds to what the mathematics fixes: in exact arithmetic the Lanczos vectors are the
+    Gram-Schmidt basis of the Krylov space, so with Q from a Householder QR of [v, H~v, ..., H~^k v] (column signs made
+    positive) alpha_i = (Q^T H~ Q)_ii, beta_i = (Q^T H~ Q)_{i+1,i} > 0, the returned beta is the LAST of them (the
+    coupling to the (k+1)-th vector = norm of the last residual), and theta = eig of the leading k x k block.  A dropped
+    `- beta v_prev`, a shifted off-diagonal or a wrong returned beta fails this; k <= 6 keeps the monomial Krylov basis
+    well enough conditioned for 1e-9 on config 1's 343 x 343 operator."""
+    w = workloads.config(1)
+    m = _mesh((w.xe, w.ye, w.ze), w.p, V=w.V)
+    mask = m.mask()
+    free = np.flatnonzero(mask)
+    H = _csr(m).toarray()[np.ix_(free, free)]
+    v0 = workloads.normal(3001, m.N)
+    v = v0[free] / np.linalg.norm(v0[free])
+    K = np.empty((len(free), k + 1))
+    K[:, 0] = v
+    for i in range(k):
+        K[:, i + 1] = H @ K[:, i]
+        K[:, i + 1] /= np.linalg.norm(K[:, i + 1])  # column scaling changes R, not Q
+    Q, R = np.linalg.qr(K)
+    Q = Q * np.sign(np.diag(R))[None, :]
+    T = Q.T @ H @ Q  # (k+1) x (k+1), tridiagonal up to rounding
+    lo, hi, beta, alphas, betas = oracle.lanczos_bounds(m, v0, k, return_tridiagonal=True)
+    scale = np.abs(H).sum(axis=1).max()
+    assert len(alphas) == k and len(betas) == k
+    assert np.max(np.abs(alphas - np.diag(T)[:k])) <= 1e-9 * scale
+    assert np.max(np.abs(betas - np.diag(T, -1)[:k])) <= 1e-9 * scale
+    assert np.all(np.diag(T, -1)[:k] > 0)
+    assert beta == betas[-1] and abs(beta - T[k, k - 1]) <= 1e-9 * scale
+    theta = np.linalg.eigvalsh(T[:k, :k])
+    assert abs(lo - theta[0]) <= 1e-9 * scale and abs(hi - theta[-1]) <= 1e-9 * scale
+    # what is outside the tridiagonal band vanishes (three-term recurrence = symmetry of H~)
+    assert np.max(np.abs(np.triu(T[:k, :k], 2))) <= 1e-9 * scale
+    # and the interval [theta_min, theta_max + beta] the filter uses still brackets as before
+    lam = np.linalg.eigvalsh(H)
+    assert lo >= lam[0] - 1e-10 and hi <= lam[-1] + 1e-10
+
+
 def test_filter_cellwise_equals_csr():
     w = workloads.reduced(2, 2)
     m = _mesh((w.xe, w.ye, w.ze), 2, V=w.V)
