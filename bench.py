@@ -1,11 +1,14 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the fused Chebyshev-filter H~X path on the BASELINE.json workloads.
 
-A "step" is one cheb_filter call (m fused operator steps: gather -> cell contraction -> scatter + recurrence) on
-one block of B vectors.  metric = GDoF-vectors/s = N_free * B * m * steps / time (reading R14).  Prints ONE JSON
-line (rank 0).  See DESIGN.md "Measurement" for the roofline arithmetic.
+A "step" is one cheb_filter call (m fused operator steps: gather -> cell contraction -> scatter + recurrence) on one block
+of B vectors (config 5: its 200 shifted applies).  metric = GDoF-vectors/s = N_free * B * m * steps / time (reading R14).
+Rank 0 prints ONE JSON line.  The line's `value` is the largest single-GPU workload (config 4); `workloads` carries the
+same measurement (value, roofline, clocks) for the other roofline workloads 2, 3 and 5; `peaks` the step-0 ceilings
+measured in the same run (fe_diag_peak).  See DESIGN.md "Measurement" for the roofline arithmetic.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 2|3|4|5] [--extra] [--impl reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 2|3|4|5] [--also 2,3,5] [--orders] [--consumers]
+                  [--scaling weak|strong] [--impl reference] [--stub]
 """
 import argparse
 import json
@@ -24,19 +27,35 @@ import workloads  # noqa: E402
 
 METRIC = "FE H~X GDoF-vectors/s (FP64) in Chebyshev filter"
 UNIT = "GDoF-vectors/s"
-# FP64 ALU roofline: 148 SMs x 64 DFMA/clk/SM x 2 flop x 1.965 GHz (MEASURED_PEAKS.json sm_max_mhz)
-FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+# nominal FP64 ALU peak: 148 SMs x 64 DFMA/clk/SM x 2 flop x 1.965 GHz (MEASURED_PEAKS.json sm_max_mhz)
+FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 
-
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE k_apply_tma launch from the committed `ncu --set full` captures
-# (profiles/r1b_c2_k_apply_tma_full.md, profiles/r1b_c3_k_apply_tma_full.md)
-NCU_TRAFFIC_BYTES = {2: 296.28e6 + 221.12e6, 3: 3.4418e9 + 3.1540e9}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE k_apply_tma launch, copied from the committed `ncu --set full`
+# captures named here (profiles/); not measured in this run
+NCU_TRAFFIC = {
+    2: (296.28e6 + 221.12e6, "profiles/r1b_c2_k_apply_tma_full.md"),
+    3: (3.4418e9 + 3.1540e9, "profiles/r1b_c3_k_apply_tma_full.md"),
+}
 
 
 def algorithmic_flops_per_cell_vector(p):
-    """matrix-free sum factorisation, 24 n^4 + 9 n^3 flops per cell-vector."""
+    """matrix-free sum factorisation in the generic 12-sweep form, 24 n^4 + 9 n^3 flops per cell-vector."""
     n = p + 1
     return 24 * n**4 + 9 * n**3
+
+
+def executed_fp64_per_cell_vector(p):
+    """What k_apply_tma executes per cell-vector (counted from the kernel's structure, cross-checked against the ncu opcode
+    mix in profiles/): 10 even-odd sweeps of n^2 lines -- a line costs n DMUL, c h + h (h-1) DFMA and 4 h DADD with
+    h = n // 2, c = (n + 1) // 2 -- plus 2 DMUL + 3 DFMA per point (scalings, V, the two geometry ratios).
+    Returns (instructions, flops)."""
+    n = p + 1
+    h, c = n // 2, (n + 1) // 2
+    mul, fma, add = n, c * h + h * (h - 1), 4 * h
+    lines = 10 * n * n
+    instr = lines * (mul + fma + add) + 5 * n**3
+    flops = lines * (mul + add + 2 * fma) + (2 + 2 * 3) * n**3
+    return instr, flops
 
 
 def spectrum_bounds(w):
@@ -74,7 +93,7 @@ class ClockSampler:
             self.p.kill()
         self.f.flush()
         self.f.seek(0)
-        sm, mx, reasons = [], [], set()
+        sm, mx, pw, reasons = [], [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for line in self.f:
             parts = [s.strip() for s in line.split(",")]
@@ -83,6 +102,7 @@ class ClockSampler:
             try:
                 sm.append(float(parts[0]))
                 mx.append(float(parts[1]))
+                pw.append(float(parts[2]))
             except ValueError:
                 continue
             for nme, val in zip(names, parts[3:7]):
@@ -91,15 +111,20 @@ class ClockSampler:
         self.f.close()
         os.unlink(self.f.name)
         if sm:
-            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons), samples=len(sm))
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons), samples=len(sm),
+                       power_w_max=float(max(pw)) if pw else None)
         return out
 
 
-def cpu_baseline(w_index, budget_cells, steps=1, all_cores=True):
-    """The oracle as it stands, on a bounded sample: the same recipe on a centred sub-mesh of budget_cells^3 cells,
-    all B columns, full degree m (config 5: 4 shifted applies).  Setup (cell matrices, CSR) is not timed."""
+# ---- the oracle on the host cores (cpu_baseline leg and --impl reference) -------------------------------------------------
+def cpu_baseline(w_index, sample, steps=1, all_cores=True):
+    """The oracle as it stands, on a bounded sample: the same recipe on a centred sub-mesh of budget_cells^3 cells, the
+    first ncols columns of the block (columns are independent, R22), full degree m (config 5: 4 shifted applies).
+    Setup (cell matrices, CSR) is not timed."""
     import oracle
+    budget_cells, ncols = sample
     w = workloads.reduced(w_index, budget_cells)
+    w.B = min(w.B, ncols)
     om = oracle.OracleMesh(w.xe, w.ye, w.ze, w.p)
     om.set_potential(w.V(om.quad_coords()))
     om.assemble()
@@ -121,7 +146,7 @@ def cpu_baseline(w_index, budget_cells, steps=1, all_cores=True):
 
     t1 = run(1)
     out = {"value": om.N_free * w.B * napply / t1 / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
-           "sample": "%s: centred %d^3-cell sub-mesh (N=%d), all B=%d columns, %d applies, serial CSR oracle; setup untimed"
+           "sample": "%s: centred %d^3-cell sub-mesh (N=%d), %d columns, %d applies, serial CSR oracle; setup untimed"
                      % (w.name, budget_cells, om.N, w.B, napply),
            "seconds_per_step": t1}
     if all_cores:
@@ -132,7 +157,7 @@ def cpu_baseline(w_index, budget_cells, steps=1, all_cores=True):
     return out
 
 
-SAMPLE_CELLS = {2: 6, 3: 4, 4: 4, 5: 6}
+SAMPLE_CELLS = {2: (6, 64), 3: (4, 8), 4: (4, 8), 5: (6, 64)}  # (cells per axis, columns) of the oracle's timed sample
 
 
 def run_reference(args):
@@ -142,7 +167,7 @@ def run_reference(args):
         return
     w = workloads.config(args.workload)
     for _ in range(min(args.warmup, 1)):
-        cpu_baseline(args.workload, 2, 1, all_cores=False)
+        cpu_baseline(args.workload, (2, 2), 1, all_cores=False)
     cb = cpu_baseline(args.workload, SAMPLE_CELLS[args.workload], max(1, args.steps), all_cores=False)
     line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": cb["seconds_per_step"] * 1e3,
@@ -154,24 +179,66 @@ def run_reference(args):
     print(json.dumps(line))
 
 
-def time_workload(fe, torch, w, steps, warmup, dev, seed_offset=0, with_e2e=False, dist=None, sample_clocks=False,
-                  variant=0):
-    """Device-resident timing of `steps` cheb_filter calls (config 5: blocks of 200 shifted applies)."""
+# ---- rank plumbing (one process per GPU; columns are sharded with no exchange) --------------------------------------------
+def respawn_under_torchrun(args):
+    """`python bench.py --gpus N` without a torchrun environment: start N ranks of this script on this node."""
+    import socket
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
+
+
+def columns_of_rank(w, rank, world, scaling):
+    """weak: every rank filters its own B-column block; strong: the B columns of the workload are dealt to the ranks."""
+    from paper_2510_10529_b200.colsplit import column_slice
+    if scaling == "weak":
+        return w.B
+    lo, hi = column_slice(w.B, rank, world)
+    return hi - lo
+
+
+def job_line(w, per_rank, world, dist, device, steps, warmup, scaling):
+    """Whole-job numbers from the per-rank measurement: times are the max over ranks, units the sum over ranks."""
+    from paper_2510_10529_b200.colsplit import job_throughput, max_over_ranks
+    ms_step, e2e_ms = max_over_ranks([per_rank["ms_per_step"], per_rank.get("e2e_ms_per_step", 0.0)], dist, device)
+    cols = per_rank["B"] * world if scaling == "weak" else w.B
+    units = per_rank["N_free"] * cols * per_rank["napply"]  # DoF-vectors per step, all ranks
+    value = job_throughput(units / world, world, ms_step * 1e-3) / 1e9
+    e2e = job_throughput(units / world, world, e2e_ms * 1e-3) / 1e9 if e2e_ms > 0 else None
+    return {"value": value, "ms_per_step": ms_step, "e2e_value": e2e, "e2e_ms_per_step": e2e_ms, "n_gpus": world,
+            "steps": steps, "warmup": warmup, "scaling": scaling, "columns_total": cols}
+
+
+def stub_measurement(w, rank, B):
+    """--stub: no GPU work; a fixed fake step time per rank, so that the spawning, the barrier, the max over ranks and the
+    whole-job aggregation can be exercised on CPU (gloo).  The line says "data": "stub"."""
+    return {"ms_per_step": 10.0 * (1 + rank), "e2e_ms_per_step": 20.0 * (1 + rank), "napply": max(w.m, 1), "N": w.N,
+            "N_free": w.N_free, "B": B, "ncells": w.ncells, "launches": 0, "clocks": None, "e2e_bytes": 0}
+
+
+# ---- device timing --------------------------------------------------------------------------------------------------------
+def time_workload(fe, torch, w, B, steps, warmup, dev, seed_offset=0, with_e2e=False, dist=None, variant=0):
+    """Device-resident timing of `steps` cheb_filter calls (config 5: blocks of 200 shifted applies), CUDA events on the
+    launching stream around every step; clocks sampled during the timed region."""
     gm = fe.FEMesh(w.xe, w.ye, w.ze, w.p, device=dev)
     if variant:
         gm.set_variant(variant)
     Vq = w.V(gm.quad_coords())
     gm.set_potential(Vq)
     mask = torch.as_tensor(gm.mask().astype(np.float64), device="cuda")[:, None]
-    N, B = gm.N, w.B
+    N = gm.N
     nrot = 3 if N * B * 8 < 1 << 30 else 1  # rotate buffer sets when one block is L2-scale (config 2/5)
     gen = torch.Generator(device="cuda")
     gen.manual_seed(1234 + w.x_seed + seed_offset)
-    pristine = torch.randn(N, B, dtype=torch.float64, device="cuda", generator=gen) * mask
+    pristine = torch.randn(N, B, dtype=torch.float64, device="cuda", generator=gen)
+    pristine.mul_(mask)
     Xs = [torch.empty_like(pristine) for _ in range(nrot)]
     works = [torch.empty(2 * N * B, dtype=torch.float64, device="cuda") for _ in range(nrot)]
     a0, a, b = spectrum_bounds(w)
-    eps = torch.as_tensor(w.eps(), device="cuda") if w.eps_seed is not None else None
+    eps = torch.as_tensor(w.eps()[:B], device="cuda") if w.eps_seed is not None else None
     napply = w.m if w.m > 0 else w.n_applies
 
     def one_step(i):
@@ -190,7 +257,7 @@ def time_workload(fe, torch, w, steps, warmup, dev, seed_offset=0, with_e2e=Fals
         restore(i)
         one_step(i)
     torch.cuda.synchronize()
-    sampler = ClockSampler(dev) if sample_clocks else None
+    sampler = ClockSampler(dev)
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
     l0 = gm.launches
     if dist is not None:
@@ -204,41 +271,115 @@ def time_workload(fe, torch, w, steps, warmup, dev, seed_offset=0, with_e2e=Fals
     torch.cuda.synchronize()
     if dist is not None:
         dist.barrier()
-    clocks = sampler.stop() if sampler else None
+    clocks = sampler.stop()
     ms = [e0.elapsed_time(e1) for e0, e1 in ev]
-    total_ms = float(sum(ms))
-    res = {"gm": gm, "ms_per_step": total_ms / steps, "ms_min": float(min(ms)), "launches": gm.launches - l0,
-           "napply": napply, "N": N, "N_free": gm.N_free, "B": B, "clocks": clocks, "ncells": gm.ncells}
+    res = {"ms_per_step": float(sum(ms)) / steps, "ms_min": float(min(ms)), "launches": gm.launches - l0,
+           "napply": napply, "N": N, "N_free": gm.N_free, "B": B, "clocks": clocks, "ncells": gm.ncells,
+           "l2": ("%d rotating buffer sets of 3 x %.0f MB blocks > 126 MB L2" % (nrot, N * B * 8 / 1e6)) if nrot > 1
+                 else "blocks of %.2f GB >> L2" % (N * B * 8 / 1e9)}
     if with_e2e:
-        # end to end through the public API with HOST buffers: pinned H2D of the block, filter, D2H of the result
-        host_in = pristine.cpu().pin_memory()
-        host_out = torch.empty_like(host_in).pin_memory()
+        # end to end through the public API with HOST buffers, every step: pinned H2D of the block, the filter, D2H of
+        # the result (config 2-4: the C-ABI host call cheb_filter_host; config 5: copies around the 200 applies)
+        host_io = torch.empty(N, B, dtype=torch.float64, pin_memory=True)
+        host_io.copy_(pristine)
         X, wk = Xs[0], works[0]
-        e2e_steps = max(1, min(steps, 3))
+        if w.m > 0:  # the host call owns its device staging: release this function's blocks first
+            Xs.clear()
+            works.clear()
+            X = wk = None
+            torch.cuda.empty_cache()
 
         def e2e_step():
-            if w.m > 0:  # the C-ABI host-buffer call: H2D, filter, D2H (column chunks pipelined), synchronous
-                gm.cheb_filter_host(host_io, w.m, a, b, a0)
+            if w.m > 0:
+                gm.cheb_filter_host(host_io, w.m, a, b, a0)  # synchronous
             else:
-                X.copy_(host_in, non_blocking=True)
+                X.copy_(host_io, non_blocking=True)
                 one_step(0)
-                host_out.copy_(wk[:N * B].view(N, B), non_blocking=True)
+                host_io.copy_(wk[:N * B].view(N, B), non_blocking=True)
+                torch.cuda.synchronize()
 
-        host_io = host_in.clone().pin_memory() if w.m > 0 else None
         e2e_step()
+        host_io.copy_(pristine)
         torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
         t0 = time.perf_counter()
-        for _ in range(e2e_steps):
+        for _ in range(steps):
             e2e_step()
         torch.cuda.synchronize()
-        res["e2e_s_per_step"] = (time.perf_counter() - t0) / e2e_steps
-        res["e2e_bytes"] = host_in.numel() * 8
+        res["e2e_ms_per_step"] = (time.perf_counter() - t0) / steps * 1e3
+        res["e2e_bytes"] = N * B * 8
+    gm.close()
     return res
 
 
+def roofline_block(w, r, ms_step, peaks, hbm_peak):
+    """The dominant kernel of the step is k_apply_tma (98-99 % of the step: profiles/*launches*): one launch = step / m."""
+    flops_launch = algorithmic_flops_per_cell_vector(w.p) * r["ncells"] * r["B"]
+    dur = ms_step * 1e-3 / r["napply"]
+    ach = flops_launch / dur / 1e12
+    instr_cv, flops_cv = executed_fp64_per_cell_vector(w.p)
+    peak = (peaks or {}).get("dfma_tflops") or FP64_NOMINAL_TFLOPS
+    ck = r.get("clocks") or {}
+    alg_bytes = (24 if w.m > 0 else 16) * r["N"] * r["B"]
+    traffic = NCU_TRAFFIC.get(w.index)
+    out = {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+           "peak_source": ("measured in this run: fe_diag_peak kind 0 (register-resident DFMA chains, best launch)"
+                           if (peaks or {}).get("dfma_tflops") else "nominal (no --peaks leg in this run)"),
+           "peak_nominal": FP64_NOMINAL_TFLOPS, "frac_of_nominal": ach / FP64_NOMINAL_TFLOPS,
+           "frac_kind": "useful work: ALGORITHMIC flops (24 n^4 + 9 n^3 per cell-vector, SURVEY 8(d)) / duration / peak; "
+                        "the even-odd kernel EXECUTES fewer flops (executed_*), so 1.0 is not the ceiling of this number",
+           "executed_tflops": flops_cv * r["ncells"] * r["B"] / dur / 1e12,
+           "executed_over_algorithmic_flops": flops_cv / algorithmic_flops_per_cell_vector(w.p),
+           "kernel": "k_apply_tma<p=%d> (one fused operator step: step time / m, CUDA events on the launching stream)" % w.p,
+           "launch_ms": dur * 1e3, "algorithmic_bytes": alg_bytes,
+           "traffic": traffic[0] if traffic else None,
+           "traffic_source": ("committed ncu capture %s (not measured in this run)" % traffic[1]) if traffic else None,
+           "hbm_frac_of_measured": (alg_bytes / dur / 1e9 / hbm_peak) if hbm_peak else None}
+    if ck.get("sm_mhz"):
+        # share of the FP64 pipe's issue cycles the executed instruction count needs at the sampled clock (the number ncu
+        # reports as sm__pipe_fp64_cycles_active: a warp-wide FP64 instruction holds a sub-partition's pipe for 2 cycles)
+        warp_instr = instr_cv * r["ncells"] * r["B"] / 32.0
+        out["fp64_pipe_busy_est"] = warp_instr * 2.0 / (148 * 4 * dur * ck["sm_mhz"] * 1e6)
+        if ck.get("sm_max_mhz"):
+            out["frac_at_sampled_clock"] = out["frac_of_nominal"] * ck["sm_max_mhz"] / ck["sm_mhz"]
+    return out
+
+
+def measure_peaks(fe, dev):
+    """Step-0 ceilings, measured through the C ABI (fe_diag_peak) before the timed workloads."""
+    sampler = ClockSampler(dev)
+    out = {"dfma_tflops": fe.fe_diag_peak(0, 0.4, dev), "dmma_tflops": fe.fe_diag_peak(1, 0.4, dev),
+           "stream_2r1w_gbs": fe.fe_diag_peak(2, 0.3, dev), "bulk_reduce_add_gbs": fe.fe_diag_peak(3, 0.3, dev),
+           "red_global_add_gbs": fe.fe_diag_peak(4, 0.3, dev)}
+    out["clocks"] = sampler.stop()
+    out["how"] = ("fe_diag_peak: best launch of >= 0.3 s back to back; DFMA = 8 chains x 8 warps x 4 CTAs/SM; DMMA = "
+                  "mma.sync.m8n8k4.f64 chains; stream = y = a x + z on 1 GiB arrays (3 x 8 B per element); reduce-add = "
+                  "payload bytes of cp.reduce.async.bulk.add.f64 / red.global.add.f64 into a 1 GiB array")
+    return out
+
+
+def time_orders(fe, torch, dev, peaks, hbm_peak, steps, warmup):
+    """--orders: every Lagrange order p = 2..8 on one ~2 M-node uniform mesh (B = 64, degree-12 filter, the config-2 well),
+    default launch shapes: the table of DESIGN.md 6.2."""
+    out = {}
+    for p in range(2, 9):
+        cells = max(2, int(round((2.0e6 ** (1.0 / 3.0) - 1) / p)))
+        e = workloads.uniform_edges(-10.0, 10.0, cells)
+        w = workloads.Workload(20 + p, "orders-p%d" % p, (e, e, e), p, 64, 12, "single", x_seed=20 + p)
+        r = time_workload(fe, torch, w, w.B, steps, warmup, dev)
+        rf = roofline_block(w, r, r["ms_per_step"], peaks, hbm_peak)
+        out["p%d" % p] = {"cells": cells, "N": r["N"], "ms_per_apply": r["ms_per_step"] / w.m,
+                          "value": r["N_free"] * w.B * w.m / (r["ms_per_step"] * 1e-3) / 1e9, "unit": UNIT,
+                          "frac": rf["frac"], "frac_of_nominal": rf["frac_of_nominal"],
+                          "fp64_pipe_busy_est": rf.get("fp64_pipe_busy_est"), "sm_mhz": (r["clocks"] or {}).get("sm_mhz")}
+        torch.cuda.empty_cache()
+    return out
+
+
 def time_consumers(fe, torch, w, dev):
-    """NEXT-1 / NEXT-2 on the workload's mesh (informational, --extra): one Rayleigh-Ritz call on a filtered block and
-    a fixed number of preconditioned MINRES steps with the config-5 shifts."""
+    """--consumers: NEXT-1 / NEXT-2 on the workload's mesh (informational): one Rayleigh-Ritz call on a filtered block,
+    the Gram product alone, and a fixed number of preconditioned MINRES steps with the config-5 shifts."""
     gm = fe.FEMesh(w.xe, w.ye, w.ze, w.p, device=dev)
     gm.set_potential(w.V(gm.quad_coords()))
     N, B = gm.N, w.B
@@ -272,114 +413,114 @@ def time_consumers(fe, torch, w, dev):
     _, _, it = gm.minres_shifted(G, eps, maxit=48, tol=0.0)
     torch.cuda.synchronize()
     mr_ms = (time.perf_counter() - t0) * 1e3 / it
+    gm.close()
     return {"mesh": w.describe(), "rayleigh_ritz_ms": rr_ms, "gram_ms": gram_ms,
             "gram_tflops": 2.0 * N * B * B / (gram_ms * 1e-3) / 1e12, "gram_gbs": 16.0 * N * B / (gram_ms * 1e-3) / 1e9,
             "minres_ms_per_step": mr_ms, "minres_steps_timed": it}
 
 
-def summarize(w, r, total_ms_per_step, n_ranks=1):
-    dofvec = r["N_free"] * r["B"] * r["napply"] * n_ranks
-    value = dofvec / (total_ms_per_step * 1e-3) / 1e9
-    flops_launch = algorithmic_flops_per_cell_vector(w.p) * r["ncells"] * r["B"]
-    dur = total_ms_per_step * 1e-3 / r["napply"]
-    ach = flops_launch / dur / 1e12
-    return value, {"bound": "alu", "achieved": ach, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
-                   "frac": ach / FP64_PEAK_TFLOPS, "traffic": None,
-                   "kernel": "k_apply_tma<p=%d> (one fused operator step: filter time / m, CUDA events on the launching stream)" % w.p,
-                   "launch_ms": dur * 1e3,
-                   "peak_source": "derived: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md); DFMA microbenchmark 36.8",
-                   "hbm_frac_of_measured": None}
-
-
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", type=int, default=2, choices=[2, 3, 4, 5])
+    ap.add_argument("--workload", type=int, default=4, choices=[2, 3, 4, 5],
+                    help="the workload of the line's `value` (default: config 4, the largest single-GPU one)")
+    ap.add_argument("--also", default="2,3,5", help="other roofline workloads measured into `workloads` ('' = none)")
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
-    ap.add_argument("--extra", action="store_true", help="also time the other roofline workloads (3, 4, 5)")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"])
+    ap.add_argument("--orders", action="store_true", help="also time p = 2..8 on one ~2 M-node mesh (DESIGN.md 6.2)")
+    ap.add_argument("--consumers", action="store_true", help="also time Rayleigh-Ritz / Gram / MINRES on config 2's mesh")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-peaks", action="store_true")
     ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--stub", action="store_true", help="rank-plumbing self-test on CPU (gloo): no GPU work, fake step times")
     args = ap.parse_args()
+    if args.warmup < 3 and not args.stub and args.impl == "native":
+        args.warmup = 3  # timing rule: at least three warm-up steps
     if args.impl == "reference":
         run_reference(args)
         return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        respawn_under_torchrun(args)
 
     import torch
-    import paper_2510_10529_b200 as fe
-    fe.load_library()  # fails loudly if the CUDA extension is missing
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    torch.cuda.set_device(local)
     w = workloads.config(args.workload)
-    r = time_workload(fe, torch, w, args.steps, args.warmup, local, seed_offset=rank, with_e2e=True, dist=dist,
-                      sample_clocks=(rank == 0), variant=args.variant)
-    from paper_2510_10529_b200.colsplit import max_over_ranks
-    # max over ranks; columns are sharded with no exchange (weak scaling)
-    ms_step, e2e_ms = max_over_ranks([r["ms_per_step"], r["e2e_s_per_step"] * 1e3], dist, device="cuda")
-    value, roof = summarize(w, r, ms_step, world)
-    hbm_peak = None
-    try:
-        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
-            hbm_peak = json.load(f)["hbm_gbs"]
-    except Exception:
-        pass
-    alg_bytes = (24 if w.m > 0 else 16) * r["N"] * r["B"]
-    roof["traffic"] = NCU_TRAFFIC_BYTES.get(args.workload)
-    roof["algorithmic_bytes"] = alg_bytes
-    roof["hbm_frac_of_measured"] = (alg_bytes / (roof["launch_ms"] * 1e-3) / 1e9 / hbm_peak) if hbm_peak else None
-    ck = r.get("clocks") or {}
-    if ck.get("sm_mhz") and ck.get("sm_max_mhz"):
-        # the FP64 peak above assumes the maximum SM clock; long runs sit in sw_power_cap below it
-        roof["frac_at_sampled_clock"] = roof["frac"] * ck["sm_max_mhz"] / ck["sm_mhz"]
+    B = columns_of_rank(w, rank, world, args.scaling)
+    dist = None
+    if args.stub:
+        device = "cpu"
+        if world > 1:
+            import torch.distributed as dist
+            dist.init_process_group("gloo")
+            dist.barrier()
+        r = stub_measurement(w, rank, B)
+        fe = peaks = hbm_peak = None
+    else:
+        import paper_2510_10529_b200 as fe
+        fe.load_library()  # fails loudly if the CUDA extension is missing
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+        device = "cuda"
+        if world > 1:
+            import torch.distributed as dist
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        torch.cuda.set_device(local)
+        hbm_peak = None
+        try:
+            with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+                hbm_peak = json.load(f)["hbm_gbs"]
+        except Exception:
+            pass
+        peaks = None if args.no_peaks else measure_peaks(fe, local)
+        r = time_workload(fe, torch, w, B, args.steps, args.warmup, local, seed_offset=rank, with_e2e=True, dist=dist,
+                          variant=args.variant)
+    job = job_line(w, r, world, dist, device, args.steps, args.warmup, args.scaling)
+    others = {}
+    if not args.stub:
+        torch.cuda.empty_cache()
+        for idx in [int(s) for s in args.also.split(",") if s.strip()]:
+            if idx == args.workload:
+                continue
+            wi = workloads.config(idx)
+            Bi = columns_of_rank(wi, rank, world, args.scaling)
+            ri = time_workload(fe, torch, wi, Bi, args.steps, args.warmup, local, seed_offset=rank, dist=dist,
+                               variant=args.variant)
+            ji = job_line(wi, ri, world, dist, device, args.steps, args.warmup, args.scaling)
+            others["cfg%d" % idx] = {"workload": wi.describe(), "value": ji["value"], "unit": UNIT,
+                                     "ms_per_step": ji["ms_per_step"], "l2": ri["l2"],
+                                     "filtered_blocks_per_s": world / (ji["ms_per_step"] * 1e-3) if wi.m > 0 else None,
+                                     "roofline": roofline_block(wi, ri, ji["ms_per_step"], peaks, hbm_peak),
+                                     "clocks": ri["clocks"], "gpu_launches": int(ri["launches"])}
+            torch.cuda.empty_cache()
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
         return
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": w.describe(), "columns_per_gpu": w.B,
-                       "l2": "3 rotating buffer sets, 3 x 141 MB blocks per filter > 126 MB L2" if r["N"] * r["B"] * 8 < 1 << 30
-                       else "blocks of %.2f GB >> L2" % (r["N"] * r["B"] * 8 / 1e9),
-                       "parallelism": "columns split over %d GPU(s), no collective" % world},
-            "roofline": roof, "clocks": r["clocks"], "gpu_launches": int(r["launches"]),
-            "e2e": {"value": r["N_free"] * r["B"] * r["napply"] * world / (e2e_ms * 1e-3) / 1e9, "unit": UNIT,
-                    "h2d_bytes_per_step": r["e2e_bytes"], "d2h_bytes_per_step": r["e2e_bytes"]},
-            "filtered_blocks_per_s": world / (ms_step * 1e-3) if w.m > 0 else None}
-    del r["gm"]
-    torch.cuda.empty_cache()
-    if args.extra and world == 1:
-        extra = {}
-        for idx in (3, 4, 5):
-            if idx == args.workload:
-                continue
-            wi = workloads.config(idx)
-            try:
-                ri = time_workload(fe, torch, wi, 2 if idx == 4 else 3, 1 if idx == 4 else 2, local, variant=args.variant)
-                vi, rfi = summarize(wi, ri, ri["ms_per_step"])
-                extra["cfg%d" % idx] = {"workload": wi.describe(), "value": vi, "unit": UNIT, "ms_per_step": ri["ms_per_step"],
-                                        "roofline_frac": rfi["frac"], "achieved_tflops": rfi["achieved"]}
-                del ri
-            except Exception as ex:  # e.g. out of memory on a smaller part
-                extra["cfg%d" % idx] = {"error": str(ex)[:200]}
-            torch.cuda.empty_cache()
-        line["other_workloads"] = extra
-        try:
-            line["consumers"] = time_consumers(fe, torch, w, local)
-        except Exception as ex:
-            line["consumers"] = {"error": str(ex)[:200]}
-        torch.cuda.empty_cache()
-    if world == 1 and not args.no_cpu_baseline:
-        line["cpu_baseline"] = cpu_baseline(args.workload, SAMPLE_CELLS[args.workload])
+    line = {"metric": METRIC, "value": job["value"], "unit": UNIT, "n_gpus": job["n_gpus"], "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": job["ms_per_step"], "higher_is_better": True, "scaling": args.scaling,
+            "vs_baseline": None, "dtype": "f64", "data": "stub" if args.stub else "synthetic",
+            "config": {"workload": w.describe(), "columns_per_gpu": B, "columns_total": job["columns_total"],
+                       "l2": r.get("l2"), "parallelism": "columns split over %d GPU(s), no collective" % world},
+            "gpu_launches": int(r["launches"]),
+            "e2e": {"value": job["e2e_value"], "unit": UNIT, "h2d_bytes_per_step": r["e2e_bytes"],
+                    "d2h_bytes_per_step": r["e2e_bytes"], "steps": args.steps,
+                    "how": "cheb_filter_host on a pinned HOST block: H2D, filter, D2H inside the timed region, every step"},
+            "filtered_blocks_per_s": world / (job["ms_per_step"] * 1e-3) if w.m > 0 else None}
+    if not args.stub:
+        line["roofline"] = roofline_block(w, r, job["ms_per_step"], peaks, hbm_peak)
+        line["clocks"] = r["clocks"]
+        line["workloads"] = others
+        line["peaks"] = peaks
+        if args.orders and world == 1:
+            line["orders"] = time_orders(fe, torch, local, peaks, hbm_peak, 3, 3)
+        if args.consumers and world == 1:
+            line["consumers"] = time_consumers(fe, torch, workloads.config(2), local)
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(args.workload, SAMPLE_CELLS[args.workload])
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()

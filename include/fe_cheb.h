@@ -143,6 +143,15 @@ int fe_set_variant(fe_mesh* m, int variant);
 /* Kernels launched by this handle since creation (bench.py's gpu_launches). */
 int64_t fe_launch_count(const fe_mesh* m);
 
+/* Step-0 ceilings of the device (not on the product path): a diagnostic kernel of the given
+ * kind is launched back to back for at least min_seconds (0 < min_seconds <= 30) and the best launch is reported in
+ * *value_host (HOST):  kind 0 = register-resident DFMA chains, TFLOP/s (the FP64 pipe that bounds fe_apply_H / cheb_filter);
+ * 1 = mma.sync.m8n8k4.f64 chains, TFLOP/s (the FP64 tensor path; tcgen05 has no FP64 kind);  2 = y = a x + z over 1 GiB
+ * arrays, GB/s of the two reads and one write (the 24 B per node-vector of a filter step);  3 = cp.reduce.async.bulk
+ * .add.f64 shared -> global, GB/s of payload (the scatter of the TMA kernel);  4 = red.global.add.f64, GB/s of payload (the
+ * scatter of the legacy kernel).  Allocates and frees its own buffers (up to 3 GiB).  Synchronous. */
+int fe_diag_peak(int cuda_device, int kind, double min_seconds, double* value_host);
+
 const char* fe_last_error(void);
 
 #ifdef __cplusplus

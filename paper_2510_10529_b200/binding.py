@@ -7,14 +7,14 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.environ.get("FECHEB_LIB") or os.path.join(_HERE, "libfecheb.so")  # FECHEB_LIB: A/B builds of the library
+_SO = os.path.join(_HERE, "libfecheb.so")
 _lib = None
 
 EXPORTS = (
     "fe_mesh_create", "fe_mesh_destroy", "fe_num_nodes", "fe_num_free", "fe_num_cells", "fe_nodes_per_cell",
     "fe_quad_per_cell", "fe_get_l2g", "fe_get_node_coords", "fe_get_quad_coords", "fe_get_mass",
     "fe_get_dirichlet_mask", "fe_set_potential", "fe_apply_H", "cheb_filter", "cheb_filter_host", "fe_rayleigh_ritz", "fe_minres_shifted", "fe_add_subspace", "fe_gram", "fe_density", "fe_lanczos_bounds", "fe_apply_potential",
-    "fe_set_variant",
+    "fe_set_variant", "fe_diag_peak",
     "fe_launch_count", "fe_last_error",
 )
 
@@ -63,6 +63,7 @@ def load_library():
     L.fe_gram.restype, L.fe_gram.argtypes = C.c_int, [vp, vp, vp, C.c_int, vp, vp]
     L.fe_add_subspace.restype, L.fe_add_subspace.argtypes = C.c_int, [vp, vp, vp, vp, C.c_int, vp]
     L.fe_set_variant.restype, L.fe_set_variant.argtypes = C.c_int, [vp, C.c_int]
+    L.fe_diag_peak.restype, L.fe_diag_peak.argtypes = C.c_int, [C.c_int, C.c_int, C.c_double, dp]
     L.fe_last_error.restype, L.fe_last_error.argtypes = C.c_char_p, []
     _lib = L
     return L
@@ -276,6 +277,13 @@ def fe_add_subspace(h, Psi, D, P, stream=None):
     _check(load_library().fe_add_subspace(h, _dev_ptr(Psi, "Psi"), Dh.ctypes.data_as(C.c_void_p),
                                           _dev_ptr(P, "P", Psi.numel()), B, _stream(stream)))
     return P
+
+
+def fe_diag_peak(kind, min_seconds=0.3, cuda_device=0):
+    """Measured ceiling of the device: kind 0 DFMA / 1 DMMA in TFLOP/s, 2 stream / 3 bulk reduce-add / 4 red.add in GB/s."""
+    out = C.c_double(0.0)
+    _check(load_library().fe_diag_peak(int(cuda_device), int(kind), float(min_seconds), C.byref(out)))
+    return out.value
 
 
 def fe_set_variant(h, variant):

@@ -19,6 +19,7 @@
 
 #include "fe_apply_tma.cuh"
 #include "fe_density.cuh"
+#include "fe_diag.cuh"
 #include "fe_minres.cuh"
 #include "fe_rr.cuh"
 #include "fe_kernels.cuh"
@@ -1028,4 +1029,67 @@ int fe_apply_potential(fe_mesh* m, const double* Uq_dev, const double* X, double
     if (e != cudaSuccess) return fail(FE_ERR_CUDA, "fe_apply_potential: launch failed: %s", cudaGetErrorString(e));
     m->launches += 1 + nl;
     return FE_OK;
+}
+
+// ---- step-0 ceilings (fe_diag.cuh): not on the product path; bench.py prints them beside the roofline ---------------------
+int fe_diag_peak(int cuda_device, int kind, double min_seconds, double* value_host)
+{
+    if (!value_host) return fail(FE_ERR_INVALID, "fe_diag_peak: NULL result");
+    if (kind < 0 || kind > 4) return fail(FE_ERR_INVALID, "fe_diag_peak: kind %d outside 0..4", kind);
+    if (!(min_seconds > 0.0) || min_seconds > 30.0) return fail(FE_ERR_INVALID, "fe_diag_peak: min_seconds outside (0, 30]");
+    CUDA_TRY(cudaSetDevice(cuda_device));
+    cudaDeviceProp prop;
+    CUDA_TRY(cudaGetDeviceProperties(&prop, cuda_device));
+    const int sms = prop.multiProcessorCount;
+    const long long n = 1ll << 27;  // doubles per array of the memory kinds: 1 GiB, far beyond the 126 MB L2
+    double *a = nullptr, *b = nullptr, *c = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    int rc = FE_OK;
+    double work = 0.0;  // flops or bytes per launch
+    auto launch = [&]() {
+        switch (kind) {
+            case 0: k_diag_dfma<8><<<sms * 4, 256>>>(a, 4096, 0.999999, 1e-7); break;
+            case 1: k_diag_dmma<<<sms * 4, 256>>>(a, 4096, 0.25, 1e-3); break;
+            case 2: k_diag_stream<<<sms * 16, 256>>>((const double2*)a, (const double2*)b, (double2*)c, n / 2, 0.5); break;
+            case 3: k_diag_bulk_red<16384><<<sms * 4, 128, 16384>>>(a, n * 8 / 16384); break;
+            default: k_diag_red<<<sms * 16, 256>>>(a, n, 1.0); break;
+        }
+    };
+    do {
+        const size_t small = (size_t)sms * 4 * 256 * sizeof(double);
+        cudaError_t ce = cudaMalloc((void**)&a, kind <= 1 ? small : (size_t)n * sizeof(double));
+        if (ce == cudaSuccess && kind == 2) ce = cudaMalloc((void**)&b, (size_t)n * sizeof(double));
+        if (ce == cudaSuccess && kind == 2) ce = cudaMalloc((void**)&c, (size_t)n * sizeof(double));
+        if (ce == cudaSuccess && kind >= 2) ce = cudaMemset(a, 0, (size_t)n * sizeof(double));
+        if (ce == cudaSuccess && kind == 2) ce = cudaMemset(b, 0, (size_t)n * sizeof(double));
+        if (ce == cudaSuccess) ce = cudaEventCreate(&e0);
+        if (ce == cudaSuccess) ce = cudaEventCreate(&e1);
+        if (ce != cudaSuccess) { rc = fail(FE_ERR_NOMEM, "fe_diag_peak: setup failed: %s", cudaGetErrorString(ce)); break; }
+        const double threads = (double)sms * 4 * 256;
+        if (kind == 0) work = threads * 4096.0 * 16 * 8 * 2;            // iters x unroll x chains x (mul + add)
+        else if (kind == 1) work = threads / 32 * 4096.0 * 8 * 4 * 512;  // warps x iters x unroll x chains x 8*8*4*2
+        else if (kind == 2) work = 3.0 * n * 8;
+        else work = 1.0 * n * 8;                                          // payload bytes added into global memory
+        if (kind == 3) cudaFuncSetAttribute(k_diag_bulk_red<16384>, cudaFuncAttributeMaxDynamicSharedMemorySize, 16384);
+        launch();  // warm-up
+        ce = cudaDeviceSynchronize();
+        if (ce != cudaSuccess) { rc = fail(FE_ERR_CUDA, "fe_diag_peak: kernel failed: %s", cudaGetErrorString(ce)); break; }
+        double best = 0.0, total = 0.0;
+        while (total < min_seconds) {
+            cudaEventRecord(e0);
+            launch();
+            cudaEventRecord(e1);
+            ce = cudaEventSynchronize(e1);
+            float ms = 0.f;
+            if (ce == cudaSuccess) ce = cudaEventElapsedTime(&ms, e0, e1);
+            if (ce != cudaSuccess || !(ms > 0.f)) { rc = fail(FE_ERR_CUDA, "fe_diag_peak: timing failed: %s", cudaGetErrorString(ce)); break; }
+            total += ms * 1e-3;
+            best = std::max(best, work / (ms * 1e-3));
+        }
+        *value_host = best * (kind <= 1 ? 1e-12 : 1e-9);  // TFLOP/s or GB/s, best launch
+    } while (false);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaFree(a); cudaFree(b); cudaFree(c);
+    return rc;
 }

@@ -74,3 +74,36 @@ def test_column_split_world2(tmp_path):
     F = np.concatenate([np.load(tmp_path / ("F%d.npy" % r)) for r in range(world)], axis=1)
     assert np.array_equal(Y, om.apply(X, eps))
     assert np.array_equal(F, om.filter(X, 6, 3.0, 25.0, 1.0))
+
+
+def _bench_stub(*flags):
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--stub", "--workload", "2", "--steps", "2",
+                          *flags], capture_output=True, text=True, env=env, timeout=600)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [ln for ln in out.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, out.stdout  # rank 0 alone prints
+    return json.loads(lines[0])
+
+
+def test_bench_rank_logic_world2_gloo():
+    """bench.py's own N > 1 path on CPU: `python bench.py --gpus 2` with no torchrun environment must start two ranks
+    itself; the step time of the line is the MAX over ranks, the value the units of ALL ranks over that time (weak
+    scaling: every rank its own B columns; strong: the B columns dealt out).  --stub replaces the GPU step by a fixed fake
+    time per rank (10 ms x (rank + 1)); everything else is the code path the driver runs."""
+    w = workloads.config(2)
+    one = _bench_stub("--gpus", "1")
+    assert one["n_gpus"] == 1 and one["data"] == "stub" and one["ms_per_step"] == 10.0
+    assert one["value"] == pytest.approx(w.N_free * w.B * w.m / 0.010 / 1e9)
+    two = _bench_stub("--gpus", "2")
+    assert two["n_gpus"] == 2 and two["scaling"] == "weak" and two["ms_per_step"] == 20.0  # the slower rank
+    assert two["config"]["columns_per_gpu"] == w.B and two["config"]["columns_total"] == 2 * w.B
+    assert two["value"] == pytest.approx(2 * w.N_free * w.B * w.m / 0.020 / 1e9)
+    assert two["e2e"]["value"] == pytest.approx(2 * w.N_free * w.B * w.m / 0.040 / 1e9)
+    strong = _bench_stub("--gpus", "2", "--scaling", "strong")
+    assert strong["config"]["columns_per_gpu"] == w.B // 2 and strong["config"]["columns_total"] == w.B
+    assert strong["value"] == pytest.approx(w.N_free * w.B * w.m / 0.020 / 1e9)

@@ -1,0 +1,213 @@
+"""GPU parity at the FULL BASELINE.json sizes, in the launch configurations bench.py times (readings R16, R19, R20, R22).
+
+Configs 2 and 5 (p=4, 274 625 nodes, B=64): the oracle affords everything -- every cell matrix by explicit quadrature,
+the assembled CSR of H~ (57 M non-zeros), the serial three-term recurrence on ALL 64 columns -- so the filter (m=20), the
+five filter + Rayleigh-Ritz cycles and calls 1, 2 and 200 of the shifted-apply sequence are compared directly.
+Configs 3 and 4 (p=6, 3 M / 14 M nodes): the oracle computes sampled rows of one apply straight from Eq. 17
+(orc_apply_rows), on the real B=128 block at config 4; the filter at the configured degree is tied to fe_apply_H by the
+three-term recurrence assembled from single applies (a property that holds at any size).
+"""
+import os
+
+import numpy as np
+import pytest
+
+import workloads
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL_APPLY = 1e-11
+TOL_FILTER = 1e-9
+TOL_RITZ = 1e-9
+NT = os.cpu_count() or 1
+
+
+def _dev(a):
+    return torch.as_tensor(np.ascontiguousarray(a), device="cuda")
+
+
+def _relerr(Yg, Yo, free):
+    return np.linalg.norm(Yg[free] - Yo[free]) / max(np.linalg.norm(Yo[free]), 1e-300)
+
+
+@pytest.fixture(scope="module")
+def cfg2():
+    """Config 2's mesh and potential (config 5 uses the same): oracle with all cell matrices and the CSR, GPU mesh."""
+    import oracle
+    import paper_2510_10529_b200 as fe
+    w = workloads.config(2)
+    om = oracle.OracleMesh(w.xe, w.ye, w.ze, w.p)
+    Vq = w.V(om.quad_coords())
+    om.set_potential(Vq)
+    om.assemble()
+    gm = fe.FEMesh(w.xe, w.ye, w.ze, w.p)
+    gm.set_potential(Vq)
+    assert np.array_equal(gm.mask(), om.mask()) and np.array_equal(gm.l2g(), om.l2g())
+    th_min, th_max, beta = oracle.lanczos_bounds(om, workloads.normal(3002, om.N), 20, nthreads=NT)
+    return w, om, gm, (th_min, th_max + beta)
+
+
+def test_filter_config2_full_size_all_columns(cfg2):
+    """BASELINE config 2 as configured: 16^3 cells, p=4, B=64, m=20, bounds from 20 Lanczos steps (R10) -- cheb_filter
+    against the oracle's CSR recurrence on every column (R16: <= 1e-9 over free rows; Dirichlet rows exactly 0)."""
+    w, om, gm, (a0, b) = cfg2
+    mask = om.mask()
+    free = mask.astype(bool)
+    X = w.X(mask)
+    a = a0 + 0.1 * (b - a0)
+    Yo = om.filter(X, w.m, a, b, a0, nthreads=NT)
+    Yg = gm.cheb_filter(_dev(X), w.m, a, b, a0).cpu().numpy()
+    assert _relerr(Yg, Yo, free) <= TOL_FILTER
+    worst = max(_relerr(Yg[:, j:j + 1], Yo[:, j:j + 1], free) for j in range(w.B))
+    assert worst <= TOL_FILTER  # column by column: columns 0 and 63 and both 32-vector tiles included
+    assert np.all(Yg[~free] == 0)
+
+
+def test_config2_five_filter_rr_cycles_full_size(cfg2):
+    """R20 at full size (N = 274 625, B = 64): every cycle the GPU filter is fed the oracle's block (lock-step gate
+    <= 1e-9), and the free-running device cycles (cheb_filter + fe_rayleigh_ritz, window from the previous Ritz values)
+    must give the oracle's Ritz values of the final cycle to <= 1e-9 (R16)."""
+    import oracle
+    w, om, gm, (a0, b) = cfg2
+    mask = om.mask()
+    free = mask.astype(bool)
+    Xo = w.X(mask)
+    Xg = _dev(Xo)
+    a = a0 + 0.1 * (b - a0)
+    ag, a0g = a, a0
+    work = torch.empty(2 * Xg.numel(), dtype=torch.float64, device="cuda")
+    for cycle in range(5):
+        Yo = om.filter(Xo, w.m, a, b, a0, nthreads=NT)
+        Ylock = gm.cheb_filter(_dev(Xo), w.m, a, b, a0, work).cpu().numpy()
+        assert _relerr(Ylock, Yo, free) <= TOL_FILTER, cycle
+        theta_o, Xo, _ = oracle.rayleigh_ritz(om, Yo, nthreads=NT)
+        gm.cheb_filter(Xg, w.m, ag, b, a0g, work)
+        theta_g = gm.rayleigh_ritz(Xg, work[:Xg.numel()])
+        a, a0 = theta_o[-1], theta_o[0]
+        ag, a0g = theta_g[-1], theta_g[0]
+    assert np.max(np.abs(theta_g - theta_o) / np.maximum(1.0, np.abs(theta_o))) <= TOL_RITZ
+    Q = Xg.cpu().numpy()
+    assert np.max(np.abs(Q.T @ Q - np.eye(w.B))) <= 1e-12
+    assert np.all(Q[~free] == 0)
+
+
+def test_config5_calls_1_2_200(cfg2):
+    """R19: 200 calls Y_t = (H~ - eps) X_{t mod 2} alternating two seeded input blocks and two output blocks, as bench.py
+    times them; the outputs of calls 1, 2 and 200 against the oracle's CSR apply on ALL rows and columns (<= 1e-11)."""
+    _, om, gm, _ = cfg2
+    w = workloads.config(5)
+    mask = om.mask()
+    free = mask.astype(bool)
+    eps = w.eps()
+    X = [w.X(mask), w.X(mask, seed=w.x_seed + 100)]
+    Yo = [om.apply(X[i], eps, nthreads=NT) for i in range(2)]
+    Xd = [_dev(X[0]), _dev(X[1])]
+    Yd = [torch.full_like(Xd[0], 3.5), torch.full_like(Xd[0], -1.25)]  # dirty output blocks
+    ed = _dev(eps)
+    for t in range(w.n_applies):
+        gm.apply_H(Xd[t % 2], Yd[t % 2], ed)
+        if t in (0, 1, w.n_applies - 1):
+            Yg = Yd[t % 2].cpu().numpy()
+            assert _relerr(Yg, Yo[t % 2], free) <= TOL_APPLY, t + 1
+            assert np.all(Yg[~free] == 0)
+
+
+# ---- configs 3 and 4: sampled rows of one apply, filter through the recurrence property -----------------------------------
+def _cells_of_row(w, g):
+    """All cells (ex, ey, ez) whose node set contains global node g (R3 numbering)."""
+    nx, ny, _ = w.nodes_per_axis
+    idx = (g % nx, (g // nx) % ny, g // (nx * ny))
+    per_axis = []
+    for d, c in zip(idx, w.cells):
+        cand = {min(d // w.p, c - 1)}
+        if d % w.p == 0 and d > 0:
+            cand.add(d // w.p - 1)
+        per_axis.append(sorted(cand))
+    return [(ex, ey, ez) for ez in per_axis[2] for ey in per_axis[1] for ex in per_axis[0]]
+
+
+def test_apply_config4_full_block_B128_sampled_rows():
+    """Config 4 in the shape the bench times: the graded 40^3-cell p=6 mesh with the real B = 128 block (four 32-vector
+    tiles per cell, 14.3 GB per block, byte offsets beyond 2^32, the blocked walk with 256 000 units).  The oracle
+    evaluates sampled rows (all 128 columns) one entry of Eq. 17 at a time; rows include the last z-slabs.  Only the rows
+    of X those entries touch are brought to the host (the host copy of X is a lazily committed zero array)."""
+    import oracle
+    import paper_2510_10529_b200 as fe
+    w = workloads.config(4)
+    om = oracle.OracleMesh(w.xe, w.ye, w.ze, w.p)
+    Vq = w.V(om.quad_coords())
+    om.set_potential(Vq, build=False)
+    gm = fe.FEMesh(w.xe, w.ye, w.ze, w.p)
+    gm.set_potential(Vq)
+    B = w.B
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(4128)
+    Xd = torch.randn(gm.N, B, dtype=torch.float64, device="cuda", generator=gen)  # Dirichlet rows hold data too (R5)
+    nx, ny, nz = w.nodes_per_axis
+    u = workloads.uniform01(9128, 0, 3 * 36).reshape(36, 3)
+    gx = np.minimum((u[:, 0] * nx).astype(np.int64), nx - 1)
+    gy = np.minimum((u[:, 1] * ny).astype(np.int64), ny - 1)
+    gz = np.minimum((u[:, 2] * nz).astype(np.int64), nz - 1)
+    gz[:12] = nz - 2 - (gz[:12] % 13)          # the last two z-slabs of cells: element offsets g*B > 2^32 / 8
+    gx[:9] = (gx[:9] // w.p) * w.p             # cell faces / edges / vertices
+    gy[:5] = (gy[:5] // w.p) * w.p
+    gz[9:12] = nz - 1 - w.p                    # a cell face in z near the end of the block
+    rows = np.unique(gx + nx * (gy + ny * gz))
+    assert rows.max() * B * 8 > 2**32
+    l2g = om.l2g()
+    cx, cy, _ = w.cells
+    need = np.unique(np.concatenate([l2g[ex + cx * (ey + cy * ez)] for g in rows for ex, ey, ez in _cells_of_row(w, int(g))]))
+    X = np.zeros((om.N, B))  # calloc: pages are committed only where written
+    mask = om.mask()
+    X[need] = Xd[torch.as_tensor(need, device="cuda")].cpu().numpy() * mask[need, None]
+    Yo = om.apply_rows(X, rows, None)
+    del X
+    Yg = gm.apply_H(Xd)
+    Ys = Yg[torch.as_tensor(rows, device="cuda")].cpu().numpy()
+    assert np.linalg.norm(Ys - Yo) <= TOL_APPLY * np.linalg.norm(Yo)
+    for t in range(4):  # every 32-vector tile on its own
+        sl = slice(32 * t, 32 * t + 32)
+        assert np.linalg.norm(Ys[:, sl] - Yo[:, sl]) <= TOL_APPLY * np.linalg.norm(Yo[:, sl]), t
+    bnd = torch.as_tensor(np.flatnonzero(mask == 0)[::97], device="cuda")
+    assert float(Yg[bnd].abs().max()) == 0.0
+
+
+@pytest.mark.parametrize("cfg", [2, 3, 4])
+def test_filter_full_size_configured_degree(cfg):
+    """cheb_filter at the CONFIGURED degree (m = 20 / 30 / 40, so m mod 3 = 2, 0, 1: every final-copy case of the rotating
+    blocks) on the full block, in the launch shapes bench.py times, equals the three-term recurrence (R7) assembled from
+    fe_apply_H calls, which the sampled-row tests tie to the oracle.  Holds at any size; the recurrence runs in place on
+    three blocks so that config 4 (14.3 GB per block) fits."""
+    import paper_2510_10529_b200 as fe
+    w = workloads.config(cfg)
+    gm = fe.FEMesh(w.xe, w.ye, w.ze, w.p)
+    gm.set_potential(w.V(gm.quad_coords()))
+    mask = _dev(gm.mask().astype(np.float64))[:, None]
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(5100 + cfg)
+    X = torch.randn(gm.N, w.B, dtype=torch.float64, device="cuda", generator=gen)
+    X.mul_(mask)
+    a0, a, b = {2: (-6.0, -0.5, 190.0), 3: (-12.0, -1.0, 1200.0), 4: (-30.0, -2.0, 4.0e4)}[cfg]
+    m = w.m
+    Yf = X.clone()
+    work = torch.empty(2 * X.numel(), dtype=torch.float64, device="cuda")
+    gm.cheb_filter(Yf, m, a, b, a0, work)
+    del work
+    e, c = (b - a) / 2, (b + a) / 2
+    s1 = e / (a0 - c)
+    s = s1
+    Ykm, Yk = X, torch.empty_like(X)
+    gm.apply_H(Ykm, Yk)
+    Yk.add_(Ykm, alpha=-c).mul_(s1 / e)
+    H = torch.empty_like(X)
+    for _ in range(1, m):
+        sn = 1.0 / (2.0 / s1 - s)
+        gm.apply_H(Yk, H)
+        H.add_(Yk, alpha=-c).mul_(2 * sn / e).add_(Ykm, alpha=-s * sn)
+        Ykm, Yk, H = Yk, H, Ykm
+        s = sn
+    del Ykm, H
+    Yf.sub_(Yk).mul_(mask)
+    Yk.mul_(mask)
+    assert float(torch.linalg.norm(Yf) / torch.linalg.norm(Yk)) <= 1e-12

@@ -431,30 +431,6 @@ def _sample_rows(w, count, seed):
     return np.unique(gx + nx * (gy + ny * gz))
 
 
-def test_apply_config4_mesh_sampled_rows():
-    """Config 4's graded 40^3-cell p=6 mesh (14 M nodes) at full size, in the persistent 32-vector launch shape the
-    bench times, on a 32-column slice of the block (columns are independent, R22): sampled rows against Eq. 17."""
-    import oracle
-    fe = _fe()
-    w = workloads.config(4)
-    om = oracle.OracleMesh(w.xe, w.ye, w.ze, w.p)
-    Vq = w.V(om.quad_coords())
-    om.set_potential(Vq, build=False)
-    gm = fe.FEMesh(w.xe, w.ye, w.ze, w.p)
-    gm.set_potential(Vq)
-    B = 32
-    gen = torch.Generator(device="cuda")
-    gen.manual_seed(4004)
-    Xd = torch.randn(gm.N, B, dtype=torch.float64, device="cuda", generator=gen)  # seeded device input, copied out below
-    rows = _sample_rows(w, 40, 9004)
-    # the oracle needs the whole block on the host only where the sampled rows reach: copy it once
-    X = Xd.cpu().numpy()
-    Yo = om.apply_rows(X * om.mask()[:, None], rows, None)
-    Yg = gm.apply_H(Xd)
-    Ys = Yg[torch.as_tensor(rows, device="cuda")].cpu().numpy()
-    assert np.linalg.norm(Ys - Yo) <= TOL_APPLY * np.linalg.norm(Yo)
-
-
 @pytest.mark.parametrize("cfg", [2, 5, 3])
 def test_apply_full_size_sampled_rows(cfg):
     """Full BASELINE sizes in the launch configuration bench.py times; the oracle computes sampled rows one by one
@@ -481,30 +457,71 @@ def test_apply_full_size_sampled_rows(cfg):
     assert float(Yg[bnd].abs().max()) == 0.0
 
 
-@pytest.mark.parametrize("cfg", [2, 3])
-def test_filter_full_size_property(cfg):
-    """Configs 2 and 3 at full size, in the launch shapes bench.py times (one CTA per unit at p=4, the persistent
-    32-wide CTA at p=6): cheb_filter (pre-initialised recurrence) equals the three-term recurrence assembled from
-    fe_apply_H calls (which the sampled-row tests tie to the oracle); holds at any size."""
+# ---- the persistent loop of k_apply_tma (default at p = 5, 7, 8 and the 32-wide p = 6 shape; variants 7 / 8 elsewhere) ----
+BIG = (np.array([0.0, 0.5, 1.1, 1.5, 2.2, 2.6, 3.3]), np.array([-1.0, -0.6, 0.1, 0.5, 1.2, 1.5, 2.0]),
+       np.array([0.0, 0.4, 0.7, 1.3, 1.6, 2.1]))  # 6 x 6 x 5 = 180 unequal cells: more units than the 148 persistent CTAs
+
+
+@pytest.mark.parametrize("p,B,variant", [(5, 6, 0), (5, 34, 0), (7, 6, 0), (7, 34, 0), (8, 6, 0), (8, 34, 0), (6, 34, 0),
+                                         (2, 130, 7), (3, 130, 7), (4, 130, 7), (6, 34, 7), (6, 6, 8), (6, 34, 8), (6, 34, 6)])
+def test_persistent_loop_parity(p, B, variant):
+    """A mesh with more units than resident CTAs, so that every persistent CTA walks several units (bar[1] handshake,
+    rec / recN swap, mid-unit next-tile request, the BT = 16 shape with two planes per warp at p = 7, 8; B = 130 gives
+    the several-CTAs-per-SM shapes of p <= 4 more units than their 888 / 592 / 444 resident CTAs).  One shifted
+    apply: sampled rows against the oracle's entry-by-entry Eq. 17 and ALL rows against the colour-ordered legacy kernel
+    (variant 4, the race oracle of R17).  A degree-5 filter: against the legacy kernel's recurrence."""
+    import oracle
     fe = _fe()
-    w = workloads.config(cfg)
-    gm = fe.FEMesh(w.xe, w.ye, w.ze, w.p)
-    gm.set_potential(w.V(gm.quad_coords()))
-    mask = _dev(gm.mask().astype(np.float64))[:, None]
-    gen = torch.Generator(device="cuda")
-    gen.manual_seed(5000 + cfg)
-    X = torch.randn(gm.N, w.B, dtype=torch.float64, device="cuda", generator=gen) * mask
-    a0, a, b, m = -6.0, -0.5, (190.0 if cfg == 2 else 1200.0), 7
-    e, c = (b - a) / 2, (b + a) / 2
-    s1 = e / (a0 - c)
-    s = s1
-    Ykm, Yk = X, (s1 / e) * (gm.apply_H(X) - c * X)
-    for _ in range(1, m):
-        sn = 1.0 / (2.0 / s1 - s)
-        Ykm, Yk = Yk, (2 * sn / e) * (gm.apply_H(Yk) - c * Yk) - s * sn * Ykm
-        s = sn
-    Yf = gm.cheb_filter(X.clone(), m, a, b, a0)
-    assert float(torch.linalg.norm((Yf - Yk) * mask) / torch.linalg.norm(Yk * mask)) <= 1e-12
+    om = oracle.OracleMesh(*BIG, p)
+    Vq = _coulomb(om.quad_coords())
+    om.set_potential(Vq, build=False)
+    gm = fe.FEMesh(*BIG, p)
+    gm.set_potential(Vq)
+    mask = om.mask()
+    X = workloads.random_block(1300 + p, om.N, B)  # data in the Dirichlet rows: ignored
+    eps = workloads.shifts(2300 + p, B)
+    rows = np.unique((workloads.uniform01(9300 + p, 0, 120) * om.N).astype(np.int64))
+    Yo = om.apply_rows(X * mask[:, None], rows, eps)
+    Xd, ed = _dev(X), _dev(eps)
+    gm.set_variant(4)
+    Yref = gm.apply_H(Xd, eps=ed).clone()
+    Fref = gm.cheb_filter(Xd.clone(), 5, -2.0, 900.0, -12.0)
+    gm.set_variant(variant)
+    Yg = gm.apply_H(Xd, eps=ed)
+    Ys = Yg[torch.as_tensor(rows, device="cuda")].cpu().numpy()
+    assert np.linalg.norm(Ys - Yo) <= TOL_APPLY * np.linalg.norm(Yo)
+    assert float(torch.linalg.norm(Yg - Yref) / torch.linalg.norm(Yref)) <= 1e-13
+    assert np.all(Yg.cpu().numpy()[mask == 0] == 0)
+    Fg = gm.cheb_filter(Xd.clone(), 5, -2.0, 900.0, -12.0)
+    assert float(torch.linalg.norm(Fg - Fref) / torch.linalg.norm(Fref)) <= 1e-12
+    assert np.all(Fg.cpu().numpy()[mask == 0] == 0)
+
+
+def test_adjoint_scratch_survives_host_filter():
+    """One handle: fe_apply_potential, then cheb_filter_host on a wider block (its staging is regrown), then
+    fe_apply_potential again -- the adjoint scratch must stay valid across the regrowth."""
+    import oracle
+    fe = _fe()
+    p = 3
+    om = oracle.OracleMesh(*UNEQUAL, p)
+    gm = fe.FEMesh(*UNEQUAL, p)
+    Vq = _coulomb(om.quad_coords())
+    om.set_potential(Vq)
+    om.assemble()
+    gm.set_potential(Vq)
+    mask = om.mask()
+    Uq = np.cos(om.quad_coords()).prod(axis=1) - 0.3
+    Psi = workloads.random_block(1400, om.N, 6, mask)
+    Go = oracle.adjoint_rhs(om, Psi, np.ones(6), Uq, np.zeros((6, 6)))
+    G1 = gm.apply_potential(_dev(Uq), _dev(Psi)).cpu().numpy()
+    assert _relerr(G1, Go, mask) <= TOL_APPLY
+    for B in (4, 64, 96):  # growing staging
+        Xh = workloads.random_block(1401 + B, om.N, B, mask)
+        Yo = om.filter(Xh, 4, 3.0, 2500.0, -10.0)
+        gm.cheb_filter_host(Xh, 4, 3.0, 2500.0, -10.0)
+        assert _relerr(Xh, Yo, mask) <= TOL_FILTER
+        G2 = gm.apply_potential(_dev(Uq), _dev(Psi)).cpu().numpy()
+        assert _relerr(G2, Go, mask) <= TOL_APPLY
 
 
 # ---- error behaviour -------------------------------------------------------------------------------------------------
