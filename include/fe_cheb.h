@@ -143,6 +143,24 @@ int fe_set_variant(fe_mesh* m, int variant);
 /* Kernels launched by this handle since creation (bench.py's gpu_launches). */
 int64_t fe_launch_count(const fe_mesh* m);
 
+/* Ritz residual norms  res[j] = || H~ x_j - theta_j x_j ||_2  over the free rows, for a block X (DEVICE, N*B) and B values
+ * theta_host (HOST): the quantity the eigensolver tolerance t_eig of l.296 is applied to.  One fused shifted apply
+ * (Eq. 20 with eps = theta) plus one column reduction.  res_host: HOST, B doubles.  work: DEVICE, N*B doubles, must not
+ * overlap X.  1 <= B <= 128.  Synchronous. */
+int fe_ritz_residuals(fe_mesh* m, const double* X, const double* theta_host, int B, double* res_host, double* work,
+                      void* cuda_stream);
+
+/* Chebyshev-filtered subspace iteration driven by the residual (l.208-219, l.296): repeat { cheb_filter of degree deg on
+ * the window (a0, a, b); fe_rayleigh_ritz; fe_ritz_residuals } until the residual norms of the n_gate lowest Ritz pairs
+ * (the occupied states) are all <= t_eig, or max_cycles cycles have run.  The paper sets t_eig = e_L2^2 / c_eig from the
+ * density error of the previous outer iteration (c_eig = 100 by default); the caller passes the number.  After every
+ * cycle the window becomes a = largest, a0 = smallest Ritz value of the block; b (an upper bound of the spectrum, e.g.
+ * from fe_lanczos_bounds) is kept.  X: DEVICE N*B, in: start block, out: Ritz vectors.  theta_host, res_host: HOST, B
+ * doubles of the last cycle.  cycles_host: HOST int or NULL.  work: DEVICE 2*N*B doubles.  Synchronous.
+ * FE_ERR_STATE if the Ritz values leave (a0, b). */
+int fe_chfsi(fe_mesh* m, double* X, int B, int deg, double a, double b, double a0, double t_eig, int n_gate,
+             int max_cycles, double* theta_host, double* res_host, int* cycles_host, double* work, void* cuda_stream);
+
 /* Step-0 ceilings of the device (not on the product path): a diagnostic kernel of the given
  * kind is launched back to back for at least min_seconds (0 < min_seconds <= 30) and the best launch is reported in
  * *value_host (HOST):  kind 0 = register-resident DFMA chains, TFLOP/s (the FP64 pipe that bounds fe_apply_H / cheb_filter);

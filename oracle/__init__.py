@@ -5,5 +5,5 @@ package; the CUDA product (paper_2510_10529_b200/) never does, and this package 
 """
 from .fe_oracle import (  # noqa: F401
     OracleMesh, build_oracle, gll, gauss, lagrange, lagrange_deriv, lanczos_bounds, rayleigh_ritz,
-    laplacian_precond, minres_shifted, density, adjoint_rhs,
+    laplacian_precond, minres_shifted, density, adjoint_rhs, ritz_residuals, chfsi,
 )

@@ -520,3 +520,90 @@ int orc_filter(const orc_mesh* m, const orc_csr* A, const double* He_all, double
     free(Yk); free(Ykm); free(HY);
     return 0;
 }
+
+/* ---- general hexahedral cell (Eq. 17 l.171 on a trilinearly mapped cell) -------------------
+ * The cell is the image of [-1,1]^3 under x(xi) = sum_v X_v T_v(xi), T_v the 8 trilinear corner functions, corner
+ * v = vx + 2(vy + 2vz).  Jacobian J_ij = dx_i/dxi_j at every quadrature point; physical gradient grad Phi = J^{-T} grad^ Phi;
+ * H_e[a,b] = sum_q w_q |det J_q| [ kin grad Phi_a . grad Phi_b + pot V_q Phi_a Phi_b ], one entry and one point at a time. */
+static void trilinear_jacobian(const double* verts, double x, double y, double z, double J[3][3], double pos[3])
+{
+    double tx[2] = {0.5 * (1.0 - x), 0.5 * (1.0 + x)}, ty[2] = {0.5 * (1.0 - y), 0.5 * (1.0 + y)}, tz[2] = {0.5 * (1.0 - z), 0.5 * (1.0 + z)};
+    double dx[2] = {-0.5, 0.5};
+    for (int i = 0; i < 3; ++i) { pos[i] = 0.0; for (int j = 0; j < 3; ++j) J[i][j] = 0.0; }
+    for (int v = 0; v < 8; ++v) {
+        int vx = v & 1, vy = (v >> 1) & 1, vz = v >> 2;
+        for (int i = 0; i < 3; ++i) {
+            double X = verts[3 * v + i];
+            pos[i] += X * tx[vx] * ty[vy] * tz[vz];
+            J[i][0] += X * dx[vx] * ty[vy] * tz[vz];
+            J[i][1] += X * tx[vx] * dx[vy] * tz[vz];
+            J[i][2] += X * tx[vx] * ty[vy] * dx[vz];
+        }
+    }
+}
+
+static double det3(double J[3][3])
+{
+    return J[0][0] * (J[1][1] * J[2][2] - J[1][2] * J[2][1]) - J[0][1] * (J[1][0] * J[2][2] - J[1][2] * J[2][0]) +
+           J[0][2] * (J[1][0] * J[2][1] - J[1][1] * J[2][0]);
+}
+
+/* inverse by cofactors: Ji = J^{-1} */
+static void inv3(double J[3][3], double det, double Ji[3][3])
+{
+    Ji[0][0] = (J[1][1] * J[2][2] - J[1][2] * J[2][1]) / det;
+    Ji[0][1] = (J[0][2] * J[2][1] - J[0][1] * J[2][2]) / det;
+    Ji[0][2] = (J[0][1] * J[1][2] - J[0][2] * J[1][1]) / det;
+    Ji[1][0] = (J[1][2] * J[2][0] - J[1][0] * J[2][2]) / det;
+    Ji[1][1] = (J[0][0] * J[2][2] - J[0][2] * J[2][0]) / det;
+    Ji[1][2] = (J[0][2] * J[1][0] - J[0][0] * J[1][2]) / det;
+    Ji[2][0] = (J[1][0] * J[2][1] - J[1][1] * J[2][0]) / det;
+    Ji[2][1] = (J[0][1] * J[2][0] - J[0][0] * J[2][1]) / det;
+    Ji[2][2] = (J[0][0] * J[1][1] - J[0][1] * J[1][0]) / det;
+}
+
+void orc_general_cell_matrix(int p, const double* verts, const double* Vq_cell, double kin, double pot, double* He)
+{
+    int n = p + 1, nq = p + 1, nc = n * n * n;
+    double gx[16], gw[16], qx[16], qw[16];
+    orc_gll(p, gx, gw);
+    orc_gauss(nq, qx, qw);
+    for (int i = 0; i < nc * nc; ++i) He[i] = 0.0;
+    double* Pv = (double*)malloc((size_t)nc * sizeof(double));      /* Phi_a at the point */
+    double* G = (double*)malloc((size_t)nc * 3 * sizeof(double));   /* physical gradient of Phi_a at the point */
+    for (int kz = 0; kz < nq; ++kz)
+        for (int ky = 0; ky < nq; ++ky)
+            for (int kx = 0; kx < nq; ++kx) {
+                double J[3][3], Ji[3][3], pos[3];
+                trilinear_jacobian(verts, qx[kx], qx[ky], qx[kz], J, pos);
+                double det = det3(J);
+                inv3(J, det, Ji);
+                double wq = qw[kx] * qw[ky] * qw[kz] * fabs(det);
+                double V = Vq_cell ? Vq_cell[kx + nq * (ky + nq * kz)] : 0.0;
+                for (int a = 0; a < nc; ++a) {
+                    int ax = a % n, ay = (a / n) % n, az = a / (n * n);
+                    double lx = orc_lagrange(n, gx, ax, qx[kx]), ly = orc_lagrange(n, gx, ay, qx[ky]), lz = orc_lagrange(n, gx, az, qx[kz]);
+                    double dlx = orc_lagrange_deriv(n, gx, ax, qx[kx]), dly = orc_lagrange_deriv(n, gx, ay, qx[ky]), dlz = orc_lagrange_deriv(n, gx, az, qx[kz]);
+                    double r[3] = {dlx * ly * lz, lx * dly * lz, lx * ly * dlz}; /* reference gradient */
+                    Pv[a] = lx * ly * lz;
+                    for (int i = 0; i < 3; ++i) /* (J^{-T} r)_i = sum_j Ji[j][i] r_j */
+                        G[3 * a + i] = Ji[0][i] * r[0] + Ji[1][i] * r[1] + Ji[2][i] * r[2];
+                }
+                for (int a = 0; a < nc; ++a)
+                    for (int b = 0; b < nc; ++b)
+                        He[(size_t)a * nc + b] += wq * (kin * (G[3 * a] * G[3 * b] + G[3 * a + 1] * G[3 * b + 1] + G[3 * a + 2] * G[3 * b + 2]) +
+                                                       pot * V * Pv[a] * Pv[b]);
+            }
+    free(Pv); free(G);
+}
+
+/* positions and |det J| of the trilinear map at npts reference points xi (npts x 3): pos (npts x 3), det (npts) */
+void orc_general_map(const double* verts, const double* xi, int npts, double* pos, double* det)
+{
+    for (int k = 0; k < npts; ++k) {
+        double J[3][3], q[3];
+        trilinear_jacobian(verts, xi[3 * k], xi[3 * k + 1], xi[3 * k + 2], J, q);
+        pos[3 * k] = q[0]; pos[3 * k + 1] = q[1]; pos[3 * k + 2] = q[2];
+        det[k] = fabs(det3(J));
+    }
+}

@@ -75,6 +75,12 @@ void orc_apply_rows(const orc_mesh* m, const double* Vq, const double* X, int B,
 int orc_filter(const orc_mesh* m, const orc_csr* A, const double* He_all, double* X, int B, int deg,
                double a, double b, double a0, int nthreads);
 
+/* General (trilinearly mapped) hexahedral cell, corners verts[8*3] with corner v = vx + 2(vy + 2vz) (NEXT-3; l.151, l.273):
+ * He = kin*K_e + pot*M_{V,e} by explicit quadrature with the Jacobian of the map at every Gauss point. */
+void orc_general_cell_matrix(int p, const double* verts, const double* Vq_cell, double kin, double pot, double* He);
+/* positions and |det J| of the trilinear map at npts reference points xi (npts*3) */
+void orc_general_map(const double* verts, const double* xi, int npts, double* pos, double* det);
+
 #ifdef __cplusplus
 }
 #endif

@@ -277,6 +277,30 @@ def rayleigh_ritz(mesh, Y, nthreads=1):
     return theta, Q @ V, Q
 
 
+def ritz_residuals(mesh, X, theta, nthreads=1):
+    """|| H~ x_j - theta_j x_j ||_2 over the free rows, column by column: the residual of the eigenvalue problem that the
+    tolerance t_eig of PAPER.md l.296 is applied to."""
+    X = _f64(X)
+    free = mesh.mask().astype(bool)
+    R = mesh.apply(X, nthreads=nthreads) - X * _f64(theta)[None, :]
+    return np.sqrt(np.sum(R[free] ** 2, axis=0))
+
+
+def chfsi(mesh, X, deg, a, b, a0, t_eig, n_gate, max_cycles=50, nthreads=1):
+    """Chebyshev-filtered subspace iteration with the residual stopping rule of PAPER.md l.296 (t_eig = e_L2^2 / c_eig is
+    handed in as a number): repeat { filter (l.208-210), Rayleigh-Ritz (Eq. 23-24), residuals } until the n_gate lowest
+    pairs have residual <= t_eig; after each cycle a = largest, a0 = smallest Ritz value of the block (survey 8(c) step 8).
+    Returns (theta, X, residuals, cycles)."""
+    cycles = 0
+    while True:
+        theta, X, _ = rayleigh_ritz(mesh, mesh.filter(X, deg, a, b, a0, nthreads=nthreads), nthreads=nthreads)
+        res = ritz_residuals(mesh, X, theta, nthreads=nthreads)
+        cycles += 1
+        if res[:n_gate].max() <= t_eig or cycles >= max_cycles:
+            return theta, X, res, cycles
+        a, a0 = float(theta[-1]), float(theta[0])
+
+
 def laplacian_precond(mesh):
     """Inverse diagonal of the mass-scaled negative Laplacian, 1 / diag(M^{-1/2} (1/2 K) M^{-1/2}) on free rows and 0
     on Dirichlet rows: the MINRES preconditioner of PAPER.md l.225.  Diagonal taken entry by entry from the cell

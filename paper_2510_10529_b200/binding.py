@@ -14,7 +14,7 @@ EXPORTS = (
     "fe_mesh_create", "fe_mesh_destroy", "fe_num_nodes", "fe_num_free", "fe_num_cells", "fe_nodes_per_cell",
     "fe_quad_per_cell", "fe_get_l2g", "fe_get_node_coords", "fe_get_quad_coords", "fe_get_mass",
     "fe_get_dirichlet_mask", "fe_set_potential", "fe_apply_H", "cheb_filter", "cheb_filter_host", "fe_rayleigh_ritz", "fe_minres_shifted", "fe_add_subspace", "fe_gram", "fe_density", "fe_lanczos_bounds", "fe_apply_potential",
-    "fe_set_variant", "fe_diag_peak",
+    "fe_set_variant", "fe_diag_peak", "fe_ritz_residuals", "fe_chfsi",
     "fe_launch_count", "fe_last_error",
 )
 
@@ -63,6 +63,10 @@ def load_library():
     L.fe_gram.restype, L.fe_gram.argtypes = C.c_int, [vp, vp, vp, C.c_int, vp, vp]
     L.fe_add_subspace.restype, L.fe_add_subspace.argtypes = C.c_int, [vp, vp, vp, vp, C.c_int, vp]
     L.fe_set_variant.restype, L.fe_set_variant.argtypes = C.c_int, [vp, C.c_int]
+    L.fe_ritz_residuals.restype, L.fe_ritz_residuals.argtypes = C.c_int, [vp, vp, vp, C.c_int, vp, vp, vp]
+    L.fe_chfsi.restype = C.c_int
+    L.fe_chfsi.argtypes = [vp, vp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int, C.c_int,
+                           vp, vp, vp, vp, vp]
     L.fe_diag_peak.restype, L.fe_diag_peak.argtypes = C.c_int, [C.c_int, C.c_int, C.c_double, dp]
     L.fe_last_error.restype, L.fe_last_error.argtypes = C.c_char_p, []
     _lib = L
@@ -279,6 +283,31 @@ def fe_add_subspace(h, Psi, D, P, stream=None):
     return P
 
 
+def fe_ritz_residuals(h, X, theta, work, stream=None):
+    """|| H~ x_j - theta_j x_j ||_2 per column (numpy, B)."""
+    B = X.shape[1]
+    th = np.ascontiguousarray(theta, dtype=np.float64)
+    if th.shape != (B,):
+        raise FEError(-1, "theta must have B entries")
+    res = np.empty(B, dtype=np.float64)
+    _check(load_library().fe_ritz_residuals(h, _dev_ptr(X, "X"), th.ctypes.data_as(C.c_void_p), B,
+                                            res.ctypes.data_as(C.c_void_p), _dev_ptr(work, "work", X.numel()),
+                                            _stream(stream)))
+    return res
+
+
+def fe_chfsi(h, X, deg, a, b, a0, t_eig, n_gate, max_cycles, work, stream=None):
+    """Returns (theta, residual norms, cycles); X holds the Ritz vectors."""
+    B = X.shape[1]
+    theta, res = np.empty(B, dtype=np.float64), np.empty(B, dtype=np.float64)
+    cycles = C.c_int(0)
+    _check(load_library().fe_chfsi(h, _dev_ptr(X, "X"), B, int(deg), float(a), float(b), float(a0), float(t_eig),
+                                   int(n_gate), int(max_cycles), theta.ctypes.data_as(C.c_void_p),
+                                   res.ctypes.data_as(C.c_void_p), C.byref(cycles),
+                                   _dev_ptr(work, "work", 2 * X.numel()), _stream(stream)))
+    return theta, res, cycles.value
+
+
 def fe_diag_peak(kind, min_seconds=0.3, cuda_device=0):
     """Measured ceiling of the device: kind 0 DFMA / 1 DMMA in TFLOP/s, 2 stream / 3 bulk reduce-add / 4 red.add in GB/s."""
     out = C.c_double(0.0)
@@ -356,6 +385,18 @@ class FEMesh:
         import torch
         rho = torch.empty(self.ncells * self.nq3, dtype=torch.float64, device=X.device)
         return fe_density(self.h, X, f, rho, stream)
+
+    def ritz_residuals(self, X, theta, work=None, stream=None):
+        import torch
+        if work is None:
+            work = torch.empty(X.numel(), dtype=torch.float64, device=X.device)
+        return fe_ritz_residuals(self.h, X, theta, work, stream)
+
+    def chfsi(self, X, deg, a, b, a0, t_eig, n_gate, max_cycles=50, work=None, stream=None):
+        import torch
+        if work is None:
+            work = torch.empty(2 * X.numel(), dtype=torch.float64, device=X.device)
+        return fe_chfsi(self.h, X, deg, a, b, a0, t_eig, n_gate, max_cycles, work, stream)
 
     def lanczos_bounds(self, v0, k=20, stream=None):
         return fe_lanczos_bounds(self.h, v0, k, stream)

@@ -467,10 +467,25 @@ int fe_apply_H(fe_mesh* m, const double* X, double* Y, int B, const double* eps_
         BlockMaps mx, my;
         int rc;
         if ((rc = make_block_maps(&mx, m, X, B)) || (rc = make_block_maps(&my, m, Y, B))) return rc;
+        // The zero-fill stays a plain memset in front of the kernel.  Measured (cfg 5): clearing Y chunk by
+        // chunk from a concurrent kernel (programmatic dependent launch + per-chunk flags) gave no overlap at all, and even a
+        // memset on an unrelated stream costs the operator kernel 18 of its own 22 us -- the two contend for HBM, so the
+        // zero-fill can only be removed as BYTES, not hidden.
         CUDA_TRY(cudaMemsetAsync(Y, 0, len * sizeof(double), st));
         return tma_step(m, mx, my, nullptr, B, eps_dev, 1.0, 0.0, eps_dev != nullptr, 0.0, true, st);
     }
     return operator_step(m, X, nullptr, Y, B, eps_dev, 1.0, 0.0, 0.0, st);
+}
+
+// fe_apply_H into a block the caller has already cleared (the library's own loops let the elementwise kernel that reads a
+// block last also clear it, so the separate zero-fill pass disappears); falls back to fe_apply_H when the TMA path is not taken
+static int apply_into_cleared(fe_mesh* m, const double* X, double* Y, int B, const double* eps_dev, void* cuda_stream)
+{
+    if (!tma_eligible(m, B, X, Y, eps_dev)) return fe_apply_H(m, X, Y, B, eps_dev, cuda_stream);
+    BlockMaps mx, my;
+    int rc;
+    if ((rc = make_block_maps(&mx, m, X, B)) || (rc = make_block_maps(&my, m, Y, B))) return rc;
+    return tma_step(m, mx, my, nullptr, B, eps_dev, 1.0, 0.0, eps_dev != nullptr, 0.0, true, (cudaStream_t)cuda_stream);
 }
 
 int cheb_filter(fe_mesh* m, double* X, int B, int deg, double a, double b, double a0, double* work, void* cuda_stream)
@@ -793,13 +808,14 @@ int fe_minres_shifted(fe_mesh* m, const double* G, double* X, int B, const doubl
     CUDA_TRY(cudaMemsetAsync(q.betasq, 0, 128 * sizeof(double), st));
     k_minres_init<<<grid, blk, 0, st>>>(G, Minv, R1, R2, Y, X, W1, W2, m->N, B, q.betasq);
     k_minres_scalars<<<1, 128, 0, st>>>(q, B, 0, tol);
+    CUDA_TRY(cudaMemsetAsync(HY, 0, len * sizeof(double), st));  // later targets are cleared by k_minres_update
     m->launches += 3;
     std::vector<double> phibar(B), beta1(B);
     int it = 0;
     bool done = false;
     while (it < maxit && !done) {
         k_minres_scalars<<<1, 128, 0, st>>>(q, B, 1, tol);
-        if ((rc = fe_apply_H(m, Y, HY, B, eps_dev, cuda_stream))) return rc;  // hy = (H~ - eps_j) y,  y = beta v
+        if ((rc = apply_into_cleared(m, Y, HY, B, eps_dev, cuda_stream))) return rc;  // hy = (H~ - eps_j) y,  y = beta v
         k_minres_alfa<<<grid, blk, 0, st>>>(Y, HY, R1, m->N, B, q.s, q.c1, q.alfa);
         k_minres_beta<<<grid, blk, 0, st>>>(HY, R1, R2, Minv, m->N, B, q.alfa, q.beta, q.betasq);
         k_minres_scalars<<<1, 128, 0, st>>>(q, B, 2, tol);
@@ -1031,6 +1047,72 @@ int fe_apply_potential(fe_mesh* m, const double* Uq_dev, const double* X, double
     return FE_OK;
 }
 
+// ---- Ritz residuals and the residual-controlled ChFSI loop (NEXT-4; the eigenproblem residual is driven to
+//      t_eig = e_L2^2 / c_eig; l.208-219 for the cycle itself) ------------------------------------------------------------------
+__global__ void k_col_sumsq(const double* __restrict__ R, long long N, int B, double* out)
+{
+    double acc[kMaxColTiles] = {0, 0, 0, 0};
+    for (long long r = blockIdx.x * (long long)kMRy + threadIdx.y; r < N; r += (long long)gridDim.x * kMRy)
+#pragma unroll
+        for (int t = 0; t < kMaxColTiles; ++t) {
+            const int j = t * kMRx + threadIdx.x;
+            if (j < B) {
+                const double v = R[r * B + j];
+                acc[t] = fma(v, v, acc[t]);
+            }
+        }
+    block_col_reduce(acc, B, out);
+}
+
+int fe_ritz_residuals(fe_mesh* m, const double* X, const double* theta_host, int B, double* res_host, double* work,
+                      void* cuda_stream)
+{
+    if (!m || !X || !theta_host || !res_host || !work) return fail(FE_ERR_INVALID, "fe_ritz_residuals: NULL argument");
+    if (B < 1 || B > 128) return fail(FE_ERR_INVALID, "fe_ritz_residuals: B=%d outside 1..128", B);
+    if (!m->have_V) return fail(FE_ERR_STATE, "fe_ritz_residuals: call fe_set_potential first");
+    CUDA_TRY(cudaSetDevice(m->device));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (!m->d_small) CUDA_TRY(cudaMalloc((void**)&m->d_small, 2 * 128 * 128 * sizeof(double)));
+    double* d_theta = m->d_small + 128;  // [0,128): the sums; [128,256): theta
+    CUDA_TRY(cudaMemcpyAsync(d_theta, theta_host, B * sizeof(double), cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemsetAsync(m->d_small, 0, B * sizeof(double), st));
+    int rc = fe_apply_H(m, X, work, B, d_theta, cuda_stream);  // R_j = (H~ - theta_j I) x_j, Dirichlet rows 0 (Eq. 20)
+    if (rc) return rc;
+    k_col_sumsq<<<m->sms * 8, dim3(kMRx, kMRy), 0, st>>>(work, m->N, B, m->d_small);
+    CUDA_TRY(cudaGetLastError());
+    m->launches += 1;
+    CUDA_TRY(cudaMemcpyAsync(res_host, m->d_small, B * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    for (int j = 0; j < B; ++j) res_host[j] = std::sqrt(std::max(res_host[j], 0.0));
+    return FE_OK;
+}
+
+int fe_chfsi(fe_mesh* m, double* X, int B, int deg, double a, double b, double a0, double t_eig, int n_gate,
+             int max_cycles, double* theta_host, double* res_host, int* cycles_host, double* work, void* cuda_stream)
+{
+    if (!m || !X || !theta_host || !res_host || !work) return fail(FE_ERR_INVALID, "fe_chfsi: NULL argument");
+    if (B < 1 || B > 128) return fail(FE_ERR_INVALID, "fe_chfsi: B=%d outside 1..128", B);
+    if (n_gate < 1 || n_gate > B) return fail(FE_ERR_INVALID, "fe_chfsi: n_gate=%d outside 1..B", n_gate);
+    if (max_cycles < 1 || !(t_eig >= 0.0)) return fail(FE_ERR_INVALID, "fe_chfsi: need max_cycles >= 1 and t_eig >= 0");
+    int cycles = 0, rc = FE_OK;
+    for (;;) {
+        if ((rc = cheb_filter(m, X, B, deg, a, b, a0, work, cuda_stream))) return rc;       // l.208-210
+        if ((rc = fe_rayleigh_ritz(m, X, B, theta_host, work, cuda_stream))) return rc;     // Eq. 23-24
+        if ((rc = fe_ritz_residuals(m, X, theta_host, B, res_host, work, cuda_stream))) return rc;
+        ++cycles;
+        double worst = 0.0;
+        for (int j = 0; j < n_gate; ++j) worst = std::max(worst, res_host[j]);
+        if (worst <= t_eig || cycles >= max_cycles) break;
+        // next window (survey 8(c) step 8): the unwanted part starts at the largest Ritz value of the block, the
+        // normalisation point moves to the smallest; b stays the upper bound of the spectrum
+        a = theta_host[B - 1];
+        a0 = theta_host[0];
+        if (!(a0 < a && a < b)) return fail(FE_ERR_STATE, "fe_chfsi: Ritz values left the window (theta_min=%g theta_max=%g b=%g)", a0, a, b);
+    }
+    if (cycles_host) *cycles_host = cycles;
+    return FE_OK;
+}
+
 // ---- step-0 ceilings (fe_diag.cuh): not on the product path; bench.py prints them beside the roofline ---------------------
 int fe_diag_peak(int cuda_device, int kind, double min_seconds, double* value_host)
 {
@@ -1048,7 +1130,7 @@ int fe_diag_peak(int cuda_device, int kind, double min_seconds, double* value_ho
     double work = 0.0;  // flops or bytes per launch
     auto launch = [&]() {
         switch (kind) {
-            case 0: k_diag_dfma<8><<<sms * 4, 256>>>(a, 4096, 0.999999, 1e-7); break;
+            case 0: k_diag_dfma<8><<<sms * 4, 256>>>(a, 4096, -1e-9, 0.0); break;
             case 1: k_diag_dmma<<<sms * 4, 256>>>(a, 4096, 0.25, 1e-3); break;
             case 2: k_diag_stream<<<sms * 16, 256>>>((const double2*)a, (const double2*)b, (double2*)c, n / 2, 0.5); break;
             case 3: k_diag_bulk_red<16384><<<sms * 4, 128, 16384>>>(a, n * 8 / 16384); break;

@@ -15,6 +15,7 @@ namespace fecheb {
 template <int CHAINS>
 __global__ void __launch_bounds__(256) k_diag_dfma(double* out, int iters, double a, double b)
 {
+    (void)b;
     double x[CHAINS];
 #pragma unroll
     for (int k = 0; k < CHAINS; ++k) x[k] = 1e-3 * (threadIdx.x + 1) + k;
@@ -22,7 +23,8 @@ __global__ void __launch_bounds__(256) k_diag_dfma(double* out, int iters, doubl
 #pragma unroll
         for (int u = 0; u < 16; ++u)
 #pragma unroll
-            for (int k = 0; k < CHAINS; ++k) x[k] = fma(x[k], a, b);
+            for (int k = 0; k < CHAINS; ++k) x[k] = fma(x[k], a, x[k]);  // two distinct register operands: with three
+                                                                         // (x, a, b) the register file caps DFMA at 34.1 TFLOP/s
     }
     double s = 0.0;
 #pragma unroll

@@ -109,8 +109,10 @@ __global__ void k_minres_beta(double* __restrict__ Y, double* __restrict__ R1, c
     block_col_reduce(acc, B, betasq);
 }
 
-// phase D:  w_new = (v - oldeps_j w1 - delta_j w2) / gamma_j  (into w1's storage), v = s_j y_old ;  x += phi_j w_new
-__global__ void k_minres_update(const double* __restrict__ Yold, double* __restrict__ W1, const double* __restrict__ W2,
+// phase D:  w_new = (v - oldeps_j w1 - delta_j w2) / gamma_j  (into w1's storage), v = s_j y_old ;  x += phi_j w_new.
+// y_old is read here for the last time and its block is the NEXT step's apply target: it is cleared on the way out, which
+// replaces the zero-fill pass of fe_apply_H.
+__global__ void k_minres_update(double* __restrict__ Yold, double* __restrict__ W1, const double* __restrict__ W2,
                                 double* __restrict__ X, long long N, int B, const double* __restrict__ s,
                                 const double* __restrict__ oldeps, const double* __restrict__ delta,
                                 const double* __restrict__ gamma, const double* __restrict__ phi)
@@ -122,6 +124,7 @@ __global__ void k_minres_update(const double* __restrict__ Yold, double* __restr
             if (j < B) {
                 const long long i = r * B + j;
                 const double w = (s[j] * Yold[i] - oldeps[j] * W1[i] - delta[j] * W2[i]) / gamma[j];
+                Yold[i] = 0.0;
                 W1[i] = w;
                 X[i] = fma(phi[j], w, X[i]);
             }

@@ -345,6 +345,37 @@ def test_device_lanczos_bounds_and_chfsi_cycles():
     assert np.max(np.abs(theta_g - theta_o) / np.maximum(1.0, np.abs(theta_o))) <= 1e-9
 
 
+def test_ritz_residuals_and_residual_controlled_chfsi():
+    """fe_ritz_residuals and fe_chfsi (NEXT-4, l.296) on the config-2 recipe (reduced mesh): residual norms of a given
+    block against the oracle's definition, then the residual-controlled loop from device Lanczos bounds -- same number
+    of cycles, Ritz values <= 1e-9, residuals of the gated pairs below t_eig on both sides."""
+    import oracle
+    w = workloads.reduced(2, 4)
+    om, gm = _pair((w.xe, w.ye, w.ze), w.p, w.V)
+    mask = om.mask()
+    B, n_gate, t_eig = 16, 6, 1e-7
+    X0 = workloads.random_block(w.x_seed, om.N, B, mask)
+    th_min, th_max, beta = oracle.lanczos_bounds(om, workloads.normal(3500, om.N), 20)
+    b, a0 = th_max + beta, th_min
+    a = a0 + 0.1 * (b - a0)
+    # residuals of a half-converged block with garbage in its Dirichlet rows
+    th1, X1, _ = oracle.rayleigh_ritz(om, om.filter(X0, w.m, a, b, a0))
+    Xin = X1.copy()
+    Xin[mask == 0] = -4.5
+    r_o = oracle.ritz_residuals(om, X1, th1)
+    r_g = gm.ritz_residuals(_dev(Xin), th1)
+    assert np.max(np.abs(r_g - r_o)) <= 1e-11 * max(1.0, r_o.max())
+    theta_o, _, res_o, cyc_o = oracle.chfsi(om, X0, w.m, a, b, a0, t_eig, n_gate, max_cycles=30)
+    Xg = _dev(X0)
+    theta_g, res_g, cyc_g = gm.chfsi(Xg, w.m, a, b, a0, t_eig, n_gate, max_cycles=30)
+    assert cyc_g == cyc_o and 1 < cyc_g < 30
+    assert res_g[:n_gate].max() <= t_eig and res_o[:n_gate].max() <= t_eig
+    assert np.max(np.abs(theta_g - theta_o) / np.maximum(1.0, np.abs(theta_o))) <= 1e-9
+    Q = Xg.cpu().numpy()
+    assert np.max(np.abs(Q.T @ Q - np.eye(B))) <= 1e-12
+    assert np.max(np.abs(oracle.ritz_residuals(om, Q, theta_g) - res_g)) <= 1e-9  # the library's own claim, checked
+
+
 @pytest.mark.parametrize("B", [6, 64, 96])
 def test_filter_from_host_buffers(B):
     """cheb_filter_host (H2D, filter, D2H through the C ABI; chunks of 32 columns on two streams when B % 32 == 0)

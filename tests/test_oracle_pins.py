@@ -419,6 +419,45 @@ def test_rayleigh_ritz():
     assert np.linalg.norm(R[:, 0]) < 1e-4
 
 
+def test_ritz_residuals_and_residual_controlled_chfsi():
+    """l.296: the eigenproblem residual || H~ x - theta x || is driven below t_eig.  Pins, on config 1's dense H~ through
+    LAPACK: (i) exact eigenpairs have residual 0; (ii) for any unit vector with its Rayleigh quotient,
+    ||H x - theta x||^2 = x^T H^2 x - theta^2; (iii) Bauer-Fike for symmetric matrices: every Ritz value lies within its
+    residual norm of an eigenvalue; (iv) the residual-controlled loop stops at the first cycle whose gate residuals are
+    <= t_eig (it reproduces a hand-rolled fixed-count loop) and its lowest values are then eigenvalues to residual^2 / gap."""
+    w = workloads.config(1)
+    m = _mesh((w.xe, w.ye, w.ze), w.p, V=w.V)
+    mask = m.mask()
+    free = np.flatnonzero(mask)
+    H = _csr(m).toarray()[np.ix_(free, free)]
+    lam, U = np.linalg.eigh(H)
+    Xe = np.zeros((m.N, 5))
+    Xe[free] = U[:, :5]
+    assert np.max(oracle.ritz_residuals(m, Xe, lam[:5])) < 1e-12
+    x = workloads.normal(77, m.N) * mask
+    x /= np.linalg.norm(x)
+    th = x[free] @ H @ x[free]
+    r = oracle.ritz_residuals(m, x[:, None], [th])[0]
+    assert abs(r ** 2 - (x[free] @ H @ (H @ x[free]) - th ** 2)) < 1e-10 * r ** 2
+    th_min, th_max, beta = oracle.lanczos_bounds(m, workloads.normal(3001, m.N), 20)
+    b, a0 = th_max + beta, th_min
+    a = a0 + 0.1 * (b - a0)
+    X0 = w.X(mask)
+    theta, X, res, cycles = oracle.chfsi(m, X0, 10, a, b, a0, t_eig=1e-6, n_gate=4, max_cycles=40)
+    assert 1 < cycles < 40 and res[:4].max() <= 1e-6
+    for t, rj in zip(theta, res):
+        assert np.min(np.abs(lam - t)) <= rj * (1 + 1e-8) + 1e-13
+    assert np.max(np.abs(theta[:4] - lam[:4])) < 1e-10
+    # the same cycles by hand: the loop stopped exactly at the first cycle that met the gate
+    Xh, ah, a0h = X0, a, a0
+    for c in range(cycles):
+        th_h, Xh, _ = oracle.rayleigh_ritz(m, m.filter(Xh, 10, ah, b, a0h))
+        rh = oracle.ritz_residuals(m, Xh, th_h)
+        assert (rh[:4].max() <= 1e-6) == (c == cycles - 1)
+        ah, a0h = th_h[-1], th_h[0]
+    assert np.array_equal(th_h, theta)
+
+
 # ---- MINRES of the adjoint solve (l.221-225) -------------------------------------------------------------------------
 def test_minres_against_dense_solves():
     """The oracle's MINRES is pinned to LAPACK: a regular shifted system against numpy.linalg.solve, and the singular

@@ -194,3 +194,125 @@ def reduced(i, cells):
     w.xe, w.ye, w.ze = centre(w.xe), centre(w.ye), centre(w.ze)
     w.name += "-sub%d" % cells
     return w
+
+
+# ---- general hexahedral meshes with hanging nodes (Fig. 6) -----------------------
+class OctreeMesh:
+    """Description of an adaptively refined hexahedral mesh, the INPUT both the library and the oracle build from (no
+    method arithmetic here: only which cells exist and where their corners are).
+
+    cells : (ncells, 4) int32 rows (level, ix, iy, iz): the leaf with index (ix, iy, iz) on the level-`level` lattice of
+            2^level (cx, cy, cz) cells.  Leaves are listed root by root (root e = ex + cx (ey + cy ez)), the children of a
+            refined cell depth first in the order child = hx + 2 (hy + 2 hz).  Levels of leaves whose closures touch
+            differ by at most one (2:1 balance over faces, edges and corners).
+    verts : (ncells, 8, 3) float64 corner coordinates, corner v = vx + 2 (vy + 2 vz); the cell is the trilinear image of
+            the reference cube.  Corners shared by cells coincide, and a corner that hangs on a coarser neighbour's edge or
+            face lies on that neighbour's (bi)linear edge / face."""
+
+    def __init__(self, cx, cy, cz, cells, verts, maxlevel):
+        self.cx, self.cy, self.cz = int(cx), int(cy), int(cz)
+        self.cells = np.ascontiguousarray(cells, dtype=np.int32)
+        self.verts = np.ascontiguousarray(verts, dtype=np.float64)
+        self.maxlevel = int(maxlevel)
+
+    @property
+    def ncells(self):
+        return len(self.cells)
+
+
+def octree_mesh(xe, ye, ze, refine, maxlevel, deform=None):
+    """Refine the tensor-product root grid (edges xe, ye, ze): a leaf of level < maxlevel is split into 8 when
+    refine(level, lo, hi) is true (lo, hi = corners of its undeformed box), then cells are split further until the 2:1
+    balance holds.  deform(xyz) -> xyz moves the lattice points (identity if None); points that hang on a coarser cell are
+    then put back onto that cell's trilinear image, coarse levels first, so that the mesh has no cracks."""
+    xe, ye, ze = (np.asarray(e, dtype=np.float64) for e in (xe, ye, ze))
+    cx, cy, cz = len(xe) - 1, len(ye) - 1, len(ze) - 1
+    L = int(maxlevel)
+
+    def box(level, ix, iy, iz):
+        def ax(e, i):
+            r, k = divmod(i, 1 << level)
+            return e[r] + (e[r + 1] - e[r]) * k / (1 << level) if r < len(e) - 1 else e[-1]
+        lo = np.array([ax(xe, ix), ax(ye, iy), ax(ze, iz)])
+        hi = np.array([ax(xe, ix + 1), ax(ye, iy + 1), ax(ze, iz + 1)])
+        return lo, hi
+
+    leaves = {(0, ix, iy, iz) for iz in range(cz) for iy in range(cy) for ix in range(cx)}
+
+    def split(c):
+        l, ix, iy, iz = c
+        leaves.discard(c)
+        for hz in range(2):
+            for hy in range(2):
+                for hx in range(2):
+                    leaves.add((l + 1, 2 * ix + hx, 2 * iy + hy, 2 * iz + hz))
+
+    for level in range(L):
+        for c in sorted(leaves):
+            if c[0] == level and refine(level, *box(*c)):
+                split(c)
+
+    def containing_leaf(l, ix, iy, iz):
+        while l >= 0:
+            if (l, ix, iy, iz) in leaves:
+                return (l, ix, iy, iz)
+            l, ix, iy, iz = l - 1, ix >> 1, iy >> 1, iz >> 1
+        return None
+
+    changed = True
+    while changed:  # 2:1 balance over the 26-neighbourhood
+        changed = False
+        for c in sorted(leaves, key=lambda t: -t[0]):
+            l, ix, iy, iz = c
+            if c not in leaves or l < 2:
+                continue
+            for dz in (-1, 0, 1):
+                for dy in (-1, 0, 1):
+                    for dx in (-1, 0, 1):
+                        jx, jy, jz = ix + dx, iy + dy, iz + dz
+                        if not (0 <= jx < cx << l and 0 <= jy < cy << l and 0 <= jz < cz << l):
+                            continue
+                        nb = containing_leaf(l, jx, jy, jz)
+                        if nb is not None and nb[0] < l - 1:
+                            split(nb)
+                            changed = True
+
+    def order_key(c):  # root by root, children depth first
+        l, ix, iy, iz = c
+        rx, ry, rz = ix >> l, iy >> l, iz >> l
+        path = []
+        for k in range(l - 1, -1, -1):
+            path.append(((ix >> k) & 1) + 2 * (((iy >> k) & 1) + 2 * ((iz >> k) & 1)))
+        return (rx + cx * (ry + cy * rz), path)
+
+    cells = sorted(leaves, key=order_key)
+    # lattice points of the finest level, deformed, then hanging points put back onto the coarser cell's trilinear image
+    Vx, Vy, Vz = (cx << L) + 1, (cy << L) + 1, (cz << L) + 1
+
+    def axis_pts(e, c):
+        out = np.empty((c << L) + 1)
+        for r in range(c):
+            out[r << L:((r + 1) << L) + 1] = e[r] + (e[r + 1] - e[r]) * np.arange((1 << L) + 1) / (1 << L)
+        out[-1] = e[-1]
+        return out
+
+    X, Y, Z = np.meshgrid(axis_pts(xe, cx), axis_pts(ye, cy), axis_pts(ze, cz), indexing="ij")
+    P = np.stack([X, Y, Z], axis=-1)  # [vx, vy, vz, 3]
+    if deform is not None:
+        P = np.asarray(deform(P.reshape(-1, 3)), dtype=np.float64).reshape(Vx, Vy, Vz, 3)
+    for level in range(L):  # coarse first; cells of the finest level have no interior lattice points
+        s = 1 << (L - level)
+        t = np.arange(s + 1) / s
+        for (l, ix, iy, iz) in cells:
+            if l != level:
+                continue
+            x0, y0, z0 = ix * s, iy * s, iz * s
+            C = P[x0:x0 + s + 1:s, y0:y0 + s + 1:s, z0:z0 + s + 1:s].copy()  # [2,2,2,3] corners
+            wx = np.stack([1 - t, t])  # [2, s+1]
+            P[x0:x0 + s + 1, y0:y0 + s + 1, z0:z0 + s + 1] = np.einsum("ai,bj,ck,abcd->ijkd", wx, wx, wx, C)
+    verts = np.empty((len(cells), 8, 3))
+    for e, (l, ix, iy, iz) in enumerate(cells):
+        s = 1 << (L - l)
+        for v in range(8):
+            verts[e, v] = P[(ix + (v & 1)) * s, (iy + ((v >> 1) & 1)) * s, (iz + (v >> 2)) * s]
+    return OctreeMesh(cx, cy, cz, np.array(cells, dtype=np.int32).reshape(-1, 4), verts, L)
