@@ -7,3 +7,4 @@ from .fe_oracle import (  # noqa: F401
     OracleMesh, build_oracle, gll, gauss, lagrange, lagrange_deriv, lanczos_bounds, rayleigh_ritz,
     laplacian_precond, minres_shifted, density, adjoint_rhs, ritz_residuals, chfsi,
 )
+from .fe_general import GeneralOracleMesh  # noqa: F401,E402
