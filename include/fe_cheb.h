@@ -56,6 +56,28 @@ int fe_get_quad_coords(const fe_mesh* m, double* xyz);     /* cells*n_q^3*3: whe
 int fe_get_mass(const fe_mesh* m, double* Mdiag);          /* N, diagonal of the GLL-lumped M (l.185) */
 int fe_get_dirichlet_mask(const fe_mesh* m, uint8_t* mask); /* N, 1 = free, 0 = boundary */
 
+/* General hexahedral mesh with hanging nodes (the adaptively refined meshes of l.151, l.273, Fig. 6): the leaves of an
+ * octree refinement of a cx x cy x cz root grid.  cells: HOST, ncells rows (level, ix, iy, iz) -- leaf (ix, iy, iz) of the
+ * level-`level` lattice of 2^level (cx, cy, cz) cells; levels of leaves whose closures touch may differ by at most one.
+ * verts: HOST, ncells*8*3 corner coordinates, corner v = vx + 2*(vy + 2*vz); a cell is the trilinear image of [-1,1]^3, so
+ * the metric is a full symmetric 3x3 matrix per quadrature point.  Corners shared by cells must coincide and a corner hanging
+ * on a coarser neighbour must lie on that neighbour's edge / face (not checked).  Numbering (reading R23): cells in the
+ * given order, local nodes a = ax + n*(ay + n*az); unconstrained nodes get ids 0..N-1 in order of first appearance, hanging
+ * nodes (nodes of a cell lying on a coarser leaf) ids N..N_all-1 likewise.  Blocks X, Y have N = fe_num_nodes rows: hanging
+ * nodes are no degrees of freedom, their values are u_h = sum_k c_hk u_k (fe_get_constraints).  Lumped mass of the
+ * constrained problem: diag(C^T m) with m the GLL-quadrature nodal masses (R25).  Dirichlet on the surface of the root box.
+ * On such a handle fe_set_potential, fe_apply_H, cheb_filter, cheb_filter_host, fe_rayleigh_ritz, fe_ritz_residuals,
+ * fe_chfsi, fe_lanczos_bounds, fe_gram and fe_add_subspace work as on a box mesh; fe_minres_shifted, fe_density and
+ * fe_apply_potential return FE_ERR_INVALID.  FE_ERR_INVALID for an inconsistent leaf list.  cuda_device = -1 builds the
+ * tables only (sizes, l2g, constraints, coordinates, mass, mask can be queried; no potential can be set).  Synchronous. */
+int fe_mesh_create_general(int cx, int cy, int cz, const int32_t* cells, int64_t ncells, const double* verts, int p,
+                           int cuda_device, fe_mesh** out);
+int64_t fe_num_all_nodes(const fe_mesh* m);          /* N_all: rows of fe_get_node_coords, range of fe_get_l2g */
+int64_t fe_num_constraint_entries(const fe_mesh* m); /* non-zeros of the hanging rows */
+/* Hanging-node constraints as CSR over the rows h = N..N_all-1: row_ptr (HOST, N_all-N+1 int64), col (unconstrained node
+ * ids), val (weights).  A box mesh has none (row_ptr[0] = 0). */
+int fe_get_constraints(const fe_mesh* m, int64_t* row_ptr, int32_t* col, double* val);
+
 /* V = v_H + v_N + v_xc (l.68) at the quadrature points: Vq_dev is a DEVICE array of cells*n_q^3 doubles, cell-major,
  * q = qx + n_q*(qy + n_q*qz) inside a cell.  The library stores J*w_q*V_q in its own buffer (one kernel on
  * cuda_stream); `copy` is accepted for ABI stability and ignored: Vq_dev is never retained.  Asynchronous. */

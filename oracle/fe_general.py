@@ -202,7 +202,7 @@ class GeneralOracleMesh:
         S = sp.diags(s)
         self.Ht = (S @ self.Hc @ S).tocsr()
 
-    def apply(self, X, eps=None):
+    def apply(self, X, eps=None, nthreads=1):
         X = np.ascontiguousarray(X, dtype=np.float64)
         free = self._mask.astype(bool)
         Xm = X * free[:, None]
@@ -212,7 +212,7 @@ class GeneralOracleMesh:
         Y[~free] = 0.0
         return Y
 
-    def filter(self, X, m, a, b, a0):
+    def filter(self, X, m, a, b, a0, nthreads=1):
         """Scaled three-term recurrence of reading R7 (l.208-210), serial."""
         if not (a0 < a < b) or m < 1:
             raise ValueError("need a0 < a < b and m >= 1")

@@ -14,7 +14,8 @@ EXPORTS = (
     "fe_mesh_create", "fe_mesh_destroy", "fe_num_nodes", "fe_num_free", "fe_num_cells", "fe_nodes_per_cell",
     "fe_quad_per_cell", "fe_get_l2g", "fe_get_node_coords", "fe_get_quad_coords", "fe_get_mass",
     "fe_get_dirichlet_mask", "fe_set_potential", "fe_apply_H", "cheb_filter", "cheb_filter_host", "fe_rayleigh_ritz", "fe_minres_shifted", "fe_add_subspace", "fe_gram", "fe_density", "fe_lanczos_bounds", "fe_apply_potential",
-    "fe_set_variant", "fe_diag_peak", "fe_ritz_residuals", "fe_chfsi",
+    "fe_set_variant", "fe_diag_peak", "fe_ritz_residuals", "fe_chfsi", "fe_mesh_create_general",
+    "fe_num_all_nodes", "fe_num_constraint_entries", "fe_get_constraints",
     "fe_launch_count", "fe_last_error",
 )
 
@@ -42,7 +43,11 @@ def load_library():
     L.fe_mesh_create.restype = C.c_int
     L.fe_mesh_create.argtypes = [dp, C.c_int, dp, C.c_int, dp, C.c_int, C.c_int, C.c_int, C.POINTER(vp)]
     L.fe_mesh_destroy.restype, L.fe_mesh_destroy.argtypes = C.c_int, [vp]
-    for name in ("fe_num_nodes", "fe_num_free", "fe_num_cells", "fe_launch_count"):
+    L.fe_mesh_create_general.restype = C.c_int
+    L.fe_mesh_create_general.argtypes = [C.c_int, C.c_int, C.c_int, vp, C.c_int64, vp, C.c_int, C.c_int, C.POINTER(vp)]
+    L.fe_get_constraints.restype, L.fe_get_constraints.argtypes = C.c_int, [vp, vp, vp, vp]
+    for name in ("fe_num_nodes", "fe_num_free", "fe_num_cells", "fe_launch_count", "fe_num_all_nodes",
+                 "fe_num_constraint_entries"):
         getattr(L, name).restype, getattr(L, name).argtypes = C.c_int64, [vp]
     for name in ("fe_nodes_per_cell", "fe_quad_per_cell"):
         getattr(L, name).restype, getattr(L, name).argtypes = C.c_int, [vp]
@@ -113,6 +118,37 @@ def fe_mesh_create(xe, ye, ze, p, cuda_device=0):
     return h
 
 
+def fe_mesh_create_general(cx, cy, cz, cells, verts, p, cuda_device=0):
+    """cells: (ncells, 4) int32 rows (level, ix, iy, iz); verts: (ncells, 8, 3) float64 corners.  cuda_device=-1: tables only."""
+    L = load_library()
+    cells = np.ascontiguousarray(cells, dtype=np.int32)
+    verts = np.ascontiguousarray(verts, dtype=np.float64)
+    if cells.ndim != 2 or cells.shape[1] != 4 or verts.shape != (len(cells), 8, 3):
+        raise FEError(-1, "cells must be (ncells, 4) and verts (ncells, 8, 3)")
+    h = C.c_void_p()
+    _check(L.fe_mesh_create_general(int(cx), int(cy), int(cz), C.c_void_p(cells.ctypes.data), len(cells),
+                                    C.c_void_p(verts.ctypes.data), int(p), int(cuda_device), C.byref(h)))
+    return h
+
+
+def fe_num_all_nodes(h):
+    return load_library().fe_num_all_nodes(h)
+
+
+def fe_num_constraint_entries(h):
+    return load_library().fe_num_constraint_entries(h)
+
+
+def fe_get_constraints(h):
+    """(row_ptr, col, val) of the hanging-node rows h = N..N_all-1."""
+    nh = fe_num_all_nodes(h) - fe_num_nodes(h)
+    nnz = fe_num_constraint_entries(h)
+    rp, col, val = np.zeros(nh + 1, dtype=np.int64), np.zeros(nnz, dtype=np.int32), np.zeros(nnz, dtype=np.float64)
+    _check(load_library().fe_get_constraints(h, C.c_void_p(rp.ctypes.data), C.c_void_p(col.ctypes.data),
+                                             C.c_void_p(val.ctypes.data)))
+    return rp, col, val
+
+
 def fe_mesh_destroy(h):
     _check(load_library().fe_mesh_destroy(h))
 
@@ -152,7 +188,7 @@ def fe_get_l2g(h):
 
 
 def fe_get_node_coords(h):
-    return _fill(h, "fe_get_node_coords", (fe_num_nodes(h), 3), np.float64)
+    return _fill(h, "fe_get_node_coords", (fe_num_all_nodes(h), 3), np.float64)
 
 
 def fe_get_quad_coords(h):
@@ -323,12 +359,26 @@ def fe_set_variant(h, variant):
 class FEMesh:
     """Owns an fe_mesh handle.  All array arguments are torch CUDA float64 tensors; results stay on the device."""
 
-    def __init__(self, xe, ye, ze, p, device=0):
+    def __init__(self, xe, ye, ze, p, device=0, _handle=None):
         self.device = int(device)
-        self.h = fe_mesh_create(xe, ye, ze, p, self.device)
+        self.h = _handle if _handle is not None else fe_mesh_create(xe, ye, ze, p, self.device)
         self.p = int(p)
         self.N, self.N_free, self.ncells = fe_num_nodes(self.h), fe_num_free(self.h), fe_num_cells(self.h)
         self.nc, self.nq3 = fe_nodes_per_cell(self.h), fe_quad_per_cell(self.h)
+
+    @classmethod
+    def general(cls, mesh, p, device=0):
+        """General hexahedral mesh with hanging nodes from a leaf description with attributes cx, cy, cz, cells, verts
+        (fe_mesh_create_general); device=-1 builds the tables only."""
+        h = fe_mesh_create_general(mesh.cx, mesh.cy, mesh.cz, mesh.cells, mesh.verts, p, device)
+        return cls(None, None, None, p, device, _handle=h)
+
+    @property
+    def N_all(self):
+        return fe_num_all_nodes(self.h)
+
+    def constraints(self):
+        return fe_get_constraints(self.h)
 
     def close(self):
         if getattr(self, "h", None):

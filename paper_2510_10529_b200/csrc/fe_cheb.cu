@@ -20,6 +20,8 @@
 #include "fe_apply_tma.cuh"
 #include "fe_density.cuh"
 #include "fe_diag.cuh"
+#include "fe_general.cuh"
+#include "fe_general.h"
 #include "fe_minres.cuh"
 #include "fe_rr.cuh"
 #include "fe_kernels.cuh"
@@ -68,6 +70,16 @@ struct fe_mesh {
     size_t host_cap = 0;
     cudaStream_t hstream[2] = {nullptr, nullptr};
     double* d_small = nullptr;  // 2 * 128 * 128: B x B scratch of the Rayleigh-Ritz step
+    // general hexahedral mesh with hanging nodes (fe_mesh_create_general; fe_general.h / fe_general.cuh): N = unconstrained nodes
+    int kind = 0;  // 0: tensor-product box mesh, 1: general
+    GeneralHost* gh = nullptr;
+    int32_t* d_gl2g = nullptr;
+    double *d_gmetric = nullptr, *d_gwdet = nullptr, *d_gWV = nullptr;
+    long long* d_crow = nullptr;
+    int32_t* d_ccol = nullptr;
+    double* d_cval = nullptr;
+    double *d_Xh = nullptr, *d_Yh = nullptr;  // (N_all - N) * hcap: expanded hanging values / their scatter target
+    int hcap = 0;
     int sms = 0;  // multiprocessors of the device (persistent grid size)
     int64_t launches = 0;
 };
@@ -195,18 +207,30 @@ int fe_mesh_create(const double* xe, int cx, const double* ye, int cy, const dou
 int fe_mesh_destroy(fe_mesh* m)
 {
     if (!m) return FE_OK;
-    cudaSetDevice(m->device);
+    if (m->device >= 0) cudaSetDevice(m->device);
     cudaFree(m->d_sm); cudaFree(m->d_hx); cudaFree(m->d_hy); cudaFree(m->d_hz); cudaFree(m->d_WV);
     cudaFree(m->d_host); cudaFree(m->d_WU); cudaFree(m->d_VZU);
     for (cudaStream_t s : m->hstream) if (s) cudaStreamDestroy(s);
     cudaFree(m->d_small); cudaFree(m->d_minv); cudaFree(m->d_mask); cudaFree(m->d_scal);
     cudaFree(m->d_VZ); cudaFree(m->d_sx); cudaFree(m->d_sy); cudaFree(m->d_sz);
+    cudaFree(m->d_gl2g); cudaFree(m->d_gmetric); cudaFree(m->d_gwdet); cudaFree(m->d_gWV); cudaFree(m->d_crow);
+    cudaFree(m->d_ccol); cudaFree(m->d_cval); cudaFree(m->d_Xh); cudaFree(m->d_Yh);
+    delete m->gh;
     delete m;
     return FE_OK;
 }
 
 int64_t fe_num_nodes(const fe_mesh* m) { return m ? m->N : FE_ERR_INVALID; }
-int64_t fe_num_free(const fe_mesh* m) { return m ? (m->Nx - 2) * (m->Ny - 2) * (m->Nz - 2) : FE_ERR_INVALID; }
+int64_t fe_num_free(const fe_mesh* m)
+{
+    if (!m) return FE_ERR_INVALID;
+    if (m->kind == 0) return (m->Nx - 2) * (m->Ny - 2) * (m->Nz - 2);
+    int64_t k = 0;
+    for (uint8_t f : m->gh->mask) k += f;
+    return k;
+}
+int64_t fe_num_all_nodes(const fe_mesh* m) { return m ? (m->kind ? m->gh->N_all : m->N) : FE_ERR_INVALID; }
+int64_t fe_num_constraint_entries(const fe_mesh* m) { return m ? (m->kind ? (int64_t)m->gh->ccol.size() : 0) : FE_ERR_INVALID; }
 int64_t fe_num_cells(const fe_mesh* m) { return m ? m->ncells : FE_ERR_INVALID; }
 int fe_nodes_per_cell(const fe_mesh* m) { return m ? m->nc : FE_ERR_INVALID; }
 int fe_quad_per_cell(const fe_mesh* m) { return m ? m->nc : FE_ERR_INVALID; }
@@ -215,6 +239,7 @@ int64_t fe_launch_count(const fe_mesh* m) { return m ? m->launches : FE_ERR_INVA
 int fe_get_l2g(const fe_mesh* m, int32_t* l2g)
 {
     if (!m || !l2g) return fail(FE_ERR_INVALID, "fe_get_l2g: NULL argument");
+    if (m->kind) { memcpy(l2g, m->gh->l2g.data(), m->gh->l2g.size() * sizeof(int32_t)); return FE_OK; }
     const int n = m->n, p = m->p;
     for (int64_t ez = 0; ez < m->cz; ++ez)
         for (int64_t ey = 0; ey < m->cy; ++ey)
@@ -244,6 +269,7 @@ static void axis_coords(const std::vector<double>& e, int c, int p, const double
 int fe_get_node_coords(const fe_mesh* m, double* xyz)
 {
     if (!m || !xyz) return fail(FE_ERR_INVALID, "fe_get_node_coords: NULL argument");
+    if (m->kind) { memcpy(xyz, m->gh->node_xyz.data(), m->gh->node_xyz.size() * sizeof(double)); return FE_OK; }
     std::vector<double> X, Y, Z;
     axis_coords(m->xe, m->cx, m->p, m->tab.gll_x, true, X);
     axis_coords(m->ye, m->cy, m->p, m->tab.gll_x, true, Y);
@@ -260,6 +286,7 @@ int fe_get_node_coords(const fe_mesh* m, double* xyz)
 int fe_get_quad_coords(const fe_mesh* m, double* xyz)
 {
     if (!m || !xyz) return fail(FE_ERR_INVALID, "fe_get_quad_coords: NULL argument");
+    if (m->kind) { memcpy(xyz, m->gh->quad_xyz.data(), m->gh->quad_xyz.size() * sizeof(double)); return FE_OK; }
     const int n = m->n;
     std::vector<double> X, Y, Z;
     axis_coords(m->xe, m->cx, m->p, m->tab.gl_x, false, X);
@@ -282,6 +309,7 @@ int fe_get_quad_coords(const fe_mesh* m, double* xyz)
 int fe_get_mass(const fe_mesh* m, double* Mdiag)
 {
     if (!m || !Mdiag) return fail(FE_ERR_INVALID, "fe_get_mass: NULL argument");
+    if (m->kind) { memcpy(Mdiag, m->gh->mass.data(), m->gh->mass.size() * sizeof(double)); return FE_OK; }
     for (int64_t gz = 0; gz < m->Nz; ++gz)
         for (int64_t gy = 0; gy < m->Ny; ++gy)
             for (int64_t gx = 0; gx < m->Nx; ++gx) Mdiag[gx + m->Nx * (gy + m->Ny * gz)] = m->mx[gx] * m->my[gy] * m->mz[gz];
@@ -291,6 +319,7 @@ int fe_get_mass(const fe_mesh* m, double* Mdiag)
 int fe_get_dirichlet_mask(const fe_mesh* m, uint8_t* mask)
 {
     if (!m || !mask) return fail(FE_ERR_INVALID, "fe_get_dirichlet_mask: NULL argument");
+    if (m->kind) { memcpy(mask, m->gh->mask.data(), m->gh->mask.size()); return FE_OK; }
     for (int64_t gz = 0; gz < m->Nz; ++gz)
         for (int64_t gy = 0; gy < m->Ny; ++gy)
             for (int64_t gx = 0; gx < m->Nx; ++gx)
@@ -316,7 +345,15 @@ int fe_set_potential(fe_mesh* m, const double* Vq_dev, int copy, void* cuda_stre
 {
     (void)copy;
     if (!m || !Vq_dev) return fail(FE_ERR_INVALID, "fe_set_potential: NULL argument");
+    if (m->device < 0) return fail(FE_ERR_STATE, "fe_set_potential: the handle was created without a device (tables only)");
     CUDA_TRY(cudaSetDevice(m->device));
+    if (m->kind) {
+        k_gen_weight_potential<<<m->sms * 8, 256, 0, (cudaStream_t)cuda_stream>>>(m->d_gWV, Vq_dev, m->d_gwdet, m->ncells * m->nc);
+        CUDA_TRY(cudaGetLastError());
+        m->launches += 1;
+        m->have_V = true;
+        return FE_OK;
+    }
     ApplyParams prm;
     fill_params(m, &prm);
     launch_weight_potential(prm, m->p, Vq_dev, m->d_WV, m->d_VZ, m->ncells, m->sms, (cudaStream_t)cuda_stream);
@@ -335,9 +372,13 @@ int fe_set_variant(fe_mesh* m, int variant)
 }
 
 // one fused operator launch: Y = mu (alpha (S sum_e P_e^T y_e - (c + eps) X) + beta Z)
+static int general_step(fe_mesh* m, const double* X, const double* Z, double* Y, int B, const double* eps,
+                        double alpha, double beta, double c, cudaStream_t st);
+
 static int operator_step(fe_mesh* m, const double* X, const double* Z, double* Y, int B, const double* eps,
                          double alpha, double beta, double c, cudaStream_t st)
 {
+    if (m->kind) return general_step(m, X, Z, Y, B, eps, alpha, beta, c, st);
     ApplyParams prm;
     fill_params(m, &prm);
     prm.X = X; prm.Z = Z; prm.Y = Y; prm.eps = eps; prm.B = B;
@@ -346,6 +387,127 @@ static int operator_step(fe_mesh* m, const double* X, const double* Z, double* Y
     cudaError_t e = launch_apply(prm, m->p, m->variant, m->N, m->ncells, st, &nl);
     if (e != cudaSuccess) return fail(FE_ERR_CUDA, "operator launch failed: %s", cudaGetErrorString(e));
     m->launches += nl;
+    return FE_OK;
+}
+
+// ---- general hexahedral meshes with hanging nodes (NEXT-3; fe_general.h / fe_general.cuh) ---------------------------------------
+template <class T>
+static int upload_vec(T** dst, const std::vector<T>& src)
+{
+    if (src.empty()) { *dst = nullptr; return FE_OK; }
+    CUDA_TRY(cudaMalloc((void**)dst, src.size() * sizeof(T)));
+    CUDA_TRY(cudaMemcpy(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice));
+    return FE_OK;
+}
+
+int fe_mesh_create_general(int cx, int cy, int cz, const int32_t* cells, int64_t ncells, const double* verts, int p,
+                           int cuda_device, fe_mesh** out)
+{
+    if (!out) return fail(FE_ERR_INVALID, "fe_mesh_create_general: out is NULL");
+    *out = nullptr;
+    if (!cells || !verts) return fail(FE_ERR_INVALID, "fe_mesh_create_general: NULL array");
+    if (p < 1 || p > 8) return fail(FE_ERR_INVALID, "fe_mesh_create_general: order p=%d outside 1..8", p);
+    if (cx < 1 || cy < 1 || cz < 1 || ncells < 1) return fail(FE_ERR_INVALID, "fe_mesh_create_general: empty mesh");
+    for (int64_t i = 0; i < ncells * 24; ++i)
+        if (!std::isfinite(verts[i])) return fail(FE_ERR_INVALID, "fe_mesh_create_general: corner coordinate %lld is not finite", (long long)i);
+    fe_mesh* m = new (std::nothrow) fe_mesh;
+    if (!m) return fail(FE_ERR_NOMEM, "fe_mesh_create_general: host allocation failed");
+    m->gh = new (std::nothrow) GeneralHost;
+    if (!m->gh) { delete m; return fail(FE_ERR_NOMEM, "fe_mesh_create_general: host allocation failed"); }
+    m->kind = 1; m->p = p; m->n = p + 1; m->nc = m->n * m->n * m->n; m->cx = cx; m->cy = cy; m->cz = cz;
+    build_tables(p, &m->tab);
+    char msg[400];
+    if (build_general_mesh(cx, cy, cz, cells, ncells, verts, p, m->tab, m->gh, msg, sizeof(msg))) {
+        fe_mesh_destroy(m);
+        return fail(FE_ERR_INVALID, "%s", msg);
+    }
+    const GeneralHost& g = *m->gh;
+    m->N = g.N; m->ncells = ncells;
+    if (cuda_device == -1) {  // tables only (numbering, constraints, coordinates, mass): no device, no operator
+        m->device = -1;
+        *out = m;
+        return FE_OK;
+    }
+    int ndev = 0;
+    cudaError_t ce = cudaGetDeviceCount(&ndev);
+    if (ce != cudaSuccess || cuda_device < 0 || cuda_device >= ndev) {
+        fe_mesh_destroy(m);
+        return ce != cudaSuccess ? fail(FE_ERR_CUDA, "fe_mesh_create_general: %s", cudaGetErrorString(ce))
+                                 : fail(FE_ERR_INVALID, "fe_mesh_create_general: no CUDA device %d", cuda_device);
+    }
+    m->device = cuda_device;
+    cudaDeviceProp prop;
+    if (cudaSetDevice(cuda_device) != cudaSuccess || cudaGetDeviceProperties(&prop, cuda_device) != cudaSuccess || prop.major < 10) {
+        fe_mesh_destroy(m);
+        return fail(FE_ERR_CUDA, "fe_mesh_create_general: device %d is not an sm_100 device", cuda_device);
+    }
+    m->sms = prop.multiProcessorCount;
+    // s_g = mu_g M_c,gg^{-1/2} (Eq. 19 with the constrained lumped mass, R25); metric split into its tensor and weight parts
+    std::vector<double> sv((size_t)g.N), met((size_t)ncells * 6 * m->nc), wdet((size_t)ncells * m->nc);
+    for (int64_t i = 0; i < g.N; ++i) sv[i] = g.mask[i] ? 1.0 / std::sqrt(g.mass[i]) : 0.0;
+    for (int64_t e = 0; e < ncells; ++e) {
+        memcpy(&met[(size_t)e * 6 * m->nc], &g.metric[(size_t)e * 7 * m->nc], (size_t)6 * m->nc * sizeof(double));
+        memcpy(&wdet[(size_t)e * m->nc], &g.metric[((size_t)e * 7 + 6) * m->nc], (size_t)m->nc * sizeof(double));
+    }
+    std::vector<long long> crow(g.crow.begin(), g.crow.end());
+    int rc;
+    if ((rc = upload_vec(&m->d_sm, sv)) || (rc = upload_vec(&m->d_gl2g, g.l2g)) || (rc = upload_vec(&m->d_gmetric, met)) ||
+        (rc = upload_vec(&m->d_gwdet, wdet)) || (rc = upload_vec(&m->d_crow, crow)) || (rc = upload_vec(&m->d_ccol, g.ccol)) ||
+        (rc = upload_vec(&m->d_cval, g.cval))) {
+        fe_mesh_destroy(m);
+        return rc;
+    }
+    ce = cudaMalloc((void**)&m->d_gWV, (size_t)ncells * m->nc * sizeof(double));
+    if (ce != cudaSuccess) { fe_mesh_destroy(m); return fail(FE_ERR_NOMEM, "fe_mesh_create_general: %s", cudaGetErrorString(ce)); }
+    *out = m;
+    return FE_OK;
+}
+
+int fe_get_constraints(const fe_mesh* m, int64_t* row_ptr, int32_t* col, double* val)
+{
+    if (!m || !row_ptr) return fail(FE_ERR_INVALID, "fe_get_constraints: NULL argument");
+    if (!m->kind) { row_ptr[0] = 0; return FE_OK; }
+    const GeneralHost& g = *m->gh;
+    memcpy(row_ptr, g.crow.data(), g.crow.size() * sizeof(int64_t));
+    if (!g.ccol.empty()) {
+        if (!col || !val) return fail(FE_ERR_INVALID, "fe_get_constraints: NULL argument");
+        memcpy(col, g.ccol.data(), g.ccol.size() * sizeof(int32_t));
+        memcpy(val, g.cval.data(), g.cval.size() * sizeof(double));
+    }
+    return FE_OK;
+}
+
+// one fused operator step on a general mesh: diagonal terms (k_gen_init), expansion of the hanging values, the cell kernel,
+// the transposed expansion
+static int general_step(fe_mesh* m, const double* X, const double* Z, double* Y, int B, const double* eps,
+                        double alpha, double beta, double c, cudaStream_t st)
+{
+    const GeneralHost& g = *m->gh;
+    const long long nh = g.N_all - g.N;
+    if (nh > 0 && m->hcap < B) {
+        cudaFree(m->d_Xh); cudaFree(m->d_Yh);
+        m->d_Xh = m->d_Yh = nullptr; m->hcap = 0;
+        CUDA_TRY(cudaMalloc((void**)&m->d_Xh, (size_t)nh * B * sizeof(double)));
+        CUDA_TRY(cudaMalloc((void**)&m->d_Yh, (size_t)nh * B * sizeof(double)));
+        m->hcap = B;
+    }
+    const int grid = m->sms * 8;
+    k_gen_init<<<grid, 256, 0, st>>>(Y, X, Z, m->d_sm, eps, alpha, beta, c, g.N, B);
+    if (nh > 0) {
+        CUDA_TRY(cudaMemsetAsync(m->d_Yh, 0, (size_t)nh * B * sizeof(double), st));
+        k_gen_expand<<<grid, 256, 0, st>>>(m->d_Xh, X, m->d_sm, m->d_crow, m->d_ccol, m->d_cval, nh, B);
+    }
+    GenParams prm;
+    memset(&prm, 0, sizeof(prm));
+    prm.X = X; prm.Xh = m->d_Xh; prm.Y = Y; prm.Yh = m->d_Yh; prm.s = m->d_sm; prm.l2g = m->d_gl2g;
+    prm.metric = m->d_gmetric; prm.WV = m->d_gWV; prm.N = g.N; prm.B = B; prm.alpha = alpha;
+    const int n = m->n;
+    for (int i = 0; i < n * n; ++i) { prm.Nt[i] = m->tab.N[i]; prm.Dt[i] = m->tab.D[i]; }
+    cudaError_t e = launch_apply_gen(prm, m->p, m->ncells, st);
+    if (e != cudaSuccess) return fail(FE_ERR_CUDA, "operator launch (general mesh) failed: %s", cudaGetErrorString(e));
+    if (nh > 0) k_gen_collapse<<<grid, 256, 0, st>>>(Y, m->d_Yh, m->d_sm, m->d_crow, m->d_ccol, m->d_cval, nh, B, alpha);
+    CUDA_TRY(cudaGetLastError());
+    m->launches += nh > 0 ? 4 : 2;
     return FE_OK;
 }
 
@@ -402,7 +564,7 @@ static int make_block_maps(BlockMaps* bm, const fe_mesh* m, const double* base, 
 // bulk tensor copies need 16-byte aligned bases and row pitches (B even)
 static bool tma_eligible(const fe_mesh* m, int B, const void* a, const void* b, const void* c)
 {
-    if (m->variant == 3 || m->variant == 4) return false;
+    if (m->kind || m->variant == 3 || m->variant == 4) return false;
     if (B % 2 != 0 || !encode_fn()) return false;
     return (((uintptr_t)a | (uintptr_t)b | (uintptr_t)c) & 15) == 0;
 }
@@ -441,8 +603,20 @@ static int tma_step(fe_mesh* m, const BlockMaps& X, const BlockMaps& Y, const Bl
     return FE_OK;
 }
 
+__global__ void k_zero_masked_rows(double* __restrict__ Y, const double* __restrict__ s, long long N, int B)
+{
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N * B; i += (long long)gridDim.x * blockDim.x)
+        if (s[i / B] == 0.0) Y[i] = 0.0;
+}
+
 static int zero_faces(fe_mesh* m, double* Y, int B, cudaStream_t st)
 {
+    if (m->kind) {  // no tensor structure: the Dirichlet rows are those with s_g = 0
+        k_zero_masked_rows<<<m->sms * 8, 256, 0, st>>>(Y, m->d_sm, m->N, B);
+        CUDA_TRY(cudaGetLastError());
+        m->launches += 1;
+        return FE_OK;
+    }
     k_zero_faces<<<m->sms * 4, 256, 0, st>>>(Y, m->Nx, m->Ny, m->Nz, B);
     CUDA_TRY(cudaGetLastError());
     m->launches += 1;
@@ -785,6 +959,7 @@ int fe_minres_shifted(fe_mesh* m, const double* G, double* X, int B, const doubl
                       int precondition, double* relres_host, int* iters_host, double* work, void* cuda_stream)
 {
     if (!m || !G || !X || !work) return fail(FE_ERR_INVALID, "fe_minres_shifted: NULL argument");
+    if (m->kind) return fail(FE_ERR_INVALID, "fe_minres_shifted: not available on general meshes");
     if (B < 1 || B > 128) return fail(FE_ERR_INVALID, "fe_minres_shifted: B=%d outside 1..128", B);
     if (maxit < 1 || !(tol >= 0.0)) return fail(FE_ERR_INVALID, "fe_minres_shifted: need maxit >= 1 and tol >= 0");
     if (!m->have_V) return fail(FE_ERR_STATE, "fe_minres_shifted: call fe_set_potential first");
@@ -877,6 +1052,7 @@ int fe_gram(fe_mesh* m, const double* A, const double* Bm, int B, double* C_host
 int fe_density(fe_mesh* m, const double* X, int B, const double* f_dev, double* rho_dev, void* cuda_stream)
 {
     if (!m || !X || !f_dev || !rho_dev) return fail(FE_ERR_INVALID, "fe_density: NULL argument");
+    if (m->kind) return fail(FE_ERR_INVALID, "fe_density: not available on general meshes");
     if (B < 1) return fail(FE_ERR_INVALID, "fe_density: B=%d < 1", B);
     CUDA_TRY(cudaSetDevice(m->device));
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -1022,6 +1198,7 @@ int cheb_filter_host(fe_mesh* m, double* X_host, int B, int deg, double a, doubl
 int fe_apply_potential(fe_mesh* m, const double* Uq_dev, const double* X, double* Y, int B, void* cuda_stream)
 {
     if (!m || !Uq_dev || !X || !Y) return fail(FE_ERR_INVALID, "fe_apply_potential: NULL argument");
+    if (m->kind) return fail(FE_ERR_INVALID, "fe_apply_potential: not available on general meshes");
     if (B < 1) return fail(FE_ERR_INVALID, "fe_apply_potential: B=%d < 1", B);
     const size_t len = (size_t)m->N * B;
     if (overlap(X, len, Y, len)) return fail(FE_ERR_INVALID, "fe_apply_potential: X and Y overlap");

@@ -134,12 +134,33 @@ void build_tables(int p, Tables1D* t)
             }
         D[s][s] = diag;
     }
+    for (int s = 0; s < n; ++s)
+        for (int q = 0; q < n; ++q) t->D[s * n + q] = (double)D[s][q];
     for (int q = 0; q < n; ++q)
         for (int r = 0; r < n; ++r) {
             real g = 0.0L;
             for (int s = 0; s < n; ++s) g += gw[s] * D[s][q] * D[s][r];
             t->G[q * n + r] = (double)g;
         }
+}
+
+void lagrange_gll(const Tables1D& t, double x, double* out)
+{
+    const int n = t.n;
+    for (int j = 0; j < n; ++j)
+        if (x == t.gll_x[j]) {
+            for (int a = 0; a < n; ++a) out[a] = (a == j) ? 1.0 : 0.0;
+            return;
+        }
+    real b[kMaxN], den = 0.0L;
+    for (int a = 0; a < n; ++a) {
+        real pr = 1.0L;
+        for (int j = 0; j < n; ++j)
+            if (j != a) pr *= ((real)t.gll_x[a] - (real)t.gll_x[j]);
+        b[a] = 1.0L / (pr * ((real)x - (real)t.gll_x[a]));
+        den += b[a];
+    }
+    for (int a = 0; a < n; ++a) out[a] = (double)(b[a] / den);
 }
 
 }  // namespace fecheb
