@@ -74,7 +74,8 @@ struct fe_mesh {
     int kind = 0;  // 0: tensor-product box mesh, 1: general
     GeneralHost* gh = nullptr;
     int32_t* d_gl2g = nullptr;
-    double *d_gmetric = nullptr, *d_gwdet = nullptr, *d_gWV = nullptr;
+    double *d_gmetric = nullptr, *d_gwdet = nullptr, *d_gsc = nullptr;
+    EOTab eoD, eoDT;  // even-odd halves of the collocation derivative and its transpose (centro-antisymmetric)
     long long* d_crow = nullptr;
     int32_t* d_ccol = nullptr;
     double* d_cval = nullptr;
@@ -213,7 +214,7 @@ int fe_mesh_destroy(fe_mesh* m)
     for (cudaStream_t s : m->hstream) if (s) cudaStreamDestroy(s);
     cudaFree(m->d_small); cudaFree(m->d_minv); cudaFree(m->d_mask); cudaFree(m->d_scal);
     cudaFree(m->d_VZ); cudaFree(m->d_sx); cudaFree(m->d_sy); cudaFree(m->d_sz);
-    cudaFree(m->d_gl2g); cudaFree(m->d_gmetric); cudaFree(m->d_gwdet); cudaFree(m->d_gWV); cudaFree(m->d_crow);
+    cudaFree(m->d_gl2g); cudaFree(m->d_gmetric); cudaFree(m->d_gwdet); cudaFree(m->d_gsc); cudaFree(m->d_crow);
     cudaFree(m->d_ccol); cudaFree(m->d_cval); cudaFree(m->d_Xh); cudaFree(m->d_Yh);
     delete m->gh;
     delete m;
@@ -348,7 +349,8 @@ int fe_set_potential(fe_mesh* m, const double* Vq_dev, int copy, void* cuda_stre
     if (m->device < 0) return fail(FE_ERR_STATE, "fe_set_potential: the handle was created without a device (tables only)");
     CUDA_TRY(cudaSetDevice(m->device));
     if (m->kind) {
-        k_gen_weight_potential<<<m->sms * 8, 256, 0, (cudaStream_t)cuda_stream>>>(m->d_gWV, Vq_dev, m->d_gwdet, m->ncells * m->nc);
+        k_gen_weight_potential<<<m->sms * 8, 256, 0, (cudaStream_t)cuda_stream>>>(m->d_gmetric, Vq_dev, m->d_gwdet, m->ncells, m->nc,
+                                                                                  gen_rec_doubles(m->n));
         CUDA_TRY(cudaGetLastError());
         m->launches += 1;
         m->have_V = true;
@@ -443,22 +445,35 @@ int fe_mesh_create_general(int cx, int cy, int cz, const int32_t* cells, int64_t
     }
     m->sms = prop.multiProcessorCount;
     // s_g = mu_g M_c,gg^{-1/2} (Eq. 19 with the constrained lumped mass, R25); metric split into its tensor and weight parts
-    std::vector<double> sv((size_t)g.N), met((size_t)ncells * 6 * m->nc), wdet((size_t)ncells * m->nc);
+    const int grec = gen_rec_doubles(m->n);
+    std::vector<double> sv((size_t)g.N), met((size_t)ncells * grec, 0.0), wdet((size_t)ncells * m->nc);
     for (int64_t i = 0; i < g.N; ++i) sv[i] = g.mask[i] ? 1.0 / std::sqrt(g.mass[i]) : 0.0;
     for (int64_t e = 0; e < ncells; ++e) {
-        memcpy(&met[(size_t)e * 6 * m->nc], &g.metric[(size_t)e * 7 * m->nc], (size_t)6 * m->nc * sizeof(double));
+        memcpy(&met[(size_t)e * grec], &g.metric[(size_t)e * 7 * m->nc], (size_t)6 * m->nc * sizeof(double));
         memcpy(&wdet[(size_t)e * m->nc], &g.metric[((size_t)e * 7 + 6) * m->nc], (size_t)m->nc * sizeof(double));
     }
     std::vector<long long> crow(g.crow.begin(), g.crow.end());
+    std::vector<double> scv(g.l2g.size());
+    for (size_t i = 0; i < scv.size(); ++i) scv[i] = g.l2g[i] < g.N ? sv[g.l2g[i]] : 1.0;
+    {   // plain (unfolded) tables for the general kernel; D is centro-antisymmetric: its middle row goes to row h of S
+        const int n = m->n, h = n / 2;
+        double Dt[kMaxN * kMaxN];
+        for (int a = 0; a < n; ++a)
+            for (int b = 0; b < n; ++b) Dt[a * n + b] = m->tab.D[b * n + a];
+        make_eo(m->tab.N, n, false, &m->eoN);
+        make_eo(m->tab.N, n, true, &m->eoNT);
+        make_eo(m->tab.D, n, false, &m->eoD);
+        make_eo(Dt, n, false, &m->eoDT);
+        if (n % 2 == 1)
+            for (int k = 0; k < h; ++k) { m->eoD.S[h * h + k] = m->tab.D[h * n + k]; m->eoDT.S[h * h + k] = Dt[h * n + k]; }
+    }
     int rc;
-    if ((rc = upload_vec(&m->d_sm, sv)) || (rc = upload_vec(&m->d_gl2g, g.l2g)) || (rc = upload_vec(&m->d_gmetric, met)) ||
+    if ((rc = upload_vec(&m->d_gsc, scv)) || (rc = upload_vec(&m->d_sm, sv)) || (rc = upload_vec(&m->d_gl2g, g.l2g)) || (rc = upload_vec(&m->d_gmetric, met)) ||
         (rc = upload_vec(&m->d_gwdet, wdet)) || (rc = upload_vec(&m->d_crow, crow)) || (rc = upload_vec(&m->d_ccol, g.ccol)) ||
         (rc = upload_vec(&m->d_cval, g.cval))) {
         fe_mesh_destroy(m);
         return rc;
     }
-    ce = cudaMalloc((void**)&m->d_gWV, (size_t)ncells * m->nc * sizeof(double));
-    if (ce != cudaSuccess) { fe_mesh_destroy(m); return fail(FE_ERR_NOMEM, "fe_mesh_create_general: %s", cudaGetErrorString(ce)); }
     *out = m;
     return FE_OK;
 }
@@ -499,10 +514,9 @@ static int general_step(fe_mesh* m, const double* X, const double* Z, double* Y,
     }
     GenParams prm;
     memset(&prm, 0, sizeof(prm));
-    prm.X = X; prm.Xh = m->d_Xh; prm.Y = Y; prm.Yh = m->d_Yh; prm.s = m->d_sm; prm.l2g = m->d_gl2g;
-    prm.metric = m->d_gmetric; prm.WV = m->d_gWV; prm.N = g.N; prm.B = B; prm.alpha = alpha;
-    const int n = m->n;
-    for (int i = 0; i < n * n; ++i) { prm.Nt[i] = m->tab.N[i]; prm.Dt[i] = m->tab.D[i]; }
+    prm.X = X; prm.Xh = m->d_Xh ? m->d_Xh : X; prm.Y = Y; prm.Yh = m->d_Yh ? m->d_Yh : Y; prm.sc = m->d_gsc; prm.l2g = m->d_gl2g;
+    prm.rec = m->d_gmetric; prm.N = g.N; prm.B = B; prm.alpha = alpha;
+    prm.eoN = m->eoN; prm.eoNT = m->eoNT; prm.eoD = m->eoD; prm.eoDT = m->eoDT;
     cudaError_t e = launch_apply_gen(prm, m->p, m->ncells, st);
     if (e != cudaSuccess) return fail(FE_ERR_CUDA, "operator launch (general mesh) failed: %s", cudaGetErrorString(e));
     if (nh > 0) k_gen_collapse<<<grid, 256, 0, st>>>(Y, m->d_Yh, m->d_sm, m->d_crow, m->d_ccol, m->d_cval, nh, B, alpha);

@@ -16,7 +16,7 @@
 // Threads: lane = vector j (BT per cell tile), threadIdx.y = a plane index.  A thread owns a nodal z-plane (phases A, E),
 // the yz-plane qx = pl (phases B, D: everything along z) or the xy-plane qz = pl (phase C: everything along x and y), so
 // every 1-D matrix entry is a warp-uniform constant-bank operand; the cell tile crosses shared memory between phases
-// (four fields of n^3 x BT doubles: U/t/T/R, gz/fz, fx, fy).  Gather and scatter go through the explicit l2g; hanging
+// (three fields of n^3 x BT doubles: x/A/U/t/R, gy/fy, gz/fz).  Gather and scatter go through the explicit l2g; hanging
 // nodes read the expanded values X_h = C_h (s . X) (k_gen_expand) and scatter into Y_h, which k_gen_collapse distributes
 // to the unconstrained nodes with C_h^T.  The shift and recurrence terms are written by k_gen_init, which replaces the
 // zero-fill of Y.
@@ -25,6 +25,7 @@
 
 #include <cstdint>
 
+#include "fe_apply_tma.cuh"
 #include "fe_kernels.cuh"
 
 namespace fecheb {
@@ -34,15 +35,15 @@ struct GenParams {
     const double* Xh;    // (N_all - N) * B: expanded hanging values
     double* Y;           // N * B
     double* Yh;          // (N_all - N) * B
-    const double* s;     // N: mu_g M_c,gg^{-1/2}
     const int32_t* l2g;  // ncells * n^3
-    const double* metric;  // ncells * 6 * n^3 (fe_general.h)
-    const double* WV;      // ncells * n^3: w_q |J| V_q
+    const double* sc;    // ncells * n^3: s_g = mu_g M_c,gg^{-1/2} at the cell's unconstrained nodes, 1 at its hanging nodes
+    const double* rec;   // ncells * GREC: per-cell record, 6 metric fields (fe_general.h) then WV = w_q |J| V_q, n^3 each
     long long N;
     int B;
     double alpha;
-    double Nt[81];  // N[q*n + a] = l_a(gl_x[q])
-    double Dt[81];  // D[s*n + q] = l^_q'(gl_x[s])
+    // even-odd halves (fe_kernels.cuh): N and N^T are centro-symmetric, the collocation derivative D and D^T are
+    // centro-ANTIsymmetric (D[n-1-s][n-1-q] = -D[s][q]); for those the row i = h of S holds the middle row D[h][k], k < h
+    EOTab eoN, eoNT, eoD, eoDT;
 };
 
 // Y = mu (kappa_j X + beta Z), kappa_j = -alpha (c + eps_j): the part of the step that is diagonal in the nodes
@@ -101,80 +102,122 @@ __global__ void k_gen_collapse(double* __restrict__ Y, const double* __restrict_
     }
 }
 
-// WV[e][q] = w_q |J| V[e][q] from the weight field of the metric (component 6)
-__global__ void k_gen_weight_potential(double* __restrict__ WV, const double* __restrict__ V,
-                                       const double* __restrict__ wdet, long long total)
-{
-    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x)
-        WV[i] = wdet[i] * V[i];
-}
+// per-cell record of the general kernel: 7 fields of n^3 doubles (6 metric entries, WV), padded to a multiple of 16 bytes
+inline int gen_rec_doubles(int n) { const int r = 7 * n * n * n; return r + (r & 1); }
 
-template <int n>
-__device__ __forceinline__ void mat1d(const double* __restrict__ M, const double (&in)[n], double (&out)[n])
+// field 6 of every record: WV[e][q] = w_q |J| V[e][q]
+__global__ void k_gen_weight_potential(double* __restrict__ rec, const double* __restrict__ V,
+                                       const double* __restrict__ wdet, long long ncells, int n3, int grec)
 {
-#pragma unroll
-    for (int i = 0; i < n; ++i) {
-        double s = M[i * n] * in[0];
-#pragma unroll
-        for (int k = 1; k < n; ++k) s = fma(M[i * n + k], in[k], s);
-        out[i] = s;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < ncells * n3; i += (long long)gridDim.x * blockDim.x) {
+        const long long e = i / n3;
+        rec[e * grec + 6 * n3 + (i - e * n3)] = wdet[i] * V[i];
     }
 }
+
+// even-odd product with a centro-ANTIsymmetric matrix: out[i] = E + O, out[n-1-i] = O - E (mat1d_eo has E - O there)
 template <int n>
-__device__ __forceinline__ void mat1d_t(const double* __restrict__ M, const double (&in)[n], double (&out)[n])  // M^T in
+__device__ __forceinline__ void mat1d_eoa(const EOTab& T, const double (&in)[n], double (&out)[n])
 {
+    constexpr int h = n / 2;
+    double e[h > 0 ? h : 1], o[h > 0 ? h : 1];
 #pragma unroll
-    for (int i = 0; i < n; ++i) {
-        double s = M[i] * in[0];
+    for (int k = 0; k < h; ++k) {
+        e[k] = in[k] + in[n - 1 - k];
+        o[k] = in[k] - in[n - 1 - k];
+    }
 #pragma unroll
-        for (int k = 1; k < n; ++k) s = fma(M[k * n + i], in[k], s);
-        out[i] = s;
+    for (int i = 0; i < h; ++i) {
+        double se;
+        if (n % 2 == 1) {
+            se = T.Mid[i] * in[h];
+#pragma unroll
+            for (int k = 0; k < h; ++k) se = fma(T.S[i * h + k], e[k], se);
+        } else {
+            se = T.S[i * h] * e[0];
+#pragma unroll
+            for (int k = 1; k < h; ++k) se = fma(T.S[i * h + k], e[k], se);
+        }
+        double so = T.A[i * h] * o[0];
+#pragma unroll
+        for (int k = 1; k < h; ++k) so = fma(T.A[i * h + k], o[k], so);
+        out[i] = se + so;
+        out[n - 1 - i] = so - se;
+    }
+    if (n % 2 == 1) {
+        double sm = 0.0;
+        if (h > 0) {
+            sm = T.S[h * h] * o[0];
+#pragma unroll
+            for (int k = 1; k < h; ++k) sm = fma(T.S[h * h + k], o[k], sm);
+        }
+        out[h] = sm;
     }
 }
 
 template <int P, int BT>
-constexpr size_t gen_smem_bytes() { return (size_t)4 * (P + 1) * (P + 1) * (P + 1) * BT * sizeof(double); }
+constexpr size_t gen_smem_bytes()
+{
+    constexpr int n3 = (P + 1) * (P + 1) * (P + 1);
+    return (size_t)3 * n3 * BT * sizeof(double) + (size_t)(7 * n3 + 1) * sizeof(double) +
+           (size_t)n3 * (sizeof(double) + sizeof(int32_t)) + 32;
+}
 
 template <int P, int BT, int MINB>
 __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_gen(const __grid_constant__ GenParams prm)
 {
     constexpr int n = P + 1, n2 = n * n, n3 = n * n * n;
-    extern __shared__ double smem[];
-    double* F0 = smem;                 // A -> U -> t / T -> R
-    double* F1 = F0 + (size_t)n3 * BT;  // gz -> fz
-    double* F2 = F1 + (size_t)n3 * BT;  // fx
-    double* F3 = F2 + (size_t)n3 * BT;  // fy
-    const int lane = threadIdx.x, pl = threadIdx.y;
+    extern __shared__ __align__(128) double smem[];
+    double* F0 = smem;                  // x -> A -> U -> t -> R
+    double* F1 = F0 + (size_t)n3 * BT;  // gy -> fy
+    double* F2 = F1 + (size_t)n3 * BT;  // gz -> fz
+    double* sRec = F2 + (size_t)n3 * BT;  // the cell's record (6 metric fields, WV), one bulk copy in flight during A and B
+    constexpr int GREC = 7 * n3 + ((7 * n3) & 1);
+    double* sSc = sRec + GREC;            // [n^3] gather / scatter scale of the cell's nodes
+    unsigned long long* bar = reinterpret_cast<unsigned long long*>(sSc + n3 + (n3 & 1));
+    int32_t* sId = reinterpret_cast<int32_t*>(bar + 1);  // [n^3] global ids
+    const int lane = threadIdx.x, pl = threadIdx.y, tid = pl * BT + lane;
     const long long cell = blockIdx.x;
     const int j = blockIdx.y * BT + lane;
     const bool act = j < prm.B;
     const long long B = prm.B;
-    const int32_t* l2g = prm.l2g + cell * n3;
-    const double* Nt = prm.Nt;
-    const double* Dt = prm.Dt;
     double t[n], o[n];
 
-    // ---- phase A: gather the nodal plane az = pl, interpolate in x and y ------------------------------------------------
+    // ---- gather: ids and scales of the cell, then every thread fetches ITS nodal plane with independent 8-byte cp.async ------
+    if (tid == 0) {
+        mbar_init(bar, 1);
+        mbar_expect_tx(bar, (unsigned)(GREC * sizeof(double)));
+        bulk_load(sRec, prm.rec + cell * GREC, (unsigned)(GREC * sizeof(double)), bar);
+    }
+    for (int a = tid; a < n3; a += n * BT) {
+        sId[a] = prm.l2g[cell * n3 + a];
+        sSc[a] = prm.sc[cell * n3 + a];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < n2; ++k) {
+        const int a = pl * n2 + k;
+        const long long g = sId[a];
+        const double* src = g < prm.N ? prm.X + g * B + j : prm.Xh + (g - prm.N) * B + j;
+        cp_async8(F0 + (size_t)a * BT + lane, act ? src : prm.X, act);
+    }
+    cp_async_commit();
+    cp_async_wait_all();
+    // ---- phase A: the nodal plane az = pl: scale, interpolate in x and y (table N) ---------------------------------------------
     {
         double v[n][n];
 #pragma unroll
         for (int ay = 0; ay < n; ++ay)
 #pragma unroll
             for (int ax = 0; ax < n; ++ax) {
-                const long long g = l2g[(pl * n + ay) * n + ax];
-                double x = 0.0;
-                if (act) {
-                    if (g < prm.N) {
-                        const double sg = prm.s[g];
-                        x = sg != 0.0 ? sg * prm.X[g * B + j] : 0.0;  // Dirichlet rows of caller data are ignored (R5)
-                    } else
-                        x = prm.Xh[(g - prm.N) * B + j];
-                }
-                v[ay][ax] = x;
+                const int a = pl * n2 + ay * n + ax;
+                const double sg = sSc[a];
+                const double x = F0[(size_t)a * BT + lane];
+                v[ay][ax] = sg != 0.0 ? sg * x : 0.0;  // Dirichlet rows of caller data are ignored (R5)
             }
 #pragma unroll
         for (int ay = 0; ay < n; ++ay) {
-            mat1d<n>(Nt, v[ay], o);
+            mat1d_eo<n>(prm.eoN, v[ay], o);
 #pragma unroll
             for (int q = 0; q < n; ++q) v[ay][q] = o[q];
         }
@@ -182,121 +225,128 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_gen(const __grid_c
         for (int qx = 0; qx < n; ++qx) {
 #pragma unroll
             for (int a = 0; a < n; ++a) t[a] = v[a][qx];
-            mat1d<n>(Nt, t, o);
+            mat1d_eo<n>(prm.eoN, t, o);
 #pragma unroll
-            for (int qy = 0; qy < n; ++qy) F0[((pl * n + qy) * n + qx) * BT + lane] = o[qy];
+            for (int qy = 0; qy < n; ++qy) F0[((size_t)(pl * n + qy) * n + qx) * BT + lane] = o[qy];
         }
     }
     __syncthreads();
-    // ---- phase B: the yz-plane qx = pl: U = Nz A, gz = Dz U (lines along z) ------------------------------------------------
+    // ---- phase B: the yz-plane qx = pl: U = Nz A (table N), then gz = Dz U along z and gy = Dy U along y (table D) ---------------
+    {
+        double u[n][n];  // [qy][qz]
 #pragma unroll
-    for (int qy = 0; qy < n; ++qy) {
+        for (int qy = 0; qy < n; ++qy) {
 #pragma unroll
-        for (int az = 0; az < n; ++az) t[az] = F0[((az * n + qy) * n + pl) * BT + lane];
-        mat1d<n>(Nt, t, o);
-        mat1d<n>(Dt, o, t);
+            for (int az = 0; az < n; ++az) t[az] = F0[((size_t)(az * n + qy) * n + pl) * BT + lane];
+            mat1d_eo<n>(prm.eoN, t, u[qy]);
+#pragma unroll
+            for (int qz = 0; qz < n; ++qz) F0[((size_t)(qz * n + qy) * n + pl) * BT + lane] = u[qy][qz];
+        }
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy) {
+            mat1d_eoa<n>(prm.eoD, u[qy], o);
+#pragma unroll
+            for (int qz = 0; qz < n; ++qz) F2[((size_t)(qz * n + qy) * n + pl) * BT + lane] = o[qz];
+        }
 #pragma unroll
         for (int qz = 0; qz < n; ++qz) {
-            F0[((qz * n + qy) * n + pl) * BT + lane] = o[qz];
-            F1[((qz * n + qy) * n + pl) * BT + lane] = t[qz];
+#pragma unroll
+            for (int qy = 0; qy < n; ++qy) t[qy] = u[qy][qz];
+            mat1d_eoa<n>(prm.eoD, t, o);
+#pragma unroll
+            for (int qy = 0; qy < n; ++qy) F1[((size_t)(qz * n + qy) * n + pl) * BT + lane] = o[qy];
         }
     }
     __syncthreads();
-    // ---- phase C: the xy-plane qz = pl: gx, gy, the pointwise metric, Dx^T and Dy^T ----------------------------------------
+    // ---- phase C: the xy-plane qz = pl, row by row: gx = Dx U (table D), the metric at the points, t = WV U + Dx^T fx (D^T) ------
     {
-        double u[n][n];
         const size_t base = (size_t)pl * n2;
+        double gx[n][n];
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy) {
+#pragma unroll
+            for (int qx = 0; qx < n; ++qx) t[qx] = F0[(base + qy * n + qx) * BT + lane];
+            mat1d_eoa<n>(prm.eoD, t, gx[qy]);
+        }
+        mbar_wait(bar, 0);
+        const double* Mq = sRec + pl * n2;  // + c * n3 + qy * n + qx
+        const double* WVq = sRec + 6 * n3 + pl * n2;
 #pragma unroll
         for (int qy = 0; qy < n; ++qy)
 #pragma unroll
-            for (int qx = 0; qx < n; ++qx) u[qy][qx] = F0[(base + qy * n + qx) * BT + lane];
-        const double* Mq = prm.metric + cell * 6 * n3 + pl * n2;  // + c * n3 + qy * n + qx
-        const double* WVq = prm.WV + cell * n3 + pl * n2;
-#pragma unroll
-        for (int qy = 0; qy < n; ++qy) {
-            double gx[n], gy[n];
-            mat1d<n>(Dt, u[qy], gx);
-#pragma unroll
-            for (int qx = 0; qx < n; ++qx) {
-                double s = Dt[qy * n] * u[0][qx];
-#pragma unroll
-                for (int r = 1; r < n; ++r) s = fma(Dt[qy * n + r], u[r][qx], s);
-                gy[qx] = s;
-            }
-#pragma unroll
             for (int qx = 0; qx < n; ++qx) {
                 const int q = qy * n + qx;
-                const double gz = F1[(base + q) * BT + lane];
+                const size_t idx = (base + q) * BT + lane;
+                const double gyv = F1[idx], gzv = F2[idx], gxv = gx[qy][qx];
                 const double g0 = Mq[q], g1 = Mq[n3 + q], g2 = Mq[2 * n3 + q], g3 = Mq[3 * n3 + q], g4 = Mq[4 * n3 + q],
                              g5 = Mq[5 * n3 + q];
-                F2[(base + q) * BT + lane] = fma(g0, gx[qx], fma(g1, gy[qx], g2 * gz));
-                F3[(base + q) * BT + lane] = fma(g1, gx[qx], fma(g3, gy[qx], g4 * gz));
-                F1[(base + q) * BT + lane] = fma(g2, gx[qx], fma(g4, gy[qx], g5 * gz));
+                gx[qy][qx] = fma(g0, gxv, fma(g1, gyv, g2 * gzv));
+                F1[idx] = fma(g1, gxv, fma(g3, gyv, g4 * gzv));
+                F2[idx] = fma(g2, gxv, fma(g4, gyv, g5 * gzv));
+                F0[idx] *= WVq[q];
             }
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy) {
+            mat1d_eoa<n>(prm.eoDT, gx[qy], o);
+#pragma unroll
+            for (int qx = 0; qx < n; ++qx) F0[(base + qy * n + qx) * BT + lane] += o[qx];
         }
-        // t = WV U + Dx^T fx (rows) + Dy^T fy (columns), into F0; the thread re-reads only what it wrote itself
+    }
+    __syncthreads();
+    // ---- phase D: the yz-plane qx = pl: T = t + Dz^T fz + Dy^T fy (table D^T), R = Nz^T T (table N^T) -----------------------------
+    {
+        double T[n][n];  // [qy][qz]
 #pragma unroll
         for (int qy = 0; qy < n; ++qy) {
 #pragma unroll
-            for (int qx = 0; qx < n; ++qx) t[qx] = F2[(base + qy * n + qx) * BT + lane];
-            mat1d_t<n>(Dt, t, o);
+            for (int qz = 0; qz < n; ++qz) t[qz] = F2[((size_t)(qz * n + qy) * n + pl) * BT + lane];
+            mat1d_eoa<n>(prm.eoDT, t, o);
 #pragma unroll
-            for (int qx = 0; qx < n; ++qx) u[qy][qx] = fma(WVq[qy * n + qx], u[qy][qx], o[qx]);
+            for (int qz = 0; qz < n; ++qz) T[qy][qz] = F0[((size_t)(qz * n + qy) * n + pl) * BT + lane] + o[qz];
         }
-#pragma unroll
-        for (int qx = 0; qx < n; ++qx) {
-#pragma unroll
-            for (int qy = 0; qy < n; ++qy) t[qy] = F3[(base + qy * n + qx) * BT + lane];
-            mat1d_t<n>(Dt, t, o);
-#pragma unroll
-            for (int qy = 0; qy < n; ++qy) F0[(base + qy * n + qx) * BT + lane] = u[qy][qx] + o[qy];
-        }
-    }
-    __syncthreads();
-    // ---- phase D: the yz-plane qx = pl again: T += Dz^T fz, R = Nz^T T --------------------------------------------------------
-#pragma unroll
-    for (int qy = 0; qy < n; ++qy) {
-        double tz[n];
 #pragma unroll
         for (int qz = 0; qz < n; ++qz) {
-            t[qz] = F1[((qz * n + qy) * n + pl) * BT + lane];
-            tz[qz] = F0[((qz * n + qy) * n + pl) * BT + lane];
+#pragma unroll
+            for (int qy = 0; qy < n; ++qy) t[qy] = F1[((size_t)(qz * n + qy) * n + pl) * BT + lane];
+            mat1d_eoa<n>(prm.eoDT, t, o);
+#pragma unroll
+            for (int qy = 0; qy < n; ++qy) T[qy][qz] += o[qy];
         }
-        mat1d_t<n>(Dt, t, o);
 #pragma unroll
-        for (int qz = 0; qz < n; ++qz) tz[qz] += o[qz];
-        mat1d_t<n>(Nt, tz, o);
+        for (int qy = 0; qy < n; ++qy) {
+            mat1d_eo<n>(prm.eoNT, T[qy], o);
 #pragma unroll
-        for (int az = 0; az < n; ++az) F0[((az * n + qy) * n + pl) * BT + lane] = o[az];
+            for (int az = 0; az < n; ++az) F0[((size_t)(az * n + qy) * n + pl) * BT + lane] = o[az];
+        }
     }
     __syncthreads();
-    // ---- phase E: back-interpolate the nodal plane az = pl in y and x, scatter through the l2g -------------------------------
+    // ---- phase E: back-interpolate the nodal plane az = pl in y and x (table N^T), scatter through the l2g ---------------------------
     {
         double v[n][n];
 #pragma unroll
         for (int qy = 0; qy < n; ++qy)
 #pragma unroll
-            for (int qx = 0; qx < n; ++qx) v[qy][qx] = F0[((pl * n + qy) * n + qx) * BT + lane];
+            for (int qx = 0; qx < n; ++qx) v[qy][qx] = F0[((size_t)(pl * n + qy) * n + qx) * BT + lane];
 #pragma unroll
         for (int qx = 0; qx < n; ++qx) {
 #pragma unroll
             for (int q = 0; q < n; ++q) t[q] = v[q][qx];
-            mat1d_t<n>(Nt, t, o);
+            mat1d_eo<n>(prm.eoNT, t, o);
 #pragma unroll
             for (int a = 0; a < n; ++a) v[a][qx] = o[a];
         }
 #pragma unroll
         for (int ay = 0; ay < n; ++ay) {
-            mat1d_t<n>(Nt, v[ay], o);
+            mat1d_eo<n>(prm.eoNT, v[ay], o);
             if (act) {
 #pragma unroll
                 for (int ax = 0; ax < n; ++ax) {
-                    const long long g = l2g[(pl * n + ay) * n + ax];
-                    if (g < prm.N) {
-                        const double sg = prm.s[g];
-                        if (sg != 0.0) atomicAdd(prm.Y + g * B + j, prm.alpha * sg * o[ax]);
-                    } else
-                        atomicAdd(prm.Yh + (g - prm.N) * B + j, o[ax]);
+                    const int a = pl * n2 + ay * n + ax;
+                    const long long g = sId[a];
+                    const double sg = sSc[a];
+                    const bool master = g < prm.N;
+                    double* dst = master ? prm.Y + g * B + j : prm.Yh + (g - prm.N) * B + j;
+                    if (sg != 0.0) atomicAdd(dst, master ? prm.alpha * sg * o[ax] : o[ax]);
                 }
             }
         }
@@ -318,17 +368,17 @@ cudaError_t launch_gen(const GenParams& prm, long long ncells, cudaStream_t st)
     return cudaGetLastError();
 }
 
-// vector-tile width per order: four fields of n^3 x BT doubles must fit the 227 KB of shared memory
+// vector-tile width per order: three fields of n^3 x BT doubles per CTA, several CTAs per SM where they fit
 inline cudaError_t launch_apply_gen(const GenParams& prm, int p, long long ncells, cudaStream_t st)
 {
     switch (p) {
         case 1: return launch_gen<1, 32, 8>(prm, ncells, st);
-        case 2: return launch_gen<2, 32, 4>(prm, ncells, st);
-        case 3: return launch_gen<3, 32, 3>(prm, ncells, st);
-        case 4: return launch_gen<4, 16, 3>(prm, ncells, st);
+        case 2: return launch_gen<2, 32, 6>(prm, ncells, st);
+        case 3: return launch_gen<3, 32, 4>(prm, ncells, st);
+        case 4: return launch_gen<4, 32, 2>(prm, ncells, st);
         case 5: return launch_gen<5, 16, 2>(prm, ncells, st);
         case 6: return launch_gen<6, 16, 1>(prm, ncells, st);
-        case 7: return launch_gen<7, 8, 1>(prm, ncells, st);
+        case 7: return launch_gen<7, 8, 2>(prm, ncells, st);
         case 8: return launch_gen<8, 8, 1>(prm, ncells, st);
     }
     return cudaErrorInvalidValue;

@@ -316,3 +316,19 @@ def octree_mesh(xe, ye, ze, refine, maxlevel, deform=None):
         for v in range(8):
             verts[e, v] = P[(ix + (v & 1)) * s, (iy + ((v >> 1) & 1)) * s, (iz + (v >> 2)) * s]
     return OctreeMesh(cx, cy, cz, np.array(cells, dtype=np.int32).reshape(-1, 4), verts, L)
+
+
+def adaptive_molecule(roots=12, half=12.0, levels=2, radii=(3.0, 1.5), atom_seed=1003, n_atoms=10, zmax=8):
+    """NEXT-3 workload: the atoms of config 3 on an adaptively refined mesh -- a roots^3 root grid on [-half, half]^3,
+    refined `levels` times where a cell centre is within radii[level] of an atom (cell size half/roots*2 -> /4 near the
+    nuclei), the shape of the paper's meshes (l.273, Fig. 6).  Returns (OctreeMesh, V) with V(quad_xyz) the soft-Coulomb
+    wells of R12."""
+    e = uniform_edges(-half, half, roots)
+    R, Z = atoms(atom_seed, n_atoms, zmax)
+
+    def refine(level, lo, hi):
+        c = 0.5 * (lo + hi)
+        return bool((np.linalg.norm(R - c, axis=1) < radii[level]).any())
+
+    mesh = octree_mesh(e, e, e, refine, levels)
+    return mesh, (lambda q: soft_coulomb(q, R, Z))
