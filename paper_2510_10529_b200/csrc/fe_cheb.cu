@@ -78,7 +78,7 @@ struct fe_mesh {
     EOTab eoD, eoDT;  // even-odd halves of the collocation derivative and its transpose (centro-antisymmetric)
     long long* d_crow = nullptr;
     int32_t* d_ccol = nullptr;
-    double* d_cval = nullptr;
+    double* d_cval = nullptr;  // constraint weight times s of its unconstrained node (fe_general.cuh: cs)
     double *d_Xh = nullptr, *d_Yh = nullptr;  // (N_all - N) * hcap: expanded hanging values / their scatter target
     int hcap = 0;
     int sms = 0;  // multiprocessors of the device (persistent grid size)
@@ -453,8 +453,9 @@ int fe_mesh_create_general(int cx, int cy, int cz, const int32_t* cells, int64_t
         memcpy(&wdet[(size_t)e * m->nc], &g.metric[((size_t)e * 7 + 6) * m->nc], (size_t)m->nc * sizeof(double));
     }
     std::vector<long long> crow(g.crow.begin(), g.crow.end());
-    std::vector<double> scv(g.l2g.size());
+    std::vector<double> scv(g.l2g.size()), csv(g.cval.size());
     for (size_t i = 0; i < scv.size(); ++i) scv[i] = g.l2g[i] < g.N ? sv[g.l2g[i]] : 1.0;
+    for (size_t k = 0; k < csv.size(); ++k) csv[k] = g.cval[k] * sv[g.ccol[k]];  // constraint weight times s of its node
     {   // plain (unfolded) tables for the general kernel; D is centro-antisymmetric: its middle row goes to row h of S
         const int n = m->n, h = n / 2;
         double Dt[kMaxN * kMaxN];
@@ -470,7 +471,7 @@ int fe_mesh_create_general(int cx, int cy, int cz, const int32_t* cells, int64_t
     int rc;
     if ((rc = upload_vec(&m->d_gsc, scv)) || (rc = upload_vec(&m->d_sm, sv)) || (rc = upload_vec(&m->d_gl2g, g.l2g)) || (rc = upload_vec(&m->d_gmetric, met)) ||
         (rc = upload_vec(&m->d_gwdet, wdet)) || (rc = upload_vec(&m->d_crow, crow)) || (rc = upload_vec(&m->d_ccol, g.ccol)) ||
-        (rc = upload_vec(&m->d_cval, g.cval))) {
+        (rc = upload_vec(&m->d_cval, csv))) {
         fe_mesh_destroy(m);
         return rc;
     }
@@ -507,10 +508,14 @@ static int general_step(fe_mesh* m, const double* X, const double* Z, double* Y,
         m->hcap = B;
     }
     const int grid = m->sms * 8;
-    k_gen_init<<<grid, 256, 0, st>>>(Y, X, Z, m->d_sm, eps, alpha, beta, c, g.N, B);
+    const dim3 rows(32, kGenRows);
+    if (!Z && !eps && c == 0.0)  // plain apply: nothing diagonal to write, Y is just cleared
+        CUDA_TRY(cudaMemsetAsync(Y, 0, (size_t)g.N * B * sizeof(double), st));
+    else
+        k_gen_init<<<grid, rows, 0, st>>>(Y, X, Z, m->d_sm, eps, alpha, beta, c, g.N, B);
     if (nh > 0) {
         CUDA_TRY(cudaMemsetAsync(m->d_Yh, 0, (size_t)nh * B * sizeof(double), st));
-        k_gen_expand<<<grid, 256, 0, st>>>(m->d_Xh, X, m->d_sm, m->d_crow, m->d_ccol, m->d_cval, nh, B);
+        k_gen_expand<<<grid, rows, 0, st>>>(m->d_Xh, X, m->d_crow, m->d_ccol, m->d_cval, nh, B);
     }
     GenParams prm;
     memset(&prm, 0, sizeof(prm));
@@ -519,7 +524,7 @@ static int general_step(fe_mesh* m, const double* X, const double* Z, double* Y,
     prm.eoN = m->eoN; prm.eoNT = m->eoNT; prm.eoD = m->eoD; prm.eoDT = m->eoDT;
     cudaError_t e = launch_apply_gen(prm, m->p, m->ncells, st);
     if (e != cudaSuccess) return fail(FE_ERR_CUDA, "operator launch (general mesh) failed: %s", cudaGetErrorString(e));
-    if (nh > 0) k_gen_collapse<<<grid, 256, 0, st>>>(Y, m->d_Yh, m->d_sm, m->d_crow, m->d_ccol, m->d_cval, nh, B, alpha);
+    if (nh > 0) k_gen_collapse<<<grid, rows, 0, st>>>(Y, m->d_Yh, m->d_crow, m->d_ccol, m->d_cval, nh, B, alpha);
     CUDA_TRY(cudaGetLastError());
     m->launches += nh > 0 ? 4 : 2;
     return FE_OK;

@@ -13,10 +13,10 @@
 //   T  = t + Dx^T fx + Dy^T fy + Dz^T fz                                                                    3 sweeps
 //   y_e = (Nx^T Ny^T Nz^T) T                                                                                3 sweeps
 //
-// Threads: lane = vector j (BT per cell tile), threadIdx.y = a plane index.  A thread owns a nodal z-plane (phases A, E),
-// the yz-plane qx = pl (phases B, D: everything along z) or the xy-plane qz = pl (phase C: everything along x and y), so
-// every 1-D matrix entry is a warp-uniform constant-bank operand; the cell tile crosses shared memory between phases
-// (three fields of n^3 x BT doubles: x/A/U/t/R, gy/fy, gz/fz).  Gather and scatter go through the explicit l2g; hanging
+// Threads: lane = vector j (BT per cell tile), threadIdx.y = a line slot.  Each of the 12 sweeps is a loop over the n^2
+// lines of its direction, dealt to the line slots; a thread holds one line (n values) in registers, every 1-D matrix entry
+// is a warp-uniform operand, and the cell tile lives in shared memory (three fields of n^3 x BT doubles: x/A/U/t/R, gy/fy,
+// gz/fz) with a CTA barrier where the direction changes.  Gather and scatter go through the explicit l2g; hanging
 // nodes read the expanded values X_h = C_h (s . X) (k_gen_expand) and scatter into Y_h, which k_gen_collapse distributes
 // to the unconstrained nodes with C_h^T.  The shift and recurrence terms are written by k_gen_init, which replaces the
 // zero-fill of Y.
@@ -46,58 +46,67 @@ struct GenParams {
     EOTab eoN, eoNT, eoD, eoDT;
 };
 
+// Block shape of the row-wise helper kernels: lanes run over the vectors j of a row, threadIdx.y over rows
+constexpr int kGenRows = 8;
+
 // Y = mu (kappa_j X + beta Z), kappa_j = -alpha (c + eps_j): the part of the step that is diagonal in the nodes
 __global__ void k_gen_init(double* __restrict__ Y, const double* __restrict__ X, const double* __restrict__ Z,
                            const double* __restrict__ s, const double* __restrict__ eps, double alpha, double beta,
                            double c, long long N, int B)
 {
-    const long long total = N * B;
-    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
-        const long long g = i / B;
-        const int j = (int)(i - g * B);
-        double v = 0.0;
-        if (s[g] != 0.0) {
-            const double kappa = -alpha * (c + (eps ? eps[j] : 0.0));
-            if (kappa != 0.0) v = kappa * X[i];
-            if (Z) v = fma(beta, Z[i], v);
+    for (long long g = blockIdx.x * (long long)kGenRows + threadIdx.y; g < N; g += (long long)gridDim.x * kGenRows) {
+        const bool fr = s[g] != 0.0;
+        for (int j = threadIdx.x; j < B; j += 32) {
+            const long long i = g * B + j;
+            double v = 0.0;
+            if (fr) {
+                const double kappa = -alpha * (c + (eps ? eps[j] : 0.0));
+                if (kappa != 0.0) v = kappa * X[i];
+                if (Z) v = fma(beta, Z[i], v);
+            }
+            Y[i] = v;
         }
-        Y[i] = v;
     }
 }
 
-// X_h[r, j] = sum_k cval (s . X)[ccol, j]: values of the hanging nodes (rows r of the constraint matrix)
-__global__ void k_gen_expand(double* __restrict__ Xh, const double* __restrict__ X, const double* __restrict__ s,
-                             const long long* __restrict__ crow, const int32_t* __restrict__ ccol,
-                             const double* __restrict__ cval, long long nh, int B)
+// X_h[r, j] = sum_k cs_k X[ccol_k, j], cs = cval * s[ccol] (0 on Dirichlet rows, whose caller data is ignored): values of the
+// hanging nodes (rows r of the constraint matrix applied to s . X)
+__global__ void k_gen_expand(double* __restrict__ Xh, const double* __restrict__ X, const long long* __restrict__ crow,
+                             const int32_t* __restrict__ ccol, const double* __restrict__ cs, long long nh, int B)
 {
-    const long long total = nh * B;
-    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
-        const long long r = i / B;
-        const int j = (int)(i - r * B);
-        double v = 0.0;
-        for (long long k = crow[r]; k < crow[r + 1]; ++k) {
-            const int32_t g = ccol[k];
-            const double sg = s[g];
-            if (sg != 0.0) v = fma(cval[k] * sg, X[(long long)g * B + j], v);  // Dirichlet rows of caller data are ignored
+    for (long long r = blockIdx.x * (long long)kGenRows + threadIdx.y; r < nh; r += (long long)gridDim.x * kGenRows) {
+        const long long k0 = crow[r], k1 = crow[r + 1];
+        for (int j = threadIdx.x; j < B; j += 32) {
+            double v0 = 0.0, v1 = 0.0;
+            long long k = k0;
+            for (; k + 1 < k1; k += 2) {
+                const double c0 = cs[k], c1 = cs[k + 1];
+                const double x0 = X[(long long)ccol[k] * B + j], x1 = X[(long long)ccol[k + 1] * B + j];
+                v0 = c0 != 0.0 ? fma(c0, x0, v0) : v0;
+                v1 = c1 != 0.0 ? fma(c1, x1, v1) : v1;
+            }
+            if (k < k1) {
+                const double c0 = cs[k];
+                v0 = c0 != 0.0 ? fma(c0, X[(long long)ccol[k] * B + j], v0) : v0;
+            }
+            Xh[r * B + j] = v0 + v1;
         }
-        Xh[i] = v;
     }
 }
 
-// Y[ccol, j] += alpha s_ccol cval Y_h[r, j]: the transpose of the expansion
-__global__ void k_gen_collapse(double* __restrict__ Y, const double* __restrict__ Yh, const double* __restrict__ s,
-                               const long long* __restrict__ crow, const int32_t* __restrict__ ccol,
-                               const double* __restrict__ cval, long long nh, int B, double alpha)
+// Y[ccol_k, j] += alpha cs_k Y_h[r, j]: the transpose of the expansion
+__global__ void k_gen_collapse(double* __restrict__ Y, const double* __restrict__ Yh, const long long* __restrict__ crow,
+                               const int32_t* __restrict__ ccol, const double* __restrict__ cs, long long nh, int B,
+                               double alpha)
 {
-    const long long total = nh * B;
-    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
-        const long long r = i / B;
-        const int j = (int)(i - r * B);
-        const double y = alpha * Yh[i];
-        for (long long k = crow[r]; k < crow[r + 1]; ++k) {
-            const int32_t g = ccol[k];
-            const double sg = s[g];
-            if (sg != 0.0) atomicAdd(Y + (long long)g * B + j, cval[k] * sg * y);
+    for (long long r = blockIdx.x * (long long)kGenRows + threadIdx.y; r < nh; r += (long long)gridDim.x * kGenRows) {
+        const long long k0 = crow[r], k1 = crow[r + 1];
+        for (int j = threadIdx.x; j < B; j += 32) {
+            const double y = alpha * Yh[r * B + j];
+            for (long long k = k0; k < k1; ++k) {
+                const double c0 = cs[k];
+                if (c0 != 0.0) atomicAdd(Y + (long long)ccol[k] * B + j, c0 * y);
+            }
         }
     }
 }
@@ -163,191 +172,195 @@ constexpr size_t gen_smem_bytes()
            (size_t)n3 * (sizeof(double) + sizeof(int32_t)) + 32;
 }
 
+// line slots of a CTA: every sweep has n^2 lines per vector; ceil(n^2 / 2) slots take them in two rounds
+template <int P>
+struct GenShape {
+    static constexpr int LS = ((P + 1) * (P + 1) + 1) / 2;
+};
+
+// One CTA = one cell x BT vectors.  lane = vector, threadIdx.y = line slot.  Every sweep is a loop over the n^2 lines of
+// one direction (a line = n values, stride sx/sy/sz in the field); the fields live in shared memory, a thread holds one
+// line in registers.  The loops are NOT unrolled over lines, so the whole kernel is a few hundred FP64 instructions per
+// sweep and stays in the instruction cache (the plane-in-registers version of this kernel, 150 KB of straight-line code run
+// by 3.5 warps, spent 4 of 5 issue slots waiting for instructions).
 template <int P, int BT, int MINB>
-__global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_gen(const __grid_constant__ GenParams prm)
+__global__ void __launch_bounds__(GenShape<P>::LS * BT, MINB) k_apply_gen(const __grid_constant__ GenParams prm)
 {
-    constexpr int n = P + 1, n2 = n * n, n3 = n * n * n;
+    constexpr int n = P + 1, n2 = n * n, n3 = n * n * n, LS = GenShape<P>::LS;
+    constexpr int SX = BT, SY = n * BT, SZ = n2 * BT;  // strides of the three directions in a field [z][y][x][BT]
     extern __shared__ __align__(128) double smem[];
-    double* F0 = smem;                  // x -> A -> U -> t -> R
+    double* F0 = smem;                  // x -> A -> U -> t -> T -> R
     double* F1 = F0 + (size_t)n3 * BT;  // gy -> fy
     double* F2 = F1 + (size_t)n3 * BT;  // gz -> fz
-    double* sRec = F2 + (size_t)n3 * BT;  // the cell's record (6 metric fields, WV), one bulk copy in flight during A and B
+    double* sRec = F2 + (size_t)n3 * BT;  // the cell's record (6 metric fields, WV): one bulk copy, in flight until sweep 5
     constexpr int GREC = 7 * n3 + ((7 * n3) & 1);
     double* sSc = sRec + GREC;            // [n^3] gather / scatter scale of the cell's nodes
     unsigned long long* bar = reinterpret_cast<unsigned long long*>(sSc + n3 + (n3 & 1));
     int32_t* sId = reinterpret_cast<int32_t*>(bar + 1);  // [n^3] global ids
-    const int lane = threadIdx.x, pl = threadIdx.y, tid = pl * BT + lane;
+    const int lane = threadIdx.x, slot = threadIdx.y, tid = slot * BT + lane;
     const long long cell = blockIdx.x;
     const int j = blockIdx.y * BT + lane;
     const bool act = j < prm.B;
     const long long B = prm.B;
     double t[n], o[n];
 
-    // ---- gather: ids and scales of the cell, then every thread fetches ITS nodal plane with independent 8-byte cp.async ------
+    // ---- gather: ids and scales of the cell, then 8-byte cp.async of the node rows straight into F0 ----------------------------
     if (tid == 0) {
         mbar_init(bar, 1);
         mbar_expect_tx(bar, (unsigned)(GREC * sizeof(double)));
         bulk_load(sRec, prm.rec + cell * GREC, (unsigned)(GREC * sizeof(double)), bar);
     }
-    for (int a = tid; a < n3; a += n * BT) {
+    for (int a = tid; a < n3; a += LS * BT) {
         sId[a] = prm.l2g[cell * n3 + a];
         sSc[a] = prm.sc[cell * n3 + a];
     }
     __syncthreads();
-#pragma unroll
-    for (int k = 0; k < n2; ++k) {
-        const int a = pl * n2 + k;
+    for (int a = slot; a < n3; a += LS) {
         const long long g = sId[a];
         const double* src = g < prm.N ? prm.X + g * B + j : prm.Xh + (g - prm.N) * B + j;
         cp_async8(F0 + (size_t)a * BT + lane, act ? src : prm.X, act);
     }
     cp_async_commit();
     cp_async_wait_all();
-    // ---- phase A: the nodal plane az = pl: scale, interpolate in x and y (table N) ---------------------------------------------
-    {
-        double v[n][n];
+    __syncthreads();
+    // ---- sweep 1: x-lines (ay, az) of the nodal values: scale (mask, M^-1/2), interpolate (table N) -----------------------------
+#pragma unroll 1
+    for (int l = slot; l < n2; l += LS) {
+        double* f = F0 + (size_t)l * n * BT + lane;
+        const double* sc = sSc + l * n;
 #pragma unroll
-        for (int ay = 0; ay < n; ++ay)
-#pragma unroll
-            for (int ax = 0; ax < n; ++ax) {
-                const int a = pl * n2 + ay * n + ax;
-                const double sg = sSc[a];
-                const double x = F0[(size_t)a * BT + lane];
-                v[ay][ax] = sg != 0.0 ? sg * x : 0.0;  // Dirichlet rows of caller data are ignored (R5)
-            }
-#pragma unroll
-        for (int ay = 0; ay < n; ++ay) {
-            mat1d_eo<n>(prm.eoN, v[ay], o);
-#pragma unroll
-            for (int q = 0; q < n; ++q) v[ay][q] = o[q];
+        for (int k = 0; k < n; ++k) {
+            const double sg = sc[k];
+            t[k] = sg != 0.0 ? sg * f[k * SX] : 0.0;  // Dirichlet rows of caller data are ignored (R5)
         }
+        mat1d_eo<n>(prm.eoN, t, o);
 #pragma unroll
-        for (int qx = 0; qx < n; ++qx) {
-#pragma unroll
-            for (int a = 0; a < n; ++a) t[a] = v[a][qx];
-            mat1d_eo<n>(prm.eoN, t, o);
-#pragma unroll
-            for (int qy = 0; qy < n; ++qy) F0[((size_t)(pl * n + qy) * n + qx) * BT + lane] = o[qy];
-        }
+        for (int k = 0; k < n; ++k) f[k * SX] = o[k];
     }
     __syncthreads();
-    // ---- phase B: the yz-plane qx = pl: U = Nz A (table N), then gz = Dz U along z and gy = Dy U along y (table D) ---------------
-    {
-        double u[n][n];  // [qy][qz]
+    // ---- sweep 2: y-lines (qx, az) (table N) -----------------------------------------------------------------------------------------
+#pragma unroll 1
+    for (int l = slot; l < n2; l += LS) {
+        double* f = F0 + ((size_t)(l / n) * n2 + (l % n)) * BT + lane;
 #pragma unroll
-        for (int qy = 0; qy < n; ++qy) {
+        for (int k = 0; k < n; ++k) t[k] = f[k * SY];
+        mat1d_eo<n>(prm.eoN, t, o);
 #pragma unroll
-            for (int az = 0; az < n; ++az) t[az] = F0[((size_t)(az * n + qy) * n + pl) * BT + lane];
-            mat1d_eo<n>(prm.eoN, t, u[qy]);
-#pragma unroll
-            for (int qz = 0; qz < n; ++qz) F0[((size_t)(qz * n + qy) * n + pl) * BT + lane] = u[qy][qz];
-        }
-#pragma unroll
-        for (int qy = 0; qy < n; ++qy) {
-            mat1d_eoa<n>(prm.eoD, u[qy], o);
-#pragma unroll
-            for (int qz = 0; qz < n; ++qz) F2[((size_t)(qz * n + qy) * n + pl) * BT + lane] = o[qz];
-        }
-#pragma unroll
-        for (int qz = 0; qz < n; ++qz) {
-#pragma unroll
-            for (int qy = 0; qy < n; ++qy) t[qy] = u[qy][qz];
-            mat1d_eoa<n>(prm.eoD, t, o);
-#pragma unroll
-            for (int qy = 0; qy < n; ++qy) F1[((size_t)(qz * n + qy) * n + pl) * BT + lane] = o[qy];
-        }
+        for (int k = 0; k < n; ++k) f[k * SY] = o[k];
     }
     __syncthreads();
-    // ---- phase C: the xy-plane qz = pl, row by row: gx = Dx U (table D), the metric at the points, t = WV U + Dx^T fx (D^T) ------
-    {
-        const size_t base = (size_t)pl * n2;
-        double gx[n][n];
+    // ---- sweep 3: z-lines (qx, qy): U = Nz A (table N), then gz = Dz U on the same lines (table D) -------------------------------------
+#pragma unroll 1
+    for (int l = slot; l < n2; l += LS) {
+        double* f = F0 + (size_t)l * BT + lane;
 #pragma unroll
-        for (int qy = 0; qy < n; ++qy) {
+        for (int k = 0; k < n; ++k) t[k] = f[k * SZ];
+        mat1d_eo<n>(prm.eoN, t, o);
 #pragma unroll
-            for (int qx = 0; qx < n; ++qx) t[qx] = F0[(base + qy * n + qx) * BT + lane];
-            mat1d_eoa<n>(prm.eoD, t, gx[qy]);
-        }
-        mbar_wait(bar, 0);
-        const double* Mq = sRec + pl * n2;  // + c * n3 + qy * n + qx
-        const double* WVq = sRec + 6 * n3 + pl * n2;
+        for (int k = 0; k < n; ++k) f[k * SZ] = o[k];
+    }
+#pragma unroll 1
+    for (int l = slot; l < n2; l += LS) {
+        const size_t off = (size_t)l * BT + lane;
 #pragma unroll
-        for (int qy = 0; qy < n; ++qy)
+        for (int k = 0; k < n; ++k) t[k] = F0[off + k * SZ];
+        mat1d_eoa<n>(prm.eoD, t, o);
 #pragma unroll
-            for (int qx = 0; qx < n; ++qx) {
-                const int q = qy * n + qx;
-                const size_t idx = (base + q) * BT + lane;
-                const double gyv = F1[idx], gzv = F2[idx], gxv = gx[qy][qx];
-                const double g0 = Mq[q], g1 = Mq[n3 + q], g2 = Mq[2 * n3 + q], g3 = Mq[3 * n3 + q], g4 = Mq[4 * n3 + q],
-                             g5 = Mq[5 * n3 + q];
-                gx[qy][qx] = fma(g0, gxv, fma(g1, gyv, g2 * gzv));
-                F1[idx] = fma(g1, gxv, fma(g3, gyv, g4 * gzv));
-                F2[idx] = fma(g2, gxv, fma(g4, gyv, g5 * gzv));
-                F0[idx] *= WVq[q];
-            }
-#pragma unroll
-        for (int qy = 0; qy < n; ++qy) {
-            mat1d_eoa<n>(prm.eoDT, gx[qy], o);
-#pragma unroll
-            for (int qx = 0; qx < n; ++qx) F0[(base + qy * n + qx) * BT + lane] += o[qx];
-        }
+        for (int k = 0; k < n; ++k) F2[off + k * SZ] = o[k];
     }
     __syncthreads();
-    // ---- phase D: the yz-plane qx = pl: T = t + Dz^T fz + Dy^T fy (table D^T), R = Nz^T T (table N^T) -----------------------------
-    {
-        double T[n][n];  // [qy][qz]
+    // ---- sweep 4: y-lines (qx, qz): gy = Dy U (table D) ---------------------------------------------------------------------------------
+#pragma unroll 1
+    for (int l = slot; l < n2; l += LS) {
+        const size_t off = ((size_t)(l / n) * n2 + (l % n)) * BT + lane;
 #pragma unroll
-        for (int qy = 0; qy < n; ++qy) {
+        for (int k = 0; k < n; ++k) t[k] = F0[off + k * SY];
+        mat1d_eoa<n>(prm.eoD, t, o);
 #pragma unroll
-            for (int qz = 0; qz < n; ++qz) t[qz] = F2[((size_t)(qz * n + qy) * n + pl) * BT + lane];
-            mat1d_eoa<n>(prm.eoDT, t, o);
-#pragma unroll
-            for (int qz = 0; qz < n; ++qz) T[qy][qz] = F0[((size_t)(qz * n + qy) * n + pl) * BT + lane] + o[qz];
-        }
-#pragma unroll
-        for (int qz = 0; qz < n; ++qz) {
-#pragma unroll
-            for (int qy = 0; qy < n; ++qy) t[qy] = F1[((size_t)(qz * n + qy) * n + pl) * BT + lane];
-            mat1d_eoa<n>(prm.eoDT, t, o);
-#pragma unroll
-            for (int qy = 0; qy < n; ++qy) T[qy][qz] += o[qy];
-        }
-#pragma unroll
-        for (int qy = 0; qy < n; ++qy) {
-            mat1d_eo<n>(prm.eoNT, T[qy], o);
-#pragma unroll
-            for (int az = 0; az < n; ++az) F0[((size_t)(az * n + qy) * n + pl) * BT + lane] = o[az];
-        }
+        for (int k = 0; k < n; ++k) F1[off + k * SY] = o[k];
     }
     __syncthreads();
-    // ---- phase E: back-interpolate the nodal plane az = pl in y and x (table N^T), scatter through the l2g ---------------------------
-    {
-        double v[n][n];
+    // ---- sweep 5: x-lines (qy, qz): gx = Dx U (table D), the metric at the line's points, t = WV U + Dx^T fx (table D^T) -------------
+    mbar_wait(bar, 0);
+#pragma unroll 1
+    for (int l = slot; l < n2; l += LS) {
+        const size_t off = (size_t)l * n * BT + lane;
+        const double* Mq = sRec + l * n;  // + c * n3 + qx
+        double u[n];
 #pragma unroll
-        for (int qy = 0; qy < n; ++qy)
+        for (int k = 0; k < n; ++k) u[k] = F0[off + k * SX];
+        mat1d_eoa<n>(prm.eoD, u, o);
 #pragma unroll
-            for (int qx = 0; qx < n; ++qx) v[qy][qx] = F0[((size_t)(pl * n + qy) * n + qx) * BT + lane];
-#pragma unroll
-        for (int qx = 0; qx < n; ++qx) {
-#pragma unroll
-            for (int q = 0; q < n; ++q) t[q] = v[q][qx];
-            mat1d_eo<n>(prm.eoNT, t, o);
-#pragma unroll
-            for (int a = 0; a < n; ++a) v[a][qx] = o[a];
+        for (int k = 0; k < n; ++k) {
+            const double gxv = o[k], gyv = F1[off + k * SX], gzv = F2[off + k * SX];
+            const double g0 = Mq[k], g1 = Mq[n3 + k], g2 = Mq[2 * n3 + k], g3 = Mq[3 * n3 + k], g4 = Mq[4 * n3 + k],
+                         g5 = Mq[5 * n3 + k];
+            t[k] = fma(g0, gxv, fma(g1, gyv, g2 * gzv));
+            F1[off + k * SX] = fma(g1, gxv, fma(g3, gyv, g4 * gzv));
+            F2[off + k * SX] = fma(g2, gxv, fma(g4, gyv, g5 * gzv));
         }
+        mat1d_eoa<n>(prm.eoDT, t, o);
 #pragma unroll
-        for (int ay = 0; ay < n; ++ay) {
-            mat1d_eo<n>(prm.eoNT, v[ay], o);
-            if (act) {
+        for (int k = 0; k < n; ++k) F0[off + k * SX] = fma(Mq[6 * n3 + k], u[k], o[k]);
+    }
+    __syncthreads();
+    // ---- sweep 6: y-lines (qx, qz): t += Dy^T fy (table D^T) ------------------------------------------------------------------------------
+#pragma unroll 1
+    for (int l = slot; l < n2; l += LS) {
+        const size_t off = ((size_t)(l / n) * n2 + (l % n)) * BT + lane;
 #pragma unroll
-                for (int ax = 0; ax < n; ++ax) {
-                    const int a = pl * n2 + ay * n + ax;
-                    const long long g = sId[a];
-                    const double sg = sSc[a];
-                    const bool master = g < prm.N;
-                    double* dst = master ? prm.Y + g * B + j : prm.Yh + (g - prm.N) * B + j;
-                    if (sg != 0.0) atomicAdd(dst, master ? prm.alpha * sg * o[ax] : o[ax]);
-                }
+        for (int k = 0; k < n; ++k) t[k] = F1[off + k * SY];
+        mat1d_eoa<n>(prm.eoDT, t, o);
+#pragma unroll
+        for (int k = 0; k < n; ++k) F0[off + k * SY] += o[k];
+    }
+    __syncthreads();
+    // ---- sweep 7: z-lines (qx, qy): T = t + Dz^T fz (table D^T), then R = Nz^T T on the same lines (table N^T) -------------------------
+#pragma unroll 1
+    for (int l = slot; l < n2; l += LS) {
+        const size_t off = (size_t)l * BT + lane;
+#pragma unroll
+        for (int k = 0; k < n; ++k) t[k] = F2[off + k * SZ];
+        mat1d_eoa<n>(prm.eoDT, t, o);
+#pragma unroll
+        for (int k = 0; k < n; ++k) F0[off + k * SZ] += o[k];
+    }
+#pragma unroll 1
+    for (int l = slot; l < n2; l += LS) {
+        double* f = F0 + (size_t)l * BT + lane;
+#pragma unroll
+        for (int k = 0; k < n; ++k) t[k] = f[k * SZ];
+        mat1d_eo<n>(prm.eoNT, t, o);
+#pragma unroll
+        for (int k = 0; k < n; ++k) f[k * SZ] = o[k];
+    }
+    __syncthreads();
+    // ---- sweep 8: y-lines (qx, az) (table N^T) ----------------------------------------------------------------------------------------------
+#pragma unroll 1
+    for (int l = slot; l < n2; l += LS) {
+        double* f = F0 + ((size_t)(l / n) * n2 + (l % n)) * BT + lane;
+#pragma unroll
+        for (int k = 0; k < n; ++k) t[k] = f[k * SY];
+        mat1d_eo<n>(prm.eoNT, t, o);
+#pragma unroll
+        for (int k = 0; k < n; ++k) f[k * SY] = o[k];
+    }
+    __syncthreads();
+    // ---- sweep 9: x-lines (ay, az) (table N^T) and the scatter of the line's n nodes through the l2g -----------------------------------------
+#pragma unroll 1
+    for (int l = slot; l < n2; l += LS) {
+        const double* f = F0 + (size_t)l * n * BT + lane;
+#pragma unroll
+        for (int k = 0; k < n; ++k) t[k] = f[k * SX];
+        mat1d_eo<n>(prm.eoNT, t, o);
+        if (act) {
+#pragma unroll
+            for (int k = 0; k < n; ++k) {
+                const long long g = sId[l * n + k];
+                const double sg = sSc[l * n + k];
+                const bool master = g < prm.N;
+                double* dst = master ? prm.Y + g * B + j : prm.Yh + (g - prm.N) * B + j;
+                if (sg != 0.0) atomicAdd(dst, master ? prm.alpha * sg * o[k] : o[k]);
             }
         }
     }
@@ -356,19 +369,18 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_gen(const __grid_c
 template <int P, int BT, int MINB>
 cudaError_t launch_gen(const GenParams& prm, long long ncells, cudaStream_t st)
 {
-    constexpr int n = P + 1;
     constexpr size_t smem = gen_smem_bytes<P, BT>();
     static PerDeviceOnce once;
     cudaError_t e0 = once_per_device(once, [&] {
         return cudaFuncSetAttribute(k_apply_gen<P, BT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     });
     if (e0 != cudaSuccess) return e0;
-    dim3 grid((unsigned)ncells, (unsigned)((prm.B + BT - 1) / BT)), block(BT, n);
+    dim3 grid((unsigned)ncells, (unsigned)((prm.B + BT - 1) / BT)), block(BT, GenShape<P>::LS);
     k_apply_gen<P, BT, MINB><<<grid, block, smem, st>>>(prm);
     return cudaGetLastError();
 }
 
-// vector-tile width per order: three fields of n^3 x BT doubles per CTA, several CTAs per SM where they fit
+// vector-tile width per order: three fields of n^3 x BT doubles + the cell record per CTA, several CTAs per SM where they fit
 inline cudaError_t launch_apply_gen(const GenParams& prm, int p, long long ncells, cudaStream_t st)
 {
     switch (p) {
@@ -378,7 +390,7 @@ inline cudaError_t launch_apply_gen(const GenParams& prm, int p, long long ncell
         case 4: return launch_gen<4, 32, 2>(prm, ncells, st);
         case 5: return launch_gen<5, 16, 2>(prm, ncells, st);
         case 6: return launch_gen<6, 16, 1>(prm, ncells, st);
-        case 7: return launch_gen<7, 8, 2>(prm, ncells, st);
+        case 7: return launch_gen<7, 8, 1>(prm, ncells, st);
         case 8: return launch_gen<8, 8, 1>(prm, ncells, st);
     }
     return cudaErrorInvalidValue;
