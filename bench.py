@@ -33,8 +33,10 @@ FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE k_apply_tma launch, copied from the committed `ncu --set full`
 # captures named here (profiles/); not measured in this run
 NCU_TRAFFIC = {
-    2: (296.28e6 + 221.12e6, "profiles/r1b_c2_k_apply_tma_full.md"),
-    3: (3.4418e9 + 3.1540e9, "profiles/r1b_c3_k_apply_tma_full.md"),
+    2: (296.26e6 + 219.88e6, "profiles/r2_c2_k_apply_tma_full.md"),
+    3: (3.4587e9 + 3.1621e9, "profiles/r2_c3_k_apply_tma_full.md"),
+    4: (35.660e9 + 31.926e9, "profiles/r2_c4_k_apply_tma_full.md"),
+    5: (296.34e6 + 97.02e6, "profiles/r2_c5_k_apply_tma_full.md (the kernel alone; the zero-fill of Y writes 141 MB more)"),
 }
 
 
@@ -319,12 +321,13 @@ def roofline_block(w, r, ms_step, peaks, hbm_peak):
     dur = ms_step * 1e-3 / r["napply"]
     ach = flops_launch / dur / 1e12
     instr_cv, flops_cv = executed_fp64_per_cell_vector(w.p)
-    peak = (peaks or {}).get("dfma_tflops") or FP64_NOMINAL_TFLOPS
+    peak = max((peaks or {}).get("dfma_tflops") or 0.0, (peaks or {}).get("dmma_tflops") or 0.0) or FP64_NOMINAL_TFLOPS
     ck = r.get("clocks") or {}
     alg_bytes = (24 if w.m > 0 else 16) * r["N"] * r["B"]
     traffic = NCU_TRAFFIC.get(w.index)
     out = {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
-           "peak_source": ("measured in this run: fe_diag_peak kind 0 (register-resident DFMA chains, best launch)"
+           "peak_source": ("measured in this run: the better of fe_diag_peak kind 0 (register-resident DFMA chains) and kind 1 "
+                           "(mma.sync.m8n8k4.f64 chains), best launch -- the two share the FP64 pipe"
                            if (peaks or {}).get("dfma_tflops") else "nominal (no --peaks leg in this run)"),
            "peak_nominal": FP64_NOMINAL_TFLOPS, "frac_of_nominal": ach / FP64_NOMINAL_TFLOPS,
            "frac_kind": "useful work: ALGORITHMIC flops (24 n^4 + 9 n^3 per cell-vector, SURVEY 8(d)) / duration / peak; "
@@ -356,6 +359,56 @@ def measure_peaks(fe, dev):
     out["how"] = ("fe_diag_peak: best launch of >= 0.3 s back to back; DFMA = 8 chains x 8 warps x 4 CTAs/SM; DMMA = "
                   "mma.sync.m8n8k4.f64 chains; stream = y = a x + z on 1 GiB arrays (3 x 8 B per element); reduce-add = "
                   "payload bytes of cp.reduce.async.bulk.add.f64 / red.global.add.f64 into a 1 GiB array")
+    return out
+
+
+def time_adaptive(fe, torch, dev, peaks, hbm_peak, steps, warmup, p=6, B=64, m=30):
+    """NEXT-3 workload (not a BASELINE.json config): config 3's atoms on an adaptively refined mesh with hanging nodes
+    (workloads.adaptive_molecule: 12^3 root cells refined twice around the nuclei), cheb_filter of degree m through the
+    general-cell kernel (fe_general.cuh: explicit l2g, full 3 x 3 metric, 12 sweeps).  The roofline uses the same
+    algorithmic count 24 n^4 + 9 n^3 per cell-vector, which is exactly the 12-sweep form this kernel executes (with even-odd
+    products: fewer instructions, same count)."""
+    mesh, V = workloads.adaptive_molecule()
+    gm = fe.FEMesh.general(mesh, p, device=dev)
+    gm.set_potential(V(gm.quad_coords()))
+    N = gm.N
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(4321)
+    mask = torch.as_tensor(gm.mask().astype(np.float64), device="cuda")[:, None]
+    pristine = torch.randn(N, B, dtype=torch.float64, device="cuda", generator=gen) * mask
+    X = torch.empty_like(pristine)
+    work = torch.empty(2 * N * B, dtype=torch.float64, device="cuda")
+    a0, a, b = -40.0, 20.0, 3.0 * (2.0 * p * p / 0.5) ** 2 * 0.5 + 10.0  # steers values only
+    for _ in range(warmup):
+        X.copy_(pristine)
+        gm.cheb_filter(X, m, a, b, a0, work)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(dev)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    l0 = gm.launches
+    for i in range(steps):
+        X.copy_(pristine)
+        ev[i][0].record()
+        gm.cheb_filter(X, m, a, b, a0, work)
+        ev[i][1].record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = float(sum(e0.elapsed_time(e1) for e0, e1 in ev)) / steps
+    dur = ms * 1e-3 / m
+    n = p + 1
+    flops = algorithmic_flops_per_cell_vector(p) * gm.ncells * B
+    peak = max((peaks or {}).get("dfma_tflops") or 0.0, (peaks or {}).get("dmma_tflops") or 0.0) or FP64_NOMINAL_TFLOPS
+    alg_bytes = 24 * N * B
+    out = {"workload": "adaptive molecule: %d leaves (levels %s) p=%d N=%d unconstrained + %d hanging nodes B=%d m=%d"
+                       % (gm.ncells, np.bincount(mesh.cells[:, 0]).tolist(), p, N, gm.N_all - N, B, m),
+           "value": gm.N_free * B * m / (ms * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": ms,
+           "roofline": {"bound": "alu", "achieved": flops / dur / 1e12, "peak": peak, "unit": "TFLOP/s",
+                        "frac": flops / dur / 1e12 / peak, "frac_of_nominal": flops / dur / 1e12 / FP64_NOMINAL_TFLOPS,
+                        "kernel": "k_apply_gen<p=%d> + k_gen_init / k_gen_expand / k_gen_collapse (one operator step: step / m)" % p,
+                        "launch_ms": dur * 1e3, "algorithmic_bytes": alg_bytes, "traffic": None,
+                        "hbm_frac_of_measured": (alg_bytes / dur / 1e9 / hbm_peak) if hbm_peak else None},
+           "clocks": clocks, "gpu_launches": int(gm.launches - l0)}
+    gm.close()
     return out
 
 
@@ -433,6 +486,7 @@ def main():
     ap.add_argument("--consumers", action="store_true", help="also time Rayleigh-Ritz / Gram / MINRES on config 2's mesh")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-peaks", action="store_true")
+    ap.add_argument("--no-adaptive", action="store_true", help="skip the hanging-node workload (NEXT-3) in `workloads`")
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--stub", action="store_true", help="rank-plumbing self-test on CPU (gloo): no GPU work, fake step times")
     args = ap.parse_args()
@@ -495,6 +549,9 @@ def main():
                                      "filtered_blocks_per_s": world / (ji["ms_per_step"] * 1e-3) if wi.m > 0 else None,
                                      "roofline": roofline_block(wi, ri, ji["ms_per_step"], peaks, hbm_peak),
                                      "clocks": ri["clocks"], "gpu_launches": int(ri["launches"])}
+            torch.cuda.empty_cache()
+        if world == 1 and not args.no_adaptive:
+            others["adaptive_p6"] = time_adaptive(fe, torch, local, peaks, hbm_peak, min(args.steps, 5), 3)
             torch.cuda.empty_cache()
     if rank != 0:
         if dist is not None:
