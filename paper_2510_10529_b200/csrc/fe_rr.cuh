@@ -266,6 +266,196 @@ __global__ void __launch_bounds__(kRRThreads) k_rightmul2(const double* Y, const
     }
 }
 
+// ---- Gram product on the FP64 tensor path: mma.sync.m8n8k4.f64 (DMMA) ------------------------------------------------------
+// C = A^T Bm is a pure contraction over the N rows, so it belongs on DMMA (same peak as DFMA on sm_100a, fe_diag.cuh, but
+// 1/8 of the issue slots and no shared-memory read per FMA): every warp owns 32 x (32 NJ/4) of the BB x BB result, i.e.
+// 4 x NJ accumulator tiles of 8 x 8, and per step of 4 rows loads 4 + NJ fragments for 4 NJ MMAs.  Fragment of the row
+// block [r0, r0+4) and the column block [c0, c0+8): lane t holds M[r0 + t%4][c0 + t/4] for the A and the B operand alike
+// (A^T is the .row operand, Bm the .col operand).  Row pitch BB + 4 doubles makes those reads conflict-free.  BB = 32, 64
+// or 128; 8 warps per CTA split the result tiles and, where there are fewer than 8 tiles, the k steps among them.
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+template <int BB>
+__global__ void __launch_bounds__(256) k_gram_mma(const double* __restrict__ A, const double* __restrict__ Bm,
+                                                  long long N, double* __restrict__ C)
+{
+    constexpr int S = BB + 4, R = BB == 32 ? 64 : 32;  // smem row pitch, rows per stage
+    constexpr int TI = BB / 32;                        // 32-wide blocks of the result per dimension
+    constexpr int NJ = BB == 128 ? 8 : 4;              // 8-wide column tiles per warp (128: two 32-blocks side by side)
+    constexpr int NT = BB == 128 ? 8 : TI * TI;        // warp tiles of the result
+    constexpr int KS = 8 / NT;                         // warps that share a tile split the k steps
+    extern __shared__ __align__(16) double sm[];
+    const bool same = (A == Bm);
+    double* sA = sm;                                // [2][R][S]
+    double* sB = same ? sm : sm + 2 * R * S;        // [2][R][S]
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int tile = warp % NT, kpart = warp / NT;
+    const int i0 = (BB == 128 ? tile / 2 : tile / TI) * 32, j0 = (BB == 128 ? (tile % 2) * 64 : (tile % TI) * 32);
+    const int fr = lane & 3, fc = lane >> 2;
+    double acc[4][NJ][2];
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = 0; b < NJ; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
+    auto stage = [&](double* dst, const double* src, long long r0) {
+        constexpr int chunks = BB / 2;
+        for (int i = threadIdx.x; i < R * chunks; i += 256) {
+            const int r = i / chunks, c = i - r * chunks;
+            const bool ok = r0 + r < N;
+            rr_cp16(dst + r * S + 2 * c, src + (ok ? (r0 + r) * BB + 2 * c : 0), ok);
+        }
+    };
+    const long long ntiles = (N + R - 1) / R;
+    long long t = blockIdx.x;
+    if (t < ntiles) {
+        stage(sA, A, t * R);
+        if (!same) stage(sB, Bm, t * R);
+    }
+    rr_commit();
+    int st = 0;
+    for (; t < ntiles; t += gridDim.x, st ^= 1) {
+        const long long nxt = t + gridDim.x;
+        if (nxt < ntiles) {
+            stage(sA + (st ^ 1) * R * S, A, nxt * R);
+            if (!same) stage(sB + (st ^ 1) * R * S, Bm, nxt * R);
+        }
+        rr_commit();
+        rr_wait<1>();
+        __syncthreads();
+        const double* pa = sA + st * R * S + fr * S + i0 + fc;
+        const double* pb = sB + st * R * S + fr * S + j0 + fc;
+#pragma unroll
+        for (int kk = kpart; kk < R / 4; kk += KS) {
+            double a[4], b[NJ];
+#pragma unroll
+            for (int m = 0; m < 4; ++m) a[m] = pa[kk * 4 * S + 8 * m];
+#pragma unroll
+            for (int q = 0; q < NJ; ++q) b[q] = pb[kk * 4 * S + 8 * q];
+#pragma unroll
+            for (int m = 0; m < 4; ++m)
+#pragma unroll
+                for (int q = 0; q < NJ; ++q) dmma884(acc[m][q][0], acc[m][q][1], a[m], b[q]);
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int m = 0; m < 4; ++m)
+#pragma unroll
+        for (int q = 0; q < NJ; ++q) {
+            double* c = C + (size_t)(i0 + 8 * m + fc) * BB + j0 + 8 * q + 2 * fr;
+            atomicAdd(c, acc[m][q][0]);
+            atomicAdd(c + 1, acc[m][q][1]);
+        }
+}
+
+template <int BB>
+cudaError_t launch_gram_mma(const double* A, const double* Bm, long long N, double* C, int sms, cudaStream_t st)
+{
+    const size_t full = (size_t)4 * (BB == 32 ? 64 : 32) * (BB + 4) * sizeof(double);
+    const size_t smem = A == Bm ? full / 2 : full;
+    static PerDeviceOnce once;
+    cudaError_t e0 = once_per_device(once, [&] {
+        return cudaFuncSetAttribute(k_gram_mma<BB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)full);
+    });
+    if (e0 != cudaSuccess) return e0;
+    k_gram_mma<BB><<<sms * (BB == 128 ? 1 : 2), 256, smem, st>>>(A, Bm, N, C);
+    return cudaGetLastError();
+}
+
+// Out = Y Rm (+ Out) on DMMA: a CTA stages ROWS rows of Y (two-stage ring) and keeps the BB x BB factor in shared memory;
+// the .row operand is the Y tile (lane t holds Y[r0 + t/4][k0 + t%4]), the .col operand the factor (Rm[k0 + t%4][j0 + t/4]),
+// both conflict-free at pitch BB + 4.  Warp tiles: BB = 64: 16 rows x 32 columns (64-row tiles); BB = 128: 8 rows x 64
+// columns (32-row tiles); BB = 32: 8 rows x 32 columns (64-row tiles).  In place is fine: a tile is staged before it is written.
+template <int BB>
+__global__ void __launch_bounds__(256) k_rightmul_mma(const double* Y, const double* __restrict__ Rm, double* Out,
+                                                      int accumulate, long long N)
+{
+    constexpr int S = BB + 4;
+    constexpr int ROWS = BB == 128 ? 32 : 64;
+    constexpr int MI = BB == 64 ? 2 : 1, NJ = BB == 128 ? 8 : 4;       // warp tile = 8 MI rows x 8 NJ columns
+    constexpr int WR = ROWS / (8 * MI);                                 // warps along the rows
+    extern __shared__ __align__(16) double sm[];
+    double* sR = sm;                     // [BB][S]
+    double* sY = sm + (size_t)BB * S;    // [2][ROWS][S]
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int fr = lane & 3, fc = lane >> 2;
+    const int r0w = (warp % WR) * 8 * MI, j0 = (warp / WR) * 8 * NJ;
+    for (int i = threadIdx.x; i < BB * BB; i += 256) sR[(i / BB) * S + (i % BB)] = Rm[i];
+    auto stage = [&](double* dst, long long r0) {
+        constexpr int chunks = BB / 2;
+        for (int i = threadIdx.x; i < ROWS * chunks; i += 256) {
+            const int r = i / chunks, c = i - r * chunks;
+            const bool ok = r0 + r < N;
+            rr_cp16(dst + r * S + 2 * c, Y + (ok ? (r0 + r) * BB + 2 * c : 0), ok);
+        }
+    };
+    const long long ntiles = (N + ROWS - 1) / ROWS;
+    long long t = blockIdx.x;
+    if (t < ntiles) stage(sY, t * ROWS);
+    rr_commit();
+    int st = 0;
+    for (; t < ntiles; t += gridDim.x, st ^= 1) {
+        const long long nxt = t + gridDim.x;
+        if (nxt < ntiles) stage(sY + (st ^ 1) * ROWS * S, nxt * ROWS);
+        rr_commit();
+        rr_wait<1>();
+        __syncthreads();
+        double acc[MI][NJ][2];
+#pragma unroll
+        for (int m = 0; m < MI; ++m)
+#pragma unroll
+            for (int q = 0; q < NJ; ++q) acc[m][q][0] = acc[m][q][1] = 0.0;
+        const double* py = sY + st * ROWS * S + (r0w + fc) * S + fr;
+        const double* pr = sR + fr * S + j0 + fc;
+#pragma unroll 4
+        for (int k = 0; k < BB; k += 4) {
+            double a[MI], b[NJ];
+#pragma unroll
+            for (int m = 0; m < MI; ++m) a[m] = py[8 * m * S + k];
+#pragma unroll
+            for (int q = 0; q < NJ; ++q) b[q] = pr[k * S + 8 * q];
+#pragma unroll
+            for (int m = 0; m < MI; ++m)
+#pragma unroll
+                for (int q = 0; q < NJ; ++q) dmma884(acc[m][q][0], acc[m][q][1], a[m], b[q]);
+        }
+        const long long rg = t * ROWS + r0w + fc;
+#pragma unroll
+        for (int m = 0; m < MI; ++m) {
+            const long long r = rg + 8 * m;
+            if (r < N) {
+#pragma unroll
+                for (int q = 0; q < NJ; ++q) {
+                    double2 o = make_double2(acc[m][q][0], acc[m][q][1]);
+                    double2* dst = reinterpret_cast<double2*>(Out + r * BB + j0 + 8 * q + 2 * fr);
+                    if (accumulate) { const double2 old = *dst; o.x += old.x; o.y += old.y; }
+                    *dst = o;
+                }
+            }
+        }
+        __syncthreads();
+    }
+}
+
+template <int BB>
+cudaError_t launch_rightmul_mma(const double* Y, const double* R, double* Out, int accumulate, long long N, int sms,
+                                cudaStream_t st)
+{
+    constexpr int ROWS = BB == 128 ? 32 : 64;
+    const size_t smem = ((size_t)BB + 2 * ROWS) * (BB + 4) * sizeof(double);
+    static PerDeviceOnce once;
+    cudaError_t e0 = once_per_device(once, [&] {
+        return cudaFuncSetAttribute(k_rightmul_mma<BB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    });
+    if (e0 != cudaSuccess) return e0;
+    k_rightmul_mma<BB><<<sms * (BB == 128 ? 1 : 2), 256, smem, st>>>(Y, R, Out, accumulate, N);
+    return cudaGetLastError();
+}
+
 template <int T>
 cudaError_t launch_gram2(const double* A, const double* Bm, long long N, int B, double* C, int sms, cudaStream_t st)
 {
@@ -292,7 +482,12 @@ inline cudaError_t launch_gram(const double* A, const double* Bm, long long N, i
     const size_t smem = (size_t)2 * kRRRows * B * sizeof(double);
     const int T = (B + 15) / 16;
     if (T > 8) return cudaErrorInvalidValue;
-    if (B % 2 == 0 && (((uintptr_t)A | (uintptr_t)Bm) & 15) == 0) {  // even B, 16-byte aligned rows: the fast path
+    if ((((uintptr_t)A | (uintptr_t)Bm) & 15) == 0) {  // 16-byte aligned rows, B = 32 / 64 / 128: the DMMA kernel
+        if (B == 32) return launch_gram_mma<32>(A, Bm, N, C, sms, st);
+        if (B == 64) return launch_gram_mma<64>(A, Bm, N, C, sms, st);
+        if (B == 128) return launch_gram_mma<128>(A, Bm, N, C, sms, st);
+    }
+    if (B % 2 == 0 && (((uintptr_t)A | (uintptr_t)Bm) & 15) == 0) {  // even B, 16-byte aligned rows: the fast DFMA path
         if (T <= 2) return launch_gram2<2>(A, Bm, N, B, C, sms, st);
         if (T <= 4) return launch_gram2<4>(A, Bm, N, B, C, sms, st);
         if (T <= 6) return launch_gram2<6>(A, Bm, N, B, C, sms, st);
@@ -317,6 +512,11 @@ inline cudaError_t launch_rightmul(const double* Y, const double* R, double* Out
     const size_t smem = ((size_t)B * B + (size_t)kRRRows * (B + 1)) * sizeof(double);
     const int T = (B + 15) / 16;
     if (T > 8) return cudaErrorInvalidValue;
+    if ((((uintptr_t)Y | (uintptr_t)Out) & 15) == 0) {  // B = 32 / 64 / 128: the DMMA kernel
+        if (B == 32) return launch_rightmul_mma<32>(Y, R, Out, accumulate, N, sms, st);
+        if (B == 64) return launch_rightmul_mma<64>(Y, R, Out, accumulate, N, sms, st);
+        if (B == 128) return launch_rightmul_mma<128>(Y, R, Out, accumulate, N, sms, st);
+    }
     if (B % 2 == 0 && (((uintptr_t)Y | (uintptr_t)Out) & 15) == 0) {
         if (T <= 2) return launch_rightmul2<2, 4>(Y, R, Out, accumulate, N, B, sms, st);
         if (T <= 4) return launch_rightmul2<4, 4>(Y, R, Out, accumulate, N, B, sms, st);
