@@ -32,6 +32,7 @@ struct TmaParams {
     CUtensorMap mYp1;  // Y : box (BT,p,p,1), reduce-add of the owner term kappa_j X
     CUtensorMap mWp1;  // W : box (BT,p,p,1), store of beta' X
     const double* eps;
+    double* dots;       // DOTS kernels: dots[j] += sum_g X[g,j] Y_contribution[g,j], the column-wise x . (H~ - eps_j) x of a plain apply
     const double* rec;  // cells * REC: per-cell record  VZ = V_q hz^2/2 [qx][qy][NP] | s_g [az][ay][NP] | kz s_g | ky/kx, kx/kz
     int B, cx, cy, cz;
     int owner, preinit;
@@ -109,11 +110,13 @@ template <int P, int BT>
 constexpr size_t tma_smem_bytes()
 {
     constexpr int n = P + 1;
-    return ((size_t)2 * n * n * n * BT + 2 * TmaShape<n>::REC) * sizeof(double) + 16;
+    return ((size_t)2 * n * n * n * BT + 2 * TmaShape<n>::REC + n * BT) * sizeof(double) + 16;
 }
 
 // FIRST: X is caller data whose Dirichlet rows may hold anything (R5) -> mask them in the owner / pre-init terms.
-template <int P, int BT, int MINB, bool FIRST, bool PERSIST>
+// DOTS: also accumulate the column-wise inner products x_j . y_j of input and result (MINRES alpha, l.221-225) from
+// cell-local terms: x^T y_e = kz U^T T at the Gauss points of the line phase, plus the owner term kappa_j x^2.
+template <int P, int BT, int MINB, bool FIRST, bool PERSIST, bool DOTS = false>
 __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_constant__ TmaParams prm)
 {
     constexpr int n = P + 1, n2 = n * n, n3 = n * n * n, NP = TmaShape<n>::NP, SMALL = TmaShape<n>::SMALL,
@@ -124,6 +127,7 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
     double* rec0 = buf1 + n3 * BT;      // two cell records (double-buffered like the tiles): VZ [qx][qy][NP],
     double* rec1 = rec0 + REC;          //   s_g [az][ay][NP], kz s_g [az][ay][NP], {ky/kx, kx/kz}
     unsigned long long* bar = (unsigned long long*)(rec1 + REC);  // bar[0]: tile + record landed; bar[1]: A consumed
+    double* red = (double*)(bar + 2);   // [n][BT] DOTS: per-plane partial sums of the unit
     const int lane = threadIdx.x, pl = threadIdx.y, tid = pl * BT + lane;
     const int nbt = (prm.B + BT - 1) / BT;
     const long long nunits = (long long)prm.cx * prm.cy * prm.cz * nbt;  // unit = (cell, tile of BT vectors), tile fastest
@@ -168,6 +172,7 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
     const double ry = rec[3 * SMALL], rxz = rec[3 * SMALL + 1];  // ky/kx = hx^2/hy^2, kx/kz = hz^2/hx^2
 
     double v[n][n], t[n], o[n];
+    double dacc = 0.0;  // DOTS: this thread's share of x . y for vector j0 + lane
     double* pA = bufA + (size_t)pl * n2 * BT + lane;
     double* pB = bufB + (size_t)pl * n2 * BT + lane;
     const double* sin_pl = sIn + pl * n * NP;
@@ -187,6 +192,7 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
                     if (FIRST) x = (__double2hiint(sin_pl[ay * NP + ax]) != 0) ? x : 0.0;
                     if (prm.preinit) pA[(ay * P + ax) * BT] = prm.beta_next * x;
                     if (prm.owner) pB[(ay * P + ax) * BT] = kappa * x;
+                    if (DOTS) dacc = fma(kappa * x, x, dacc);
                 }
             fence_async_smem();
         }
@@ -282,6 +288,7 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
             __syncwarp();
             if ((tid & 31) == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar + 1)) : "memory");
         }
+        if constexpr (!DOTS) {
         // pass 2: T = VZ . U + G'z U
 #pragma unroll
         for (int qy = 0; qy < n; ++qy) {
@@ -297,6 +304,33 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
             mat1d_eo<n>(prm.eoN, t, o);
 #pragma unroll
             for (int qz = 0; qz < n; ++qz) v[qy][qz] = fma(rxz, o[qz], v[qy][qz]);
+        }
+        } else {
+        // DOTS: U must still be in v when each part of T meets it, so N'z A2 comes first and is parked in the lines of the A2
+        // field it was read from (this thread's own lines), then T = VZ . U + G'z U + (kx/kz) N'z A2 with U^T T on the way
+        double dq = 0.0, ds = 0.0;
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy) {
+#pragma unroll
+            for (int az = 0; az < n; ++az) t[az] = lb[((az * n + qy) * n) * BT];
+            mat1d_eo<n>(prm.eoN, t, o);
+#pragma unroll
+            for (int qz = 0; qz < n; ++qz) {
+                dq = fma(v[qy][qz], o[qz], dq);
+                lb[((qz * n + qy) * n) * BT] = o[qz];
+            }
+        }
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy) {
+            mat1d_eo<n>(prm.eoG, v[qy], o);
+#pragma unroll
+            for (int qz = 0; qz < n; ++qz) {
+                const double tn = fma(lv[qy * NP + qz], v[qy][qz], o[qz]);
+                ds = fma(v[qy][qz], tn, ds);
+                v[qy][qz] = fma(rxz, lb[((qz * n + qy) * n) * BT], tn);
+            }
+        }
+        dacc = fma(rec[3 * SMALL + 2], fma(rxz, dq, ds), dacc);  // x^T y_e = kz U^T T
         }
         // next-tile request, between passes 3 and 4 (measured: after pass 2 -0.7 %, after pass 4 -8 %: the tile must be
         // in flight for about a third of the unit).  The producer duty sits on warp 3: with 32-wide tiles warps map
@@ -359,6 +393,16 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
             tma_reduce_add4(&prm.mYh1, pB, j0, gx0, gy0, gz0 + pl);
         bulk_commit();
     }
+    if constexpr (DOTS) {
+        red[pl * BT + lane] = dacc;
+        __syncthreads();
+        if (pl == 0 && j0 + lane < prm.B) {
+            double sum = red[lane];
+#pragma unroll
+            for (int k = 1; k < n; ++k) sum += red[k * BT + lane];
+            atomicAdd(prm.dots + j0 + lane, sum);
+        }
+    }
     if (!PERSIST) break;
     double* tmp = rec; rec = recN; recN = tmp;
     }  // units
@@ -386,6 +430,22 @@ cudaError_t launch_tma(const TmaParams& prm, long long ncells, bool first, cudaS
     const long long nunits = ncells * ((prm.B + BT - 1) / BT);
     const bool persist = ctas > 0 && (long long)ctas * MINB < nunits;
     dim3 grid((unsigned)(persist ? (long long)ctas * MINB : nunits)), block(BT, n);
+    if (prm.dots) {  // plain apply on caller data with the column-wise dots: FIRST kernels only
+        if (!first) return cudaErrorInvalidValue;
+        static PerDeviceOnce once_d;
+        cudaError_t ed = once_per_device(once_d, [&] {
+            cudaError_t e = cudaFuncSetAttribute(k_apply_tma<P, BT, MINB, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e == cudaSuccess)
+                e = cudaFuncSetAttribute(k_apply_tma<P, BT, MINB, true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            return e;
+        });
+        if (ed != cudaSuccess) return ed;
+        if (persist)
+            k_apply_tma<P, BT, MINB, true, true, true><<<grid, block, smem, st>>>(prm);
+        else
+            k_apply_tma<P, BT, MINB, true, false, true><<<grid, block, smem, st>>>(prm);
+        return cudaGetLastError();
+    }
     if (persist) {
         if (first)
             k_apply_tma<P, BT, MINB, true, true><<<grid, block, smem, st>>>(prm);
@@ -450,7 +510,7 @@ __global__ void k_build_records(double* __restrict__ rec, int n, int cx, int cy,
         double* r = rec + e * REC;
         r[SMALL + k] = s;
         r[2 * SMALL + k] = kz * s;
-        if (k < 8) r[3 * SMALL + k] = k == 0 ? (hx[ex] * hx[ex]) / (hy[ey] * hy[ey]) : k == 1 ? (hz[ez] * hz[ez]) / (hx[ex] * hx[ex]) : 0.0;
+        if (k < 8) r[3 * SMALL + k] = k == 0 ? (hx[ex] * hx[ex]) / (hy[ey] * hy[ey]) : k == 1 ? (hz[ez] * hz[ez]) / (hx[ex] * hx[ex]) : k == 2 ? kz : 0.0;
     }
 }
 

@@ -64,7 +64,7 @@ struct fe_mesh {
     int variant = 0;
     double* d_minv = nullptr;   // N: MINRES preconditioner, 1 / diag(M^{-1/2} 1/2 K M^{-1/2}) on free rows (built on first use)
     double* d_mask = nullptr;   // N: 1 on free rows, 0 on Dirichlet rows (the unpreconditioned MINRES)
-    double* d_scal = nullptr;   // 17 * 128 doubles + 1 int: MINRES column scalars
+    double* d_scal = nullptr;   // 20 * 128 doubles + 1 int: MINRES column scalars
     double *d_WU = nullptr, *d_VZU = nullptr;  // fe_apply_potential: J w U of the caller's field (+ unused record output)
     double* d_host = nullptr;   // device staging of cheb_filter_host (grown on demand)
     size_t host_cap = 0;
@@ -605,10 +605,12 @@ static void fill_tma_params(const fe_mesh* m, TmaParams* prm, int B)
 
 // Y += alpha s sum_e yhat_e(X) + kappa X (owner),  W = beta_next X (pre-initialisation of the next target), one launch
 static int tma_step(fe_mesh* m, const BlockMaps& X, const BlockMaps& Y, const BlockMaps* W, int B, const double* eps,
-                    double alpha, double c, bool owner, double beta_next, bool first, cudaStream_t st)
+                    double alpha, double c, bool owner, double beta_next, bool first, cudaStream_t st,
+                    double* dots = nullptr)
 {
     TmaParams prm;
     fill_tma_params(m, &prm, B);
+    prm.dots = dots;
     prm.mXn = X.n3; prm.mYh1 = Y.h1; prm.mYh2 = Y.h2; prm.mYp1 = Y.p1; prm.mWp1 = W ? W->p1 : Y.p1;
     prm.eps = eps; prm.alpha = alpha; prm.c = c; prm.owner = owner ? 1 : 0;
     prm.preinit = W ? 1 : 0; prm.beta_next = beta_next;
@@ -672,13 +674,24 @@ int fe_apply_H(fe_mesh* m, const double* X, double* Y, int B, const double* eps_
 
 // fe_apply_H into a block the caller has already cleared (the library's own loops let the elementwise kernel that reads a
 // block last also clear it, so the separate zero-fill pass disappears); falls back to fe_apply_H when the TMA path is not taken
-static int apply_into_cleared(fe_mesh* m, const double* X, double* Y, int B, const double* eps_dev, void* cuda_stream)
+// dots_dev (B doubles, zero on entry) receives the column-wise x_j . y_j: from the operator kernel itself on the TMA path
+// (cell-local terms, fe_apply_tma.cuh DOTS), from one extra pass otherwise
+static int apply_into_cleared(fe_mesh* m, const double* X, double* Y, int B, const double* eps_dev, double* dots_dev,
+                              void* cuda_stream)
 {
-    if (!tma_eligible(m, B, X, Y, eps_dev)) return fe_apply_H(m, X, Y, B, eps_dev, cuda_stream);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (!tma_eligible(m, B, X, Y, eps_dev)) {
+        int rc = fe_apply_H(m, X, Y, B, eps_dev, cuda_stream);
+        if (rc || !dots_dev) return rc;
+        k_col_dot<<<m->sms * 8, dim3(kMRx, kMRy), 0, st>>>(X, Y, m->N, B, dots_dev);
+        CUDA_TRY(cudaGetLastError());
+        m->launches += 1;
+        return FE_OK;
+    }
     BlockMaps mx, my;
     int rc;
     if ((rc = make_block_maps(&mx, m, X, B)) || (rc = make_block_maps(&my, m, Y, B))) return rc;
-    return tma_step(m, mx, my, nullptr, B, eps_dev, 1.0, 0.0, eps_dev != nullptr, 0.0, true, (cudaStream_t)cuda_stream);
+    return tma_step(m, mx, my, nullptr, B, eps_dev, 1.0, 0.0, eps_dev != nullptr, 0.0, true, st, dots_dev);
 }
 
 int cheb_filter(fe_mesh* m, double* X, int B, int deg, double a, double b, double a0, double* work, void* cuda_stream)
@@ -960,7 +973,7 @@ static int ensure_minres_tables(fe_mesh* m)
     cudaError_t ce = cudaSuccess;
     if (!rc) ce = cudaMalloc((void**)&m->d_minv, (size_t)m->N * sizeof(double));
     if (!rc && ce == cudaSuccess) ce = cudaMalloc((void**)&m->d_mask, (size_t)m->N * sizeof(double));
-    if (!rc && ce == cudaSuccess) ce = cudaMalloc((void**)&m->d_scal, (17 * 128 + 2) * sizeof(double));
+    if (!rc && ce == cudaSuccess) ce = cudaMalloc((void**)&m->d_scal, (20 * 128 + 2) * sizeof(double));
     if (!rc && ce == cudaSuccess) {
         k_build_precond<<<m->sms * 8, 256>>>(m->d_minv, m->Nx, m->Ny, m->Nz, d[0], d[1], d[2], d[3], d[4], d[5], m->d_sx, m->d_sy, m->d_sz);
         k_build_scaling<<<m->sms * 8, 256>>>(m->d_sx, m->d_sy, m->d_sz, m->Nx, m->Ny, m->Nz, m->d_mask);
@@ -994,9 +1007,9 @@ int fe_minres_shifted(fe_mesh* m, const double* G, double* X, int B, const doubl
     MinresScalars q;
     double* s = m->d_scal;
     double** f[] = {&q.beta, &q.oldb, &q.alfa, &q.betasq, &q.dbar, &q.epsln, &q.oldeps, &q.phibar, &q.cs, &q.sn,
-                    &q.gamma, &q.delta, &q.phi, &q.beta1, &q.s, &q.c1, &q.c2};
-    for (int i = 0; i < 17; ++i) *f[i] = s + (size_t)i * 128;
-    q.itn = (int*)(s + 17 * 128);
+                    &q.gamma, &q.delta, &q.phi, &q.beta1, &q.s, &q.c1, &q.c2, &q.dot, &q.gam, &q.gamn};
+    for (int i = 0; i < 20; ++i) *f[i] = s + (size_t)i * 128;
+    q.itn = (int*)(s + 20 * 128);
     const int grid = m->sms * 8;
     const dim3 blk(kMRx, kMRy);
     CUDA_TRY(cudaMemsetAsync(q.betasq, 0, 128 * sizeof(double), st));
@@ -1009,9 +1022,10 @@ int fe_minres_shifted(fe_mesh* m, const double* G, double* X, int B, const doubl
     bool done = false;
     while (it < maxit && !done) {
         k_minres_scalars<<<1, 128, 0, st>>>(q, B, 1, tol);
-        if ((rc = apply_into_cleared(m, Y, HY, B, eps_dev, cuda_stream))) return rc;  // hy = (H~ - eps_j) y,  y = beta v
-        k_minres_alfa<<<grid, blk, 0, st>>>(Y, HY, R1, m->N, B, q.s, q.c1, q.alfa);
-        k_minres_beta<<<grid, blk, 0, st>>>(HY, R1, R2, Minv, m->N, B, q.alfa, q.beta, q.betasq);
+        // hy = (H~ - eps_j) y,  y = beta v, with dot_j = y_j . hy_j from the operator kernel
+        if ((rc = apply_into_cleared(m, Y, HY, B, eps_dev, q.dot, cuda_stream))) return rc;
+        k_minres_scalars<<<1, 128, 0, st>>>(q, B, 3, tol);
+        k_minres_lanczos<<<grid, blk, 0, st>>>(HY, R1, R2, Minv, m->N, B, q.s, q.c1, q.c2, q.betasq, q.gamn);
         k_minres_scalars<<<1, 128, 0, st>>>(q, B, 2, tol);
         k_minres_update<<<grid, blk, 0, st>>>(Y, W1, W2, X, m->N, B, q.s, q.oldeps, q.delta, q.gamma, q.phi);
         CUDA_TRY(cudaGetLastError());

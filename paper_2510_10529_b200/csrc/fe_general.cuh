@@ -389,7 +389,7 @@ inline cudaError_t launch_apply_gen(const GenParams& prm, int p, long long ncell
         case 3: return launch_gen<3, 32, 4>(prm, ncells, st);
         case 4: return launch_gen<4, 32, 2>(prm, ncells, st);
         case 5: return launch_gen<5, 16, 2>(prm, ncells, st);
-        case 6: return launch_gen<6, 16, 1>(prm, ncells, st);
+        case 6: return launch_gen<6, 8, 2>(prm, ncells, st);
         case 7: return launch_gen<7, 8, 1>(prm, ncells, st);
         case 8: return launch_gen<8, 8, 1>(prm, ncells, st);
     }

@@ -2,10 +2,12 @@
 //
 // Every column j solves its own system (H~ - eps_j I) p_j = g_j with its own Paige-Saunders recurrences; the
 // columns advance in lock-step so that each Krylov step is ONE fused fe_apply_H launch for the whole block.  The
-// vector updates of a step are three fused elementwise kernels (the normalised Lanczos vector v = y / beta is never
-// stored: the apply runs on y and the scale is folded into what follows) that also produce the column-wise inner
-// products (alfa_j = v_j.y_j, beta_j^2 = r_j.M^{-1} r_j); the Givens / Lanczos scalars live in device arrays of length B
-// and are advanced by a one-warp-per-block kernel, so an iteration needs no host synchronisation.
+// normalised Lanczos vector v = y / beta is never stored: the apply runs on y and the scale is folded into what follows.
+// The operator kernel itself delivers the column-wise dots y_j . (H~ - eps_j) y_j from cell-local terms (fe_apply_tma.cuh,
+// DOTS), so alfa_j is known right after the apply and the two Lanczos vector updates are ONE elementwise pass
+// (k_minres_lanczos: also beta_j^2 = r_j . M^{-1} r_j and the y . r1 of the next step); a second pass updates w and x and
+// clears the next apply target.  The Givens / Lanczos scalars live in device arrays of length B and are advanced by a
+// one-block kernel, so an iteration needs no host synchronisation.
 // Preconditioner (l.225): inverse diagonal of the mass-scaled negative Laplacian, positive on free rows.
 #pragma once
 #include <cuda_runtime.h>
@@ -15,6 +17,7 @@ namespace fecheb {
 struct MinresScalars {  // B doubles each, device
     double *beta, *oldb, *alfa, *betasq, *dbar, *epsln, *oldeps, *phibar, *cs, *sn, *gamma, *delta, *phi, *beta1;
     double *s, *c1, *c2;  // 1/beta, beta/oldb, alfa/beta of the running step
+    double *dot, *gam, *gamn;  // y.(H~-eps)y from the operator kernel; y.r1 of this step and of the next
     int* itn;
 };
 
@@ -63,33 +66,28 @@ __global__ void k_minres_init(const double* __restrict__ G, const double* __rest
     block_col_reduce(acc, B, betasq);
 }
 
-// phase B:  the apply ran on the un-normalised y (= beta v):  hy = (H~ - eps) y.  Here  y' = s_j hy - c1_j r1  and
-// alfa_j = v_j . y'_j  with  v = s_j y  formed on the fly (v is never stored); y' overwrites hy.
-__global__ void k_minres_alfa(const double* __restrict__ Yold, double* __restrict__ HY, const double* __restrict__ R1,
-                              long long N, int B, const double* __restrict__ s, const double* __restrict__ c1, double* alfa)
+// column-wise x . y of two blocks (the fallback when the operator kernel cannot deliver the dots itself)
+__global__ void k_col_dot(const double* __restrict__ X, const double* __restrict__ Y, long long N, int B, double* out)
 {
     double acc[kMaxColTiles] = {0, 0, 0, 0};
     for (long long r = blockIdx.x * (long long)kMRy + threadIdx.y; r < N; r += (long long)gridDim.x * kMRy)
 #pragma unroll
         for (int t = 0; t < kMaxColTiles; ++t) {
             const int j = t * kMRx + threadIdx.x;
-            if (j < B) {
-                const long long i = r * B + j;
-                const double sj = s[j];
-                const double y = fma(sj, HY[i], -c1[j] * R1[i]);
-                HY[i] = y;
-                acc[t] = fma(sj * Yold[i], y, acc[t]);
-            }
+            if (j < B) acc[t] = fma(X[r * B + j], Y[r * B + j], acc[t]);
         }
-    block_col_reduce(acc, B, alfa);
+    block_col_reduce(acc, B, out);
 }
 
-// phase C:  t = y - c2_j r2 ;  r1 <- t (the host swaps r1/r2 afterwards) ;  y <- Minv t ;  betasq_j = t_j . y_j
-__global__ void k_minres_beta(double* __restrict__ Y, double* __restrict__ R1, const double* __restrict__ R2,
-                              const double* __restrict__ Minv, long long N, int B, const double* __restrict__ alfa,
-                              const double* __restrict__ beta, double* betasq)
+// phases B + C in one pass.  The apply ran on the un-normalised y (= beta v): hy = (H~ - eps) y, and alfa_j = v_j . y'_j with
+// y' = s_j hy - c1_j r1 is already known from the dots of the operator kernel (k_minres_scalars stage 3), so
+//   t = s_j hy - c1_j r1 - c2_j r2 ;  r1 <- t (the host swaps r1 / r2 afterwards) ;  y_next = Minv t (into hy's block) ;
+//   betasq_j = t_j . y_next,j ;  gamn_j = y_next,j . r2_j  (the y . r1 of the NEXT step, whose r1 is this r2)
+__global__ void k_minres_lanczos(double* __restrict__ HY, double* __restrict__ R1, const double* __restrict__ R2,
+                                 const double* __restrict__ Minv, long long N, int B, const double* __restrict__ s,
+                                 const double* __restrict__ c1, const double* __restrict__ c2, double* betasq, double* gamn)
 {
-    double acc[kMaxColTiles] = {0, 0, 0, 0};
+    double acc[kMaxColTiles] = {0, 0, 0, 0}, acg[kMaxColTiles] = {0, 0, 0, 0};
     for (long long r = blockIdx.x * (long long)kMRy + threadIdx.y; r < N; r += (long long)gridDim.x * kMRy) {
         const double mi = Minv[r];
 #pragma unroll
@@ -97,16 +95,19 @@ __global__ void k_minres_beta(double* __restrict__ Y, double* __restrict__ R1, c
             const int j = t * kMRx + threadIdx.x;
             if (j < B) {
                 const long long i = r * B + j;
-                const double c2 = beta[j] > 0.0 ? alfa[j] / beta[j] : 0.0;
-                const double tt = fma(-c2, R2[i], Y[i]);
+                const double r2 = R2[i];
+                const double yp = fma(s[j], HY[i], -c1[j] * R1[i]);
+                const double tt = fma(-c2[j], r2, yp);
                 const double y = mi * tt;
                 R1[i] = tt;
-                Y[i] = y;
+                HY[i] = y;
                 acc[t] = fma(tt, y, acc[t]);
+                acg[t] = fma(y, r2, acg[t]);
             }
         }
     }
     block_col_reduce(acc, B, betasq);
+    block_col_reduce(acg, B, gamn);
 }
 
 // phase D:  w_new = (v - oldeps_j w1 - delta_j w2) / gamma_j  (into w1's storage), v = s_j y_old ;  x += phi_j w_new.
@@ -131,8 +132,8 @@ __global__ void k_minres_update(double* __restrict__ Yold, double* __restrict__ 
         }
 }
 
-// scalar recurrences, one thread per column.  stage 0: after init (beta1); stage 1: before the step (s, c1);
-// stage 2: after phase C (Lanczos beta, Givens rotation, phi)
+// scalar recurrences, one thread per column.  stage 0: after init (beta1); stage 1: before the step (s, c1); stage 3: after
+// the apply (alfa, c2 from the operator kernel's dots); stage 2: after the Lanczos pass (beta, Givens rotation, phi)
 __global__ void k_minres_scalars(MinresScalars q, int B, int stage, double tol)
 {
     const int j = blockIdx.x * blockDim.x + threadIdx.x;
@@ -140,7 +141,7 @@ __global__ void k_minres_scalars(MinresScalars q, int B, int stage, double tol)
     if (stage == 0) {
         const double b1 = sqrt(fmax(q.betasq[j], 0.0));
         q.beta1[j] = b1; q.beta[j] = b1; q.oldb[j] = 0.0; q.dbar[j] = 0.0; q.epsln[j] = 0.0; q.phibar[j] = b1;
-        q.cs[j] = -1.0; q.sn[j] = 0.0; q.betasq[j] = 0.0; q.alfa[j] = 0.0;
+        q.cs[j] = -1.0; q.sn[j] = 0.0; q.betasq[j] = 0.0; q.alfa[j] = 0.0; q.gam[j] = 0.0; q.gamn[j] = 0.0; q.dot[j] = 0.0;
         q.gamma[j] = 1.0; q.delta[j] = 0.0; q.oldeps[j] = 0.0; q.phi[j] = 0.0;
         if (j == 0) *q.itn = 0;
     } else if (stage == 1) {
@@ -150,8 +151,16 @@ __global__ void k_minres_scalars(MinresScalars q, int B, int stage, double tol)
         q.c1[j] = (live && oldb > 0.0) ? beta / oldb : 0.0;
         q.alfa[j] = 0.0;
         q.betasq[j] = 0.0;
+        q.dot[j] = 0.0;
+        q.gamn[j] = 0.0;
+    } else if (stage == 3) {  // after the apply: alfa = v . (s hy - c1 r1) = s^2 (y . hy) - c1 s (y . r1);  c2 = alfa / beta
+        const double sj = q.s[j];
+        const double alfa = sj * sj * q.dot[j] - q.c1[j] * sj * q.gam[j];
+        q.alfa[j] = alfa;
+        q.c2[j] = q.beta[j] > 0.0 ? alfa / q.beta[j] : 0.0;
     } else {
         const bool live = q.s[j] != 0.0;
+        q.gam[j] = q.gamn[j];
         const double alfa = q.alfa[j], oldb = q.beta[j];
         const double beta = sqrt(fmax(q.betasq[j], 0.0));
         if (!live) { q.phi[j] = 0.0; q.gamma[j] = 1.0; q.delta[j] = 0.0; q.oldeps[j] = 0.0; return; }
