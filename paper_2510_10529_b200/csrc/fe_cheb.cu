@@ -79,6 +79,10 @@ struct fe_mesh {
     long long* d_crow = nullptr;
     int32_t* d_ccol = nullptr;
     double* d_cval = nullptr;  // constraint weight times s of its unconstrained node (fe_general.cuh: cs)
+    long long* d_trow = nullptr;  // the same rows transposed: for every unconstrained node with hanging dependents ...
+    int32_t *d_tcol = nullptr, *d_tid = nullptr;  // ... the hanging rows (index r = h - N) that use it, and its own id
+    double* d_tval = nullptr;
+    long long nt = 0;
     double *d_Xh = nullptr, *d_Yh = nullptr;  // (N_all - N) * hcap: expanded hanging values / their scatter target
     int hcap = 0;
     int sms = 0;  // multiprocessors of the device (persistent grid size)
@@ -216,6 +220,7 @@ int fe_mesh_destroy(fe_mesh* m)
     cudaFree(m->d_VZ); cudaFree(m->d_sx); cudaFree(m->d_sy); cudaFree(m->d_sz);
     cudaFree(m->d_gl2g); cudaFree(m->d_gmetric); cudaFree(m->d_gwdet); cudaFree(m->d_gsc); cudaFree(m->d_crow);
     cudaFree(m->d_ccol); cudaFree(m->d_cval); cudaFree(m->d_Xh); cudaFree(m->d_Yh);
+    cudaFree(m->d_trow); cudaFree(m->d_tcol); cudaFree(m->d_tid); cudaFree(m->d_tval);
     delete m->gh;
     delete m;
     return FE_OK;
@@ -468,8 +473,36 @@ int fe_mesh_create_general(int cx, int cy, int cz, const int32_t* cells, int64_t
         if (n % 2 == 1)
             for (int k = 0; k < h; ++k) { m->eoD.S[h * h + k] = m->tab.D[h * n + k]; m->eoDT.S[h * h + k] = Dt[h * n + k]; }
     }
+    // transposed constraint rows (collapse without atomics): entries sorted by unconstrained node, then by hanging row
+    std::vector<long long> trow;
+    std::vector<int32_t> tcol, tid;
+    std::vector<double> tval;
+    {
+        const int64_t nh = g.N_all - g.N;
+        std::vector<int64_t> cnt((size_t)g.N + 1, 0);
+        for (int32_t c : g.ccol) cnt[(size_t)c + 1] += 1;
+        for (int64_t i = 0; i < g.N; ++i) cnt[i + 1] += cnt[i];
+        std::vector<int64_t> pos(cnt.begin(), cnt.end() - 1);
+        std::vector<int32_t> hc(g.ccol.size());
+        std::vector<double> hv(g.ccol.size());
+        for (int64_t r = 0; r < nh; ++r)
+            for (int64_t k = g.crow[r]; k < g.crow[r + 1]; ++k) {
+                const int64_t q = pos[g.ccol[k]]++;
+                hc[q] = (int32_t)r;
+                hv[q] = csv[k];
+            }
+        trow.push_back(0);
+        for (int64_t i = 0; i < g.N; ++i)
+            if (cnt[i + 1] > cnt[i]) {
+                tid.push_back((int32_t)i);
+                for (int64_t q = cnt[i]; q < cnt[i + 1]; ++q) { tcol.push_back(hc[q]); tval.push_back(hv[q]); }
+                trow.push_back((long long)tcol.size());
+            }
+        m->nt = (long long)tid.size();
+    }
     int rc;
-    if ((rc = upload_vec(&m->d_gsc, scv)) || (rc = upload_vec(&m->d_sm, sv)) || (rc = upload_vec(&m->d_gl2g, g.l2g)) || (rc = upload_vec(&m->d_gmetric, met)) ||
+    if ((rc = upload_vec(&m->d_trow, trow)) || (rc = upload_vec(&m->d_tcol, tcol)) || (rc = upload_vec(&m->d_tid, tid)) ||
+        (rc = upload_vec(&m->d_tval, tval)) || (rc = upload_vec(&m->d_gsc, scv)) || (rc = upload_vec(&m->d_sm, sv)) || (rc = upload_vec(&m->d_gl2g, g.l2g)) || (rc = upload_vec(&m->d_gmetric, met)) ||
         (rc = upload_vec(&m->d_gwdet, wdet)) || (rc = upload_vec(&m->d_crow, crow)) || (rc = upload_vec(&m->d_ccol, g.ccol)) ||
         (rc = upload_vec(&m->d_cval, csv))) {
         fe_mesh_destroy(m);
@@ -515,7 +548,7 @@ static int general_step(fe_mesh* m, const double* X, const double* Z, double* Y,
         k_gen_init<<<grid, rows, 0, st>>>(Y, X, Z, m->d_sm, eps, alpha, beta, c, g.N, B);
     if (nh > 0) {
         CUDA_TRY(cudaMemsetAsync(m->d_Yh, 0, (size_t)nh * B * sizeof(double), st));
-        k_gen_expand<<<grid, rows, 0, st>>>(m->d_Xh, X, m->d_crow, m->d_ccol, m->d_cval, nh, B);
+        k_gen_rows_times_block<<<grid, rows, 0, st>>>(m->d_Xh, X, m->d_crow, m->d_ccol, m->d_cval, nullptr, nh, B, 1.0, 0);
     }
     GenParams prm;
     memset(&prm, 0, sizeof(prm));
@@ -524,7 +557,8 @@ static int general_step(fe_mesh* m, const double* X, const double* Z, double* Y,
     prm.eoN = m->eoN; prm.eoNT = m->eoNT; prm.eoD = m->eoD; prm.eoDT = m->eoDT;
     cudaError_t e = launch_apply_gen(prm, m->p, m->ncells, st);
     if (e != cudaSuccess) return fail(FE_ERR_CUDA, "operator launch (general mesh) failed: %s", cudaGetErrorString(e));
-    if (nh > 0) k_gen_collapse<<<grid, rows, 0, st>>>(Y, m->d_Yh, m->d_crow, m->d_ccol, m->d_cval, nh, B, alpha);
+    if (nh > 0)
+        k_gen_rows_times_block<<<grid, rows, 0, st>>>(Y, m->d_Yh, m->d_trow, m->d_tcol, m->d_tval, m->d_tid, m->nt, B, alpha, 1);
     CUDA_TRY(cudaGetLastError());
     m->launches += nh > 0 ? 4 : 2;
     return FE_OK;

@@ -69,44 +69,38 @@ __global__ void k_gen_init(double* __restrict__ Y, const double* __restrict__ X,
     }
 }
 
-// X_h[r, j] = sum_k cs_k X[ccol_k, j], cs = cval * s[ccol] (0 on Dirichlet rows, whose caller data is ignored): values of the
-// hanging nodes (rows r of the constraint matrix applied to s . X)
-__global__ void k_gen_expand(double* __restrict__ Xh, const double* __restrict__ X, const long long* __restrict__ crow,
-                             const int32_t* __restrict__ ccol, const double* __restrict__ cs, long long nh, int B)
+// Sparse rows times a block:  dst[row(r), j] (+)= alpha sum_k cs_k src[ccol_k, j]  for r < nr, row(r) = rows ? rows[r] : r.
+//   expansion  X_h = C_h (s . X):        src = X,   dst = X_h, cs = cval * s[ccol] (0 on Dirichlet rows, whose data is ignored)
+//   collapse   Y += alpha s . C_h^T Y_h:  src = Y_h, dst = Y, rows = the unconstrained nodes that have hanging dependents,
+//                                          the TRANSPOSED constraint rows (no atomics: every dst row has one owner)
+// A warp works on one row (lanes = vectors); the loop over the row's entries is latency-bound (index, then the row of src),
+// so eight entries are in flight per thread and the kernel is capped at 32 registers for 64 warps per SM.
+__global__ void __launch_bounds__(32 * kGenRows, 8)
+k_gen_rows_times_block(double* __restrict__ dst, const double* __restrict__ src, const long long* __restrict__ crow,
+                       const int32_t* __restrict__ ccol, const double* __restrict__ cs, const int32_t* __restrict__ rows,
+                       long long nr, int B, double alpha, int accumulate)
 {
-    for (long long r = blockIdx.x * (long long)kGenRows + threadIdx.y; r < nh; r += (long long)gridDim.x * kGenRows) {
+    for (long long r = blockIdx.x * (long long)kGenRows + threadIdx.y; r < nr; r += (long long)gridDim.x * kGenRows) {
         const long long k0 = crow[r], k1 = crow[r + 1];
+        const long long out = rows ? rows[r] : r;
         for (int j = threadIdx.x; j < B; j += 32) {
-            double v0 = 0.0, v1 = 0.0;
+            double v = 0.0;
             long long k = k0;
-            for (; k + 1 < k1; k += 2) {
-                const double c0 = cs[k], c1 = cs[k + 1];
-                const double x0 = X[(long long)ccol[k] * B + j], x1 = X[(long long)ccol[k + 1] * B + j];
-                v0 = c0 != 0.0 ? fma(c0, x0, v0) : v0;
-                v1 = c1 != 0.0 ? fma(c1, x1, v1) : v1;
+            for (; k + 8 <= k1; k += 8) {
+                double c[8], x[8];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) c[u] = cs[k + u];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) x[u] = src[(long long)ccol[k + u] * B + j];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) v = c[u] != 0.0 ? fma(c[u], x[u], v) : v;
             }
-            if (k < k1) {
+            for (; k < k1; ++k) {
                 const double c0 = cs[k];
-                v0 = c0 != 0.0 ? fma(c0, X[(long long)ccol[k] * B + j], v0) : v0;
+                v = c0 != 0.0 ? fma(c0, src[(long long)ccol[k] * B + j], v) : v;
             }
-            Xh[r * B + j] = v0 + v1;
-        }
-    }
-}
-
-// Y[ccol_k, j] += alpha cs_k Y_h[r, j]: the transpose of the expansion
-__global__ void k_gen_collapse(double* __restrict__ Y, const double* __restrict__ Yh, const long long* __restrict__ crow,
-                               const int32_t* __restrict__ ccol, const double* __restrict__ cs, long long nh, int B,
-                               double alpha)
-{
-    for (long long r = blockIdx.x * (long long)kGenRows + threadIdx.y; r < nh; r += (long long)gridDim.x * kGenRows) {
-        const long long k0 = crow[r], k1 = crow[r + 1];
-        for (int j = threadIdx.x; j < B; j += 32) {
-            const double y = alpha * Yh[r * B + j];
-            for (long long k = k0; k < k1; ++k) {
-                const double c0 = cs[k];
-                if (c0 != 0.0) atomicAdd(Y + (long long)ccol[k] * B + j, c0 * y);
-            }
+            double* d = dst + out * B + j;
+            *d = accumulate ? fma(alpha, v, *d) : alpha * v;
         }
     }
 }
@@ -203,6 +197,17 @@ __global__ void __launch_bounds__(GenShape<P>::LS * BT, MINB) k_apply_gen(const 
     const bool act = j < prm.B;
     const long long B = prm.B;
     double t[n], o[n];
+    // the (at most) two lines of this slot in every sweep, as field offsets: x-lines (i1, i2), y-lines (i0, i2), z-lines (i0, i1)
+    const bool two = slot + LS < n2;
+    int lx[2], ly[2], lz[2], ll[2];
+#pragma unroll
+    for (int r = 0; r < 2; ++r) {
+        const int l = (r == 0 || two) ? slot + r * LS : slot;
+        ll[r] = l;
+        lx[r] = l * n * BT + lane;
+        ly[r] = ((l / n) * n2 + (l % n)) * BT + lane;
+        lz[r] = l * BT + lane;
+    }
 
     // ---- gather: ids and scales of the cell, then 8-byte cp.async of the node rows straight into F0 ----------------------------
     if (tid == 0) {
@@ -224,9 +229,10 @@ __global__ void __launch_bounds__(GenShape<P>::LS * BT, MINB) k_apply_gen(const 
     cp_async_wait_all();
     __syncthreads();
     // ---- sweep 1: x-lines (ay, az) of the nodal values: scale (mask, M^-1/2), interpolate (table N) -----------------------------
-#pragma unroll 1
-    for (int l = slot; l < n2; l += LS) {
-        double* f = F0 + (size_t)l * n * BT + lane;
+#pragma unroll
+    for (int r = 0; r < 2; ++r) if (r == 0 || two) {
+        const int l = ll[r];
+        double* f = F0 + lx[r];
         const double* sc = sSc + l * n;
 #pragma unroll
         for (int k = 0; k < n; ++k) {
@@ -239,9 +245,10 @@ __global__ void __launch_bounds__(GenShape<P>::LS * BT, MINB) k_apply_gen(const 
     }
     __syncthreads();
     // ---- sweep 2: y-lines (qx, az) (table N) -----------------------------------------------------------------------------------------
-#pragma unroll 1
-    for (int l = slot; l < n2; l += LS) {
-        double* f = F0 + ((size_t)(l / n) * n2 + (l % n)) * BT + lane;
+#pragma unroll
+    for (int r = 0; r < 2; ++r) if (r == 0 || two) {
+        const int l = ll[r];
+        double* f = F0 + ly[r];
 #pragma unroll
         for (int k = 0; k < n; ++k) t[k] = f[k * SY];
         mat1d_eo<n>(prm.eoN, t, o);
@@ -250,18 +257,20 @@ __global__ void __launch_bounds__(GenShape<P>::LS * BT, MINB) k_apply_gen(const 
     }
     __syncthreads();
     // ---- sweep 3: z-lines (qx, qy): U = Nz A (table N), then gz = Dz U on the same lines (table D) -------------------------------------
-#pragma unroll 1
-    for (int l = slot; l < n2; l += LS) {
-        double* f = F0 + (size_t)l * BT + lane;
+#pragma unroll
+    for (int r = 0; r < 2; ++r) if (r == 0 || two) {
+        const int l = ll[r];
+        double* f = F0 + lz[r];
 #pragma unroll
         for (int k = 0; k < n; ++k) t[k] = f[k * SZ];
         mat1d_eo<n>(prm.eoN, t, o);
 #pragma unroll
         for (int k = 0; k < n; ++k) f[k * SZ] = o[k];
     }
-#pragma unroll 1
-    for (int l = slot; l < n2; l += LS) {
-        const size_t off = (size_t)l * BT + lane;
+#pragma unroll
+    for (int r = 0; r < 2; ++r) if (r == 0 || two) {
+        const int l = ll[r];
+        const int off = lz[r];
 #pragma unroll
         for (int k = 0; k < n; ++k) t[k] = F0[off + k * SZ];
         mat1d_eoa<n>(prm.eoD, t, o);
@@ -270,9 +279,10 @@ __global__ void __launch_bounds__(GenShape<P>::LS * BT, MINB) k_apply_gen(const 
     }
     __syncthreads();
     // ---- sweep 4: y-lines (qx, qz): gy = Dy U (table D) ---------------------------------------------------------------------------------
-#pragma unroll 1
-    for (int l = slot; l < n2; l += LS) {
-        const size_t off = ((size_t)(l / n) * n2 + (l % n)) * BT + lane;
+#pragma unroll
+    for (int r = 0; r < 2; ++r) if (r == 0 || two) {
+        const int l = ll[r];
+        const int off = ly[r];
 #pragma unroll
         for (int k = 0; k < n; ++k) t[k] = F0[off + k * SY];
         mat1d_eoa<n>(prm.eoD, t, o);
@@ -282,9 +292,10 @@ __global__ void __launch_bounds__(GenShape<P>::LS * BT, MINB) k_apply_gen(const 
     __syncthreads();
     // ---- sweep 5: x-lines (qy, qz): gx = Dx U (table D), the metric at the line's points, t = WV U + Dx^T fx (table D^T) -------------
     mbar_wait(bar, 0);
-#pragma unroll 1
-    for (int l = slot; l < n2; l += LS) {
-        const size_t off = (size_t)l * n * BT + lane;
+#pragma unroll
+    for (int r = 0; r < 2; ++r) if (r == 0 || two) {
+        const int l = ll[r];
+        const int off = lx[r];
         const double* Mq = sRec + l * n;  // + c * n3 + qx
         double u[n];
 #pragma unroll
@@ -305,9 +316,10 @@ __global__ void __launch_bounds__(GenShape<P>::LS * BT, MINB) k_apply_gen(const 
     }
     __syncthreads();
     // ---- sweep 6: y-lines (qx, qz): t += Dy^T fy (table D^T) ------------------------------------------------------------------------------
-#pragma unroll 1
-    for (int l = slot; l < n2; l += LS) {
-        const size_t off = ((size_t)(l / n) * n2 + (l % n)) * BT + lane;
+#pragma unroll
+    for (int r = 0; r < 2; ++r) if (r == 0 || two) {
+        const int l = ll[r];
+        const int off = ly[r];
 #pragma unroll
         for (int k = 0; k < n; ++k) t[k] = F1[off + k * SY];
         mat1d_eoa<n>(prm.eoDT, t, o);
@@ -316,18 +328,20 @@ __global__ void __launch_bounds__(GenShape<P>::LS * BT, MINB) k_apply_gen(const 
     }
     __syncthreads();
     // ---- sweep 7: z-lines (qx, qy): T = t + Dz^T fz (table D^T), then R = Nz^T T on the same lines (table N^T) -------------------------
-#pragma unroll 1
-    for (int l = slot; l < n2; l += LS) {
-        const size_t off = (size_t)l * BT + lane;
+#pragma unroll
+    for (int r = 0; r < 2; ++r) if (r == 0 || two) {
+        const int l = ll[r];
+        const int off = lz[r];
 #pragma unroll
         for (int k = 0; k < n; ++k) t[k] = F2[off + k * SZ];
         mat1d_eoa<n>(prm.eoDT, t, o);
 #pragma unroll
         for (int k = 0; k < n; ++k) F0[off + k * SZ] += o[k];
     }
-#pragma unroll 1
-    for (int l = slot; l < n2; l += LS) {
-        double* f = F0 + (size_t)l * BT + lane;
+#pragma unroll
+    for (int r = 0; r < 2; ++r) if (r == 0 || two) {
+        const int l = ll[r];
+        double* f = F0 + lz[r];
 #pragma unroll
         for (int k = 0; k < n; ++k) t[k] = f[k * SZ];
         mat1d_eo<n>(prm.eoNT, t, o);
@@ -336,9 +350,10 @@ __global__ void __launch_bounds__(GenShape<P>::LS * BT, MINB) k_apply_gen(const 
     }
     __syncthreads();
     // ---- sweep 8: y-lines (qx, az) (table N^T) ----------------------------------------------------------------------------------------------
-#pragma unroll 1
-    for (int l = slot; l < n2; l += LS) {
-        double* f = F0 + ((size_t)(l / n) * n2 + (l % n)) * BT + lane;
+#pragma unroll
+    for (int r = 0; r < 2; ++r) if (r == 0 || two) {
+        const int l = ll[r];
+        double* f = F0 + ly[r];
 #pragma unroll
         for (int k = 0; k < n; ++k) t[k] = f[k * SY];
         mat1d_eo<n>(prm.eoNT, t, o);
@@ -347,9 +362,10 @@ __global__ void __launch_bounds__(GenShape<P>::LS * BT, MINB) k_apply_gen(const 
     }
     __syncthreads();
     // ---- sweep 9: x-lines (ay, az) (table N^T) and the scatter of the line's n nodes through the l2g -----------------------------------------
-#pragma unroll 1
-    for (int l = slot; l < n2; l += LS) {
-        const double* f = F0 + (size_t)l * n * BT + lane;
+#pragma unroll
+    for (int r = 0; r < 2; ++r) if (r == 0 || two) {
+        const int l = ll[r];
+        const double* f = F0 + lx[r];
 #pragma unroll
         for (int k = 0; k < n; ++k) t[k] = f[k * SX];
         mat1d_eo<n>(prm.eoNT, t, o);
