@@ -76,13 +76,12 @@ struct fe_mesh {
     int32_t* d_gl2g = nullptr;
     double *d_gmetric = nullptr, *d_gwdet = nullptr, *d_gsc = nullptr;
     EOTab eoD, eoDT;  // even-odd halves of the collocation derivative and its transpose (centro-antisymmetric)
-    long long* d_crow = nullptr;
-    int32_t* d_ccol = nullptr;
-    double* d_cval = nullptr;  // constraint weight times s of its unconstrained node (fe_general.cuh: cs)
-    long long* d_trow = nullptr;  // the same rows transposed: for every unconstrained node with hanging dependents ...
-    int32_t *d_tcol = nullptr, *d_tid = nullptr;  // ... the hanging rows (index r = h - N) that use it, and its own id
-    double* d_tval = nullptr;
-    long long nt = 0;
+    struct GenBundlesDev {  // rows with identical column lists packed for k_gen_rows_times_block (fe_general.cuh)
+        long long* bptr = nullptr;
+        int32_t *bcol = nullptr, *brow = nullptr, *out = nullptr;
+        double* bw = nullptr;
+        long long nb = 0;
+    } gexp;  // expansion X_h = C_h (s . X); the collapse Y += alpha s . C_h^T Y_h reads the same bundles the other way
     double *d_Xh = nullptr, *d_Yh = nullptr;  // (N_all - N) * hcap: expanded hanging values / their scatter target
     int hcap = 0;
     int sms = 0;  // multiprocessors of the device (persistent grid size)
@@ -218,9 +217,9 @@ int fe_mesh_destroy(fe_mesh* m)
     for (cudaStream_t s : m->hstream) if (s) cudaStreamDestroy(s);
     cudaFree(m->d_small); cudaFree(m->d_minv); cudaFree(m->d_mask); cudaFree(m->d_scal);
     cudaFree(m->d_VZ); cudaFree(m->d_sx); cudaFree(m->d_sy); cudaFree(m->d_sz);
-    cudaFree(m->d_gl2g); cudaFree(m->d_gmetric); cudaFree(m->d_gwdet); cudaFree(m->d_gsc); cudaFree(m->d_crow);
-    cudaFree(m->d_ccol); cudaFree(m->d_cval); cudaFree(m->d_Xh); cudaFree(m->d_Yh);
-    cudaFree(m->d_trow); cudaFree(m->d_tcol); cudaFree(m->d_tid); cudaFree(m->d_tval);
+    cudaFree(m->d_gl2g); cudaFree(m->d_gmetric); cudaFree(m->d_gwdet); cudaFree(m->d_gsc);
+    cudaFree(m->d_Xh); cudaFree(m->d_Yh);
+    cudaFree(m->gexp.bptr); cudaFree(m->gexp.bcol); cudaFree(m->gexp.brow); cudaFree(m->gexp.out); cudaFree(m->gexp.bw);
     delete m->gh;
     delete m;
     return FE_OK;
@@ -457,7 +456,6 @@ int fe_mesh_create_general(int cx, int cy, int cz, const int32_t* cells, int64_t
         memcpy(&met[(size_t)e * grec], &g.metric[(size_t)e * 7 * m->nc], (size_t)6 * m->nc * sizeof(double));
         memcpy(&wdet[(size_t)e * m->nc], &g.metric[((size_t)e * 7 + 6) * m->nc], (size_t)m->nc * sizeof(double));
     }
-    std::vector<long long> crow(g.crow.begin(), g.crow.end());
     std::vector<double> scv(g.l2g.size()), csv(g.cval.size());
     for (size_t i = 0; i < scv.size(); ++i) scv[i] = g.l2g[i] < g.N ? sv[g.l2g[i]] : 1.0;
     for (size_t k = 0; k < csv.size(); ++k) csv[k] = g.cval[k] * sv[g.ccol[k]];  // constraint weight times s of its node
@@ -473,38 +471,60 @@ int fe_mesh_create_general(int cx, int cy, int cz, const int32_t* cells, int64_t
         if (n % 2 == 1)
             for (int k = 0; k < h; ++k) { m->eoD.S[h * h + k] = m->tab.D[h * n + k]; m->eoDT.S[h * h + k] = Dt[h * n + k]; }
     }
-    // transposed constraint rows (collapse without atomics): entries sorted by unconstrained node, then by hanging row
-    std::vector<long long> trow;
-    std::vector<int32_t> tcol, tid;
-    std::vector<double> tval;
+    // the constraint rows and their transpose, sorted by column list and packed into bundles of rows with identical lists
+    auto pack = [&](const std::vector<std::vector<std::pair<int32_t, double>>>& rws, const std::vector<int32_t>& dst_of,
+                    fe_mesh::GenBundlesDev* dev) -> int {
+        const int64_t nr = (int64_t)rws.size();
+        std::vector<int32_t> order((size_t)nr);
+        for (int64_t i = 0; i < nr; ++i) order[i] = (int32_t)i;
+        auto same_cols = [&](int32_t a, int32_t b) {
+            if (rws[a].size() != rws[b].size()) return false;
+            for (size_t k = 0; k < rws[a].size(); ++k)
+                if (rws[a][k].first != rws[b][k].first) return false;
+            return true;
+        };
+        std::sort(order.begin(), order.end(), [&](int32_t a, int32_t b) {
+            if (rws[a].size() != rws[b].size()) return rws[a].size() < rws[b].size();
+            for (size_t k = 0; k < rws[a].size(); ++k)
+                if (rws[a][k].first != rws[b][k].first) return rws[a][k].first < rws[b][k].first;
+            return a < b;
+        });
+        std::vector<long long> bptr{0};
+        std::vector<int32_t> bcol, brow{0}, out;
+        std::vector<double> bw;
+        for (int64_t i = 0; i < nr;) {
+            int64_t e = i + 1;
+            while (e < nr && e - i < kGenBundle && same_cols(order[i], order[e])) ++e;
+            const auto& first = rws[order[i]];
+            for (size_t k = 0; k < first.size(); ++k) {
+                bcol.push_back(first[k].first);
+                for (int u = 0; u < kGenBundle; ++u) bw.push_back(i + u < e ? rws[order[i + u]][k].second : 0.0);
+            }
+            for (int64_t q = i; q < e; ++q) out.push_back(dst_of[order[q]]);
+            bptr.push_back((long long)bcol.size());
+            brow.push_back((int32_t)out.size());
+            i = e;
+        }
+        dev->nb = (long long)bptr.size() - 1;
+        int r;
+        if ((r = upload_vec(&dev->bptr, bptr)) || (r = upload_vec(&dev->bcol, bcol)) || (r = upload_vec(&dev->brow, brow)) ||
+            (r = upload_vec(&dev->out, out)) || (r = upload_vec(&dev->bw, bw)))
+            return r;
+        return FE_OK;
+    };
+    int rc = FE_OK;
     {
         const int64_t nh = g.N_all - g.N;
-        std::vector<int64_t> cnt((size_t)g.N + 1, 0);
-        for (int32_t c : g.ccol) cnt[(size_t)c + 1] += 1;
-        for (int64_t i = 0; i < g.N; ++i) cnt[i + 1] += cnt[i];
-        std::vector<int64_t> pos(cnt.begin(), cnt.end() - 1);
-        std::vector<int32_t> hc(g.ccol.size());
-        std::vector<double> hv(g.ccol.size());
-        for (int64_t r = 0; r < nh; ++r)
-            for (int64_t k = g.crow[r]; k < g.crow[r + 1]; ++k) {
-                const int64_t q = pos[g.ccol[k]]++;
-                hc[q] = (int32_t)r;
-                hv[q] = csv[k];
-            }
-        trow.push_back(0);
-        for (int64_t i = 0; i < g.N; ++i)
-            if (cnt[i + 1] > cnt[i]) {
-                tid.push_back((int32_t)i);
-                for (int64_t q = cnt[i]; q < cnt[i + 1]; ++q) { tcol.push_back(hc[q]); tval.push_back(hv[q]); }
-                trow.push_back((long long)tcol.size());
-            }
-        m->nt = (long long)tid.size();
+        std::vector<std::vector<std::pair<int32_t, double>>> fw((size_t)nh);
+        std::vector<int32_t> fdst((size_t)nh);
+        for (int64_t r = 0; r < nh; ++r) {
+            fdst[r] = (int32_t)r;
+            for (int64_t k = g.crow[r]; k < g.crow[r + 1]; ++k) fw[r].push_back({g.ccol[k], csv[k]});
+        }
+        if ((rc = pack(fw, fdst, &m->gexp))) { fe_mesh_destroy(m); return rc; }
     }
-    int rc;
-    if ((rc = upload_vec(&m->d_trow, trow)) || (rc = upload_vec(&m->d_tcol, tcol)) || (rc = upload_vec(&m->d_tid, tid)) ||
-        (rc = upload_vec(&m->d_tval, tval)) || (rc = upload_vec(&m->d_gsc, scv)) || (rc = upload_vec(&m->d_sm, sv)) || (rc = upload_vec(&m->d_gl2g, g.l2g)) || (rc = upload_vec(&m->d_gmetric, met)) ||
-        (rc = upload_vec(&m->d_gwdet, wdet)) || (rc = upload_vec(&m->d_crow, crow)) || (rc = upload_vec(&m->d_ccol, g.ccol)) ||
-        (rc = upload_vec(&m->d_cval, csv))) {
+    if ((rc = upload_vec(&m->d_gsc, scv)) || (rc = upload_vec(&m->d_sm, sv)) || (rc = upload_vec(&m->d_gl2g, g.l2g)) || (rc = upload_vec(&m->d_gmetric, met)) ||
+        (rc = upload_vec(&m->d_gwdet, wdet))) {
         fe_mesh_destroy(m);
         return rc;
     }
@@ -548,7 +568,8 @@ static int general_step(fe_mesh* m, const double* X, const double* Z, double* Y,
         k_gen_init<<<grid, rows, 0, st>>>(Y, X, Z, m->d_sm, eps, alpha, beta, c, g.N, B);
     if (nh > 0) {
         CUDA_TRY(cudaMemsetAsync(m->d_Yh, 0, (size_t)nh * B * sizeof(double), st));
-        k_gen_rows_times_block<<<grid, rows, 0, st>>>(m->d_Xh, X, m->d_crow, m->d_ccol, m->d_cval, nullptr, nh, B, 1.0, 0);
+        k_gen_rows_times_block<<<grid, rows, 0, st>>>(m->d_Xh, X, m->gexp.bptr, m->gexp.bcol, m->gexp.bw, m->gexp.brow, m->gexp.out,
+                                                      m->gexp.nb, B, 1.0, 0);
     }
     GenParams prm;
     memset(&prm, 0, sizeof(prm));
@@ -558,7 +579,8 @@ static int general_step(fe_mesh* m, const double* X, const double* Z, double* Y,
     cudaError_t e = launch_apply_gen(prm, m->p, m->ncells, st);
     if (e != cudaSuccess) return fail(FE_ERR_CUDA, "operator launch (general mesh) failed: %s", cudaGetErrorString(e));
     if (nh > 0)
-        k_gen_rows_times_block<<<grid, rows, 0, st>>>(Y, m->d_Yh, m->d_trow, m->d_tcol, m->d_tval, m->d_tid, m->nt, B, alpha, 1);
+        k_gen_collapse<<<grid, rows, 0, st>>>(Y, m->d_Yh, m->gexp.bptr, m->gexp.bcol, m->gexp.bw, m->gexp.brow, m->gexp.out, m->gexp.nb, B,
+                                              alpha);
     CUDA_TRY(cudaGetLastError());
     m->launches += nh > 0 ? 4 : 2;
     return FE_OK;

@@ -69,38 +69,78 @@ __global__ void k_gen_init(double* __restrict__ Y, const double* __restrict__ X,
     }
 }
 
-// Sparse rows times a block:  dst[row(r), j] (+)= alpha sum_k cs_k src[ccol_k, j]  for r < nr, row(r) = rows ? rows[r] : r.
-//   expansion  X_h = C_h (s . X):        src = X,   dst = X_h, cs = cval * s[ccol] (0 on Dirichlet rows, whose data is ignored)
-//   collapse   Y += alpha s . C_h^T Y_h:  src = Y_h, dst = Y, rows = the unconstrained nodes that have hanging dependents,
-//                                          the TRANSPOSED constraint rows (no atomics: every dst row has one owner)
-// A warp works on one row (lanes = vectors); the loop over the row's entries is latency-bound (index, then the row of src),
-// so eight entries are in flight per thread and the kernel is capped at 32 registers for 64 warps per SM.
-__global__ void __launch_bounds__(32 * kGenRows, 8)
-k_gen_rows_times_block(double* __restrict__ dst, const double* __restrict__ src, const long long* __restrict__ crow,
-                       const int32_t* __restrict__ ccol, const double* __restrict__ cs, const int32_t* __restrict__ rows,
-                       long long nr, int B, double alpha, int accumulate)
+// Sparse rows times a block:  dst[out_r, j] (+)= alpha sum_k w_rk src[col_k, j].
+//   expansion  X_h = C_h (s . X):        src = X,   dst = X_h, w = cval * s[col] (0 on Dirichlet rows, whose data is ignored)
+//   collapse   Y += alpha s . C_h^T Y_h:  k_gen_collapse below, the same bundles read the other way
+// The hanging nodes of one coarse face all depend on the same n^2 nodes (and the nodes of a coarse face all feed the same
+// hanging nodes), so the host sorts the rows by their column lists and packs rows with IDENTICAL lists into bundles of up to
+// kGenBundle rows (GenBundles in fe_cheb.cu): a warp (lanes = vectors) works on one bundle, reads every row of src once for
+// all its rows and the bundle's weights as one 64-byte line per entry -- row by row the kernel moved n^2 x the block through
+// L2 and was bound by L2 bandwidth.  bptr[b] .. bptr[b+1]: entries of bundle b (col, 8 weights each); brow[b] .. brow[b+1]:
+// its rows in `out`.
+constexpr int kGenBundle = 8;
+
+__global__ void __launch_bounds__(32 * kGenRows, 4)
+k_gen_rows_times_block(double* __restrict__ dst, const double* __restrict__ src, const long long* __restrict__ bptr,
+                       const int32_t* __restrict__ bcol, const double* __restrict__ bw, const int32_t* __restrict__ brow,
+                       const int32_t* __restrict__ out, long long nb, int B, double alpha, int accumulate)
 {
-    for (long long r = blockIdx.x * (long long)kGenRows + threadIdx.y; r < nr; r += (long long)gridDim.x * kGenRows) {
-        const long long k0 = crow[r], k1 = crow[r + 1];
-        const long long out = rows ? rows[r] : r;
+    for (long long b = blockIdx.x * (long long)kGenRows + threadIdx.y; b < nb; b += (long long)gridDim.x * kGenRows) {
+        const long long k0 = bptr[b], k1 = bptr[b + 1];
+        const int r0 = brow[b], m = brow[b + 1] - r0;
         for (int j = threadIdx.x; j < B; j += 32) {
-            double v = 0.0;
-            long long k = k0;
-            for (; k + 8 <= k1; k += 8) {
-                double c[8], x[8];
+            double v[kGenBundle];
 #pragma unroll
-                for (int u = 0; u < 8; ++u) c[u] = cs[k + u];
-#pragma unroll
-                for (int u = 0; u < 8; ++u) x[u] = src[(long long)ccol[k + u] * B + j];
-#pragma unroll
-                for (int u = 0; u < 8; ++u) v = c[u] != 0.0 ? fma(c[u], x[u], v) : v;
+            for (int u = 0; u < kGenBundle; ++u) v[u] = 0.0;
+#pragma unroll 2
+            for (long long k = k0; k < k1; ++k) {
+                const double x = src[(long long)bcol[k] * B + j];
+                const double4 w0 = *reinterpret_cast<const double4*>(bw + k * kGenBundle);
+                const double4 w1 = *reinterpret_cast<const double4*>(bw + k * kGenBundle + 4);
+                v[0] = w0.x != 0.0 ? fma(w0.x, x, v[0]) : v[0];
+                v[1] = w0.y != 0.0 ? fma(w0.y, x, v[1]) : v[1];
+                v[2] = w0.z != 0.0 ? fma(w0.z, x, v[2]) : v[2];
+                v[3] = w0.w != 0.0 ? fma(w0.w, x, v[3]) : v[3];
+                v[4] = w1.x != 0.0 ? fma(w1.x, x, v[4]) : v[4];
+                v[5] = w1.y != 0.0 ? fma(w1.y, x, v[5]) : v[5];
+                v[6] = w1.z != 0.0 ? fma(w1.z, x, v[6]) : v[6];
+                v[7] = w1.w != 0.0 ? fma(w1.w, x, v[7]) : v[7];
             }
-            for (; k < k1; ++k) {
-                const double c0 = cs[k];
-                v = c0 != 0.0 ? fma(c0, src[(long long)ccol[k] * B + j], v) : v;
+#pragma unroll
+            for (int u = 0; u < kGenBundle; ++u)
+                if (u < m) {
+                    double* d = dst + (long long)out[r0 + u] * B + j;
+                    *d = accumulate ? fma(alpha, v[u], *d) : alpha * v[u];
+                }
+        }
+    }
+}
+
+// Y[col_k, j] += alpha sum_u w_ku Y_h[out_u, j] over the bundles of the expansion: the transpose of k_gen_rows_times_block
+// from the SAME packed rows -- the (up to 8) hanging rows of a bundle are read once, every entry costs one red.global.add of the
+// bundle's combined contribution (an eighth of the atomics of a row-by-row transpose; sorting the transposed rows instead
+// does not bundle, because exactly-zero weights make the column lists of neighbouring nodes differ)
+__global__ void __launch_bounds__(32 * kGenRows, 4)
+k_gen_collapse(double* __restrict__ Y, const double* __restrict__ Yh, const long long* __restrict__ bptr,
+               const int32_t* __restrict__ bcol, const double* __restrict__ bw, const int32_t* __restrict__ brow,
+               const int32_t* __restrict__ out, long long nb, int B, double alpha)
+{
+    for (long long b = blockIdx.x * (long long)kGenRows + threadIdx.y; b < nb; b += (long long)gridDim.x * kGenRows) {
+        const long long k0 = bptr[b], k1 = bptr[b + 1];
+        const int r0 = brow[b], m = brow[b + 1] - r0;
+        for (int j = threadIdx.x; j < B; j += 32) {
+            double y[kGenBundle];
+#pragma unroll
+            for (int u = 0; u < kGenBundle; ++u) y[u] = u < m ? alpha * Yh[(long long)out[r0 + u] * B + j] : 0.0;
+#pragma unroll 2
+            for (long long k = k0; k < k1; ++k) {
+                const double4 w0 = *reinterpret_cast<const double4*>(bw + k * kGenBundle);
+                const double4 w1 = *reinterpret_cast<const double4*>(bw + k * kGenBundle + 4);
+                double v = w0.x * y[0];
+                v = fma(w0.y, y[1], v); v = fma(w0.z, y[2], v); v = fma(w0.w, y[3], v);
+                v = fma(w1.x, y[4], v); v = fma(w1.y, y[5], v); v = fma(w1.z, y[6], v); v = fma(w1.w, y[7], v);
+                if (v != 0.0) atomicAdd(Y + (long long)bcol[k] * B + j, v);
             }
-            double* d = dst + out * B + j;
-            *d = accumulate ? fma(alpha, v, *d) : alpha * v;
         }
     }
 }
