@@ -574,9 +574,9 @@ static int general_step(fe_mesh* m, const double* X, const double* Z, double* Y,
     GenParams prm;
     memset(&prm, 0, sizeof(prm));
     prm.X = X; prm.Xh = m->d_Xh ? m->d_Xh : X; prm.Y = Y; prm.Yh = m->d_Yh ? m->d_Yh : Y; prm.sc = m->d_gsc; prm.l2g = m->d_gl2g;
-    prm.rec = m->d_gmetric; prm.N = g.N; prm.B = B; prm.alpha = alpha;
+    prm.rec = m->d_gmetric; prm.N = g.N; prm.ncells = m->ncells; prm.B = B; prm.alpha = alpha;
     prm.eoN = m->eoN; prm.eoNT = m->eoNT; prm.eoD = m->eoD; prm.eoDT = m->eoDT;
-    cudaError_t e = launch_apply_gen(prm, m->p, m->ncells, st);
+    cudaError_t e = launch_apply_gen(prm, m->p, m->ncells, m->sms, st);
     if (e != cudaSuccess) return fail(FE_ERR_CUDA, "operator launch (general mesh) failed: %s", cudaGetErrorString(e));
     if (nh > 0)
         k_gen_collapse<<<grid, rows, 0, st>>>(Y, m->d_Yh, m->gexp.bptr, m->gexp.bcol, m->gexp.bw, m->gexp.brow, m->gexp.out, m->gexp.nb, B,

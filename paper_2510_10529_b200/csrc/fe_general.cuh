@@ -23,6 +23,7 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cstdint>
 
 #include "fe_apply_tma.cuh"
@@ -38,7 +39,7 @@ struct GenParams {
     const int32_t* l2g;  // ncells * n^3
     const double* sc;    // ncells * n^3: s_g = mu_g M_c,gg^{-1/2} at the cell's unconstrained nodes, 1 at its hanging nodes
     const double* rec;   // ncells * GREC: per-cell record, 6 metric fields (fe_general.h) then WV = w_q |J| V_q, n^3 each
-    long long N;
+    long long N, ncells;
     int B;
     double alpha;
     // even-odd halves (fe_kernels.cuh): N and N^T are centro-symmetric, the collocation derivative D and D^T are
@@ -198,12 +199,12 @@ __device__ __forceinline__ void mat1d_eoa(const EOTab& T, const double (&in)[n],
     }
 }
 
-template <int P, int BT>
+template <int P, int BT, bool PERSIST>
 constexpr size_t gen_smem_bytes()
 {
-    constexpr int n3 = (P + 1) * (P + 1) * (P + 1);
-    return (size_t)3 * n3 * BT * sizeof(double) + (size_t)(7 * n3 + 1) * sizeof(double) +
-           (size_t)n3 * (sizeof(double) + sizeof(int32_t)) + 32;
+    constexpr int n3 = (P + 1) * (P + 1) * (P + 1), NB = PERSIST ? 2 : 1;
+    return (size_t)3 * n3 * BT * sizeof(double) + (size_t)NB * (7 * n3 + 1) * sizeof(double) +
+           (size_t)NB * (n3 + 1) * (sizeof(double) + sizeof(int32_t)) + 64;
 }
 
 // line slots of a CTA: every sweep has n^2 lines per vector; ceil(n^2 / 2) slots take them in two rounds
@@ -217,24 +218,27 @@ struct GenShape {
 // line in registers.  The loops are NOT unrolled over lines, so the whole kernel is a few hundred FP64 instructions per
 // sweep and stays in the instruction cache (the plane-in-registers version of this kernel, 150 KB of straight-line code run
 // by 3.5 warps, spent 4 of 5 issue slots waiting for instructions).
-template <int P, int BT, int MINB>
+// PERSIST: the CTA walks units (cell, vector tile) u = blockIdx.x, + gridDim.x, ...; while unit u runs its last two sweeps the
+// node rows of unit u + gridDim.x are already being fetched into the field that sweep 7 has freed, and its ids, scales and
+// metric record were requested at the start of unit u (second set of buffers), so the gather latency -- a quarter of the
+// one-unit-per-CTA kernel's time (ncu) -- hides behind arithmetic.  The three fields rotate roles from unit to unit.
+template <int P, int BT, int MINB, bool PERSIST>
 __global__ void __launch_bounds__(GenShape<P>::LS * BT, MINB) k_apply_gen(const __grid_constant__ GenParams prm)
 {
-    constexpr int n = P + 1, n2 = n * n, n3 = n * n * n, LS = GenShape<P>::LS;
+    constexpr int n = P + 1, n2 = n * n, n3 = n * n * n, LS = GenShape<P>::LS, NB = PERSIST ? 2 : 1;
     constexpr int SX = BT, SY = n * BT, SZ = n2 * BT;  // strides of the three directions in a field [z][y][x][BT]
+    constexpr int GREC = 7 * n3 + ((7 * n3) & 1), N3E = n3 + (n3 & 1);
     extern __shared__ __align__(128) double smem[];
     double* F0 = smem;                  // x -> A -> U -> t -> T -> R
-    double* F1 = F0 + (size_t)n3 * BT;  // gy -> fy
+    double* F1 = F0 + (size_t)n3 * BT;  // gy -> fy          (then the next unit's x)
     double* F2 = F1 + (size_t)n3 * BT;  // gz -> fz
-    double* sRec = F2 + (size_t)n3 * BT;  // the cell's record (6 metric fields, WV): one bulk copy, in flight until sweep 5
-    constexpr int GREC = 7 * n3 + ((7 * n3) & 1);
-    double* sSc = sRec + GREC;            // [n^3] gather / scatter scale of the cell's nodes
-    unsigned long long* bar = reinterpret_cast<unsigned long long*>(sSc + n3 + (n3 & 1));
-    int32_t* sId = reinterpret_cast<int32_t*>(bar + 1);  // [n^3] global ids
+    double* sRecB = F2 + (size_t)n3 * BT;  // [NB] the cell's record (6 metric fields, WV): one bulk copy, needed from sweep 5 on
+    double* sScB = sRecB + NB * GREC;      // [NB][n^3] gather / scatter scale of the cell's nodes
+    unsigned long long* bar = reinterpret_cast<unsigned long long*>(sScB + NB * N3E);  // [2]
+    int32_t* sIdB = reinterpret_cast<int32_t*>(bar + 2);  // [NB][n^3] global ids
     const int lane = threadIdx.x, slot = threadIdx.y, tid = slot * BT + lane;
-    const long long cell = blockIdx.x;
-    const int j = blockIdx.y * BT + lane;
-    const bool act = j < prm.B;
+    const int ntile = (prm.B + BT - 1) / BT;
+    const long long nunits = prm.ncells * ntile;
     const long long B = prm.B;
     double t[n], o[n];
     // the (at most) two lines of this slot in every sweep, as field offsets: x-lines (i1, i2), y-lines (i0, i2), z-lines (i0, i1)
@@ -248,26 +252,55 @@ __global__ void __launch_bounds__(GenShape<P>::LS * BT, MINB) k_apply_gen(const 
         ly[r] = ((l / n) * n2 + (l % n)) * BT + lane;
         lz[r] = l * BT + lane;
     }
-
-    // ---- gather: ids and scales of the cell, then 8-byte cp.async of the node rows straight into F0 ----------------------------
+    // requests for a unit: ids and scales (4- / 8-byte cp.async) and the record (bulk copy on bar[buf]) ...
+    auto request_tables = [&](long long u, int buf) {
+        const long long c = u / ntile;
+        if (tid == 0) {
+            mbar_expect_tx(bar + buf, (unsigned)(GREC * sizeof(double)));
+            bulk_load(sRecB + buf * GREC, prm.rec + c * GREC, (unsigned)(GREC * sizeof(double)), bar + buf);
+        }
+        for (int a = tid; a < n3; a += LS * BT) {
+            const unsigned di = (unsigned)__cvta_generic_to_shared(sIdB + buf * n3 + a);
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(di), "l"(prm.l2g + c * n3 + a) : "memory");
+            cp_async8(sScB + buf * N3E + a, prm.sc + c * n3 + a, true);
+        }
+        cp_async_commit();
+    };
+    // ... and its node rows, once the ids are in shared memory: independent 8-byte cp.async straight into the field
+    auto request_rows = [&](long long u, int buf, double* F) {
+        const int jn = (int)(u % ntile) * BT + lane;
+        const bool an = jn < prm.B;
+        for (int a = slot; a < n3; a += LS) {
+            const long long g = sIdB[buf * n3 + a];
+            const double* src = g < prm.N ? prm.X + g * B + jn : prm.Xh + (g - prm.N) * B + jn;
+            cp_async8(F + (size_t)a * BT + lane, an ? src : prm.X, an);
+        }
+        cp_async_commit();
+    };
     if (tid == 0) {
         mbar_init(bar, 1);
-        mbar_expect_tx(bar, (unsigned)(GREC * sizeof(double)));
-        bulk_load(sRec, prm.rec + cell * GREC, (unsigned)(GREC * sizeof(double)), bar);
-    }
-    for (int a = tid; a < n3; a += LS * BT) {
-        sId[a] = prm.l2g[cell * n3 + a];
-        sSc[a] = prm.sc[cell * n3 + a];
+        mbar_init(bar + 1, 1);
     }
     __syncthreads();
-    for (int a = slot; a < n3; a += LS) {
-        const long long g = sId[a];
-        const double* src = g < prm.N ? prm.X + g * B + j : prm.Xh + (g - prm.N) * B + j;
-        cp_async8(F0 + (size_t)a * BT + lane, act ? src : prm.X, act);
+    if ((long long)blockIdx.x < nunits) {
+        request_tables(blockIdx.x, 0);
+        cp_async_wait_all();
+        __syncthreads();
+        request_rows(blockIdx.x, 0, F0);
     }
-    cp_async_commit();
+    unsigned ph0 = 0, ph1 = 0;  // phases of the two record barriers
+    int buf = 0;
+    for (long long u = blockIdx.x; u < nunits; u += gridDim.x, buf ^= (PERSIST ? 1 : 0)) {
+    const long long un = u + gridDim.x;
+    const bool more = PERSIST && un < nunits;
+    const int j = (int)(u % ntile) * BT + lane;
+    const bool act = j < prm.B;
+    const double* sRec = sRecB + buf * GREC;
+    const double* sSc = sScB + buf * N3E;
+    const int32_t* sId = sIdB + buf * n3;
     cp_async_wait_all();
-    __syncthreads();
+    __syncthreads();  // this unit's rows are in F0; the previous unit has left its buffers
+    if (more) request_tables(un, buf ^ 1);
     // ---- sweep 1: x-lines (ay, az) of the nodal values: scale (mask, M^-1/2), interpolate (table N) -----------------------------
 #pragma unroll
     for (int r = 0; r < 2; ++r) if (r == 0 || two) {
@@ -331,7 +364,7 @@ __global__ void __launch_bounds__(GenShape<P>::LS * BT, MINB) k_apply_gen(const 
     }
     __syncthreads();
     // ---- sweep 5: x-lines (qy, qz): gx = Dx U (table D), the metric at the line's points, t = WV U + Dx^T fx (table D^T) -------------
-    mbar_wait(bar, 0);
+    if (buf == 0) { mbar_wait(bar, ph0); ph0 ^= 1; } else { mbar_wait(bar + 1, ph1); ph1 ^= 1; }
 #pragma unroll
     for (int r = 0; r < 2; ++r) if (r == 0 || two) {
         const int l = ll[r];
@@ -388,7 +421,9 @@ __global__ void __launch_bounds__(GenShape<P>::LS * BT, MINB) k_apply_gen(const 
 #pragma unroll
         for (int k = 0; k < n; ++k) f[k * SZ] = o[k];
     }
+    if (more) cp_async_wait_all();  // the next unit's ids and scales (requested at the top of this unit)
     __syncthreads();
+    if (more) request_rows(un, buf ^ 1, F1);  // F1 and F2 are free from here on
     // ---- sweep 8: y-lines (qx, az) (table N^T) ----------------------------------------------------------------------------------------------
 #pragma unroll
     for (int r = 0; r < 2; ++r) if (r == 0 || two) {
@@ -420,34 +455,41 @@ __global__ void __launch_bounds__(GenShape<P>::LS * BT, MINB) k_apply_gen(const 
             }
         }
     }
+    double* Fr = F0; F0 = F1; F1 = F2; F2 = Fr;  // the field that holds the next unit's rows becomes F0
+    }  // units
 }
 
-template <int P, int BT, int MINB>
-cudaError_t launch_gen(const GenParams& prm, long long ncells, cudaStream_t st)
+template <int P, int BT, int MINB, bool PERSIST>
+cudaError_t launch_gen(const GenParams& prm, long long ncells, int sms, cudaStream_t st)
 {
-    constexpr size_t smem = gen_smem_bytes<P, BT>();
+    constexpr size_t smem = gen_smem_bytes<P, BT, PERSIST>();
     static PerDeviceOnce once;
     cudaError_t e0 = once_per_device(once, [&] {
-        return cudaFuncSetAttribute(k_apply_gen<P, BT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        return cudaFuncSetAttribute(k_apply_gen<P, BT, MINB, PERSIST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     });
     if (e0 != cudaSuccess) return e0;
-    dim3 grid((unsigned)ncells, (unsigned)((prm.B + BT - 1) / BT)), block(BT, GenShape<P>::LS);
-    k_apply_gen<P, BT, MINB><<<grid, block, smem, st>>>(prm);
+    const long long nunits = ncells * ((prm.B + BT - 1) / BT);
+    const long long ctas = PERSIST ? std::min<long long>(nunits, (long long)sms * MINB) : nunits;
+    dim3 grid((unsigned)ctas), block(BT, GenShape<P>::LS);
+    k_apply_gen<P, BT, MINB, PERSIST><<<grid, block, smem, st>>>(prm);
     return cudaGetLastError();
 }
 
-// vector-tile width per order: three fields of n^3 x BT doubles + the cell record per CTA, several CTAs per SM where they fit
-inline cudaError_t launch_apply_gen(const GenParams& prm, int p, long long ncells, cudaStream_t st)
+// vector-tile width per order: three fields of n^3 x BT doubles + the cell record per CTA, several CTAs per SM where they
+// fit.  The persistent walk with prefetched rows pays where only ONE CTA fits an SM (p = 7: 27.1 -> 31.2 GDoF-vec/s on the
+// adaptive workload); with two CTAs per SM the hardware already overlaps one CTA's gather with the other's arithmetic and
+// the loop state costs 3-4 % (p = 4, 6); p = 8 has no room for the second set of buffers.
+inline cudaError_t launch_apply_gen(const GenParams& prm, int p, long long ncells, int sms, cudaStream_t st)
 {
     switch (p) {
-        case 1: return launch_gen<1, 32, 8>(prm, ncells, st);
-        case 2: return launch_gen<2, 32, 6>(prm, ncells, st);
-        case 3: return launch_gen<3, 32, 4>(prm, ncells, st);
-        case 4: return launch_gen<4, 32, 2>(prm, ncells, st);
-        case 5: return launch_gen<5, 16, 2>(prm, ncells, st);
-        case 6: return launch_gen<6, 8, 2>(prm, ncells, st);
-        case 7: return launch_gen<7, 8, 1>(prm, ncells, st);
-        case 8: return launch_gen<8, 8, 1>(prm, ncells, st);
+        case 1: return launch_gen<1, 32, 8, false>(prm, ncells, sms, st);
+        case 2: return launch_gen<2, 32, 6, false>(prm, ncells, sms, st);
+        case 3: return launch_gen<3, 32, 4, false>(prm, ncells, sms, st);
+        case 4: return launch_gen<4, 32, 2, false>(prm, ncells, sms, st);
+        case 5: return launch_gen<5, 16, 2, false>(prm, ncells, sms, st);
+        case 6: return launch_gen<6, 8, 2, false>(prm, ncells, sms, st);
+        case 7: return launch_gen<7, 8, 1, true>(prm, ncells, sms, st);
+        case 8: return launch_gen<8, 8, 1, false>(prm, ncells, sms, st);
     }
     return cudaErrorInvalidValue;
 }

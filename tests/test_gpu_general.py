@@ -49,10 +49,11 @@ def _coulomb(q):
     return -4.0 / np.sqrt((q ** 2).sum(axis=1) + 0.25)
 
 
-@pytest.mark.parametrize("p,B", [(1, 5), (2, 34), (3, 6), (4, 33), (5, 6), (6, 18), (7, 5), (8, 10)])
+@pytest.mark.parametrize("p,B", [(1, 5), (2, 34), (3, 6), (4, 33), (5, 6), (6, 18), (7, 5), (7, 34), (8, 10)])
 def test_apply_refined_deformed_mesh_all_orders(p, B):
     """One-level refinement of a 3^3 root grid with smoothly displaced vertices (non-constant Jacobians, hanging faces and
-    edges): plain and shifted apply, ragged vector tiles, data in the Dirichlet rows."""
+    edges): plain and shifted apply, ragged vector tiles, data in the Dirichlet rows.  (7, 34): 83 leaves x 5 vector tiles are
+    more units than resident CTAs, so the persistent p = 7 kernel walks several units per CTA (prefetched rows, rotating fields)."""
     e = workloads.uniform_edges(-1.5, 1.5, 3)
     mesh = workloads.octree_mesh(e, e, e, lambda l, lo, hi: np.linalg.norm((lo + hi) / 2) < 0.9, 1, _wave)
     om, gm = _pair(mesh, p, _coulomb)
