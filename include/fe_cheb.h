@@ -67,8 +67,9 @@ int fe_get_dirichlet_mask(const fe_mesh* m, uint8_t* mask); /* N, 1 = free, 0 = 
  * nodes are no degrees of freedom, their values are u_h = sum_k c_hk u_k (fe_get_constraints).  Lumped mass of the
  * constrained problem: diag(C^T m) with m the GLL-quadrature nodal masses (R25).  Dirichlet on the surface of the root box.
  * On such a handle fe_set_potential, fe_apply_H, cheb_filter, cheb_filter_host, fe_rayleigh_ritz, fe_ritz_residuals,
- * fe_chfsi, fe_lanczos_bounds, fe_gram and fe_add_subspace work as on a box mesh; fe_minres_shifted, fe_density and
- * fe_apply_potential return FE_ERR_INVALID.  FE_ERR_INVALID for an inconsistent leaf list.  cuda_device = -1 builds the
+ * fe_chfsi, fe_lanczos_bounds, fe_minres_shifted, fe_gram, fe_add_subspace, fe_density and fe_apply_potential work as on a
+ * box mesh (the MINRES preconditioner is M_c,ii / d_i with d_i = kd_i + sum_h C_hi^2 kd_h, kd the diagonal of the assembled
+ * 1/2 K over all nodes, reading R27; psi at the quadrature points uses the hanging values u_h = sum_k c_hk u_k).  FE_ERR_INVALID for an inconsistent leaf list.  cuda_device = -1 builds the
  * tables only (sizes, l2g, constraints, coordinates, mass, mask can be queried; no potential can be set).  Synchronous. */
 int fe_mesh_create_general(int cx, int cy, int cz, const int32_t* cells, int64_t ncells, const double* verts, int p,
                            int cuda_device, fe_mesh** out);

@@ -202,6 +202,54 @@ class GeneralOracleMesh:
         S = sp.diags(s)
         self.Ht = (S @ self.Hc @ S).tocsr()
 
+    def density(self, X, f):
+        """rho[e, q] = sum_j f_j psi_j(x_q)^2 at the Gauss points of every cell (Eq. 4, l.73-77), psi = M_c^{-1/2} psi~
+        on the unconstrained nodes (zero Dirichlet rows), hanging values through the constraints, psi_j(x_q) written out
+        with the Lagrange basis of Eq. 12."""
+        X = np.ascontiguousarray(X, dtype=np.float64)
+        n = self.n
+        L1 = np.array([[fo.lagrange(self.gll_x, a, self.gl_x[q]) for a in range(n)] for q in range(n)])  # L1[q, a]
+        free = self._mask.astype(bool)
+        s = np.zeros(self.N)
+        s[free] = 1.0 / np.sqrt(self._mass[free])
+        psi_all = self.Cfull @ (X * s[:, None])
+        fw = np.ascontiguousarray(f, dtype=np.float64)
+        rho = np.zeros((self.ncells, n ** 3))
+        for e in range(self.ncells):
+            loc = psi_all[self._l2g[e]].reshape(n, n, n, -1)  # [az, ay, ax, j]
+            val = np.einsum("ra,sb,tc,cbaj->rstj", L1, L1, L1, loc)  # [qx, qy, qz, j]
+            rho[e] = np.einsum("rstj,j->rst", val ** 2, fw).transpose(2, 1, 0).reshape(-1)  # q = qx + n (qy + n qz)
+        return rho
+
+    def potential_apply(self, Uq, X):
+        """M_c^{-1/2} C^T M_U C M_c^{-1/2} X with (M_U)_ab = int N_a U N_b entry by entry from the cell matrices with the
+        kinetic part switched off: the integral of the adjoint right-hand side (Eq. 18, l.174-177) on a constrained mesh."""
+        Uq = np.ascontiguousarray(Uq, dtype=np.float64).reshape(self.ncells, self.nq3)
+        X = np.ascontiguousarray(X, dtype=np.float64)
+        free = self._mask.astype(bool)
+        s = np.zeros(self.N)
+        s[free] = 1.0 / np.sqrt(self._mass[free])
+        x_all = self.Cfull @ (X * s[:, None])
+        y_all = np.zeros_like(x_all)
+        for e in range(self.ncells):
+            g = self._l2g[e]
+            y_all[g] += self.cell_matrix(e, Uq[e], kin=0.0, pot=1.0) @ x_all[g]
+        return (self.Cfull.T @ y_all) * s[:, None]
+
+    def laplacian_precond(self):
+        """MINRES preconditioner on a constrained mesh (reading R27): M_c,ii / d_i on free rows, 0 on Dirichlet
+        rows, with d_i = kd_i + sum_h C_hi^2 kd_h and kd the diagonal of the assembled kinetic matrix 1/2 K over ALL nodes,
+        taken entry by entry from the cell matrices with the potential switched off."""
+        kd = np.zeros(self.N_all)
+        for e in range(self.ncells):
+            np.add.at(kd, self._l2g[e], np.diag(self.cell_matrix(e, None, kin=0.5, pot=0.0)))
+        Ch = self.Cfull[self.N:]
+        d = kd[:self.N] + (Ch.multiply(Ch)).T @ kd[self.N:]
+        free = self._mask.astype(bool)
+        out = np.zeros(self.N)
+        out[free] = self._mass[free] / d[free]
+        return out
+
     def apply(self, X, eps=None, nthreads=1):
         X = np.ascontiguousarray(X, dtype=np.float64)
         free = self._mask.astype(bool)

@@ -83,6 +83,7 @@ struct fe_mesh {
         long long nb = 0;
     } gexp;  // expansion X_h = C_h (s . X); the collapse Y += alpha s . C_h^T Y_h reads the same bundles the other way
     double *d_Xh = nullptr, *d_Yh = nullptr;  // (N_all - N) * hcap: expanded hanging values / their scatter target
+    double* d_grecU = nullptr;  // fe_apply_potential on a general mesh: records with zero metric and WV = w |J| U
     int hcap = 0;
     int sms = 0;  // multiprocessors of the device (persistent grid size)
     int64_t launches = 0;
@@ -218,7 +219,7 @@ int fe_mesh_destroy(fe_mesh* m)
     cudaFree(m->d_small); cudaFree(m->d_minv); cudaFree(m->d_mask); cudaFree(m->d_scal);
     cudaFree(m->d_VZ); cudaFree(m->d_sx); cudaFree(m->d_sy); cudaFree(m->d_sz);
     cudaFree(m->d_gl2g); cudaFree(m->d_gmetric); cudaFree(m->d_gwdet); cudaFree(m->d_gsc);
-    cudaFree(m->d_Xh); cudaFree(m->d_Yh);
+    cudaFree(m->d_Xh); cudaFree(m->d_Yh); cudaFree(m->d_grecU);
     cudaFree(m->gexp.bptr); cudaFree(m->gexp.bcol); cudaFree(m->gexp.brow); cudaFree(m->gexp.out); cudaFree(m->gexp.bw);
     delete m->gh;
     delete m;
@@ -380,6 +381,7 @@ int fe_set_variant(fe_mesh* m, int variant)
 // one fused operator launch: Y = mu (alpha (S sum_e P_e^T y_e - (c + eps) X) + beta Z)
 static int general_step(fe_mesh* m, const double* X, const double* Z, double* Y, int B, const double* eps,
                         double alpha, double beta, double c, cudaStream_t st);
+static int general_expand(fe_mesh* m, const double* X, int B, cudaStream_t st);
 
 static int operator_step(fe_mesh* m, const double* X, const double* Z, double* Y, int B, const double* eps,
                          double alpha, double beta, double c, cudaStream_t st)
@@ -546,6 +548,26 @@ int fe_get_constraints(const fe_mesh* m, int64_t* row_ptr, int32_t* col, double*
     return FE_OK;
 }
 
+// hanging values X_h = C_h (s . X) of a block into the handle's scratch (grown to B columns on demand)
+static int general_expand(fe_mesh* m, const double* X, int B, cudaStream_t st)
+{
+    const GeneralHost& g = *m->gh;
+    const long long nh = g.N_all - g.N;
+    if (nh <= 0) return FE_OK;
+    if (m->hcap < B) {
+        cudaFree(m->d_Xh); cudaFree(m->d_Yh);
+        m->d_Xh = m->d_Yh = nullptr; m->hcap = 0;
+        CUDA_TRY(cudaMalloc((void**)&m->d_Xh, (size_t)nh * B * sizeof(double)));
+        CUDA_TRY(cudaMalloc((void**)&m->d_Yh, (size_t)nh * B * sizeof(double)));
+        m->hcap = B;
+    }
+    k_gen_rows_times_block<<<m->sms * 8, dim3(32, kGenRows), 0, st>>>(m->d_Xh, X, m->gexp.bptr, m->gexp.bcol, m->gexp.bw, m->gexp.brow,
+                                                                      m->gexp.out, m->gexp.nb, B, 1.0, 0);
+    CUDA_TRY(cudaGetLastError());
+    m->launches += 1;
+    return FE_OK;
+}
+
 // one fused operator step on a general mesh: diagonal terms (k_gen_init), expansion of the hanging values, the cell kernel,
 // the transposed expansion
 static int general_step(fe_mesh* m, const double* X, const double* Z, double* Y, int B, const double* eps,
@@ -553,24 +575,15 @@ static int general_step(fe_mesh* m, const double* X, const double* Z, double* Y,
 {
     const GeneralHost& g = *m->gh;
     const long long nh = g.N_all - g.N;
-    if (nh > 0 && m->hcap < B) {
-        cudaFree(m->d_Xh); cudaFree(m->d_Yh);
-        m->d_Xh = m->d_Yh = nullptr; m->hcap = 0;
-        CUDA_TRY(cudaMalloc((void**)&m->d_Xh, (size_t)nh * B * sizeof(double)));
-        CUDA_TRY(cudaMalloc((void**)&m->d_Yh, (size_t)nh * B * sizeof(double)));
-        m->hcap = B;
-    }
+    int rc = general_expand(m, X, B, st);
+    if (rc) return rc;
     const int grid = m->sms * 8;
     const dim3 rows(32, kGenRows);
     if (!Z && !eps && c == 0.0)  // plain apply: nothing diagonal to write, Y is just cleared
         CUDA_TRY(cudaMemsetAsync(Y, 0, (size_t)g.N * B * sizeof(double), st));
     else
         k_gen_init<<<grid, rows, 0, st>>>(Y, X, Z, m->d_sm, eps, alpha, beta, c, g.N, B);
-    if (nh > 0) {
-        CUDA_TRY(cudaMemsetAsync(m->d_Yh, 0, (size_t)nh * B * sizeof(double), st));
-        k_gen_rows_times_block<<<grid, rows, 0, st>>>(m->d_Xh, X, m->gexp.bptr, m->gexp.bcol, m->gexp.bw, m->gexp.brow, m->gexp.out,
-                                                      m->gexp.nb, B, 1.0, 0);
-    }
+    if (nh > 0) CUDA_TRY(cudaMemsetAsync(m->d_Yh, 0, (size_t)nh * B * sizeof(double), st));
     GenParams prm;
     memset(&prm, 0, sizeof(prm));
     prm.X = X; prm.Xh = m->d_Xh ? m->d_Xh : X; prm.Y = Y; prm.Yh = m->d_Yh ? m->d_Yh : Y; prm.sc = m->d_gsc; prm.l2g = m->d_gl2g;
@@ -582,7 +595,7 @@ static int general_step(fe_mesh* m, const double* X, const double* Z, double* Y,
         k_gen_collapse<<<grid, rows, 0, st>>>(Y, m->d_Yh, m->gexp.bptr, m->gexp.bcol, m->gexp.bw, m->gexp.brow, m->gexp.out, m->gexp.nb, B,
                                               alpha);
     CUDA_TRY(cudaGetLastError());
-    m->launches += nh > 0 ? 4 : 2;
+    m->launches += nh > 0 ? 3 : 2;
     return FE_OK;
 }
 
@@ -1013,9 +1026,49 @@ __global__ void k_nonzero_to_one(double* __restrict__ a, long long n)
         a[i] = a[i] != 0.0 ? 1.0 : 0.0;
 }
 
+// general mesh (reading R27): Minv_i = M_c,ii / d_i with d_i = kd_i + sum_h C_hi^2 kd_h, kd the diagonal of the assembled
+// kinetic matrix 1/2 K over all nodes -- the diagonal of C^T (1/2 K) C without the couplings between hanging nodes
+static int ensure_minres_tables_general(fe_mesh* m)
+{
+    const GeneralHost& g = *m->gh;
+    const int n = m->n;
+    GenDiagTables tb;
+    memset(&tb, 0, sizeof(tb));
+    for (int q = 0; q < n; ++q)
+        for (int a = 0; a < n; ++a) {
+            tb.Nt[q * n + a] = m->tab.N[q * n + a];
+            double d = 0.0;
+            for (int r = 0; r < n; ++r) d += m->tab.D[q * n + r] * m->tab.N[r * n + a];  // l_a'(gl_q)
+            tb.DNt[q * n + a] = d;
+        }
+    double* d_kd = nullptr;
+    CUDA_TRY(cudaMalloc((void**)&d_kd, (size_t)g.N_all * sizeof(double)));
+    cudaError_t ce = cudaMemset(d_kd, 0, (size_t)g.N_all * sizeof(double));
+    std::vector<double> kd((size_t)g.N_all), minv((size_t)g.N), mask((size_t)g.N);
+    if (ce == cudaSuccess) {
+        k_gen_kinetic_diag<<<m->sms * 8, 256>>>(d_kd, m->d_gmetric, m->d_gl2g, m->ncells, n, gen_rec_doubles(n), tb);
+        ce = cudaMemcpy(kd.data(), d_kd, kd.size() * sizeof(double), cudaMemcpyDeviceToHost);
+    }
+    cudaFree(d_kd);
+    if (ce != cudaSuccess) return fail(FE_ERR_CUDA, "fe_minres_shifted: building the preconditioner failed: %s", cudaGetErrorString(ce));
+    m->launches += 1;
+    std::vector<double> d(kd.begin(), kd.begin() + g.N);
+    for (int64_t r = 0; r < g.N_all - g.N; ++r)
+        for (int64_t k = g.crow[r]; k < g.crow[r + 1]; ++k) d[g.ccol[k]] += g.cval[k] * g.cval[k] * kd[g.N + r];
+    for (int64_t i = 0; i < g.N; ++i) {
+        mask[i] = g.mask[i] ? 1.0 : 0.0;
+        minv[i] = g.mask[i] ? g.mass[i] / d[i] : 0.0;
+    }
+    int rc;
+    if ((rc = upload(&m->d_minv, minv)) || (rc = upload(&m->d_mask, mask))) return rc;
+    CUDA_TRY(cudaMalloc((void**)&m->d_scal, (20 * 128 + 2) * sizeof(double)));
+    return FE_OK;
+}
+
 static int ensure_minres_tables(fe_mesh* m)
 {
     if (m->d_minv) return FE_OK;
+    if (m->kind) return ensure_minres_tables_general(m);
     std::vector<double> k[3], md[3];
     axis_diagonals(m, m->xe, m->cx, k[0], md[0]);
     axis_diagonals(m, m->ye, m->cy, k[1], md[1]);
@@ -1047,7 +1100,6 @@ int fe_minres_shifted(fe_mesh* m, const double* G, double* X, int B, const doubl
                       int precondition, double* relres_host, int* iters_host, double* work, void* cuda_stream)
 {
     if (!m || !G || !X || !work) return fail(FE_ERR_INVALID, "fe_minres_shifted: NULL argument");
-    if (m->kind) return fail(FE_ERR_INVALID, "fe_minres_shifted: not available on general meshes");
     if (B < 1 || B > 128) return fail(FE_ERR_INVALID, "fe_minres_shifted: B=%d outside 1..128", B);
     if (maxit < 1 || !(tol >= 0.0)) return fail(FE_ERR_INVALID, "fe_minres_shifted: need maxit >= 1 and tol >= 0");
     if (!m->have_V) return fail(FE_ERR_STATE, "fe_minres_shifted: call fe_set_potential first");
@@ -1141,7 +1193,20 @@ int fe_gram(fe_mesh* m, const double* A, const double* Bm, int B, double* C_host
 int fe_density(fe_mesh* m, const double* X, int B, const double* f_dev, double* rho_dev, void* cuda_stream)
 {
     if (!m || !X || !f_dev || !rho_dev) return fail(FE_ERR_INVALID, "fe_density: NULL argument");
-    if (m->kind) return fail(FE_ERR_INVALID, "fe_density: not available on general meshes");
+    if (m->kind) {  // general mesh: expansion of the hanging values, then gather + interpolation + f psi^2 (fe_general.cuh)
+        CUDA_TRY(cudaSetDevice(m->device));
+        cudaStream_t gst = (cudaStream_t)cuda_stream;
+        int rcg = general_expand(m, X, B, gst);
+        if (rcg) return rcg;
+        GenDensityParams gp;
+        memset(&gp, 0, sizeof(gp));
+        gp.X = X; gp.Xh = m->d_Xh ? m->d_Xh : X; gp.f = f_dev; gp.rho = rho_dev; gp.l2g = m->d_gl2g; gp.sc = m->d_gsc;
+        gp.N = m->N; gp.B = B; gp.eoN = m->eoN;
+        CUDA_TRY(cudaMemsetAsync(rho_dev, 0, (size_t)m->ncells * m->nc * sizeof(double), gst));
+        CUDA_TRY(launch_density_gen(gp, m->p, m->ncells, gst));
+        m->launches += 1;
+        return FE_OK;
+    }
     if (B < 1) return fail(FE_ERR_INVALID, "fe_density: B=%d < 1", B);
     CUDA_TRY(cudaSetDevice(m->device));
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -1287,7 +1352,26 @@ int cheb_filter_host(fe_mesh* m, double* X_host, int B, int deg, double a, doubl
 int fe_apply_potential(fe_mesh* m, const double* Uq_dev, const double* X, double* Y, int B, void* cuda_stream)
 {
     if (!m || !Uq_dev || !X || !Y) return fail(FE_ERR_INVALID, "fe_apply_potential: NULL argument");
-    if (m->kind) return fail(FE_ERR_INVALID, "fe_apply_potential: not available on general meshes");
+    if (m->kind) {  // general mesh: the operator step on a scratch record array whose metric fields are 0 and whose WV is w |J| U
+        if (!m->have_V) return fail(FE_ERR_STATE, "fe_apply_potential: call fe_set_potential first");
+        const size_t lenk = (size_t)m->N * B;
+        if (overlap(X, lenk, Y, lenk)) return fail(FE_ERR_INVALID, "fe_apply_potential: X and Y overlap");
+        CUDA_TRY(cudaSetDevice(m->device));
+        cudaStream_t gst = (cudaStream_t)cuda_stream;
+        const int grec = gen_rec_doubles(m->n);
+        if (!m->d_grecU) {
+            CUDA_TRY(cudaMalloc((void**)&m->d_grecU, (size_t)m->ncells * grec * sizeof(double)));
+            CUDA_TRY(cudaMemset(m->d_grecU, 0, (size_t)m->ncells * grec * sizeof(double)));
+        }
+        k_gen_weight_potential<<<m->sms * 8, 256, 0, gst>>>(m->d_grecU, Uq_dev, m->d_gwdet, m->ncells, m->nc, grec);
+        CUDA_TRY(cudaGetLastError());
+        m->launches += 1;
+        double* keep = m->d_gmetric;
+        m->d_gmetric = m->d_grecU;
+        const int rcg = general_step(m, X, nullptr, Y, B, nullptr, 1.0, 0.0, 0.0, gst);
+        m->d_gmetric = keep;
+        return rcg;
+    }
     if (B < 1) return fail(FE_ERR_INVALID, "fe_apply_potential: B=%d < 1", B);
     const size_t len = (size_t)m->N * B;
     if (overlap(X, len, Y, len)) return fail(FE_ERR_INVALID, "fe_apply_potential: X and Y overlap");

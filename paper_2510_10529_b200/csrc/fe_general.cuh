@@ -146,6 +146,34 @@ k_gen_collapse(double* __restrict__ Y, const double* __restrict__ Yh, const long
     }
 }
 
+// diagonal of the assembled kinetic matrix over ALL nodes (MINRES preconditioner, l.225): kd[g] += sum_q grad^ Phi_a(q)^T G_q
+// grad^ Phi_a(q), one thread per (cell, local node), an explicit loop over the cell's quadrature points (setup, not hot).
+// Nt[q*n+a] = l_a(gl_q), DNt[q*n+a] = l_a'(gl_q).
+struct GenDiagTables {
+    double Nt[81], DNt[81];
+};
+__global__ void k_gen_kinetic_diag(double* __restrict__ kd, const double* __restrict__ rec, const int32_t* __restrict__ l2g,
+                                   long long ncells, int n, int grec, const __grid_constant__ GenDiagTables tb)
+{
+    const int n3 = n * n * n;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < ncells * n3; i += (long long)gridDim.x * blockDim.x) {
+        const long long e = i / n3;
+        const int a = (int)(i - e * n3), ax = a % n, ay = (a / n) % n, az = a / (n * n);
+        const double* M = rec + e * grec;
+        double sum = 0.0;
+        for (int qz = 0; qz < n; ++qz)
+            for (int qy = 0; qy < n; ++qy)
+                for (int qx = 0; qx < n; ++qx) {
+                    const int q = qx + n * (qy + n * qz);
+                    const double lx = tb.Nt[qx * n + ax], ly = tb.Nt[qy * n + ay], lz = tb.Nt[qz * n + az];
+                    const double dx = tb.DNt[qx * n + ax] * ly * lz, dy = lx * tb.DNt[qy * n + ay] * lz, dz = lx * ly * tb.DNt[qz * n + az];
+                    sum += M[q] * dx * dx + M[3 * n3 + q] * dy * dy + M[5 * n3 + q] * dz * dz +
+                           2.0 * (M[n3 + q] * dx * dy + M[2 * n3 + q] * dx * dz + M[4 * n3 + q] * dy * dz);
+                }
+        atomicAdd(kd + l2g[i], sum);
+    }
+}
+
 // per-cell record of the general kernel: 7 fields of n^3 doubles (6 metric entries, WV), padded to a multiple of 16 bytes
 inline int gen_rec_doubles(int n) { const int r = 7 * n * n * n; return r + (r & 1); }
 
@@ -457,6 +485,117 @@ __global__ void __launch_bounds__(GenShape<P>::LS * BT, MINB) k_apply_gen(const 
     }
     double* Fr = F0; F0 = F1; F1 = F2; F2 = Fr;  // the field that holds the next unit's rows becomes F0
     }  // units
+}
+
+// Electron density at the quadrature points on a general mesh (Eq. 4 l.73-77): rho[e][q] = sum_j f_j psi_j(x_q)^2 with
+// psi = M_c^{-1/2} psi~ expanded through the constraints -- the gather and the three interpolation sweeps of k_apply_gen,
+// then f_j U^2 summed over the BT vectors of the tile (shuffles inside the lane group) and added to rho.
+struct GenDensityParams {
+    const double* X;
+    const double* Xh;
+    const double* f;
+    double* rho;
+    const int32_t* l2g;
+    const double* sc;
+    long long N;
+    int B;
+    EOTab eoN;
+};
+
+template <int P, int BT, int MINB>
+__global__ void __launch_bounds__(GenShape<P>::LS * BT, MINB) k_density_gen(const __grid_constant__ GenDensityParams prm)
+{
+    constexpr int n = P + 1, n2 = n * n, n3 = n * n * n, LS = GenShape<P>::LS;
+    constexpr int SX = BT, SY = n * BT, SZ = n2 * BT;
+    extern __shared__ __align__(128) double smem[];
+    double* F0 = smem;
+    double* sSc = F0 + (size_t)n3 * BT;
+    int32_t* sId = reinterpret_cast<int32_t*>(sSc + n3 + (n3 & 1));
+    const int lane = threadIdx.x, slot = threadIdx.y, tid = slot * BT + lane;
+    const long long cell = blockIdx.x;
+    const int j = blockIdx.y * BT + lane;
+    const bool act = j < prm.B;
+    const long long B = prm.B;
+    double t[n], o[n];
+    for (int a = tid; a < n3; a += LS * BT) {
+        sId[a] = prm.l2g[cell * n3 + a];
+        sSc[a] = prm.sc[cell * n3 + a];
+    }
+    __syncthreads();
+    for (int a = slot; a < n3; a += LS) {
+        const long long g = sId[a];
+        const double* src = g < prm.N ? prm.X + g * B + j : prm.Xh + (g - prm.N) * B + j;
+        cp_async8(F0 + (size_t)a * BT + lane, act ? src : prm.X, act);
+    }
+    cp_async_commit();
+    cp_async_wait_all();
+    __syncthreads();
+    for (int l = slot; l < n2; l += LS) {  // x-lines: scale, interpolate
+        double* f = F0 + (size_t)l * n * BT + lane;
+#pragma unroll
+        for (int k = 0; k < n; ++k) {
+            const double sg = sSc[l * n + k];
+            t[k] = sg != 0.0 ? sg * f[k * SX] : 0.0;
+        }
+        mat1d_eo<n>(prm.eoN, t, o);
+#pragma unroll
+        for (int k = 0; k < n; ++k) f[k * SX] = o[k];
+    }
+    __syncthreads();
+    for (int l = slot; l < n2; l += LS) {  // y-lines
+        double* f = F0 + ((size_t)(l / n) * n2 + (l % n)) * BT + lane;
+#pragma unroll
+        for (int k = 0; k < n; ++k) t[k] = f[k * SY];
+        mat1d_eo<n>(prm.eoN, t, o);
+#pragma unroll
+        for (int k = 0; k < n; ++k) f[k * SY] = o[k];
+    }
+    __syncthreads();
+    const double fj = act ? prm.f[j] : 0.0;
+    for (int l = slot; l < n2; l += LS) {  // z-lines (qx, qy) = (l % n, l / n): psi at the Gauss points, squared and summed
+        const double* f = F0 + (size_t)l * BT + lane;
+#pragma unroll
+        for (int k = 0; k < n; ++k) t[k] = f[k * SZ];
+        mat1d_eo<n>(prm.eoN, t, o);
+        const unsigned peers = __activemask();  // the lane groups of this warp that have a line in this round
+#pragma unroll
+        for (int k = 0; k < n; ++k) {
+            double v = fj * o[k] * o[k];
+#pragma unroll
+            for (int d = BT / 2; d > 0; d >>= 1) v += __shfl_xor_sync(peers, v, d, BT);
+            if (lane == 0) atomicAdd(prm.rho + cell * n3 + (size_t)k * n2 + l, v);
+        }
+    }
+}
+
+template <int P, int BT, int MINB>
+cudaError_t launch_density_gen_t(const GenDensityParams& prm, long long ncells, cudaStream_t st)
+{
+    constexpr int n3 = (P + 1) * (P + 1) * (P + 1);
+    constexpr size_t smem = (size_t)n3 * BT * sizeof(double) + (size_t)(n3 + 1) * (sizeof(double) + sizeof(int32_t)) + 16;
+    static PerDeviceOnce once;
+    cudaError_t e0 = once_per_device(once, [&] {
+        return cudaFuncSetAttribute(k_density_gen<P, BT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    });
+    if (e0 != cudaSuccess) return e0;
+    dim3 grid((unsigned)ncells, (unsigned)((prm.B + BT - 1) / BT)), block(BT, GenShape<P>::LS);
+    k_density_gen<P, BT, MINB><<<grid, block, smem, st>>>(prm);
+    return cudaGetLastError();
+}
+
+inline cudaError_t launch_density_gen(const GenDensityParams& prm, int p, long long ncells, cudaStream_t st)
+{
+    switch (p) {
+        case 1: return launch_density_gen_t<1, 32, 8>(prm, ncells, st);
+        case 2: return launch_density_gen_t<2, 32, 6>(prm, ncells, st);
+        case 3: return launch_density_gen_t<3, 32, 4>(prm, ncells, st);
+        case 4: return launch_density_gen_t<4, 32, 2>(prm, ncells, st);
+        case 5: return launch_density_gen_t<5, 16, 2>(prm, ncells, st);
+        case 6: return launch_density_gen_t<6, 16, 2>(prm, ncells, st);
+        case 7: return launch_density_gen_t<7, 8, 2>(prm, ncells, st);
+        case 8: return launch_density_gen_t<8, 8, 2>(prm, ncells, st);
+    }
+    return cudaErrorInvalidValue;
 }
 
 template <int P, int BT, int MINB, bool PERSIST>

@@ -171,3 +171,56 @@ def test_refinement_improves_the_oscillator_ground_state():
         errs.append((abs(lam[0] - 1.5), np.abs(lam[1:4] - 2.5).max()))
     assert errs[1][0] < 0.25 * errs[0][0] and errs[1][1] < 0.5 * errs[0][1]
     assert errs[1][0] < 2e-3
+
+
+def test_density_preconditioner_and_potential_apply_on_constrained_meshes():
+    """(i) unrefined mesh: the general preconditioner equals the tensor oracle's (diag of the potential-free operator);
+    (ii) refined sheared mesh, a polynomial field of degree <= p sampled at the unconstrained nodes: the hanging values
+    reproduce it, so rho(x_q) = f poly(x_q)^2 in closed form and sum_q w|J| rho = the exactly known integral is matched by
+    the weights; (iii) potential_apply through its weak form: v^T (C^T M_U C) u = sum_q w|J| U u v for polynomial u, v;
+    (iv) the preconditioner is positive on free rows."""
+    xe, ye, ze = np.array([0.0, 0.7, 2.0]), np.array([-1.0, -0.5, 0.4, 1.0]), np.array([0.0, 0.3, 1.0])
+    p = 3
+    g0 = oracle.GeneralOracleMesh(workloads.octree_mesh(xe, ye, ze, lambda l, lo, hi: False, 0), p)
+    t0 = oracle.OracleMesh(xe, ye, ze, p)
+    perm = np.empty(t0.N, dtype=np.int64)
+    perm[t0.l2g().reshape(-1)] = g0.l2g().reshape(-1)
+    t0.set_potential(np.zeros(t0.ncells * t0.nq3))
+    assert np.max(np.abs(g0.laplacian_precond()[perm] - oracle.laplacian_precond(t0))) < 1e-12
+    mesh, g = _refined(p, _affine(SHEAR), 1)
+    xyz = g.node_coords()[:g.N]
+    free = g.mask().astype(bool)
+    poly = lambda x: 0.3 + x[:, 0] - 0.5 * x[:, 1] * x[:, 2] + 0.25 * x[:, 0] ** 2 * x[:, 2]  # degree <= 3 per variable
+    # psi~ = M_c^{1/2} psi with psi the polynomial; Dirichlet rows carry the polynomial too but are ignored by the density
+    sq = np.sqrt(g.mass())
+    X = np.stack([poly(xyz) * sq, (0.2 - xyz[:, 1]) * sq], axis=1)
+    # the density ignores Dirichlet rows; compare only in cells that do not touch the boundary
+    rho = g.density(X, np.array([2.0, 1.0]))
+    q = g.quad_coords().reshape(g.ncells, -1, 3)
+    touches = np.array([not free[g.l2g()[e][g.l2g()[e] < g.N]].all() for e in range(g.ncells)])
+    ref = 2.0 * poly(q.reshape(-1, 3)) ** 2 + (0.2 - q.reshape(-1, 3)[:, 1]) ** 2
+    ref = ref.reshape(g.ncells, -1)
+    inner = ~touches
+    assert inner.sum() >= 8
+    assert np.max(np.abs(rho[inner] - ref[inner])) < 1e-11 * np.abs(ref).max()
+    Mi = g.laplacian_precond()
+    assert np.all(Mi[free] > 0) and np.all(Mi[~free] == 0)
+    # weak form of the potential-only operator with U = 1 + x: v^T S^-1 [S C^T M_U C S] S^-1 u over interior-supported u, v
+    U = 1.0 + q.reshape(-1, 3)[:, 0]
+    u = np.where(free, poly(xyz), 0.0)
+    Y = g.potential_apply(U, (u * sq)[:, None])[:, 0]
+    # bilinear form with v = u: u^T C^T M_U C u = sum over cells of quadrature of U (u_h)^2, u_h = the FE interpolant of u
+    u_all = g.Cfull @ u
+    n = p + 1
+    x1, _ = oracle.gll(p)
+    xq, wq = oracle.gauss(n)
+    L1 = np.array([[oracle.lagrange(x1, a, xq[k]) for a in range(n)] for k in range(n)])
+    total = 0.0
+    for e in range(g.ncells):
+        loc = u_all[g.l2g()[e]].reshape(n, n, n)
+        val = np.einsum("ra,sb,tc,cba->rst", L1, L1, L1, loc).transpose(2, 1, 0).reshape(-1)
+        V = mesh.verts[e]
+        det = abs(np.linalg.det(np.stack([(V[1] - V[0]) / 2, (V[2] - V[0]) / 2, (V[4] - V[0]) / 2], axis=1)))
+        w3 = np.array([wq[a] * wq[b] * wq[c] for c in range(n) for b in range(n) for a in range(n)])
+        total += np.sum(w3 * det * U.reshape(g.ncells, -1)[e] * val ** 2)
+    assert abs(u @ (Y * sq) - total) < 1e-11 * abs(total)

@@ -145,13 +145,54 @@ def test_unrefined_box_mesh_agrees_with_the_tensor_product_path():
     assert np.linalg.norm(Yg - Yt) <= 1e-13 * np.linalg.norm(Yt)
 
 
-def test_general_handle_rejects_unsupported_calls():
-    import paper_2510_10529_b200 as fe
-    e = workloads.uniform_edges(-1.0, 1.0, 2)
-    gm = fe.FEMesh.general(workloads.octree_mesh(e, e, e, lambda l, lo, hi: False, 0), 2)
-    gm.set_potential(np.zeros(gm.ncells * gm.nq3))
-    X = torch.zeros(gm.N, 2, dtype=torch.float64, device="cuda")
-    with pytest.raises(fe.FEError):
-        gm.minres_shifted(X, None, maxit=2)
-    with pytest.raises(fe.FEError):
-        gm.density(X, torch.ones(2, dtype=torch.float64, device="cuda"))
+@pytest.mark.parametrize("precondition", [False, True])
+def test_block_minres_on_a_hanging_node_mesh(precondition):
+    """fe_minres_shifted (l.221-225) on a refined, smoothly deformed mesh: the same Paige-Saunders iteration as the oracle's,
+    compared after a fixed 25 steps (<= 1e-9) and at convergence through the true residual with the oracle's operator; the
+    preconditioner of reading R27 against the oracle's (through the iterates: both sides build their own)."""
+    import oracle
+    e = workloads.uniform_edges(-1.5, 1.5, 3)
+    mesh = workloads.octree_mesh(e, e, e, lambda l, lo, hi: np.linalg.norm((lo + hi) / 2) < 0.9, 1, _wave)
+    om, gm = _pair(mesh, 3, _coulomb)
+    mask = om.mask()
+    free = mask.astype(bool)
+    B = 6
+    G = workloads.random_block(1900, om.N, B)  # Dirichlet rows hold data that must be ignored
+    eps = workloads.shifts(2900, B)
+    Mi = om.laplacian_precond() if precondition else None
+    Xo, relo, ito = oracle.minres_shifted(om, G, eps, maxit=25, tol=0.0, Minv=Mi)
+    Xg, relg, itg = gm.minres_shifted(_dev(G), _dev(eps), maxit=25, tol=0.0, precondition=precondition)
+    Xg = Xg.cpu().numpy()
+    assert itg == 25 and ito == 25
+    assert _relerr(Xg, Xo, mask) <= 1e-9
+    assert np.max(np.abs(relg - relo)) <= 1e-9
+    assert np.all(Xg[~free] == 0)
+    Xc, relc, itc = gm.minres_shifted(_dev(G), _dev(eps), maxit=4000, tol=1e-9, precondition=precondition)
+    R = (om.apply(Xc.cpu().numpy(), eps) - G * mask[:, None])[free]
+    assert np.all(relc <= 1e-9) and itc < 4000
+    assert np.linalg.norm(R) <= 1e-6 * np.linalg.norm(G[free])
+    if precondition:
+        _, _, it_plain = gm.minres_shifted(_dev(G), _dev(eps), maxit=4000, tol=1e-9, precondition=False)
+        assert itc < it_plain
+
+
+@pytest.mark.parametrize("p,B", [(1, 3), (2, 8), (3, 33), (4, 20), (6, 9), (7, 12), (8, 5)])
+def test_density_and_potential_apply_on_a_hanging_node_mesh(p, B):
+    """fe_density (Eq. 4) and fe_apply_potential (the integral of Eq. 18) on a refined, smoothly deformed mesh against the
+    oracle's definitions: several vector tiles, ragged tails, data in the Dirichlet rows; the operator set by
+    fe_set_potential is untouched afterwards."""
+    e = workloads.uniform_edges(-1.5, 1.5, 3)
+    mesh = workloads.octree_mesh(e, e, e, lambda l, lo, hi: np.linalg.norm((lo + hi) / 2) < 0.9, 1, _wave)
+    om, gm = _pair(mesh, p, _coulomb)
+    mask = om.mask()
+    X = workloads.random_block(2000 + p, om.N, B)
+    f = 2.0 * workloads.uniform01(2001 + p, 0, B)
+    rho_o = om.density(X, f).reshape(-1)
+    rho_g = gm.density(_dev(X), _dev(f)).cpu().numpy()
+    assert np.linalg.norm(rho_g - rho_o) <= 1e-12 * np.linalg.norm(rho_o)
+    Uq = np.cos(om.quad_coords()).prod(axis=1) - 0.3
+    Yo = om.potential_apply(Uq, X * mask[:, None])
+    Yg = gm.apply_potential(_dev(Uq), _dev(X)).cpu().numpy()
+    assert _relerr(Yg, Yo, mask) <= TOL_APPLY
+    assert np.all(Yg[mask == 0] == 0)
+    assert _relerr(gm.apply_H(_dev(X)).cpu().numpy(), om.apply(X), mask) <= TOL_APPLY
