@@ -33,7 +33,7 @@ struct TmaParams {
     CUtensorMap mWp1;  // W : box (BT,p,p,1), store of beta' X
     const double* eps;
     double* dots;       // DOTS kernels: dots[j] += sum_g X[g,j] Y_contribution[g,j], the column-wise x . (H~ - eps_j) x of a plain apply
-    const double* rec;  // cells * REC: per-cell record  VZ = V_q hz^2/2 [qx][qy][NP] | s_g [az][ay][NP] | kz s_g | ky/kx, kx/kz
+    const double* rec;  // cells * REC: per-cell record  VZ = V_q hz^2/2 [qx][qy][NP] | s_g [az][ay][NP] | ky/kx, kx/kz, kz | kz s_g
     int B, cx, cy, cz;
     int owner, preinit;
     int blk;   // block edge T of the walk order (walk_cell), a divisor of cy and cz
@@ -102,30 +102,37 @@ template <int n>
 struct TmaShape {
     static constexpr int NP = n + (n & 1);  // rows of the small tiles padded to an even length (16-byte LDS.128)
     static constexpr int SMALL = n * n * NP;
-    // per-cell record in global memory, brought in by ONE bulk copy per unit: VZ | s_g | kz s_g | ry, rxz, pad
+    // per-cell record in global memory, brought in by ONE bulk copy per unit: VZ | s_g | ry, rxz, kz, pad | kz s_g
     static constexpr int REC = 3 * SMALL + 8;
+    static constexpr int TAIL = 2 * SMALL, SOUT = 2 * SMALL + 8;
+    static constexpr int REC_SLIM = 2 * SMALL + 8;  // SLIM kernels leave the kz s_g tile out and multiply by kz instead
 };
 
-template <int P, int BT>
+template <int P, int BT, bool SLIM = false>
 constexpr size_t tma_smem_bytes()
 {
     constexpr int n = P + 1;
+    if (SLIM) return ((size_t)2 * n * n * n * BT + TmaShape<n>::REC_SLIM) * sizeof(double) + 16;
     return ((size_t)2 * n * n * n * BT + 2 * TmaShape<n>::REC + n * BT) * sizeof(double) + 16;
 }
 
 // FIRST: X is caller data whose Dirichlet rows may hold anything (R5) -> mask them in the owner / pre-init terms.
 // DOTS: also accumulate the column-wise inner products x_j . y_j of input and result (MINRES alpha, l.221-225) from
 // cell-local terms: x^T y_e = kz U^T T at the Gauss points of the line phase, plus the owner term kappa_j x^2.
-template <int P, int BT, int MINB, bool FIRST, bool PERSIST, bool DOTS = false>
+// SLIM (one CTA per unit only): one record buffer without the kz s_g tile and no DOTS scratch, so that two 6-warp CTAs of
+// p = 5 fit one SM (12 warps, three per sub-partition, instead of one persistent CTA whose 6 warps sit 2,2,1,1).
+template <int P, int BT, int MINB, bool FIRST, bool PERSIST, bool DOTS = false, bool SLIM = false>
 __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_constant__ TmaParams prm)
 {
+    static_assert(!SLIM || (!PERSIST && !DOTS), "SLIM kernels run one unit and deliver no dots");
     constexpr int n = P + 1, n2 = n * n, n3 = n * n * n, NP = TmaShape<n>::NP, SMALL = TmaShape<n>::SMALL,
-                  REC = TmaShape<n>::REC;
+                  REC = SLIM ? TmaShape<n>::REC_SLIM : TmaShape<n>::REC, RECG = TmaShape<n>::REC,
+                  TAIL = TmaShape<n>::TAIL, SOUT = TmaShape<n>::SOUT;
     extern __shared__ __align__(128) double smem[];
     double* buf0 = smem;                // [n^3][BT]  bufA: X -> A (dead after pass 1 of the line phase) -> next unit's X
     double* buf1 = smem + n3 * BT;      // [n^3][BT]  bufB: owner term -> A2 -> R -> scaled output (source of the reduce-add)
     double* rec0 = buf1 + n3 * BT;      // two cell records (double-buffered like the tiles): VZ [qx][qy][NP],
-    double* rec1 = rec0 + REC;          //   s_g [az][ay][NP], kz s_g [az][ay][NP], {ky/kx, kx/kz}
+    double* rec1 = SLIM ? rec0 : rec0 + REC;  //   s_g [az][ay][NP], {ky/kx, kx/kz, kz}, kz s_g [az][ay][NP]
     unsigned long long* bar = (unsigned long long*)(rec1 + REC);  // bar[0]: tile + record landed; bar[1]: A consumed
     double* red = (double*)(bar + 2);   // [n][BT] DOTS: per-plane partial sums of the unit
     const int lane = threadIdx.x, pl = threadIdx.y, tid = pl * BT + lane;
@@ -143,7 +150,7 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
         const int cell = ex + prm.cx * (ey + prm.cy * ez);
         mbar_expect_tx(bar, (unsigned)((n3 * BT + REC) * sizeof(double)));
         tma_load4(buf0, &prm.mXn, (int)(u % nbt) * BT, ex * P, ey * P, ez * P, bar);
-        bulk_load(rec0, prm.rec + (size_t)cell * REC, (unsigned)(REC * sizeof(double)), bar);
+        bulk_load(rec0, prm.rec + (size_t)cell * RECG, (unsigned)(REC * sizeof(double)), bar);
     }
     __syncthreads();
     unsigned parity = 0;
@@ -168,8 +175,9 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
     parity ^= 1;
     const double* sVZ = rec;
     const double* sIn = rec + SMALL;
-    const double* sOut = rec + 2 * SMALL;
-    const double ry = rec[3 * SMALL], rxz = rec[3 * SMALL + 1];  // ky/kx = hx^2/hy^2, kx/kz = hz^2/hx^2
+    const double* sOut = SLIM ? sIn : rec + SOUT;
+    const double ry = rec[TAIL], rxz = rec[TAIL + 1];  // ky/kx = hx^2/hy^2, kx/kz = hz^2/hx^2
+    const double kzs = SLIM ? rec[TAIL + 2] : 1.0;     // SLIM: the output scale is kz times the gather scale
 
     double v[n][n], t[n], o[n];
     double dacc = 0.0;  // DOTS: this thread's share of x . y for vector j0 + lane
@@ -330,7 +338,7 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
                 v[qy][qz] = fma(rxz, lb[((qz * n + qy) * n) * BT], tn);
             }
         }
-        dacc = fma(rec[3 * SMALL + 2], fma(rxz, dq, ds), dacc);  // x^T y_e = kz U^T T
+        dacc = fma(rec[TAIL + 2], fma(rxz, dq, ds), dacc);  // x^T y_e = kz U^T T
         }
         // next-tile request, between passes 3 and 4 (measured: after pass 2 -0.7 %, after pass 4 -8 %: the tile must be
         // in flight for about a third of the unit).  The producer duty sits on warp 3: with 32-wide tiles warps map
@@ -344,7 +352,7 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
             mbar_wait(bar + 1, parity ^ 1);  // parity was flipped after this unit's tile wait
             mbar_expect_tx(bar, (unsigned)((n3 * BT + REC) * sizeof(double)));
             tma_load4(bufA, &prm.mXn, (int)(un % nbt) * BT, nx * P, ny * P, nz * P, bar);
-            bulk_load(recN, prm.rec + (size_t)cn * REC, (unsigned)(REC * sizeof(double)), bar);
+            bulk_load(recN, prm.rec + (size_t)cn * RECG, (unsigned)(REC * sizeof(double)), bar);
         }
         // pass 4: R = N'z^T T, into the lines of the A2 field this thread has just consumed
 #pragma unroll
@@ -374,7 +382,8 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
     for (int ay = 0; ay < n; ++ay) {
         mat1d_eo<n>(prm.eoNTa, v[ay], o);
 #pragma unroll
-        for (int ax = 0; ax < n; ++ax) pB[(ay * n + ax) * BT] = sout_pl[ay * NP + ax] * o[ax];
+        for (int ax = 0; ax < n; ++ax)
+            pB[(ay * n + ax) * BT] = (SLIM ? kzs * sout_pl[ay * NP + ax] : sout_pl[ay * NP + ax]) * o[ax];
         if (ay == H1 - 1 && H1 < n) {
             fence_async_smem();
             __syncwarp();
@@ -460,6 +469,28 @@ cudaError_t launch_tma(const TmaParams& prm, long long ncells, bool first, cudaS
     return cudaGetLastError();
 }
 
+// one SLIM CTA per unit (p = 5)
+template <int P, int BT, int MINB>
+cudaError_t launch_tma_slim(const TmaParams& prm, long long ncells, bool first, cudaStream_t st)
+{
+    constexpr int n = P + 1;
+    constexpr size_t smem = tma_smem_bytes<P, BT, true>();
+    static PerDeviceOnce once;
+    cudaError_t e0 = once_per_device(once, [&] {
+        cudaError_t e = cudaFuncSetAttribute(k_apply_tma<P, BT, MINB, true, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(k_apply_tma<P, BT, MINB, false, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        return e;
+    });
+    if (e0 != cudaSuccess) return e0;
+    dim3 grid((unsigned)(ncells * ((prm.B + BT - 1) / BT))), block(BT, n);
+    if (first)
+        k_apply_tma<P, BT, MINB, true, false, false, true><<<grid, block, smem, st>>>(prm);
+    else
+        k_apply_tma<P, BT, MINB, false, false, false, true><<<grid, block, smem, st>>>(prm);
+    return cudaGetLastError();
+}
+
 // Launch shape of the TMA kernel.  Variants: 0 = default, 5 = one CTA per unit everywhere, 6 = 32-wide box at p = 6 with
 // one CTA per unit, 7 = persistent everywhere, 8 = 32-wide persistent at p = 6 (= the default when B > 16).
 // p = 6 default: ONE persistent 7-warp CTA per SM walking (cell, 32 vectors) units.  Its warps run the same 74 KB of
@@ -480,6 +511,8 @@ inline cudaError_t launch_apply_tma(const TmaParams& prm, int p, long long ncell
     const bool one_cta = wide6 || p == 5 || p >= 7;
     if (!(variant == 7 || variant == 8 || (variant == 0 && one_cta))) sms = 0;
     if (wide6) return launch_tma<6, 32, 1>(prm, ncells, first, st, sms);
+    // p = 5 default: two one-unit SLIM CTAs per SM (variant 7 keeps the persistent CTA; the dots need the full kernel)
+    if (p == 5 && variant == 0 && !prm.dots) return launch_tma_slim<5, 32, 2>(prm, ncells, first, st);
     switch (p) {
         case 1: return launch_tma<1, 32, 8>(prm, ncells, first, st, sms);
         case 2: return launch_tma<2, 32, 6>(prm, ncells, first, st, sms);
@@ -509,8 +542,8 @@ __global__ void k_build_records(double* __restrict__ rec, int n, int cx, int cy,
         const double kz = 0.25 * hx[ex] * hy[ey] / hz[ez];  // 2J/hz^2, J = hx hy hz / 8
         double* r = rec + e * REC;
         r[SMALL + k] = s;
-        r[2 * SMALL + k] = kz * s;
-        if (k < 8) r[3 * SMALL + k] = k == 0 ? (hx[ex] * hx[ex]) / (hy[ey] * hy[ey]) : k == 1 ? (hz[ez] * hz[ez]) / (hx[ex] * hx[ex]) : k == 2 ? kz : 0.0;
+        r[2 * SMALL + 8 + k] = kz * s;
+        if (k < 8) r[2 * SMALL + k] = k == 0 ? (hx[ex] * hx[ex]) / (hy[ey] * hy[ey]) : k == 1 ? (hz[ez] * hz[ez]) / (hx[ex] * hx[ex]) : k == 2 ? kz : 0.0;
     }
 }
 

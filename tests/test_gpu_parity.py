@@ -493,10 +493,11 @@ BIG = (np.array([0.0, 0.5, 1.1, 1.5, 2.2, 2.6, 3.3]), np.array([-1.0, -0.6, 0.1,
        np.array([0.0, 0.4, 0.7, 1.3, 1.6, 2.1]))  # 6 x 6 x 5 = 180 unequal cells: more units than the 148 persistent CTAs
 
 
-@pytest.mark.parametrize("p,B,variant", [(5, 6, 0), (5, 34, 0), (7, 6, 0), (7, 34, 0), (8, 6, 0), (8, 34, 0), (6, 34, 0),
+@pytest.mark.parametrize("p,B,variant", [(5, 6, 0), (5, 34, 0), (5, 34, 7), (7, 6, 0), (7, 34, 0), (8, 6, 0), (8, 34, 0), (6, 34, 0),
                                          (2, 130, 7), (3, 130, 7), (4, 130, 7), (6, 34, 7), (6, 6, 8), (6, 34, 8), (6, 34, 6)])
 def test_persistent_loop_parity(p, B, variant):
-    """A mesh with more units than resident CTAs, so that every persistent CTA walks several units (bar[1] handshake,
+    """(p = 5, variant 0 is the two-CTAs-per-SM SLIM shape, one unit per CTA; variant 7 its persistent predecessor.)
+    A mesh with more units than resident CTAs, so that every persistent CTA walks several units (bar[1] handshake,
     rec / recN swap, mid-unit next-tile request, the BT = 16 shape with two planes per warp at p = 7, 8; B = 130 gives
     the several-CTAs-per-SM shapes of p <= 4 more units than their 888 / 592 / 444 resident CTAs).  One shifted
     apply: sampled rows against the oracle's entry-by-entry Eq. 17 and ALL rows against the colour-ordered legacy kernel
