@@ -405,7 +405,9 @@ def time_adaptive(fe, torch, dev, peaks, hbm_peak, steps, warmup, p=6, B=64, m=3
            "roofline": {"bound": "alu", "achieved": flops / dur / 1e12, "peak": peak, "unit": "TFLOP/s",
                         "frac": flops / dur / 1e12 / peak, "frac_of_nominal": flops / dur / 1e12 / FP64_NOMINAL_TFLOPS,
                         "kernel": "k_apply_gen<p=%d> + k_gen_init / k_gen_expand / k_gen_collapse (one operator step: step / m)" % p,
-                        "launch_ms": dur * 1e3, "algorithmic_bytes": alg_bytes, "traffic": None,
+                        "launch_ms": dur * 1e3, "algorithmic_bytes": alg_bytes, "traffic": 1.101e9 + 0.469e9,
+                        "traffic_source": "committed ncu capture profiles/r2_general_k_apply_gen.md (k_apply_gen alone, not "
+                                          "measured in this run)",
                         "hbm_frac_of_measured": (alg_bytes / dur / 1e9 / hbm_peak) if hbm_peak else None},
            "clocks": clocks, "gpu_launches": int(gm.launches - l0)}
     gm.close()
