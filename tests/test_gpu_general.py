@@ -66,6 +66,10 @@ def test_apply_refined_deformed_mesh_all_orders(p, B):
     Yg = gm.apply_H(_dev(X), eps=_dev(eps)).cpu().numpy()
     assert _relerr(Yg, om.apply(X, eps), mask) <= TOL_APPLY
     assert np.all(Yg[mask == 0] == 0)
+    Xbad = X.copy()
+    Xbad[mask == 0] = np.nan  # R5: even NaN in the Dirichlet rows (also those feeding hanging nodes) is ignored
+    Yg = gm.apply_H(_dev(Xbad)).cpu().numpy()
+    assert np.all(np.isfinite(Yg)) and _relerr(Yg, om.apply(X), mask) <= TOL_APPLY
 
 
 @pytest.mark.parametrize("p,B,deg", [(2, 8, 7), (4, 16, 10), (6, 6, 4)])

@@ -556,6 +556,35 @@ def test_adjoint_scratch_survives_host_filter():
         assert _relerr(G2, Go, mask) <= TOL_APPLY
 
 
+def test_nan_in_dirichlet_rows_is_ignored():
+    """R5: boundary rows of X are IGNORED -- even NaN / Inf there (an uninitialised block) must not reach any free node, in
+    fe_apply_H (both kernel generations), cheb_filter, fe_density and fe_apply_potential."""
+    om, gm = _pair(UNEQUAL, 4, _coulomb)
+    mask = om.mask()
+    B = 6
+    X = workloads.random_block(1500, om.N, B, mask)
+    Xbad = X.copy()
+    bnd = np.flatnonzero(mask == 0)
+    Xbad[bnd[0::3]] = np.nan
+    Xbad[bnd[1::3]] = np.inf
+    Xbad[bnd[2::3]] = -np.inf
+    Yo = om.apply(X)
+    for variant in (0, 3):
+        gm.set_variant(variant)
+        Yg = gm.apply_H(_dev(Xbad)).cpu().numpy()
+        assert np.all(np.isfinite(Yg)) and _relerr(Yg, Yo, mask) <= TOL_APPLY and np.all(Yg[mask == 0] == 0)
+        Fg = gm.cheb_filter(_dev(Xbad).clone(), 5, -2.0, 400.0, -12.0).cpu().numpy()
+        assert np.all(np.isfinite(Fg)) and _relerr(Fg, om.filter(X, 5, -2.0, 400.0, -12.0), mask) <= TOL_FILTER
+    gm.set_variant(0)
+    import oracle
+    f = np.ones(B)
+    rho = gm.density(_dev(Xbad), _dev(f)).cpu().numpy()
+    assert np.all(np.isfinite(rho)) and np.linalg.norm(rho - oracle.density(om, X, f).reshape(-1)) <= 1e-12 * np.linalg.norm(rho)
+    Uq = np.cos(om.quad_coords()).prod(axis=1)
+    G = gm.apply_potential(_dev(Uq), _dev(Xbad)).cpu().numpy()
+    assert np.all(np.isfinite(G))
+
+
 # ---- error behaviour -------------------------------------------------------------------------------------------------
 def test_error_codes():
     fe = _fe()
