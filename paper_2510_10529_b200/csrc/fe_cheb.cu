@@ -1128,10 +1128,18 @@ int fe_minres_shifted(fe_mesh* m, const double* G, double* X, int B, const doubl
     std::vector<double> phibar(B), beta1(B);
     int it = 0;
     bool done = false;
+    // the two blocks the apply alternates between: their tensor maps are encoded once, not every step
+    const bool tma = tma_eligible(m, B, Y, HY, eps_dev);
+    BlockMaps mapY, mapHY;
+    if (tma && ((rc = make_block_maps(&mapY, m, Y, B)) || (rc = make_block_maps(&mapHY, m, HY, B)))) return rc;
     while (it < maxit && !done) {
         k_minres_scalars<<<1, 128, 0, st>>>(q, B, 1, tol);
         // hy = (H~ - eps_j) y,  y = beta v, with dot_j = y_j . hy_j from the operator kernel
-        if ((rc = apply_into_cleared(m, Y, HY, B, eps_dev, q.dot, cuda_stream))) return rc;
+        if (tma)
+            rc = tma_step(m, mapY, mapHY, nullptr, B, eps_dev, 1.0, 0.0, eps_dev != nullptr, 0.0, true, st, q.dot);
+        else
+            rc = apply_into_cleared(m, Y, HY, B, eps_dev, q.dot, cuda_stream);
+        if (rc) return rc;
         k_minres_scalars<<<1, 128, 0, st>>>(q, B, 3, tol);
         k_minres_lanczos<<<grid, blk, 0, st>>>(HY, R1, R2, Minv, m->N, B, q.s, q.c1, q.c2, q.betasq, q.gamn);
         k_minres_scalars<<<1, 128, 0, st>>>(q, B, 2, tol);
@@ -1139,6 +1147,7 @@ int fe_minres_shifted(fe_mesh* m, const double* G, double* X, int B, const doubl
         CUDA_TRY(cudaGetLastError());
         m->launches += 5;
         std::swap(Y, HY);  // the preconditioned residual of this step is the next step's y
+        std::swap(mapY, mapHY);
         std::swap(R1, R2);
         std::swap(W1, W2);
         ++it;
