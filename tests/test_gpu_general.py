@@ -200,3 +200,39 @@ def test_density_and_potential_apply_on_a_hanging_node_mesh(p, B):
     assert _relerr(Yg, Yo, mask) <= TOL_APPLY
     assert np.all(Yg[mask == 0] == 0)
     assert _relerr(gm.apply_H(_dev(X)).cpu().numpy(), om.apply(X), mask) <= TOL_APPLY
+
+
+def test_adaptive_workload_full_size_properties():
+    """The adaptive-molecule workload bench.py times (4 066 leaves on three levels, p = 6, 857 011 unconstrained + 100 507
+    hanging nodes, B = 64), where the oracle's cell matrices are out of reach: (i) the operator is symmetric,
+    <X, H~Y> = <H~X, Y> column by column -- gather, constraint expansion, scatter and collapse are transposes of each other at
+    this size too; (ii) cheb_filter at the timed degree equals the three-term recurrence assembled from fe_apply_H calls,
+    which the small-mesh tests tie to the oracle; (iii) Dirichlet rows stay exactly 0."""
+    import paper_2510_10529_b200 as fe
+    mesh, V = workloads.adaptive_molecule()
+    gm = fe.FEMesh.general(mesh, 6)
+    assert gm.N_all > gm.N and gm.ncells == mesh.ncells
+    gm.set_potential(V(gm.quad_coords()))
+    B, m = 64, 30
+    mask = _dev(gm.mask().astype(np.float64))[:, None]
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(6100)
+    X = torch.randn(gm.N, B, dtype=torch.float64, device="cuda", generator=gen) * mask
+    Y = torch.randn(gm.N, B, dtype=torch.float64, device="cuda", generator=gen) * mask
+    HX, HY = gm.apply_H(X), gm.apply_H(Y)
+    lhs, rhs = (X * HY).sum(dim=0), (HX * Y).sum(dim=0)
+    scale = torch.sqrt((X * X).sum(dim=0) * (HY * HY).sum(dim=0))
+    assert float(((lhs - rhs).abs() / scale).max()) <= 1e-12
+    assert float((HX * (1 - mask)).abs().max()) == 0.0
+    a0, a, b = -40.0, 20.0, 4000.0
+    e, c = (b - a) / 2, (b + a) / 2
+    s1 = e / (a0 - c)
+    s = s1
+    Ykm, Yk = X, (s1 / e) * (gm.apply_H(X) - c * X)
+    for _ in range(1, m):
+        sn = 1.0 / (2.0 / s1 - s)
+        Ykm, Yk = Yk, (2 * sn / e) * (gm.apply_H(Yk) - c * Yk) - s * sn * Ykm
+        s = sn
+    Yf = gm.cheb_filter(X.clone(), m, a, b, a0)
+    assert float(torch.linalg.norm(Yf - Yk) / torch.linalg.norm(Yk)) <= 1e-12
+    assert float((Yf * (1 - mask)).abs().max()) == 0.0
