@@ -75,9 +75,12 @@ class GeneralOracleMesh:
             U = self._logical(e)
             l = int(lev[e])
             coarser = np.flatnonzero(lev < l)
+            if len(coarser):  # only coarser leaves whose closed box meets this cell's can contain one of its nodes
+                coarser = coarser[np.all((hi[coarser] >= lo[e] - 1e-12) & (lo[coarser] <= hi[e] + 1e-12), axis=1)]
+            keys = np.round(U * 2.0 ** 32).astype(np.int64).tolist()  # rounded logical coordinates of the cell's nodes
             for a in range(nc):
                 u = U[a]
-                key = (l,) + tuple(np.round(u * 2.0 ** 32).astype(np.int64))
+                key = (l, keys[a][0], keys[a][1], keys[a][2])
                 s = key_of.get(key)
                 if s is None:
                     parent = -1
@@ -259,6 +262,38 @@ class GeneralOracleMesh:
             Y = Y - Xm * np.asarray(eps, dtype=np.float64)[None, :]
         Y[~free] = 0.0
         return Y
+
+    def apply_rows(self, X, rows, Vq, eps=None):
+        """Selected rows of H~ X - X diag(eps) straight from the definition, without assembling anything (meshes whose cell
+        matrices are out of reach): row i of C^T H_all C collects, for node i and every hanging node that depends on it
+        (weight C_hi), the rows of the cell matrices of the cells that contain that node, applied to x_all = C (s . X).
+        Cell matrices are computed on demand by explicit quadrature and cached."""
+        X = np.ascontiguousarray(X, dtype=np.float64)
+        Vq = np.ascontiguousarray(Vq, dtype=np.float64).reshape(self.ncells, self.nq3)
+        free = self._mask.astype(bool)
+        s = np.zeros(self.N)
+        s[free] = 1.0 / np.sqrt(self._mass[free])
+        x_all = self.Cfull @ (X * s[:, None])
+        Ccsc = self.Cfull.tocsc()
+        flat = self._l2g.reshape(-1).astype(np.int64)
+        order = np.argsort(flat, kind="stable")
+        starts = np.searchsorted(flat[order], np.arange(self.N_all + 1))
+        cache = {}
+        out = np.zeros((len(rows), X.shape[1]))
+        for r, i in enumerate(rows):
+            if not free[i]:
+                continue
+            acc = np.zeros(X.shape[1])
+            for a, w in zip(Ccsc.indices[Ccsc.indptr[i]:Ccsc.indptr[i + 1]], Ccsc.data[Ccsc.indptr[i]:Ccsc.indptr[i + 1]]):
+                for pos in order[starts[a]:starts[a + 1]]:
+                    e, la = divmod(int(pos), self.nc)
+                    if e not in cache:
+                        cache[e] = self.cell_matrix(e, Vq[e])
+                    acc += w * (cache[e][la] @ x_all[self._l2g[e]])
+            out[r] = s[i] * acc
+            if eps is not None:
+                out[r] -= np.asarray(eps, dtype=np.float64) * X[i]
+        return out
 
     def filter(self, X, m, a, b, a0, nthreads=1):
         """Scaled three-term recurrence of reading R7 (l.208-210), serial."""

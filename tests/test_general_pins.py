@@ -224,3 +224,17 @@ def test_density_preconditioner_and_potential_apply_on_constrained_meshes():
         w3 = np.array([wq[a] * wq[b] * wq[c] for c in range(n) for b in range(n) for a in range(n)])
         total += np.sum(w3 * det * U.reshape(g.ncells, -1)[e] * val ** 2)
     assert abs(u @ (Y * sq) - total) < 1e-11 * abs(total)
+
+
+def test_apply_rows_equals_the_assembled_operator():
+    """apply_rows (the row-by-row definition used at sizes where nothing can be assembled) against the assembled H~ on a
+    two-level refined sheared mesh: every row, including unconstrained nodes that hanging nodes depend on."""
+    mesh, g = _refined(2, _affine(SHEAR), 2)
+    Vq = -4.0 / np.sqrt((g.quad_coords() ** 2).sum(axis=1) + 0.25)
+    g.set_potential(Vq)
+    X = workloads.random_block(90, g.N, 3, g.mask())
+    eps = np.array([-0.5, 0.0, 0.7])
+    rows = np.arange(0, g.N, 3)
+    Yr = g.apply_rows(X, rows, Vq, eps)
+    Y = g.apply(X, eps)
+    assert np.linalg.norm(Yr - Y[rows]) < 1e-12 * np.linalg.norm(Y[rows])

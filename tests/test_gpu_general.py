@@ -220,6 +220,19 @@ def test_adaptive_workload_full_size_properties():
     X = torch.randn(gm.N, B, dtype=torch.float64, device="cuda", generator=gen) * mask
     Y = torch.randn(gm.N, B, dtype=torch.float64, device="cuda", generator=gen) * mask
     HX, HY = gm.apply_H(X), gm.apply_H(Y)
+    # (0) sampled rows of one apply against the oracle's row-by-row definition (cell matrices by explicit quadrature on demand):
+    # nodes inside refined cells, on coarse faces that hanging nodes depend on, and near the boundary
+    import oracle
+    om = oracle.GeneralOracleMesh(mesh, 6)
+    assert np.array_equal(om.l2g(), gm.l2g())
+    rp, col, _ = gm.constraints()
+    masters_with_dependents = np.unique(col)
+    pick = np.concatenate([masters_with_dependents[:: max(1, len(masters_with_dependents) // 5)][:5],
+                           (workloads.uniform01(9600, 0, 7) * om.N).astype(np.int64)])
+    rows = np.unique(pick)
+    Yo = om.apply_rows(X.cpu().numpy(), rows, V(om.quad_coords()))
+    Ys = HX[torch.as_tensor(rows, device="cuda")].cpu().numpy()
+    assert np.linalg.norm(Ys - Yo) <= TOL_APPLY * np.linalg.norm(Yo)
     lhs, rhs = (X * HY).sum(dim=0), (HX * Y).sum(dim=0)
     scale = torch.sqrt((X * X).sum(dim=0) * (HY * HY).sum(dim=0))
     assert float(((lhs - rhs).abs() / scale).max()) <= 1e-12
