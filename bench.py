@@ -222,7 +222,7 @@ def stub_measurement(w, rank, B):
 
 
 # ---- device timing --------------------------------------------------------------------------------------------------------
-def time_workload(fe, torch, w, B, steps, warmup, dev, seed_offset=0, with_e2e=False, dist=None, variant=0):
+def time_workload(fe, torch, w, B, steps, warmup, dev, seed_offset=0, with_e2e=False, dist=None, variant=0, chain=False):
     """Device-resident timing of `steps` cheb_filter calls (config 5: blocks of 200 shifted applies), CUDA events on the
     launching stream around every step; clocks sampled during the timed region."""
     gm = fe.FEMesh(w.xe, w.ye, w.ze, w.p, device=dev)
@@ -250,7 +250,11 @@ def time_workload(fe, torch, w, B, steps, warmup, dev, seed_offset=0, with_e2e=F
         else:  # R19: alternate two input and two output blocks
             Y0, Y1 = wk[:N * B].view(N, B), wk[N * B:].view(N, B)
             for t in range(w.n_applies):
-                gm.apply_H(X if t % 2 == 0 else pristine, Y0 if t % 2 == 0 else Y1, eps)
+                if chain:  # the zero-fill of the next output block rides on this launch (fe_apply_H_chain)
+                    gm.apply_H_chain(X if t % 2 == 0 else pristine, Y0 if t % 2 == 0 else Y1, Y1 if t % 2 == 0 else Y0, eps,
+                                     y_is_clear=(t > 0))
+                else:
+                    gm.apply_H(X if t % 2 == 0 else pristine, Y0 if t % 2 == 0 else Y1, eps)
 
     def restore(i):  # only the block the coming step filters
         Xs[i % nrot].copy_(pristine)
@@ -551,6 +555,14 @@ def main():
                                      "filtered_blocks_per_s": world / (ji["ms_per_step"] * 1e-3) if wi.m > 0 else None,
                                      "roofline": roofline_block(wi, ri, ji["ms_per_step"], peaks, hbm_peak),
                                      "clocks": ri["clocks"], "gpu_launches": int(ri["launches"])}
+            if idx == 5:  # the same 200 applies as a chain: every call clears the next call's output block
+                rc5 = time_workload(fe, torch, wi, Bi, args.steps, args.warmup, local, seed_offset=rank, dist=dist,
+                                    variant=args.variant, chain=True)
+                jc5 = job_line(wi, rc5, world, dist, device, args.steps, args.warmup, args.scaling)
+                others["cfg5_chain"] = {"workload": wi.describe() + " through fe_apply_H_chain", "value": jc5["value"], "unit": UNIT,
+                                        "ms_per_step": jc5["ms_per_step"], "l2": rc5["l2"], "filtered_blocks_per_s": None,
+                                        "roofline": roofline_block(wi, rc5, jc5["ms_per_step"], peaks, hbm_peak),
+                                        "clocks": rc5["clocks"], "gpu_launches": int(rc5["launches"])}
             torch.cuda.empty_cache()
         if world == 1 and not args.no_adaptive:
             others["adaptive_p6"] = time_adaptive(fe, torch, local, peaks, hbm_peak, min(args.steps, 5), 3)

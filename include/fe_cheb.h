@@ -90,6 +90,15 @@ int fe_set_potential(fe_mesh* m, const double* Vq_dev, int copy, void* cuda_stre
  * Asynchronous on cuda_stream. */
 int fe_apply_H(fe_mesh* m, const double* X, double* Y, int B, const double* eps_dev, void* cuda_stream);
 
+/* fe_apply_H for a CHAIN of applies into alternating blocks (the operator inside a Krylov iteration, l.221-225; BASELINE
+ * config 5): the result is the same Y, but the zero-fill that fe_apply_H needs in front of every call is taken over by the
+ * previous call -- while this call computes Y it also clears Ynext (DEVICE, N*B doubles, may be NULL), the block the caller
+ * will pass as Y next time, through the store path of the operator kernel.  y_is_clear != 0 promises that Y was cleared that
+ * way (or is all zero) and has not been written since; with y_is_clear == 0 the call clears Y itself like fe_apply_H.
+ * X, Y, Ynext must not overlap.  Asynchronous on cuda_stream. */
+int fe_apply_H_chain(fe_mesh* m, const double* X, double* Y, double* Ynext, int B, const double* eps_dev, int y_is_clear,
+                     void* cuda_stream);
+
 /* Chebyshev filter of ChFSI (l.208-210), in place, by the scaled three-term recurrence (R7):
  *   e=(b-a)/2, c=(b+a)/2, s1=e/(a0-c);  Y1=(s1/e)(H~-c)X;  s_{k+1}=1/(2/s1-s_k);
  *   Y_{k+1} = (2 s_{k+1}/e)(H~-c)Y_k - s_k s_{k+1} Y_{k-1};   X <- Y_m  (= T_m((H~-c)/e) X / T_m((a0-c)/e)).

@@ -14,7 +14,7 @@ EXPORTS = (
     "fe_mesh_create", "fe_mesh_destroy", "fe_num_nodes", "fe_num_free", "fe_num_cells", "fe_nodes_per_cell",
     "fe_quad_per_cell", "fe_get_l2g", "fe_get_node_coords", "fe_get_quad_coords", "fe_get_mass",
     "fe_get_dirichlet_mask", "fe_set_potential", "fe_apply_H", "cheb_filter", "cheb_filter_host", "fe_rayleigh_ritz", "fe_minres_shifted", "fe_add_subspace", "fe_gram", "fe_density", "fe_lanczos_bounds", "fe_apply_potential",
-    "fe_set_variant", "fe_diag_peak", "fe_ritz_residuals", "fe_chfsi", "fe_mesh_create_general",
+    "fe_set_variant", "fe_diag_peak", "fe_ritz_residuals", "fe_chfsi", "fe_mesh_create_general", "fe_apply_H_chain",
     "fe_num_all_nodes", "fe_num_constraint_entries", "fe_get_constraints",
     "fe_launch_count", "fe_last_error",
 )
@@ -55,6 +55,7 @@ def load_library():
         getattr(L, name).restype, getattr(L, name).argtypes = C.c_int, [vp, vp]
     L.fe_set_potential.restype, L.fe_set_potential.argtypes = C.c_int, [vp, vp, C.c_int, vp]
     L.fe_apply_H.restype, L.fe_apply_H.argtypes = C.c_int, [vp, vp, vp, C.c_int, vp, vp]
+    L.fe_apply_H_chain.restype, L.fe_apply_H_chain.argtypes = C.c_int, [vp, vp, vp, vp, C.c_int, vp, C.c_int, vp]
     L.cheb_filter.restype = C.c_int
     L.cheb_filter.argtypes = [vp, vp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, vp, vp]
     L.cheb_filter_host.restype = C.c_int
@@ -214,6 +215,17 @@ def fe_apply_H(h, X, Y, eps=None, stream=None):
     B = X.shape[1]
     ep = _dev_ptr(eps, "eps", B) if eps is not None else None
     _check(load_library().fe_apply_H(h, _dev_ptr(X, "X"), _dev_ptr(Y, "Y", X.numel()), B, ep, _stream(stream)))
+    return Y
+
+
+def fe_apply_H_chain(h, X, Y, Ynext=None, eps=None, y_is_clear=False, stream=None):
+    if X.dim() != 2 or X.shape[0] != fe_num_nodes(h):
+        raise FEError(-1, "X must be N x B")
+    B = X.shape[1]
+    ep = _dev_ptr(eps, "eps", B) if eps is not None else None
+    yn = _dev_ptr(Ynext, "Ynext", X.numel()) if Ynext is not None else None
+    _check(load_library().fe_apply_H_chain(h, _dev_ptr(X, "X"), _dev_ptr(Y, "Y", X.numel()), yn, B, ep,
+                                           int(bool(y_is_clear)), _stream(stream)))
     return Y
 
 
@@ -408,6 +420,9 @@ class FEMesh:
         if Y is None:
             Y = torch.empty_like(X)
         return fe_apply_H(self.h, X, Y, eps, stream)
+
+    def apply_H_chain(self, X, Y, Ynext=None, eps=None, y_is_clear=False, stream=None):
+        return fe_apply_H_chain(self.h, X, Y, Ynext, eps, y_is_clear, stream)
 
     def cheb_filter(self, X, m, a, b, a0, work=None, stream=None):
         import torch

@@ -763,6 +763,35 @@ static int apply_into_cleared(fe_mesh* m, const double* X, double* Y, int B, con
     return tma_step(m, mx, my, nullptr, B, eps_dev, 1.0, 0.0, eps_dev != nullptr, 0.0, true, st, dots_dev);
 }
 
+int fe_apply_H_chain(fe_mesh* m, const double* X, double* Y, double* Ynext, int B, const double* eps_dev, int y_is_clear,
+                     void* cuda_stream)
+{
+    if (!m || !X || !Y) return fail(FE_ERR_INVALID, "fe_apply_H_chain: NULL argument");
+    if (B < 1) return fail(FE_ERR_INVALID, "fe_apply_H_chain: B=%d < 1", B);
+    if (!m->have_V) return fail(FE_ERR_STATE, "fe_apply_H_chain: call fe_set_potential first");
+    const size_t len = (size_t)m->N * B;
+    if (overlap(X, len, Y, len) || (Ynext && (overlap(X, len, Ynext, len) || overlap(Y, len, Ynext, len))))
+        return fail(FE_ERR_INVALID, "fe_apply_H_chain: X, Y and Ynext must not overlap");
+    CUDA_TRY(cudaSetDevice(m->device));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (m->kind == 0 && tma_eligible(m, B, X, Y, eps_dev) && (!Ynext || tma_eligible(m, B, Ynext, Ynext, Ynext))) {
+        // the clearing of the NEXT target rides on this launch as the pre-initialisation store (beta' = 0) of the owner boxes;
+        // the far boundary faces, which no owner box covers, are cleared by k_zero_faces
+        BlockMaps mx, my, mw;
+        int rc;
+        if ((rc = make_block_maps(&mx, m, X, B)) || (rc = make_block_maps(&my, m, Y, B))) return rc;
+        if (Ynext && (rc = make_block_maps(&mw, m, Ynext, B))) return rc;
+        if (!y_is_clear) CUDA_TRY(cudaMemsetAsync(Y, 0, len * sizeof(double), st));
+        if (Ynext && (rc = zero_faces(m, Ynext, B, st))) return rc;
+        return tma_step(m, mx, my, Ynext ? &mw : nullptr, B, eps_dev, 1.0, 0.0, eps_dev != nullptr, 0.0, true, st);
+    }
+    // other paths (general meshes, odd B, unaligned blocks): plain apply, then clear the next target
+    int rc = fe_apply_H(m, X, Y, B, eps_dev, cuda_stream);
+    if (rc) return rc;
+    if (Ynext) CUDA_TRY(cudaMemsetAsync(Ynext, 0, len * sizeof(double), st));
+    return FE_OK;
+}
+
 int cheb_filter(fe_mesh* m, double* X, int B, int deg, double a, double b, double a0, double* work, void* cuda_stream)
 {
     if (!m || !X || !work) return fail(FE_ERR_INVALID, "cheb_filter: NULL argument");

@@ -113,6 +113,27 @@ def test_config5_calls_1_2_200(cfg2):
             assert np.all(Yg[~free] == 0)
 
 
+def test_config5_chain_calls_1_2_200(cfg2):
+    """The same R19 sequence through fe_apply_H_chain: every call clears the block the next call writes (the zero-fill rides
+    on the operator launch); the first call starts from dirty blocks.  Outputs of calls 1, 2 and 200 against the oracle."""
+    _, om, gm, _ = cfg2
+    w = workloads.config(5)
+    mask = om.mask()
+    free = mask.astype(bool)
+    eps = w.eps()
+    X = [w.X(mask), w.X(mask, seed=w.x_seed + 100)]
+    Yo = [om.apply(X[i], eps, nthreads=NT) for i in range(2)]
+    Xd = [_dev(X[0]), _dev(X[1])]
+    Yd = [torch.full_like(Xd[0], 3.5), torch.full_like(Xd[0], -1.25)]  # dirty output blocks
+    ed = _dev(eps)
+    for t in range(w.n_applies):
+        gm.apply_H_chain(Xd[t % 2], Yd[t % 2], Yd[(t + 1) % 2], ed, y_is_clear=(t > 0))
+        if t in (0, 1, w.n_applies - 1):
+            Yg = Yd[t % 2].cpu().numpy()
+            assert _relerr(Yg, Yo[t % 2], free) <= TOL_APPLY, t + 1
+            assert np.all(Yg[~free] == 0)
+
+
 # ---- configs 3 and 4: sampled rows of one apply, filter through the recurrence property -----------------------------------
 def _cells_of_row(w, g):
     """All cells (ex, ey, ez) whose node set contains global node g (R3 numbering)."""

@@ -585,6 +585,24 @@ def test_nan_in_dirichlet_rows_is_ignored():
     assert np.all(np.isfinite(G))
 
 
+@pytest.mark.parametrize("p,B", [(2, 6), (4, 34), (6, 8), (3, 5)])
+def test_apply_chain(p, B):
+    """fe_apply_H_chain on the unequal mesh: three chained applies into two alternating blocks equal three fe_apply_H calls;
+    B = 5 takes the fallback (plain apply + memset of the next target)."""
+    om, gm = _pair(UNEQUAL, p, _coulomb)
+    mask = om.mask()
+    eps = workloads.shifts(2700 + p, B)
+    Xs = [workloads.random_block(1700 + p + i, om.N, B) for i in range(3)]  # Dirichlet rows hold data
+    Y = [torch.full((om.N, B), 9.0, dtype=torch.float64, device="cuda"), torch.full((om.N, B), -7.0, dtype=torch.float64, device="cuda")]
+    for t in range(3):
+        gm.apply_H_chain(_dev(Xs[t]), Y[t % 2], Y[(t + 1) % 2], _dev(eps), y_is_clear=(t > 0))
+        Yg = Y[t % 2].cpu().numpy()
+        assert _relerr(Yg, om.apply(Xs[t], eps), mask) <= TOL_APPLY, t
+        assert np.all(Yg[mask == 0] == 0)
+    gm.apply_H_chain(_dev(Xs[0]), Y[1], None, None, y_is_clear=True)  # last link: nothing to clear, no shift
+    assert _relerr(Y[1].cpu().numpy(), om.apply(Xs[0]), mask) <= TOL_APPLY
+
+
 # ---- error behaviour -------------------------------------------------------------------------------------------------
 def test_error_codes():
     fe = _fe()
