@@ -14,6 +14,10 @@
  * exactness; brute-force l2g; sum(M) = volume; K.1 = 0; K(x^2+y^2+z^2) = -6 M; the textbook 8x8
  * trilinear Laplacian; symmetry; sum of cells == assembled CSR; 3-D harmonic oscillator levels
  * 1.5 / 2.5 / 3.5 converging with p; filter == T_m through a LAPACK eigendecomposition.
+ * General (trilinearly mapped) cells and hanging nodes (orc_general_*, oracle/fe_general.py) are pinned in
+ * tests/test_general_pins.py: an unrefined undeformed mesh reproduces everything above; a sheared cell equals the analytically
+ * transformed reference matrix; continuity and patch tests (K_c linear = 0, K_c r^2 = -6 M_c) through hanging faces and edges;
+ * density, potential-only operator and preconditioner through closed forms; apply_rows against the assembled operator.
  * "parity unpinned": the soft-Coulomb eigenvalues of configs 2-4 have no external truth; those
  * configs are pinned only through the invariants above.
  */
