@@ -169,8 +169,9 @@ int fe_apply_potential(fe_mesh* m, const double* Uq_dev, const double* X, double
 /* Kernel variant for experiments and tests: 0 = default (TMA generation when B is even and the blocks are 16-byte
  * aligned, else the legacy atomics kernel), 3 = legacy kernel always, 4 = legacy kernel with a colour-ordered
  * scatter (the 8 parity classes of the cell grid launched in order: cells of one class share no node, so every sum
- * has a fixed order and results are bit-reproducible; slower), 5..8 = launch shapes of the TMA kernel
- * (fe_apply_tma.cuh).  FE_ERR_INVALID if unknown. */
+ * has a fixed order and results are bit-reproducible; slower; on a general mesh: cells coloured greedily so that no two
+ * cells of a colour share a node, launched colour by colour, hanging contributions collapsed over the transposed constraint
+ * rows), 5..8 = launch shapes of the TMA kernel (fe_apply_tma.cuh; test and experiment hooks).  FE_ERR_INVALID if unknown. */
 int fe_set_variant(fe_mesh* m, int variant);
 /* Kernels launched by this handle since creation (bench.py's gpu_launches). */
 int64_t fe_launch_count(const fe_mesh* m);

@@ -81,7 +81,10 @@ struct fe_mesh {
         int32_t *bcol = nullptr, *brow = nullptr, *out = nullptr;
         double* bw = nullptr;
         long long nb = 0;
-    } gexp;  // expansion X_h = C_h (s . X); the collapse Y += alpha s . C_h^T Y_h reads the same bundles the other way
+    } gexp,  // expansion X_h = C_h (s . X); the collapse Y += alpha s . C_h^T Y_h reads the same bundles the other way
+      gtr;   // variant 4 only: the transposed rows, one owner per row of Y (a collapse without atomics)
+    int32_t* d_colcells = nullptr;        // variant 4: cells sorted by colour (cells of one colour share no node)
+    std::vector<int64_t> colour_off;      //   colour c = cells [colour_off[c], colour_off[c+1])
     double *d_Xh = nullptr, *d_Yh = nullptr;  // (N_all - N) * hcap: expanded hanging values / their scatter target
     double* d_grecU = nullptr;  // fe_apply_potential on a general mesh: records with zero metric and WV = w |J| U
     int hcap = 0;
@@ -221,6 +224,8 @@ int fe_mesh_destroy(fe_mesh* m)
     cudaFree(m->d_gl2g); cudaFree(m->d_gmetric); cudaFree(m->d_gwdet); cudaFree(m->d_gsc);
     cudaFree(m->d_Xh); cudaFree(m->d_Yh); cudaFree(m->d_grecU);
     cudaFree(m->gexp.bptr); cudaFree(m->gexp.bcol); cudaFree(m->gexp.brow); cudaFree(m->gexp.out); cudaFree(m->gexp.bw);
+    cudaFree(m->gtr.bptr); cudaFree(m->gtr.bcol); cudaFree(m->gtr.brow); cudaFree(m->gtr.out); cudaFree(m->gtr.bw);
+    cudaFree(m->d_colcells);
     delete m->gh;
     delete m;
     return FE_OK;
@@ -408,6 +413,49 @@ static int upload_vec(T** dst, const std::vector<T>& src)
     return FE_OK;
 }
 
+// sort sparse rows by column list and pack rows with identical lists into bundles for k_gen_rows_times_block / k_gen_collapse
+static int pack_bundles(const std::vector<std::vector<std::pair<int32_t, double>>>& rws, const std::vector<int32_t>& dst_of,
+                    fe_mesh::GenBundlesDev* dev)
+{
+    const int64_t nr = (int64_t)rws.size();
+    std::vector<int32_t> order((size_t)nr);
+    for (int64_t i = 0; i < nr; ++i) order[i] = (int32_t)i;
+    auto same_cols = [&](int32_t a, int32_t b) {
+        if (rws[a].size() != rws[b].size()) return false;
+        for (size_t k = 0; k < rws[a].size(); ++k)
+            if (rws[a][k].first != rws[b][k].first) return false;
+        return true;
+    };
+    std::sort(order.begin(), order.end(), [&](int32_t a, int32_t b) {
+        if (rws[a].size() != rws[b].size()) return rws[a].size() < rws[b].size();
+        for (size_t k = 0; k < rws[a].size(); ++k)
+            if (rws[a][k].first != rws[b][k].first) return rws[a][k].first < rws[b][k].first;
+        return a < b;
+    });
+    std::vector<long long> bptr{0};
+    std::vector<int32_t> bcol, brow{0}, out;
+    std::vector<double> bw;
+    for (int64_t i = 0; i < nr;) {
+        int64_t e = i + 1;
+        while (e < nr && e - i < kGenBundle && same_cols(order[i], order[e])) ++e;
+        const auto& first = rws[order[i]];
+        for (size_t k = 0; k < first.size(); ++k) {
+            bcol.push_back(first[k].first);
+            for (int u = 0; u < kGenBundle; ++u) bw.push_back(i + u < e ? rws[order[i + u]][k].second : 0.0);
+        }
+        for (int64_t q = i; q < e; ++q) out.push_back(dst_of[order[q]]);
+        bptr.push_back((long long)bcol.size());
+        brow.push_back((int32_t)out.size());
+        i = e;
+    }
+    dev->nb = (long long)bptr.size() - 1;
+    int r;
+    if ((r = upload_vec(&dev->bptr, bptr)) || (r = upload_vec(&dev->bcol, bcol)) || (r = upload_vec(&dev->brow, brow)) ||
+        (r = upload_vec(&dev->out, out)) || (r = upload_vec(&dev->bw, bw)))
+        return r;
+    return FE_OK;
+}
+
 int fe_mesh_create_general(int cx, int cy, int cz, const int32_t* cells, int64_t ncells, const double* verts, int p,
                            int cuda_device, fe_mesh** out)
 {
@@ -474,46 +522,6 @@ int fe_mesh_create_general(int cx, int cy, int cz, const int32_t* cells, int64_t
             for (int k = 0; k < h; ++k) { m->eoD.S[h * h + k] = m->tab.D[h * n + k]; m->eoDT.S[h * h + k] = Dt[h * n + k]; }
     }
     // the constraint rows and their transpose, sorted by column list and packed into bundles of rows with identical lists
-    auto pack = [&](const std::vector<std::vector<std::pair<int32_t, double>>>& rws, const std::vector<int32_t>& dst_of,
-                    fe_mesh::GenBundlesDev* dev) -> int {
-        const int64_t nr = (int64_t)rws.size();
-        std::vector<int32_t> order((size_t)nr);
-        for (int64_t i = 0; i < nr; ++i) order[i] = (int32_t)i;
-        auto same_cols = [&](int32_t a, int32_t b) {
-            if (rws[a].size() != rws[b].size()) return false;
-            for (size_t k = 0; k < rws[a].size(); ++k)
-                if (rws[a][k].first != rws[b][k].first) return false;
-            return true;
-        };
-        std::sort(order.begin(), order.end(), [&](int32_t a, int32_t b) {
-            if (rws[a].size() != rws[b].size()) return rws[a].size() < rws[b].size();
-            for (size_t k = 0; k < rws[a].size(); ++k)
-                if (rws[a][k].first != rws[b][k].first) return rws[a][k].first < rws[b][k].first;
-            return a < b;
-        });
-        std::vector<long long> bptr{0};
-        std::vector<int32_t> bcol, brow{0}, out;
-        std::vector<double> bw;
-        for (int64_t i = 0; i < nr;) {
-            int64_t e = i + 1;
-            while (e < nr && e - i < kGenBundle && same_cols(order[i], order[e])) ++e;
-            const auto& first = rws[order[i]];
-            for (size_t k = 0; k < first.size(); ++k) {
-                bcol.push_back(first[k].first);
-                for (int u = 0; u < kGenBundle; ++u) bw.push_back(i + u < e ? rws[order[i + u]][k].second : 0.0);
-            }
-            for (int64_t q = i; q < e; ++q) out.push_back(dst_of[order[q]]);
-            bptr.push_back((long long)bcol.size());
-            brow.push_back((int32_t)out.size());
-            i = e;
-        }
-        dev->nb = (long long)bptr.size() - 1;
-        int r;
-        if ((r = upload_vec(&dev->bptr, bptr)) || (r = upload_vec(&dev->bcol, bcol)) || (r = upload_vec(&dev->brow, brow)) ||
-            (r = upload_vec(&dev->out, out)) || (r = upload_vec(&dev->bw, bw)))
-            return r;
-        return FE_OK;
-    };
     int rc = FE_OK;
     {
         const int64_t nh = g.N_all - g.N;
@@ -523,7 +531,7 @@ int fe_mesh_create_general(int cx, int cy, int cz, const int32_t* cells, int64_t
             fdst[r] = (int32_t)r;
             for (int64_t k = g.crow[r]; k < g.crow[r + 1]; ++k) fw[r].push_back({g.ccol[k], csv[k]});
         }
-        if ((rc = pack(fw, fdst, &m->gexp))) { fe_mesh_destroy(m); return rc; }
+        if ((rc = pack_bundles(fw, fdst, &m->gexp))) { fe_mesh_destroy(m); return rc; }
     }
     if ((rc = upload_vec(&m->d_gsc, scv)) || (rc = upload_vec(&m->d_sm, sv)) || (rc = upload_vec(&m->d_gl2g, g.l2g)) || (rc = upload_vec(&m->d_gmetric, met)) ||
         (rc = upload_vec(&m->d_gwdet, wdet))) {
@@ -568,6 +576,64 @@ static int general_expand(fe_mesh* m, const double* X, int B, cudaStream_t st)
     return FE_OK;
 }
 
+// Colour-ordered (deterministic) scatter on a general mesh (variant 4; S8(a) a3 "atomic or colour-ordered"): cells are
+// coloured greedily so that no two cells of a colour share a node (unconstrained or hanging); the cell kernel is launched
+// colour by colour, and the collapse runs over the transposed constraint rows (one owner per row of Y), so every sum has a
+// fixed order and the result is bit-reproducible.  Built on first use.
+static int ensure_general_colours(fe_mesh* m)
+{
+    if (m->d_colcells) return FE_OK;
+    const GeneralHost& g = *m->gh;
+    const int nc = m->nc;
+    std::vector<int64_t> cnt((size_t)g.N_all + 1, 0);
+    for (int32_t id : g.l2g) cnt[(size_t)id + 1] += 1;
+    for (int64_t i = 0; i < g.N_all; ++i) cnt[i + 1] += cnt[i];
+    std::vector<int32_t> cells_of((size_t)g.l2g.size());
+    {
+        std::vector<int64_t> pos(cnt.begin(), cnt.end() - 1);
+        for (int64_t e = 0; e < g.ncells; ++e)
+            for (int a = 0; a < nc; ++a) cells_of[pos[g.l2g[(size_t)e * nc + a]]++] = (int32_t)e;
+    }
+    std::vector<int> colour((size_t)g.ncells, -1);
+    int ncol = 0;
+    std::vector<char> used;
+    for (int64_t e = 0; e < g.ncells; ++e) {
+        used.assign((size_t)ncol + 1, 0);
+        for (int a = 0; a < nc; ++a) {
+            const int32_t id = g.l2g[(size_t)e * nc + a];
+            for (int64_t q = cnt[id]; q < cnt[id + 1]; ++q) {
+                const int c = colour[cells_of[q]];
+                if (c >= 0) used[c] = 1;
+            }
+        }
+        int c = 0;
+        while (c < ncol && used[c]) ++c;
+        colour[e] = c;
+        if (c == ncol) ++ncol;
+    }
+    std::vector<int32_t> sorted;
+    m->colour_off.assign(1, 0);
+    for (int c = 0; c < ncol; ++c) {
+        for (int64_t e = 0; e < g.ncells; ++e)
+            if (colour[e] == c) sorted.push_back((int32_t)e);
+        m->colour_off.push_back((int64_t)sorted.size());
+    }
+    // transposed constraint rows: for every unconstrained node with hanging dependents, (hanging row, weight * s)
+    const int64_t nh = g.N_all - g.N;
+    std::vector<std::vector<std::pair<int32_t, double>>> tr;
+    std::vector<int32_t> tdst, tindex((size_t)g.N, -1);
+    for (int64_t r = 0; r < nh; ++r)
+        for (int64_t k = g.crow[r]; k < g.crow[r + 1]; ++k) {
+            int32_t& ti = tindex[g.ccol[k]];
+            if (ti < 0) { ti = (int32_t)tr.size(); tr.emplace_back(); tdst.push_back(g.ccol[k]); }
+            const double sk = g.mask[g.ccol[k]] ? 1.0 / std::sqrt(g.mass[g.ccol[k]]) : 0.0;
+            tr[ti].push_back({(int32_t)r, g.cval[k] * sk});
+        }
+    int rc;
+    if (!tr.empty() && (rc = pack_bundles(tr, tdst, &m->gtr))) return rc;
+    return upload_vec(&m->d_colcells, sorted);
+}
+
 // one fused operator step on a general mesh: diagonal terms (k_gen_init), expansion of the hanging values, the cell kernel,
 // the transposed expansion
 static int general_step(fe_mesh* m, const double* X, const double* Z, double* Y, int B, const double* eps,
@@ -589,6 +655,21 @@ static int general_step(fe_mesh* m, const double* X, const double* Z, double* Y,
     prm.X = X; prm.Xh = m->d_Xh ? m->d_Xh : X; prm.Y = Y; prm.Yh = m->d_Yh ? m->d_Yh : Y; prm.sc = m->d_gsc; prm.l2g = m->d_gl2g;
     prm.rec = m->d_gmetric; prm.N = g.N; prm.ncells = m->ncells; prm.B = B; prm.alpha = alpha;
     prm.eoN = m->eoN; prm.eoNT = m->eoNT; prm.eoD = m->eoD; prm.eoDT = m->eoDT;
+    if (m->variant == 4) {  // colour-ordered, bit-reproducible
+        if ((rc = ensure_general_colours(m))) return rc;
+        for (size_t c = 0; c + 1 < m->colour_off.size(); ++c) {
+            prm.cell_list = m->d_colcells + m->colour_off[c];
+            prm.ncells = m->colour_off[c + 1] - m->colour_off[c];
+            cudaError_t ec = launch_apply_gen(prm, m->p, prm.ncells, m->sms, st);
+            if (ec != cudaSuccess) return fail(FE_ERR_CUDA, "operator launch (general mesh) failed: %s", cudaGetErrorString(ec));
+        }
+        if (nh > 0)
+            k_gen_rows_times_block<<<grid, rows, 0, st>>>(Y, m->d_Yh, m->gtr.bptr, m->gtr.bcol, m->gtr.bw, m->gtr.brow, m->gtr.out,
+                                                          m->gtr.nb, B, alpha, 1);
+        CUDA_TRY(cudaGetLastError());
+        m->launches += (int64_t)m->colour_off.size() + (nh > 0 ? 2 : 1);
+        return FE_OK;
+    }
     cudaError_t e = launch_apply_gen(prm, m->p, m->ncells, m->sms, st);
     if (e != cudaSuccess) return fail(FE_ERR_CUDA, "operator launch (general mesh) failed: %s", cudaGetErrorString(e));
     if (nh > 0)

@@ -39,6 +39,7 @@ struct GenParams {
     const int32_t* l2g;  // ncells * n^3
     const double* sc;    // ncells * n^3: s_g = mu_g M_c,gg^{-1/2} at the cell's unconstrained nodes, 1 at its hanging nodes
     const double* rec;   // ncells * GREC: per-cell record, 6 metric fields (fe_general.h) then WV = w_q |J| V_q, n^3 each
+    const int32_t* cell_list;  // NULL: all cells 0..ncells-1; else the ncells cells of one colour (colour-ordered scatter)
     long long N, ncells;
     int B;
     double alpha;
@@ -282,7 +283,8 @@ __global__ void __launch_bounds__(GenShape<P>::LS * BT, MINB) k_apply_gen(const 
     }
     // requests for a unit: ids and scales (4- / 8-byte cp.async) and the record (bulk copy on bar[buf]) ...
     auto request_tables = [&](long long u, int buf) {
-        const long long c = u / ntile;
+        const long long cu = u / ntile;
+        const long long c = prm.cell_list ? prm.cell_list[cu] : cu;
         if (tid == 0) {
             mbar_expect_tx(bar + buf, (unsigned)(GREC * sizeof(double)));
             bulk_load(sRecB + buf * GREC, prm.rec + c * GREC, (unsigned)(GREC * sizeof(double)), bar + buf);

@@ -202,6 +202,31 @@ def test_density_and_potential_apply_on_a_hanging_node_mesh(p, B):
     assert _relerr(gm.apply_H(_dev(X)).cpu().numpy(), om.apply(X), mask) <= TOL_APPLY
 
 
+def test_colour_ordered_scatter_on_a_hanging_node_mesh():
+    """Variant 4 on a general mesh (S8(a) a3 "atomic or colour-ordered"): cells launched colour by colour, collapse over the
+    transposed rows -- two runs are bit-identical, the result matches the oracle, and the atomic path agrees with it to
+    rounding (the deterministic mode doubles as a race oracle, R17)."""
+    mesh = _atom_mesh(2)
+    om, gm = _pair(mesh, 3, _coulomb)
+    mask = om.mask()
+    B = 10
+    X = workloads.random_block(2100, om.N, B, mask)
+    eps = workloads.shifts(3100, B)
+    Xd, ed = _dev(X), _dev(eps)
+    gm.set_variant(4)
+    Y1 = gm.apply_H(Xd, eps=ed).clone()
+    Y2 = gm.apply_H(Xd, eps=ed).clone()
+    F1 = gm.cheb_filter(Xd.clone(), 6, -2.0, 400.0, -12.0)
+    F2 = gm.cheb_filter(Xd.clone(), 6, -2.0, 400.0, -12.0)
+    assert torch.equal(Y1, Y2) and torch.equal(F1, F2)
+    assert _relerr(Y1.cpu().numpy(), om.apply(X, eps), mask) <= TOL_APPLY
+    gm.set_variant(0)
+    Ya = gm.apply_H(Xd, eps=ed)
+    Fa = gm.cheb_filter(Xd.clone(), 6, -2.0, 400.0, -12.0)
+    assert float(torch.linalg.norm(Ya - Y1) / torch.linalg.norm(Y1)) <= 1e-14
+    assert float(torch.linalg.norm(Fa - F1) / torch.linalg.norm(F1)) <= 1e-13
+
+
 def test_adaptive_workload_full_size_properties():
     """The adaptive-molecule workload bench.py times (4 066 leaves on three levels, p = 6, 857 011 unconstrained + 100 507
     hanging nodes, B = 64), where the oracle's cell matrices are out of reach: (i) the operator is symmetric,
@@ -233,6 +258,11 @@ def test_adaptive_workload_full_size_properties():
     Yo = om.apply_rows(X.cpu().numpy(), rows, V(om.quad_coords()))
     Ys = HX[torch.as_tensor(rows, device="cuda")].cpu().numpy()
     assert np.linalg.norm(Ys - Yo) <= TOL_APPLY * np.linalg.norm(Yo)
+    gm.set_variant(4)  # ALL rows against the colour-ordered deterministic path (no atomics anywhere): a race check at scale
+    HXd = gm.apply_H(X)
+    gm.set_variant(0)
+    assert float(torch.linalg.norm(HX - HXd) / torch.linalg.norm(HXd)) <= 1e-14
+    del HXd
     lhs, rhs = (X * HY).sum(dim=0), (HX * Y).sum(dim=0)
     scale = torch.sqrt((X * X).sum(dim=0) * (HY * HY).sum(dim=0))
     assert float(((lhs - rhs).abs() / scale).max()) <= 1e-12
