@@ -64,7 +64,7 @@ struct fe_mesh {
     int variant = 0;
     double* d_minv = nullptr;   // N: MINRES preconditioner, 1 / diag(M^{-1/2} 1/2 K M^{-1/2}) on free rows (built on first use)
     double* d_mask = nullptr;   // N: 1 on free rows, 0 on Dirichlet rows (the unpreconditioned MINRES)
-    double* d_scal = nullptr;   // 20 * 128 doubles + 1 int: MINRES column scalars
+    double* d_scal = nullptr;   // 21 * 128 doubles: MINRES column scalars
     double *d_WU = nullptr, *d_VZU = nullptr;  // fe_apply_potential: J w U of the caller's field (+ unused record output)
     double* d_host = nullptr;   // device staging of cheb_filter_host (grown on demand)
     size_t host_cap = 0;
@@ -1171,7 +1171,7 @@ static int ensure_minres_tables_general(fe_mesh* m)
     }
     int rc;
     if ((rc = upload(&m->d_minv, minv)) || (rc = upload(&m->d_mask, mask))) return rc;
-    CUDA_TRY(cudaMalloc((void**)&m->d_scal, (20 * 128 + 2) * sizeof(double)));
+    CUDA_TRY(cudaMalloc((void**)&m->d_scal, 21 * 128 * sizeof(double)));
     return FE_OK;
 }
 
@@ -1192,7 +1192,7 @@ static int ensure_minres_tables(fe_mesh* m)
     cudaError_t ce = cudaSuccess;
     if (!rc) ce = cudaMalloc((void**)&m->d_minv, (size_t)m->N * sizeof(double));
     if (!rc && ce == cudaSuccess) ce = cudaMalloc((void**)&m->d_mask, (size_t)m->N * sizeof(double));
-    if (!rc && ce == cudaSuccess) ce = cudaMalloc((void**)&m->d_scal, (20 * 128 + 2) * sizeof(double));
+    if (!rc && ce == cudaSuccess) ce = cudaMalloc((void**)&m->d_scal, 21 * 128 * sizeof(double));
     if (!rc && ce == cudaSuccess) {
         k_build_precond<<<m->sms * 8, 256>>>(m->d_minv, m->Nx, m->Ny, m->Nz, d[0], d[1], d[2], d[3], d[4], d[5], m->d_sx, m->d_sy, m->d_sz);
         k_build_scaling<<<m->sms * 8, 256>>>(m->d_sx, m->d_sy, m->d_sz, m->Nx, m->Ny, m->Nz, m->d_mask);
@@ -1225,11 +1225,12 @@ int fe_minres_shifted(fe_mesh* m, const double* G, double* X, int B, const doubl
     MinresScalars q;
     double* s = m->d_scal;
     double** f[] = {&q.beta, &q.oldb, &q.alfa, &q.betasq, &q.dbar, &q.epsln, &q.oldeps, &q.phibar, &q.cs, &q.sn,
-                    &q.gamma, &q.delta, &q.phi, &q.beta1, &q.s, &q.c1, &q.c2, &q.dot, &q.gam, &q.gamn};
-    for (int i = 0; i < 20; ++i) *f[i] = s + (size_t)i * 128;
-    q.itn = (int*)(s + 20 * 128);
+                    &q.gamma, &q.delta, &q.phi, &q.beta1, &q.s, &q.c1, &q.c2, &q.dot, &q.gam, &q.gamn, &q.sv};
+    for (int i = 0; i < 21; ++i) *f[i] = s + (size_t)i * 128;
     const int grid = m->sms * 8;
     const dim3 blk(kMRx, kMRy);
+    // even B and 16-byte aligned blocks: the two elementwise passes move 16 bytes per access
+    const bool vec2 = B % 2 == 0 && (((uintptr_t)X | (uintptr_t)work) & 15) == 0;
     CUDA_TRY(cudaMemsetAsync(q.betasq, 0, 128 * sizeof(double), st));
     k_minres_init<<<grid, blk, 0, st>>>(G, Minv, R1, R2, Y, X, W1, W2, m->N, B, q.betasq);
     k_minres_scalars<<<1, 128, 0, st>>>(q, B, 0, tol);
@@ -1242,8 +1243,9 @@ int fe_minres_shifted(fe_mesh* m, const double* G, double* X, int B, const doubl
     const bool tma = tma_eligible(m, B, Y, HY, eps_dev);
     BlockMaps mapY, mapHY;
     if (tma && ((rc = make_block_maps(&mapY, m, Y, B)) || (rc = make_block_maps(&mapHY, m, HY, B)))) return rc;
+    k_minres_scalars<<<1, 128, 0, st>>>(q, B, 1, tol);  // the later steps' s, c1 come from stage 2 of the step before
+    m->launches += 1;
     while (it < maxit && !done) {
-        k_minres_scalars<<<1, 128, 0, st>>>(q, B, 1, tol);
         // hy = (H~ - eps_j) y,  y = beta v, with dot_j = y_j . hy_j from the operator kernel
         if (tma)
             rc = tma_step(m, mapY, mapHY, nullptr, B, eps_dev, 1.0, 0.0, eps_dev != nullptr, 0.0, true, st, q.dot);
@@ -1251,11 +1253,25 @@ int fe_minres_shifted(fe_mesh* m, const double* G, double* X, int B, const doubl
             rc = apply_into_cleared(m, Y, HY, B, eps_dev, q.dot, cuda_stream);
         if (rc) return rc;
         k_minres_scalars<<<1, 128, 0, st>>>(q, B, 3, tol);
-        k_minres_lanczos<<<grid, blk, 0, st>>>(HY, R1, R2, Minv, m->N, B, q.s, q.c1, q.c2, q.betasq, q.gamn);
+        if (vec2 && B <= 64)
+            k_minres_lanczos2<1, 2><<<grid, blk, 0, st>>>((double2*)HY, (double2*)R1, (const double2*)R2, Minv, m->N, B, q.s, q.c1,
+                                                          q.c2, q.betasq, q.gamn);
+        else if (vec2)
+            k_minres_lanczos2<2, 1><<<grid, blk, 0, st>>>((double2*)HY, (double2*)R1, (const double2*)R2, Minv, m->N, B, q.s, q.c1,
+                                                          q.c2, q.betasq, q.gamn);
+        else
+            k_minres_lanczos<<<grid, blk, 0, st>>>(HY, R1, R2, Minv, m->N, B, q.s, q.c1, q.c2, q.betasq, q.gamn);
         k_minres_scalars<<<1, 128, 0, st>>>(q, B, 2, tol);
-        k_minres_update<<<grid, blk, 0, st>>>(Y, W1, W2, X, m->N, B, q.s, q.oldeps, q.delta, q.gamma, q.phi);
+        if (vec2 && B <= 64)
+            k_minres_update2<1, 2><<<grid, blk, 0, st>>>((double2*)Y, (double2*)W1, (const double2*)W2, (double2*)X, m->N, B, q.sv,
+                                                         q.oldeps, q.delta, q.gamma, q.phi);
+        else if (vec2)
+            k_minres_update2<2, 1><<<grid, blk, 0, st>>>((double2*)Y, (double2*)W1, (const double2*)W2, (double2*)X, m->N, B, q.sv,
+                                                         q.oldeps, q.delta, q.gamma, q.phi);
+        else
+            k_minres_update<<<grid, blk, 0, st>>>(Y, W1, W2, X, m->N, B, q.sv, q.oldeps, q.delta, q.gamma, q.phi);
         CUDA_TRY(cudaGetLastError());
-        m->launches += 5;
+        m->launches += 4;
         std::swap(Y, HY);  // the preconditioned residual of this step is the next step's y
         std::swap(mapY, mapHY);
         std::swap(R1, R2);
