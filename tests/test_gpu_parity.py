@@ -264,6 +264,26 @@ def test_block_minres_shifted(precondition):
         assert itc < it_plain
 
 
+@pytest.mark.parametrize("B", [7, 66, 128])
+def test_block_minres_block_widths(B):
+    """The elementwise passes of a MINRES step have three launch shapes: 16-byte accesses with one tile of 64 columns (even
+    B <= 64, covered above), with two tiles (even B up to 128), and 8-byte accesses for odd B.  Fixed 12 steps, all columns."""
+    import oracle
+    w = workloads.reduced(5, 4)
+    om, gm = _pair((w.xe, w.ye, w.ze), w.p, w.V)
+    mask = om.mask()
+    G = workloads.random_block(610 + B, om.N, B)
+    eps = workloads.shifts(2610 + B, B)
+    Mi = oracle.laplacian_precond(om)
+    Xo, relo, ito = oracle.minres_shifted(om, G, eps, maxit=12, tol=0.0, Minv=Mi)
+    Xg, relg, itg = gm.minres_shifted(_dev(G), _dev(eps), maxit=12, tol=0.0, precondition=True)
+    Xg = Xg.cpu().numpy()
+    assert itg == 12 and ito == 12
+    assert _relerr(Xg, Xo, mask) <= 1e-9
+    assert np.max(np.abs(relg - relo)) <= 1e-9
+    assert np.all(Xg[~mask.astype(bool)] == 0)
+
+
 def test_adjoint_null_space_completion():
     """l.221-223: eps_k = Ritz values, g orthogonal to the Ritz vectors; after the MINRES solve the component along
     Psi is replaced by d (Eq. 8 supplies d; here seeded): P += Psi (d - Psi^T P)."""
