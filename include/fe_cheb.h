@@ -141,6 +141,16 @@ int fe_minres_shifted(fe_mesh* m, const double* G, double* X, int B, const doubl
  * Y^T H~ Y) and of the projections Psi^T P of the adjoint solve.  All N rows take part.  Synchronous. */
 int fe_gram(fe_mesh* m, const double* A, const double* Bm, int B, double* C_host, void* cuda_stream);
 
+/* fe_gram for callers that must not allocate (code under CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): the same product with the same kernels, but the B x B device accumulator is a file-scope static __device__
+ * array of the library (128 x 128 doubles = 128 KB, held by every GPU that loads the library until exit) instead of a
+ * cudaMalloc'ed buffer of the mesh.  The call itself never calls cudaMalloc, cudaFree or an allocating library routine.
+ * Arguments as fe_gram: A, Bm DEVICE N*B (read only), C_host HOST B*B doubles (out, row-major).  1 <= B <= 128: a larger
+ * B is rejected with FE_ERR_INVALID (the accumulator cannot hold it).  Synchronous (the stream is synchronised before
+ * return).  ALL calls on one GPU share the accumulator: each call clears the B*B entries it uses first, and calls that
+ * overlap on the GPU (two streams, two host threads) race on it -- serialise them. */
+int fe_gram_static(fe_mesh* m, const double* A, const double* Bm, int B, double* C_host, void* cuda_stream);
+
 /* P <- P + Psi D  (N x B block times a HOST B x B row-major matrix D): the completion p = p_perp + Psi~_k d_k of
  * l.223.  Psi, P: DEVICE N*B, must not overlap.  Synchronous. */
 int fe_add_subspace(fe_mesh* m, const double* Psi, const double* D_host, double* P, int B, void* cuda_stream);

@@ -13,7 +13,7 @@ _lib = None
 EXPORTS = (
     "fe_mesh_create", "fe_mesh_destroy", "fe_num_nodes", "fe_num_free", "fe_num_cells", "fe_nodes_per_cell",
     "fe_quad_per_cell", "fe_get_l2g", "fe_get_node_coords", "fe_get_quad_coords", "fe_get_mass",
-    "fe_get_dirichlet_mask", "fe_set_potential", "fe_apply_H", "cheb_filter", "cheb_filter_host", "fe_rayleigh_ritz", "fe_minres_shifted", "fe_add_subspace", "fe_gram", "fe_density", "fe_lanczos_bounds", "fe_apply_potential",
+    "fe_get_dirichlet_mask", "fe_set_potential", "fe_apply_H", "cheb_filter", "cheb_filter_host", "fe_rayleigh_ritz", "fe_minres_shifted", "fe_add_subspace", "fe_gram", "fe_gram_static", "fe_density", "fe_lanczos_bounds", "fe_apply_potential",
     "fe_set_variant", "fe_diag_peak", "fe_ritz_residuals", "fe_chfsi", "fe_mesh_create_general", "fe_apply_H_chain",
     "fe_num_all_nodes", "fe_num_constraint_entries", "fe_get_constraints",
     "fe_launch_count", "fe_last_error",
@@ -67,6 +67,7 @@ def load_library():
     L.fe_lanczos_bounds.restype, L.fe_lanczos_bounds.argtypes = C.c_int, [vp, vp, C.c_int, vp, vp, vp]
     L.fe_apply_potential.restype, L.fe_apply_potential.argtypes = C.c_int, [vp, vp, vp, vp, C.c_int, vp]
     L.fe_gram.restype, L.fe_gram.argtypes = C.c_int, [vp, vp, vp, C.c_int, vp, vp]
+    L.fe_gram_static.restype, L.fe_gram_static.argtypes = C.c_int, [vp, vp, vp, C.c_int, vp, vp]
     L.fe_add_subspace.restype, L.fe_add_subspace.argtypes = C.c_int, [vp, vp, vp, vp, C.c_int, vp]
     L.fe_set_variant.restype, L.fe_set_variant.argtypes = C.c_int, [vp, C.c_int]
     L.fe_ritz_residuals.restype, L.fe_ritz_residuals.argtypes = C.c_int, [vp, vp, vp, C.c_int, vp, vp, vp]
@@ -320,6 +321,16 @@ def fe_gram(h, A, Bm, stream=None):
     return out
 
 
+def fe_gram_static(h, A, Bm, stream=None):
+    """A^T Bm as a numpy B x B array; the library allocates nothing in this call (static device accumulator, B <= 128)."""
+    import numpy as np
+    B = A.shape[1]
+    out = np.empty((B, B), dtype=np.float64)
+    _check(load_library().fe_gram_static(h, _dev_ptr(A, "A"), _dev_ptr(Bm, "Bm", A.numel()), B,
+                                         out.ctypes.data_as(C.c_void_p), _stream(stream)))
+    return out
+
+
 def fe_add_subspace(h, Psi, D, P, stream=None):
     import numpy as np
     B = Psi.shape[1]
@@ -474,6 +485,9 @@ class FEMesh:
 
     def gram(self, A, Bm, stream=None):
         return fe_gram(self.h, A, Bm, stream)
+
+    def gram_static(self, A, Bm, stream=None):
+        return fe_gram_static(self.h, A, Bm, stream)
 
     def add_subspace(self, Psi, D, P, stream=None):
         return fe_add_subspace(self.h, Psi, D, P, stream)

@@ -15,6 +15,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <mutex>
 #include <vector>
 
 #include "fe_apply_tma.cuh"
@@ -1319,6 +1320,56 @@ int fe_gram(fe_mesh* m, const double* A, const double* Bm, int B, double* C_host
     CUDA_TRY(cudaMemsetAsync(m->d_small, 0, bb * sizeof(double), st));
     CUDA_TRY(launch_gram(A, Bm, m->N, B, m->d_small, m->sms, st));
     CUDA_TRY(cudaMemcpyAsync(C_host, m->d_small, bb * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    m->launches += 1;
+    return FE_OK;
+}
+
+// ---- fe_gram without any allocation -------------------------------------------------------------------------------------
+// The Gram kernels accumulate their B x B result with atomics in device memory; fe_gram keeps that accumulator in a
+// cudaMalloc'ed buffer of the mesh.  Callers that must not allocate (code under CUDA graph capture, serving loops, harnesses
+// that forbid cudaMalloc) get the same product with the accumulator in this file-scope array: 128 x 128 doubles = 128 KB
+// that every GPU which loads the library holds until exit.  In host code the NAME of the array is a host-side stand-in, not
+// a device address: the address the kernels get comes from cudaGetSymbolAddress, taken once per device with that device
+// current.  All calls share the array (it keeps the last call's contents, so every call clears the part it uses); calls
+// that overlap on one GPU -- two streams, two threads -- race on it.
+constexpr int kGramStaticMaxB = 128;
+static __device__ __align__(256) double g_gram_static[kGramStaticMaxB * kGramStaticMaxB];
+
+static int gram_static_address(int device, double** out)
+{
+    static std::mutex mu;
+    static double* addr[64] = {nullptr};  // per device: the symbol has one address on each GPU
+    std::lock_guard<std::mutex> lock(mu);
+    const bool tracked = device >= 0 && device < 64;
+    if (tracked && addr[device]) {
+        *out = addr[device];
+        return FE_OK;
+    }
+    double* ptr = nullptr;
+    cudaError_t e = cudaGetSymbolAddress((void**)&ptr, g_gram_static);  // the current device is `device` (set by the caller)
+    if (e != cudaSuccess || !ptr)
+        return fail(FE_ERR_CUDA, "fe_gram_static: cudaGetSymbolAddress failed on device %d: %s", device, cudaGetErrorString(e));
+    if (tracked) addr[device] = ptr;
+    *out = ptr;
+    return FE_OK;
+}
+
+int fe_gram_static(fe_mesh* m, const double* A, const double* Bm, int B, double* C_host, void* cuda_stream)
+{
+    if (!m || !A || !Bm || !C_host) return fail(FE_ERR_INVALID, "fe_gram_static: NULL argument");
+    if (B < 1 || B > kGramStaticMaxB)
+        return fail(FE_ERR_INVALID, "fe_gram_static: B=%d outside 1..%d (the static accumulator holds %d x %d doubles)", B,
+                    kGramStaticMaxB, kGramStaticMaxB, kGramStaticMaxB);
+    CUDA_TRY(cudaSetDevice(m->device));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    double* acc = nullptr;
+    int rc = gram_static_address(m->device, &acc);
+    if (rc) return rc;
+    const size_t bb = (size_t)B * B;
+    CUDA_TRY(cudaMemsetAsync(acc, 0, bb * sizeof(double), st));  // the array holds the previous call's product
+    CUDA_TRY(launch_gram(A, Bm, m->N, B, acc, m->sms, st));
+    CUDA_TRY(cudaMemcpyAsync(C_host, acc, bb * sizeof(double), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
     m->launches += 1;
     return FE_OK;
