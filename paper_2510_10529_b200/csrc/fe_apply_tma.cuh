@@ -189,6 +189,19 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
     for (int ay = 0; ay < n; ++ay)
 #pragma unroll
         for (int ax = 0; ax < n; ++ax) v[ay][ax] = pA[(ay * n + ax) * BT];
+    if (FIRST) {
+        // Caller data may hold NaN / Inf in the Dirichlet rows (R5: "ignored"): those values are selected to 0 here, once,
+        // and only in the cells that touch the box surface (s_g = 0 nowhere else; the branch is uniform over the CTA), so
+        // the interior cells run exactly the arithmetic of the later steps.  (Selecting at every use cost 5 % of a FIRST
+        // launch: 3 instructions per value against one DMUL.)
+        if (ex == 0 || ey == 0 || ez == 0 || ex == prm.cx - 1 || ey == prm.cy - 1 || ez == prm.cz - 1) {
+#pragma unroll
+            for (int ay = 0; ay < n; ++ay)
+#pragma unroll
+                for (int ax = 0; ax < n; ++ax)
+                    v[ay][ax] = (__double2hiint(sin_pl[ay * NP + ax]) != 0) ? v[ay][ax] : 0.0;
+        }
+    }
     if (early) {
         if (pl < P) {
             // compact p x p sub-planes: beta' X -> own plane of bufA (store to W), kappa X -> own plane of bufB (add to Y)
@@ -196,8 +209,7 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
             for (int ay = 0; ay < P; ++ay)
 #pragma unroll
                 for (int ax = 0; ax < P; ++ax) {
-                    double x = v[ay][ax];
-                    if (FIRST) x = (__double2hiint(sin_pl[ay * NP + ax]) != 0) ? x : 0.0;
+                    const double x = v[ay][ax];
                     if (prm.preinit) pA[(ay * P + ax) * BT] = prm.beta_next * x;
                     if (prm.owner) pB[(ay * P + ax) * BT] = kappa * x;
                     if (DOTS) dacc = fma(kappa * x, x, dacc);
@@ -211,15 +223,11 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
             bulk_commit();
         }
     }
-    // a1: xhat = mu_g s_g x.  Caller data (FIRST) may hold NaN / Inf in the Dirichlet rows (R5: "ignored"), so those
-    // rows are selected to 0 instead of multiplied by s_g = 0
+    // a1: xhat = mu_g s_g x (the Dirichlet rows of caller data are already 0)
 #pragma unroll
     for (int ay = 0; ay < n; ++ay)
 #pragma unroll
-        for (int ax = 0; ax < n; ++ax) {
-            const double sg = sin_pl[ay * NP + ax];
-            v[ay][ax] = (!FIRST || __double2hiint(sg) != 0) ? v[ay][ax] * sg : 0.0;
-        }
+        for (int ax = 0; ax < n; ++ax) v[ay][ax] *= sin_pl[ay * NP + ax];
 #pragma unroll
     for (int ay = 0; ay < n; ++ay) {
         mat1d_eo<n>(prm.eoN, v[ay], o);
