@@ -83,6 +83,7 @@ __device__ __forceinline__ void tma_store4(const CUtensorMap* m, const void* src
 }
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read1() { asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory"); }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // Walk order of the cells: x fastest inside T x T blocks of (y, z) columns (T divides cy and cz; T = 1 is the plain
@@ -108,12 +109,18 @@ struct TmaShape {
     static constexpr int REC_SLIM = 2 * SMALL + 8;  // SLIM kernels leave the kz s_g tile out and multiply by kz instead
 };
 
-template <int P, int BT, bool SLIM = false>
+// STAGED shapes (p = 6 at 32 vectors, p = 7): the last rows of every output plane leave from a staging tile of their own instead
+// of bufB, so the next unit can write bufB while the bulk engine still reads them (k_apply_tma, plane phase 2)
+template <int P, int BT, bool SLIM, bool DOTS>
+__host__ __device__ constexpr bool tma_staged() { return !SLIM && !DOTS && ((P == 6 && BT == 32) || P == 7); }
+
+template <int P, int BT, bool SLIM = false, bool DOTS = false>
 constexpr size_t tma_smem_bytes()
 {
     constexpr int n = P + 1;
     if (SLIM) return ((size_t)2 * n * n * n * BT + TmaShape<n>::REC_SLIM) * sizeof(double) + 16;
-    return ((size_t)2 * n * n * n * BT + 2 * TmaShape<n>::REC + n * BT) * sizeof(double) + 16;
+    return ((size_t)2 * n * n * n * BT + 2 * TmaShape<n>::REC + (DOTS ? n * BT : 0) +
+            (tma_staged<P, BT, SLIM, DOTS>() ? n * (n / 2) * n * BT : 0)) * sizeof(double) + 16;
 }
 
 // FIRST: X is caller data whose Dirichlet rows may hold anything (R5) -> mask them in the owner / pre-init terms.
@@ -133,7 +140,10 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
     double* buf1 = smem + n3 * BT;      // [n^3][BT]  bufB: owner term -> A2 -> R -> scaled output (source of the reduce-add)
     double* rec0 = buf1 + n3 * BT;      // two cell records (double-buffered like the tiles): VZ [qx][qy][NP],
     double* rec1 = SLIM ? rec0 : rec0 + REC;  //   s_g [az][ay][NP], {ky/kx, kx/kz, kz}, kz s_g [az][ay][NP]
-    unsigned long long* bar = (unsigned long long*)(rec1 + REC);  // bar[0]: tile + record landed; bar[1]: A consumed
+    constexpr bool STG = tma_staged<P, BT, SLIM, DOTS>();
+    constexpr int H2 = n / 2, CPL = H2 * n * BT;  // staging tile: the last H2 rows of each output plane
+    double* bufC = rec1 + REC;
+    unsigned long long* bar = (unsigned long long*)(bufC + (STG ? n * CPL : 0));  // bar[0]: tile + record landed; bar[1]: A consumed
     double* red = (double*)(bar + 2);   // [n][BT] DOTS: per-plane partial sums of the unit
     const int lane = threadIdx.x, pl = threadIdx.y, tid = pl * BT + lane;
     const int nbt = (prm.B + BT - 1) / BT;
@@ -169,7 +179,9 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
         const int j = j0 + lane;
         kappa = -prm.alpha * (prm.c + ((prm.eps && j < prm.B) ? prm.eps[j] : 0.0));
     }
-    if (lane == 0) bulk_wait_read0();  // the previous unit's reduce-add has read its source (bufB)
+    if (lane == 0) {  // the previous unit's reduce-adds have read their sources in bufB (the staged last one may still be reading)
+        if (STG) bulk_wait_read1(); else bulk_wait_read0();
+    }
     __syncwarp();
     mbar_wait(bar, parity);
     parity ^= 1;
@@ -386,12 +398,18 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
     }
     const double* sout_pl = sOut + pl * n * NP;
     constexpr int H1 = (n + 1) / 2;  // the plane leaves in two bulk reduce-adds: the first overlaps the remaining rows
+    double* pC = STG ? bufC + (size_t)pl * CPL + lane - (size_t)H1 * n * BT : pB;  // rows ay >= H1 (staged: a tile of their own)
+    if (STG) {  // the previous unit's last reduce-add (a whole unit ago) has read the staging tile
+        if (lane == 0) bulk_wait_read0();
+        __syncwarp();
+    }
 #pragma unroll
     for (int ay = 0; ay < n; ++ay) {
         mat1d_eo<n>(prm.eoNTa, v[ay], o);
+        double* dst = ay < H1 ? pB : pC;
 #pragma unroll
         for (int ax = 0; ax < n; ++ax)
-            pB[(ay * n + ax) * BT] = (SLIM ? kzs * sout_pl[ay * NP + ax] : sout_pl[ay * NP + ax]) * o[ax];
+            dst[(ay * n + ax) * BT] = (SLIM ? kzs * sout_pl[ay * NP + ax] : sout_pl[ay * NP + ax]) * o[ax];
         if (ay == H1 - 1 && H1 < n) {
             fence_async_smem();
             __syncwarp();
@@ -405,7 +423,7 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_tma(const __grid_c
     __syncwarp();
     if (lane == 0) {
         if (H1 < n)
-            tma_reduce_add4(&prm.mYh2, pB + (size_t)H1 * n * BT, j0, gx0, gy0 + H1, gz0 + pl);
+            tma_reduce_add4(&prm.mYh2, pC + (size_t)H1 * n * BT, j0, gx0, gy0 + H1, gz0 + pl);
         else
             tma_reduce_add4(&prm.mYh1, pB, j0, gx0, gy0, gz0 + pl);
         bulk_commit();
@@ -431,7 +449,7 @@ template <int P, int BT, int MINB>
 cudaError_t launch_tma(const TmaParams& prm, long long ncells, bool first, cudaStream_t st, int ctas)
 {
     constexpr int n = P + 1;
-    constexpr size_t smem = tma_smem_bytes<P, BT>();
+    constexpr size_t smem = tma_smem_bytes<P, BT>(), smem_d = tma_smem_bytes<P, BT, false, true>();
     static PerDeviceOnce once;
     cudaError_t e0 = once_per_device(once, [&] {
         cudaError_t e = cudaFuncSetAttribute(k_apply_tma<P, BT, MINB, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -451,16 +469,16 @@ cudaError_t launch_tma(const TmaParams& prm, long long ncells, bool first, cudaS
         if (!first) return cudaErrorInvalidValue;
         static PerDeviceOnce once_d;
         cudaError_t ed = once_per_device(once_d, [&] {
-            cudaError_t e = cudaFuncSetAttribute(k_apply_tma<P, BT, MINB, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            cudaError_t e = cudaFuncSetAttribute(k_apply_tma<P, BT, MINB, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_d);
             if (e == cudaSuccess)
-                e = cudaFuncSetAttribute(k_apply_tma<P, BT, MINB, true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+                e = cudaFuncSetAttribute(k_apply_tma<P, BT, MINB, true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_d);
             return e;
         });
         if (ed != cudaSuccess) return ed;
         if (persist)
-            k_apply_tma<P, BT, MINB, true, true, true><<<grid, block, smem, st>>>(prm);
+            k_apply_tma<P, BT, MINB, true, true, true><<<grid, block, smem_d, st>>>(prm);
         else
-            k_apply_tma<P, BT, MINB, true, false, true><<<grid, block, smem, st>>>(prm);
+            k_apply_tma<P, BT, MINB, true, false, true><<<grid, block, smem_d, st>>>(prm);
         return cudaGetLastError();
     }
     if (persist) {
