@@ -181,7 +181,9 @@ int fe_apply_potential(fe_mesh* m, const double* Uq_dev, const double* X, double
  * scatter (the 8 parity classes of the cell grid launched in order: cells of one class share no node, so every sum
  * has a fixed order and results are bit-reproducible; slower; on a general mesh: cells coloured greedily so that no two
  * cells of a colour share a node, launched colour by colour, hanging contributions collapsed over the transposed constraint
- * rows), 5..8 = launch shapes of the TMA kernel (fe_apply_tma.cuh; test and experiment hooks).  FE_ERR_INVALID if unknown. */
+ * rows), 5..8 = launch shapes of the TMA kernel (fe_apply_tma.cuh; test and experiment hooks), 9 = on a general mesh whose
+ * cells are all axis-aligned boxes: the generic 12-sweep cell kernel instead of the 10-sweep box-cell kernel (cross-check).
+ * FE_ERR_INVALID if unknown. */
 int fe_set_variant(fe_mesh* m, int variant);
 /* Kernels launched by this handle since creation (bench.py's gpu_launches). */
 int64_t fe_launch_count(const fe_mesh* m);

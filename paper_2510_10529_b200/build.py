@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libfecheb.so")
 SOURCES = ["fe_cheb.cu", "fe_tables.cpp", "fe_general.cpp"]
-DEPS = SOURCES + ["fe_kernels.cuh", "fe_apply_tma.cuh", "fe_rr.cuh", "fe_minres.cuh", "fe_density.cuh", "fe_diag.cuh", "fe_general.cuh", "fe_general.h", "fe_tables.h", os.path.join("..", "..", "include", "fe_cheb.h")]
+DEPS = SOURCES + ["fe_kernels.cuh", "fe_apply_tma.cuh", "fe_rr.cuh", "fe_minres.cuh", "fe_density.cuh", "fe_diag.cuh", "fe_general.cuh", "fe_gbox.cuh", "fe_general.h", "fe_tables.h", os.path.join("..", "..", "include", "fe_cheb.h")]
 
 
 def nvcc_command(extra=()):

@@ -22,6 +22,7 @@
 #include "fe_density.cuh"
 #include "fe_diag.cuh"
 #include "fe_general.cuh"
+#include "fe_gbox.cuh"
 #include "fe_general.h"
 #include "fe_minres.cuh"
 #include "fe_rr.cuh"
@@ -88,6 +89,10 @@ struct fe_mesh {
     std::vector<int64_t> colour_off;      //   colour c = cells [colour_off[c], colour_off[c+1])
     double *d_Xh = nullptr, *d_Yh = nullptr;  // (N_all - N) * hcap: expanded hanging values / their scatter target
     double* d_grecU = nullptr;  // fe_apply_potential on a general mesh: records with zero metric and WV = w |J| U
+    // general mesh whose cells are all axis-aligned boxes (octree leaves of a box): the 10-sweep kernel of fe_gbox.cuh
+    bool gbox = false, gbox_off = false;  // gbox_off: fe_apply_potential borrows the generic kernel (records with zero metric)
+    double* d_gbrec = nullptr;            // ncells * gbox_rec_doubles(n)
+    EOTab bxN, bxNT, bxG;                 // folded tables N', N'^T, G' (as on box meshes)
     int hcap = 0;
     int sms = 0;  // multiprocessors of the device (persistent grid size)
     int64_t launches = 0;
@@ -113,7 +118,7 @@ static void make_eo(const double* M, int n, bool transpose, EOTab* T)
 static int small_tile(int n) { return 3 * n * n * (n + (n & 1)) + 8; }  // REC of fe_apply_tma.cuh
 
 // Gauss weights folded into the 1-D tables (fe_apply_tma.cuh): N' = diag(sqrt w) N, G' = diag(w^-1/2) G diag(w^-1/2)
-static void build_folded_tables(fe_mesh* m)
+static void build_folded_tables(const fe_mesh* m, EOTab* eoN, EOTab* eoNT, EOTab* eoG)
 {
     const int n = m->n;
     double Np[kMaxN * kMaxN], Gp[kMaxN * kMaxN];
@@ -122,9 +127,9 @@ static void build_folded_tables(fe_mesh* m)
             Np[q * n + a] = std::sqrt(m->tab.gl_w[q]) * m->tab.N[q * n + a];
             Gp[q * n + a] = m->tab.G[q * n + a] / std::sqrt(m->tab.gl_w[q] * m->tab.gl_w[a]);
         }
-    make_eo(Np, n, false, &m->eoN);
-    make_eo(Np, n, true, &m->eoNT);
-    make_eo(Gp, n, false, &m->eoG);
+    make_eo(Np, n, false, eoN);
+    make_eo(Np, n, true, eoNT);
+    make_eo(Gp, n, false, eoG);
 }
 
 static void axis_mass(const std::vector<double>& e, int c, int p, const Tables1D& t, std::vector<double>& m)
@@ -208,7 +213,7 @@ int fe_mesh_create(const double* xe, int cx, const double* ye, int cy, const dou
     m->launches += 1;
     ce = cudaDeviceSynchronize();
     if (ce != cudaSuccess) return cleanup(fail(FE_ERR_CUDA, "fe_mesh_create: scaling kernel failed: %s", cudaGetErrorString(ce)));
-    build_folded_tables(m);
+    build_folded_tables(m, &m->eoN, &m->eoNT, &m->eoG);
     *out = m;
     return cleanup(FE_OK);
 }
@@ -223,7 +228,7 @@ int fe_mesh_destroy(fe_mesh* m)
     cudaFree(m->d_small); cudaFree(m->d_minv); cudaFree(m->d_mask); cudaFree(m->d_scal);
     cudaFree(m->d_VZ); cudaFree(m->d_sx); cudaFree(m->d_sy); cudaFree(m->d_sz);
     cudaFree(m->d_gl2g); cudaFree(m->d_gmetric); cudaFree(m->d_gwdet); cudaFree(m->d_gsc);
-    cudaFree(m->d_Xh); cudaFree(m->d_Yh); cudaFree(m->d_grecU);
+    cudaFree(m->d_Xh); cudaFree(m->d_Yh); cudaFree(m->d_grecU); cudaFree(m->d_gbrec);
     cudaFree(m->gexp.bptr); cudaFree(m->gexp.bcol); cudaFree(m->gexp.brow); cudaFree(m->gexp.out); cudaFree(m->gexp.bw);
     cudaFree(m->gtr.bptr); cudaFree(m->gtr.bcol); cudaFree(m->gtr.brow); cudaFree(m->gtr.out); cudaFree(m->gtr.bw);
     cudaFree(m->d_colcells);
@@ -364,6 +369,11 @@ int fe_set_potential(fe_mesh* m, const double* Vq_dev, int copy, void* cuda_stre
                                                                                   gen_rec_doubles(m->n));
         CUDA_TRY(cudaGetLastError());
         m->launches += 1;
+        if (m->gbox) {
+            k_gbox_weight_potential<<<m->sms * 8, 256, 0, (cudaStream_t)cuda_stream>>>(m->d_gbrec, Vq_dev, m->ncells, m->n);
+            CUDA_TRY(cudaGetLastError());
+            m->launches += 1;
+        }
         m->have_V = true;
         return FE_OK;
     }
@@ -539,6 +549,46 @@ int fe_mesh_create_general(int cx, int cy, int cz, const int32_t* cells, int64_t
         fe_mesh_destroy(m);
         return rc;
     }
+    // Octree leaves of an undeformed box (the paper's adaptive meshes, l.273): every cell is an axis-aligned box, the metric
+    // is diagonal and constant per cell, and the 10-sweep kernel of fe_gbox.cuh applies.  Corner v = vx + 2 (vy + 2 vz).
+    if (gbox_supported(p)) {
+        const int n = m->n, NP = n + (n & 1), SMALL = n * n * NP, brec = gbox_rec_doubles(n);
+        std::vector<double> br((size_t)ncells * brec, 0.0);
+        bool all_boxes = true;
+        for (int64_t e = 0; e < ncells && all_boxes; ++e) {
+            const double* c = verts + e * 24;
+            double lo[3], h[3];
+            for (int d = 0; d < 3; ++d) { lo[d] = c[d]; h[d] = c[3 * (1 << d) + d] - c[d]; }
+            for (int v = 0; v < 8 && all_boxes; ++v)
+                for (int d = 0; d < 3; ++d) {
+                    const double want = lo[d] + (((v >> d) & 1) ? h[d] : 0.0);
+                    if (!(h[d] > 0.0) || std::fabs(c[3 * v + d] - want) > 1e-13 * (std::fabs(want) + h[d])) all_boxes = false;
+                }
+            if (!all_boxes) break;
+            double* r = &br[(size_t)e * brec];
+            const double kz = 0.25 * h[0] * h[1] / h[2];  // 2J/hz^2, J = hx hy hz / 8
+            bool dirichlet = false;
+            for (int az = 0; az < n; ++az)
+                for (int ay = 0; ay < n; ++ay)
+                    for (int ax = 0; ax < n; ++ax) {
+                        const double sc = scv[(size_t)e * m->nc + ax + n * (ay + n * az)];
+                        r[SMALL + (az * n + ay) * NP + ax] = sc;
+                        r[2 * SMALL + 8 + (az * n + ay) * NP + ax] = kz * sc;
+                        dirichlet = dirichlet || sc == 0.0;
+                    }
+            r[2 * SMALL + 0] = (h[0] * h[0]) / (h[1] * h[1]);
+            r[2 * SMALL + 1] = (h[2] * h[2]) / (h[0] * h[0]);
+            r[2 * SMALL + 2] = kz;
+            r[2 * SMALL + 3] = 0.5 * h[2] * h[2];
+            r[2 * SMALL + 4] = dirichlet ? 1.0 : 0.0;
+            memcpy(r + 3 * SMALL + 8, &g.l2g[(size_t)e * m->nc], (size_t)m->nc * sizeof(int32_t));
+        }
+        if (all_boxes) {
+            if ((rc = upload_vec(&m->d_gbrec, br))) { fe_mesh_destroy(m); return rc; }
+            build_folded_tables(m, &m->bxN, &m->bxNT, &m->bxG);
+            m->gbox = true;
+        }
+    }
     *out = m;
     return FE_OK;
 }
@@ -651,31 +701,44 @@ static int general_step(fe_mesh* m, const double* X, const double* Z, double* Y,
     else
         k_gen_init<<<grid, rows, 0, st>>>(Y, X, Z, m->d_sm, eps, alpha, beta, c, g.N, B);
     if (nh > 0) CUDA_TRY(cudaMemsetAsync(m->d_Yh, 0, (size_t)nh * B * sizeof(double), st));
+    // all cells axis-aligned boxes: the 10-sweep kernel (variant 9 keeps the generic 12-sweep kernel as a cross-check)
+    const bool box = m->gbox && !m->gbox_off && m->variant != 9;
     GenParams prm;
     memset(&prm, 0, sizeof(prm));
     prm.X = X; prm.Xh = m->d_Xh ? m->d_Xh : X; prm.Y = Y; prm.Yh = m->d_Yh ? m->d_Yh : Y; prm.sc = m->d_gsc; prm.l2g = m->d_gl2g;
     prm.rec = m->d_gmetric; prm.N = g.N; prm.ncells = m->ncells; prm.B = B; prm.alpha = alpha;
     prm.eoN = m->eoN; prm.eoNT = m->eoNT; prm.eoD = m->eoD; prm.eoDT = m->eoDT;
+    GBoxParams bp;
+    if (box) {
+        memset(&bp, 0, sizeof(bp));
+        bp.X = prm.X; bp.Xh = prm.Xh; bp.Y = prm.Y; bp.Yh = prm.Yh; bp.rec = m->d_gbrec; bp.N = g.N; bp.ncells = m->ncells; bp.B = B;
+        bp.eoN = m->bxN; bp.eoNT = m->bxNT; bp.eoG = m->bxG; bp.eoNTa = m->bxNT;
+        for (double& x : bp.eoNTa.S) x *= alpha;
+        for (double& x : bp.eoNTa.A) x *= alpha;
+        for (double& x : bp.eoNTa.Mid) x *= alpha;
+    }
+    // the box kernel delivers alpha yhat to the hanging targets too (alpha sits in its last table): the collapse runs with 1
+    const double alpha_h = box ? 1.0 : alpha;
     if (m->variant == 4) {  // colour-ordered, bit-reproducible
         if ((rc = ensure_general_colours(m))) return rc;
         for (size_t c = 0; c + 1 < m->colour_off.size(); ++c) {
-            prm.cell_list = m->d_colcells + m->colour_off[c];
-            prm.ncells = m->colour_off[c + 1] - m->colour_off[c];
-            cudaError_t ec = launch_apply_gen(prm, m->p, prm.ncells, m->sms, st);
+            prm.cell_list = bp.cell_list = m->d_colcells + m->colour_off[c];
+            prm.ncells = bp.ncells = m->colour_off[c + 1] - m->colour_off[c];
+            cudaError_t ec = box ? launch_apply_gbox(bp, m->p, bp.ncells, m->sms, st) : launch_apply_gen(prm, m->p, prm.ncells, m->sms, st);
             if (ec != cudaSuccess) return fail(FE_ERR_CUDA, "operator launch (general mesh) failed: %s", cudaGetErrorString(ec));
         }
         if (nh > 0)
             k_gen_rows_times_block<<<grid, rows, 0, st>>>(Y, m->d_Yh, m->gtr.bptr, m->gtr.bcol, m->gtr.bw, m->gtr.brow, m->gtr.out,
-                                                          m->gtr.nb, B, alpha, 1);
+                                                          m->gtr.nb, B, alpha_h, 1);
         CUDA_TRY(cudaGetLastError());
         m->launches += (int64_t)m->colour_off.size() + (nh > 0 ? 2 : 1);
         return FE_OK;
     }
-    cudaError_t e = launch_apply_gen(prm, m->p, m->ncells, m->sms, st);
+    cudaError_t e = box ? launch_apply_gbox(bp, m->p, m->ncells, m->sms, st) : launch_apply_gen(prm, m->p, m->ncells, m->sms, st);
     if (e != cudaSuccess) return fail(FE_ERR_CUDA, "operator launch (general mesh) failed: %s", cudaGetErrorString(e));
     if (nh > 0)
         k_gen_collapse<<<grid, rows, 0, st>>>(Y, m->d_Yh, m->gexp.bptr, m->gexp.bcol, m->gexp.bw, m->gexp.brow, m->gexp.out, m->gexp.nb, B,
-                                              alpha);
+                                              alpha_h);
     CUDA_TRY(cudaGetLastError());
     m->launches += nh > 0 ? 3 : 2;
     return FE_OK;
@@ -1554,7 +1617,9 @@ int fe_apply_potential(fe_mesh* m, const double* Uq_dev, const double* X, double
         m->launches += 1;
         double* keep = m->d_gmetric;
         m->d_gmetric = m->d_grecU;
+        m->gbox_off = true;  // the potential-only operator goes through the generic kernel (zero metric)
         const int rcg = general_step(m, X, nullptr, Y, B, nullptr, 1.0, 0.0, 0.0, gst);
+        m->gbox_off = false;
         m->d_gmetric = keep;
         return rcg;
     }

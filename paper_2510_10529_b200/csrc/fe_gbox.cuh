@@ -1,0 +1,302 @@
+// fe_gbox.cuh -- the fused operator step on a general mesh (explicit l2g, hanging nodes) whose cells are all AXIS-ALIGNED
+// BOXES: the leaves of an octree refinement of a box, the shape of the paper's adaptive meshes (Fig. 6).
+//
+// On such a cell the metric of Eq. 17 (l.171) is diagonal and constant, so the kinetic term separates and the cell
+// contraction is the 10-sweep, plane-in-registers form of the box-mesh kernel (fe_apply_tma.cuh: A = N'y N'x xhat,
+// A2 = G'x A + (ky/kx) G'y A per nodal plane; U = N'z A, T = VZ.U + G'z U + (kx/kz) N'z A2, R = N'z^T T per line;
+// yhat / kz = N'x^T N'y^T R per nodal plane) instead of the generic 12 sweeps over shared-memory lines of k_apply_gen
+// (fe_general.cuh).  What differs from the box-mesh kernel is the data movement: a refined mesh is no tensor, so
+//   gather  : every thread copies the n x n rows of ITS nodal plane through the explicit l2g (8-byte cp.async into the field
+//             it will read itself; unconstrained nodes from X, hanging nodes from the expanded values X_h = C_h (s . X));
+//             the copies of the next unit are issued when the line phase has released the field, and run under plane phase 2;
+//   scatter : red.global.add.f64 per value into Y (unconstrained) or Y_h (hanging; k_gen_collapse distributes it);
+//   record  : one bulk copy per unit brings V_q hz^2/2, the gather and scatter scales, the cell's ratios and its n^3 ids.
+// The diagonal terms of the step (shift, recurrence) are written by k_gen_init as for every general mesh.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdint>
+
+#include "fe_apply_tma.cuh"
+#include "fe_kernels.cuh"
+
+namespace fecheb {
+
+// per-cell record: VZ [qx][qy][NP] | s [az][ay][NP] (gather scale: s_g, 1 at hanging nodes) | tail (8) | kz s [az][ay][NP]
+// | ids (n^3 int32, padded to a multiple of 4).  tail = { ky/kx, kx/kz, kz, hz^2/2, 1 if a node of the cell is a Dirichlet
+// node, 0, 0, 0 }
+template <int n>
+struct GBoxShape {
+    static constexpr int NP = n + (n & 1), SMALL = n * n * NP, N3P = (n * n * n + 3) & ~3;
+    static constexpr int TAIL = 2 * SMALL, SOUT = 2 * SMALL + 8, IDS = 3 * SMALL + 8;
+    static constexpr int REC = IDS + N3P / 2;  // doubles (even: every piece is)
+};
+__host__ __device__ inline int gbox_rec_doubles(int n) { const int NP = n + (n & 1); return 3 * n * n * NP + 8 + (((n * n * n + 3) & ~3) / 2); }
+
+struct GBoxParams {
+    const double* X;     // N * B
+    const double* Xh;    // (N_all - N) * B: expanded hanging values
+    double* Y;           // N * B, holds the diagonal terms (k_gen_init)
+    double* Yh;          // (N_all - N) * B, zero on entry
+    const double* rec;   // ncells * REC
+    const int32_t* cell_list;  // NULL: all cells; else the cells of one colour (colour-ordered scatter)
+    long long N, ncells;
+    int B;
+    EOTab eoN, eoNT, eoG;  // even-odd halves of N' = diag(sqrt w) N, N'^T, G' = diag(w^-1/2) G diag(w^-1/2)
+    EOTab eoNTa;           // alpha N'^T: unconstrained AND hanging targets receive alpha yhat (the collapse then runs with 1)
+};
+
+// VZ tile of every record from the caller's V[e][q], q = qx + n (qy + n qz)
+__global__ void k_gbox_weight_potential(double* __restrict__ rec, const double* __restrict__ V, long long ncells, int n)
+{
+    const int NP = n + (n & 1), n3 = n * n * n, REC = gbox_rec_doubles(n), TAIL = 2 * n * n * NP;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < ncells * n3; i += (long long)gridDim.x * blockDim.x) {
+        const long long e = i / n3;
+        const int q = (int)(i - e * n3), qx = q % n, qy = (q / n) % n, qz = q / (n * n);
+        rec[e * REC + (qx * n + qy) * NP + qz] = rec[e * REC + TAIL + 3] * V[i];
+    }
+}
+
+template <int P, int BT>
+constexpr size_t gbox_smem_bytes()
+{
+    constexpr int n = P + 1;
+    return ((size_t)2 * n * n * n * BT + 2 * GBoxShape<n>::REC) * sizeof(double) + 16;
+}
+
+// Block (BT lanes = vectors, n nodal planes).  A CTA walks units (cell, tile of BT vectors) u = blockIdx.x, + gridDim.x, ...
+template <int P, int BT, int MINB>
+__global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_gbox(const __grid_constant__ GBoxParams prm)
+{
+    constexpr int n = P + 1, n2 = n * n, n3 = n * n * n, NP = GBoxShape<n>::NP, SMALL = GBoxShape<n>::SMALL,
+                  REC = GBoxShape<n>::REC, TAIL = GBoxShape<n>::TAIL, SOUT = GBoxShape<n>::SOUT, IDS = GBoxShape<n>::IDS;
+    extern __shared__ __align__(128) double smem[];
+    double* bufA = smem;               // [n^3][BT]  gathered X -> A (free once the line phase is over) -> next unit's X
+    double* bufB = smem + n3 * BT;     // [n^3][BT]  A2 -> R
+    double* recs = bufB + n3 * BT;     // [2][REC]
+    unsigned long long* bar = (unsigned long long*)(recs + 2 * REC);  // bar[b]: record b landed
+    const int lane = threadIdx.x, pl = threadIdx.y, tid = pl * BT + lane;
+    const int nbt = (prm.B + BT - 1) / BT;
+    const long long nunits = prm.ncells * nbt, B = prm.B;
+
+    auto request_rec = [&](long long u, int b) {  // one thread
+        const long long cu = u / nbt, c = prm.cell_list ? (long long)prm.cell_list[cu] : cu;
+        mbar_expect_tx(bar + b, (unsigned)(REC * sizeof(double)));
+        bulk_load(recs + b * REC, prm.rec + c * REC, (unsigned)(REC * sizeof(double)), bar + b);
+    };
+    // the rows of this thread's nodal plane, straight into the plane of bufA it reads itself (no CTA barrier in between)
+    auto request_rows = [&](long long u, int b) {
+        const int32_t* ids = reinterpret_cast<const int32_t*>(recs + b * REC + IDS) + pl * n2;
+        const int j = (int)(u % nbt) * BT + lane;
+        const bool act = j < prm.B;
+        double* dst = bufA + (size_t)pl * n2 * BT + lane;
+#pragma unroll
+        for (int a = 0; a < n2; ++a) {
+            const long long g = ids[a];
+            const double* src = g < prm.N ? prm.X + g * B + j : prm.Xh + (g - prm.N) * B + j;
+            cp_async8(dst + a * BT, act ? src : prm.X, act);
+        }
+        cp_async_commit();
+    };
+
+    if (tid == 0) {
+        mbar_init(bar, 1);
+        mbar_init(bar + 1, 1);
+    }
+    __syncthreads();
+    unsigned ph0 = 0, ph1 = 0;
+    if ((long long)blockIdx.x < nunits) {
+        if (tid == 0) request_rec(blockIdx.x, 0);
+        mbar_wait(bar, ph0);
+        ph0 ^= 1;
+        request_rows(blockIdx.x, 0);
+    }
+    int buf = 0;
+    for (long long u = blockIdx.x; u < nunits; u += gridDim.x, buf ^= 1) {
+    const long long un = u + gridDim.x;
+    const bool more = un < nunits;
+    const int j = (int)(u % nbt) * BT + lane;
+    const bool act = j < prm.B;
+    const double* rec = recs + buf * REC;
+    const double* sVZ = rec;
+    const double ry = rec[TAIL], rxz = rec[TAIL + 1];
+    const bool surface = rec[TAIL + 4] != 0.0;
+
+    double v[n][n], t[n], o[n];
+    double* pA = bufA + (size_t)pl * n2 * BT + lane;
+    double* pB = bufB + (size_t)pl * n2 * BT + lane;
+    const double* sin_pl = rec + SMALL + pl * n * NP;
+    cp_async_wait_all();  // this thread's own copies: the plane it reads now
+    // ---- plane phase 1 -----------------------------------------------------------------------------------------------
+#pragma unroll
+    for (int ay = 0; ay < n; ++ay)
+#pragma unroll
+        for (int ax = 0; ax < n; ++ax) v[ay][ax] = pA[(ay * n + ax) * BT];
+    if (surface) {  // Dirichlet rows of caller data are ignored (R5), whatever they hold; uniform over the CTA
+#pragma unroll
+        for (int ay = 0; ay < n; ++ay)
+#pragma unroll
+            for (int ax = 0; ax < n; ++ax)
+                v[ay][ax] = (__double2hiint(sin_pl[ay * NP + ax]) != 0) ? v[ay][ax] : 0.0;
+    }
+#pragma unroll
+    for (int ay = 0; ay < n; ++ay)
+#pragma unroll
+        for (int ax = 0; ax < n; ++ax) v[ay][ax] *= sin_pl[ay * NP + ax];
+#pragma unroll
+    for (int ay = 0; ay < n; ++ay) {
+        mat1d_eo<n>(prm.eoN, v[ay], o);
+#pragma unroll
+        for (int q = 0; q < n; ++q) v[ay][q] = o[q];
+    }
+#pragma unroll
+    for (int qx = 0; qx < n; ++qx) {
+#pragma unroll
+        for (int a = 0; a < n; ++a) t[a] = v[a][qx];
+        mat1d_eo<n>(prm.eoN, t, o);
+#pragma unroll
+        for (int q = 0; q < n; ++q) v[q][qx] = o[q];
+    }
+    if constexpr (n >= 7) {
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy)
+#pragma unroll
+            for (int qx = 0; qx < n; ++qx) pA[(qy * n + qx) * BT] = v[qy][qx];
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy) {
+            mat1d_eo<n>(prm.eoG, v[qy], o);
+#pragma unroll
+            for (int qx = 0; qx < n; ++qx) v[qy][qx] = o[qx];
+        }
+#pragma unroll
+        for (int qx = 0; qx < n; ++qx) {
+#pragma unroll
+            for (int a = 0; a < n; ++a) t[a] = pA[(a * n + qx) * BT];
+            mat1d_eo<n>(prm.eoG, t, o);
+#pragma unroll
+            for (int qy = 0; qy < n; ++qy) pB[(qy * n + qx) * BT] = fma(ry, o[qy], v[qy][qx]);
+        }
+    } else {
+        double v2[n][n];
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy) mat1d_eo<n>(prm.eoG, v[qy], v2[qy]);
+#pragma unroll
+        for (int qx = 0; qx < n; ++qx) {
+#pragma unroll
+            for (int a = 0; a < n; ++a) t[a] = v[a][qx];
+            mat1d_eo<n>(prm.eoG, t, o);
+#pragma unroll
+            for (int qy = 0; qy < n; ++qy) v2[qy][qx] = fma(ry, o[qy], v2[qy][qx]);
+        }
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy)
+#pragma unroll
+            for (int qx = 0; qx < n; ++qx) {
+                pA[(qy * n + qx) * BT] = v[qy][qx];
+                pB[(qy * n + qx) * BT] = v2[qy][qx];
+            }
+    }
+    __syncthreads();
+    // every thread is past the previous unit: its record buffer can take the next unit's record (needed at plane phase 2)
+    if (more && tid == 0) request_rec(un, buf ^ 1);
+    // ---- line phase: the thread owns the yz-plane qx = pl ----------------------------------------------------------------
+    {
+        double* la = bufA + (size_t)pl * BT + lane;
+        double* lb = bufB + (size_t)pl * BT + lane;
+        const double* lv = sVZ + pl * n * NP;
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy) {
+#pragma unroll
+            for (int az = 0; az < n; ++az) t[az] = la[((az * n + qy) * n) * BT];
+            mat1d_eo<n>(prm.eoN, t, v[qy]);
+        }
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy) {
+            mat1d_eo<n>(prm.eoG, v[qy], o);
+#pragma unroll
+            for (int qz = 0; qz < n; ++qz) v[qy][qz] = fma(lv[qy * NP + qz], v[qy][qz], o[qz]);
+        }
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy) {
+#pragma unroll
+            for (int az = 0; az < n; ++az) t[az] = lb[((az * n + qy) * n) * BT];
+            mat1d_eo<n>(prm.eoN, t, o);
+#pragma unroll
+            for (int qz = 0; qz < n; ++qz) v[qy][qz] = fma(rxz, o[qz], v[qy][qz]);
+        }
+#pragma unroll
+        for (int qy = 0; qy < n; ++qy) {
+            mat1d_eo<n>(prm.eoNT, v[qy], o);
+#pragma unroll
+            for (int az = 0; az < n; ++az) lb[((az * n + qy) * n) * BT] = o[az];
+        }
+    }
+    __syncthreads();
+    // bufA is free: the next unit's rows travel while this unit is back-interpolated and scattered
+    if (more) {
+        if (buf == 0) { mbar_wait(bar + 1, ph1); ph1 ^= 1; } else { mbar_wait(bar, ph0); ph0 ^= 1; }
+        request_rows(un, buf ^ 1);
+    }
+    // ---- plane phase 2: back-interpolate in y and x, scale by alpha kz s, scatter through the l2g -------------------------------
+#pragma unroll
+    for (int qy = 0; qy < n; ++qy)
+#pragma unroll
+        for (int qx = 0; qx < n; ++qx) v[qy][qx] = pB[(qy * n + qx) * BT];
+#pragma unroll
+    for (int qx = 0; qx < n; ++qx) {
+#pragma unroll
+        for (int q = 0; q < n; ++q) t[q] = v[q][qx];
+        mat1d_eo<n>(prm.eoNT, t, o);
+#pragma unroll
+        for (int a = 0; a < n; ++a) v[a][qx] = o[a];
+    }
+    const double* sout_pl = rec + SOUT + pl * n * NP;
+    const int32_t* ids = reinterpret_cast<const int32_t*>(rec + IDS) + pl * n2;
+#pragma unroll
+    for (int ay = 0; ay < n; ++ay) {
+        mat1d_eo<n>(prm.eoNTa, v[ay], o);
+#pragma unroll
+        for (int ax = 0; ax < n; ++ax) {
+            const double sc = sout_pl[ay * NP + ax];
+            const long long g = ids[ay * n + ax];
+            double* dst = g < prm.N ? prm.Y + g * B + j : prm.Yh + (g - prm.N) * B + j;
+            if (act && __double2hiint(sc) != 0) atomicAdd(dst, sc * o[ax]);
+        }
+    }
+    }  // units
+}
+
+template <int P, int BT, int MINB>
+cudaError_t launch_gbox_t(const GBoxParams& prm, long long ncells, int sms, cudaStream_t st)
+{
+    constexpr size_t smem = gbox_smem_bytes<P, BT>();
+    static PerDeviceOnce once;
+    cudaError_t e0 = once_per_device(once, [&] {
+        return cudaFuncSetAttribute(k_apply_gbox<P, BT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    });
+    if (e0 != cudaSuccess) return e0;
+    const long long nunits = ncells * ((prm.B + BT - 1) / BT);
+    if (nunits <= 0) return cudaSuccess;
+    dim3 grid((unsigned)std::min<long long>(nunits, (long long)sms * MINB)), block(BT, P + 1);
+    k_apply_gbox<P, BT, MINB><<<grid, block, smem, st>>>(prm);
+    return cudaGetLastError();
+}
+
+inline bool gbox_supported(int p) { return p >= 1 && p <= 7; }
+
+inline cudaError_t launch_apply_gbox(const GBoxParams& prm, int p, long long ncells, int sms, cudaStream_t st)
+{
+    switch (p) {
+        case 1: return launch_gbox_t<1, 32, 8>(prm, ncells, sms, st);
+        case 2: return launch_gbox_t<2, 32, 6>(prm, ncells, sms, st);
+        case 3: return launch_gbox_t<3, 32, 4>(prm, ncells, sms, st);
+        case 4: return launch_gbox_t<4, 32, 3>(prm, ncells, sms, st);
+        case 5: return launch_gbox_t<5, 32, 1>(prm, ncells, sms, st);
+        case 6: return launch_gbox_t<6, 32, 1>(prm, ncells, sms, st);
+        case 7: return launch_gbox_t<7, 16, 1>(prm, ncells, sms, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+}  // namespace fecheb

@@ -358,7 +358,7 @@ cudaError_t launch_v3(const ApplyParams& prm, long long ncells, cudaStream_t st)
 inline bool variant_supported(int p, int variant)
 {
     (void)p;
-    return variant == 0 || variant == 3 || variant == 4 || (variant >= 5 && variant <= 8);
+    return variant == 0 || variant == 3 || variant == 4 || (variant >= 5 && variant <= 9);
 }
 
 // One fused operator step.  *nlaunch = kernels (and memsets) enqueued.

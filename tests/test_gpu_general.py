@@ -279,3 +279,53 @@ def test_adaptive_workload_full_size_properties():
     Yf = gm.cheb_filter(X.clone(), m, a, b, a0)
     assert float(torch.linalg.norm(Yf - Yk) / torch.linalg.norm(Yk)) <= 1e-12
     assert float((Yf * (1 - mask)).abs().max()) == 0.0
+
+
+def _graded_box_mesh(levels=1):
+    """Undeformed octree leaves on an UNEQUALLY spaced root grid (hx != hy != hz, graded): every cell an axis-aligned box,
+    one or two levels of refinement near a corner region so that hanging faces and edges appear."""
+    ex = np.array([-1.6, -0.7, 0.1, 1.4])
+    ey = np.array([-1.2, -0.5, 0.4, 1.3])
+    ez = np.array([-1.5, -0.2, 0.5, 1.1])
+    r = {0: 1.0, 1: 0.55}
+    return workloads.octree_mesh(ex, ey, ez, lambda l, lo, hi: np.linalg.norm((lo + hi) / 2 - 0.2) < r[l], levels)
+
+
+@pytest.mark.parametrize("p,B", [(1, 5), (2, 34), (3, 6), (4, 66), (5, 40), (6, 18), (6, 70), (7, 5), (7, 34), (8, 10)])
+def test_box_cell_fast_path_on_octree_leaves(p, B):
+    """A general mesh whose cells are all axis-aligned boxes (the paper's adaptive meshes: octree leaves of a box, l.273)
+    takes the 10-sweep box-cell kernel of fe_gbox.cuh (p <= 7): apply (plain, shifted, NaN in the Dirichlet rows) against the
+    oracle <= 1e-11, agreement with the generic 12-sweep kernel (variant 9), the colour-ordered mode bit-reproducible, and a
+    filter <= 1e-9.  The larger B make the persistent CTAs walk several units (prefetched records and rows)."""
+    mesh = _graded_box_mesh(2 if p <= 3 else 1)
+    om, gm = _pair(mesh, p, _coulomb)
+    assert om.N_all > om.N
+    mask = om.mask()
+    X = workloads.random_block(1900 + p, om.N, B)
+    eps = workloads.shifts(2900 + p, B)
+    Yo, Yoe = om.apply(X), om.apply(X, eps)
+    Yg = gm.apply_H(_dev(X)).cpu().numpy()
+    assert _relerr(Yg, Yo, mask) <= TOL_APPLY and np.all(Yg[mask == 0] == 0)
+    Yge = gm.apply_H(_dev(X), eps=_dev(eps)).cpu().numpy()
+    assert _relerr(Yge, Yoe, mask) <= TOL_APPLY and np.all(Yge[mask == 0] == 0)
+    Xbad = X.copy()
+    Xbad[mask == 0] = np.nan
+    Yb = gm.apply_H(_dev(Xbad)).cpu().numpy()
+    assert np.all(np.isfinite(Yb)) and _relerr(Yb, Yo, mask) <= TOL_APPLY
+    gm.set_variant(9)  # the generic kernel on the same handle
+    Y9 = gm.apply_H(_dev(X), eps=_dev(eps)).cpu().numpy()
+    assert _relerr(Y9, Yoe, mask) <= TOL_APPLY and _relerr(Yge, Y9, mask) <= 1e-12
+    gm.set_variant(4)  # colour-ordered scatter through the box-cell kernel
+    Y4a = gm.apply_H(_dev(X), eps=_dev(eps)).cpu().numpy()
+    Y4b = gm.apply_H(_dev(X), eps=_dev(eps)).cpu().numpy()
+    assert np.array_equal(Y4a, Y4b) and _relerr(Y4a, Yoe, mask) <= TOL_APPLY
+    gm.set_variant(0)
+    import oracle
+    lo_o, hi_o, be_o = oracle.lanczos_bounds(om, workloads.normal(3900 + p, om.N), 20)
+    b, a0 = hi_o + be_o, lo_o
+    a = a0 + 0.1 * (b - a0)
+    deg = 7
+    Fo = om.filter(X, deg, a, b, a0)
+    work = torch.full((2 * om.N * B,), 7.5, dtype=torch.float64, device="cuda")
+    Fg = gm.cheb_filter(_dev(X).clone(), deg, a, b, a0, work).cpu().numpy()
+    assert _relerr(Fg, Fo, mask) <= TOL_FILTER and np.all(Fg[mask == 0] == 0)
