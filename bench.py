@@ -366,14 +366,20 @@ def measure_peaks(fe, dev):
     return out
 
 
-def time_adaptive(fe, torch, dev, peaks, hbm_peak, steps, warmup, p=6, B=64, m=30):
+GBOX_TRAFFIC = None  # ncu DRAM read + write of one k_apply_gbox launch on the adaptive workload (profiles/r2b_gbox_*)
+
+
+def time_adaptive(fe, torch, dev, peaks, hbm_peak, steps, warmup, p=6, B=64, m=30, generic=False):
     """NEXT-3 workload (not a BASELINE.json config): config 3's atoms on an adaptively refined mesh with hanging nodes
     (workloads.adaptive_molecule: 12^3 root cells refined twice around the nuclei), cheb_filter of degree m through the
-    general-cell kernel (fe_general.cuh: explicit l2g, full 3 x 3 metric, 12 sweeps).  The roofline uses the same
-    algorithmic count 24 n^4 + 9 n^3 per cell-vector, which is exactly the 12-sweep form this kernel executes (with even-odd
-    products: fewer instructions, same count)."""
+    general-mesh path (explicit l2g, constraint expansion / collapse).  The leaves are axis-aligned boxes, so the default is
+    the 10-sweep box-cell kernel of fe_gbox.cuh; generic=True (fe_set_variant 9) times the 12-sweep kernel with a full 3 x 3
+    metric (fe_general.cuh) that deformed cells need, on the same mesh.  The roofline uses the algorithmic count
+    24 n^4 + 9 n^3 per cell-vector of SURVEY 8(d) for both."""
     mesh, V = workloads.adaptive_molecule()
     gm = fe.FEMesh.general(mesh, p, device=dev)
+    if generic:
+        gm.set_variant(9)
     gm.set_potential(V(gm.quad_coords()))
     N = gm.N
     gen = torch.Generator(device="cuda")
@@ -408,10 +414,12 @@ def time_adaptive(fe, torch, dev, peaks, hbm_peak, steps, warmup, p=6, B=64, m=3
            "value": gm.N_free * B * m / (ms * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": ms,
            "roofline": {"bound": "alu", "achieved": flops / dur / 1e12, "peak": peak, "unit": "TFLOP/s",
                         "frac": flops / dur / 1e12 / peak, "frac_of_nominal": flops / dur / 1e12 / FP64_NOMINAL_TFLOPS,
-                        "kernel": "k_apply_gen<p=%d> + k_gen_init / k_gen_expand / k_gen_collapse (one operator step: step / m)" % p,
-                        "launch_ms": dur * 1e3, "algorithmic_bytes": alg_bytes, "traffic": 1.101e9 + 0.469e9,
-                        "traffic_source": "committed ncu capture profiles/r2_general_k_apply_gen.md (k_apply_gen alone, not "
-                                          "measured in this run)",
+                        "kernel": "%s<p=%d> + k_gen_init / k_gen_expand / k_gen_collapse (one operator step: step / m)"
+                                  % ("k_apply_gen" if generic else "k_apply_gbox", p),
+                        "launch_ms": dur * 1e3, "algorithmic_bytes": alg_bytes,
+                        "traffic": (1.101e9 + 0.469e9) if generic else GBOX_TRAFFIC,
+                        "traffic_source": "committed ncu capture profiles/%s (the cell kernel alone, not measured in this run)"
+                                          % ("r2_general_k_apply_gen.md" if generic else "r2b_gbox_k_apply_gbox.md"),
                         "hbm_frac_of_measured": (alg_bytes / dur / 1e9 / hbm_peak) if hbm_peak else None},
            "clocks": clocks, "gpu_launches": int(gm.launches - l0)}
     gm.close()
@@ -566,6 +574,7 @@ def main():
             torch.cuda.empty_cache()
         if world == 1 and not args.no_adaptive:
             others["adaptive_p6"] = time_adaptive(fe, torch, local, peaks, hbm_peak, min(args.steps, 5), 3)
+            others["adaptive_p6_generic"] = time_adaptive(fe, torch, local, peaks, hbm_peak, min(args.steps, 5), 3, generic=True)
             torch.cuda.empty_cache()
     if rank != 0:
         if dist is not None:

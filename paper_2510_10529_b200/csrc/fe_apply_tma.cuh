@@ -109,10 +109,10 @@ struct TmaShape {
     static constexpr int REC_SLIM = 2 * SMALL + 8;  // SLIM kernels leave the kz s_g tile out and multiply by kz instead
 };
 
-// STAGED shapes (p = 6 at 32 vectors, p = 7): the last rows of every output plane leave from a staging tile of their own instead
+// STAGED shape (p = 6 at 32 vectors; p = 7 measured no gain): the last rows of every output plane leave from a staging tile of their own instead
 // of bufB, so the next unit can write bufB while the bulk engine still reads them (k_apply_tma, plane phase 2)
 template <int P, int BT, bool SLIM, bool DOTS>
-__host__ __device__ constexpr bool tma_staged() { return !SLIM && !DOTS && ((P == 6 && BT == 32) || P == 7); }
+__host__ __device__ constexpr bool tma_staged() { return !SLIM && !DOTS && P == 6 && BT == 32; }
 
 template <int P, int BT, bool SLIM = false, bool DOTS = false>
 constexpr size_t tma_smem_bytes()

@@ -85,17 +85,26 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_gbox(const __grid_
         mbar_expect_tx(bar + b, (unsigned)(REC * sizeof(double)));
         bulk_load(recs + b * REC, prm.rec + c * REC, (unsigned)(REC * sizeof(double)), bar + b);
     };
+    // Addresses in 32-bit pieces: ids and N fit 32 bits (int32 l2g), so the row of node g starts at base + g * (8 B) bytes with
+    // ONE wide multiply-add, base = X (unconstrained) or X_h - N * 8 B (hanging: g - N is its row of X_h).  (The plain 64-bit
+    // form g * B + j with a two-way pointer select cost ~25 integer instructions per node and direction: ncu, 56 % of the
+    // kernel's instructions were not FP64.)
+    const unsigned N32 = (unsigned)prm.N, B8 = (unsigned)prm.B * 8u;
+    const unsigned long long hoff = (unsigned long long)N32 * B8;
     // the rows of this thread's nodal plane, straight into the plane of bufA it reads itself (no CTA barrier in between)
     auto request_rows = [&](long long u, int b) {
         const int32_t* ids = reinterpret_cast<const int32_t*>(recs + b * REC + IDS) + pl * n2;
         const int j = (int)(u % nbt) * BT + lane;
         const bool act = j < prm.B;
-        double* dst = bufA + (size_t)pl * n2 * BT + lane;
+        const char* bX = reinterpret_cast<const char*>(prm.X + (act ? j : 0));
+        const char* bH = reinterpret_cast<const char*>(prm.Xh + (act ? j : 0)) - hoff;
+        const unsigned d0 = smem_u32(bufA + (size_t)pl * n2 * BT + lane);
+        const int sz = act ? 8 : 0;  // src-size 0 zero-fills the 8 destination bytes
 #pragma unroll
         for (int a = 0; a < n2; ++a) {
-            const long long g = ids[a];
-            const double* src = g < prm.N ? prm.X + g * B + j : prm.Xh + (g - prm.N) * B + j;
-            cp_async8(dst + a * BT, act ? src : prm.X, act);
+            const unsigned g = (unsigned)ids[a];
+            const char* src = (g < N32 ? bX : bH) + (unsigned long long)g * B8;
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(d0 + (unsigned)(a * BT * 8)), "l"(src), "r"(sz) : "memory");
         }
         cp_async_commit();
     };
@@ -253,15 +262,19 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_gbox(const __grid_
     }
     const double* sout_pl = rec + SOUT + pl * n * NP;
     const int32_t* ids = reinterpret_cast<const int32_t*>(rec + IDS) + pl * n2;
+    char* yX = reinterpret_cast<char*>(prm.Y + (act ? j : 0));
+    char* yH = reinterpret_cast<char*>(prm.Yh + (act ? j : 0)) - hoff;
 #pragma unroll
     for (int ay = 0; ay < n; ++ay) {
         mat1d_eo<n>(prm.eoNTa, v[ay], o);
 #pragma unroll
         for (int ax = 0; ax < n; ++ax) {
             const double sc = sout_pl[ay * NP + ax];
-            const long long g = ids[ay * n + ax];
-            double* dst = g < prm.N ? prm.Y + g * B + j : prm.Yh + (g - prm.N) * B + j;
-            if (act && __double2hiint(sc) != 0) atomicAdd(dst, sc * o[ax]);
+            const unsigned g = (unsigned)ids[ay * n + ax];
+            char* dst = (g < N32 ? yX : yH) + (unsigned long long)g * B8;
+            const int on = (act && __double2hiint(sc) != 0) ? 1 : 0;  // Dirichlet nodes (scale 0) and idle lanes add nothing
+            asm volatile("{ .reg .pred p; setp.ne.b32 p, %2, 0; @p red.global.add.f64 [%0], %1; }"
+                         ::"l"(dst), "d"(sc * o[ax]), "r"(on) : "memory");
         }
     }
     }  // units
