@@ -597,6 +597,14 @@ def main():
         line["peaks"] = peaks
         if args.orders and world == 1:
             line["orders"] = time_orders(fe, torch, local, peaks, hbm_peak, 3, 3)
+            # the adaptive hanging-node mesh at the orders of the paper's Table 1: box-cell kernel and generic kernel
+            line["orders_adaptive"] = {}
+            for p_ in (4, 5, 6, 7):
+                for generic in (False, True):
+                    r_ = time_adaptive(fe, torch, local, peaks, hbm_peak, 3, 3, p=p_, m=12, generic=generic)
+                    line["orders_adaptive"]["p%d%s" % (p_, "_generic" if generic else "")] = {
+                        "value": r_["value"], "unit": UNIT, "ms_per_apply": r_["ms_per_step"] / 12, "frac": r_["roofline"]["frac"]}
+                    torch.cuda.empty_cache()
         if args.consumers and world == 1:
             line["consumers"] = time_consumers(fe, torch, workloads.config(2), local)
         if world == 1 and not args.no_cpu_baseline:

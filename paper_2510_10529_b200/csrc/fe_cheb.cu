@@ -396,7 +396,8 @@ int fe_set_variant(fe_mesh* m, int variant)
 
 // one fused operator launch: Y = mu (alpha (S sum_e P_e^T y_e - (c + eps) X) + beta Z)
 static int general_step(fe_mesh* m, const double* X, const double* Z, double* Y, int B, const double* eps,
-                        double alpha, double beta, double c, cudaStream_t st);
+                        double alpha, double beta, double c, cudaStream_t st, double* W = nullptr, double beta_next = 0.0,
+                        bool y_ready = false);
 static int general_expand(fe_mesh* m, const double* X, int B, cudaStream_t st);
 
 static int operator_step(fe_mesh* m, const double* X, const double* Z, double* Y, int B, const double* eps,
@@ -554,6 +555,7 @@ int fe_mesh_create_general(int cx, int cy, int cz, const int32_t* cells, int64_t
     if (gbox_supported(p)) {
         const int n = m->n, NP = n + (n & 1), SMALL = n * n * NP, brec = gbox_rec_doubles(n);
         std::vector<double> br((size_t)ncells * brec, 0.0);
+        std::vector<char> owned((size_t)g.N, 0);  // owner cell of an unconstrained node = the first cell that lists it
         bool all_boxes = true;
         for (int64_t e = 0; e < ncells && all_boxes; ++e) {
             const double* c = verts + e * 24;
@@ -581,7 +583,12 @@ int fe_mesh_create_general(int cx, int cy, int cz, const int32_t* cells, int64_t
             r[2 * SMALL + 2] = kz;
             r[2 * SMALL + 3] = 0.5 * h[2] * h[2];
             r[2 * SMALL + 4] = dirichlet ? 1.0 : 0.0;
-            memcpy(r + 3 * SMALL + 8, &g.l2g[(size_t)e * m->nc], (size_t)m->nc * sizeof(int32_t));
+            int32_t* ids = reinterpret_cast<int32_t*>(r + 3 * SMALL + 8);
+            for (int a = 0; a < m->nc; ++a) {
+                const int32_t id = g.l2g[(size_t)e * m->nc + a];
+                ids[a] = id;
+                if (id < g.N && !owned[id]) { owned[id] = 1; ids[a] = (int32_t)((uint32_t)id | 0x80000000u); }  // bit 31: owner
+            }
         }
         if (all_boxes) {
             if ((rc = upload_vec(&m->d_gbrec, br))) { fe_mesh_destroy(m); return rc; }
@@ -687,8 +694,12 @@ static int ensure_general_colours(fe_mesh* m)
 
 // one fused operator step on a general mesh: diagonal terms (k_gen_init), expansion of the hanging values, the cell kernel,
 // the transposed expansion
+// Box-cell kernel only (general_fused): y_ready = Y already holds beta Y_{k-1} (written by the previous step's
+// pre-initialisation; Z is not read), W != NULL = this step stores beta_next X into W for the step after it
+static bool general_fused(const fe_mesh* m) { return m->kind && m->gbox && !m->gbox_off && m->variant != 9 && m->variant != 4; }
+
 static int general_step(fe_mesh* m, const double* X, const double* Z, double* Y, int B, const double* eps,
-                        double alpha, double beta, double c, cudaStream_t st)
+                        double alpha, double beta, double c, cudaStream_t st, double* W, double beta_next, bool y_ready)
 {
     const GeneralHost& g = *m->gh;
     const long long nh = g.N_all - g.N;
@@ -696,10 +707,18 @@ static int general_step(fe_mesh* m, const double* X, const double* Z, double* Y,
     if (rc) return rc;
     const int grid = m->sms * 8;
     const dim3 rows(32, kGenRows);
-    if (!Z && !eps && c == 0.0)  // plain apply: nothing diagonal to write, Y is just cleared
+    // box-cell kernel without a Z block: the shift term kappa_j X comes from the owner cells inside the kernel
+    const bool fuse = general_fused(m) && !Z;
+    if ((W || y_ready) && !fuse) return fail(FE_ERR_STATE, "general_step: pre-initialisation needs the box-cell kernel");
+    bool init_kernel = false;
+    if (y_ready) {
+        // Y was pre-initialised by the previous step
+    } else if (fuse || (!Z && !eps && c == 0.0))  // nothing diagonal to write here: Y is just cleared
         CUDA_TRY(cudaMemsetAsync(Y, 0, (size_t)g.N * B * sizeof(double), st));
-    else
+    else {
         k_gen_init<<<grid, rows, 0, st>>>(Y, X, Z, m->d_sm, eps, alpha, beta, c, g.N, B);
+        init_kernel = true;
+    }
     if (nh > 0) CUDA_TRY(cudaMemsetAsync(m->d_Yh, 0, (size_t)nh * B * sizeof(double), st));
     // all cells axis-aligned boxes: the 10-sweep kernel (variant 9 keeps the generic 12-sweep kernel as a cross-check)
     const bool box = m->gbox && !m->gbox_off && m->variant != 9;
@@ -716,6 +735,10 @@ static int general_step(fe_mesh* m, const double* X, const double* Z, double* Y,
         for (double& x : bp.eoNTa.S) x *= alpha;
         for (double& x : bp.eoNTa.A) x *= alpha;
         for (double& x : bp.eoNTa.Mid) x *= alpha;
+        if (fuse) {
+            bp.W = W; bp.beta_next = beta_next; bp.eps = eps; bp.alpha = alpha; bp.c = c;
+            bp.owner = (eps != nullptr || c != 0.0) ? 1 : 0;
+        }
     }
     // the box kernel delivers alpha yhat to the hanging targets too (alpha sits in its last table): the collapse runs with 1
     const double alpha_h = box ? 1.0 : alpha;
@@ -731,7 +754,7 @@ static int general_step(fe_mesh* m, const double* X, const double* Z, double* Y,
             k_gen_rows_times_block<<<grid, rows, 0, st>>>(Y, m->d_Yh, m->gtr.bptr, m->gtr.bcol, m->gtr.bw, m->gtr.brow, m->gtr.out,
                                                           m->gtr.nb, B, alpha_h, 1);
         CUDA_TRY(cudaGetLastError());
-        m->launches += (int64_t)m->colour_off.size() + (nh > 0 ? 2 : 1);
+        m->launches += (int64_t)m->colour_off.size() - 1 + (nh > 0 ? 1 : 0) + (init_kernel ? 1 : 0);
         return FE_OK;
     }
     cudaError_t e = box ? launch_apply_gbox(bp, m->p, m->ncells, m->sms, st) : launch_apply_gen(prm, m->p, m->ncells, m->sms, st);
@@ -740,7 +763,7 @@ static int general_step(fe_mesh* m, const double* X, const double* Z, double* Y,
         k_gen_collapse<<<grid, rows, 0, st>>>(Y, m->d_Yh, m->gexp.bptr, m->gexp.bcol, m->gexp.bw, m->gexp.brow, m->gexp.out, m->gexp.nb, B,
                                               alpha_h);
     CUDA_TRY(cudaGetLastError());
-    m->launches += nh > 0 ? 3 : 2;
+    m->launches += (nh > 0 ? 2 : 1) + (init_kernel ? 1 : 0);  // cell kernel, collapse, k_gen_init (memsets are not counted)
     return FE_OK;
 }
 
@@ -970,6 +993,22 @@ int cheb_filter(fe_mesh* m, double* X, int B, int deg, double a, double b, doubl
             rc = tma_step(m, bm[k % 3], bm[(k + 1) % 3], pre ? &bm[(k + 2) % 3] : nullptr, B, nullptr, alpha, c, true,
                           -s_cur * s_next, k == 0, st);
             if (rc) return rc;
+            s_cur = s_next;
+        }
+        if (deg % 3 != 0) CUDA_TRY(cudaMemcpyAsync(X, buf[deg % 3], len * sizeof(double), cudaMemcpyDeviceToDevice, st));
+        return FE_OK;
+    }
+    if (general_fused(m)) {
+        // general mesh of box cells: the pre-initialised recurrence of the TMA path through the owner cells of k_apply_gbox
+        // (every unconstrained node has an owner, Dirichlet rows are stored as 0: no face clears)
+        double s_cur = sigma1;
+        for (int k = 0; k < deg; ++k) {  // step 0 clears its own target
+            const double s_next = 1.0 / (2.0 / sigma1 - s_cur);
+            const double alpha = (k == 0) ? s_cur / e : 2.0 * s_cur / e;
+            const bool pre = k + 1 < deg;
+            int rcg = general_step(m, buf[k % 3], nullptr, buf[(k + 1) % 3], B, nullptr, alpha, 0.0, c, st,
+                                   pre ? buf[(k + 2) % 3] : nullptr, -s_cur * s_next, k > 0);
+            if (rcg) return rcg;
             s_cur = s_next;
         }
         if (deg % 3 != 0) CUDA_TRY(cudaMemcpyAsync(X, buf[deg % 3], len * sizeof(double), cudaMemcpyDeviceToDevice, st));

@@ -11,7 +11,9 @@
 //             the copies of the next unit are issued when the line phase has released the field, and run under plane phase 2;
 //   scatter : red.global.add.f64 per value into Y (unconstrained) or Y_h (hanging; k_gen_collapse distributes it);
 //   record  : one bulk copy per unit brings V_q hz^2/2, the gather and scatter scales, the cell's ratios and its n^3 ids.
-// The diagonal terms of the step (shift, recurrence) are written by k_gen_init as for every general mesh.
+// The diagonal terms of the step (shift, recurrence) come from the owner cell of each node as in the box-mesh kernel (store of
+// beta' X into the next target, kappa_j X added to Y), so a filter step reads no Y_{k-1} and needs no k_gen_init pass; callers
+// that pass a Z block, and the colour-ordered mode, keep k_gen_init.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -45,6 +47,13 @@ struct GBoxParams {
     int B;
     EOTab eoN, eoNT, eoG;  // even-odd halves of N' = diag(sqrt w) N, N'^T, G' = diag(w^-1/2) G diag(w^-1/2)
     EOTab eoNTa;           // alpha N'^T: unconstrained AND hanging targets receive alpha yhat (the collapse then runs with 1)
+    // diagonal terms from the OWNER cell of every unconstrained node (the first cell that lists it; bit 31 of its id in that
+    // cell's record), as in the box-mesh kernel: Y += kappa_j X with kappa_j = -alpha (c + eps_j) when `owner`, and the
+    // pre-initialisation W = beta_next X of the NEXT filter step's target when W != NULL (no k_gen_init pass, no read of Y_{k-1})
+    double* W;
+    const double* eps;
+    double alpha, c, beta_next;
+    int owner;
 };
 
 // VZ tile of every record from the caller's V[e][q], q = qx + n (qy + n qz)
@@ -102,7 +111,7 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_gbox(const __grid_
         const int sz = act ? 8 : 0;  // src-size 0 zero-fills the 8 destination bytes
 #pragma unroll
         for (int a = 0; a < n2; ++a) {
-            const unsigned g = (unsigned)ids[a];
+            const unsigned g = (unsigned)ids[a] & 0x7fffffffu;
             const char* src = (g < N32 ? bX : bH) + (unsigned long long)g * B8;
             asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(d0 + (unsigned)(a * BT * 8)), "l"(src), "r"(sz) : "memory");
         }
@@ -148,6 +157,27 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_gbox(const __grid_
 #pragma unroll
             for (int ax = 0; ax < n; ++ax)
                 v[ay][ax] = (__double2hiint(sin_pl[ay * NP + ax]) != 0) ? v[ay][ax] : 0.0;
+    }
+    if (prm.W != nullptr || prm.owner) {  // uniform over the grid
+        const int32_t* idp = reinterpret_cast<const int32_t*>(rec + IDS) + pl * n2;
+        const int jj = act ? j : 0;
+        char* wX = reinterpret_cast<char*>(prm.W + jj);
+        char* aX = reinterpret_cast<char*>(prm.Y + jj);
+        const double kappa = prm.owner ? -prm.alpha * (prm.c + ((prm.eps && act) ? prm.eps[j] : 0.0)) : 0.0;
+#pragma unroll
+        for (int ay = 0; ay < n; ++ay)
+#pragma unroll
+            for (int ax = 0; ax < n; ++ax) {
+                const int enc = idp[ay * n + ax];
+                const unsigned long long off = (unsigned long long)((unsigned)enc & 0x7fffffffu) * B8;
+                const int own = (act && enc < 0) ? 1 : 0;
+                if (prm.W != nullptr)
+                    asm volatile("{ .reg .pred p; setp.ne.b32 p, %2, 0; @p st.global.f64 [%0], %1; }"
+                                 ::"l"(wX + off), "d"(prm.beta_next * v[ay][ax]), "r"(own) : "memory");
+                if (prm.owner)
+                    asm volatile("{ .reg .pred p; setp.ne.b32 p, %2, 0; @p red.global.add.f64 [%0], %1; }"
+                                 ::"l"(aX + off), "d"(kappa * v[ay][ax]), "r"(own) : "memory");
+            }
     }
 #pragma unroll
     for (int ay = 0; ay < n; ++ay)
@@ -270,7 +300,7 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_gbox(const __grid_
 #pragma unroll
         for (int ax = 0; ax < n; ++ax) {
             const double sc = sout_pl[ay * NP + ax];
-            const unsigned g = (unsigned)ids[ay * n + ax];
+            const unsigned g = (unsigned)ids[ay * n + ax] & 0x7fffffffu;
             char* dst = (g < N32 ? yX : yH) + (unsigned long long)g * B8;
             const int on = (act && __double2hiint(sc) != 0) ? 1 : 0;  // Dirichlet nodes (scale 0) and idle lanes add nothing
             asm volatile("{ .reg .pred p; setp.ne.b32 p, %2, 0; @p red.global.add.f64 [%0], %1; }"
