@@ -159,24 +159,28 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_gbox(const __grid_
                 v[ay][ax] = (__double2hiint(sin_pl[ay * NP + ax]) != 0) ? v[ay][ax] : 0.0;
     }
     if (prm.W != nullptr || prm.owner) {  // uniform over the grid
+        // The store is predicated (owner cells only); the add is UNCONDITIONAL with the value selected to 0 elsewhere: ptxas
+        // turns a predicated red.global into a branch with uniform-register spills around it (11 instructions per node).
         const int32_t* idp = reinterpret_cast<const int32_t*>(rec + IDS) + pl * n2;
         const int jj = act ? j : 0;
         char* wX = reinterpret_cast<char*>(prm.W + jj);
         char* aX = reinterpret_cast<char*>(prm.Y + jj);
-        const double kappa = prm.owner ? -prm.alpha * (prm.c + ((prm.eps && act) ? prm.eps[j] : 0.0)) : 0.0;
+        char* aH = reinterpret_cast<char*>(prm.Yh + jj) - hoff;
+        const double kappa = (prm.owner && act) ? -prm.alpha * (prm.c + (prm.eps ? prm.eps[j] : 0.0)) : 0.0;
+        const double bnext = prm.beta_next;
+        const bool has_w = prm.W != nullptr;
 #pragma unroll
         for (int ay = 0; ay < n; ++ay)
 #pragma unroll
             for (int ax = 0; ax < n; ++ax) {
                 const int enc = idp[ay * n + ax];
-                const unsigned long long off = (unsigned long long)((unsigned)enc & 0x7fffffffu) * B8;
-                const int own = (act && enc < 0) ? 1 : 0;
-                if (prm.W != nullptr)
-                    asm volatile("{ .reg .pred p; setp.ne.b32 p, %2, 0; @p st.global.f64 [%0], %1; }"
-                                 ::"l"(wX + off), "d"(prm.beta_next * v[ay][ax]), "r"(own) : "memory");
-                if (prm.owner)
-                    asm volatile("{ .reg .pred p; setp.ne.b32 p, %2, 0; @p red.global.add.f64 [%0], %1; }"
-                                 ::"l"(aX + off), "d"(kappa * v[ay][ax]), "r"(own) : "memory");
+                const unsigned g = (unsigned)enc & 0x7fffffffu;
+                const bool own = act && enc < 0;
+                const double x = v[ay][ax];
+                if (own && has_w) *reinterpret_cast<double*>(wX + (unsigned long long)g * B8) = bnext * x;
+                // nodes this cell does not own receive +0.0 at their own address (hanging nodes, never owned, in Y_h): spread
+                // over the block like the real adds, no hot spot
+                atomicAdd(reinterpret_cast<double*>((g < N32 ? aX : aH) + (unsigned long long)g * B8), own ? kappa * x : 0.0);
             }
     }
 #pragma unroll
@@ -302,9 +306,9 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_gbox(const __grid_
             const double sc = sout_pl[ay * NP + ax];
             const unsigned g = (unsigned)ids[ay * n + ax] & 0x7fffffffu;
             char* dst = (g < N32 ? yX : yH) + (unsigned long long)g * B8;
-            const int on = (act && __double2hiint(sc) != 0) ? 1 : 0;  // Dirichlet nodes (scale 0) and idle lanes add nothing
-            asm volatile("{ .reg .pred p; setp.ne.b32 p, %2, 0; @p red.global.add.f64 [%0], %1; }"
-                         ::"l"(dst), "d"(sc * o[ax]), "r"(on) : "memory");
+            // unconditional add (a predicated red.global becomes a branch): Dirichlet nodes (scale 0) and idle lanes (column 0
+            // of their node) add +0.0, which changes nothing
+            atomicAdd(reinterpret_cast<double*>(dst), (act && __double2hiint(sc) != 0) ? sc * o[ax] : 0.0);
         }
     }
     }  // units

@@ -329,3 +329,23 @@ def test_box_cell_fast_path_on_octree_leaves(p, B):
     work = torch.full((2 * om.N * B,), 7.5, dtype=torch.float64, device="cuda")
     Fg = gm.cheb_filter(_dev(X).clone(), deg, a, b, a0, work).cpu().numpy()
     assert _relerr(Fg, Fo, mask) <= TOL_FILTER and np.all(Fg[mask == 0] == 0)
+
+
+@pytest.mark.parametrize("p,B", [(1, 224), (2, 160), (3, 130), (4, 100), (5, 70)])
+def test_box_cell_kernel_walks_several_units_per_cta(p, B):
+    """More (cell, vector tile) units than resident CTAs at the orders with several CTAs per SM (8, 6, 4, 3, 1 at p = 1..5):
+    every CTA of the box-cell kernel walks several units (double-buffered records, rows of the next unit copied under plane
+    phase 2, owner terms).  Shifted apply <= 1e-11 and a degree-8 filter <= 1e-9 against the oracle on the twice-refined mesh."""
+    import oracle
+    mesh = _graded_box_mesh(2 if p <= 4 else 1)
+    om, gm = _pair(mesh, p, _coulomb)
+    mask = om.mask()
+    X = workloads.random_block(2100 + p, om.N, B)
+    eps = workloads.shifts(3100 + p, B)
+    Yg = gm.apply_H(_dev(X), eps=_dev(eps)).cpu().numpy()
+    assert _relerr(Yg, om.apply(X, eps), mask) <= TOL_APPLY and np.all(Yg[mask == 0] == 0)
+    lo_o, hi_o, be_o = oracle.lanczos_bounds(om, workloads.normal(4100 + p, om.N), 20)
+    b, a0 = hi_o + be_o, lo_o
+    a = a0 + 0.1 * (b - a0)
+    Fg = gm.cheb_filter(_dev(X).clone(), 8, a, b, a0).cpu().numpy()
+    assert _relerr(Fg, om.filter(X, 8, a, b, a0), mask) <= TOL_FILTER and np.all(Fg[mask == 0] == 0)
