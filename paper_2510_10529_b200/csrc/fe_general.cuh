@@ -474,14 +474,16 @@ __global__ void __launch_bounds__(GenShape<P>::LS * BT, MINB) k_apply_gen(const 
 #pragma unroll
         for (int k = 0; k < n; ++k) t[k] = f[k * SX];
         mat1d_eo<n>(prm.eoNT, t, o);
-        if (act) {
+        {   // unconditional adds: a predicated red.global becomes a branch with uniform-register spills around it (fe_gbox.cuh);
+            // Dirichlet nodes (scale 0) and idle lanes (column 0 of their node) add +0.0, which changes nothing
+            const int jj = act ? j : 0;
 #pragma unroll
             for (int k = 0; k < n; ++k) {
                 const long long g = sId[l * n + k];
                 const double sg = sSc[l * n + k];
                 const bool master = g < prm.N;
-                double* dst = master ? prm.Y + g * B + j : prm.Yh + (g - prm.N) * B + j;
-                if (sg != 0.0) atomicAdd(dst, master ? prm.alpha * sg * o[k] : o[k]);
+                double* dst = master ? prm.Y + g * B + jj : prm.Yh + (g - prm.N) * B + jj;
+                atomicAdd(dst, (act && sg != 0.0) ? (master ? prm.alpha * sg * o[k] : o[k]) : 0.0);
             }
         }
     }
