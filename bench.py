@@ -366,7 +366,7 @@ def measure_peaks(fe, dev):
     return out
 
 
-GBOX_TRAFFIC = None  # ncu DRAM read + write of one k_apply_gbox launch on the adaptive workload (profiles/r2b_gbox_*)
+GBOX_TRAFFIC = 1.072e9 + 0.900e9  # ncu DRAM read + write of one k_apply_gbox launch on the adaptive workload (profiles/r2b_gbox_*)
 
 
 def time_adaptive(fe, torch, dev, peaks, hbm_peak, steps, warmup, p=6, B=64, m=30, generic=False):

@@ -341,7 +341,7 @@ inline cudaError_t launch_apply_gbox(const GBoxParams& prm, int p, long long nce
         case 4: return launch_gbox_t<4, 32, 3>(prm, ncells, sms, st);
         case 5: return launch_gbox_t<5, 32, 1>(prm, ncells, sms, st);
         case 6: return launch_gbox_t<6, 32, 1>(prm, ncells, sms, st);
-        case 7: return launch_gbox_t<7, 16, 1>(prm, ncells, sms, st);
+        case 7: return launch_gbox_t<7, 24, 1>(prm, ncells, sms, st);
     }
     return cudaErrorInvalidValue;
 }
