@@ -87,7 +87,7 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_gbox(const __grid_
     unsigned long long* bar = (unsigned long long*)(recs + 2 * REC);  // bar[b]: record b landed
     const int lane = threadIdx.x, pl = threadIdx.y, tid = pl * BT + lane;
     const int nbt = (prm.B + BT - 1) / BT;
-    const long long nunits = prm.ncells * nbt, B = prm.B;
+    const long long nunits = prm.ncells * nbt;
 
     auto request_rec = [&](long long u, int b) {  // one thread
         const long long cu = u / nbt, c = prm.cell_list ? (long long)prm.cell_list[cu] : cu;

@@ -141,7 +141,7 @@ k_gen_collapse(double* __restrict__ Y, const double* __restrict__ Yh, const long
                 double v = w0.x * y[0];
                 v = fma(w0.y, y[1], v); v = fma(w0.z, y[2], v); v = fma(w0.w, y[3], v);
                 v = fma(w1.x, y[4], v); v = fma(w1.y, y[5], v); v = fma(w1.z, y[6], v); v = fma(w1.w, y[7], v);
-                if (v != 0.0) atomicAdd(Y + (long long)bcol[k] * B + j, v);
+                atomicAdd(Y + (long long)bcol[k] * B + j, v);  // unconditional: a predicated red.global becomes a branch (fe_gbox.cuh)
             }
         }
     }
@@ -268,7 +268,6 @@ __global__ void __launch_bounds__(GenShape<P>::LS * BT, MINB) k_apply_gen(const 
     const int lane = threadIdx.x, slot = threadIdx.y, tid = slot * BT + lane;
     const int ntile = (prm.B + BT - 1) / BT;
     const long long nunits = prm.ncells * ntile;
-    const long long B = prm.B;
     double t[n], o[n];
     // the (at most) two lines of this slot in every sweep, as field offsets: x-lines (i1, i2), y-lines (i0, i2), z-lines (i0, i1)
     const bool two = slot + LS < n2;
@@ -297,13 +296,18 @@ __global__ void __launch_bounds__(GenShape<P>::LS * BT, MINB) k_apply_gen(const 
         cp_async_commit();
     };
     // ... and its node rows, once the ids are in shared memory: independent 8-byte cp.async straight into the field
+    // node addresses in 32-bit pieces (ids and N fit 32 bits): row of node g = base + g * (8 B) bytes with one wide
+    // multiply-add, base = X (unconstrained) or X_h - N * 8 B (hanging) -- fe_gbox.cuh
+    const unsigned N32 = (unsigned)prm.N, B8 = (unsigned)prm.B * 8u;
+    const unsigned long long hoff = (unsigned long long)N32 * B8;
     auto request_rows = [&](long long u, int buf, double* F) {
         const int jn = (int)(u % ntile) * BT + lane;
         const bool an = jn < prm.B;
+        const char* bX = reinterpret_cast<const char*>(prm.X + (an ? jn : 0));
+        const char* bH = reinterpret_cast<const char*>(prm.Xh + (an ? jn : 0)) - hoff;
         for (int a = slot; a < n3; a += LS) {
-            const long long g = sIdB[buf * n3 + a];
-            const double* src = g < prm.N ? prm.X + g * B + jn : prm.Xh + (g - prm.N) * B + jn;
-            cp_async8(F + (size_t)a * BT + lane, an ? src : prm.X, an);
+            const unsigned g = (unsigned)sIdB[buf * n3 + a];
+            cp_async8(F + (size_t)a * BT + lane, (g < N32 ? bX : bH) + (unsigned long long)g * B8, an);
         }
         cp_async_commit();
     };
@@ -477,12 +481,14 @@ __global__ void __launch_bounds__(GenShape<P>::LS * BT, MINB) k_apply_gen(const 
         {   // unconditional adds: a predicated red.global becomes a branch with uniform-register spills around it (fe_gbox.cuh);
             // Dirichlet nodes (scale 0) and idle lanes (column 0 of their node) add +0.0, which changes nothing
             const int jj = act ? j : 0;
+            char* yX = reinterpret_cast<char*>(prm.Y + jj);
+            char* yH = reinterpret_cast<char*>(prm.Yh + jj) - hoff;
 #pragma unroll
             for (int k = 0; k < n; ++k) {
-                const long long g = sId[l * n + k];
+                const unsigned g = (unsigned)sId[l * n + k];
                 const double sg = sSc[l * n + k];
-                const bool master = g < prm.N;
-                double* dst = master ? prm.Y + g * B + jj : prm.Yh + (g - prm.N) * B + jj;
+                const bool master = g < N32;
+                double* dst = reinterpret_cast<double*>((master ? yX : yH) + (unsigned long long)g * B8);
                 atomicAdd(dst, (act && sg != 0.0) ? (master ? prm.alpha * sg * o[k] : o[k]) : 0.0);
             }
         }

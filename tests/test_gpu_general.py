@@ -349,3 +349,30 @@ def test_box_cell_kernel_walks_several_units_per_cta(p, B):
     a = a0 + 0.1 * (b - a0)
     Fg = gm.cheb_filter(_dev(X).clone(), 8, a, b, a0).cpu().numpy()
     assert _relerr(Fg, om.filter(X, 8, a, b, a0), mask) <= TOL_FILTER and np.all(Fg[mask == 0] == 0)
+
+
+@pytest.mark.parametrize("p,B", [(3, 6), (6, 10)])
+def test_consumers_on_a_box_cell_mesh(p, B):
+    """The consumers of the operator on a mesh that takes the box-cell kernel: block MINRES with the preconditioner of R27
+    (shifted applies with the owner terms inside the kernel), the density, and fe_apply_potential -- which borrows the GENERIC
+    kernel for one call (records with zero metric) and must leave the box-cell operator as it was."""
+    import oracle
+    mesh = _graded_box_mesh(1)
+    om, gm = _pair(mesh, p, _coulomb)
+    mask = om.mask()
+    free = mask.astype(bool)
+    X = workloads.random_block(2200 + p, om.N, B)
+    eps = workloads.shifts(3200 + p, B)
+    Xo, relo, ito = oracle.minres_shifted(om, X, eps, maxit=25, tol=0.0, Minv=om.laplacian_precond())
+    Xg, relg, itg = gm.minres_shifted(_dev(X), _dev(eps), maxit=25, tol=0.0, precondition=True)
+    assert itg == 25 and ito == 25
+    assert _relerr(Xg.cpu().numpy(), Xo, mask) <= 1e-9 and np.max(np.abs(relg - relo)) <= 1e-9
+    f = 2.0 * workloads.uniform01(2201 + p, 0, B)
+    rho_o = om.density(X, f).reshape(-1)
+    rho_g = gm.density(_dev(X), _dev(f)).cpu().numpy()
+    assert np.linalg.norm(rho_g - rho_o) <= 1e-12 * np.linalg.norm(rho_o)
+    Uq = np.cos(om.quad_coords()).prod(axis=1) - 0.3
+    Yg = gm.apply_potential(_dev(Uq), _dev(X)).cpu().numpy()
+    assert _relerr(Yg, om.potential_apply(Uq, X * mask[:, None]), mask) <= TOL_APPLY and np.all(Yg[~free] == 0)
+    Yg = gm.apply_H(_dev(X), eps=_dev(eps)).cpu().numpy()  # the box-cell operator after the borrowed call
+    assert _relerr(Yg, om.apply(X, eps), mask) <= TOL_APPLY
