@@ -60,7 +60,10 @@ int fe_get_dirichlet_mask(const fe_mesh* m, uint8_t* mask); /* N, 1 = free, 0 = 
  * octree refinement of a cx x cy x cz root grid.  cells: HOST, ncells rows (level, ix, iy, iz) -- leaf (ix, iy, iz) of the
  * level-`level` lattice of 2^level (cx, cy, cz) cells; levels of leaves whose closures touch may differ by at most one.
  * verts: HOST, ncells*8*3 corner coordinates, corner v = vx + 2*(vy + 2*vz); a cell is the trilinear image of [-1,1]^3, so
- * the metric is a full symmetric 3x3 matrix per quadrature point.  Corners shared by cells must coincide and a corner hanging
+ * the metric is a full symmetric 3x3 matrix per quadrature point -- unless EVERY cell is an axis-aligned box (the leaves of an
+ * octree refinement of an undeformed box, the paper's meshes): the library detects that from the corners and, for p <= 7, runs the
+ * 10-sweep box-cell kernel instead of the generic 12-sweep one (same results to rounding; fe_set_variant(m, 9) forces the generic
+ * kernel).  Corners shared by cells must coincide and a corner hanging
  * on a coarser neighbour must lie on that neighbour's edge / face (not checked).  Numbering (reading R23): cells in the
  * given order, local nodes a = ax + n*(ay + n*az); unconstrained nodes get ids 0..N-1 in order of first appearance, hanging
  * nodes (nodes of a cell lying on a coarser leaf) ids N..N_all-1 likewise.  Blocks X, Y have N = fe_num_nodes rows: hanging
