@@ -452,6 +452,11 @@ static int pack_bundles(const std::vector<std::vector<std::pair<int32_t, double>
         while (e < nr && e - i < kGenBundle && same_cols(order[i], order[e])) ++e;
         const auto& first = rws[order[i]];
         for (size_t k = 0; k < first.size(); ++k) {
+            // an entry whose weights are 0 for every row of the bundle (a Dirichlet node: the weights carry s = 0) is dropped, so
+            // the kernels never read such a row of the block -- whatever it holds (R5) -- and need no per-weight test
+            bool any = false;
+            for (int64_t q = i; q < e; ++q) any = any || rws[order[q]][k].second != 0.0;
+            if (!any) continue;
             bcol.push_back(first[k].first);
             for (int u = 0; u < kGenBundle; ++u) bw.push_back(i + u < e ? rws[order[i + u]][k].second : 0.0);
         }
@@ -628,7 +633,7 @@ static int general_expand(fe_mesh* m, const double* X, int B, cudaStream_t st)
         m->hcap = B;
     }
     k_gen_rows_times_block<<<m->sms * 8, dim3(32, kGenRows), 0, st>>>(m->d_Xh, X, m->gexp.bptr, m->gexp.bcol, m->gexp.bw, m->gexp.brow,
-                                                                      m->gexp.out, m->gexp.nb, B, 1.0, 0);
+                                                                      m->gexp.out, m->gexp.nb, B, 1.0, 0, m->d_Yh);  // also clears Y_h
     CUDA_TRY(cudaGetLastError());
     m->launches += 1;
     return FE_OK;
@@ -719,7 +724,7 @@ static int general_step(fe_mesh* m, const double* X, const double* Z, double* Y,
         k_gen_init<<<grid, rows, 0, st>>>(Y, X, Z, m->d_sm, eps, alpha, beta, c, g.N, B);
         init_kernel = true;
     }
-    if (nh > 0) CUDA_TRY(cudaMemsetAsync(m->d_Yh, 0, (size_t)nh * B * sizeof(double), st));
+    // Y_h (the scatter target of the hanging nodes) was cleared by the expansion kernel: every hanging row is in one bundle
     // all cells axis-aligned boxes: the 10-sweep kernel (variant 9 keeps the generic 12-sweep kernel as a cross-check)
     const bool box = m->gbox && !m->gbox_off && m->variant != 9;
     GenParams prm;
@@ -752,7 +757,7 @@ static int general_step(fe_mesh* m, const double* X, const double* Z, double* Y,
         }
         if (nh > 0)
             k_gen_rows_times_block<<<grid, rows, 0, st>>>(Y, m->d_Yh, m->gtr.bptr, m->gtr.bcol, m->gtr.bw, m->gtr.brow, m->gtr.out,
-                                                          m->gtr.nb, B, alpha_h, 1);
+                                                          m->gtr.nb, B, alpha_h, 1, nullptr);
         CUDA_TRY(cudaGetLastError());
         m->launches += (int64_t)m->colour_off.size() - 1 + (nh > 0 ? 1 : 0) + (init_kernel ? 1 : 0);
         return FE_OK;

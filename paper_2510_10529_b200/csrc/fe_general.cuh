@@ -72,7 +72,8 @@ __global__ void k_gen_init(double* __restrict__ Y, const double* __restrict__ X,
 }
 
 // Sparse rows times a block:  dst[out_r, j] (+)= alpha sum_k w_rk src[col_k, j].
-//   expansion  X_h = C_h (s . X):        src = X,   dst = X_h, w = cval * s[col] (0 on Dirichlet rows, whose data is ignored)
+//   expansion  X_h = C_h (s . X):        src = X,   dst = X_h, w = cval * s[col] (entries of Dirichlet nodes, s = 0, are dropped
+//                                        when the bundles are packed: their rows of X are never read)
 //   collapse   Y += alpha s . C_h^T Y_h:  k_gen_collapse below, the same bundles read the other way
 // The hanging nodes of one coarse face all depend on the same n^2 nodes (and the nodes of a coarse face all feed the same
 // hanging nodes), so the host sorts the rows by their column lists and packs rows with IDENTICAL lists into bundles of up to
@@ -85,7 +86,8 @@ constexpr int kGenBundle = 8;
 __global__ void __launch_bounds__(32 * kGenRows, 4)
 k_gen_rows_times_block(double* __restrict__ dst, const double* __restrict__ src, const long long* __restrict__ bptr,
                        const int32_t* __restrict__ bcol, const double* __restrict__ bw, const int32_t* __restrict__ brow,
-                       const int32_t* __restrict__ out, long long nb, int B, double alpha, int accumulate)
+                       const int32_t* __restrict__ out, long long nb, int B, double alpha, int accumulate,
+                       double* __restrict__ zero)  // zero != NULL: the same rows of this second block are cleared (Y_h of the step)
 {
     for (long long b = blockIdx.x * (long long)kGenRows + threadIdx.y; b < nb; b += (long long)gridDim.x * kGenRows) {
         const long long k0 = bptr[b], k1 = bptr[b + 1];
@@ -99,20 +101,16 @@ k_gen_rows_times_block(double* __restrict__ dst, const double* __restrict__ src,
                 const double x = src[(long long)bcol[k] * B + j];
                 const double4 w0 = *reinterpret_cast<const double4*>(bw + k * kGenBundle);
                 const double4 w1 = *reinterpret_cast<const double4*>(bw + k * kGenBundle + 4);
-                v[0] = w0.x != 0.0 ? fma(w0.x, x, v[0]) : v[0];
-                v[1] = w0.y != 0.0 ? fma(w0.y, x, v[1]) : v[1];
-                v[2] = w0.z != 0.0 ? fma(w0.z, x, v[2]) : v[2];
-                v[3] = w0.w != 0.0 ? fma(w0.w, x, v[3]) : v[3];
-                v[4] = w1.x != 0.0 ? fma(w1.x, x, v[4]) : v[4];
-                v[5] = w1.y != 0.0 ? fma(w1.y, x, v[5]) : v[5];
-                v[6] = w1.z != 0.0 ? fma(w1.z, x, v[6]) : v[6];
-                v[7] = w1.w != 0.0 ? fma(w1.w, x, v[7]) : v[7];
+                // no test of the weights: entries of Dirichlet nodes (all weights 0, data to be ignored) are not in the bundles
+                v[0] = fma(w0.x, x, v[0]); v[1] = fma(w0.y, x, v[1]); v[2] = fma(w0.z, x, v[2]); v[3] = fma(w0.w, x, v[3]);
+                v[4] = fma(w1.x, x, v[4]); v[5] = fma(w1.y, x, v[5]); v[6] = fma(w1.z, x, v[6]); v[7] = fma(w1.w, x, v[7]);
             }
 #pragma unroll
             for (int u = 0; u < kGenBundle; ++u)
                 if (u < m) {
-                    double* d = dst + (long long)out[r0 + u] * B + j;
-                    *d = accumulate ? fma(alpha, v[u], *d) : alpha * v[u];
+                    const long long i = (long long)out[r0 + u] * B + j;
+                    dst[i] = accumulate ? fma(alpha, v[u], dst[i]) : alpha * v[u];
+                    if (zero) zero[i] = 0.0;
                 }
         }
     }
