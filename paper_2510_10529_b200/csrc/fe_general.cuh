@@ -89,29 +89,51 @@ k_gen_rows_times_block(double* __restrict__ dst, const double* __restrict__ src,
                        const int32_t* __restrict__ out, long long nb, int B, double alpha, int accumulate,
                        double* __restrict__ zero)  // zero != NULL: the same rows of this second block are cleared (Y_h of the step)
 {
-    for (long long b = blockIdx.x * (long long)kGenRows + threadIdx.y; b < nb; b += (long long)gridDim.x * kGenRows) {
+    // A warp stages 32 entries of its bundle (column ids and the 8 weights each, coalesced) in shared memory and then walks
+    // them with the rows of src as INDEPENDENT loads, eight in flight: read straight from global memory the chain
+    // column id -> row address -> value made every entry two dependent round trips, and the kernel was bound by that latency.
+    __shared__ int32_t s_col[kGenRows][32];
+    __shared__ __align__(16) double s_w[kGenRows][32][kGenBundle];
+    const int ty = threadIdx.y, lane = threadIdx.x;
+    for (long long b = blockIdx.x * (long long)kGenRows + ty; b < nb; b += (long long)gridDim.x * kGenRows) {
         const long long k0 = bptr[b], k1 = bptr[b + 1];
         const int r0 = brow[b], m = brow[b + 1] - r0;
-        for (int j = threadIdx.x; j < B; j += 32) {
+        for (int j0 = 0; j0 < B; j0 += 32) {
+            const int j = j0 + lane;
+            const bool act = j < B;
+            const double* sj = src + (act ? j : 0);
             double v[kGenBundle];
 #pragma unroll
             for (int u = 0; u < kGenBundle; ++u) v[u] = 0.0;
-#pragma unroll 2
-            for (long long k = k0; k < k1; ++k) {
-                const double x = src[(long long)bcol[k] * B + j];
-                const double4 w0 = *reinterpret_cast<const double4*>(bw + k * kGenBundle);
-                const double4 w1 = *reinterpret_cast<const double4*>(bw + k * kGenBundle + 4);
-                // no test of the weights: entries of Dirichlet nodes (all weights 0, data to be ignored) are not in the bundles
-                v[0] = fma(w0.x, x, v[0]); v[1] = fma(w0.y, x, v[1]); v[2] = fma(w0.z, x, v[2]); v[3] = fma(w0.w, x, v[3]);
-                v[4] = fma(w1.x, x, v[4]); v[5] = fma(w1.y, x, v[5]); v[6] = fma(w1.z, x, v[6]); v[7] = fma(w1.w, x, v[7]);
-            }
-#pragma unroll
-            for (int u = 0; u < kGenBundle; ++u)
-                if (u < m) {
-                    const long long i = (long long)out[r0 + u] * B + j;
-                    dst[i] = accumulate ? fma(alpha, v[u], dst[i]) : alpha * v[u];
-                    if (zero) zero[i] = 0.0;
+            for (long long kc = k0; kc < k1; kc += 32) {
+                __syncwarp();
+                if (kc + lane < k1) {
+                    s_col[ty][lane] = bcol[kc + lane];
+                    const double4* wsrc = reinterpret_cast<const double4*>(bw + (kc + lane) * kGenBundle);
+                    *reinterpret_cast<double4*>(&s_w[ty][lane][0]) = wsrc[0];
+                    *reinterpret_cast<double4*>(&s_w[ty][lane][4]) = wsrc[1];
                 }
+                __syncwarp();
+                const int cnt = (int)((k1 - kc) < 32 ? (k1 - kc) : 32);
+#pragma unroll 8
+                for (int e = 0; e < cnt; ++e) {
+                    const double x = sj[(long long)s_col[ty][e] * B];
+                    const double4 w0 = *reinterpret_cast<const double4*>(&s_w[ty][e][0]);
+                    const double4 w1 = *reinterpret_cast<const double4*>(&s_w[ty][e][4]);
+                    // no test of the weights: entries of Dirichlet nodes (all weights 0, data to be ignored) are not in the bundles
+                    v[0] = fma(w0.x, x, v[0]); v[1] = fma(w0.y, x, v[1]); v[2] = fma(w0.z, x, v[2]); v[3] = fma(w0.w, x, v[3]);
+                    v[4] = fma(w1.x, x, v[4]); v[5] = fma(w1.y, x, v[5]); v[6] = fma(w1.z, x, v[6]); v[7] = fma(w1.w, x, v[7]);
+                }
+            }
+            if (act) {
+#pragma unroll
+                for (int u = 0; u < kGenBundle; ++u)
+                    if (u < m) {
+                        const long long i = (long long)out[r0 + u] * B + j;
+                        dst[i] = accumulate ? fma(alpha, v[u], dst[i]) : alpha * v[u];
+                        if (zero) zero[i] = 0.0;
+                    }
+            }
         }
     }
 }
