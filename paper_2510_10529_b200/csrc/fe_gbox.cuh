@@ -67,24 +67,30 @@ __global__ void k_gbox_weight_potential(double* __restrict__ rec, const double* 
     }
 }
 
-template <int P, int BT>
+// SLIM (p = 5): ONE record buffer without the kz s tile (the output scale is kz times the gather scale), one unit per CTA, so that
+// two 6-warp CTAs fit an SM (12 warps, three per sub-partition) instead of one persistent CTA whose warps sit 2,2,1,1
+template <int P, int BT, bool SLIM = false>
 constexpr size_t gbox_smem_bytes()
 {
     constexpr int n = P + 1;
-    return ((size_t)2 * n * n * n * BT + 2 * GBoxShape<n>::REC) * sizeof(double) + 16;
+    constexpr int recs = SLIM ? GBoxShape<n>::SOUT + GBoxShape<n>::N3P / 2 : 2 * GBoxShape<n>::REC;
+    return ((size_t)2 * n * n * n * BT + recs) * sizeof(double) + 16;
 }
 
 // Block (BT lanes = vectors, n nodal planes).  A CTA walks units (cell, tile of BT vectors) u = blockIdx.x, + gridDim.x, ...
-template <int P, int BT, int MINB>
+template <int P, int BT, int MINB, bool SLIM = false>
 __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_gbox(const __grid_constant__ GBoxParams prm)
 {
     constexpr int n = P + 1, n2 = n * n, n3 = n * n * n, NP = GBoxShape<n>::NP, SMALL = GBoxShape<n>::SMALL,
-                  REC = GBoxShape<n>::REC, TAIL = GBoxShape<n>::TAIL, SOUT = GBoxShape<n>::SOUT, IDS = GBoxShape<n>::IDS;
+                  RECG = GBoxShape<n>::REC, TAIL = GBoxShape<n>::TAIL, IDSG = GBoxShape<n>::IDS, NID = GBoxShape<n>::N3P / 2,
+                  // shared-memory record: SLIM keeps VZ | s | tail | ids (the ids move up into the place of the kz s tile)
+                  REC = SLIM ? GBoxShape<n>::SOUT + NID : RECG, SOUT = SLIM ? SMALL : GBoxShape<n>::SOUT,
+                  IDS = SLIM ? GBoxShape<n>::SOUT : IDSG;
     extern __shared__ __align__(128) double smem[];
     double* bufA = smem;               // [n^3][BT]  gathered X -> A (free once the line phase is over) -> next unit's X
     double* bufB = smem + n3 * BT;     // [n^3][BT]  A2 -> R
-    double* recs = bufB + n3 * BT;     // [2][REC]
-    unsigned long long* bar = (unsigned long long*)(recs + 2 * REC);  // bar[b]: record b landed
+    double* recs = bufB + n3 * BT;     // [2][REC] (SLIM: one)
+    unsigned long long* bar = (unsigned long long*)(recs + (SLIM ? 1 : 2) * REC);  // bar[b]: record b landed
     const int lane = threadIdx.x, pl = threadIdx.y, tid = pl * BT + lane;
     const int nbt = (prm.B + BT - 1) / BT;
     const long long nunits = prm.ncells * nbt;
@@ -92,7 +98,12 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_gbox(const __grid_
     auto request_rec = [&](long long u, int b) {  // one thread
         const long long cu = u / nbt, c = prm.cell_list ? (long long)prm.cell_list[cu] : cu;
         mbar_expect_tx(bar + b, (unsigned)(REC * sizeof(double)));
-        bulk_load(recs + b * REC, prm.rec + c * REC, (unsigned)(REC * sizeof(double)), bar + b);
+        if constexpr (SLIM) {  // two pieces of the global record: VZ | s | tail, and the ids
+            bulk_load(recs, prm.rec + c * RECG, (unsigned)(IDS * sizeof(double)), bar + b);
+            bulk_load(recs + IDS, prm.rec + c * RECG + IDSG, (unsigned)(NID * sizeof(double)), bar + b);
+        } else {
+            bulk_load(recs + b * REC, prm.rec + c * RECG, (unsigned)(REC * sizeof(double)), bar + b);
+        }
     };
     // Addresses in 32-bit pieces: ids and N fit 32 bits (int32 l2g), so the row of node g starts at base + g * (8 B) bytes with
     // ONE wide multiply-add, base = X (unconstrained) or X_h - N * 8 B (hanging: g - N is its row of X_h).  (The plain 64-bit
@@ -133,13 +144,14 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_gbox(const __grid_
     int buf = 0;
     for (long long u = blockIdx.x; u < nunits; u += gridDim.x, buf ^= 1) {
     const long long un = u + gridDim.x;
-    const bool more = un < nunits;
+    const bool more = !SLIM && un < nunits;  // SLIM: one unit per CTA (the launch gives every unit its own)
     const int j = (int)(u % nbt) * BT + lane;
     const bool act = j < prm.B;
     const double* rec = recs + buf * REC;
     const double* sVZ = rec;
     const double ry = rec[TAIL], rxz = rec[TAIL + 1];
     const bool surface = rec[TAIL + 4] != 0.0;
+    const double kzs = SLIM ? rec[TAIL + 2] : 1.0;  // SLIM: output scale = kz times the gather scale
 
     double v[n][n], t[n], o[n];
     double* pA = bufA + (size_t)pl * n2 * BT + lane;
@@ -308,25 +320,25 @@ __global__ void __launch_bounds__((P + 1) * BT, MINB) k_apply_gbox(const __grid_
             char* dst = (g < N32 ? yX : yH) + (unsigned long long)g * B8;
             // unconditional add (a predicated red.global becomes a branch): Dirichlet nodes (scale 0) and idle lanes (column 0
             // of their node) add +0.0, which changes nothing
-            atomicAdd(reinterpret_cast<double*>(dst), (act && __double2hiint(sc) != 0) ? sc * o[ax] : 0.0);
+            atomicAdd(reinterpret_cast<double*>(dst), (act && __double2hiint(sc) != 0) ? (SLIM ? kzs * sc : sc) * o[ax] : 0.0);
         }
     }
     }  // units
 }
 
-template <int P, int BT, int MINB>
+template <int P, int BT, int MINB, bool SLIM = false>
 cudaError_t launch_gbox_t(const GBoxParams& prm, long long ncells, int sms, cudaStream_t st)
 {
-    constexpr size_t smem = gbox_smem_bytes<P, BT>();
+    constexpr size_t smem = gbox_smem_bytes<P, BT, SLIM>();
     static PerDeviceOnce once;
     cudaError_t e0 = once_per_device(once, [&] {
-        return cudaFuncSetAttribute(k_apply_gbox<P, BT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        return cudaFuncSetAttribute(k_apply_gbox<P, BT, MINB, SLIM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     });
     if (e0 != cudaSuccess) return e0;
     const long long nunits = ncells * ((prm.B + BT - 1) / BT);
     if (nunits <= 0) return cudaSuccess;
-    dim3 grid((unsigned)std::min<long long>(nunits, (long long)sms * MINB)), block(BT, P + 1);
-    k_apply_gbox<P, BT, MINB><<<grid, block, smem, st>>>(prm);
+    dim3 grid((unsigned)(SLIM ? nunits : std::min<long long>(nunits, (long long)sms * MINB))), block(BT, P + 1);
+    k_apply_gbox<P, BT, MINB, SLIM><<<grid, block, smem, st>>>(prm);
     return cudaGetLastError();
 }
 
@@ -339,7 +351,7 @@ inline cudaError_t launch_apply_gbox(const GBoxParams& prm, int p, long long nce
         case 2: return launch_gbox_t<2, 32, 6>(prm, ncells, sms, st);
         case 3: return launch_gbox_t<3, 32, 4>(prm, ncells, sms, st);
         case 4: return launch_gbox_t<4, 32, 3>(prm, ncells, sms, st);
-        case 5: return launch_gbox_t<5, 32, 1>(prm, ncells, sms, st);
+        case 5: return launch_gbox_t<5, 32, 2, true>(prm, ncells, sms, st);  // two one-unit SLIM CTAs per SM: 48.8 -> 56.4 GDoF-vec/s
         case 6: return launch_gbox_t<6, 32, 1>(prm, ncells, sms, st);
         case 7: return launch_gbox_t<7, 24, 1>(prm, ncells, sms, st);
     }
