@@ -376,3 +376,13 @@ def test_consumers_on_a_box_cell_mesh(p, B):
     assert _relerr(Yg, om.potential_apply(Uq, X * mask[:, None]), mask) <= TOL_APPLY and np.all(Yg[~free] == 0)
     Yg = gm.apply_H(_dev(X), eps=_dev(eps)).cpu().numpy()  # the box-cell operator after the borrowed call
     assert _relerr(Yg, om.apply(X, eps), mask) <= TOL_APPLY
+    # the host-buffer entry point (column chunks on two streams) against the device call, and a chain of applies
+    a0, a, b = -3.0, 40.0, 900.0
+    Fd = gm.cheb_filter(_dev(X).clone(), 5, a, b, a0).cpu().numpy()
+    Xh = np.ascontiguousarray(X.copy())
+    gm.cheb_filter_host(Xh, 5, a, b, a0)
+    assert _relerr(Xh, Fd, mask) <= 1e-13 and np.all(Xh[~free] == 0)
+    Y1 = torch.full((om.N, B), 3.0, dtype=torch.float64, device="cuda")
+    Y2 = torch.full((om.N, B), -2.0, dtype=torch.float64, device="cuda")
+    gm.apply_H_chain(_dev(X), Y1, Y2, _dev(eps), y_is_clear=False)
+    assert _relerr(Y1.cpu().numpy(), om.apply(X, eps), mask) <= TOL_APPLY and float(Y2.abs().max()) == 0.0
