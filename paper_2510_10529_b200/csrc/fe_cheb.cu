@@ -1613,10 +1613,21 @@ int cheb_filter_host(fe_mesh* m, double* X_host, int B, int deg, double a, doubl
     if (!m->have_V) return fail(FE_ERR_STATE, "cheb_filter_host: call fe_set_potential first");
     CUDA_TRY(cudaSetDevice(m->device));
     // columns are independent in the filter: chunks of 32 columns go through copy-in, filter, copy-out
-    // on alternating streams, so the PCIe transfers of one chunk overlap the filter of the other
-    const int BC = (B % 32 == 0 && B > 32) ? 32 : B;
-    const int nchunks = B / BC;
-    const size_t clen = (size_t)m->N * BC;
+    // on alternating streams, so the PCIe transfers of one chunk overlap the filter of the other.  What stays exposed is the
+    // copy-in of the first chunk and the copy-out of the last: where 16-column tiles run well (p >= 6: the 16-wide launch
+    // shape) the first and the last chunk are 16 columns wide, which halves that.
+    std::vector<int> width;
+    if (B % 32 == 0 && B > 32) {
+        const bool edges16 = m->kind == 0 && m->p >= 6;
+        if (edges16) width.push_back(16);
+        for (int c = 0; c < B / 32 - (edges16 ? 1 : 0); ++c) width.push_back(32);
+        if (edges16) width.push_back(16);
+    } else {
+        width.push_back(B);
+    }
+    const int nchunks = (int)width.size();
+    const int BCmax = *std::max_element(width.begin(), width.end());
+    const size_t clen = (size_t)m->N * BCmax;
     const int nbuf = nchunks > 1 ? 2 : 1;
     if (m->host_cap < clen * 3 * nbuf) {
         cudaFree(m->d_host);  // only the staging: d_WU / d_VZU belong to fe_apply_potential and stay valid
@@ -1628,14 +1639,18 @@ int cheb_filter_host(fe_mesh* m, double* X_host, int B, int deg, double a, doubl
     for (int i = 0; i < 2; ++i)
         if (!m->hstream[i]) CUDA_TRY(cudaStreamCreateWithFlags(&m->hstream[i], cudaStreamNonBlocking));
     CUDA_TRY(cudaDeviceSynchronize());
-    const size_t hp = (size_t)B * sizeof(double), dp = (size_t)BC * sizeof(double);
+    const size_t hp = (size_t)B * sizeof(double);
+    int col = 0;
     for (int c = 0; c < nchunks; ++c) {
+        const int BC = width[c];
+        const size_t dp = (size_t)BC * sizeof(double), cl = (size_t)m->N * BC;
         cudaStream_t st = m->hstream[c % nbuf];
         double* Xd = m->d_host + (size_t)(c % nbuf) * 3 * clen;
-        CUDA_TRY(cudaMemcpy2DAsync(Xd, dp, X_host + (size_t)c * BC, hp, dp, (size_t)m->N, cudaMemcpyHostToDevice, st));
-        int rc = cheb_filter(m, Xd, BC, deg, a, b, a0, Xd + clen, (void*)st);
+        CUDA_TRY(cudaMemcpy2DAsync(Xd, dp, X_host + col, hp, dp, (size_t)m->N, cudaMemcpyHostToDevice, st));
+        int rc = cheb_filter(m, Xd, BC, deg, a, b, a0, Xd + cl, (void*)st);
         if (rc) return rc;
-        CUDA_TRY(cudaMemcpy2DAsync(X_host + (size_t)c * BC, hp, Xd, dp, dp, (size_t)m->N, cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(cudaMemcpy2DAsync(X_host + col, hp, Xd, dp, dp, (size_t)m->N, cudaMemcpyDeviceToHost, st));
+        col += BC;
     }
     for (int i = 0; i < nbuf; ++i) CUDA_TRY(cudaStreamSynchronize(m->hstream[i]));
     return FE_OK;

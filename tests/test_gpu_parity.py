@@ -416,6 +416,24 @@ def test_filter_from_host_buffers(B):
     assert _relerr(Xn, Yd, mask) <= 1e-13
 
 
+@pytest.mark.parametrize("B", [64, 128])
+def test_filter_from_host_buffers_edge_chunks(B):
+    """cheb_filter_host at p = 6, where the first and the last column chunk are 16 wide (16, 32, ..., 32, 16: the exposed
+    copy-in / copy-out halves) and run the 16-wide launch shape while the middle chunks run the 32-wide one: against the
+    oracle and against the device-resident call."""
+    xe, ye, ze = np.array([0.0, 0.8, 2.0]), np.array([-1.0, -0.2, 0.5, 1.4]), np.array([0.0, 0.9, 1.7])
+    om, gm = _pair((xe, ye, ze), 6, lambda q: -3.0 / np.sqrt(((q - 0.7) ** 2).sum(axis=1) + 0.25))
+    mask = om.mask()
+    X = workloads.random_block(900 + B, om.N, B)
+    a0, a, b = -4.0, 30.0, 2600.0
+    Xh = torch.as_tensor(X.copy()).pin_memory()
+    gm.cheb_filter_host(Xh, 5, a, b, a0)
+    Yd = gm.cheb_filter(_dev(X).clone(), 5, a, b, a0).cpu().numpy()
+    assert _relerr(Xh.numpy(), Yd, mask) <= 1e-13 and np.all(Xh.numpy()[mask == 0] == 0)
+    if B == 64:
+        assert _relerr(Xh.numpy(), om.filter(X * mask[:, None], 5, a, b, a0), mask) <= TOL_FILTER
+
+
 def test_colour_ordered_scatter_is_reproducible_and_agrees():
     """Variant 4 (SURVEY a3 "atomic or colour-ordered"): two runs are bit-identical, and the atomic paths (TMA bulk
     reduce-add, legacy red.global) agree with it to rounding — the deterministic mode doubles as a race oracle (R17)."""
