@@ -113,7 +113,8 @@ int cheb_filter(fe_mesh* m, double* X, int B, int deg, double a, double b, doubl
 /* The same filter end to end from a HOST block (N*B doubles, X[a*B+j], filtered in place; pinned memory makes the
  * copies asynchronous): host->device copy, cheb_filter, device->host copy.  Columns are independent, so for B a
  * multiple of 32 (B > 32) chunks of 32 columns are pipelined on two internal streams and the PCIe transfers of one
- * chunk overlap the filter of the other.  The device staging (3*N*min(B,64) doubles) lives in the handle.
+ * chunk overlap the filter of the other (box meshes at p >= 6: the first and the last chunk are 16 columns wide, which halves
+ * the copy-in and copy-out that nothing can overlap).  The device staging (3*N*min(B,64) doubles) lives in the handle.
  * SYNCHRONOUS: returns when X_host holds the result.  This is the call bench.py's `e2e` times. */
 int cheb_filter_host(fe_mesh* m, double* X_host, int B, int deg, double a, double b, double a0);
 
