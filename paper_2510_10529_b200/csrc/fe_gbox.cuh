@@ -26,7 +26,8 @@
 namespace fecheb {
 
 // per-cell record: VZ [qx][qy][NP] | s [az][ay][NP] (gather scale: s_g, 1 at hanging nodes) | tail (8) | kz s [az][ay][NP]
-// | ids (n^3 int32, padded to a multiple of 4).  tail = { ky/kx, kx/kz, kz, hz^2/2, 1 if a node of the cell is a Dirichlet
+// | ids (n^3 int32, padded to a multiple of 4; bit 31 set where this cell is the OWNER of the node: the first cell that lists
+// it).  tail = { ky/kx, kx/kz, kz, hz^2/2, 1 if a node of the cell is a Dirichlet
 // node, 0, 0, 0 }
 template <int n>
 struct GBoxShape {
