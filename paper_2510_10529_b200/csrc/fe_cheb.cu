@@ -958,7 +958,12 @@ int fe_apply_H_chain(fe_mesh* m, const double* X, double* Y, double* Ynext, int 
         if (Ynext && (rc = zero_faces(m, Ynext, B, st))) return rc;
         return tma_step(m, mx, my, Ynext ? &mw : nullptr, B, eps_dev, 1.0, 0.0, eps_dev != nullptr, 0.0, true, st);
     }
-    // other paths (general meshes, odd B, unaligned blocks): plain apply, then clear the next target
+    if (general_fused(m)) {
+        // general mesh of box cells: the owner cells of k_apply_gbox store 0 into every row of the next target (beta' = 0)
+        if (!y_is_clear) CUDA_TRY(cudaMemsetAsync(Y, 0, len * sizeof(double), st));
+        return general_step(m, X, nullptr, Y, B, eps_dev, 1.0, 0.0, 0.0, st, Ynext, 0.0, true);
+    }
+    // other paths (general meshes with deformed cells, odd B, unaligned blocks): plain apply, then clear the next target
     int rc = fe_apply_H(m, X, Y, B, eps_dev, cuda_stream);
     if (rc) return rc;
     if (Ynext) CUDA_TRY(cudaMemsetAsync(Ynext, 0, len * sizeof(double), st));

@@ -386,3 +386,6 @@ def test_consumers_on_a_box_cell_mesh(p, B):
     Y2 = torch.full((om.N, B), -2.0, dtype=torch.float64, device="cuda")
     gm.apply_H_chain(_dev(X), Y1, Y2, _dev(eps), y_is_clear=False)
     assert _relerr(Y1.cpu().numpy(), om.apply(X, eps), mask) <= TOL_APPLY and float(Y2.abs().max()) == 0.0
+    X2 = workloads.random_block(2300 + p, om.N, B)
+    gm.apply_H_chain(_dev(X2), Y2, Y1, None, y_is_clear=True)  # the target the first call cleared; clears Y1 in turn
+    assert _relerr(Y2.cpu().numpy(), om.apply(X2), mask) <= TOL_APPLY and float(Y1.abs().max()) == 0.0
