@@ -923,7 +923,9 @@ static int apply_into_cleared(fe_mesh* m, const double* X, double* Y, int B, con
 {
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (!tma_eligible(m, B, X, Y, eps_dev)) {
-        int rc = fe_apply_H(m, X, Y, B, eps_dev, cuda_stream);
+        // general mesh of box cells: the cell kernel adds into the cleared block (owner terms inside), no second zero-fill
+        int rc = general_fused(m) ? general_step(m, X, nullptr, Y, B, eps_dev, 1.0, 0.0, 0.0, st, nullptr, 0.0, true)
+                                  : fe_apply_H(m, X, Y, B, eps_dev, cuda_stream);
         if (rc || !dots_dev) return rc;
         k_col_dot<<<m->sms * 8, dim3(kMRx, kMRy), 0, st>>>(X, Y, m->N, B, dots_dev);
         CUDA_TRY(cudaGetLastError());
